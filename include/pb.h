@@ -1,0 +1,190 @@
+/*
+ * pb.h -- C ABI of the B200-native treecode-BEM Poisson-Boltzmann hot path
+ *         (arXiv:1810.03698; citations "P:<line>" = PAPER.md line, "D:" = DESIGN.md section).
+ *
+ * One closed triangulated molecular surface, piecewise-constant collocation BEM,
+ * Yoon-Lenhoff system Eq. (5), point multipoles up to quadrupoles with induced
+ * dipoles, solvation energy Eq. (19)/(24).
+ *
+ * Conventions
+ *  - Every function returns PB_OK (0) or a negative pb_status; pb_last_error() gives a
+ *    library-owned, NUL-terminated message for the last failure on that context.
+ *  - Unless a parameter is marked HOST, every array argument is a DEVICE pointer owned by
+ *    the caller (e.g. a torch tensor), fp64 / int32, row-major, in the caller's ORIGINAL
+ *    panel and site order.  The internal Morton permutation never leaks.
+ *  - Work is enqueued on the context's cudaStream_t.  Calls that return host values
+ *    (pb_solve, pb_gmres, pb_get_stats, the *_host variants) synchronise that stream;
+ *    pb_matvec, pb_rhs_multipole, pb_reaction_field and pb_multipole_field do not.
+ *  - Device memory for internal state is obtained through the allocator callbacks
+ *    (pb_set_allocator: the Python binding hands out torch tensors); with no allocator set
+ *    the library falls back to cudaMalloc/cudaFree.  Memory is released by pb_destroy or
+ *    when the state it belongs to is rebuilt.
+ *  - Units: Angstrom, e.  Potentials carry the 1/(4 pi) of Eq. (4).  Energies in
+ *    pb_result are kcal/mol: 4 pi * 332.0636 * G, G from Eq. (24) (D: R-1).
+ *  - There is no CPU fallback anywhere: without a CUDA device pb_create fails.
+ */
+#ifndef PB_B200_H
+#define PB_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pb_ctx pb_ctx;
+
+typedef enum pb_status {
+    PB_OK = 0,
+    PB_ERR_INVALID_ARG = -1,
+    PB_ERR_BAD_MESH = -2,       /* degenerate panel, too many panels around one vertex       */
+    PB_ERR_NOT_READY = -3,      /* call order: mesh -> (sites) -> tree -> operators          */
+    PB_ERR_CUDA = -4,
+    PB_ERR_ALLOC = -5,
+    PB_ERR_NO_CONVERGENCE = -6  /* GMRES or SCF hit its iteration limit (results still set)  */
+} pb_status;
+
+/* Free parameters of the method.  pb_default_params() fills the values used for
+ * BASELINE.json configs[1]: eps 1/80, kappa 0.125, theta 0.5, P 6, K 7/19, tau 2. */
+typedef struct pb_params {
+    double eps_in;          /* eps_1, solute                                        */
+    double eps_out;         /* eps_2, solvent                                                 */
+    double kappa;           /* inverse Debye length, 1/Angstrom                        */
+    double theta;           /* multipole acceptance parameter, Eq. (28);
+                               0 => direct mode: every pair by P2P (the oracle's operator)   */
+    int32_t order_P;        /* Taylor order, 0..10                                    */
+    int32_t ncrit;          /* max source Gauss points per leaf cell           */
+    int32_t K_far;          /* Gauss points per panel, far rule: 1, 3, 4 or 7         */
+    int32_t K_near;         /* near-singular rule: 19                                 */
+    double near_tau;        /* near-singular zone |c_i-c_j| < tau*sqrt(A_i)    */
+    int32_t nq_edge;        /* Gauss-Legendre points per edge, semi-analytic rule (D: R-16)   */
+    int32_t precond;        /* 1: right block-diagonal preconditioner in GMRES, 0: none       */
+    double gmres_tol;       /* relative residual ||b-Ax||/||b||                       */
+    int32_t gmres_restart;
+    int32_t gmres_maxit;
+    double scf_tol_debye;   /* RMS change of induced dipoles, Debye (D: R-19)          */
+    double scf_omega;       /* SOR factor, 0.7                                        */
+    int32_t scf_maxit;
+    int32_t reserved;
+    double thole_a;         /* Thole damping constant, 0.39 (D: R-17)                  */
+} pb_params;
+
+/* Result of one polarizable solve (HOST struct). */
+typedef struct pb_result {
+    double dG_solv;             /* Eq. (19): G_solvterm + G_mult_diss - G_vac, kcal/mol        */
+    double G_solvterm;          /* Eq. (24) on phi_solv (reaction potential)                   */
+    double G_mult_diss;         /* Eq. (24) on the multipole potential with dissolved mu       */
+    double G_vac;               /* Eq. (24) on the multipole potential with vacuum mu^v        */
+    double final_scf_delta_debye;
+    double final_gmres_relres;
+    int32_t scf_iters;
+    int32_t scf_iters_vac;
+    int32_t gmres_iters_total;
+    int32_t matvecs_total;
+    int32_t status;             /* PB_OK or PB_ERR_NO_CONVERGENCE                              */
+    int32_t reserved;
+} pb_result;
+
+/* Counters and sizes of the built tree and lists (HOST struct). */
+typedef struct pb_stats {
+    int64_t n_panels, n_sources, n_sites;
+    int64_t n_cells, n_leaves, n_levels;
+    int64_t n_groups;           /* target groups (blocks of consecutive Morton-ordered panels) */
+    int64_t p2p_pairs;          /* (target, source Gauss point) pairs per matvec               */
+    int64_t m2p_pairs;          /* (target, cell) pairs per matvec                             */
+    int64_t near_entries;       /* SELF+ADJ+NEAR correction-table entries                      */
+    int64_t n_terms;            /* far-field terms per cell and layer (130 at P=6)             */
+    int64_t matvec_calls;
+    int64_t device_bytes;       /* bytes currently held through the allocator                  */
+    double last_matvec_ms[8];   /* CUDA-event times of the last pb_matvec_timed call:
+                                   0 weights, 1 P2M+M2M+convert, 2 M2P, 3 P2P, 4 near table +
+                                   combine, 5 total                                            */
+} pb_stats;
+
+typedef void* (*pb_alloc_fn)(void* user, size_t bytes);     /* returns a 256-byte aligned device pointer or NULL */
+typedef void (*pb_free_fn)(void* user, void* ptr);
+
+/* ---- lifetime ---------------------------------------------------------------------- */
+int pb_create(pb_ctx** out, int device, void* cuda_stream /* cudaStream_t, may be NULL */);
+int pb_destroy(pb_ctx* ctx);
+const char* pb_last_error(const pb_ctx* ctx);
+int pb_set_allocator(pb_ctx* ctx, pb_alloc_fn alloc, pb_free_fn free_, void* user);
+void pb_default_params(pb_params* out /* HOST */);
+/* Changing a parameter that shapes the operator (kappa, theta, P, ncrit, K, tau, nq_edge)
+ * invalidates the tree: pb_tree_build must be called again. */
+int pb_set_params(pb_ctx* ctx, const pb_params* p /* HOST */);
+int pb_get_params(const pb_ctx* ctx, pb_params* out /* HOST */);
+
+/* ---- inputs ------------------------------------------------------------------------ */
+/* Closed, outward-oriented triangulated surface.  Computes per panel the
+ * area, unit normal (pointing into the solvent) and centroid = collocation point.
+ * verts [nv][3] fp64, tris [nt][3] int32.  The arrays are copied; PB_ERR_BAD_MESH if a
+ * panel has zero area or an index is out of range. */
+int pb_mesh_load(pb_ctx* ctx, const double* verts, int64_t nv, const int32_t* tris, int64_t nt);
+
+/* Point multipoles of Eq. (7): charge q [na], permanent dipole dip [na][3],
+ * traceless quadrupole quad [na][6] = xx,xy,xz,yy,yz,zz in the convention of Eq. (7)
+ * (potential term Q_ij d_i d_j / (2 R^5)), isotropic polarizability alpha [na] in
+ * Angstrom^3 (D: R-2), polarization group [na].  Copied. */
+int pb_sites_load(pb_ctx* ctx, int64_t na, const double* pos, const double* q, const double* dip,
+                  const double* quad, const double* alpha, const int32_t* group);
+
+/* ---- setup: octree, interaction lists, near/singular table --------------- */
+/* Morton-sorts the panels (63-bit key of the centroid), builds the octree over the K_far
+ * Gauss points of whole panels (leaf <= ncrit points), the per-target-group M2P / P2P
+ * lists by the MAC of Eq. (28), and the SELF/ADJ/NEAR correction table (semi-analytic and
+ * K_near-point entries).  Needs pb_mesh_load. */
+int pb_tree_build(pb_ctx* ctx);
+
+/* ---- operators --------------------------------------------------------------------- */
+/* b [2 nt]: b[0:nt] = Eq. (8) at the collocation points with p = dip + mu_induced
+ * (Eq. 10; mu_induced [na][3] or NULL), b[nt:2nt] = 0. */
+int pb_rhs_multipole(pb_ctx* ctx, const double* mu_induced, double* b);
+
+/* y = A x, the left side of Eq. (5), x = [phi (nt); dphi/dn (nt)]:
+ *   y[i]      = phi_i/2 + K_L phi - V_L dphi
+ *   y[nt + i] = phi_i/2 - K_Y phi + (eps_in/eps_out) V_Y dphi
+ * by the treecode (theta > 0) or by direct summation (theta == 0).  x != y. */
+int pb_matvec(pb_ctx* ctx, const double* x, double* y);
+/* Same, with CUDA events around each phase; times land in pb_stats.last_matvec_ms.  Synchronises. */
+int pb_matvec_timed(pb_ctx* ctx, const double* x, double* y);
+/* Same operation with HOST buffers: copies x in, runs, copies y out, synchronises. */
+int pb_matvec_host(pb_ctx* ctx, const double* x_host, double* y_host);
+
+/* Reaction potential of the surface layers at the sites, Eq. (12)
+ * phi_solv = -K_L(phi) + V_L(dphi), its gradient (Eq. 13) and Hessian (Eq. 21,
+ * P:195; 6-vector xx,xy,xz,yy,yz,zz).  phi [na], grad [na][3], hess [na][6]; NULL outputs
+ * are skipped.  Direct sum over all source points; K_near rule for panels with
+ * |r_m - c_j| < tau*sqrt(A_j) (D: R-9). */
+int pb_reaction_field(pb_ctx* ctx, const double* x, double* phi, double* grad, double* hess);
+
+/* Coulomb potential, gradient, Hessian at each site of the multipoles on all OTHER sites,
+ * Eq. (7), (14), (31), (32) times 1/(4 pi eps_in), with p = dip (permanent part, dropped for
+ * same-group pairs when use_mask != 0) and the induced dipoles mu [na][3] (or
+ * NULL), Thole-damped, never masked. */
+int pb_multipole_field(pb_ctx* ctx, const double* mu, int use_mask, double* phi, double* grad,
+                       double* hess);
+
+/* ---- solvers ----------------------------------------------------------------------- */
+/* Restarted GMRES on A x = b, initial guess = x on entry.  iters/relres are HOST
+ * outputs (may be NULL).  relres is the true ||b - A x|| / ||b||. */
+int pb_gmres(pb_ctx* ctx, const double* b, double* x, int32_t* iters, double* relres);
+
+/* One polarizable solve: vacuum SCF for mu^v, then the solvent SCF
+ * (rhs -> GMRES -> reaction field + multipole field -> SOR update) to scf_tol_debye, then
+ * the energies.  x_out [2 nt] and mu_out [na][3] may be NULL.  result is HOST. */
+int pb_solve(pb_ctx* ctx, double* x_out, double* mu_out, pb_result* result);
+/* Same with HOST outputs (x_host [2 nt], mu_host [na][3], either may be NULL). */
+int pb_solve_host(pb_ctx* ctx, double* x_host, double* mu_host, pb_result* result);
+
+int pb_get_stats(pb_ctx* ctx, pb_stats* out /* HOST */);
+
+/* Measured FP64 FMA throughput of the device in TFLOP/s (independent DFMA chains, no memory
+ * traffic): the denominator check for the ALU roofline of the P2P / M2P kernels.  Synchronises. */
+int pb_fp64_peak_probe(pb_ctx* ctx, double* tflops_out /* HOST */);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PB_B200_H */

@@ -1,0 +1,407 @@
+// pb_api.cu -- context lifetime, memory, parameters, mesh and site loading (include/pb.h).
+#include <stdarg.h>
+#include <math.h>
+#include "pb_internal.cuh"
+
+int pb_fail(pb_ctx* ctx, int code, const char* fmt, ...)
+{
+    if (ctx) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(ctx->err, sizeof(ctx->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+// ---- memory -----------------------------------------------------------------------------
+int pb_dalloc(pb_ctx* ctx, void** out, size_t bytes, int cat)
+{
+    *out = nullptr;
+    if (bytes == 0) bytes = 256;
+    bytes = (bytes + 255) & ~(size_t)255;
+    void* p = nullptr;
+    if (ctx->alloc) {
+        p = ctx->alloc(ctx->user, bytes);
+        if (!p) return pb_fail(ctx, PB_ERR_ALLOC, "allocator callback returned NULL for %zu bytes", bytes);
+    } else {
+        cudaError_t e = cudaMalloc(&p, bytes);
+        if (e != cudaSuccess)
+            return pb_fail(ctx, PB_ERR_ALLOC, "cudaMalloc(%zu) failed: %s", bytes, cudaGetErrorString(e));
+    }
+    ctx->allocs.push_back({p, bytes, cat});
+    ctx->bytes_held += bytes;
+    *out = p;
+    return PB_OK;
+}
+
+void pb_dfree_cat(pb_ctx* ctx, int cat)
+{
+    bool any = false;
+    for (auto& a : ctx->allocs) any = any || (a.cat == cat || cat < 0);
+    if (any) cudaStreamSynchronize(ctx->stream);   // nothing in flight may still use the memory
+    std::vector<pb_allocation> keep;
+    for (auto& a : ctx->allocs) {
+        if (a.cat == cat || cat < 0) {
+            if (ctx->free_) ctx->free_(ctx->user, a.ptr);
+            else if (!ctx->alloc) cudaFree(a.ptr);
+            ctx->bytes_held -= a.bytes;
+        } else
+            keep.push_back(a);
+    }
+    ctx->allocs.swap(keep);
+}
+
+int pb_scratch(pb_ctx* ctx, size_t bytes)
+{
+    if (ctx->scratch_bytes >= bytes) return PB_OK;
+    // scratch is allocated once, generously, outside the categories (freed at destroy)
+    size_t want = bytes < ((size_t)1 << 20) ? ((size_t)1 << 20) : bytes;
+    void* p;
+    PB_TRY(pb_dalloc(ctx, &p, want, -2));
+    ctx->scratch = (double*)p;
+    ctx->scratch_bytes = want;
+    return PB_OK;
+}
+
+int pb_pinned(pb_ctx* ctx, size_t bytes)
+{
+    if (ctx->h_pinned_bytes >= bytes) return PB_OK;
+    if (ctx->h_pinned) cudaFreeHost(ctx->h_pinned);
+    ctx->h_pinned = nullptr;
+    ctx->h_pinned_bytes = 0;
+    size_t want = bytes < 4096 ? 4096 : bytes;
+    PB_CUDA(cudaMallocHost((void**)&ctx->h_pinned, want));
+    ctx->h_pinned_bytes = want;
+    return PB_OK;
+}
+
+// ---- lifetime -----------------------------------------------------------------------------
+extern "C" void pb_default_params(pb_params* p)
+{
+    memset(p, 0, sizeof(*p));
+    p->eps_in = 1.0;
+    p->eps_out = 80.0;
+    p->kappa = 0.125;
+    p->theta = 0.5;
+    p->order_P = 6;
+    p->ncrit = 64;
+    p->K_far = 7;
+    p->K_near = 19;
+    p->near_tau = 2.0;
+    p->nq_edge = 16;
+    p->precond = 1;
+    p->gmres_tol = 1e-6;
+    p->gmres_restart = 100;
+    p->gmres_maxit = 1000;
+    p->scf_tol_debye = 1e-7;
+    p->scf_omega = 0.7;
+    p->scf_maxit = 200;
+    p->thole_a = 0.39;
+}
+
+extern "C" int pb_create(pb_ctx** out, int device, void* cuda_stream)
+{
+    if (!out) return PB_ERR_INVALID_ARG;
+    *out = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0 || device < 0 || device >= ndev)
+        return PB_ERR_CUDA;   // no CPU fallback: without a CUDA device there is no library
+    if (cudaSetDevice(device) != cudaSuccess) return PB_ERR_CUDA;
+    pb_ctx* ctx = new pb_ctx();
+    ctx->device = device;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    pb_default_params(&ctx->prm);
+    *out = ctx;
+    return PB_OK;
+}
+
+extern "C" int pb_destroy(pb_ctx* ctx)
+{
+    if (!ctx) return PB_ERR_INVALID_ARG;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    pb_dfree_cat(ctx, -1);
+    if (ctx->h_pinned) cudaFreeHost(ctx->h_pinned);
+    if (ctx->ev_made)
+        for (int i = 0; i < 8; ++i) cudaEventDestroy(ctx->ev[i]);
+    delete ctx;
+    return PB_OK;
+}
+
+extern "C" const char* pb_last_error(const pb_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+extern "C" int pb_set_allocator(pb_ctx* ctx, pb_alloc_fn alloc, pb_free_fn free_, void* user)
+{
+    if (!ctx) return PB_ERR_INVALID_ARG;
+    if (!ctx->allocs.empty())
+        return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_set_allocator must be called before any allocation");
+    ctx->alloc = alloc;
+    ctx->free_ = free_;
+    ctx->user = user;
+    return PB_OK;
+}
+
+extern "C" int pb_get_params(const pb_ctx* ctx, pb_params* out)
+{
+    if (!ctx || !out) return PB_ERR_INVALID_ARG;
+    *out = ctx->prm;
+    return PB_OK;
+}
+
+extern "C" int pb_set_params(pb_ctx* ctx, const pb_params* p)
+{
+    if (!ctx || !p) return PB_ERR_INVALID_ARG;
+    if (!(p->eps_in > 0) || !(p->eps_out > 0) || !(p->kappa >= 0))
+        return pb_fail(ctx, PB_ERR_INVALID_ARG, "eps_in, eps_out must be > 0 and kappa >= 0");
+    if (!(p->theta >= 0) || !(p->theta < 1))
+        return pb_fail(ctx, PB_ERR_INVALID_ARG, "theta must be in [0, 1)");
+    if (p->order_P < 0 || p->order_P > PB_MAX_P)
+        return pb_fail(ctx, PB_ERR_INVALID_ARG, "order_P must be in [0, %d]", PB_MAX_P);
+    if (!(p->K_far == 1 || p->K_far == 3 || p->K_far == 4 || p->K_far == 7))
+        return pb_fail(ctx, PB_ERR_INVALID_ARG, "K_far must be 1, 3, 4 or 7");
+    if (!(p->K_near == 1 || p->K_near == 3 || p->K_near == 4 || p->K_near == 7 || p->K_near == 19))
+        return pb_fail(ctx, PB_ERR_INVALID_ARG, "K_near must be 1, 3, 4, 7 or 19");
+    if (p->ncrit < 1 || p->nq_edge < 1 || p->nq_edge > 64 || !(p->near_tau >= 0))
+        return pb_fail(ctx, PB_ERR_INVALID_ARG, "ncrit >= 1, 1 <= nq_edge <= 64, near_tau >= 0 required");
+    if (p->gmres_restart < 1 || p->gmres_maxit < 1 || p->scf_maxit < 1 || !(p->gmres_tol > 0) ||
+        !(p->scf_tol_debye > 0) || !(p->scf_omega > 0))
+        return pb_fail(ctx, PB_ERR_INVALID_ARG, "solver limits/tolerances must be positive");
+    const pb_params& o = ctx->prm;
+    bool shape = o.kappa != p->kappa || o.theta != p->theta || o.order_P != p->order_P ||
+                 o.ncrit != p->ncrit || o.K_far != p->K_far || o.K_near != p->K_near ||
+                 o.near_tau != p->near_tau || o.nq_edge != p->nq_edge || o.eps_in != p->eps_in ||
+                 o.eps_out != p->eps_out;
+    ctx->prm = *p;
+    if (shape && ctx->tree.built) {
+        pb_dfree_cat(ctx, CAT_TREE);
+        pb_dfree_cat(ctx, CAT_SITE_NEAR);
+        pb_dfree_cat(ctx, CAT_SOLVE);
+        ctx->gws = pb_gmres_ws();
+        ctx->tree = pb_tree();
+        ctx->sites.near_built = false;
+    }
+    return PB_OK;
+}
+
+// ---- mesh ---------------------------------------------------------------------------------
+// Per panel: centroid (v0+v1+v2)/3 = collocation point; flags degenerate panels.
+__global__ void k_mesh_check(int64_t nt, int64_t nv, const double* __restrict__ verts,
+                             const int32_t* __restrict__ tris, double* __restrict__ cen, int* __restrict__ bad)
+{
+    int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (j >= nt) return;
+    int32_t a = tris[3 * j], b = tris[3 * j + 1], c = tris[3 * j + 2];
+    if (a < 0 || b < 0 || c < 0 || a >= nv || b >= nv || c >= nv) { atomicOr(bad, 1); return; }
+    double v[9];
+    for (int d = 0; d < 3; ++d) { v[d] = verts[3 * (int64_t)a + d]; v[3 + d] = verts[3 * (int64_t)b + d]; v[6 + d] = verts[3 * (int64_t)c + d]; }
+    double e1[3], e2[3];
+    for (int d = 0; d < 3; ++d) {
+        e1[d] = v[3 + d] - v[d];
+        e2[d] = v[6 + d] - v[d];
+        cen[3 * j + d] = (v[d] + v[3 + d] + v[6 + d]) / 3.0;
+    }
+    double cx = e1[1] * e2[2] - e1[2] * e2[1], cy = e1[2] * e2[0] - e1[0] * e2[2], cz = e1[0] * e2[1] - e1[1] * e2[0];
+    double l = sqrt(cx * cx + cy * cy + cz * cz);
+    if (!(l > 0.0) || !isfinite(l)) atomicOr(bad, 2);
+}
+
+extern "C" int pb_mesh_load(pb_ctx* ctx, const double* verts, int64_t nv, const int32_t* tris, int64_t nt)
+{
+    if (!ctx) return PB_ERR_INVALID_ARG;
+    if (!verts || !tris || nv < 3 || nt < 1) return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_mesh_load: empty mesh or NULL pointer");
+    if (nt > (int64_t)200000000 || nv > (int64_t)2000000000) return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_mesh_load: mesh too large for int32 indexing");
+    PB_CUDA(cudaSetDevice(ctx->device));
+    pb_dfree_cat(ctx, CAT_TREE);
+    pb_dfree_cat(ctx, CAT_SITE_NEAR);
+    pb_dfree_cat(ctx, CAT_SOLVE);
+    ctx->gws = pb_gmres_ws();
+    pb_dfree_cat(ctx, CAT_MESH);
+    ctx->tree = pb_tree();
+    ctx->sites.near_built = false;
+    ctx->mesh_loaded = false;
+    ctx->nv = nv;
+    ctx->nt = nt;
+    PB_TRY(pb_dalloc_t(ctx, &ctx->verts, 3 * nv, CAT_MESH));
+    PB_TRY(pb_dalloc_t(ctx, &ctx->tris, 3 * nt, CAT_MESH));
+    PB_TRY(pb_dalloc_t(ctx, &ctx->cen, 3 * nt, CAT_MESH));
+    PB_CUDA(cudaMemcpyAsync(ctx->verts, verts, sizeof(double) * 3 * nv, cudaMemcpyDeviceToDevice, ctx->stream));
+    PB_CUDA(cudaMemcpyAsync(ctx->tris, tris, sizeof(int32_t) * 3 * nt, cudaMemcpyDeviceToDevice, ctx->stream));
+    PB_TRY(pb_scratch(ctx, 1 << 20));
+    int* bad = (int*)ctx->scratch;
+    PB_CUDA(cudaMemsetAsync(bad, 0, sizeof(int), ctx->stream));
+    k_mesh_check<<<pb_blocks(nt, 256), 256, 0, ctx->stream>>>(nt, nv, ctx->verts, ctx->tris, ctx->cen, bad);
+    PB_LAUNCH_CHECK();
+    int hbad = 0;
+    PB_CUDA(cudaMemcpyAsync(&hbad, bad, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    PB_CUDA(cudaStreamSynchronize(ctx->stream));
+    if (hbad & 1) return pb_fail(ctx, PB_ERR_BAD_MESH, "pb_mesh_load: triangle vertex index out of range");
+    if (hbad & 2) return pb_fail(ctx, PB_ERR_BAD_MESH, "pb_mesh_load: degenerate (zero-area or non-finite) panel");
+    ctx->mesh_loaded = true;
+    return PB_OK;
+}
+
+// ---- sites --------------------------------------------------------------------------------
+extern "C" int pb_sites_load(pb_ctx* ctx, int64_t na, const double* pos, const double* q, const double* dip,
+                             const double* quad, const double* alpha, const int32_t* group)
+{
+    if (!ctx) return PB_ERR_INVALID_ARG;
+    if (na < 1 || !pos || !q || !dip || !quad || !alpha || !group)
+        return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_sites_load: na >= 1 and non-NULL arrays required");
+    PB_CUDA(cudaSetDevice(ctx->device));
+    pb_dfree_cat(ctx, CAT_SITE_NEAR);
+    pb_dfree_cat(ctx, CAT_SITES);
+    pb_sites& s = ctx->sites;
+    s = pb_sites();
+    s.na = na;
+    PB_TRY(pb_dalloc_t(ctx, &s.pos, 3 * na, CAT_SITES));
+    PB_TRY(pb_dalloc_t(ctx, &s.q, na, CAT_SITES));
+    PB_TRY(pb_dalloc_t(ctx, &s.dip, 3 * na, CAT_SITES));
+    PB_TRY(pb_dalloc_t(ctx, &s.quad, 6 * na, CAT_SITES));
+    PB_TRY(pb_dalloc_t(ctx, &s.alpha, na, CAT_SITES));
+    PB_TRY(pb_dalloc_t(ctx, &s.group, na, CAT_SITES));
+    cudaStream_t st = ctx->stream;
+    PB_CUDA(cudaMemcpyAsync(s.pos, pos, sizeof(double) * 3 * na, cudaMemcpyDeviceToDevice, st));
+    PB_CUDA(cudaMemcpyAsync(s.q, q, sizeof(double) * na, cudaMemcpyDeviceToDevice, st));
+    PB_CUDA(cudaMemcpyAsync(s.dip, dip, sizeof(double) * 3 * na, cudaMemcpyDeviceToDevice, st));
+    PB_CUDA(cudaMemcpyAsync(s.quad, quad, sizeof(double) * 6 * na, cudaMemcpyDeviceToDevice, st));
+    PB_CUDA(cudaMemcpyAsync(s.alpha, alpha, sizeof(double) * na, cudaMemcpyDeviceToDevice, st));
+    PB_CUDA(cudaMemcpyAsync(s.group, group, sizeof(int32_t) * na, cudaMemcpyDeviceToDevice, st));
+    s.loaded = true;
+    return PB_OK;
+}
+
+// ---- setup -------------------------------------------------------------------------------
+extern "C" int pb_tree_build(pb_ctx* ctx)
+{
+    if (!ctx) return PB_ERR_INVALID_ARG;
+    if (!ctx->mesh_loaded) return pb_fail(ctx, PB_ERR_NOT_READY, "pb_tree_build: call pb_mesh_load first");
+    PB_CUDA(cudaSetDevice(ctx->device));
+    pb_dfree_cat(ctx, CAT_TREE);
+    pb_dfree_cat(ctx, CAT_SITE_NEAR);
+    pb_dfree_cat(ctx, CAT_SOLVE);
+    ctx->gws = pb_gmres_ws();
+    ctx->tree = pb_tree();
+    ctx->sites.near_built = false;
+    PB_TRY(pb_upload_rules(ctx));
+    PB_TRY(pb_tree_build_impl(ctx));
+    PB_TRY(pb_farfield_setup(ctx));
+    PB_TRY(pb_near_build(ctx));
+    PB_CUDA(cudaStreamSynchronize(ctx->stream));
+    ctx->tree.built = true;
+    return PB_OK;
+}
+
+extern "C" int pb_get_stats(pb_ctx* ctx, pb_stats* out)
+{
+    if (!ctx || !out) return PB_ERR_INVALID_ARG;
+    memset(out, 0, sizeof(*out));
+    const pb_tree& t = ctx->tree;
+    out->n_panels = ctx->nt;
+    out->n_sources = t.Ns;
+    out->n_sites = ctx->sites.na;
+    out->n_cells = t.n_cells;
+    out->n_leaves = t.n_leaves;
+    out->n_levels = t.n_levels;
+    out->n_groups = t.n_groups;
+    out->p2p_pairs = t.p2p_pairs;
+    out->m2p_pairs = t.m2p_pairs;
+    out->near_entries = t.near_entries;
+    out->n_terms = t.NT;
+    out->matvec_calls = ctx->matvec_calls;
+    out->device_bytes = (int64_t)ctx->bytes_held;
+    for (int i = 0; i < 8; ++i) out->last_matvec_ms[i] = ctx->last_ms[i];
+    return PB_OK;
+}
+
+// ---- exclusive scan of int32 (single block, chunked; setup-time only) ---------------------
+__global__ void k_scan_i32(const int32_t* __restrict__ in, int32_t* __restrict__ out, int64_t n, int64_t* total)
+{
+    __shared__ int32_t warp_sums[32];
+    __shared__ int64_t carry_s;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    if (tid == 0) carry_s = 0;
+    __syncthreads();
+    for (int64_t base = 0; base < n; base += blockDim.x) {
+        int64_t i = base + tid;
+        int32_t v = (i < n) ? in[i] : 0;
+        int32_t incl = v;
+        for (int o = 1; o < 32; o <<= 1) {
+            int32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += t;
+        }
+        if (lane == 31) warp_sums[wid] = incl;
+        __syncthreads();
+        if (wid == 0) {
+            int32_t w = (lane < (int)(blockDim.x >> 5)) ? warp_sums[lane] : 0;
+            int32_t wi = w;
+            for (int o = 1; o < 32; o <<= 1) {
+                int32_t t = __shfl_up_sync(0xffffffffu, wi, o);
+                if (lane >= o) wi += t;
+            }
+            warp_sums[lane] = wi - w;   // exclusive warp offsets
+        }
+        __syncthreads();
+        int64_t carry = carry_s;
+        int64_t excl = carry + warp_sums[wid] + (incl - v);
+        if (i < n) out[i] = (int32_t)excl;
+        __syncthreads();
+        if (tid == blockDim.x - 1) carry_s = excl + v;
+        __syncthreads();
+    }
+    if (tid == 0 && total) *total = carry_s;
+}
+
+int pb_exclusive_scan_i32(pb_ctx* ctx, const int32_t* in, int32_t* out, int64_t n, int64_t* total_host)
+{
+    PB_TRY(pb_scratch(ctx, 1 << 20));
+    // the total lives at the END of the scratch area so callers may use its start
+    int64_t* dtotal = (int64_t*)((char*)ctx->scratch + ctx->scratch_bytes - 256);
+    k_scan_i32<<<1, 1024, 0, ctx->stream>>>(in, out, n, dtotal);
+    PB_LAUNCH_CHECK();
+    if (total_host) {
+        PB_CUDA(cudaMemcpyAsync(total_host, dtotal, sizeof(int64_t), cudaMemcpyDeviceToHost, ctx->stream));
+        PB_CUDA(cudaStreamSynchronize(ctx->stream));
+        if (*total_host > 2147483647LL)
+            return pb_fail(ctx, PB_ERR_ALLOC, "list too long for int32 offsets (%lld entries)", (long long)*total_host);
+    }
+    return PB_OK;
+}
+
+// ---- FP64 peak probe: independent DFMA chains, no memory traffic (roofline denominator check) --------
+__global__ void __launch_bounds__(256) k_dfma_probe(int iters, double a, double b, double* __restrict__ out)
+{
+    double x0 = threadIdx.x * 1e-3, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+    for (int i = 0; i < iters; ++i) {
+        x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+        x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+    }
+    double s = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
+    if (s == 123.456) out[0] = s;   // never true; keeps the chains alive
+}
+
+extern "C" int pb_fp64_peak_probe(pb_ctx* ctx, double* tflops_out)
+{
+    if (!ctx || !tflops_out) return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(ctx->device));
+    PB_TRY(pb_scratch(ctx, 1 << 20));
+    cudaEvent_t e0, e1;
+    PB_CUDA(cudaEventCreate(&e0));
+    PB_CUDA(cudaEventCreate(&e1));
+    const int iters = 20000, blocks = 148 * 8, threads = 256;
+    double best = 0;
+    for (int rep = 0; rep < 4; ++rep) {
+        PB_CUDA(cudaEventRecord(e0, ctx->stream));
+        k_dfma_probe<<<blocks, threads, 0, ctx->stream>>>(iters, 0.999999, 1e-6, ctx->scratch);
+        PB_CUDA(cudaEventRecord(e1, ctx->stream));
+        PB_CUDA(cudaEventSynchronize(e1));
+        float ms = 0;
+        PB_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+        double tf = 2.0 * 8.0 * (double)iters * blocks * threads / (ms * 1e-3) / 1e12;
+        if (rep > 0 && tf > best) best = tf;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    *tflops_out = best;
+    return PB_OK;
+}

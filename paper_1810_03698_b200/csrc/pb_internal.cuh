@@ -1,0 +1,195 @@
+// pb_internal.cuh -- shared declarations of the CUDA library behind include/pb.h.
+// Product code.  Nothing here includes, links or calls anything under oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+#include <vector>
+#include <utility>
+
+#include "../../include/pb.h"
+
+#define PB_INV4PI 0.079577471545947667884
+#define PB_MAX_P 10
+#define PB_TG 64            // targets (panels) per target group = threads per M2P/P2P block
+#define PB_KCAL 332.0636    // e^2/Angstrom -> kcal/mol (D: R-1)
+#define PB_DEBYE 4.80320    // 1 e*Angstrom in Debye (D: R-1)
+
+enum pb_mem_cat { CAT_MESH = 0, CAT_SITES = 1, CAT_TREE = 2, CAT_SOLVE = 3, CAT_SITE_NEAR = 4, CAT_TMP = 5, CAT_COUNT = 6 };
+
+// Symmetric Gauss rule on the triangle (barycentric nodes, weights summing to 1) and a
+// Gauss-Legendre rule on [-1,1]; passed to kernels by value.
+struct pb_rule_t { int K; double lam[19][3]; double w[19]; };
+struct pb_gl_t { int n; double x[64]; double w[64]; };
+
+struct pb_allocation { void* ptr; size_t bytes; int cat; };
+
+// Source-point and panel arrays in MORTON order (built by pb_tree_build).
+struct pb_tree {
+    bool built = false;
+    int64_t N = 0, Ns = 0;
+    int K = 0;
+    int32_t* perm = nullptr;      // [N] Morton position -> original panel index
+    // panels (SoA)
+    double* pc[3] = {0, 0, 0};    // centroid
+    double* pn[3] = {0, 0, 0};    // unit normal
+    double* parea = nullptr;
+    double* pv[9] = {0};          // vertices v0x v0y v0z v1x ...
+    int32_t* ptri[3] = {0, 0, 0}; // vertex indices
+    // source Gauss points (SoA), s = panel*K + g
+    double* sx[3] = {0, 0, 0};
+    double* swA = nullptr;        // w_g * A_j
+    // per-matvec source weights
+    double* qV = nullptr;         // w A dphi
+    double* qK[3] = {0, 0, 0};    // w A phi n
+    double* xphi = nullptr;       // [N] phi in Morton order
+    double* xdphi = nullptr;      // [N]
+    // cells
+    int64_t n_cells = 0, n_leaves = 0, n_levels = 0;
+    int32_t* c_first = nullptr;   // [cells] first panel
+    int32_t* c_last = nullptr;    // one past last panel
+    int32_t* c_child = nullptr;   // first child cell (-1 for leaves)
+    int32_t* c_nchild = nullptr;
+    double* c_ctr[3] = {0, 0, 0};
+    double* c_rad = nullptr;
+    double* c_box = nullptr;      // [cells][6] lo, hi
+    std::vector<int64_t> gen_start; // BFS generations: cells [gen_start[g], gen_start[g+1])
+    int32_t* leaf_ids = nullptr;  // [n_leaves]
+    // target groups
+    int64_t n_groups = 0;
+    double* g_ctr[3] = {0, 0, 0};
+    double* g_rad = nullptr;
+    // lists (CSR per group)
+    int32_t* m2p_off = nullptr;   // [groups+1]
+    int32_t* m2p_cell = nullptr;
+    int32_t* p2p_off = nullptr;   // [groups+1]
+    int32_t* p2p_lo = nullptr;    // source-point ranges [lo, hi)
+    int32_t* p2p_hi = nullptr;
+    int64_t p2p_pairs = 0, m2p_pairs = 0;
+    // far-field data
+    int P = 0, Nk = 0, NT = 0;
+    double* M = nullptr;          // [cells][2][Nk] Cartesian moments (V, K)
+    double2* FF = nullptr;        // [cells][NT] converted far-field terms {V, K}
+    int32_t* cv_off = nullptr;    // [NT+1] conversion table (CSR over source moment indices)
+    int32_t* cv_idx = nullptr;
+    double* cv_coef = nullptr;
+    // near / singular correction table (CSR per target, Morton order)
+    int64_t near_entries = 0;
+    int32_t* nr_off = nullptr;    // [N+1]
+    int32_t* nr_col = nullptr;    // [entries] source panel (Morton)
+    double* nr_val = nullptr;     // [4][entries] VL, KL, VY, KY corrections
+    double* precond = nullptr;    // [N][4] inverse 2x2 diagonal blocks
+    // partial accumulators
+    int nslice_p2p = 1, nslice_m2p = 1;
+    double* accP = nullptr;       // [nslice_p2p][4][N]
+    double* accM = nullptr;       // [nslice_m2p][4][N]
+};
+
+struct pb_sites {
+    bool loaded = false;
+    int64_t na = 0;
+    double* pos = nullptr;        // [na][3]
+    double* q = nullptr;
+    double* dip = nullptr;        // [na][3]
+    double* quad = nullptr;       // [na][6]
+    double* alpha = nullptr;
+    int32_t* group = nullptr;
+    // near (site, panel) pairs for the reaction field (D: R-9); built lazily
+    bool near_built = false;
+    int64_t n_near = 0;
+    int32_t* near_site = nullptr;
+    int32_t* near_panel = nullptr; // Morton index
+};
+
+// GMRES workspace, kept between solves while the system size and restart length are unchanged
+struct pb_gmres_ws {
+    int64_t n = 0;
+    int m = 0;
+    double *V = nullptr, *w = nullptr, *z = nullptr, *r = nullptr, *u = nullptr;
+    double *partial = nullptr, *hdev = nullptr, *coef = nullptr;
+    int nblk = 0;
+};
+
+struct pb_ctx {
+    int device = 0;
+    cudaStream_t stream = 0;
+    char err[512] = {0};
+    pb_alloc_fn alloc = nullptr;
+    pb_free_fn free_ = nullptr;
+    void* user = nullptr;
+    std::vector<pb_allocation> allocs;
+    size_t bytes_held = 0;
+    pb_params prm;
+    pb_rule_t ruleF, ruleN;       // far and near-singular rules
+    pb_gl_t gl;                   // edge rule of the semi-analytic integrals (D: R-16)
+    // mesh, original order
+    bool mesh_loaded = false;
+    int64_t nv = 0, nt = 0;
+    double* verts = nullptr;      // [nv][3]
+    int32_t* tris = nullptr;      // [nt][3]
+    double* cen = nullptr;        // [nt][3] centroids, original order (RHS targets)
+    pb_tree tree;
+    pb_sites sites;
+    pb_gmres_ws gws;
+    // scratch
+    double* scratch = nullptr;    // small device scratch for reductions
+    size_t scratch_bytes = 0;
+    double* h_pinned = nullptr;   // pinned host staging
+    size_t h_pinned_bytes = 0;
+    int64_t matvec_calls = 0;
+    double last_ms[8] = {0};
+    cudaEvent_t ev[8] = {0};
+    bool ev_made = false;
+};
+
+// ---- error handling ---------------------------------------------------------------------
+int pb_fail(pb_ctx* ctx, int code, const char* fmt, ...);
+
+#define PB_CUDA(call)                                                                          \
+    do {                                                                                       \
+        cudaError_t e__ = (call);                                                              \
+        if (e__ != cudaSuccess)                                                                \
+            return pb_fail(ctx, PB_ERR_CUDA, "%s:%d %s: %s", __FILE__, __LINE__, #call,        \
+                           cudaGetErrorString(e__));                                           \
+    } while (0)
+
+#define PB_LAUNCH_CHECK() PB_CUDA(cudaGetLastError())
+
+#define PB_TRY(call)                                                                           \
+    do {                                                                                       \
+        int rc__ = (call);                                                                     \
+        if (rc__ != PB_OK) return rc__;                                                        \
+    } while (0)
+
+// ---- memory -----------------------------------------------------------------------------
+int pb_dalloc(pb_ctx* ctx, void** out, size_t bytes, int cat);
+void pb_dfree_cat(pb_ctx* ctx, int cat);
+int pb_scratch(pb_ctx* ctx, size_t bytes);           // ensures ctx->scratch >= bytes
+int pb_pinned(pb_ctx* ctx, size_t bytes);            // ensures ctx->h_pinned >= bytes
+
+template <typename T>
+static inline int pb_dalloc_t(pb_ctx* ctx, T** out, size_t count, int cat)
+{
+    return pb_dalloc(ctx, (void**)out, count * sizeof(T), cat);
+}
+
+static inline int pb_blocks(int64_t n, int threads) { return (int)((n + threads - 1) / threads); }
+
+// ---- cross-file entry points -------------------------------------------------------------
+// pb_scan.cu
+int pb_exclusive_scan_i32(pb_ctx* ctx, const int32_t* in, int32_t* out, int64_t n, int64_t* total_host);
+// pb_tree.cu
+int pb_tree_build_impl(pb_ctx* ctx);
+// pb_near.cu
+int pb_near_build(pb_ctx* ctx);
+int pb_make_rule(int K, pb_rule_t* r);
+int pb_upload_rules(pb_ctx* ctx);   // fills ctx->ruleF, ruleN, gl from the parameters
+// pb_matvec.cu
+int pb_farfield_setup(pb_ctx* ctx);
+int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed);
+int pb_weights(pb_ctx* ctx, const double* x);
+// pb_sites.cu
+int pb_site_near_build(pb_ctx* ctx);
+// pb_solve.cu
+int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters, double* relres, int32_t* matvecs);

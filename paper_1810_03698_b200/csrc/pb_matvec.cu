@@ -1,0 +1,548 @@
+// pb_matvec.cu -- the treecode matrix-vector product of Eq. (5):
+// source weights, P2M / M2M Cartesian-Taylor moments, M2P far field, P2P near field,
+// near/singular table and the final combine (D: sections 5-7).
+//
+// Far field (D: section 6).  For a cell with centre y_c and a target x, d = x - y_c, the
+// order-P Taylor sum  sum_{|k|<=P} a_k(x,y_c) M_k  of P:251 (a_k = (1/k!) D_y^k G) is
+// evaluated without forming the a_k.  G is radial, G = f(|d-h|^2), and
+//   f(s - 2 d.h + |h|^2) = sum_m f^(m)(s)/m! (-2 d.h + |h|^2)^m ,
+// so collecting total degree <= P in h gives EXACTLY the same truncated sum as
+//   sum_{p+2j<=P} u_{p+j}(R) T_{p,j},   T_{p,j} = sum_{|alpha|=p} d^alpha F_{alpha,j},
+//   F_{alpha,j} = (-1)^j / (2^j alpha!) sum_{|beta|=j} M_{alpha+2beta} / beta! ,
+//   u_m = (-2)^m f^(m):  u_0 = G, u_1 = e^{-kR}(1+kR)/R^3, u_{m+1} = ((2m+1) u_m + k^2 u_{m-1})/R^2
+// (k = 0 for the Laplace kernel).  The F (130 numbers per layer at P = 6) are kernel
+// independent, so one pass over them serves V_L, K_L, V_Y and K_Y.
+#include <math.h>
+#include "pb_internal.cuh"
+
+// ---- index tables ------------------------------------------------------------------------------
+__host__ __device__ static inline int mom_index(int a, int b, int c)
+{
+    int n = a + b + c, m = b + c;
+    return n * (n + 1) * (n + 2) / 6 + m * (m + 1) / 2 + c;
+}
+
+__host__ __device__ static constexpr int pb_nk(int P) { return (P + 1) * (P + 2) * (P + 3) / 6; }
+__host__ __device__ static constexpr int pb_nt(int P)
+{
+    int t = 0;
+    for (int a = 0; a <= P; ++a)
+        for (int b = 0; b <= P - a; ++b)
+            for (int c = 0; c <= P - a - b; ++c) t += (P - a - b - c) / 2 + 1;
+    return t;
+}
+
+#define PB_MAX_NK 286   // pb_nk(10)
+__constant__ unsigned char c_ka[PB_MAX_NK], c_kb[PB_MAX_NK], c_kc[PB_MAX_NK];
+__constant__ double c_binom[PB_MAX_P + 1][PB_MAX_P + 1];
+
+static double factorial(int n) { double f = 1; for (int i = 2; i <= n; ++i) f *= i; return f; }
+
+int pb_farfield_setup(pb_ctx* ctx)
+{
+    pb_tree& t = ctx->tree;
+    cudaStream_t st = ctx->stream;
+    const int P = ctx->prm.order_P;
+    t.P = P;
+    t.Nk = pb_nk(P);
+    t.NT = pb_nt(P);
+    if (ctx->prm.theta <= 0.0) return PB_OK;   // direct mode: no far field
+    // exponent tables
+    unsigned char ka[PB_MAX_NK], kb[PB_MAX_NK], kc[PB_MAX_NK];
+    for (int a = 0; a <= P; ++a)
+        for (int b = 0; b <= P - a; ++b)
+            for (int c = 0; c <= P - a - b; ++c) {
+                int k = mom_index(a, b, c);
+                ka[k] = (unsigned char)a; kb[k] = (unsigned char)b; kc[k] = (unsigned char)c;
+            }
+    double binom[PB_MAX_P + 1][PB_MAX_P + 1];
+    for (int n = 0; n <= PB_MAX_P; ++n)
+        for (int k = 0; k <= PB_MAX_P; ++k) binom[n][k] = k <= n ? factorial(n) / (factorial(k) * factorial(n - k)) : 0.0;
+    PB_CUDA(cudaMemcpyToSymbolAsync(c_ka, ka, t.Nk, 0, cudaMemcpyHostToDevice, st));
+    PB_CUDA(cudaMemcpyToSymbolAsync(c_kb, kb, t.Nk, 0, cudaMemcpyHostToDevice, st));
+    PB_CUDA(cudaMemcpyToSymbolAsync(c_kc, kc, t.Nk, 0, cudaMemcpyHostToDevice, st));
+    PB_CUDA(cudaMemcpyToSymbolAsync(c_binom, binom, sizeof(binom), 0, cudaMemcpyHostToDevice, st));
+    // conversion table M -> F, entries in the order the M2P kernel consumes them
+    std::vector<int32_t> off, idx;
+    std::vector<double> coef;
+    off.push_back(0);
+    for (int a = 0; a <= P; ++a)
+        for (int b = 0; b <= P - a; ++b)
+            for (int c = 0; c <= P - a - b; ++c) {
+                int n = a + b + c;
+                for (int j = 0; j <= (P - n) / 2; ++j) {
+                    double pref = ((j & 1) ? -1.0 : 1.0) / (ldexp(1.0, j) * factorial(a) * factorial(b) * factorial(c));
+                    for (int ba = 0; ba <= j; ++ba)
+                        for (int bb = 0; bb <= j - ba; ++bb) {
+                            int bc = j - ba - bb;
+                            idx.push_back(mom_index(a + 2 * ba, b + 2 * bb, c + 2 * bc));
+                            coef.push_back(pref / (factorial(ba) * factorial(bb) * factorial(bc)));
+                        }
+                    off.push_back((int32_t)idx.size());
+                }
+            }
+    if ((int)off.size() - 1 != t.NT) return pb_fail(ctx, PB_ERR_INVALID_ARG, "internal: far-field term count mismatch");
+    PB_TRY(pb_dalloc_t(ctx, &t.cv_off, off.size(), CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.cv_idx, idx.size(), CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.cv_coef, coef.size(), CAT_TREE));
+    PB_CUDA(cudaMemcpyAsync(t.cv_off, off.data(), sizeof(int32_t) * off.size(), cudaMemcpyHostToDevice, st));
+    PB_CUDA(cudaMemcpyAsync(t.cv_idx, idx.data(), sizeof(int32_t) * idx.size(), cudaMemcpyHostToDevice, st));
+    PB_CUDA(cudaMemcpyAsync(t.cv_coef, coef.data(), sizeof(double) * coef.size(), cudaMemcpyHostToDevice, st));
+    PB_CUDA(cudaStreamSynchronize(st));   // host vectors go out of scope
+    PB_TRY(pb_dalloc_t(ctx, &t.M, (size_t)t.n_cells * 2 * t.Nk, CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.FF, (size_t)t.n_cells * t.NT, CAT_TREE));
+    return PB_OK;
+}
+
+// ---- source weights (H5): q^V_g = w_g A_j dphi_j ,  q^K_g = w_g A_j phi_j n_j ------------------------
+__global__ void k_weights(int64_t N, int K, const int32_t* __restrict__ perm, const double* __restrict__ x,
+                          const double* __restrict__ swA, const double* __restrict__ nx,
+                          const double* __restrict__ ny, const double* __restrict__ nz, double* __restrict__ xphi,
+                          double* __restrict__ xdphi, double* __restrict__ qV, double* __restrict__ qKx,
+                          double* __restrict__ qKy, double* __restrict__ qKz)
+{
+    int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (s >= N * K) return;
+    int64_t i = s / K;
+    int64_t o = perm[i];
+    double phi = x[o], dphi = x[N + o], w = swA[s];
+    if (s == i * K) { xphi[i] = phi; xdphi[i] = dphi; }
+    qV[s] = w * dphi;
+    double wp = w * phi;
+    qKx[s] = wp * nx[i];
+    qKy[s] = wp * ny[i];
+    qKz[s] = wp * nz[i];
+}
+
+int pb_weights(pb_ctx* ctx, const double* x)
+{
+    pb_tree& t = ctx->tree;
+    k_weights<<<pb_blocks(t.Ns, 256), 256, 0, ctx->stream>>>(t.N, t.K, t.perm, x, t.swA, t.pn[0], t.pn[1], t.pn[2],
+                                                            t.xphi, t.xdphi, t.qV, t.qK[0], t.qK[1], t.qK[2]);
+    PB_LAUNCH_CHECK();
+    return PB_OK;
+}
+
+// ---- P2M at the leaves: M^V_k = sum_g q^V_g h^k,  M^K_k = sum_g sum_d q^K_{g,d} k_d h^{k-e_d} ---
+#define P2M_CH 32
+__global__ void __launch_bounds__(128)
+k_p2m_leaf(int P, int Nk, int K, const int32_t* __restrict__ leaf_ids, const int32_t* __restrict__ c_first,
+           const int32_t* __restrict__ c_last, const double* __restrict__ cx, const double* __restrict__ cy,
+           const double* __restrict__ cz, const double* __restrict__ sx, const double* __restrict__ sy,
+           const double* __restrict__ sz, const double* __restrict__ qV, const double* __restrict__ qKx,
+           const double* __restrict__ qKy, const double* __restrict__ qKz, double* __restrict__ M)
+{
+    __shared__ double pw[3][PB_MAX_P + 1][P2M_CH];
+    __shared__ double wq[4][P2M_CH];
+    const int32_t c = leaf_ids[blockIdx.x];
+    const int64_t s0 = (int64_t)c_first[c] * K, s1 = (int64_t)c_last[c] * K;
+    const double yc[3] = {cx[c], cy[c], cz[c]};
+    double mv[3] = {0, 0, 0}, mk[3] = {0, 0, 0};   // up to 3 terms per thread (Nk <= 286 < 3*128)
+    for (int64_t base = s0; base < s1; base += P2M_CH) {
+        int np = (int)((s1 - base) < P2M_CH ? (s1 - base) : P2M_CH);
+        __syncthreads();
+        if (threadIdx.x < np) {
+            int64_t s = base + threadIdx.x;
+            double h[3] = {sx[s] - yc[0], sy[s] - yc[1], sz[s] - yc[2]};
+            for (int d = 0; d < 3; ++d) {
+                double p = 1.0;
+                for (int e = 0; e <= P; ++e) { pw[d][e][threadIdx.x] = p; p *= h[d]; }
+            }
+            wq[0][threadIdx.x] = qV[s];
+            wq[1][threadIdx.x] = qKx[s];
+            wq[2][threadIdx.x] = qKy[s];
+            wq[3][threadIdx.x] = qKz[s];
+        }
+        __syncthreads();
+        for (int r = 0; r < 3; ++r) {
+            int k = threadIdx.x + r * 128;
+            if (k >= Nk) break;
+            int a = c_ka[k], b = c_kb[k], cc = c_kc[k];
+            double sv = 0, sk = 0;
+            for (int p = 0; p < np; ++p) {
+                double xa = pw[0][a][p], yb = pw[1][b][p], zc = pw[2][cc][p];
+                sv += wq[0][p] * xa * yb * zc;
+                double t = 0;
+                if (a) t += wq[1][p] * a * pw[0][a - 1][p] * yb * zc;
+                if (b) t += wq[2][p] * b * xa * pw[1][b - 1][p] * zc;
+                if (cc) t += wq[3][p] * cc * xa * yb * pw[2][cc - 1][p];
+                sk += t;
+            }
+            mv[r] += sv;
+            mk[r] += sk;
+        }
+    }
+    for (int r = 0; r < 3; ++r) {
+        int k = threadIdx.x + r * 128;
+        if (k >= Nk) break;
+        M[((int64_t)c * 2 + 0) * Nk + k] = mv[r];
+        M[((int64_t)c * 2 + 1) * Nk + k] = mk[r];
+    }
+}
+
+// ---- M2M: moments of a parent from its children, M'_k = sum_{l<=k} C(k,l) t^{k-l} M_l -------------
+__global__ void __launch_bounds__(128)
+k_m2m(int64_t c0, int P, int Nk, const int32_t* __restrict__ c_child, const int32_t* __restrict__ c_nchild,
+      const double* __restrict__ cx, const double* __restrict__ cy, const double* __restrict__ cz,
+      double* __restrict__ M)
+{
+    __shared__ double cm[2][PB_MAX_NK];
+    __shared__ double tp[3][PB_MAX_P + 1];
+    const int64_t c = c0 + blockIdx.x;
+    const int32_t ch = c_child[c];
+    if (ch < 0) return;
+    const int nc = c_nchild[c];
+    double acc[2][3] = {{0, 0, 0}, {0, 0, 0}};
+    for (int q = 0; q < nc; ++q) {
+        const int64_t cc = ch + q;
+        __syncthreads();
+        for (int k = threadIdx.x; k < 2 * Nk; k += 128) cm[k / Nk][k % Nk] = M[cc * 2 * Nk + k];
+        if (threadIdx.x < 3) {
+            const double* ctr = threadIdx.x == 0 ? cx : (threadIdx.x == 1 ? cy : cz);
+            double tt = ctr[cc] - ctr[c], p = 1.0;
+            for (int e = 0; e <= P; ++e) { tp[threadIdx.x][e] = p; p *= tt; }
+        }
+        __syncthreads();
+        for (int r = 0; r < 3; ++r) {
+            int k = threadIdx.x + r * 128;
+            if (k >= Nk) break;
+            int a = c_ka[k], b = c_kb[k], c3 = c_kc[k];
+            double s0 = 0, s1 = 0;
+            for (int la = 0; la <= a; ++la) {
+                double fa = c_binom[a][la] * tp[0][a - la];
+                for (int lb = 0; lb <= b; ++lb) {
+                    double fb = fa * c_binom[b][lb] * tp[1][b - lb];
+                    for (int lc = 0; lc <= c3; ++lc) {
+                        double f = fb * c_binom[c3][lc] * tp[2][c3 - lc];
+                        int l = mom_index(la, lb, lc);
+                        s0 += f * cm[0][l];
+                        s1 += f * cm[1][l];
+                    }
+                }
+            }
+            acc[0][r] += s0;
+            acc[1][r] += s1;
+        }
+    }
+    for (int r = 0; r < 3; ++r) {
+        int k = threadIdx.x + r * 128;
+        if (k >= Nk) break;
+        M[(c * 2 + 0) * Nk + k] = acc[0][r];
+        M[(c * 2 + 1) * Nk + k] = acc[1][r];
+    }
+}
+
+// ---- M -> F conversion ---------------------------------------------------------------------------------
+__global__ void k_convert(int64_t ncell, int Nk, int NT, const int32_t* __restrict__ cv_off,
+                          const int32_t* __restrict__ cv_idx, const double* __restrict__ cv_coef,
+                          const double* __restrict__ M, double2* __restrict__ FF)
+{
+    int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (g >= ncell * NT) return;
+    int64_t c = g / NT;
+    int e = (int)(g - c * NT);
+    const double* mv = M + c * 2 * Nk;
+    const double* mk = mv + Nk;
+    double v = 0, k = 0;
+    for (int q = cv_off[e]; q < cv_off[e + 1]; ++q) {
+        int l = cv_idx[q];
+        double f = cv_coef[q];
+        v += f * mv[l];
+        k += f * mk[l];
+    }
+    FF[g] = make_double2(v, k);
+}
+
+// ---- M2P (H6; "box-target" interactions) -----------------------------------------------------------
+template <int P>
+__device__ __forceinline__ void m2p_terms(const double2* __restrict__ ff, double dx, double dy, double dz,
+                                          double (&WV)[P + 1], double (&WK)[P + 1])
+{
+    int e = 0;
+    double xa = 1.0;
+#pragma unroll
+    for (int a = 0; a <= P; ++a) {
+        double xy = xa;
+#pragma unroll
+        for (int b = 0; b <= P - a; ++b) {
+            double mono = xy;
+#pragma unroll
+            for (int c = 0; c <= P - a - b; ++c) {
+                const int n = a + b + c;
+#pragma unroll
+                for (int j = 0; j <= (P - n) / 2; ++j) {
+                    const double2 f = ff[e];
+                    ++e;
+                    WV[n + j] = fma(mono, f.x, WV[n + j]);
+                    WK[n + j] = fma(mono, f.y, WK[n + j]);
+                }
+                mono *= dz;
+            }
+            xy *= dy;
+        }
+        xa *= dx;
+    }
+}
+
+// One block per (target group, list slice); one target per thread.  The cell's F terms are
+// staged in shared memory and read as broadcast 16-byte loads.
+template <int P>
+__global__ void __launch_bounds__(PB_TG)
+k_m2p(int64_t N, int nslice, double kappa, const int32_t* __restrict__ m2p_off, const int32_t* __restrict__ m2p_cell,
+      const double* __restrict__ cx, const double* __restrict__ cy, const double* __restrict__ cz,
+      const double2* __restrict__ FF, const double* __restrict__ px, const double* __restrict__ py,
+      const double* __restrict__ pz, double* __restrict__ acc)
+{
+    constexpr int NT = pb_nt(P);
+    __shared__ double2 ff[NT];
+    __shared__ double ctr[3];
+    const int64_t g = blockIdx.x;
+    const int slice = blockIdx.y;
+    const int64_t i = g * PB_TG + threadIdx.x;
+    const bool live = i < N;
+    const double tx = live ? px[i] : 0.0, ty = live ? py[i] : 0.0, tz = live ? pz[i] : 0.0;
+    double VL = 0, KL = 0, VY = 0, KY = 0;
+    const double k2 = kappa * kappa;
+    for (int32_t e = m2p_off[g] + slice; e < m2p_off[g + 1]; e += nslice) {
+        const int32_t c = m2p_cell[e];
+        __syncthreads();
+        for (int q = threadIdx.x; q < NT; q += PB_TG) ff[q] = FF[(int64_t)c * NT + q];
+        if (threadIdx.x == 0) { ctr[0] = cx[c]; ctr[1] = cy[c]; ctr[2] = cz[c]; }
+        __syncthreads();
+        const double dx = tx - ctr[0], dy = ty - ctr[1], dz = tz - ctr[2];
+        double WV[P + 1], WK[P + 1];
+#pragma unroll
+        for (int m = 0; m <= P; ++m) { WV[m] = 0.0; WK[m] = 0.0; }
+        m2p_terms<P>(ff, dx, dy, dz, WV, WK);
+        const double R2 = dx * dx + dy * dy + dz * dz;
+        const double ri = rsqrt(R2), R = R2 * ri, ri2 = ri * ri;
+        const double ex = exp(-kappa * R);
+        double uL = ri, uY0 = ex * ri, uY1 = ex * (1.0 + kappa * R) * ri * ri2;
+        VL = fma(uL, WV[0], VL); KL = fma(uL, WK[0], KL);
+        VY = fma(uY0, WV[0], VY); KY = fma(uY0, WK[0], KY);
+#pragma unroll
+        for (int m = 1; m <= P; ++m) {
+            uL = (2 * m - 1) * uL * ri2;
+            VL = fma(uL, WV[m], VL); KL = fma(uL, WK[m], KL);
+            VY = fma(uY1, WV[m], VY); KY = fma(uY1, WK[m], KY);
+            const double un = ((2 * m + 1) * uY1 + k2 * uY0) * ri2;
+            uY0 = uY1;
+            uY1 = un;
+        }
+    }
+    if (live) {
+        double* a = acc + (int64_t)slice * 4 * N;
+        a[i] = VL; a[N + i] = KL; a[2 * N + i] = VY; a[3 * N + i] = KY;
+    }
+}
+
+// ---- P2P (H7; "source-target" interactions) ---------------------------------------------------------
+// Kernels of Eq. (3)-(4) without the 1/(4 pi), which the combine step applies once:
+//   VL += qV/R, KL += (qK.d)/R^3, VY += qV e^{-kR}/R, KY += (qK.d) e^{-kR}(1+kR)/R^3,  d = x - y.
+#define P2P_TILE 128
+template <bool CHECK_SELF>
+__device__ __forceinline__ void p2p_tile(const double (*__restrict__ sm)[P2P_TILE], int cnt, int32_t s0, int32_t selfLo,
+                                         int K, double kappa, double tx, double ty, double tz, double& VL,
+                                         double& KL, double& VY, double& KY)
+{
+#pragma unroll 2
+    for (int k = 0; k < cnt; ++k) {
+        if (CHECK_SELF && (unsigned)(s0 + k - selfLo) < (unsigned)K) continue;   // own panel: by index (D: R-11)
+        const double dx = tx - sm[0][k], dy = ty - sm[1][k], dz = tz - sm[2][k];
+        const double r2 = dx * dx + dy * dy + dz * dz;
+        const double ri = rsqrt(r2);
+        const double r = r2 * ri, ri3 = ri * ri * ri;
+        const double nd = sm[4][k] * dx + sm[5][k] * dy + sm[6][k] * dz;
+        const double qv = sm[3][k];
+        const double ex = exp(-kappa * r);
+        VL = fma(qv, ri, VL);
+        const double kl = nd * ri3;
+        KL += kl;
+        VY = fma(qv * ri, ex, VY);
+        KY = fma(kl * ex, fma(kappa, r, 1.0), KY);
+    }
+}
+
+__global__ void __launch_bounds__(PB_TG)
+k_p2p(int64_t N, int K, int nslice, double kappa, const int32_t* __restrict__ p2p_off,
+      const int32_t* __restrict__ p2p_lo, const int32_t* __restrict__ p2p_hi, const double* __restrict__ sx,
+      const double* __restrict__ sy, const double* __restrict__ sz, const double* __restrict__ qV,
+      const double* __restrict__ qKx, const double* __restrict__ qKy, const double* __restrict__ qKz,
+      const double* __restrict__ px, const double* __restrict__ py, const double* __restrict__ pz,
+      double* __restrict__ acc)
+{
+    __shared__ double sm[7][P2P_TILE];
+    const int64_t g = blockIdx.x;
+    const int slice = blockIdx.y;
+    const int64_t i = g * PB_TG + threadIdx.x;
+    const bool live = i < N;
+    const double tx = live ? px[i] : 1e30, ty = live ? py[i] : 1e30, tz = live ? pz[i] : 1e30;
+    const int32_t selfLo = (int32_t)(i * K);
+    const int64_t i1 = (g + 1) * PB_TG < N ? (g + 1) * PB_TG : N;
+    const int32_t grpLo = (int32_t)(g * PB_TG * K), grpHi = (int32_t)(i1 * K);
+    double VL = 0, KL = 0, VY = 0, KY = 0;
+    int64_t tile = 0;
+    for (int32_t r = p2p_off[g]; r < p2p_off[g + 1]; ++r) {
+        const int32_t lo = p2p_lo[r], hi = p2p_hi[r];
+        for (int32_t s0 = lo; s0 < hi; s0 += P2P_TILE, ++tile) {
+            if ((int)(tile % nslice) != slice) continue;
+            const int cnt = hi - s0 < P2P_TILE ? hi - s0 : P2P_TILE;
+            __syncthreads();
+            for (int k = threadIdx.x; k < cnt; k += PB_TG) {
+                sm[0][k] = sx[s0 + k]; sm[1][k] = sy[s0 + k]; sm[2][k] = sz[s0 + k]; sm[3][k] = qV[s0 + k];
+                sm[4][k] = qKx[s0 + k]; sm[5][k] = qKy[s0 + k]; sm[6][k] = qKz[s0 + k];
+            }
+            __syncthreads();
+            if (s0 < grpHi && s0 + cnt > grpLo)
+                p2p_tile<true>(sm, cnt, s0, selfLo, K, kappa, tx, ty, tz, VL, KL, VY, KY);
+            else
+                p2p_tile<false>(sm, cnt, s0, selfLo, K, kappa, tx, ty, tz, VL, KL, VY, KY);
+        }
+    }
+    if (live) {
+        double* a = acc + (int64_t)slice * 4 * N;
+        a[i] = VL; a[N + i] = KL; a[2 * N + i] = VY; a[3 * N + i] = KY;
+    }
+}
+
+// ---- near/singular table + Eq. (5) combine + un-permute (H8) ------------------------------------------------
+__global__ void k_combine(int64_t N, int nsP, int nsM, double eps_ratio, const double* __restrict__ accP,
+                          const double* __restrict__ accM, const int32_t* __restrict__ nr_off,
+                          const int32_t* __restrict__ nr_col, const double* __restrict__ nr_val, int64_t ne,
+                          const double* __restrict__ xphi, const double* __restrict__ xdphi,
+                          const int32_t* __restrict__ perm, double* __restrict__ y)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    double s[4] = {0, 0, 0, 0};
+    for (int q = 0; q < nsP; ++q)
+        for (int m = 0; m < 4; ++m) s[m] += accP[((int64_t)q * 4 + m) * N + i];
+    for (int q = 0; q < nsM; ++q)
+        for (int m = 0; m < 4; ++m) s[m] += accM[((int64_t)q * 4 + m) * N + i];
+    double VL = PB_INV4PI * s[0], KL = PB_INV4PI * s[1], VY = PB_INV4PI * s[2], KY = PB_INV4PI * s[3];
+    for (int32_t e = nr_off[i]; e < nr_off[i + 1]; ++e) {
+        int32_t j = nr_col[e];
+        double ph = xphi[j], dp = xdphi[j];
+        VL = fma(nr_val[e], dp, VL);
+        KL = fma(nr_val[ne + e], ph, KL);
+        VY = fma(nr_val[2 * ne + e], dp, VY);
+        KY = fma(nr_val[3 * ne + e], ph, KY);
+    }
+    const double phi = xphi[i];
+    const int64_t o = perm[i];
+    y[o] = 0.5 * phi + KL - VL;                    // Eq. (5), first row
+    y[N + o] = 0.5 * phi - KY + eps_ratio * VY;    // Eq. (5), second row
+}
+
+// ---- host driver ----------------------------------------------------------------------------------------------
+template <int P>
+static void launch_m2p(pb_ctx* ctx)
+{
+    pb_tree& t = ctx->tree;
+    dim3 grid((unsigned)t.n_groups, (unsigned)t.nslice_m2p);
+    k_m2p<P><<<grid, PB_TG, 0, ctx->stream>>>(t.N, t.nslice_m2p, ctx->prm.kappa, t.m2p_off, t.m2p_cell, t.c_ctr[0],
+                                            t.c_ctr[1], t.c_ctr[2], t.FF, t.pc[0], t.pc[1], t.pc[2], t.accM);
+}
+
+int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed)
+{
+    pb_tree& t = ctx->tree;
+    cudaStream_t st = ctx->stream;
+    if (!t.built) return pb_fail(ctx, PB_ERR_NOT_READY, "pb_matvec: call pb_tree_build first");
+    if (!x || !y || x == y) return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_matvec: x and y must be distinct non-NULL device arrays");
+    if (timed && !ctx->ev_made) {
+        for (int k = 0; k < 8; ++k) PB_CUDA(cudaEventCreate(&ctx->ev[k]));
+        ctx->ev_made = true;
+    }
+    const bool far = ctx->prm.theta > 0.0;
+    if (timed) PB_CUDA(cudaEventRecord(ctx->ev[0], st));
+    PB_TRY(pb_weights(ctx, x));
+    if (timed) PB_CUDA(cudaEventRecord(ctx->ev[1], st));
+    if (far) {
+        k_p2m_leaf<<<(unsigned)t.n_leaves, 128, 0, st>>>(t.P, t.Nk, t.K, t.leaf_ids, t.c_first, t.c_last, t.c_ctr[0],
+                                                        t.c_ctr[1], t.c_ctr[2], t.sx[0], t.sx[1], t.sx[2], t.qV,
+                                                        t.qK[0], t.qK[1], t.qK[2], t.M);
+        PB_LAUNCH_CHECK();
+        for (int g = (int)t.gen_start.size() - 2; g >= 0; --g) {
+            int64_t c0 = t.gen_start[g], c1 = t.gen_start[g + 1];
+            k_m2m<<<(unsigned)(c1 - c0), 128, 0, st>>>(c0, t.P, t.Nk, t.c_child, t.c_nchild, t.c_ctr[0], t.c_ctr[1],
+                                                      t.c_ctr[2], t.M);
+            PB_LAUNCH_CHECK();
+        }
+        k_convert<<<pb_blocks(t.n_cells * t.NT, 256), 256, 0, st>>>(t.n_cells, t.Nk, t.NT, t.cv_off, t.cv_idx, t.cv_coef,
+                                                                   t.M, t.FF);
+        PB_LAUNCH_CHECK();
+    }
+    if (timed) PB_CUDA(cudaEventRecord(ctx->ev[2], st));
+    if (far) {
+        switch (t.P) {
+        case 0: launch_m2p<0>(ctx); break;
+        case 1: launch_m2p<1>(ctx); break;
+        case 2: launch_m2p<2>(ctx); break;
+        case 3: launch_m2p<3>(ctx); break;
+        case 4: launch_m2p<4>(ctx); break;
+        case 5: launch_m2p<5>(ctx); break;
+        case 6: launch_m2p<6>(ctx); break;
+        case 7: launch_m2p<7>(ctx); break;
+        case 8: launch_m2p<8>(ctx); break;
+        case 9: launch_m2p<9>(ctx); break;
+        case 10: launch_m2p<10>(ctx); break;
+        default: return pb_fail(ctx, PB_ERR_INVALID_ARG, "unsupported order_P %d", t.P);
+        }
+        PB_LAUNCH_CHECK();
+    }
+    if (timed) PB_CUDA(cudaEventRecord(ctx->ev[3], st));
+    {
+        dim3 grid((unsigned)t.n_groups, (unsigned)t.nslice_p2p);
+        k_p2p<<<grid, PB_TG, 0, st>>>(t.N, t.K, t.nslice_p2p, ctx->prm.kappa, t.p2p_off, t.p2p_lo, t.p2p_hi, t.sx[0],
+                                      t.sx[1], t.sx[2], t.qV, t.qK[0], t.qK[1], t.qK[2], t.pc[0], t.pc[1], t.pc[2],
+                                      t.accP);
+        PB_LAUNCH_CHECK();
+    }
+    if (timed) PB_CUDA(cudaEventRecord(ctx->ev[4], st));
+    k_combine<<<pb_blocks(t.N, 128), 128, 0, st>>>(t.N, t.nslice_p2p, far ? t.nslice_m2p : 0,
+                                                  ctx->prm.eps_in / ctx->prm.eps_out, t.accP, t.accM, t.nr_off,
+                                                  t.nr_col, t.nr_val, t.near_entries, t.xphi, t.xdphi, t.perm, y);
+    PB_LAUNCH_CHECK();
+    ctx->matvec_calls++;
+    if (timed) {
+        PB_CUDA(cudaEventRecord(ctx->ev[5], st));
+        PB_CUDA(cudaEventSynchronize(ctx->ev[5]));
+        float ms;
+        for (int k = 0; k < 5; ++k) {
+            PB_CUDA(cudaEventElapsedTime(&ms, ctx->ev[k], ctx->ev[k + 1]));
+            ctx->last_ms[k] = ms;
+        }
+        PB_CUDA(cudaEventElapsedTime(&ms, ctx->ev[0], ctx->ev[5]));
+        ctx->last_ms[5] = ms;
+    }
+    return PB_OK;
+}
+
+extern "C" int pb_matvec(pb_ctx* ctx, const double* x, double* y)
+{
+    if (!ctx) return PB_ERR_INVALID_ARG;
+    return pb_matvec_impl(ctx, x, y, false);
+}
+
+extern "C" int pb_matvec_timed(pb_ctx* ctx, const double* x, double* y)
+{
+    if (!ctx) return PB_ERR_INVALID_ARG;
+    return pb_matvec_impl(ctx, x, y, true);
+}
+
+extern "C" int pb_matvec_host(pb_ctx* ctx, const double* x_host, double* y_host)
+{
+    if (!ctx) return PB_ERR_INVALID_ARG;
+    if (!ctx->tree.built) return pb_fail(ctx, PB_ERR_NOT_READY, "pb_matvec_host: call pb_tree_build first");
+    if (!x_host || !y_host) return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_matvec_host: NULL buffer");
+    const size_t n = 2 * (size_t)ctx->nt;
+    PB_TRY(pb_scratch(ctx, 2 * n * sizeof(double) + 4096));
+    double* dx = ctx->scratch;
+    double* dy = ctx->scratch + n;
+    PB_CUDA(cudaMemcpyAsync(dx, x_host, n * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    PB_TRY(pb_matvec_impl(ctx, dx, dy, false));
+    PB_CUDA(cudaMemcpyAsync(y_host, dy, n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    PB_CUDA(cudaStreamSynchronize(ctx->stream));
+    return PB_OK;
+}

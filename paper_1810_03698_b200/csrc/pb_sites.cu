@@ -1,0 +1,393 @@
+// pb_sites.cu -- atom-side kernels: multipole right-hand side Eq. (8), reaction
+// potential / field / field gradient of the surface layers Eq. (12), (13), (21)
+// and the Coulomb field of the multipoles with group mask and Thole damping Eq. (14), (31), (32)
+// (derivative tensors re-derived in D: App. A.2, A.5).
+#include <math.h>
+#include "pb_internal.cuh"
+
+// ---- H10: right-hand side -----------------------------------------------------------------------------
+// b_i = 1/(4 pi eps_in) sum_k [ q_k/R + p_k.d/R^3 + d.Q_k.d/(2 R^5) ],  d = c_i - r_k,  p = dip + mu.
+#define RHS_TILE 64
+__global__ void __launch_bounds__(128)
+k_rhs(int64_t N, int64_t na, const double* __restrict__ cen, const double* __restrict__ pos,
+      const double* __restrict__ q, const double* __restrict__ dip, const double* __restrict__ mu,
+      const double* __restrict__ quad, double inv_eps, double* __restrict__ b)
+{
+    __shared__ double s[13][RHS_TILE];
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const bool live = i < N;
+    const double x = live ? cen[3 * i] : 1e30, y = live ? cen[3 * i + 1] : 1e30, z = live ? cen[3 * i + 2] : 1e30;
+    double sum = 0;
+    for (int64_t k0 = 0; k0 < na; k0 += RHS_TILE) {
+        const int cnt = (int)(na - k0 < RHS_TILE ? na - k0 : RHS_TILE);
+        __syncthreads();
+        for (int k = threadIdx.x; k < cnt; k += blockDim.x) {
+            const int64_t m = k0 + k;
+            for (int d = 0; d < 3; ++d) {
+                s[d][k] = pos[3 * m + d];
+                s[4 + d][k] = dip[3 * m + d] + (mu ? mu[3 * m + d] : 0.0);
+            }
+            s[3][k] = q[m];
+            for (int d = 0; d < 6; ++d) s[7 + d][k] = quad[6 * m + d];
+        }
+        __syncthreads();
+        for (int k = 0; k < cnt; ++k) {
+            const double dx = x - s[0][k], dy = y - s[1][k], dz = z - s[2][k];
+            const double r2 = dx * dx + dy * dy + dz * dz;
+            const double ri = rsqrt(r2), ri2 = ri * ri, ri3 = ri * ri2, ri5 = ri3 * ri2;
+            const double pd = s[4][k] * dx + s[5][k] * dy + s[6][k] * dz;
+            const double dQd = s[7][k] * dx * dx + s[10][k] * dy * dy + s[12][k] * dz * dz +
+                               2.0 * (s[8][k] * dx * dy + s[9][k] * dx * dz + s[11][k] * dy * dz);
+            sum += s[3][k] * ri + pd * ri3 + 0.5 * dQd * ri5;
+        }
+    }
+    if (live) {
+        b[i] = PB_INV4PI * inv_eps * sum;
+        b[N + i] = 0.0;   // second block of Eq. (5)'s right side
+    }
+}
+
+extern "C" int pb_rhs_multipole(pb_ctx* ctx, const double* mu_induced, double* b)
+{
+    if (!ctx) return PB_ERR_INVALID_ARG;
+    if (!ctx->mesh_loaded || !ctx->sites.loaded) return pb_fail(ctx, PB_ERR_NOT_READY, "pb_rhs_multipole: load mesh and sites first");
+    if (!b) return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_rhs_multipole: NULL output");
+    const pb_sites& s = ctx->sites;
+    k_rhs<<<pb_blocks(ctx->nt, 128), 128, 0, ctx->stream>>>(ctx->nt, s.na, ctx->cen, s.pos, s.q, s.dip, mu_induced, s.quad,
+                                                          1.0 / ctx->prm.eps_in, b);
+    PB_LAUNCH_CHECK();
+    return PB_OK;
+}
+
+// ---- H11: reaction potential, field, field gradient at the sites ---------------------------------------
+// One source point y with single-layer weight wS (= w A dphi) and double-layer vector
+// wK (= w A phi n') adds, at a target with d = r - y (times 1/(4 pi), applied at the end):
+//   phi  += wS/R - (wK.d)/R^3
+//   grad += -wS d/R^3 - [ wK/R^3 - 3 (wK.d) d/R^5 ]
+//   hess += wS (3 d d^T/R^5 - I/R^3) + 3 [wK d^T + d wK^T + (wK.d) I]/R^5 - 15 (wK.d) d d^T/R^7
+template <bool HESS>
+__device__ __forceinline__ void react_point(double dx, double dy, double dz, double wS, double kx, double ky,
+                                            double kz, double* __restrict__ o)
+{
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    const double ri = rsqrt(r2), ri2 = ri * ri, ri3 = ri * ri2, ri5 = ri3 * ri2;
+    const double kd = kx * dx + ky * dy + kz * dz;
+    o[0] += wS * ri - kd * ri3;
+    const double g = -wS * ri3 + 3.0 * kd * ri5;   // coefficient of d
+    o[1] += g * dx - kx * ri3;
+    o[2] += g * dy - ky * ri3;
+    o[3] += g * dz - kz * ri3;
+    if (HESS) {
+        const double ri7 = ri5 * ri2;
+        const double a = 3.0 * wS * ri5 - 15.0 * kd * ri7;    // coefficient of d d^T
+        const double dl = -wS * ri3 + 3.0 * kd * ri5;         // coefficient of I
+        const double c3 = 3.0 * ri5;
+        o[4] += a * dx * dx + dl + c3 * 2.0 * kx * dx;
+        o[5] += a * dx * dy + c3 * (kx * dy + ky * dx);
+        o[6] += a * dx * dz + c3 * (kx * dz + kz * dx);
+        o[7] += a * dy * dy + dl + c3 * 2.0 * ky * dy;
+        o[8] += a * dy * dz + c3 * (ky * dz + kz * dy);
+        o[9] += a * dz * dz + dl + c3 * 2.0 * kz * dz;
+    }
+}
+
+#define RF_ST 4        // sites per block (register tile)
+#define RF_THREADS 128
+template <bool HESS>
+__global__ void __launch_bounds__(RF_THREADS)
+k_reaction(int64_t Ns, int64_t chunk, int64_t na, const double* __restrict__ pos, const double* __restrict__ sx,
+           const double* __restrict__ sy, const double* __restrict__ sz, const double* __restrict__ qV,
+           const double* __restrict__ qKx, const double* __restrict__ qKy, const double* __restrict__ qKz,
+           double* __restrict__ partial /*[gridDim.x][na][10]*/)
+{
+    constexpr int NO = HESS ? 10 : 4;
+    __shared__ double red[RF_THREADS / 32][RF_ST][NO];
+    const int64_t m0 = (int64_t)blockIdx.y * RF_ST;
+    double r[RF_ST][3];
+    double acc[RF_ST][NO];
+#pragma unroll
+    for (int t = 0; t < RF_ST; ++t) {
+        const int64_t m = m0 + t < na ? m0 + t : na - 1;   // clamp: duplicates are not written
+        r[t][0] = pos[3 * m]; r[t][1] = pos[3 * m + 1]; r[t][2] = pos[3 * m + 2];
+#pragma unroll
+        for (int c = 0; c < NO; ++c) acc[t][c] = 0.0;
+    }
+    const int64_t s0 = blockIdx.x * chunk, s1 = s0 + chunk < Ns ? s0 + chunk : Ns;
+    for (int64_t s = s0 + threadIdx.x; s < s1; s += RF_THREADS) {
+        const double yx = sx[s], yy = sy[s], yz = sz[s], wS = qV[s], kx = qKx[s], ky = qKy[s], kz = qKz[s];
+#pragma unroll
+        for (int t = 0; t < RF_ST; ++t) react_point<HESS>(r[t][0] - yx, r[t][1] - yy, r[t][2] - yz, wS, kx, ky, kz, acc[t]);
+    }
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+    for (int t = 0; t < RF_ST; ++t)
+#pragma unroll
+        for (int c = 0; c < NO; ++c) {
+            double v = acc[t][c];
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            if (lane == 0) red[w][t][c] = v;
+        }
+    __syncthreads();
+    if (threadIdx.x < RF_ST * NO) {
+        const int t = threadIdx.x / NO, c = threadIdx.x % NO;
+        if (m0 + t < na) {
+            double v = 0;
+            for (int k = 0; k < RF_THREADS / 32; ++k) v += red[k][t][c];
+            partial[((int64_t)blockIdx.x * na + (m0 + t)) * 10 + c] = v;
+        }
+    }
+}
+
+// sum the per-chunk partials (fixed order), apply 1/(4 pi), write phi/grad/hess
+__global__ void k_reaction_finish(int64_t na, int nchunk, int NO, const double* __restrict__ partial,
+                                  double* __restrict__ phi, double* __restrict__ grad, double* __restrict__ hess)
+{
+    int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (g >= na * NO) return;
+    int64_t m = g / NO;
+    int c = (int)(g % NO);
+    double v = 0;
+    for (int k = 0; k < nchunk; ++k) v += partial[((int64_t)k * na + m) * 10 + c];
+    v *= PB_INV4PI;
+    if (c == 0) { if (phi) phi[m] = v; }
+    else if (c < 4) { if (grad) grad[3 * m + c - 1] = v; }
+    else if (hess) hess[6 * m + c - 4] = v;
+}
+
+// near (site, panel) pairs: |r_m - c_j| < tau*sqrt(A_j) (D: R-9).  Thread per panel.
+template <int PASS>
+__global__ void k_site_near_find(int64_t N, int64_t na, double tau, const double* __restrict__ px,
+                                 const double* __restrict__ py, const double* __restrict__ pz,
+                                 const double* __restrict__ parea, const double* __restrict__ pos,
+                                 int32_t* __restrict__ cnt, const int32_t* __restrict__ off,
+                                 int32_t* __restrict__ psite, int32_t* __restrict__ ppanel)
+{
+    int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (j >= N) return;
+    const double x = px[j], y = py[j], z = pz[j], rho = tau * sqrt(parea[j]);
+    int n = 0;
+    int64_t o = PASS ? off[j] : 0;
+    for (int64_t m = 0; m < na; ++m) {
+        double dx = pos[3 * m] - x, dy = pos[3 * m + 1] - y, dz = pos[3 * m + 2] - z;
+        if (sqrt(dx * dx + dy * dy + dz * dz) < rho) {
+            if (PASS) { psite[o + n] = (int32_t)m; ppanel[o + n] = (int32_t)j; }
+            ++n;
+        }
+    }
+    if (!PASS) cnt[j] = n;
+}
+
+int pb_site_near_build(pb_ctx* ctx)
+{
+    pb_tree& t = ctx->tree;
+    pb_sites& s = ctx->sites;
+    cudaStream_t st = ctx->stream;
+    pb_dfree_cat(ctx, CAT_SITE_NEAR);
+    s.near_built = false;
+    int32_t *cnt, *off;
+    PB_TRY(pb_dalloc_t(ctx, &cnt, t.N + 1, CAT_SITE_NEAR));
+    PB_TRY(pb_dalloc_t(ctx, &off, t.N + 1, CAT_SITE_NEAR));
+    PB_CUDA(cudaMemsetAsync(cnt, 0, sizeof(int32_t) * (t.N + 1), st));
+    k_site_near_find<0><<<pb_blocks(t.N, 128), 128, 0, st>>>(t.N, s.na, ctx->prm.near_tau, t.pc[0], t.pc[1], t.pc[2],
+                                                            t.parea, s.pos, cnt, nullptr, nullptr, nullptr);
+    PB_LAUNCH_CHECK();
+    int64_t np = 0;
+    PB_TRY(pb_exclusive_scan_i32(ctx, cnt, off, t.N + 1, &np));
+    s.n_near = np;
+    PB_TRY(pb_dalloc_t(ctx, &s.near_site, np, CAT_SITE_NEAR));
+    PB_TRY(pb_dalloc_t(ctx, &s.near_panel, np, CAT_SITE_NEAR));
+    if (np > 0) {
+        k_site_near_find<1><<<pb_blocks(t.N, 128), 128, 0, st>>>(t.N, s.na, ctx->prm.near_tau, t.pc[0], t.pc[1], t.pc[2],
+                                                                t.parea, s.pos, cnt, off, s.near_site, s.near_panel);
+        PB_LAUNCH_CHECK();
+    }
+    s.near_built = true;
+    return PB_OK;
+}
+
+// correction of one near (site, panel) pair: K_near-point rule minus the K_far-point rule
+struct rf_corr_args {
+    int64_t np;
+    int K;
+    const int32_t *psite, *ppanel;
+    const double* pos;
+    const double* pv[9];
+    const double *nx, *ny, *nz, *parea, *xphi, *xdphi;
+    const double *sx, *sy, *sz, *qV, *qKx, *qKy, *qKz;
+    double *phi, *grad, *hess;
+};
+
+__global__ void k_reaction_corr(rf_corr_args a, pb_rule_t ruleN)
+{
+    int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (e >= a.np) return;
+    const int32_t m = a.psite[e], j = a.ppanel[e];
+    const double r[3] = {a.pos[3 * m], a.pos[3 * m + 1], a.pos[3 * m + 2]};
+    double v[9];
+    for (int k = 0; k < 9; ++k) v[k] = a.pv[k][j];
+    const double area = a.parea[j], ph = a.xphi[j], dp = a.xdphi[j];
+    const double n[3] = {a.nx[j], a.ny[j], a.nz[j]};
+    double fine[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, coarse[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    for (int g = 0; g < ruleN.K; ++g) {
+        double y[3];
+        for (int c = 0; c < 3; ++c) y[c] = ruleN.lam[g][0] * v[c] + ruleN.lam[g][1] * v[3 + c] + ruleN.lam[g][2] * v[6 + c];
+        const double wa = ruleN.w[g] * area;
+        react_point<true>(r[0] - y[0], r[1] - y[1], r[2] - y[2], wa * dp, wa * ph * n[0], wa * ph * n[1], wa * ph * n[2], fine);
+    }
+    for (int g = 0; g < a.K; ++g) {
+        const int64_t s = (int64_t)j * a.K + g;
+        react_point<true>(r[0] - a.sx[s], r[1] - a.sy[s], r[2] - a.sz[s], a.qV[s], a.qKx[s], a.qKy[s], a.qKz[s], coarse);
+    }
+    if (a.phi) atomicAdd(&a.phi[m], PB_INV4PI * (fine[0] - coarse[0]));
+    if (a.grad)
+        for (int c = 0; c < 3; ++c) atomicAdd(&a.grad[3 * m + c], PB_INV4PI * (fine[1 + c] - coarse[1 + c]));
+    if (a.hess)
+        for (int c = 0; c < 6; ++c) atomicAdd(&a.hess[6 * m + c], PB_INV4PI * (fine[4 + c] - coarse[4 + c]));
+}
+
+extern "C" int pb_reaction_field(pb_ctx* ctx, const double* x, double* phi, double* grad, double* hess)
+{
+    if (!ctx) return PB_ERR_INVALID_ARG;
+    pb_tree& t = ctx->tree;
+    pb_sites& s = ctx->sites;
+    if (!t.built || !s.loaded) return pb_fail(ctx, PB_ERR_NOT_READY, "pb_reaction_field: needs pb_tree_build and pb_sites_load");
+    if (!x) return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_reaction_field: NULL x");
+    if (!phi && !grad && !hess) return PB_OK;
+    cudaStream_t st = ctx->stream;
+    if (!s.near_built) PB_TRY(pb_site_near_build(ctx));
+    PB_TRY(pb_weights(ctx, x));
+    const int64_t ntile = (s.na + RF_ST - 1) / RF_ST;
+    // enough source chunks to fill the GPU, each at least 4 sweeps of the block
+    int64_t nchunk = (148 * 16 + ntile - 1) / ntile;
+    int64_t maxchunk = (t.Ns + 4 * RF_THREADS - 1) / (4 * RF_THREADS);
+    if (nchunk > maxchunk) nchunk = maxchunk;
+    if (nchunk < 1) nchunk = 1;
+    if (nchunk > 1024) nchunk = 1024;
+    int64_t chunk = (t.Ns + nchunk - 1) / nchunk;
+    nchunk = (t.Ns + chunk - 1) / chunk;
+    PB_TRY(pb_scratch(ctx, (size_t)nchunk * s.na * 10 * sizeof(double) + 4096));
+    double* partial = ctx->scratch;
+    dim3 grid((unsigned)nchunk, (unsigned)ntile);
+    const bool H = hess != nullptr;
+    if (H)
+        k_reaction<true><<<grid, RF_THREADS, 0, st>>>(t.Ns, chunk, s.na, s.pos, t.sx[0], t.sx[1], t.sx[2], t.qV, t.qK[0],
+                                                      t.qK[1], t.qK[2], partial);
+    else
+        k_reaction<false><<<grid, RF_THREADS, 0, st>>>(t.Ns, chunk, s.na, s.pos, t.sx[0], t.sx[1], t.sx[2], t.qV, t.qK[0],
+                                                       t.qK[1], t.qK[2], partial);
+    PB_LAUNCH_CHECK();
+    const int NO = H ? 10 : 4;
+    k_reaction_finish<<<pb_blocks(s.na * NO, 128), 128, 0, st>>>(s.na, (int)nchunk, NO, partial, phi, grad, hess);
+    PB_LAUNCH_CHECK();
+    if (s.n_near > 0) {
+        rf_corr_args a;
+        a.np = s.n_near; a.K = t.K; a.psite = s.near_site; a.ppanel = s.near_panel; a.pos = s.pos;
+        for (int k = 0; k < 9; ++k) a.pv[k] = t.pv[k];
+        a.nx = t.pn[0]; a.ny = t.pn[1]; a.nz = t.pn[2]; a.parea = t.parea; a.xphi = t.xphi; a.xdphi = t.xdphi;
+        a.sx = t.sx[0]; a.sy = t.sx[1]; a.sz = t.sx[2]; a.qV = t.qV; a.qKx = t.qK[0]; a.qKy = t.qK[1]; a.qKz = t.qK[2];
+        a.phi = phi; a.grad = grad; a.hess = hess;
+        k_reaction_corr<<<pb_blocks(s.n_near, 64), 64, 0, st>>>(a, ctx->ruleN);
+        PB_LAUNCH_CHECK();
+    }
+    return PB_OK;
+}
+
+// ---- H12: Coulomb potential / field / field gradient of the multipoles at the other sites ------------------
+#define MF_TILE 32
+__global__ void __launch_bounds__(64)
+k_multipole_field(int64_t na, const double* __restrict__ pos, const double* __restrict__ q,
+                  const double* __restrict__ dip, const double* __restrict__ quad, const double* __restrict__ mu,
+                  const double* __restrict__ alpha, const int32_t* __restrict__ group, double thole_a, double inv_eps,
+                  int use_mask, double* __restrict__ phi, double* __restrict__ grad, double* __restrict__ hess)
+{
+    __shared__ double s[17][MF_TILE];
+    __shared__ int32_t sg[MF_TILE];
+    const int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const bool live = l < na;
+    const int64_t lc = live ? l : na - 1;
+    const double x = pos[3 * lc], y = pos[3 * lc + 1], z = pos[3 * lc + 2], al = alpha[lc];
+    const int32_t gl = group[lc];
+    double P = 0, G[3] = {0, 0, 0}, H[6] = {0, 0, 0, 0, 0, 0};
+    for (int64_t m0 = 0; m0 < na; m0 += MF_TILE) {
+        const int cnt = (int)(na - m0 < MF_TILE ? na - m0 : MF_TILE);
+        __syncthreads();
+        for (int k = threadIdx.x; k < cnt; k += blockDim.x) {
+            const int64_t m = m0 + k;
+            for (int d = 0; d < 3; ++d) {
+                s[d][k] = pos[3 * m + d];
+                s[4 + d][k] = dip[3 * m + d];
+                s[13 + d][k] = mu ? mu[3 * m + d] : 0.0;
+            }
+            s[3][k] = q[m];
+            for (int d = 0; d < 6; ++d) s[7 + d][k] = quad[6 * m + d];
+            s[16][k] = alpha[m];
+            sg[k] = group[m];
+        }
+        __syncthreads();
+        if (!live) continue;
+        for (int k = 0; k < cnt; ++k) {
+            if (m0 + k == l) continue;
+            const double d[3] = {x - s[0][k], y - s[1][k], z - s[2][k]};
+            const double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+            const double R = sqrt(r2), i1 = 1.0 / R, i2 = i1 * i1, i3 = i1 * i2, i5 = i3 * i2, i7 = i5 * i2, i9 = i7 * i2;
+            if (!(use_mask && sg[k] == gl)) {
+                // permanent charge, dipole, quadrupole of m (Eq. 7, 31, 32 with the corrections of App. A.2)
+                const double qm = s[3][k];
+                const double p[3] = {s[4][k], s[5][k], s[6][k]};
+                const double Q[6] = {s[7][k], s[8][k], s[9][k], s[10][k], s[11][k], s[12][k]};
+                const double pd = p[0] * d[0] + p[1] * d[1] + p[2] * d[2];
+                const double Qd[3] = {Q[0] * d[0] + Q[1] * d[1] + Q[2] * d[2], Q[1] * d[0] + Q[3] * d[1] + Q[4] * d[2],
+                                      Q[2] * d[0] + Q[4] * d[1] + Q[5] * d[2]};
+                const double dQd = Qd[0] * d[0] + Qd[1] * d[1] + Qd[2] * d[2];
+                P += qm * i1 + pd * i3 + 0.5 * dQd * i5;
+                const double gd = -qm * i3 - 3.0 * pd * i5 - 2.5 * dQd * i7;   // coefficient of d in the gradient
+                for (int c = 0; c < 3; ++c) G[c] += gd * d[c] + p[c] * i3 + Qd[c] * i5;
+                const double hdd = 3.0 * qm * i5 + 15.0 * pd * i7 + 17.5 * dQd * i9;   // coefficient of d d^T
+                const double hI = -qm * i3 - 3.0 * pd * i5 - 2.5 * dQd * i7;           // coefficient of I
+                int idx = 0;
+                for (int a = 0; a < 3; ++a)
+                    for (int b = a; b < 3; ++b, ++idx)
+                        H[idx] += hdd * d[a] * d[b] + (a == b ? hI : 0.0) - 3.0 * (p[a] * d[b] + p[b] * d[a]) * i5 +
+                                  Q[idx] * i5 - 5.0 * (Qd[a] * d[b] + Qd[b] * d[a]) * i7;
+            }
+            if (mu) {
+                // induced dipole of m: never masked, Thole-damped (App. A.5)
+                const double u[3] = {s[13][k], s[14][k], s[15][k]};
+                double l3 = 1.0, l5 = 1.0, l7 = 1.0;
+                const double aa = al * s[16][k];
+                if (aa > 0.0) {
+                    const double au3 = thole_a * r2 * R / sqrt(aa);
+                    const double E = exp(-au3);
+                    l3 = 1.0 - E;
+                    l5 = 1.0 - (1.0 + au3) * E;
+                    l7 = 1.0 - (1.0 + au3 + 0.6 * au3 * au3) * E;
+                }
+                const double ud = u[0] * d[0] + u[1] * d[1] + u[2] * d[2];
+                P += l3 * ud * i3;
+                for (int c = 0; c < 3; ++c) G[c] += l3 * u[c] * i3 - 3.0 * l5 * ud * d[c] * i5;
+                int idx = 0;
+                for (int a = 0; a < 3; ++a)
+                    for (int b = a; b < 3; ++b, ++idx)
+                        H[idx] += -3.0 * l5 * (u[a] * d[b] + u[b] * d[a] + (a == b ? ud : 0.0)) * i5 +
+                                  15.0 * l7 * ud * d[a] * d[b] * i7;
+            }
+        }
+    }
+    if (!live) return;
+    const double sc = PB_INV4PI * inv_eps;
+    if (phi) phi[l] = sc * P;
+    if (grad) for (int c = 0; c < 3; ++c) grad[3 * l + c] = sc * G[c];
+    if (hess) for (int c = 0; c < 6; ++c) hess[6 * l + c] = sc * H[c];
+}
+
+extern "C" int pb_multipole_field(pb_ctx* ctx, const double* mu, int use_mask, double* phi, double* grad, double* hess)
+{
+    if (!ctx) return PB_ERR_INVALID_ARG;
+    const pb_sites& s = ctx->sites;
+    if (!s.loaded) return pb_fail(ctx, PB_ERR_NOT_READY, "pb_multipole_field: call pb_sites_load first");
+    k_multipole_field<<<pb_blocks(s.na, 64), 64, 0, ctx->stream>>>(s.na, s.pos, s.q, s.dip, s.quad, mu, s.alpha, s.group,
+                                                                   ctx->prm.thole_a, 1.0 / ctx->prm.eps_in, use_mask, phi,
+                                                                   grad, hess);
+    PB_LAUNCH_CHECK();
+    return PB_OK;
+}

@@ -1,0 +1,456 @@
+// pb_solve.cu -- GMRES on Eq. (5) with device dot products / Arnoldi updates (H9), the
+// self-consistent induced-dipole loop with SOR (H13) and the energies of Eq. (19)/(24)
+// (H14).  Host code only steers: Givens rotations on the (m+1) x m Hessenberg matrix
+// and the convergence tests; every vector operation is a kernel.
+#include <math.h>
+#include <vector>
+#include "pb_internal.cuh"
+
+#define DOT_CHUNK 1024
+#define DOT_THREADS 256
+
+// partial[blk][j] = sum over the block's chunk of V_j . w   (one warp per j, fixed order)
+__global__ void __launch_bounds__(DOT_THREADS)
+k_dots(int64_t n, int nv, const double* __restrict__ V, int64_t ld, const double* __restrict__ w,
+       double* __restrict__ partial)
+{
+    __shared__ double sw[DOT_CHUNK];
+    const int64_t e0 = (int64_t)blockIdx.x * DOT_CHUNK;
+    const int cnt = (int)(n - e0 < DOT_CHUNK ? n - e0 : DOT_CHUNK);
+    for (int k = threadIdx.x; k < DOT_CHUNK; k += DOT_THREADS) sw[k] = k < cnt ? w[e0 + k] : 0.0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    for (int j = wid; j < nv; j += DOT_THREADS / 32) {
+        const double* v = V + (int64_t)j * ld + e0;
+        double s = 0;
+        for (int k = lane; k < cnt; k += 32) s = fma(v[k], sw[k], s);
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        if (lane == 0) partial[(int64_t)blockIdx.x * nv + j] = s;
+    }
+}
+
+// w -= sum_j h_j V_j with h_j = sum_blk partial[blk][j]; block 0 also publishes h (+= if accumulate)
+__global__ void __launch_bounds__(256)
+k_arnoldi_update(int64_t n, int nv, int nblk, const double* __restrict__ V, int64_t ld,
+                 const double* __restrict__ partial, double* __restrict__ w, double* __restrict__ hout)
+{
+    extern __shared__ double sh[];
+    for (int j = threadIdx.x; j < nv; j += blockDim.x) {
+        double s = 0;
+        for (int b = 0; b < nblk; ++b) s += partial[(int64_t)b * nv + j];
+        sh[j] = s;
+        if (blockIdx.x == 0) hout[j] = s;
+    }
+    __syncthreads();
+    const int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    double acc = w[e];
+    for (int j = 0; j < nv; ++j) acc = fma(-sh[j], V[(int64_t)j * ld + e], acc);
+    w[e] = acc;
+}
+
+// vnext = w / sqrt(sum partial); block 0 publishes the squared norm
+__global__ void __launch_bounds__(256)
+k_normalize(int64_t n, int nblk, const double* __restrict__ partial, const double* __restrict__ w,
+            double* __restrict__ vnext, double* __restrict__ nrm2_out)
+{
+    __shared__ double inv;
+    if (threadIdx.x == 0) {
+        double s = 0;
+        for (int b = 0; b < nblk; ++b) s += partial[b];
+        if (blockIdx.x == 0) *nrm2_out = s;
+        inv = s > 0 ? 1.0 / sqrt(s) : 0.0;
+    }
+    __syncthreads();
+    const int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (e < n) vnext[e] = w[e] * inv;
+}
+
+// z = Minv v: per panel the inverse 2x2 diagonal block (SELF entries), original panel order
+__global__ void k_precond(int64_t N, const double* __restrict__ pc, const double* __restrict__ v, double* __restrict__ z)
+{
+    int64_t o = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (o >= N) return;
+    double a = v[o], b = v[N + o];
+    z[o] = pc[o] * a + pc[N + o] * b;
+    z[N + o] = pc[2 * N + o] * a + pc[3 * N + o] * b;
+}
+
+// r = b - y
+__global__ void k_residual(int64_t n, const double* __restrict__ b, const double* __restrict__ y, double* __restrict__ r)
+{
+    int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (e < n) r[e] = b[e] - y[e];
+}
+
+// u = sum_j c_j V_j
+__global__ void __launch_bounds__(256)
+k_lincomb(int64_t n, int nv, const double* __restrict__ V, int64_t ld, const double* __restrict__ coef, double* __restrict__ u)
+{
+    extern __shared__ double sh[];
+    for (int j = threadIdx.x; j < nv; j += blockDim.x) sh[j] = coef[j];
+    __syncthreads();
+    const int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    double acc = 0;
+    for (int j = 0; j < nv; ++j) acc = fma(sh[j], V[(int64_t)j * ld + e], acc);
+    u[e] = acc;
+}
+
+__global__ void k_axpy(int64_t n, double a, const double* __restrict__ x, double* __restrict__ y)
+{
+    int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (e < n) y[e] = fma(a, x[e], y[e]);
+}
+
+typedef pb_gmres_ws gmres_ws;
+
+static int dot_into(pb_ctx* ctx, gmres_ws& ws, int nv, const double* V, const double* w)
+{
+    k_dots<<<ws.nblk, DOT_THREADS, 0, ctx->stream>>>(ws.n, nv, V, ws.n, w, ws.partial);
+    PB_LAUNCH_CHECK();
+    return PB_OK;
+}
+
+// ||v||^2 on the host (synchronises)
+static int norm2_host(pb_ctx* ctx, gmres_ws& ws, const double* v, double* out)
+{
+    PB_TRY(dot_into(ctx, ws, 1, v, v));
+    k_normalize<<<1, 32, 0, ctx->stream>>>(0, ws.nblk, ws.partial, nullptr, nullptr, ws.hdev);
+    PB_LAUNCH_CHECK();
+    PB_CUDA(cudaMemcpyAsync(out, ws.hdev, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    PB_CUDA(cudaStreamSynchronize(ctx->stream));
+    return PB_OK;
+}
+
+int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, double* relres_out, int32_t* matvecs_out)
+{
+    pb_tree& t = ctx->tree;
+    cudaStream_t st = ctx->stream;
+    if (!t.built) return pb_fail(ctx, PB_ERR_NOT_READY, "pb_gmres: call pb_tree_build first");
+    const int64_t n = 2 * t.N;
+    int m = ctx->prm.gmres_restart;
+    if (m > n) m = (int)n;
+    // workspace (kept until the system size or the restart length changes)
+    gmres_ws& ws = ctx->gws;
+    if (ws.n != n || ws.m != m || !ws.V) {
+        pb_dfree_cat(ctx, CAT_SOLVE);
+        ws = gmres_ws();
+        ws.nblk = (int)((n + DOT_CHUNK - 1) / DOT_CHUNK);
+        PB_TRY(pb_dalloc_t(ctx, &ws.V, (size_t)(m + 1) * n, CAT_SOLVE));
+        PB_TRY(pb_dalloc_t(ctx, &ws.w, n, CAT_SOLVE));
+        PB_TRY(pb_dalloc_t(ctx, &ws.z, n, CAT_SOLVE));
+        PB_TRY(pb_dalloc_t(ctx, &ws.r, n, CAT_SOLVE));
+        PB_TRY(pb_dalloc_t(ctx, &ws.u, n, CAT_SOLVE));
+        PB_TRY(pb_dalloc_t(ctx, &ws.partial, (size_t)ws.nblk * (m + 2), CAT_SOLVE));
+        PB_TRY(pb_dalloc_t(ctx, &ws.hdev, 2 * (m + 2) + 8, CAT_SOLVE));
+        PB_TRY(pb_dalloc_t(ctx, &ws.coef, m + 2, CAT_SOLVE));
+        ws.n = n;
+        ws.m = m;
+    }
+    PB_TRY(pb_pinned(ctx, (3 * (size_t)m + 64) * sizeof(double)));
+    double* hh = ctx->h_pinned;                    // staging for h columns
+    const bool pc = ctx->prm.precond != 0;
+    const double tol = ctx->prm.gmres_tol;
+    const int maxit = ctx->prm.gmres_maxit;
+    int iters = 0, matvecs = 0;
+    int rc = PB_OK;
+
+    double bn2 = 0;
+    PB_TRY(norm2_host(ctx, ws, b, &bn2));
+    const double bnorm = sqrt(bn2);
+    double relres = 0.0;
+    if (bnorm == 0.0) {
+        PB_CUDA(cudaMemsetAsync(x, 0, sizeof(double) * n, st));
+        if (iters_out) *iters_out = 0;
+        if (relres_out) *relres_out = 0.0;
+        if (matvecs_out) *matvecs_out = 0;
+        return PB_OK;
+    }
+    std::vector<double> H((size_t)(m + 1) * m, 0.0), cs(m, 0.0), sn(m, 0.0), g(m + 1, 0.0), yv(m, 0.0);
+    const int tb = 256;
+    const int nb = pb_blocks(n, tb);
+    for (;;) {
+        // true residual r = b - A x
+        PB_TRY(pb_matvec_impl(ctx, x, ws.w, false));
+        ++matvecs;
+        k_residual<<<nb, tb, 0, st>>>(n, b, ws.w, ws.r);
+        PB_LAUNCH_CHECK();
+        PB_TRY(dot_into(ctx, ws, 1, ws.r, ws.r));
+        k_normalize<<<nb, tb, 0, st>>>(n, ws.nblk, ws.partial, ws.r, ws.V, ws.hdev);   // V_0 = r/||r||
+        PB_LAUNCH_CHECK();
+        double r2 = 0;
+        PB_CUDA(cudaMemcpyAsync(&r2, ws.hdev, sizeof(double), cudaMemcpyDeviceToHost, st));
+        PB_CUDA(cudaStreamSynchronize(st));
+        const double beta = sqrt(r2);
+        relres = beta / bnorm;
+        if (relres <= tol) break;
+        if (iters >= maxit) { rc = PB_ERR_NO_CONVERGENCE; break; }
+        std::fill(g.begin(), g.end(), 0.0);
+        g[0] = beta;
+        int j = 0;
+        for (; j < m && iters < maxit;) {
+            const double* vj = ws.V + (size_t)j * n;
+            const double* zin = vj;
+            if (pc) {
+                k_precond<<<pb_blocks(t.N, tb), tb, 0, st>>>(t.N, t.precond, vj, ws.z);
+                PB_LAUNCH_CHECK();
+                zin = ws.z;
+            }
+            PB_TRY(pb_matvec_impl(ctx, zin, ws.w, false));
+            ++matvecs;
+            const int nv = j + 1;
+            // classical Gram-Schmidt, twice
+            double* hA = ws.hdev;
+            double* hB = ws.hdev + (m + 2);
+            PB_TRY(dot_into(ctx, ws, nv, ws.V, ws.w));
+            k_arnoldi_update<<<nb, tb, nv * sizeof(double), st>>>(n, nv, ws.nblk, ws.V, n, ws.partial, ws.w, hA);
+            PB_LAUNCH_CHECK();
+            PB_TRY(dot_into(ctx, ws, nv, ws.V, ws.w));
+            k_arnoldi_update<<<nb, tb, nv * sizeof(double), st>>>(n, nv, ws.nblk, ws.V, n, ws.partial, ws.w, hB);
+            PB_LAUNCH_CHECK();
+            PB_TRY(dot_into(ctx, ws, 1, ws.w, ws.w));
+            k_normalize<<<nb, tb, 0, st>>>(n, ws.nblk, ws.partial, ws.w, ws.V + (size_t)(j + 1) * n, ws.hdev + 2 * (m + 2));
+            PB_LAUNCH_CHECK();
+            PB_CUDA(cudaMemcpyAsync(hh, ws.hdev, sizeof(double) * (2 * (m + 2) + 1), cudaMemcpyDeviceToHost, st));
+            PB_CUDA(cudaStreamSynchronize(st));
+            double* col = &H[(size_t)j * (m + 1)];
+            for (int i = 0; i < nv; ++i) col[i] = hh[i] + hh[(m + 2) + i];
+            const double hnext = sqrt(hh[2 * (m + 2)]);
+            col[nv] = hnext;
+            // Givens rotations (host, O(j))
+            for (int i = 0; i < j; ++i) {
+                double a = cs[i] * col[i] + sn[i] * col[i + 1];
+                col[i + 1] = -sn[i] * col[i] + cs[i] * col[i + 1];
+                col[i] = a;
+            }
+            double den = hypot(col[j], col[j + 1]);
+            if (den == 0.0) { ++j; ++iters; break; }
+            cs[j] = col[j] / den;
+            sn[j] = col[j + 1] / den;
+            col[j] = den;
+            col[j + 1] = 0.0;
+            g[j + 1] = -sn[j] * g[j];
+            g[j] = cs[j] * g[j];
+            ++j;
+            ++iters;
+            relres = fabs(g[j]) / bnorm;
+            if (relres <= tol || hnext <= 1e-300) break;
+        }
+        // y = R^{-1} g ; x += Minv (V y)
+        for (int i = j - 1; i >= 0; --i) {
+            double s = g[i];
+            for (int k = i + 1; k < j; ++k) s -= H[(size_t)k * (m + 1) + i] * yv[k];
+            yv[i] = s / H[(size_t)i * (m + 1) + i];
+        }
+        for (int i = 0; i < j; ++i) hh[i] = yv[i];
+        PB_CUDA(cudaMemcpyAsync(ws.coef, hh, sizeof(double) * j, cudaMemcpyHostToDevice, st));
+        k_lincomb<<<nb, tb, j * sizeof(double), st>>>(n, j, ws.V, n, ws.coef, ws.u);
+        PB_LAUNCH_CHECK();
+        if (pc) {
+            k_precond<<<pb_blocks(t.N, tb), tb, 0, st>>>(t.N, t.precond, ws.u, ws.z);
+            PB_LAUNCH_CHECK();
+            k_axpy<<<nb, tb, 0, st>>>(n, 1.0, ws.z, x);
+        } else
+            k_axpy<<<nb, tb, 0, st>>>(n, 1.0, ws.u, x);
+        PB_LAUNCH_CHECK();
+        PB_CUDA(cudaStreamSynchronize(st));   // hh is reused
+    }
+    if (iters_out) *iters_out = iters;
+    if (relres_out) *relres_out = relres;
+    if (matvecs_out) *matvecs_out = matvecs;
+    if (rc != PB_OK) return pb_fail(ctx, rc, "GMRES: %d iterations, relative residual %.3e > %.3e", iters, relres, tol);
+    return PB_OK;
+}
+
+extern "C" int pb_gmres(pb_ctx* ctx, const double* b, double* x, int32_t* iters, double* relres)
+{
+    if (!ctx) return PB_ERR_INVALID_ARG;
+    if (!b || !x) return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_gmres: NULL vector");
+    return pb_gmres_impl(ctx, b, x, iters, relres, nullptr);
+}
+
+// ---- SCF and energy kernels ------------------------------------------------------------------------
+// mu_new = (1-w) mu + w alpha 4 pi E,  E = -(grad_solv + grad_mult)   (Eq. 9, 15; SOR P:160; D: R-2)
+// out[0] = sum_m |mu_new - mu|^2
+__global__ void __launch_bounds__(256)
+k_scf_update(int64_t na, const double* __restrict__ alpha, const double* __restrict__ gsolv,
+             const double* __restrict__ gmult, double omega, double* __restrict__ mu, double* __restrict__ out)
+{
+    __shared__ double red[8];
+    double s = 0;
+    for (int64_t e = threadIdx.x; e < 3 * na; e += blockDim.x) {
+        double E = -(gsolv ? gsolv[e] : 0.0) - gmult[e];
+        double old = mu[e];
+        double nw = (1.0 - omega) * old + omega * alpha[e / 3] * (4.0 * 3.14159265358979323846) * E;
+        mu[e] = nw;
+        s += (nw - old) * (nw - old);
+    }
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double v = 0;
+        for (int k = 0; k < 8; ++k) v += red[k];
+        out[0] = v;
+    }
+}
+
+// G = 1/2 sum_m [ q phi + d.grad phi + (1/6) Q : hess phi ]  with the PERMANENT dipole (Eq. 24)
+__global__ void __launch_bounds__(256)
+k_energy(int64_t na, const double* __restrict__ q, const double* __restrict__ dip, const double* __restrict__ quad,
+         const double* __restrict__ phi, const double* __restrict__ grad, const double* __restrict__ hess,
+         double* __restrict__ out)
+{
+    __shared__ double red[8];
+    double s = 0;
+    for (int64_t m = threadIdx.x; m < na; m += blockDim.x) {
+        const double* Q = quad + 6 * m;
+        const double* Hm = hess + 6 * m;
+        double QH = Q[0] * Hm[0] + Q[3] * Hm[3] + Q[5] * Hm[5] + 2.0 * (Q[1] * Hm[1] + Q[2] * Hm[2] + Q[4] * Hm[4]);
+        s += q[m] * phi[m] + dip[3 * m] * grad[3 * m] + dip[3 * m + 1] * grad[3 * m + 1] + dip[3 * m + 2] * grad[3 * m + 2] +
+             QH / 6.0;
+    }
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double v = 0;
+        for (int k = 0; k < 8; ++k) v += red[k];
+        out[0] = 0.5 * v;
+    }
+}
+
+__global__ void k_any_nonzero(int64_t n, const double* __restrict__ a, int* __restrict__ flag)
+{
+    int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (e < n && a[e] != 0.0) *flag = 1;
+}
+
+static int pb_solve_core(pb_ctx* ctx, double* x_out, double* mu_out, pb_result* res, bool host_out)
+{
+    pb_tree& t = ctx->tree;
+    pb_sites& s = ctx->sites;
+    cudaStream_t st = ctx->stream;
+    if (!t.built || !s.loaded) return pb_fail(ctx, PB_ERR_NOT_READY, "pb_solve: needs pb_mesh_load, pb_sites_load, pb_tree_build");
+    if (!res) return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_solve: NULL result");
+    memset(res, 0, sizeof(*res));
+    const int64_t n = 2 * t.N, na = s.na;
+    // solve-scoped buffers from the scratch category (GMRES re-allocates CAT_SOLVE, so use CAT_TMP here)
+    pb_dfree_cat(ctx, CAT_TMP);
+    double *b, *x, *mu, *muv, *gs, *gm, *phi, *hess, *dscal;
+    PB_TRY(pb_dalloc_t(ctx, &b, n, CAT_TMP));
+    PB_TRY(pb_dalloc_t(ctx, &x, n, CAT_TMP));
+    PB_TRY(pb_dalloc_t(ctx, &mu, 3 * na, CAT_TMP));
+    PB_TRY(pb_dalloc_t(ctx, &muv, 3 * na, CAT_TMP));
+    PB_TRY(pb_dalloc_t(ctx, &gs, 3 * na, CAT_TMP));
+    PB_TRY(pb_dalloc_t(ctx, &gm, 3 * na, CAT_TMP));
+    PB_TRY(pb_dalloc_t(ctx, &phi, na, CAT_TMP));
+    PB_TRY(pb_dalloc_t(ctx, &hess, 6 * na, CAT_TMP));
+    PB_TRY(pb_dalloc_t(ctx, &dscal, 8, CAT_TMP));
+    PB_CUDA(cudaMemsetAsync(x, 0, sizeof(double) * n, st));
+    PB_CUDA(cudaMemsetAsync(mu, 0, sizeof(double) * 3 * na, st));
+    PB_CUDA(cudaMemsetAsync(muv, 0, sizeof(double) * 3 * na, st));
+    PB_CUDA(cudaMemsetAsync(dscal, 0, sizeof(double) * 8, st));
+    int hflag = 0;
+    k_any_nonzero<<<pb_blocks(na, 256), 256, 0, st>>>(na, s.alpha, (int*)dscal);
+    PB_LAUNCH_CHECK();
+    PB_CUDA(cudaMemcpyAsync(&hflag, dscal, sizeof(int), cudaMemcpyDeviceToHost, st));
+    PB_CUDA(cudaStreamSynchronize(st));
+    const bool polarizable = hflag != 0;
+    const double tol = ctx->prm.scf_tol_debye, omega = ctx->prm.scf_omega;
+    int status = PB_OK;
+    double h[2];
+
+    // --- vacuum SCF: mu^v from the multipole field alone
+    int it_v = 0;
+    if (polarizable) {
+        bool conv = false;
+        for (it_v = 1; it_v <= ctx->prm.scf_maxit; ++it_v) {
+            PB_TRY(pb_multipole_field(ctx, muv, 1, nullptr, gm, nullptr));
+            k_scf_update<<<1, 256, 0, st>>>(na, s.alpha, nullptr, gm, omega, muv, dscal);
+            PB_LAUNCH_CHECK();
+            PB_CUDA(cudaMemcpyAsync(h, dscal, sizeof(double), cudaMemcpyDeviceToHost, st));
+            PB_CUDA(cudaStreamSynchronize(st));
+            if (sqrt(h[0] / (double)na) * PB_DEBYE < tol) { conv = true; break; }
+        }
+        if (!conv) { status = PB_ERR_NO_CONVERGENCE; it_v = ctx->prm.scf_maxit; }
+    }
+    res->scf_iters_vac = it_v;
+
+    // --- solvent SCF (steps 1-6)
+    int it = 0, gm_total = 0, mv_total = 0;
+    double delta = 0, relres = 0;
+    bool conv = false;
+    for (it = 1; it <= ctx->prm.scf_maxit; ++it) {
+        int32_t gi = 0, mv = 0;
+        PB_TRY(pb_rhs_multipole(ctx, mu, b));                        // step 2: Eq. (5) with p = d + mu
+        int rc = pb_gmres_impl(ctx, b, x, &gi, &relres, &mv);
+        if (rc == PB_ERR_NO_CONVERGENCE) status = rc; else if (rc != PB_OK) return rc;
+        gm_total += gi;
+        mv_total += mv;
+        if (!polarizable) { conv = true; break; }
+        PB_TRY(pb_reaction_field(ctx, x, nullptr, gs, nullptr));      // step 3: Eq. (13)
+        PB_TRY(pb_multipole_field(ctx, mu, 1, nullptr, gm, nullptr)); // step 3: Eq. (14)
+        k_scf_update<<<1, 256, 0, st>>>(na, s.alpha, gs, gm, omega, mu, dscal);   // steps 4-5 + SOR
+        PB_LAUNCH_CHECK();
+        PB_CUDA(cudaMemcpyAsync(h, dscal, sizeof(double), cudaMemcpyDeviceToHost, st));
+        PB_CUDA(cudaStreamSynchronize(st));
+        delta = sqrt(h[0] / (double)na) * PB_DEBYE;
+        if (delta < tol) {                                            // step 6
+            // surface solution consistent with the final mu
+            PB_TRY(pb_rhs_multipole(ctx, mu, b));
+            rc = pb_gmres_impl(ctx, b, x, &gi, &relres, &mv);
+            if (rc == PB_ERR_NO_CONVERGENCE) status = rc; else if (rc != PB_OK) return rc;
+            gm_total += gi;
+            mv_total += mv;
+            conv = true;
+            break;
+        }
+    }
+    if (!conv) { status = PB_ERR_NO_CONVERGENCE; it = ctx->prm.scf_maxit; }
+    res->scf_iters = it;
+    res->gmres_iters_total = gm_total;
+    res->matvecs_total = mv_total;
+    res->final_scf_delta_debye = delta;
+    res->final_gmres_relres = relres;
+
+    // --- energies: Delta G = G[phi_solv] + G[phi_mult(mu)] - G[phi_vac(mu^v)]   (Eq. 19, 24)
+    PB_TRY(pb_reaction_field(ctx, x, phi, gs, hess));
+    k_energy<<<1, 256, 0, st>>>(na, s.q, s.dip, s.quad, phi, gs, hess, dscal + 1);
+    PB_LAUNCH_CHECK();
+    PB_TRY(pb_multipole_field(ctx, mu, 0, phi, gm, hess));
+    k_energy<<<1, 256, 0, st>>>(na, s.q, s.dip, s.quad, phi, gm, hess, dscal + 2);
+    PB_LAUNCH_CHECK();
+    PB_TRY(pb_multipole_field(ctx, muv, 0, phi, gm, hess));
+    k_energy<<<1, 256, 0, st>>>(na, s.q, s.dip, s.quad, phi, gm, hess, dscal + 3);
+    PB_LAUNCH_CHECK();
+    double G[3];
+    PB_CUDA(cudaMemcpyAsync(G, dscal + 1, 3 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (x_out)
+        PB_CUDA(cudaMemcpyAsync(x_out, x, sizeof(double) * n, host_out ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, st));
+    if (mu_out)
+        PB_CUDA(cudaMemcpyAsync(mu_out, mu, sizeof(double) * 3 * na, host_out ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, st));
+    PB_CUDA(cudaStreamSynchronize(st));
+    const double c = 4.0 * 3.14159265358979323846 * PB_KCAL;
+    res->G_solvterm = c * G[0];
+    res->G_mult_diss = c * G[1];
+    res->G_vac = c * G[2];
+    res->dG_solv = c * (G[0] + G[1] - G[2]);
+    res->status = status;
+    pb_dfree_cat(ctx, CAT_TMP);
+    if (status != PB_OK) return pb_fail(ctx, status, "pb_solve: iteration limit reached (scf %d, gmres relres %.3e)", it, relres);
+    return PB_OK;
+}
+
+extern "C" int pb_solve(pb_ctx* ctx, double* x_out, double* mu_out, pb_result* result)
+{
+    if (!ctx) return PB_ERR_INVALID_ARG;
+    return pb_solve_core(ctx, x_out, mu_out, result, false);
+}
+
+extern "C" int pb_solve_host(pb_ctx* ctx, double* x_host, double* mu_host, pb_result* result)
+{
+    if (!ctx) return PB_ERR_INVALID_ARG;
+    return pb_solve_core(ctx, x_host, mu_host, result, true);
+}

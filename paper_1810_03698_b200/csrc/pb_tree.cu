@@ -1,0 +1,584 @@
+// pb_tree.cu -- device-built Morton octree over whole panels, target groups and the
+// M2P / P2P interaction lists by the MAC of Eq. (28) (D: sections 5-6).
+#include <math.h>
+#include "pb_internal.cuh"
+
+// ---- bounding cube of the centroids ---------------------------------------------------------
+__global__ void k_bbox(int64_t n, const double* __restrict__ cen, double* __restrict__ out /*[6]*/)
+{
+    __shared__ double s[6][32];
+    double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+    for (int64_t i = threadIdx.x; i < n; i += blockDim.x)
+        for (int d = 0; d < 3; ++d) {
+            double v = cen[3 * i + d];
+            lo[d] = fmin(lo[d], v);
+            hi[d] = fmax(hi[d], v);
+        }
+    for (int o = 16; o > 0; o >>= 1)
+        for (int d = 0; d < 3; ++d) {
+            lo[d] = fmin(lo[d], __shfl_xor_sync(0xffffffffu, lo[d], o));
+            hi[d] = fmax(hi[d], __shfl_xor_sync(0xffffffffu, hi[d], o));
+        }
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0)
+        for (int d = 0; d < 3; ++d) { s[d][w] = lo[d]; s[3 + d][w] = hi[d]; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int nw = blockDim.x >> 5;
+        for (int d = 0; d < 3; ++d) {
+            double a = s[d][0], b = s[3 + d][0];
+            for (int k = 1; k < nw; ++k) { a = fmin(a, s[d][k]); b = fmax(b, s[3 + d][k]); }
+            out[d] = a;
+            out[3 + d] = b;
+        }
+    }
+}
+
+__device__ __forceinline__ uint64_t spread21(uint64_t v)
+{
+    v &= 0x1fffffULL;
+    v = (v | (v << 32)) & 0x1f00000000ffffULL;
+    v = (v | (v << 16)) & 0x1f0000ff0000ffULL;
+    v = (v | (v << 8)) & 0x100f00f00f00f00fULL;
+    v = (v | (v << 4)) & 0x10c30c30c30c30c3ULL;
+    v = (v | (v << 2)) & 0x1249249249249249ULL;
+    return v;
+}
+
+// 63-bit Morton key of each centroid, 21 bits per axis inside the bounding cube.
+__global__ void k_morton(int64_t n, const double* __restrict__ cen, const double* __restrict__ box,
+                         uint64_t* __restrict__ keys, int32_t* __restrict__ vals)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double side = fmax(fmax(box[3] - box[0], box[4] - box[1]), box[5] - box[2]);
+    side = side > 0 ? side * (1.0 + 1e-9) : 1.0;
+    uint64_t q[3];
+    for (int d = 0; d < 3; ++d) {
+        double t = (cen[3 * i + d] - box[d]) / side * 2097152.0;
+        long long u = (long long)t;
+        u = u < 0 ? 0 : (u > 2097151 ? 2097151 : u);
+        q[d] = (uint64_t)u;
+    }
+    keys[i] = (spread21(q[0]) << 2) | (spread21(q[1]) << 1) | spread21(q[2]);
+    vals[i] = (int32_t)i;
+}
+
+// ---- LSD radix sort, 8-bit digits, stable; one warp owns a contiguous sub-tile -------------
+#define RS_WARPS 8
+#define RS_ITEMS 16
+#define RS_TILE (32 * RS_ITEMS)
+
+__global__ void k_rs_hist(const uint64_t* __restrict__ keys, int64_t n, int shift, int64_t nwt,
+                          int32_t* __restrict__ hist /*[256][nwt]*/)
+{
+    __shared__ int32_t cnt[RS_WARPS][256];
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int64_t wt = blockIdx.x * (int64_t)RS_WARPS + w;
+    for (int d = lane; d < 256; d += 32) cnt[w][d] = 0;
+    __syncwarp();
+    if (wt < nwt) {
+        for (int c = 0; c < RS_ITEMS; ++c) {
+            int64_t i = wt * RS_TILE + c * 32 + lane;
+            if (i < n) atomicAdd(&cnt[w][(int)((keys[i] >> shift) & 255)], 1);
+        }
+        __syncwarp();
+        for (int d = lane; d < 256; d += 32) hist[(int64_t)d * nwt + wt] = cnt[w][d];
+    }
+}
+
+__global__ void k_rs_scatter(const uint64_t* __restrict__ kin, const int32_t* __restrict__ vin,
+                             uint64_t* __restrict__ kout, int32_t* __restrict__ vout, int64_t n, int shift,
+                             int64_t nwt, const int32_t* __restrict__ hist)
+{
+    __shared__ int32_t off[RS_WARPS][256];
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int64_t wt = blockIdx.x * (int64_t)RS_WARPS + w;
+    if (wt >= nwt) return;
+    for (int d = lane; d < 256; d += 32) off[w][d] = hist[(int64_t)d * nwt + wt];
+    __syncwarp();
+    for (int c = 0; c < RS_ITEMS; ++c) {
+        int64_t i = wt * RS_TILE + c * 32 + lane;
+        bool valid = i < n;
+        uint64_t key = valid ? kin[i] : 0;
+        int dg = valid ? (int)((key >> shift) & 255) : (256 + lane);
+        unsigned peers = __match_any_sync(0xffffffffu, dg);
+        int rank = __popc(peers & ((1u << lane) - 1u));
+        int pos = valid ? off[w][dg] + rank : 0;
+        __syncwarp();
+        if (valid && rank == 0) off[w][dg] += __popc(peers);
+        __syncwarp();
+        if (valid) { kout[pos] = key; vout[pos] = vin[i]; }
+    }
+}
+
+// ---- panels and Gauss points in Morton order -----------------------------------------------
+struct geo_ptrs {
+    double *pc[3], *pn[3], *parea, *pv[9];
+    int32_t* ptri[3];
+    double *sx[3], *swA;
+};
+
+__global__ void k_gather(int64_t N, const int32_t* __restrict__ perm, const double* __restrict__ verts,
+                         const int32_t* __restrict__ tris, pb_rule_t rule, geo_ptrs g)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int64_t o = perm[i];
+    double v[9];
+    for (int b = 0; b < 3; ++b) {
+        int32_t vi = tris[3 * o + b];
+        g.ptri[b][i] = vi;
+        for (int d = 0; d < 3; ++d) v[3 * b + d] = verts[3 * (int64_t)vi + d];
+    }
+    double e1[3], e2[3], c[3];
+    for (int d = 0; d < 3; ++d) {
+        e1[d] = v[3 + d] - v[d];
+        e2[d] = v[6 + d] - v[d];
+        g.pc[d][i] = (v[d] + v[3 + d] + v[6 + d]) / 3.0;
+    }
+    c[0] = e1[1] * e2[2] - e1[2] * e2[1];
+    c[1] = e1[2] * e2[0] - e1[0] * e2[2];
+    c[2] = e1[0] * e2[1] - e1[1] * e2[0];
+    double l = sqrt(c[0] * c[0] + c[1] * c[1] + c[2] * c[2]);
+    double area = 0.5 * l;
+    g.parea[i] = area;
+    for (int d = 0; d < 3; ++d) g.pn[d][i] = c[d] / l;
+    for (int k = 0; k < 9; ++k) g.pv[k][i] = v[k];
+    for (int q = 0; q < rule.K; ++q) {
+        int64_t s = i * rule.K + q;
+        for (int d = 0; d < 3; ++d)
+            g.sx[d][s] = rule.lam[q][0] * v[d] + rule.lam[q][1] * v[3 + d] + rule.lam[q][2] * v[6 + d];
+        g.swA[s] = rule.w[q] * area;
+    }
+}
+
+// ---- octree topology, one BFS generation at a time -----------------------------------------
+// A cell is a range of Morton-sorted panels.  It is split at the highest 3-bit digit in
+// which its first and last keys differ, so every internal cell has >= 2 children.
+__global__ void k_cell_split(int64_t c0, int64_t c1, const uint64_t* __restrict__ keys,
+                             const int32_t* __restrict__ c_first, const int32_t* __restrict__ c_last, int K,
+                             int ncrit, int32_t* __restrict__ nchild, int32_t* __restrict__ bounds /*[c1-c0][9]*/)
+{
+    int64_t c = c0 + blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (c >= c1) return;
+    int32_t f = c_first[c], l = c_last[c];
+    int32_t* b = bounds + 9 * (c - c0);
+    int nc = 0;
+    if ((int64_t)(l - f) * K > ncrit && l - f > 1 && keys[f] != keys[l - 1]) {
+        uint64_t x = keys[f] ^ keys[l - 1];
+        int hb = 63 - __clzll((long long)x);
+        int shift = 3 * (hb / 3);
+        b[0] = f;
+        b[8] = l;
+        for (int v = 1; v < 8; ++v) {
+            int32_t lo = f, hi = l;   // first index whose digit >= v
+            while (lo < hi) {
+                int32_t mid = lo + ((hi - lo) >> 1);
+                if ((int)((keys[mid] >> shift) & 7) >= v) hi = mid; else lo = mid + 1;
+            }
+            b[v] = lo;
+        }
+        for (int v = 0; v < 8; ++v) nc += (b[v + 1] > b[v]);
+    }
+    nchild[c - c0] = nc;
+}
+
+__global__ void k_cell_emit(int64_t c0, int64_t c1, const int32_t* __restrict__ nchild,
+                            const int32_t* __restrict__ choff, const int32_t* __restrict__ bounds, int64_t base,
+                            int32_t* __restrict__ c_first, int32_t* __restrict__ c_last,
+                            int32_t* __restrict__ c_child, int32_t* __restrict__ c_nchild)
+{
+    int64_t c = c0 + blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (c >= c1) return;
+    int nc = nchild[c - c0];
+    c_nchild[c] = nc;
+    if (nc == 0) { c_child[c] = -1; return; }
+    int64_t first = base + choff[c - c0];
+    c_child[c] = (int32_t)first;
+    const int32_t* b = bounds + 9 * (c - c0);
+    int k = 0;
+    for (int v = 0; v < 8; ++v)
+        if (b[v + 1] > b[v]) {
+            c_first[first + k] = b[v];
+            c_last[first + k] = b[v + 1];
+            ++k;
+        }
+}
+
+__global__ void k_mark_leaves(int64_t nc, const int32_t* __restrict__ c_child, int32_t* __restrict__ flag)
+{
+    int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (c < nc) flag[c] = c_child[c] < 0 ? 1 : 0;
+}
+
+__global__ void k_compact_leaves(int64_t nc, const int32_t* __restrict__ c_child, const int32_t* __restrict__ off,
+                                 int32_t* __restrict__ leaf_ids)
+{
+    int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (c < nc && c_child[c] < 0) leaf_ids[off[c]] = (int32_t)c;
+}
+
+// ---- cell geometry: tight box, expansion centre = box centre, bounding radius (D: R-13) -----
+// leaves: one warp per leaf, exact box and radius over its Gauss points
+__global__ void k_leaf_geom(int64_t nl, const int32_t* __restrict__ leaf_ids, const int32_t* __restrict__ c_first,
+                            const int32_t* __restrict__ c_last, int K, const double* __restrict__ sx,
+                            const double* __restrict__ sy, const double* __restrict__ sz, double* __restrict__ cx,
+                            double* __restrict__ cy, double* __restrict__ cz, double* __restrict__ crad,
+                            double* __restrict__ cbox)
+{
+    int64_t w = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    int lane = threadIdx.x & 31;
+    if (w >= nl) return;
+    int32_t c = leaf_ids[w];
+    int64_t s0 = (int64_t)c_first[c] * K, s1 = (int64_t)c_last[c] * K;
+    double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+    for (int64_t s = s0 + lane; s < s1; s += 32) {
+        double p[3] = {sx[s], sy[s], sz[s]};
+        for (int d = 0; d < 3; ++d) { lo[d] = fmin(lo[d], p[d]); hi[d] = fmax(hi[d], p[d]); }
+    }
+    for (int o = 16; o > 0; o >>= 1)
+        for (int d = 0; d < 3; ++d) {
+            lo[d] = fmin(lo[d], __shfl_xor_sync(0xffffffffu, lo[d], o));
+            hi[d] = fmax(hi[d], __shfl_xor_sync(0xffffffffu, hi[d], o));
+        }
+    double ctr[3] = {0.5 * (lo[0] + hi[0]), 0.5 * (lo[1] + hi[1]), 0.5 * (lo[2] + hi[2])};
+    double r2 = 0;
+    for (int64_t s = s0 + lane; s < s1; s += 32) {
+        double dx = sx[s] - ctr[0], dy = sy[s] - ctr[1], dz = sz[s] - ctr[2];
+        r2 = fmax(r2, dx * dx + dy * dy + dz * dz);
+    }
+    for (int o = 16; o > 0; o >>= 1) r2 = fmax(r2, __shfl_xor_sync(0xffffffffu, r2, o));
+    if (lane == 0) {
+        cx[c] = ctr[0]; cy[c] = ctr[1]; cz[c] = ctr[2];
+        crad[c] = sqrt(r2) * (1.0 + 1e-14);
+        for (int d = 0; d < 3; ++d) { cbox[6 * (int64_t)c + d] = lo[d]; cbox[6 * (int64_t)c + 3 + d] = hi[d]; }
+    }
+}
+
+// internal cells of one generation (children are already done): box = union of the
+// children's boxes; radius = min(half diagonal, max over children of |c_child - c| + r_child)
+__global__ void k_inner_geom(int64_t c0, int64_t c1, const int32_t* __restrict__ c_child,
+                             const int32_t* __restrict__ c_nchild, double* __restrict__ cx, double* __restrict__ cy,
+                             double* __restrict__ cz, double* __restrict__ crad, double* __restrict__ cbox)
+{
+    int64_t c = c0 + blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (c >= c1) return;
+    int32_t ch = c_child[c];
+    if (ch < 0) return;
+    int nc = c_nchild[c];
+    double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+    for (int k = 0; k < nc; ++k)
+        for (int d = 0; d < 3; ++d) {
+            lo[d] = fmin(lo[d], cbox[6 * (int64_t)(ch + k) + d]);
+            hi[d] = fmax(hi[d], cbox[6 * (int64_t)(ch + k) + 3 + d]);
+        }
+    double ctr[3] = {0.5 * (lo[0] + hi[0]), 0.5 * (lo[1] + hi[1]), 0.5 * (lo[2] + hi[2])};
+    double hd = 0.5 * sqrt((hi[0] - lo[0]) * (hi[0] - lo[0]) + (hi[1] - lo[1]) * (hi[1] - lo[1]) +
+                           (hi[2] - lo[2]) * (hi[2] - lo[2]));
+    double rr = 0;
+    for (int k = 0; k < nc; ++k) {
+        double dx = cx[ch + k] - ctr[0], dy = cy[ch + k] - ctr[1], dz = cz[ch + k] - ctr[2];
+        rr = fmax(rr, sqrt(dx * dx + dy * dy + dz * dz) + crad[ch + k]);
+    }
+    cx[c] = ctr[0]; cy[c] = ctr[1]; cz[c] = ctr[2];
+    crad[c] = fmin(hd, rr) * (1.0 + 1e-14);
+    for (int d = 0; d < 3; ++d) { cbox[6 * c + d] = lo[d]; cbox[6 * c + 3 + d] = hi[d]; }
+}
+
+// ---- target groups: PB_TG consecutive Morton-ordered collocation points ----------------------
+__global__ void k_group_geom(int64_t ng, int64_t N, const double* __restrict__ px, const double* __restrict__ py,
+                             const double* __restrict__ pz, double* __restrict__ gx, double* __restrict__ gy,
+                             double* __restrict__ gz, double* __restrict__ grad)
+{
+    int64_t w = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    int lane = threadIdx.x & 31;
+    if (w >= ng) return;
+    int64_t i0 = w * PB_TG, i1 = i0 + PB_TG < N ? i0 + PB_TG : N;
+    double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+    for (int64_t i = i0 + lane; i < i1; i += 32) {
+        double p[3] = {px[i], py[i], pz[i]};
+        for (int d = 0; d < 3; ++d) { lo[d] = fmin(lo[d], p[d]); hi[d] = fmax(hi[d], p[d]); }
+    }
+    for (int o = 16; o > 0; o >>= 1)
+        for (int d = 0; d < 3; ++d) {
+            lo[d] = fmin(lo[d], __shfl_xor_sync(0xffffffffu, lo[d], o));
+            hi[d] = fmax(hi[d], __shfl_xor_sync(0xffffffffu, hi[d], o));
+        }
+    double ctr[3] = {0.5 * (lo[0] + hi[0]), 0.5 * (lo[1] + hi[1]), 0.5 * (lo[2] + hi[2])};
+    double r2 = 0;
+    for (int64_t i = i0 + lane; i < i1; i += 32) {
+        double dx = px[i] - ctr[0], dy = py[i] - ctr[1], dz = pz[i] - ctr[2];
+        r2 = fmax(r2, dx * dx + dy * dy + dz * dz);
+    }
+    for (int o = 16; o > 0; o >>= 1) r2 = fmax(r2, __shfl_xor_sync(0xffffffffu, r2, o));
+    if (lane == 0) { gx[w] = ctr[0]; gy[w] = ctr[1]; gz[w] = ctr[2]; grad[w] = sqrt(r2) * (1.0 + 1e-14); }
+}
+
+// ---- interaction lists: top-down traversal per target group (Eq. 28) ------------
+// A cell is accepted (M2P) for the whole group when R_b / R_tb < theta with R_b the cell's
+// bounding radius and R_tb = |centre_cell - centre_group| - r_group, the smallest possible
+// box-target distance over the group; otherwise its children are visited, and leaves go to
+// the P2P list as source-point ranges (adjacent ranges merged).  Cells with fewer than
+// `m2p_min` source points are never accepted: summing them directly is cheaper and exact.
+struct list_args {
+    int64_t ng, N, Ns;
+    int K;
+    double theta;
+    int m2p_min;
+    const int32_t *c_first, *c_last, *c_child, *c_nchild;
+    const double *cx, *cy, *cz, *crad;
+    const double *gx, *gy, *gz, *grad;
+    int32_t *n_m2p, *n_p2p;           // pass 0: counts ; pass 1: offsets (read)
+    int32_t *m2p_cell, *p2p_lo, *p2p_hi;
+    unsigned long long* pair_counts;  // [2] p2p, m2p pairs (pass 0)
+};
+
+template <int PASS>
+__global__ void k_lists(list_args a)
+{
+    int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (g >= a.ng) return;
+    int64_t ntg = (g + 1) * PB_TG <= a.N ? PB_TG : a.N - g * PB_TG;
+    int nm = 0, nr = 0;
+    int64_t om = PASS ? a.n_m2p[g] : 0, op = PASS ? a.n_p2p[g] : 0;
+    unsigned long long pp = 0;
+    if (a.theta <= 0.0) {   // direct mode: one range, every source point
+        if (PASS) { a.p2p_lo[op] = 0; a.p2p_hi[op] = (int32_t)a.Ns; }
+        nr = 1;
+        pp = (unsigned long long)a.Ns;
+    } else {
+        int32_t stack[192];
+        int sp = 0;
+        stack[sp++] = 0;
+        double tx = a.gx[g], ty = a.gy[g], tz = a.gz[g], tr = a.grad[g];
+        int32_t last_hi = -1;
+        while (sp > 0) {
+            int32_t c = stack[--sp];
+            double dx = a.cx[c] - tx, dy = a.cy[c] - ty, dz = a.cz[c] - tz;
+            double sep = sqrt(dx * dx + dy * dy + dz * dz) - tr;
+            int32_t f = a.c_first[c], l = a.c_last[c];
+            int32_t ch = a.c_child[c];
+            int64_t nsrc = (int64_t)(l - f) * a.K;
+            if (sep > 0.0 && a.crad[c] < a.theta * sep && nsrc >= a.m2p_min) {
+                if (PASS) a.m2p_cell[om + nm] = c;
+                ++nm;
+            } else if (ch < 0) {
+                int32_t lo = f * a.K, hi = l * a.K;
+                if (lo == last_hi) {
+                    if (PASS) a.p2p_hi[op + nr - 1] = hi;
+                } else {
+                    if (PASS) { a.p2p_lo[op + nr] = lo; a.p2p_hi[op + nr] = hi; }
+                    ++nr;
+                }
+                last_hi = hi;
+                pp += (unsigned long long)(hi - lo);
+            } else {
+                int nc = a.c_nchild[c];
+                for (int k = nc - 1; k >= 0; --k) stack[sp++] = ch + k;   // popped in Morton order
+            }
+        }
+    }
+    if (!PASS) {
+        a.n_m2p[g] = nm;
+        a.n_p2p[g] = nr;
+        atomicAdd(&a.pair_counts[0], pp * (unsigned long long)ntg);
+        atomicAdd(&a.pair_counts[1], (unsigned long long)nm * (unsigned long long)ntg);
+    }
+}
+
+// ---- host driver ----------------------------------------------------------------------------
+int pb_tree_build_impl(pb_ctx* ctx)
+{
+    pb_tree& t = ctx->tree;
+    cudaStream_t st = ctx->stream;
+    const int64_t N = ctx->nt;
+    const int K = ctx->prm.K_far;
+    if (N * K >= 2147483647LL) return pb_fail(ctx, PB_ERR_INVALID_ARG, "too many source points for int32 indexing");
+    t.N = N;
+    t.K = K;
+    t.Ns = N * K;
+    const int64_t Ns = t.Ns;
+
+    // --- Morton keys and sort
+    PB_TRY(pb_scratch(ctx, 1 << 20));
+    double* box = ctx->scratch;
+    k_bbox<<<1, 1024, 0, st>>>(N, ctx->cen, box);
+    PB_LAUNCH_CHECK();
+    uint64_t *k0, *k1;
+    int32_t *v0, *v1;
+    PB_TRY(pb_dalloc_t(ctx, &k0, N, CAT_TMP));    // the sorted keys are needed for the cell build only
+    PB_TRY(pb_dalloc_t(ctx, &k1, N, CAT_TMP));
+    PB_TRY(pb_dalloc_t(ctx, &v0, N, CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &v1, N, CAT_TMP));
+    k_morton<<<pb_blocks(N, 256), 256, 0, st>>>(N, ctx->cen, box, k0, v0);
+    PB_LAUNCH_CHECK();
+    {
+        int64_t nwt = (N + RS_TILE - 1) / RS_TILE;
+        int32_t* hist;
+        PB_TRY(pb_dalloc_t(ctx, &hist, 256 * nwt, CAT_TMP));
+        int nb = (int)((nwt + RS_WARPS - 1) / RS_WARPS);
+        uint64_t *ka = k0, *kb = k1;
+        int32_t *va = v0, *vb = v1;
+        for (int pass = 0; pass < 8; ++pass) {
+            int shift = 8 * pass;
+            k_rs_hist<<<nb, 32 * RS_WARPS, 0, st>>>(ka, N, shift, nwt, hist);
+            PB_LAUNCH_CHECK();
+            PB_TRY(pb_exclusive_scan_i32(ctx, hist, hist, 256 * nwt, nullptr));
+            k_rs_scatter<<<nb, 32 * RS_WARPS, 0, st>>>(ka, va, kb, vb, N, shift, nwt, hist);
+            PB_LAUNCH_CHECK();
+            uint64_t* tk = ka; ka = kb; kb = tk;
+            int32_t* tv = va; va = vb; vb = tv;
+        }
+        // 8 passes: the result is back in (k0, v0)
+    }
+    t.perm = v0;
+    const uint64_t* keys = k0;
+
+    // --- geometry in Morton order
+    for (int d = 0; d < 3; ++d) {
+        PB_TRY(pb_dalloc_t(ctx, &t.pc[d], N, CAT_TREE));
+        PB_TRY(pb_dalloc_t(ctx, &t.pn[d], N, CAT_TREE));
+        PB_TRY(pb_dalloc_t(ctx, &t.ptri[d], N, CAT_TREE));
+        PB_TRY(pb_dalloc_t(ctx, &t.sx[d], Ns, CAT_TREE));
+        PB_TRY(pb_dalloc_t(ctx, &t.qK[d], Ns, CAT_TREE));
+    }
+    for (int k = 0; k < 9; ++k) PB_TRY(pb_dalloc_t(ctx, &t.pv[k], N, CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.parea, N, CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.swA, Ns, CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.qV, Ns, CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.xphi, N, CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.xdphi, N, CAT_TREE));
+    {
+        geo_ptrs g;
+        for (int d = 0; d < 3; ++d) { g.pc[d] = t.pc[d]; g.pn[d] = t.pn[d]; g.ptri[d] = t.ptri[d]; g.sx[d] = t.sx[d]; }
+        for (int k = 0; k < 9; ++k) g.pv[k] = t.pv[k];
+        g.parea = t.parea;
+        g.swA = t.swA;
+        k_gather<<<pb_blocks(N, 128), 128, 0, st>>>(N, t.perm, ctx->verts, ctx->tris, ctx->ruleF, g);
+        PB_LAUNCH_CHECK();
+    }
+
+    // --- octree topology
+    const int64_t cap = 2 * N + 8;
+    PB_TRY(pb_dalloc_t(ctx, &t.c_first, cap, CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.c_last, cap, CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.c_child, cap, CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.c_nchild, cap, CAT_TREE));
+    int32_t *nchild, *choff, *bounds;
+    PB_TRY(pb_dalloc_t(ctx, &nchild, cap, CAT_TMP));
+    PB_TRY(pb_dalloc_t(ctx, &choff, cap, CAT_TMP));
+    PB_TRY(pb_dalloc_t(ctx, &bounds, 9 * cap, CAT_TMP));
+    {
+        int32_t root[2] = {0, (int32_t)N};
+        PB_CUDA(cudaMemcpyAsync(t.c_first, &root[0], sizeof(int32_t), cudaMemcpyHostToDevice, st));
+        PB_CUDA(cudaMemcpyAsync(t.c_last, &root[1], sizeof(int32_t), cudaMemcpyHostToDevice, st));
+        PB_CUDA(cudaStreamSynchronize(st));
+    }
+    t.gen_start.clear();
+    t.gen_start.push_back(0);
+    t.gen_start.push_back(1);
+    int64_t ncell = 1;
+    for (;;) {
+        int64_t c0 = t.gen_start[t.gen_start.size() - 2], c1 = t.gen_start.back();
+        int64_t ng = c1 - c0;
+        k_cell_split<<<pb_blocks(ng, 128), 128, 0, st>>>(c0, c1, keys, t.c_first, t.c_last, K, ctx->prm.ncrit, nchild, bounds);
+        PB_LAUNCH_CHECK();
+        int64_t total = 0;
+        PB_TRY(pb_exclusive_scan_i32(ctx, nchild, choff, ng, &total));
+        if (ncell + total > cap) return pb_fail(ctx, PB_ERR_ALLOC, "octree cell capacity exceeded");
+        k_cell_emit<<<pb_blocks(ng, 128), 128, 0, st>>>(c0, c1, nchild, choff, bounds, ncell, t.c_first, t.c_last,
+                                                       t.c_child, t.c_nchild);
+        PB_LAUNCH_CHECK();
+        if (total == 0) break;
+        ncell += total;
+        t.gen_start.push_back(ncell);
+    }
+    t.n_cells = ncell;
+    t.n_levels = (int64_t)t.gen_start.size() - 1;
+    // leaves
+    {
+        int32_t* flag = nchild;   // reuse
+        k_mark_leaves<<<pb_blocks(ncell, 256), 256, 0, st>>>(ncell, t.c_child, flag);
+        PB_LAUNCH_CHECK();
+        int64_t nl = 0;
+        PB_TRY(pb_exclusive_scan_i32(ctx, flag, choff, ncell, &nl));
+        t.n_leaves = nl;
+        PB_TRY(pb_dalloc_t(ctx, &t.leaf_ids, nl, CAT_TREE));
+        k_compact_leaves<<<pb_blocks(ncell, 256), 256, 0, st>>>(ncell, t.c_child, choff, t.leaf_ids);
+        PB_LAUNCH_CHECK();
+    }
+    // --- cell geometry, bottom-up
+    for (int d = 0; d < 3; ++d) PB_TRY(pb_dalloc_t(ctx, &t.c_ctr[d], ncell, CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.c_rad, ncell, CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.c_box, 6 * ncell, CAT_TREE));
+    k_leaf_geom<<<pb_blocks(t.n_leaves * 32, 128), 128, 0, st>>>(t.n_leaves, t.leaf_ids, t.c_first, t.c_last, K, t.sx[0],
+                                                                t.sx[1], t.sx[2], t.c_ctr[0], t.c_ctr[1], t.c_ctr[2],
+                                                                t.c_rad, t.c_box);
+    PB_LAUNCH_CHECK();
+    for (int g = (int)t.gen_start.size() - 2; g >= 0; --g) {
+        int64_t c0 = t.gen_start[g], c1 = t.gen_start[g + 1];
+        k_inner_geom<<<pb_blocks(c1 - c0, 128), 128, 0, st>>>(c0, c1, t.c_child, t.c_nchild, t.c_ctr[0], t.c_ctr[1],
+                                                             t.c_ctr[2], t.c_rad, t.c_box);
+        PB_LAUNCH_CHECK();
+    }
+
+    // --- target groups
+    t.n_groups = (N + PB_TG - 1) / PB_TG;
+    const int64_t G = t.n_groups;
+    for (int d = 0; d < 3; ++d) PB_TRY(pb_dalloc_t(ctx, &t.g_ctr[d], G, CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.g_rad, G, CAT_TREE));
+    k_group_geom<<<pb_blocks(G * 32, 128), 128, 0, st>>>(G, N, t.pc[0], t.pc[1], t.pc[2], t.g_ctr[0], t.g_ctr[1],
+                                                        t.g_ctr[2], t.g_rad);
+    PB_LAUNCH_CHECK();
+
+    // --- interaction lists: count, scan, fill
+    PB_TRY(pb_dalloc_t(ctx, &t.m2p_off, G + 1, CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.p2p_off, G + 1, CAT_TREE));
+    list_args a;
+    a.ng = G; a.N = N; a.Ns = Ns; a.K = K;
+    a.theta = ctx->prm.theta;
+    a.m2p_min = 8;   // an M2P pair costs about as much as 8 P2P pairs (D: section 7)
+    a.c_first = t.c_first; a.c_last = t.c_last; a.c_child = t.c_child; a.c_nchild = t.c_nchild;
+    a.cx = t.c_ctr[0]; a.cy = t.c_ctr[1]; a.cz = t.c_ctr[2]; a.crad = t.c_rad;
+    a.gx = t.g_ctr[0]; a.gy = t.g_ctr[1]; a.gz = t.g_ctr[2]; a.grad = t.g_rad;
+    int32_t *cnt_m, *cnt_p;
+    PB_TRY(pb_dalloc_t(ctx, &cnt_m, G + 1, CAT_TMP));
+    PB_TRY(pb_dalloc_t(ctx, &cnt_p, G + 1, CAT_TMP));
+    PB_CUDA(cudaMemsetAsync(cnt_m, 0, sizeof(int32_t) * (G + 1), st));
+    PB_CUDA(cudaMemsetAsync(cnt_p, 0, sizeof(int32_t) * (G + 1), st));
+    unsigned long long* pc = (unsigned long long*)ctx->scratch;
+    PB_CUDA(cudaMemsetAsync(pc, 0, 2 * sizeof(unsigned long long), st));
+    a.n_m2p = cnt_m; a.n_p2p = cnt_p; a.m2p_cell = nullptr; a.p2p_lo = nullptr; a.p2p_hi = nullptr;
+    a.pair_counts = pc;
+    k_lists<0><<<pb_blocks(G, 64), 64, 0, st>>>(a);
+    PB_LAUNCH_CHECK();
+    unsigned long long hpc[2];
+    PB_CUDA(cudaMemcpyAsync(hpc, pc, sizeof(hpc), cudaMemcpyDeviceToHost, st));
+    int64_t tot_m = 0, tot_p = 0;
+    PB_TRY(pb_exclusive_scan_i32(ctx, cnt_m, t.m2p_off, G + 1, &tot_m));
+    PB_TRY(pb_exclusive_scan_i32(ctx, cnt_p, t.p2p_off, G + 1, &tot_p));
+    t.p2p_pairs = (int64_t)hpc[0];
+    t.m2p_pairs = (int64_t)hpc[1];
+    PB_TRY(pb_dalloc_t(ctx, &t.m2p_cell, tot_m, CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.p2p_lo, tot_p, CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.p2p_hi, tot_p, CAT_TREE));
+    a.n_m2p = t.m2p_off; a.n_p2p = t.p2p_off; a.m2p_cell = t.m2p_cell; a.p2p_lo = t.p2p_lo; a.p2p_hi = t.p2p_hi;
+    k_lists<1><<<pb_blocks(G, 64), 64, 0, st>>>(a);
+    PB_LAUNCH_CHECK();
+
+    // partial-sum slices: enough blocks to fill 148 SMs several times over on small meshes
+    {
+        int64_t want = 148 * 8;
+        int ns = (int)((want + G - 1) / G);
+        if (ns < 1) ns = 1;
+        if (ns > 64) ns = 64;
+        t.nslice_p2p = ns;
+        t.nslice_m2p = ns;
+        PB_TRY(pb_dalloc_t(ctx, &t.accP, (size_t)t.nslice_p2p * 4 * N, CAT_TREE));
+        PB_TRY(pb_dalloc_t(ctx, &t.accM, (size_t)t.nslice_m2p * 4 * N, CAT_TREE));
+    }
+    PB_CUDA(cudaStreamSynchronize(st));
+    pb_dfree_cat(ctx, CAT_TMP);
+    return PB_OK;
+}
