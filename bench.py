@@ -1,0 +1,338 @@
+#!/usr/bin/env python
+"""bench.py -- one polarizable Poisson-Boltzmann solve per step on seeded synthetic input.
+
+A step is one pass of the whole hot path over one workload:
+pb_mesh_load -> pb_sites_load -> pb_tree_build (Morton octree, lists, near/singular table) ->
+pb_solve (vacuum SCF, then {RHS -> GMRES with one treecode matvec per iteration -> reaction
+field -> multipole field -> SOR update} to 1e-7 Debye, then the energies).
+
+  metric  = treecode matvec interactions per second over the whole step
+            (P2P (target, Gauss point) pairs + M2P (target, cell) pairs, times the matvecs done)
+  ms_per_step = time per polarizable PB solve (the second half of BASELINE.json's metric)
+  e2e     = the same through the host-buffer C-ABI calls (inputs in pinned host memory copied in
+            every step, x and mu copied out)
+  roofline = the dominant kernel (P2P), FP64 ALU bound, CUDA-event timed inside the step
+  cpu_baseline = the oracle's direct O(N^2 K) matvec on this box's host cores
+
+python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C1] [--impl reference]
+N > 1 (torchrun): the path has no data-path exchange on one GPU; ranks run independent
+replicas of the workload ("weak" scaling), timed as the max over ranks.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "treecode_matvec_interactions_per_s"
+UNIT = "interactions/s"
+# Algorithmic FP64 work per unit: one P2P pair = the four kernels of
+# Eq. (3)-(4) for one (target, Gauss point) pair; one M2P pair at order P = 4*NT + Nk + 6P + 30.
+P2P_FLOP_PER_PAIR = 80.0
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # SMs x FP64 FMA lanes x 2 x max SM clock
+
+
+def m2p_flop_per_pair(P, n_terms):
+    nk = (P + 1) * (P + 2) * (P + 3) // 6
+    return 4.0 * n_terms + nk + 6.0 * P + 30.0
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index = index
+        self.samples = []
+        self.stop_flag = threading.Event()
+
+    def run(self):
+        q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        while not self.stop_flag.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-i",
+                                      str(self.index)], capture_output=True, text=True, timeout=5).stdout.strip()
+                f = [s.strip() for s in out.split(",")]
+                if len(f) >= 6:
+                    self.samples.append(f)
+            except Exception:
+                pass
+            self.stop_flag.wait(0.2)
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
+        sm = sorted(float(s[0]) for s in self.samples)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(s[2 + k].lower().startswith("active") for s in self.samples)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.samples[0][1]), "reasons": reasons,
+                "samples": len(sm)}
+
+
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def max_over_ranks(value, world, device=None):
+    """Max of a python float over ranks (identity when world == 1).  gloo or nccl."""
+    if world == 1:
+        return value
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def sum_over_ranks(value, world, device=None):
+    if world == 1:
+        return value
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def load_workload(name):
+    from paper_1810_03698_b200.workloads import make_config
+    return make_config(name)
+
+
+def oracle_matvec_rate(w, budget_s=12.0):
+    """The oracle as it stands: direct O(N^2 K) matvec over all host cores."""
+    import numpy as np
+    from oracle import pb_oracle as po
+    po.build()
+    orc = po.Oracle(w.verts, w.tris, po.Params(K_far=w.params["K_far"]))
+    n = orc.nt
+    x = np.random.Generator(np.random.PCG64(7)).normal(size=2 * n)
+    rows = None
+    pairs_per_call = float(n) * n * w.params["K_far"]
+    if pairs_per_call > 2e9:                      # bounded sample of target rows on big meshes
+        rows = np.random.Generator(np.random.PCG64(8)).choice(n, size=4096, replace=False)
+        pairs_per_call = 4096.0 * n * w.params["K_far"]
+    orc.matvec(x, rows)                            # warm-up (thread pool, page faults)
+    t0 = time.perf_counter()
+    reps = 0
+    while True:
+        orc.matvec(x, rows)
+        reps += 1
+        el = time.perf_counter() - t0
+        if el > budget_s or reps >= 50:
+            break
+    return dict(value=pairs_per_call * reps / el, unit=UNIT, cores=po.num_threads(), kind="oracle",
+                sample=f"{reps} direct O(N^2 K) oracle matvecs of {w.name}"
+                       + (" on 4096 sampled target rows" if rows is not None else " (all rows)")
+                       + f", {el:.1f} s", ms_per_call=1e3 * el / reps)
+
+
+def run_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return
+    w = load_workload(args.workload)
+    import numpy as np
+    from oracle import pb_oracle as po
+    po.build()
+    orc = po.Oracle(w.verts, w.tris, po.Params(K_far=w.params["K_far"]))
+    n = orc.nt
+    x = np.random.Generator(np.random.PCG64(7)).normal(size=2 * n)
+    rows = None
+    pairs = float(n) * n * w.params["K_far"]
+    if pairs > 2e9:
+        rows = np.random.Generator(np.random.PCG64(8)).choice(n, size=4096, replace=False)
+        pairs = 4096.0 * n * w.params["K_far"]
+    for _ in range(args.warmup):
+        orc.matvec(x, rows)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        orc.matvec(x, rows)
+    el = time.perf_counter() - t0
+    val = pairs * args.steps / el
+    sample = (f"each step = one direct O(N^2 K) oracle matvec of {w.name}"
+              + (" on 4096 sampled target rows" if rows is not None else " (all rows)"))
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "panels": int(n), "K_far": int(w.params["K_far"]), "what": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": po.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    rank, local_rank, world = dist_env()
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    from paper_1810_03698_b200 import pb
+    pb.lib()                                       # fails loudly if the CUDA library is missing
+
+    w = load_workload(args.workload)               # every rank: its own replica of the workload
+    names = {k for k, _ in pb.Params._fields_}
+    prm = {k: v for k, v in w.params.items() if k in names}
+    if args.theta is not None:
+        prm["theta"] = args.theta
+    if args.order is not None:
+        prm["order_P"] = args.order
+    if args.ncrit is not None:
+        prm["ncrit"] = args.ncrit
+    ctx = pb.PB(local_rank, **prm)
+    s = w.sites
+    f64, i32 = torch.float64, torch.int32
+    host = dict(verts=torch.from_numpy(np.ascontiguousarray(w.verts)).pin_memory(),
+                tris=torch.from_numpy(np.ascontiguousarray(w.tris, dtype=np.int32)).pin_memory(),
+                pos=torch.from_numpy(np.ascontiguousarray(s["pos"])).pin_memory(),
+                q=torch.from_numpy(np.ascontiguousarray(s["q"])).pin_memory(),
+                dip=torch.from_numpy(np.ascontiguousarray(s["dip"])).pin_memory(),
+                quad=torch.from_numpy(np.ascontiguousarray(s["quad"])).pin_memory(),
+                alpha=torch.from_numpy(np.ascontiguousarray(s["alpha"])).pin_memory(),
+                group=torch.from_numpy(np.ascontiguousarray(s["group"], dtype=np.int32)).pin_memory())
+    resident = {k: v.to(dev) for k, v in host.items()}
+    nt, na = int(w.tris.shape[0]), int(s["pos"].shape[0])
+    x_host = torch.empty(2 * nt, dtype=f64).pin_memory()
+    mu_host = torch.empty(na, 3, dtype=f64).pin_memory()
+    h2d = sum(v.numel() * v.element_size() for v in host.values())
+    d2h = x_host.numel() * 8 + mu_host.numel() * 8
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+
+    def step_resident():
+        d = resident
+        ctx.mesh_load(d["verts"], d["tris"])
+        ctx.sites_load(d["pos"], d["q"], d["dip"], d["quad"], d["alpha"], d["group"])
+        ctx.tree_build()
+        return ctx.solve()[2]
+
+    def step_e2e():
+        d = {k: v.to(dev, non_blocking=True) for k, v in host.items()}
+        ctx.mesh_load(d["verts"], d["tris"])
+        ctx.sites_load(d["pos"], d["q"], d["dip"], d["quad"], d["alpha"], d["group"])
+        ctx.tree_build()
+        return ctx.solve_host(x_host, mu_host)
+
+    def barrier():
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, steps):
+        tot_ms, last = 0.0, None
+        for _ in range(steps):
+            flush.zero_()                          # L2 flush, outside the event pair
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            last = fn()
+            e1.record()
+            e1.synchronize()
+            tot_ms += e0.elapsed_time(e1)
+        return tot_ms, last
+
+    for _ in range(max(args.warmup, 3)):
+        res = step_resident()
+    step_e2e()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    ctx.set_profiling(True)
+    st0 = ctx.stats()
+    barrier()
+    ms_total, res = timed(step_resident, args.steps)
+    barrier()
+    st1 = ctx.stats()
+    ctx.set_profiling(False)
+    barrier()
+    ms_e2e, res_e2e = timed(step_e2e, args.steps)
+    barrier()
+    sampler.stop_flag.set()
+    sampler.join(timeout=2)
+
+    ms_total = max_over_ranks(ms_total, world, dev)
+    ms_e2e = max_over_ranks(ms_e2e, world, dev)
+    inter_per_mv = st1["p2p_pairs"] + st1["m2p_pairs"]
+    mv_timed = st1["matvec_calls"] - st0["matvec_calls"]
+    units = sum_over_ranks(float(inter_per_mv) * mv_timed, world, dev)
+    units_e2e = sum_over_ranks(float(inter_per_mv) * res_e2e["matvecs_total"] * args.steps, world, dev)
+    value = units / (ms_total * 1e-3)
+    value_e2e = units_e2e / (ms_e2e * 1e-3)
+    launches = st1["kernel_launches"] - st0["kernel_launches"]
+
+    # roofline of the dominant kernel, from the CUDA-event pairs recorded inside the timed steps
+    P = int(ctx.get_params().order_P)
+    p2p_ms = st1["prof_p2p_ms"] / max(st1["prof_p2p_launches"], 1)
+    m2p_ms = st1["prof_m2p_ms"] / max(st1["prof_m2p_launches"], 1)
+    p2p_tf = P2P_FLOP_PER_PAIR * st1["p2p_pairs"] / (p2p_ms * 1e-3) / 1e12 if p2p_ms > 0 else 0.0
+    m2p_tf = (m2p_flop_per_pair(P, st1["n_terms"]) * st1["m2p_pairs"] / (m2p_ms * 1e-3) / 1e12) if m2p_ms > 0 else 0.0
+    dominant = "k_p2p" if st1["prof_p2p_ms"] >= st1["prof_m2p_ms"] else "k_m2p"
+    ach = p2p_tf if dominant == "k_p2p" else m2p_tf
+    roofline = {"bound": "alu", "kernel": dominant, "achieved": ach, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                "frac": ach / FP64_PEAK_TFLOPS, "traffic": None,
+                "peak_source": "148 SM x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md section 7); "
+                               "pb_fp64_peak_probe measured %.1f TFLOP/s on this GPU" % ctx.fp64_peak_probe(),
+                "p2p": {"ms_per_launch": p2p_ms, "launches": st1["prof_p2p_launches"], "pairs": st1["p2p_pairs"],
+                        "tflops": p2p_tf, "share_of_step": st1["prof_p2p_ms"] / ms_total},
+                "m2p": {"ms_per_launch": m2p_ms, "launches": st1["prof_m2p_launches"], "pairs": st1["m2p_pairs"],
+                        "tflops": m2p_tf, "share_of_step": st1["prof_m2p_ms"] / ms_total}}
+    if rank != 0:
+        return
+    cpu = oracle_matvec_rate(w) if world == 1 and not args.no_cpu_baseline else None
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "panels": nt, "gauss_points": int(st1["n_sources"]), "sites": na,
+                   "theta": float(ctx.get_params().theta), "order_P": P, "ncrit": int(ctx.get_params().ncrit),
+                   "K_far": int(w.params["K_far"]), "gmres_tol": float(ctx.get_params().gmres_tol),
+                   "scf_tol_debye": float(ctx.get_params().scf_tol_debye),
+                   "l2": "flushed between steps (256 MiB device write, outside the event pairs)",
+                   "parallelism": "replicas only" if world > 1 else "1 GPU"},
+        "solve": {"time_per_polarizable_solve_ms": ms_total / args.steps, "dG_solv_kcal_mol": res["dG_solv"],
+                  "scf_iters": res["scf_iters"], "gmres_iters": res["gmres_iters_total"], "matvecs": res["matvecs_total"],
+                  "interactions_per_matvec": int(inter_per_mv), "status": res["status"]},
+        "e2e": {"value": value_e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                "ms_per_step": ms_e2e / args.steps},
+        "gpu_launches": int(launches),
+        "roofline": roofline,
+        "clocks": sampler.summary(),
+    }
+    if cpu is not None:
+        line["cpu_baseline"] = cpu
+    print(json.dumps(line))
+    ctx.close()
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C1", help="C1 (BASELINE configs[1], default), C0, C2, C3, C4")
+    ap.add_argument("--theta", type=float, default=None)
+    ap.add_argument("--order", type=int, default=None)
+    ap.add_argument("--ncrit", type=int, default=None)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

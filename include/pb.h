@@ -97,6 +97,11 @@ typedef struct pb_stats {
     int64_t n_terms;            /* far-field terms per cell and layer (130 at P=6)             */
     int64_t matvec_calls;
     int64_t device_bytes;       /* bytes currently held through the allocator                  */
+    int64_t kernel_launches;    /* kernels launched by this context so far                     */
+    int64_t prof_p2p_launches;  /* with pb_set_profiling(ctx, 1): P2P launches timed so far     */
+    int64_t prof_m2p_launches;
+    double prof_p2p_ms;         /* ... and their summed CUDA-event durations                   */
+    double prof_m2p_ms;
     double last_matvec_ms[8];   /* CUDA-event times of the last pb_matvec_timed call:
                                    0 weights, 1 P2M+M2M+convert, 2 M2P, 3 P2P, 4 near table +
                                    combine, 5 total                                            */
@@ -179,6 +184,23 @@ int pb_solve(pb_ctx* ctx, double* x_out, double* mu_out, pb_result* result);
 int pb_solve_host(pb_ctx* ctx, double* x_host, double* mu_host, pb_result* result);
 
 int pb_get_stats(pb_ctx* ctx, pb_stats* out /* HOST */);
+
+/* Profiling: when on, every P2P and M2P launch is bracketed by a CUDA-event pair on the
+ * context's stream; pb_get_stats drains the pairs and reports summed durations and counts.
+ * Turning it on resets the sums. */
+int pb_set_profiling(pb_ctx* ctx, int on);
+
+/* HOST-only helpers (no GPU needed): the library's own tables, exported so they can be tested.
+ * pb_quadrature_rule: K in {1,3,4,7,19}; lam [K][3] barycentric nodes, w [K] weights (sum 1).
+ * pb_gauss_legendre: n <= 64 nodes x and weights w on [-1,1].
+ * pb_farfield_table: the M -> F conversion of the far field (D: section 6) for order P <= 10:
+ *   returns the number of terms NT (or a negative pb_status); expo [NT][4] = (a,b,c,j) of each
+ *   term; off [NT+1], idx/coef [off[NT]] the CSR combination of Cartesian moments, moment
+ *   (a,b,c) living at index n(n+1)(n+2)/6 + (b+c)(b+c+1)/2 + c, n=a+b+c.  Arrays may be NULL to
+ *   query sizes: *nnz_out receives off[NT]. */
+int pb_quadrature_rule(int K, double* lam, double* w);
+int pb_gauss_legendre(int n, double* x, double* w);
+int pb_farfield_table(int P, int32_t* expo, int32_t* off, int32_t* idx, double* coef, int64_t* nnz_out);
 
 /* Measured FP64 FMA throughput of the device in TFLOP/s (independent DFMA chains, no memory
  * traffic): the denominator check for the ALU roofline of the P2P / M2P kernels.  Synchronises. */

@@ -125,6 +125,7 @@ extern "C" int pb_destroy(pb_ctx* ctx)
     if (ctx->h_pinned) cudaFreeHost(ctx->h_pinned);
     if (ctx->ev_made)
         for (int i = 0; i < 8; ++i) cudaEventDestroy(ctx->ev[i]);
+    for (auto e : ctx->prof_ev) cudaEventDestroy(e);
     delete ctx;
     return PB_OK;
 }
@@ -310,6 +311,12 @@ extern "C" int pb_get_stats(pb_ctx* ctx, pb_stats* out)
     out->n_terms = t.NT;
     out->matvec_calls = ctx->matvec_calls;
     out->device_bytes = (int64_t)ctx->bytes_held;
+    out->kernel_launches = ctx->launches;
+    PB_TRY(pb_prof_drain(ctx));
+    out->prof_p2p_launches = ctx->prof_launches[0];
+    out->prof_m2p_launches = ctx->prof_launches[1];
+    out->prof_p2p_ms = ctx->prof_ms[0];
+    out->prof_m2p_ms = ctx->prof_ms[1];
     for (int i = 0; i < 8; ++i) out->last_matvec_ms[i] = ctx->last_ms[i];
     return PB_OK;
 }
@@ -403,5 +410,75 @@ extern "C" int pb_fp64_peak_probe(pb_ctx* ctx, double* tflops_out)
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     *tflops_out = best;
+    return PB_OK;
+}
+
+// ---- profiling ring: event pairs around the P2P / M2P launches ------------------------------------------
+#define PROF_SLOTS 512
+extern "C" int pb_set_profiling(pb_ctx* ctx, int on)
+{
+    if (!ctx) return PB_ERR_INVALID_ARG;
+    PB_CUDA(cudaSetDevice(ctx->device));
+    if (on && ctx->prof_ev.empty()) {
+        ctx->prof_ev.resize(PROF_SLOTS * 4);
+        ctx->prof_mask.assign(PROF_SLOTS, 0);
+        for (auto& e : ctx->prof_ev) PB_CUDA(cudaEventCreate(&e));
+    }
+    PB_CUDA(cudaStreamSynchronize(ctx->stream));
+    ctx->prof_head = 0;
+    ctx->prof_pending = 0;
+    if (on) { ctx->prof_ms[0] = ctx->prof_ms[1] = 0; ctx->prof_launches[0] = ctx->prof_launches[1] = 0; }
+    ctx->profiling = on != 0;
+    return PB_OK;
+}
+
+// one slot per matvec; a full ring is drained (stream sync) before it wraps
+int pb_prof_drain(pb_ctx* ctx)
+{
+    if (ctx->prof_pending == 0) return PB_OK;
+    PB_CUDA(cudaStreamSynchronize(ctx->stream));
+    for (int slot = 0; slot < ctx->prof_pending; ++slot)
+        for (int kern = 0; kern < 2; ++kern) {
+            if (!(ctx->prof_mask[slot] & (1 << kern))) continue;
+            float ms = 0;
+            PB_CUDA(cudaEventElapsedTime(&ms, ctx->prof_ev[(slot * 2 + kern) * 2], ctx->prof_ev[(slot * 2 + kern) * 2 + 1]));
+            ctx->prof_ms[kern] += ms;
+            ctx->prof_launches[kern] += 1;
+        }
+    ctx->prof_pending = 0;
+    ctx->prof_head = 0;
+    return PB_OK;
+}
+
+int pb_prof_begin(pb_ctx* ctx, int kernel)
+{
+    if (!ctx->profiling) return PB_OK;
+    if (ctx->prof_head >= PROF_SLOTS) PB_TRY(pb_prof_drain(ctx));
+    if (ctx->prof_pending <= ctx->prof_head) { ctx->prof_mask[ctx->prof_head] = 0; ctx->prof_pending = ctx->prof_head + 1; }
+    PB_CUDA(cudaEventRecord(ctx->prof_ev[(ctx->prof_head * 2 + kernel) * 2], ctx->stream));
+    return PB_OK;
+}
+
+int pb_prof_end(pb_ctx* ctx, int kernel)
+{
+    if (!ctx->profiling) return PB_OK;
+    PB_CUDA(cudaEventRecord(ctx->prof_ev[(ctx->prof_head * 2 + kernel) * 2 + 1], ctx->stream));
+    ctx->prof_mask[ctx->prof_head] |= (unsigned char)(1 << kernel);
+    return PB_OK;
+}
+
+void pb_prof_next(pb_ctx* ctx)
+{
+    if (ctx->profiling && ctx->prof_pending > ctx->prof_head) ctx->prof_head++;
+}
+
+extern "C" int pb_quadrature_rule(int K, double* lam, double* w)
+{
+    pb_rule_t r;
+    if (!lam || !w || pb_make_rule(K, &r) != 0) return PB_ERR_INVALID_ARG;
+    for (int i = 0; i < K; ++i) {
+        for (int d = 0; d < 3; ++d) lam[3 * i + d] = r.lam[i][d];
+        w[i] = r.w[i];
+    }
     return PB_OK;
 }

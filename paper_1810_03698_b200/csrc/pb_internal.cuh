@@ -138,6 +138,14 @@ struct pb_ctx {
     double* h_pinned = nullptr;   // pinned host staging
     size_t h_pinned_bytes = 0;
     int64_t matvec_calls = 0;
+    int64_t launches = 0;         // kernels launched by this context
+    // profiling: CUDA-event pairs around every P2P and M2P launch (pb_set_profiling)
+    bool profiling = false;
+    std::vector<cudaEvent_t> prof_ev;   // ring: [slot][kernel 0=p2p,1=m2p][begin,end]
+    std::vector<unsigned char> prof_mask;
+    int prof_head = 0, prof_pending = 0;
+    double prof_ms[2] = {0, 0};
+    int64_t prof_launches[2] = {0, 0};
     double last_ms[8] = {0};
     cudaEvent_t ev[8] = {0};
     bool ev_made = false;
@@ -154,7 +162,11 @@ int pb_fail(pb_ctx* ctx, int code, const char* fmt, ...);
                            cudaGetErrorString(e__));                                           \
     } while (0)
 
-#define PB_LAUNCH_CHECK() PB_CUDA(cudaGetLastError())
+#define PB_LAUNCH_CHECK()                                                                      \
+    do {                                                                                       \
+        ++ctx->launches;                                                                       \
+        PB_CUDA(cudaGetLastError());                                                           \
+    } while (0)
 
 #define PB_TRY(call)                                                                           \
     do {                                                                                       \
@@ -191,5 +203,10 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed);
 int pb_weights(pb_ctx* ctx, const double* x);
 // pb_sites.cu
 int pb_site_near_build(pb_ctx* ctx);
+// pb_api.cu: profiling ring
+int pb_prof_begin(pb_ctx* ctx, int kernel);
+int pb_prof_end(pb_ctx* ctx, int kernel);
+int pb_prof_drain(pb_ctx* ctx);
+void pb_prof_next(pb_ctx* ctx);
 // pb_solve.cu
 int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters, double* relres, int32_t* matvecs);

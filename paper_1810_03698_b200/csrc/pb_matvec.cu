@@ -38,6 +38,44 @@ __constant__ double c_binom[PB_MAX_P + 1][PB_MAX_P + 1];
 
 static double factorial(int n) { double f = 1; for (int i = 2; i <= n; ++i) f *= i; return f; }
 
+// The M -> F conversion table for order P, terms in the order the M2P kernel consumes them
+// (nested a, b, c loops, then j): F_{(a,b,c),j} = (-1)^j / (2^j a! b! c!) sum_{|beta|=j} M_{alpha+2beta}/beta!
+static void farfield_table(int P, std::vector<int32_t>& expo, std::vector<int32_t>& off, std::vector<int32_t>& idx,
+                           std::vector<double>& coef)
+{
+    off.assign(1, 0);
+    for (int a = 0; a <= P; ++a)
+        for (int b = 0; b <= P - a; ++b)
+            for (int c = 0; c <= P - a - b; ++c) {
+                int n = a + b + c;
+                for (int j = 0; j <= (P - n) / 2; ++j) {
+                    double pref = ((j & 1) ? -1.0 : 1.0) / (ldexp(1.0, j) * factorial(a) * factorial(b) * factorial(c));
+                    for (int ba = 0; ba <= j; ++ba)
+                        for (int bb = 0; bb <= j - ba; ++bb) {
+                            int bc = j - ba - bb;
+                            idx.push_back(mom_index(a + 2 * ba, b + 2 * bb, c + 2 * bc));
+                            coef.push_back(pref / (factorial(ba) * factorial(bb) * factorial(bc)));
+                        }
+                    off.push_back((int32_t)idx.size());
+                    expo.push_back(a); expo.push_back(b); expo.push_back(c); expo.push_back(j);
+                }
+            }
+}
+
+extern "C" int pb_farfield_table(int P, int32_t* expo, int32_t* off, int32_t* idx, double* coef, int64_t* nnz_out)
+{
+    if (P < 0 || P > PB_MAX_P) return PB_ERR_INVALID_ARG;
+    std::vector<int32_t> e, o, i;
+    std::vector<double> c;
+    farfield_table(P, e, o, i, c);
+    if (nnz_out) *nnz_out = (int64_t)i.size();
+    if (expo) memcpy(expo, e.data(), sizeof(int32_t) * e.size());
+    if (off) memcpy(off, o.data(), sizeof(int32_t) * o.size());
+    if (idx) memcpy(idx, i.data(), sizeof(int32_t) * i.size());
+    if (coef) memcpy(coef, c.data(), sizeof(double) * c.size());
+    return (int)o.size() - 1;
+}
+
 int pb_farfield_setup(pb_ctx* ctx)
 {
     pb_tree& t = ctx->tree;
@@ -63,24 +101,9 @@ int pb_farfield_setup(pb_ctx* ctx)
     PB_CUDA(cudaMemcpyToSymbolAsync(c_kc, kc, t.Nk, 0, cudaMemcpyHostToDevice, st));
     PB_CUDA(cudaMemcpyToSymbolAsync(c_binom, binom, sizeof(binom), 0, cudaMemcpyHostToDevice, st));
     // conversion table M -> F, entries in the order the M2P kernel consumes them
-    std::vector<int32_t> off, idx;
+    std::vector<int32_t> off, idx, expo;
     std::vector<double> coef;
-    off.push_back(0);
-    for (int a = 0; a <= P; ++a)
-        for (int b = 0; b <= P - a; ++b)
-            for (int c = 0; c <= P - a - b; ++c) {
-                int n = a + b + c;
-                for (int j = 0; j <= (P - n) / 2; ++j) {
-                    double pref = ((j & 1) ? -1.0 : 1.0) / (ldexp(1.0, j) * factorial(a) * factorial(b) * factorial(c));
-                    for (int ba = 0; ba <= j; ++ba)
-                        for (int bb = 0; bb <= j - ba; ++bb) {
-                            int bc = j - ba - bb;
-                            idx.push_back(mom_index(a + 2 * ba, b + 2 * bb, c + 2 * bc));
-                            coef.push_back(pref / (factorial(ba) * factorial(bb) * factorial(bc)));
-                        }
-                    off.push_back((int32_t)idx.size());
-                }
-            }
+    farfield_table(P, expo, off, idx, coef);
     if ((int)off.size() - 1 != t.NT) return pb_fail(ctx, PB_ERR_INVALID_ARG, "internal: far-field term count mismatch");
     PB_TRY(pb_dalloc_t(ctx, &t.cv_off, off.size(), CAT_TREE));
     PB_TRY(pb_dalloc_t(ctx, &t.cv_idx, idx.size(), CAT_TREE));
@@ -475,6 +498,7 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed)
     }
     if (timed) PB_CUDA(cudaEventRecord(ctx->ev[2], st));
     if (far) {
+        PB_TRY(pb_prof_begin(ctx, 1));
         switch (t.P) {
         case 0: launch_m2p<0>(ctx); break;
         case 1: launch_m2p<1>(ctx); break;
@@ -490,14 +514,18 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed)
         default: return pb_fail(ctx, PB_ERR_INVALID_ARG, "unsupported order_P %d", t.P);
         }
         PB_LAUNCH_CHECK();
+        PB_TRY(pb_prof_end(ctx, 1));
     }
     if (timed) PB_CUDA(cudaEventRecord(ctx->ev[3], st));
     {
         dim3 grid((unsigned)t.n_groups, (unsigned)t.nslice_p2p);
+        PB_TRY(pb_prof_begin(ctx, 0));
         k_p2p<<<grid, PB_TG, 0, st>>>(t.N, t.K, t.nslice_p2p, ctx->prm.kappa, t.p2p_off, t.p2p_lo, t.p2p_hi, t.sx[0],
                                       t.sx[1], t.sx[2], t.qV, t.qK[0], t.qK[1], t.qK[2], t.pc[0], t.pc[1], t.pc[2],
                                       t.accP);
         PB_LAUNCH_CHECK();
+        PB_TRY(pb_prof_end(ctx, 0));
+        pb_prof_next(ctx);
     }
     if (timed) PB_CUDA(cudaEventRecord(ctx->ev[4], st));
     k_combine<<<pb_blocks(t.N, 128), 128, 0, st>>>(t.N, t.nslice_p2p, far ? t.nslice_m2p : 0,

@@ -103,6 +103,15 @@ static void make_gl(int n, pb_gl_t* g)
     }
 }
 
+extern "C" int pb_gauss_legendre(int n, double* x, double* w)
+{
+    if (n < 1 || n > 64 || !x || !w) return PB_ERR_INVALID_ARG;
+    pb_gl_t g;
+    make_gl(n, &g);
+    for (int i = 0; i < n; ++i) { x[i] = g.x[i]; w[i] = g.w[i]; }
+    return PB_OK;
+}
+
 int pb_upload_rules(pb_ctx* ctx)
 {
     if (pb_make_rule(ctx->prm.K_far, &ctx->ruleF) != 0) return pb_fail(ctx, PB_ERR_INVALID_ARG, "no %d-point rule", ctx->prm.K_far);

@@ -26,7 +26,8 @@ EXPORTS = [
     "pb_create", "pb_destroy", "pb_last_error", "pb_set_allocator", "pb_default_params", "pb_set_params",
     "pb_get_params", "pb_mesh_load", "pb_sites_load", "pb_tree_build", "pb_rhs_multipole", "pb_matvec",
     "pb_matvec_timed", "pb_matvec_host", "pb_reaction_field", "pb_multipole_field", "pb_gmres", "pb_solve",
-    "pb_solve_host", "pb_get_stats", "pb_fp64_peak_probe",
+    "pb_solve_host", "pb_get_stats", "pb_fp64_peak_probe", "pb_set_profiling", "pb_quadrature_rule",
+    "pb_gauss_legendre", "pb_farfield_table",
 ]
 
 
@@ -67,7 +68,10 @@ class Stats(ctypes.Structure):
         ("n_cells", ctypes.c_int64), ("n_leaves", ctypes.c_int64), ("n_levels", ctypes.c_int64),
         ("n_groups", ctypes.c_int64), ("p2p_pairs", ctypes.c_int64), ("m2p_pairs", ctypes.c_int64),
         ("near_entries", ctypes.c_int64), ("n_terms", ctypes.c_int64), ("matvec_calls", ctypes.c_int64),
-        ("device_bytes", ctypes.c_int64), ("last_matvec_ms", ctypes.c_double * 8),
+        ("device_bytes", ctypes.c_int64), ("kernel_launches", ctypes.c_int64),
+        ("prof_p2p_launches", ctypes.c_int64), ("prof_m2p_launches", ctypes.c_int64),
+        ("prof_p2p_ms", ctypes.c_double), ("prof_m2p_ms", ctypes.c_double),
+        ("last_matvec_ms", ctypes.c_double * 8),
     ]
 
     def as_dict(self):
@@ -126,6 +130,10 @@ def lib():
         L.pb_solve_host.argtypes = [vp, vp, vp, ctypes.POINTER(Result)]
         L.pb_get_stats.argtypes = [vp, ctypes.POINTER(Stats)]
         L.pb_fp64_peak_probe.argtypes = [vp, ctypes.POINTER(dbl)]
+        L.pb_set_profiling.argtypes = [vp, ctypes.c_int]
+        L.pb_quadrature_rule.argtypes = [ctypes.c_int, vp, vp]
+        L.pb_gauss_legendre.argtypes = [ctypes.c_int, vp, vp]
+        L.pb_farfield_table.argtypes = [ctypes.c_int, vp, vp, vp, vp, ctypes.POINTER(i64)]
         for name in EXPORTS:
             if name not in ("pb_last_error", "pb_default_params"):
                 getattr(L, name).restype = ctypes.c_int
@@ -137,6 +145,43 @@ def default_params() -> Params:
     p = Params()
     lib().pb_default_params(ctypes.byref(p))
     return p
+
+
+def quadrature_rule(K: int):
+    """The library's own K-point triangle rule (host-only call): (lam [K][3], w [K])."""
+    import numpy as np
+    lam = np.zeros((K, 3))
+    w = np.zeros(K)
+    rc = lib().pb_quadrature_rule(K, lam.ctypes.data, w.ctypes.data)
+    if rc != PB_OK:
+        raise PBError(rc, f"no {K}-point rule")
+    return lam, w
+
+
+def gauss_legendre(n: int):
+    import numpy as np
+    x = np.zeros(n)
+    w = np.zeros(n)
+    rc = lib().pb_gauss_legendre(n, x.ctypes.data, w.ctypes.data)
+    if rc != PB_OK:
+        raise PBError(rc, "pb_gauss_legendre")
+    return x, w
+
+
+def farfield_table(P: int):
+    """The library's M -> F conversion table for order P (host-only call):
+    (expo [NT][4] = a,b,c,j ; off [NT+1] ; idx ; coef)."""
+    import numpy as np
+    nnz = ctypes.c_int64(0)
+    nt = lib().pb_farfield_table(P, None, None, None, None, ctypes.byref(nnz))
+    if nt < 0:
+        raise PBError(nt, "pb_farfield_table")
+    expo = np.zeros((nt, 4), dtype=np.int32)
+    off = np.zeros(nt + 1, dtype=np.int32)
+    idx = np.zeros(nnz.value, dtype=np.int32)
+    coef = np.zeros(nnz.value)
+    lib().pb_farfield_table(P, expo.ctypes.data, off.ctypes.data, idx.ctypes.data, coef.ctypes.data, ctypes.byref(nnz))
+    return expo, off, idx, coef
 
 
 def _ptr(t):
@@ -311,6 +356,9 @@ class PB:
         s = Stats()
         self._ck(self._L.pb_get_stats(self._h, ctypes.byref(s)))
         return s.as_dict()
+
+    def set_profiling(self, on: bool):
+        self._ck(self._L.pb_set_profiling(self._h, 1 if on else 0))
 
     def fp64_peak_probe(self) -> float:
         v = ctypes.c_double(0.0)
