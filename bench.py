@@ -249,7 +249,12 @@ def run_ours(args):
     ctx.set_profiling(True)
     st0 = ctx.stats()
     barrier()
+    if args.profiler_range:                        # ncu --profile-from-start off captures exactly the timed steps
+        torch.cuda.profiler.start()
     ms_total, res = timed(step_resident, args.steps)
+    if args.profiler_range:
+        torch.cuda.synchronize()
+        torch.cuda.profiler.stop()
     barrier()
     st1 = ctx.stats()
     ctx.set_profiling(False)
@@ -327,6 +332,8 @@ def main():
     ap.add_argument("--order", type=int, default=None)
     ap.add_argument("--ncrit", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--profiler-range", action="store_true",
+                    help="bracket the timed resident steps with cudaProfilerStart/Stop (for ncu --profile-from-start off)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
