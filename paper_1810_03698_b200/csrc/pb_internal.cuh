@@ -9,6 +9,7 @@
 #include <utility>
 
 #include "../../include/pb.h"
+#include "pb_device.cuh"
 
 #define PB_INV4PI 0.079577471545947667884
 #define PB_MAX_P 10
@@ -40,9 +41,10 @@ struct pb_tree {
     // source Gauss points (SoA), s = panel*K + g
     double* sx[3] = {0, 0, 0};
     double* swA = nullptr;        // w_g * A_j
-    // per-matvec source weights
-    double* qV = nullptr;         // w A dphi
-    double* qK[3] = {0, 0, 0};    // w A phi n
+    // per-matvec source records, 64 B per Gauss point: srec[2s] = (y_x, y_y, y_z, w A dphi),
+    // srec[2s+1] = (w A phi n_x, w A phi n_y, w A phi n_z, 0)   (written by k_weights)
+    double4* srec = nullptr;
+    pb_expk ek;                   // constants of exp(-kappa r) for this kappa
     double* xphi = nullptr;       // [N] phi in Morton order
     double* xdphi = nullptr;      // [N]
     // cells
@@ -201,6 +203,7 @@ int pb_upload_rules(pb_ctx* ctx);   // fills ctx->ruleF, ruleN, gl from the para
 int pb_farfield_setup(pb_ctx* ctx);
 int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed);
 int pb_weights(pb_ctx* ctx, const double* x);
+void pb_make_expk(double kappa, pb_expk* out);
 // pb_sites.cu
 int pb_site_near_build(pb_ctx* ctx);
 // pb_api.cu: profiling ring

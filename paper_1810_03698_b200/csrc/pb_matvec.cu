@@ -118,11 +118,14 @@ int pb_farfield_setup(pb_ctx* ctx)
 }
 
 // ---- source weights (H5): q^V_g = w_g A_j dphi_j ,  q^K_g = w_g A_j phi_j n_j ------------------------
+// Writes the 64-byte source records the P2P / P2M / reaction kernels stream (coordinates repeated
+// so that one contiguous TMA bulk copy brings a whole tile of sources into shared memory).
 __global__ void k_weights(int64_t N, int K, const int32_t* __restrict__ perm, const double* __restrict__ x,
-                          const double* __restrict__ swA, const double* __restrict__ nx,
-                          const double* __restrict__ ny, const double* __restrict__ nz, double* __restrict__ xphi,
-                          double* __restrict__ xdphi, double* __restrict__ qV, double* __restrict__ qKx,
-                          double* __restrict__ qKy, double* __restrict__ qKz)
+                          const double* __restrict__ swA, const double* __restrict__ sx,
+                          const double* __restrict__ sy, const double* __restrict__ sz,
+                          const double* __restrict__ nx, const double* __restrict__ ny,
+                          const double* __restrict__ nz, double* __restrict__ xphi, double* __restrict__ xdphi,
+                          double4* __restrict__ srec)
 {
     int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (s >= N * K) return;
@@ -130,20 +133,32 @@ __global__ void k_weights(int64_t N, int K, const int32_t* __restrict__ perm, co
     int64_t o = perm[i];
     double phi = x[o], dphi = x[N + o], w = swA[s];
     if (s == i * K) { xphi[i] = phi; xdphi[i] = dphi; }
-    qV[s] = w * dphi;
     double wp = w * phi;
-    qKx[s] = wp * nx[i];
-    qKy[s] = wp * ny[i];
-    qKz[s] = wp * nz[i];
+    srec[2 * s] = make_double4(sx[s], sy[s], sz[s], w * dphi);
+    srec[2 * s + 1] = make_double4(wp * nx[i], wp * ny[i], wp * nz[i], 0.0);
 }
 
 int pb_weights(pb_ctx* ctx, const double* x)
 {
     pb_tree& t = ctx->tree;
-    k_weights<<<pb_blocks(t.Ns, 256), 256, 0, ctx->stream>>>(t.N, t.K, t.perm, x, t.swA, t.pn[0], t.pn[1], t.pn[2],
-                                                            t.xphi, t.xdphi, t.qV, t.qK[0], t.qK[1], t.qK[2]);
+    k_weights<<<pb_blocks(t.Ns, 256), 256, 0, ctx->stream>>>(t.N, t.K, t.perm, x, t.swA, t.sx[0], t.sx[1], t.sx[2], t.pn[0],
+                                                            t.pn[1], t.pn[2], t.xphi, t.xdphi, t.srec);
     PB_LAUNCH_CHECK();
     return PB_OK;
+}
+
+// constants of pb_exp_mkr (pb_device.cuh)
+void pb_make_expk(double kappa, pb_expk* k)
+{
+    const double ln2 = 0.693147180559945309417232121458;
+    k->c1 = 32.0 * kappa / ln2;
+    k->Lk = kappa > 0.0 ? ln2 / (32.0 * kappa) : 0.0;
+    double f = 1.0;
+    for (int m = 0; m <= 6; ++m) {
+        k->c[m] = f;
+        f *= -kappa / (double)(m + 1);
+    }
+    for (int j = 0; j < 32; ++j) k->T[j] = exp2(-(double)j / 32.0);
 }
 
 // ---- P2M at the leaves: M^V_k = sum_g q^V_g h^k,  M^K_k = sum_g sum_d q^K_{g,d} k_d h^{k-e_d} ---
@@ -151,9 +166,7 @@ int pb_weights(pb_ctx* ctx, const double* x)
 __global__ void __launch_bounds__(128)
 k_p2m_leaf(int P, int Nk, int K, const int32_t* __restrict__ leaf_ids, const int32_t* __restrict__ c_first,
            const int32_t* __restrict__ c_last, const double* __restrict__ cx, const double* __restrict__ cy,
-           const double* __restrict__ cz, const double* __restrict__ sx, const double* __restrict__ sy,
-           const double* __restrict__ sz, const double* __restrict__ qV, const double* __restrict__ qKx,
-           const double* __restrict__ qKy, const double* __restrict__ qKz, double* __restrict__ M)
+           const double* __restrict__ cz, const double4* __restrict__ srec, double* __restrict__ M)
 {
     __shared__ double pw[3][PB_MAX_P + 1][P2M_CH];
     __shared__ double wq[4][P2M_CH];
@@ -166,15 +179,16 @@ k_p2m_leaf(int P, int Nk, int K, const int32_t* __restrict__ leaf_ids, const int
         __syncthreads();
         if (threadIdx.x < np) {
             int64_t s = base + threadIdx.x;
-            double h[3] = {sx[s] - yc[0], sy[s] - yc[1], sz[s] - yc[2]};
+            const double4 ra = srec[2 * s], rb = srec[2 * s + 1];
+            double h[3] = {ra.x - yc[0], ra.y - yc[1], ra.z - yc[2]};
             for (int d = 0; d < 3; ++d) {
                 double p = 1.0;
                 for (int e = 0; e <= P; ++e) { pw[d][e][threadIdx.x] = p; p *= h[d]; }
             }
-            wq[0][threadIdx.x] = qV[s];
-            wq[1][threadIdx.x] = qKx[s];
-            wq[2][threadIdx.x] = qKy[s];
-            wq[3][threadIdx.x] = qKz[s];
+            wq[0][threadIdx.x] = ra.w;
+            wq[1][threadIdx.x] = rb.x;
+            wq[2][threadIdx.x] = rb.y;
+            wq[3][threadIdx.x] = rb.z;
         }
         __syncthreads();
         for (int r = 0; r < 3; ++r) {
@@ -362,69 +376,134 @@ k_m2p(int64_t N, int nslice, double kappa, const int32_t* __restrict__ m2p_off, 
 // ---- P2P (H7; "source-target" interactions) ---------------------------------------------------------
 // Kernels of Eq. (3)-(4) without the 1/(4 pi), which the combine step applies once:
 //   VL += qV/R, KL += (qK.d)/R^3, VY += qV e^{-kR}/R, KY += (qK.d) e^{-kR}(1+kR)/R^3,  d = x - y.
-#define P2P_TILE 128
+// One block = one target group (PB_TG consecutive Morton-ordered collocation points) x one slice of
+// the group's source list.  The slice is streamed through shared memory in tiles of 64-byte source
+// records by TMA bulk copies (double-buffered, mbarrier completion).  The block's P2P_S sub-slices
+// (2 warps each) take interleaved sources of a tile for the same 64 targets, so every shared-memory
+// read is a warp-wide broadcast; their partial sums are added in a fixed order at the end.
+// Per pair: 35 FP64-pipe instructions (D: section 7).
+#define P2P_S 4
+#define P2P_THREADS (PB_TG * P2P_S)
+#define P2P_TILE 256
+static_assert(P2P_S == 4, "the final reduction maps one of the 4 outputs to each sub-slice");
+
 template <bool CHECK_SELF>
-__device__ __forceinline__ void p2p_tile(const double (*__restrict__ sm)[P2P_TILE], int cnt, int32_t s0, int32_t selfLo,
-                                         int K, double kappa, double tx, double ty, double tz, double& VL,
-                                         double& KL, double& VY, double& KY)
+__device__ __forceinline__ void p2p_tile(const double4* __restrict__ buf, int cnt, int sub, int32_t s0, int32_t selfLo,
+                                         int K, double kappa, const pb_expk& ek, const double* __restrict__ Ts,
+                                         double tx, double ty, double tz, double& VL, double& KL, double& VY,
+                                         double& KY)
 {
-#pragma unroll 2
-    for (int k = 0; k < cnt; ++k) {
+#pragma unroll 4
+    for (int k = sub; k < cnt; k += P2P_S) {
         if (CHECK_SELF && (unsigned)(s0 + k - selfLo) < (unsigned)K) continue;   // own panel: by index (D: R-11)
-        const double dx = tx - sm[0][k], dy = ty - sm[1][k], dz = tz - sm[2][k];
-        const double r2 = dx * dx + dy * dy + dz * dz;
-        const double ri = rsqrt(r2);
-        const double r = r2 * ri, ri3 = ri * ri * ri;
-        const double nd = sm[4][k] * dx + sm[5][k] * dy + sm[6][k] * dz;
-        const double qv = sm[3][k];
-        const double ex = exp(-kappa * r);
-        VL = fma(qv, ri, VL);
-        const double kl = nd * ri3;
+        const double4 a = buf[2 * k], b = buf[2 * k + 1];
+        const double dx = tx - a.x, dy = ty - a.y, dz = tz - a.z;
+        const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+        const double nd = fma(b.z, dz, fma(b.y, dy, b.x * dx));
+        const double ri = pb_rsqrt(r2);
+        const double r = r2 * ri, ri2 = ri * ri;
+        const double ex = pb_exp_mkr(r, ek, Ts);
+        const double qr = a.w * ri;
+        const double kl = nd * (ri2 * ri);
+        VL += qr;
         KL += kl;
-        VY = fma(qv * ri, ex, VY);
+        VY = fma(qr, ex, VY);
         KY = fma(kl * ex, fma(kappa, r, 1.0), KY);
     }
 }
 
-__global__ void __launch_bounds__(PB_TG)
-k_p2p(int64_t N, int K, int nslice, double kappa, const int32_t* __restrict__ p2p_off,
-      const int32_t* __restrict__ p2p_lo, const int32_t* __restrict__ p2p_hi, const double* __restrict__ sx,
-      const double* __restrict__ sy, const double* __restrict__ sz, const double* __restrict__ qV,
-      const double* __restrict__ qKx, const double* __restrict__ qKy, const double* __restrict__ qKz,
+__global__ void __launch_bounds__(P2P_THREADS)
+k_p2p(int64_t N, int K, int nslice, double kappa, pb_expk ek, const int32_t* __restrict__ p2p_off,
+      const int32_t* __restrict__ p2p_lo, const int32_t* __restrict__ p2p_hi, const double4* __restrict__ srec,
       const double* __restrict__ px, const double* __restrict__ py, const double* __restrict__ pz,
       double* __restrict__ acc)
 {
-    __shared__ double sm[7][P2P_TILE];
+    __shared__ __align__(128) double4 tile[2][2 * P2P_TILE];
+    __shared__ __align__(8) uint64_t bar[2];
+    __shared__ double Ts[32];
+    const int tid = threadIdx.x;
+    const int tgt = tid & (PB_TG - 1), sub = tid / PB_TG;
     const int64_t g = blockIdx.x;
     const int slice = blockIdx.y;
-    const int64_t i = g * PB_TG + threadIdx.x;
-    const bool live = i < N;
-    const double tx = live ? px[i] : 1e30, ty = live ? py[i] : 1e30, tz = live ? pz[i] : 1e30;
-    const int32_t selfLo = (int32_t)(i * K);
+    if (tid < 32) Ts[tid] = ek.T[tid];
+    if (tid == 0) {
+        pb_mbar_init(&bar[0], 1);
+        pb_mbar_init(&bar[1], 1);
+        pb_mbar_fence_init();
+    }
+    __syncthreads();
+    const int64_t i = g * PB_TG + tgt;
+    const int64_t ic = i < N ? i : N - 1;            // padding lanes repeat the last target; never stored
+    const double tx = px[ic], ty = py[ic], tz = pz[ic];
+    const int32_t selfLo = (int32_t)(ic * K);
     const int64_t i1 = (g + 1) * PB_TG < N ? (g + 1) * PB_TG : N;
     const int32_t grpLo = (int32_t)(g * PB_TG * K), grpHi = (int32_t)(i1 * K);
-    double VL = 0, KL = 0, VY = 0, KY = 0;
-    int64_t tile = 0;
-    for (int32_t r = p2p_off[g]; r < p2p_off[g + 1]; ++r) {
-        const int32_t lo = p2p_lo[r], hi = p2p_hi[r];
-        for (int32_t s0 = lo; s0 < hi; s0 += P2P_TILE, ++tile) {
-            if ((int)(tile % nslice) != slice) continue;
-            const int cnt = hi - s0 < P2P_TILE ? hi - s0 : P2P_TILE;
-            __syncthreads();
-            for (int k = threadIdx.x; k < cnt; k += PB_TG) {
-                sm[0][k] = sx[s0 + k]; sm[1][k] = sy[s0 + k]; sm[2][k] = sz[s0 + k]; sm[3][k] = qV[s0 + k];
-                sm[4][k] = qKx[s0 + k]; sm[5][k] = qKy[s0 + k]; sm[6][k] = qKz[s0 + k];
-            }
-            __syncthreads();
-            if (s0 < grpHi && s0 + cnt > grpLo)
-                p2p_tile<true>(sm, cnt, s0, selfLo, K, kappa, tx, ty, tz, VL, KL, VY, KY);
-            else
-                p2p_tile<false>(sm, cnt, s0, selfLo, K, kappa, tx, ty, tz, VL, KL, VY, KY);
-        }
+
+    // this slice's share of the group's source list: [begin, begin + remaining) of the concatenated ranges
+    int32_t r = p2p_off[g];
+    const int32_t rend = p2p_off[g + 1];
+    int64_t total = 0;
+    for (int32_t q = r; q < rend; ++q) total += p2p_hi[q] - p2p_lo[q];
+    int64_t begin = total * slice / nslice;
+    int64_t remaining = total * (slice + 1) / nslice - begin;
+    int32_t a = r < rend ? p2p_lo[r] : 0;
+    while (r < rend && begin > 0) {                  // skip `begin` sources
+        const int32_t len = p2p_hi[r] - a;
+        if (begin < len) { a += (int32_t)begin; begin = 0; }
+        else { begin -= len; ++r; if (r < rend) a = p2p_lo[r]; }
     }
-    if (live) {
-        double* a = acc + (int64_t)slice * 4 * N;
-        a[i] = VL; a[N + i] = KL; a[2 * N + i] = VY; a[3 * N + i] = KY;
+    auto next_tile = [&](int32_t& s0, int& cnt) -> bool {
+        while (remaining > 0 && r < rend) {
+            const int32_t hi = p2p_hi[r];
+            if (a >= hi) { ++r; if (r < rend) a = p2p_lo[r]; continue; }
+            int64_t c = hi - a;
+            if (c > P2P_TILE) c = P2P_TILE;
+            if (c > remaining) c = remaining;
+            s0 = a; cnt = (int)c;
+            a += (int32_t)c; remaining -= c;
+            return true;
+        }
+        return false;
+    };
+
+    double VL = 0, KL = 0, VY = 0, KY = 0;
+    int32_t cs0 = 0, ns0 = 0;
+    int ccnt = 0, ncnt = 0;
+    bool have = next_tile(cs0, ccnt);
+    if (have && tid == 0) {
+        pb_mbar_expect_tx(&bar[0], (uint32_t)ccnt * 64u);
+        pb_bulk_g2s(tile[0], srec + 2 * (int64_t)cs0, (uint32_t)ccnt * 64u, &bar[0]);
+    }
+    for (uint32_t it = 0; have; ++it) {
+        const int st = it & 1;
+        const bool more = next_tile(ns0, ncnt);
+        if (more && tid == 0) {                       // the other buffer was released by the barrier below
+            pb_mbar_expect_tx(&bar[st ^ 1], (uint32_t)ncnt * 64u);
+            pb_bulk_g2s(tile[st ^ 1], srec + 2 * (int64_t)ns0, (uint32_t)ncnt * 64u, &bar[st ^ 1]);
+        }
+        pb_mbar_wait(&bar[st], (it >> 1) & 1u);
+        if (cs0 < grpHi && cs0 + ccnt > grpLo)
+            p2p_tile<true>(tile[st], ccnt, sub, cs0, selfLo, K, kappa, ek, Ts, tx, ty, tz, VL, KL, VY, KY);
+        else
+            p2p_tile<false>(tile[st], ccnt, sub, cs0, selfLo, K, kappa, ek, Ts, tx, ty, tz, VL, KL, VY, KY);
+        __syncthreads();
+        have = more;
+        cs0 = ns0;
+        ccnt = ncnt;
+    }
+    // add the sub-slices in a fixed order (tile[0] is free: every thread passed the last barrier)
+    double* red = reinterpret_cast<double*>(tile[0]);   // [P2P_S][4][PB_TG]
+    red[(sub * 4 + 0) * PB_TG + tgt] = VL;
+    red[(sub * 4 + 1) * PB_TG + tgt] = KL;
+    red[(sub * 4 + 2) * PB_TG + tgt] = VY;
+    red[(sub * 4 + 3) * PB_TG + tgt] = KY;
+    __syncthreads();
+    {
+        const int m = tid / PB_TG;                     // 0..3 (P2P_S == 4 outputs per target)
+        double v = 0;
+#pragma unroll
+        for (int q = 0; q < P2P_S; ++q) v += red[(q * 4 + m) * PB_TG + tgt];
+        if (i < N) acc[((int64_t)slice * 4 + m) * N + i] = v;
     }
 }
 
@@ -483,8 +562,7 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed)
     if (timed) PB_CUDA(cudaEventRecord(ctx->ev[1], st));
     if (far) {
         k_p2m_leaf<<<(unsigned)t.n_leaves, 128, 0, st>>>(t.P, t.Nk, t.K, t.leaf_ids, t.c_first, t.c_last, t.c_ctr[0],
-                                                        t.c_ctr[1], t.c_ctr[2], t.sx[0], t.sx[1], t.sx[2], t.qV,
-                                                        t.qK[0], t.qK[1], t.qK[2], t.M);
+                                                        t.c_ctr[1], t.c_ctr[2], t.srec, t.M);
         PB_LAUNCH_CHECK();
         for (int g = (int)t.gen_start.size() - 2; g >= 0; --g) {
             int64_t c0 = t.gen_start[g], c1 = t.gen_start[g + 1];
@@ -520,9 +598,8 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed)
     {
         dim3 grid((unsigned)t.n_groups, (unsigned)t.nslice_p2p);
         PB_TRY(pb_prof_begin(ctx, 0));
-        k_p2p<<<grid, PB_TG, 0, st>>>(t.N, t.K, t.nslice_p2p, ctx->prm.kappa, t.p2p_off, t.p2p_lo, t.p2p_hi, t.sx[0],
-                                      t.sx[1], t.sx[2], t.qV, t.qK[0], t.qK[1], t.qK[2], t.pc[0], t.pc[1], t.pc[2],
-                                      t.accP);
+        k_p2p<<<grid, P2P_THREADS, 0, st>>>(t.N, t.K, t.nslice_p2p, ctx->prm.kappa, t.ek, t.p2p_off, t.p2p_lo, t.p2p_hi,
+                                            t.srec, t.pc[0], t.pc[1], t.pc[2], t.accP);
         PB_LAUNCH_CHECK();
         PB_TRY(pb_prof_end(ctx, 0));
         pb_prof_next(ctx);

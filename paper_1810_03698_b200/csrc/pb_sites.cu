@@ -95,9 +95,7 @@ __device__ __forceinline__ void react_point(double dx, double dy, double dz, dou
 #define RF_THREADS 128
 template <bool HESS>
 __global__ void __launch_bounds__(RF_THREADS)
-k_reaction(int64_t Ns, int64_t chunk, int64_t na, const double* __restrict__ pos, const double* __restrict__ sx,
-           const double* __restrict__ sy, const double* __restrict__ sz, const double* __restrict__ qV,
-           const double* __restrict__ qKx, const double* __restrict__ qKy, const double* __restrict__ qKz,
+k_reaction(int64_t Ns, int64_t chunk, int64_t na, const double* __restrict__ pos, const double4* __restrict__ srec,
            double* __restrict__ partial /*[gridDim.x][na][10]*/)
 {
     constexpr int NO = HESS ? 10 : 4;
@@ -114,7 +112,8 @@ k_reaction(int64_t Ns, int64_t chunk, int64_t na, const double* __restrict__ pos
     }
     const int64_t s0 = blockIdx.x * chunk, s1 = s0 + chunk < Ns ? s0 + chunk : Ns;
     for (int64_t s = s0 + threadIdx.x; s < s1; s += RF_THREADS) {
-        const double yx = sx[s], yy = sy[s], yz = sz[s], wS = qV[s], kx = qKx[s], ky = qKy[s], kz = qKz[s];
+        const double4 ra = srec[2 * s], rb = srec[2 * s + 1];
+        const double yx = ra.x, yy = ra.y, yz = ra.z, wS = ra.w, kx = rb.x, ky = rb.y, kz = rb.z;
 #pragma unroll
         for (int t = 0; t < RF_ST; ++t) react_point<HESS>(r[t][0] - yx, r[t][1] - yy, r[t][2] - yz, wS, kx, ky, kz, acc[t]);
     }
@@ -213,7 +212,7 @@ struct rf_corr_args {
     const double* pos;
     const double* pv[9];
     const double *nx, *ny, *nz, *parea, *xphi, *xdphi;
-    const double *sx, *sy, *sz, *qV, *qKx, *qKy, *qKz;
+    const double4* srec;
     double *phi, *grad, *hess;
 };
 
@@ -236,7 +235,8 @@ __global__ void k_reaction_corr(rf_corr_args a, pb_rule_t ruleN)
     }
     for (int g = 0; g < a.K; ++g) {
         const int64_t s = (int64_t)j * a.K + g;
-        react_point<true>(r[0] - a.sx[s], r[1] - a.sy[s], r[2] - a.sz[s], a.qV[s], a.qKx[s], a.qKy[s], a.qKz[s], coarse);
+        const double4 ra = a.srec[2 * s], rb = a.srec[2 * s + 1];
+        react_point<true>(r[0] - ra.x, r[1] - ra.y, r[2] - ra.z, ra.w, rb.x, rb.y, rb.z, coarse);
     }
     if (a.phi) atomicAdd(&a.phi[m], PB_INV4PI * (fine[0] - coarse[0]));
     if (a.grad)
@@ -270,11 +270,9 @@ extern "C" int pb_reaction_field(pb_ctx* ctx, const double* x, double* phi, doub
     dim3 grid((unsigned)nchunk, (unsigned)ntile);
     const bool H = hess != nullptr;
     if (H)
-        k_reaction<true><<<grid, RF_THREADS, 0, st>>>(t.Ns, chunk, s.na, s.pos, t.sx[0], t.sx[1], t.sx[2], t.qV, t.qK[0],
-                                                      t.qK[1], t.qK[2], partial);
+        k_reaction<true><<<grid, RF_THREADS, 0, st>>>(t.Ns, chunk, s.na, s.pos, t.srec, partial);
     else
-        k_reaction<false><<<grid, RF_THREADS, 0, st>>>(t.Ns, chunk, s.na, s.pos, t.sx[0], t.sx[1], t.sx[2], t.qV, t.qK[0],
-                                                       t.qK[1], t.qK[2], partial);
+        k_reaction<false><<<grid, RF_THREADS, 0, st>>>(t.Ns, chunk, s.na, s.pos, t.srec, partial);
     PB_LAUNCH_CHECK();
     const int NO = H ? 10 : 4;
     k_reaction_finish<<<pb_blocks(s.na * NO, 128), 128, 0, st>>>(s.na, (int)nchunk, NO, partial, phi, grad, hess);
@@ -284,7 +282,7 @@ extern "C" int pb_reaction_field(pb_ctx* ctx, const double* x, double* phi, doub
         a.np = s.n_near; a.K = t.K; a.psite = s.near_site; a.ppanel = s.near_panel; a.pos = s.pos;
         for (int k = 0; k < 9; ++k) a.pv[k] = t.pv[k];
         a.nx = t.pn[0]; a.ny = t.pn[1]; a.nz = t.pn[2]; a.parea = t.parea; a.xphi = t.xphi; a.xdphi = t.xdphi;
-        a.sx = t.sx[0]; a.sy = t.sx[1]; a.sz = t.sx[2]; a.qV = t.qV; a.qKx = t.qK[0]; a.qKy = t.qK[1]; a.qKz = t.qK[2];
+        a.srec = t.srec;
         a.phi = phi; a.grad = grad; a.hess = hess;
         k_reaction_corr<<<pb_blocks(s.n_near, 64), 64, 0, st>>>(a, ctx->ruleN);
         PB_LAUNCH_CHECK();

@@ -398,6 +398,7 @@ int pb_tree_build_impl(pb_ctx* ctx)
     t.N = N;
     t.K = K;
     t.Ns = N * K;
+    pb_make_expk(ctx->prm.kappa, &t.ek);
     const int64_t Ns = t.Ns;
 
     // --- Morton keys and sort
@@ -441,12 +442,11 @@ int pb_tree_build_impl(pb_ctx* ctx)
         PB_TRY(pb_dalloc_t(ctx, &t.pn[d], N, CAT_TREE));
         PB_TRY(pb_dalloc_t(ctx, &t.ptri[d], N, CAT_TREE));
         PB_TRY(pb_dalloc_t(ctx, &t.sx[d], Ns, CAT_TREE));
-        PB_TRY(pb_dalloc_t(ctx, &t.qK[d], Ns, CAT_TREE));
     }
     for (int k = 0; k < 9; ++k) PB_TRY(pb_dalloc_t(ctx, &t.pv[k], N, CAT_TREE));
     PB_TRY(pb_dalloc_t(ctx, &t.parea, N, CAT_TREE));
     PB_TRY(pb_dalloc_t(ctx, &t.swA, Ns, CAT_TREE));
-    PB_TRY(pb_dalloc_t(ctx, &t.qV, Ns, CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.srec, 2 * Ns, CAT_TREE));
     PB_TRY(pb_dalloc_t(ctx, &t.xphi, N, CAT_TREE));
     PB_TRY(pb_dalloc_t(ctx, &t.xdphi, N, CAT_TREE));
     {
@@ -573,8 +573,12 @@ int pb_tree_build_impl(pb_ctx* ctx)
         int ns = (int)((want + G - 1) / G);
         if (ns < 1) ns = 1;
         if (ns > 64) ns = 64;
-        t.nslice_p2p = ns;
         t.nslice_m2p = ns;
+        // P2P blocks hold 8 warps: 4 blocks per SM fill the schedulers
+        ns = (int)((148 * 4 + G - 1) / G);
+        if (ns < 1) ns = 1;
+        if (ns > 32) ns = 32;
+        t.nslice_p2p = ns;
         PB_TRY(pb_dalloc_t(ctx, &t.accP, (size_t)t.nslice_p2p * 4 * N, CAT_TREE));
         PB_TRY(pb_dalloc_t(ctx, &t.accM, (size_t)t.nslice_m2p * 4 * N, CAT_TREE));
     }
