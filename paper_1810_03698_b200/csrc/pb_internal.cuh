@@ -73,6 +73,15 @@ struct pb_tree {
     int P = 0, Nk = 0, NT = 0;
     double* M = nullptr;          // [cells][2][Nk] Cartesian moments (V, K)
     double2* FF = nullptr;        // [cells][NT] converted far-field terms {V, K}
+    int32_t* mm_off = nullptr;    // [Nk+1] M2M table (CSR over k): packed (l | dx<<12 | dy<<16 | dz<<20), binomials
+    int32_t* mm_ent = nullptr;
+    double* mm_coef = nullptr;
+    int64_t m2p_total = 0;        // entries of m2p_cell
+    int64_t n_used = 0, n_need_leaf = 0;
+    int32_t* used_cells = nullptr;   // cells that appear in an M2P list (get F terms)
+    int32_t* need_leaf = nullptr;    // leaves whose moments are needed (P2M)
+    int32_t* m2m_cells = nullptr;    // internal cells whose moments are needed, by generation
+    std::vector<int64_t> m2m_start;  // m2m_cells[m2m_start[g] .. m2m_start[g+1]) = generation g
     int32_t* cv_off = nullptr;    // [NT+1] conversion table (CSR over source moment indices)
     int32_t* cv_idx = nullptr;
     double* cv_coef = nullptr;

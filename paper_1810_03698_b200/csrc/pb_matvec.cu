@@ -34,7 +34,6 @@ __host__ __device__ static constexpr int pb_nt(int P)
 
 #define PB_MAX_NK 286   // pb_nk(10)
 __constant__ unsigned char c_ka[PB_MAX_NK], c_kb[PB_MAX_NK], c_kc[PB_MAX_NK];
-__constant__ double c_binom[PB_MAX_P + 1][PB_MAX_P + 1];
 
 static double factorial(int n) { double f = 1; for (int i = 2; i <= n; ++i) f *= i; return f; }
 
@@ -93,13 +92,9 @@ int pb_farfield_setup(pb_ctx* ctx)
                 int k = mom_index(a, b, c);
                 ka[k] = (unsigned char)a; kb[k] = (unsigned char)b; kc[k] = (unsigned char)c;
             }
-    double binom[PB_MAX_P + 1][PB_MAX_P + 1];
-    for (int n = 0; n <= PB_MAX_P; ++n)
-        for (int k = 0; k <= PB_MAX_P; ++k) binom[n][k] = k <= n ? factorial(n) / (factorial(k) * factorial(n - k)) : 0.0;
     PB_CUDA(cudaMemcpyToSymbolAsync(c_ka, ka, t.Nk, 0, cudaMemcpyHostToDevice, st));
     PB_CUDA(cudaMemcpyToSymbolAsync(c_kb, kb, t.Nk, 0, cudaMemcpyHostToDevice, st));
     PB_CUDA(cudaMemcpyToSymbolAsync(c_kc, kc, t.Nk, 0, cudaMemcpyHostToDevice, st));
-    PB_CUDA(cudaMemcpyToSymbolAsync(c_binom, binom, sizeof(binom), 0, cudaMemcpyHostToDevice, st));
     // conversion table M -> F, entries in the order the M2P kernel consumes them
     std::vector<int32_t> off, idx, expo;
     std::vector<double> coef;
@@ -111,7 +106,65 @@ int pb_farfield_setup(pb_ctx* ctx)
     PB_CUDA(cudaMemcpyAsync(t.cv_off, off.data(), sizeof(int32_t) * off.size(), cudaMemcpyHostToDevice, st));
     PB_CUDA(cudaMemcpyAsync(t.cv_idx, idx.data(), sizeof(int32_t) * idx.size(), cudaMemcpyHostToDevice, st));
     PB_CUDA(cudaMemcpyAsync(t.cv_coef, coef.data(), sizeof(double) * coef.size(), cudaMemcpyHostToDevice, st));
-    PB_CUDA(cudaStreamSynchronize(st));   // host vectors go out of scope
+    // M2M table: for every k the triples (l, k - l, C(k,l)), l <= k componentwise
+    std::vector<int32_t> mo(1, 0), me;
+    std::vector<double> mc;
+    for (int k = 0; k < t.Nk; ++k) {
+        const int a = ka[k], b = kb[k], c = kc[k];
+        for (int la = 0; la <= a; ++la)
+            for (int lb = 0; lb <= b; ++lb)
+                for (int lc = 0; lc <= c; ++lc) {
+                    me.push_back(mom_index(la, lb, lc) | ((a - la) << 12) | ((b - lb) << 16) | ((c - lc) << 20));
+                    mc.push_back(factorial(a) / (factorial(la) * factorial(a - la)) * factorial(b) /
+                                 (factorial(lb) * factorial(b - lb)) * factorial(c) / (factorial(lc) * factorial(c - lc)));
+                }
+        mo.push_back((int32_t)me.size());
+    }
+    PB_TRY(pb_dalloc_t(ctx, &t.mm_off, mo.size(), CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.mm_ent, me.size(), CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.mm_coef, mc.size(), CAT_TREE));
+    PB_CUDA(cudaMemcpyAsync(t.mm_off, mo.data(), sizeof(int32_t) * mo.size(), cudaMemcpyHostToDevice, st));
+    PB_CUDA(cudaMemcpyAsync(t.mm_ent, me.data(), sizeof(int32_t) * me.size(), cudaMemcpyHostToDevice, st));
+    PB_CUDA(cudaMemcpyAsync(t.mm_coef, mc.data(), sizeof(double) * mc.size(), cudaMemcpyHostToDevice, st));
+
+    // Which cells need moments: the ones in some M2P list ("used") and every descendant of a used
+    // cell (M2M builds a parent from ALL its children).  Bookkeeping on the host, once per tree.
+    const int64_t nc = t.n_cells;
+    std::vector<int32_t> child(nc), nchild(nc), lists(t.m2p_total > 0 ? t.m2p_total : 1);
+    PB_CUDA(cudaMemcpyAsync(child.data(), t.c_child, sizeof(int32_t) * nc, cudaMemcpyDeviceToHost, st));
+    PB_CUDA(cudaMemcpyAsync(nchild.data(), t.c_nchild, sizeof(int32_t) * nc, cudaMemcpyDeviceToHost, st));
+    if (t.m2p_total > 0)
+        PB_CUDA(cudaMemcpyAsync(lists.data(), t.m2p_cell, sizeof(int32_t) * t.m2p_total, cudaMemcpyDeviceToHost, st));
+    PB_CUDA(cudaStreamSynchronize(st));   // also: the host vectors above go out of scope
+    std::vector<char> used(nc, 0), need(nc, 0);
+    for (int64_t e = 0; e < t.m2p_total; ++e) used[lists[e]] = 1;
+    std::vector<int32_t> used_list, leaf_list, m2m_list;
+    t.m2m_start.assign(1, 0);
+    for (size_t g = 0; g + 1 < t.gen_start.size(); ++g) {     // cells are numbered generation by generation
+        for (int64_t c = t.gen_start[g]; c < t.gen_start[g + 1]; ++c) {
+            need[c] = need[c] || used[c];
+            if (used[c]) used_list.push_back((int32_t)c);
+            if (!need[c]) continue;
+            if (child[c] < 0) leaf_list.push_back((int32_t)c);
+            else {
+                m2m_list.push_back((int32_t)c);
+                for (int q = 0; q < nchild[c]; ++q) need[child[c] + q] = 1;
+            }
+        }
+        t.m2m_start.push_back((int64_t)m2m_list.size());
+    }
+    t.n_used = (int64_t)used_list.size();
+    t.n_need_leaf = (int64_t)leaf_list.size();
+    PB_TRY(pb_dalloc_t(ctx, &t.used_cells, used_list.size(), CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.need_leaf, leaf_list.size(), CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.m2m_cells, m2m_list.size(), CAT_TREE));
+    if (!used_list.empty())
+        PB_CUDA(cudaMemcpyAsync(t.used_cells, used_list.data(), sizeof(int32_t) * used_list.size(), cudaMemcpyHostToDevice, st));
+    if (!leaf_list.empty())
+        PB_CUDA(cudaMemcpyAsync(t.need_leaf, leaf_list.data(), sizeof(int32_t) * leaf_list.size(), cudaMemcpyHostToDevice, st));
+    if (!m2m_list.empty())
+        PB_CUDA(cudaMemcpyAsync(t.m2m_cells, m2m_list.data(), sizeof(int32_t) * m2m_list.size(), cudaMemcpyHostToDevice, st));
+    PB_CUDA(cudaStreamSynchronize(st));
     PB_TRY(pb_dalloc_t(ctx, &t.M, (size_t)t.n_cells * 2 * t.Nk, CAT_TREE));
     PB_TRY(pb_dalloc_t(ctx, &t.FF, (size_t)t.n_cells * t.NT, CAT_TREE));
     return PB_OK;
@@ -218,16 +271,19 @@ k_p2m_leaf(int P, int Nk, int K, const int32_t* __restrict__ leaf_ids, const int
 }
 
 // ---- M2M: moments of a parent from its children, M'_k = sum_{l<=k} C(k,l) t^{k-l} M_l -------------
+// Table driven: for every k the (l, k-l, C(k,l)) triples are listed once on the host (mm_*), so a
+// thread does no index arithmetic.  Only cells some M2P list needs (directly or through an accepted
+// ancestor) are visited: `cells` is the compacted list for one BFS generation.
 __global__ void __launch_bounds__(128)
-k_m2m(int64_t c0, int P, int Nk, const int32_t* __restrict__ c_child, const int32_t* __restrict__ c_nchild,
-      const double* __restrict__ cx, const double* __restrict__ cy, const double* __restrict__ cz,
-      double* __restrict__ M)
+k_m2m(const int32_t* __restrict__ cells, int P, int Nk, const int32_t* __restrict__ c_child,
+      const int32_t* __restrict__ c_nchild, const double* __restrict__ cx, const double* __restrict__ cy,
+      const double* __restrict__ cz, const int32_t* __restrict__ mm_off, const int32_t* __restrict__ mm_ent,
+      const double* __restrict__ mm_coef, double* __restrict__ M)
 {
     __shared__ double cm[2][PB_MAX_NK];
     __shared__ double tp[3][PB_MAX_P + 1];
-    const int64_t c = c0 + blockIdx.x;
+    const int64_t c = cells[blockIdx.x];
     const int32_t ch = c_child[c];
-    if (ch < 0) return;
     const int nc = c_nchild[c];
     double acc[2][3] = {{0, 0, 0}, {0, 0, 0}};
     for (int q = 0; q < nc; ++q) {
@@ -240,44 +296,42 @@ k_m2m(int64_t c0, int P, int Nk, const int32_t* __restrict__ c_child, const int3
             for (int e = 0; e <= P; ++e) { tp[threadIdx.x][e] = p; p *= tt; }
         }
         __syncthreads();
+#pragma unroll
         for (int r = 0; r < 3; ++r) {
-            int k = threadIdx.x + r * 128;
-            if (k >= Nk) break;
-            int a = c_ka[k], b = c_kb[k], c3 = c_kc[k];
-            double s0 = 0, s1 = 0;
-            for (int la = 0; la <= a; ++la) {
-                double fa = c_binom[a][la] * tp[0][a - la];
-                for (int lb = 0; lb <= b; ++lb) {
-                    double fb = fa * c_binom[b][lb] * tp[1][b - lb];
-                    for (int lc = 0; lc <= c3; ++lc) {
-                        double f = fb * c_binom[c3][lc] * tp[2][c3 - lc];
-                        int l = mom_index(la, lb, lc);
-                        s0 += f * cm[0][l];
-                        s1 += f * cm[1][l];
-                    }
+            const int k = threadIdx.x + r * 128;
+            if (k < Nk) {
+                double s0 = 0, s1 = 0;
+                for (int e = mm_off[k]; e < mm_off[k + 1]; ++e) {
+                    const int32_t ent = mm_ent[e];
+                    const double f = mm_coef[e] * tp[0][(ent >> 12) & 15] * tp[1][(ent >> 16) & 15] * tp[2][(ent >> 20) & 15];
+                    const int l = ent & 0xfff;
+                    s0 = fma(f, cm[0][l], s0);
+                    s1 = fma(f, cm[1][l], s1);
                 }
+                acc[0][r] += s0;
+                acc[1][r] += s1;
             }
-            acc[0][r] += s0;
-            acc[1][r] += s1;
         }
     }
+#pragma unroll
     for (int r = 0; r < 3; ++r) {
-        int k = threadIdx.x + r * 128;
-        if (k >= Nk) break;
-        M[(c * 2 + 0) * Nk + k] = acc[0][r];
-        M[(c * 2 + 1) * Nk + k] = acc[1][r];
+        const int k = threadIdx.x + r * 128;
+        if (k < Nk) {
+            M[(c * 2 + 0) * Nk + k] = acc[0][r];
+            M[(c * 2 + 1) * Nk + k] = acc[1][r];
+        }
     }
 }
 
-// ---- M -> F conversion ---------------------------------------------------------------------------------
-__global__ void k_convert(int64_t ncell, int Nk, int NT, const int32_t* __restrict__ cv_off,
-                          const int32_t* __restrict__ cv_idx, const double* __restrict__ cv_coef,
-                          const double* __restrict__ M, double2* __restrict__ FF)
+// ---- M -> F conversion (cells that appear in an M2P list only) ---------------------------------------
+__global__ void k_convert(int64_t nused, const int32_t* __restrict__ used, int Nk, int NT,
+                          const int32_t* __restrict__ cv_off, const int32_t* __restrict__ cv_idx,
+                          const double* __restrict__ cv_coef, const double* __restrict__ M, double2* __restrict__ FF)
 {
     int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (g >= ncell * NT) return;
-    int64_t c = g / NT;
-    int e = (int)(g - c * NT);
+    if (g >= nused * NT) return;
+    const int64_t c = used[g / NT];
+    const int e = (int)(g % NT);
     const double* mv = M + c * 2 * Nk;
     const double* mk = mv + Nk;
     double v = 0, k = 0;
@@ -287,7 +341,7 @@ __global__ void k_convert(int64_t ncell, int Nk, int NT, const int32_t* __restri
         v += f * mv[l];
         k += f * mk[l];
     }
-    FF[g] = make_double2(v, k);
+    FF[c * NT + e] = make_double2(v, k);
 }
 
 // ---- M2P (H6; "box-target" interactions) -----------------------------------------------------------
@@ -561,18 +615,23 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed)
     PB_TRY(pb_weights(ctx, x));
     if (timed) PB_CUDA(cudaEventRecord(ctx->ev[1], st));
     if (far) {
-        k_p2m_leaf<<<(unsigned)t.n_leaves, 128, 0, st>>>(t.P, t.Nk, t.K, t.leaf_ids, t.c_first, t.c_last, t.c_ctr[0],
-                                                        t.c_ctr[1], t.c_ctr[2], t.srec, t.M);
-        PB_LAUNCH_CHECK();
-        for (int g = (int)t.gen_start.size() - 2; g >= 0; --g) {
-            int64_t c0 = t.gen_start[g], c1 = t.gen_start[g + 1];
-            k_m2m<<<(unsigned)(c1 - c0), 128, 0, st>>>(c0, t.P, t.Nk, t.c_child, t.c_nchild, t.c_ctr[0], t.c_ctr[1],
-                                                      t.c_ctr[2], t.M);
+        if (t.n_need_leaf > 0) {
+            k_p2m_leaf<<<(unsigned)t.n_need_leaf, 128, 0, st>>>(t.P, t.Nk, t.K, t.need_leaf, t.c_first, t.c_last, t.c_ctr[0],
+                                                               t.c_ctr[1], t.c_ctr[2], t.srec, t.M);
             PB_LAUNCH_CHECK();
         }
-        k_convert<<<pb_blocks(t.n_cells * t.NT, 256), 256, 0, st>>>(t.n_cells, t.Nk, t.NT, t.cv_off, t.cv_idx, t.cv_coef,
-                                                                   t.M, t.FF);
-        PB_LAUNCH_CHECK();
+        for (int g = (int)t.m2m_start.size() - 2; g >= 0; --g) {   // deepest generation first
+            const int64_t n = t.m2m_start[g + 1] - t.m2m_start[g];
+            if (n == 0) continue;
+            k_m2m<<<(unsigned)n, 128, 0, st>>>(t.m2m_cells + t.m2m_start[g], t.P, t.Nk, t.c_child, t.c_nchild, t.c_ctr[0],
+                                               t.c_ctr[1], t.c_ctr[2], t.mm_off, t.mm_ent, t.mm_coef, t.M);
+            PB_LAUNCH_CHECK();
+        }
+        if (t.n_used > 0) {
+            k_convert<<<pb_blocks(t.n_used * t.NT, 256), 256, 0, st>>>(t.n_used, t.used_cells, t.Nk, t.NT, t.cv_off, t.cv_idx,
+                                                                      t.cv_coef, t.M, t.FF);
+            PB_LAUNCH_CHECK();
+        }
     }
     if (timed) PB_CUDA(cudaEventRecord(ctx->ev[2], st));
     if (far) {

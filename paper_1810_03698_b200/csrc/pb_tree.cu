@@ -560,6 +560,7 @@ int pb_tree_build_impl(pb_ctx* ctx)
     PB_TRY(pb_exclusive_scan_i32(ctx, cnt_p, t.p2p_off, G + 1, &tot_p));
     t.p2p_pairs = (int64_t)hpc[0];
     t.m2p_pairs = (int64_t)hpc[1];
+    t.m2p_total = tot_m;
     PB_TRY(pb_dalloc_t(ctx, &t.m2p_cell, tot_m, CAT_TREE));
     PB_TRY(pb_dalloc_t(ctx, &t.p2p_lo, tot_p, CAT_TREE));
     PB_TRY(pb_dalloc_t(ctx, &t.p2p_hi, tot_p, CAT_TREE));
