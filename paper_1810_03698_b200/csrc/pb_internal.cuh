@@ -24,6 +24,11 @@ enum pb_mem_cat { CAT_MESH = 0, CAT_SITES = 1, CAT_TREE = 2, CAT_SOLVE = 3, CAT_
 struct pb_rule_t { int K; double lam[19][3]; double w[19]; };
 struct pb_gl_t { int n; double x[64]; double w[64]; };
 
+// One thread block's share of a target group's P2P or M2P list (pb_tree.cu).
+// P2P: r = index of the first source range, a = first source point, count = source points.
+// M2P: r = index of the first list entry (cell), count = cells.
+struct __align__(16) pb_item { int32_t group, slot, r, a; int32_t count, pad; };
+
 struct pb_allocation { void* ptr; size_t bytes; int cat; };
 
 // Source-point and panel arrays in MORTON order (built by pb_tree_build).
@@ -65,6 +70,7 @@ struct pb_tree {
     // lists (CSR per group)
     int32_t* m2p_off = nullptr;   // [groups+1]
     int32_t* m2p_cell = nullptr;
+    double4* m2p_ctr = nullptr;   // [entries] centre of m2p_cell[e] (one contiguous TMA copy per tile of cells)
     int32_t* p2p_off = nullptr;   // [groups+1]
     int32_t* p2p_lo = nullptr;    // source-point ranges [lo, hi)
     int32_t* p2p_hi = nullptr;
@@ -92,9 +98,15 @@ struct pb_tree {
     double* nr_val = nullptr;     // [4][entries] VL, KL, VY, KY corrections
     double* precond = nullptr;    // [N][4] inverse 2x2 diagonal blocks
     // partial accumulators
-    int nslice_p2p = 1, nslice_m2p = 1;
-    double* accP = nullptr;       // [nslice_p2p][4][N]
-    double* accM = nullptr;       // [nslice_m2p][4][N]
+    // work items (one thread block each) and their accumulator slots
+    pb_item* itemP = nullptr;     // [n_itemP]
+    pb_item* itemM = nullptr;     // [n_itemM]
+    int32_t* itemP_off = nullptr; // [groups+1]: group g owns items/slots itemP_off[g] .. itemP_off[g+1]
+    int32_t* itemM_off = nullptr;
+    int64_t n_itemP = 0, n_itemM = 0;
+    int nslot_p2p = 1, nslot_m2p = 1;   // largest number of items of one group
+    double* accP = nullptr;       // [nslot_p2p][4][N]
+    double* accM = nullptr;       // [nslot_m2p][4][N]
 };
 
 struct pb_sites {

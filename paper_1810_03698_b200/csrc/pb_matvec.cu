@@ -375,55 +375,125 @@ __device__ __forceinline__ void m2p_terms(const double2* __restrict__ ff, double
     }
 }
 
-// One block per (target group, list slice); one target per thread.  The cell's F terms are
-// staged in shared memory and read as broadcast 16-byte loads.
+// One block = one work item: a target group (PB_TG targets) x a run of its accepted cells.  The
+// cells' F terms (N_T x {V,K}, contiguous per cell) and centres arrive in shared memory by TMA bulk
+// copies, CT cells per stage, two stages; the block's M2P_S sub-slices (2 warps each) take different
+// cells of a stage for the same targets, so all shared-memory reads are warp-wide broadcasts.
+#define M2P_S 4
+#define M2P_THREADS (PB_TG * M2P_S)
+static_assert(M2P_S == 4, "the final reduction maps one of the 4 outputs to each sub-slice");
+
+template <int P> struct m2p_cfg {
+    static constexpr int NT = pb_nt(P);
+    static constexpr int CT = P <= 6 ? 8 : 4;                    // cells per stage
+    static constexpr size_t RED_BYTES = (size_t)M2P_S * 4 * PB_TG * sizeof(double);   // final reduction reuses the stages
+    static constexpr size_t FF_BYTES0 = (size_t)2 * CT * NT * sizeof(double2);
+    static constexpr size_t FF_BYTES = FF_BYTES0 > RED_BYTES ? FF_BYTES0 : RED_BYTES;
+    static constexpr size_t SMEM = FF_BYTES + 2 * CT * sizeof(double4) + 2 * sizeof(uint64_t) + 32 * sizeof(double);
+};
+
 template <int P>
-__global__ void __launch_bounds__(PB_TG)
-k_m2p(int64_t N, int nslice, double kappa, const int32_t* __restrict__ m2p_off, const int32_t* __restrict__ m2p_cell,
-      const double* __restrict__ cx, const double* __restrict__ cy, const double* __restrict__ cz,
-      const double2* __restrict__ FF, const double* __restrict__ px, const double* __restrict__ py,
-      const double* __restrict__ pz, double* __restrict__ acc)
+__global__ void __launch_bounds__(M2P_THREADS)
+k_m2p(int64_t N, double kappa, pb_expk ek, const pb_item* __restrict__ items, const int32_t* __restrict__ m2p_cell,
+      const double4* __restrict__ m2p_ctr, const double2* __restrict__ FF, const double* __restrict__ px,
+      const double* __restrict__ py, const double* __restrict__ pz, double* __restrict__ acc)
 {
-    constexpr int NT = pb_nt(P);
-    __shared__ double2 ff[NT];
-    __shared__ double ctr[3];
-    const int64_t g = blockIdx.x;
-    const int slice = blockIdx.y;
-    const int64_t i = g * PB_TG + threadIdx.x;
-    const bool live = i < N;
-    const double tx = live ? px[i] : 0.0, ty = live ? py[i] : 0.0, tz = live ? pz[i] : 0.0;
+    constexpr int NT = m2p_cfg<P>::NT, CT = m2p_cfg<P>::CT;
+    extern __shared__ __align__(128) unsigned char smraw[];
+    double2* ff = reinterpret_cast<double2*>(smraw);                                  // [2][CT][NT]
+    double4* ctr = reinterpret_cast<double4*>(smraw + m2p_cfg<P>::FF_BYTES);           // [2][CT]
+    uint64_t* bar = reinterpret_cast<uint64_t*>(ctr + 2 * CT);                         // [2]
+    double* Ts = reinterpret_cast<double*>(bar + 2);                                   // [32]
+    const int tid = threadIdx.x;
+    const int tgt = tid & (PB_TG - 1), sub = tid / PB_TG;
+    const pb_item item = items[blockIdx.x];
+    const int64_t g = item.group;
+    const int32_t e0 = item.r, count = item.count;
+    if (tid < 32) Ts[tid] = ek.T[tid];
+    if (tid == 0) {
+        pb_mbar_init(&bar[0], 1);
+        pb_mbar_init(&bar[1], 1);
+        pb_mbar_fence_init();
+    }
+    __syncthreads();
+    const int64_t i = g * PB_TG + tgt;
+    const int64_t ic = i < N ? i : N - 1;
+    const double tx = px[ic], ty = py[ic], tz = pz[ic];
+    const int ntile = (count + CT - 1) / CT;
+
+    // thread 0 is the producer: cell ids are fetched one tile ahead of the copies that need them
+    int32_t idn[CT];
+    auto load_ids = [&](int t) {
+#pragma unroll
+        for (int j = 0; j < CT; ++j) {
+            const int32_t e = t * CT + j;
+            idn[j] = e < count ? m2p_cell[e0 + e] : 0;
+        }
+    };
+    auto issue = [&](int t, int stage) {
+        const int n = count - t * CT < CT ? count - t * CT : CT;
+        pb_mbar_expect_tx(&bar[stage], (uint32_t)(n * (sizeof(double4) + NT * sizeof(double2))));
+        pb_bulk_g2s(ctr + stage * CT, m2p_ctr + e0 + t * CT, (uint32_t)(n * sizeof(double4)), &bar[stage]);
+#pragma unroll
+        for (int j = 0; j < CT; ++j)
+            if (j < n)
+                pb_bulk_g2s(ff + ((size_t)stage * CT + j) * NT, FF + (int64_t)idn[j] * NT, (uint32_t)(NT * sizeof(double2)),
+                            &bar[stage]);
+    };
+    if (tid == 0 && ntile > 0) {
+        load_ids(0);
+        issue(0, 0);
+        if (ntile > 1) load_ids(1);
+    }
     double VL = 0, KL = 0, VY = 0, KY = 0;
     const double k2 = kappa * kappa;
-    for (int32_t e = m2p_off[g] + slice; e < m2p_off[g + 1]; e += nslice) {
-        const int32_t c = m2p_cell[e];
-        __syncthreads();
-        for (int q = threadIdx.x; q < NT; q += PB_TG) ff[q] = FF[(int64_t)c * NT + q];
-        if (threadIdx.x == 0) { ctr[0] = cx[c]; ctr[1] = cy[c]; ctr[2] = cz[c]; }
-        __syncthreads();
-        const double dx = tx - ctr[0], dy = ty - ctr[1], dz = tz - ctr[2];
-        double WV[P + 1], WK[P + 1];
-#pragma unroll
-        for (int m = 0; m <= P; ++m) { WV[m] = 0.0; WK[m] = 0.0; }
-        m2p_terms<P>(ff, dx, dy, dz, WV, WK);
-        const double R2 = dx * dx + dy * dy + dz * dz;
-        const double ri = rsqrt(R2), R = R2 * ri, ri2 = ri * ri;
-        const double ex = exp(-kappa * R);
-        double uL = ri, uY0 = ex * ri, uY1 = ex * (1.0 + kappa * R) * ri * ri2;
-        VL = fma(uL, WV[0], VL); KL = fma(uL, WK[0], KL);
-        VY = fma(uY0, WV[0], VY); KY = fma(uY0, WK[0], KY);
-#pragma unroll
-        for (int m = 1; m <= P; ++m) {
-            uL = (2 * m - 1) * uL * ri2;
-            VL = fma(uL, WV[m], VL); KL = fma(uL, WK[m], KL);
-            VY = fma(uY1, WV[m], VY); KY = fma(uY1, WK[m], KY);
-            const double un = ((2 * m + 1) * uY1 + k2 * uY0) * ri2;
-            uY0 = uY1;
-            uY1 = un;
+    for (int t = 0; t < ntile; ++t) {
+        const int st = t & 1;
+        if (tid == 0 && t + 1 < ntile) {              // the other stage was released by the barrier below
+            issue(t + 1, st ^ 1);
+            if (t + 2 < ntile) load_ids(t + 2);
         }
+        pb_mbar_wait(&bar[st], (t >> 1) & 1u);
+        const int cnt = count - t * CT < CT ? count - t * CT : CT;
+#pragma unroll 1
+        for (int j = sub; j < cnt; j += M2P_S) {
+            const double4 cc = ctr[st * CT + j];
+            const double dx = tx - cc.x, dy = ty - cc.y, dz = tz - cc.z;
+            double WV[P + 1], WK[P + 1];
+#pragma unroll
+            for (int m = 0; m <= P; ++m) { WV[m] = 0.0; WK[m] = 0.0; }
+            m2p_terms<P>(ff + ((size_t)st * CT + j) * NT, dx, dy, dz, WV, WK);
+            const double R2 = dx * dx + dy * dy + dz * dz;
+            const double ri = pb_rsqrt(R2), R = R2 * ri, ri2 = ri * ri;
+            const double ex = pb_exp_mkr(R, ek, Ts);
+            double uL = ri, uY0 = ex * ri, uY1 = ex * fma(kappa, R, 1.0) * ri * ri2;
+            VL = fma(uL, WV[0], VL); KL = fma(uL, WK[0], KL);
+            VY = fma(uY0, WV[0], VY); KY = fma(uY0, WK[0], KY);
+#pragma unroll
+            for (int m = 1; m <= P; ++m) {
+                uL = (2 * m - 1) * uL * ri2;
+                VL = fma(uL, WV[m], VL); KL = fma(uL, WK[m], KL);
+                VY = fma(uY1, WV[m], VY); KY = fma(uY1, WK[m], KY);
+                const double un = ((2 * m + 1) * uY1 + k2 * uY0) * ri2;
+                uY0 = uY1;
+                uY1 = un;
+            }
+        }
+        __syncthreads();
     }
-    if (live) {
-        double* a = acc + (int64_t)slice * 4 * N;
-        a[i] = VL; a[N + i] = KL; a[2 * N + i] = VY; a[3 * N + i] = KY;
+    // add the sub-slices in a fixed order (the stages are free: every thread passed the last barrier)
+    double* red = reinterpret_cast<double*>(smraw);   // [M2P_S][4][PB_TG]
+    red[(sub * 4 + 0) * PB_TG + tgt] = VL;
+    red[(sub * 4 + 1) * PB_TG + tgt] = KL;
+    red[(sub * 4 + 2) * PB_TG + tgt] = VY;
+    red[(sub * 4 + 3) * PB_TG + tgt] = KY;
+    __syncthreads();
+    {
+        const int m = tid / PB_TG;
+        double v = 0;
+#pragma unroll
+        for (int q = 0; q < M2P_S; ++q) v += red[(q * 4 + m) * PB_TG + tgt];
+        if (i < N) acc[((int64_t)item.slot * 4 + m) * N + i] = v;
     }
 }
 
@@ -467,7 +537,7 @@ __device__ __forceinline__ void p2p_tile(const double4* __restrict__ buf, int cn
 }
 
 __global__ void __launch_bounds__(P2P_THREADS)
-k_p2p(int64_t N, int K, int nslice, double kappa, pb_expk ek, const int32_t* __restrict__ p2p_off,
+k_p2p(int64_t N, int K, double kappa, pb_expk ek, const pb_item* __restrict__ items,
       const int32_t* __restrict__ p2p_lo, const int32_t* __restrict__ p2p_hi, const double4* __restrict__ srec,
       const double* __restrict__ px, const double* __restrict__ py, const double* __restrict__ pz,
       double* __restrict__ acc)
@@ -477,8 +547,9 @@ k_p2p(int64_t N, int K, int nslice, double kappa, pb_expk ek, const int32_t* __r
     __shared__ double Ts[32];
     const int tid = threadIdx.x;
     const int tgt = tid & (PB_TG - 1), sub = tid / PB_TG;
-    const int64_t g = blockIdx.x;
-    const int slice = blockIdx.y;
+    const pb_item item = items[blockIdx.x];
+    const int64_t g = item.group;
+    const int slice = item.slot;
     if (tid < 32) Ts[tid] = ek.T[tid];
     if (tid == 0) {
         pb_mbar_init(&bar[0], 1);
@@ -493,23 +564,13 @@ k_p2p(int64_t N, int K, int nslice, double kappa, pb_expk ek, const int32_t* __r
     const int64_t i1 = (g + 1) * PB_TG < N ? (g + 1) * PB_TG : N;
     const int32_t grpLo = (int32_t)(g * PB_TG * K), grpHi = (int32_t)(i1 * K);
 
-    // this slice's share of the group's source list: [begin, begin + remaining) of the concatenated ranges
-    int32_t r = p2p_off[g];
-    const int32_t rend = p2p_off[g + 1];
-    int64_t total = 0;
-    for (int32_t q = r; q < rend; ++q) total += p2p_hi[q] - p2p_lo[q];
-    int64_t begin = total * slice / nslice;
-    int64_t remaining = total * (slice + 1) / nslice - begin;
-    int32_t a = r < rend ? p2p_lo[r] : 0;
-    while (r < rend && begin > 0) {                  // skip `begin` sources
-        const int32_t len = p2p_hi[r] - a;
-        if (begin < len) { a += (int32_t)begin; begin = 0; }
-        else { begin -= len; ++r; if (r < rend) a = p2p_lo[r]; }
-    }
+    // this item's share of the group's source list: `count` points from point `a` of range `r` on
+    int32_t r = item.r, a = item.a;
+    int32_t hi = p2p_hi[r];
+    int64_t remaining = item.count;
     auto next_tile = [&](int32_t& s0, int& cnt) -> bool {
-        while (remaining > 0 && r < rend) {
-            const int32_t hi = p2p_hi[r];
-            if (a >= hi) { ++r; if (r < rend) a = p2p_lo[r]; continue; }
+        while (remaining > 0) {
+            if (a >= hi) { ++r; a = p2p_lo[r]; hi = p2p_hi[r]; continue; }
             int64_t c = hi - a;
             if (c > P2P_TILE) c = P2P_TILE;
             if (c > remaining) c = remaining;
@@ -562,7 +623,8 @@ k_p2p(int64_t N, int K, int nslice, double kappa, pb_expk ek, const int32_t* __r
 }
 
 // ---- near/singular table + Eq. (5) combine + un-permute (H8) ------------------------------------------------
-__global__ void k_combine(int64_t N, int nsP, int nsM, double eps_ratio, const double* __restrict__ accP,
+__global__ void k_combine(int64_t N, const int32_t* __restrict__ itemP_off, const int32_t* __restrict__ itemM_off,
+                          double eps_ratio, const double* __restrict__ accP,
                           const double* __restrict__ accM, const int32_t* __restrict__ nr_off,
                           const int32_t* __restrict__ nr_col, const double* __restrict__ nr_val, int64_t ne,
                           const double* __restrict__ xphi, const double* __restrict__ xdphi,
@@ -571,6 +633,9 @@ __global__ void k_combine(int64_t N, int nsP, int nsM, double eps_ratio, const d
     int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (i >= N) return;
     double s[4] = {0, 0, 0, 0};
+    const int64_t g = i / PB_TG;
+    const int nsP = itemP_off[g + 1] - itemP_off[g];
+    const int nsM = itemM_off ? itemM_off[g + 1] - itemM_off[g] : 0;
     for (int q = 0; q < nsP; ++q)
         for (int m = 0; m < 4; ++m) s[m] += accP[((int64_t)q * 4 + m) * N + i];
     for (int q = 0; q < nsM; ++q)
@@ -592,12 +657,18 @@ __global__ void k_combine(int64_t N, int nsP, int nsM, double eps_ratio, const d
 
 // ---- host driver ----------------------------------------------------------------------------------------------
 template <int P>
-static void launch_m2p(pb_ctx* ctx)
+static cudaError_t launch_m2p(pb_ctx* ctx)
 {
     pb_tree& t = ctx->tree;
-    dim3 grid((unsigned)t.n_groups, (unsigned)t.nslice_m2p);
-    k_m2p<P><<<grid, PB_TG, 0, ctx->stream>>>(t.N, t.nslice_m2p, ctx->prm.kappa, t.m2p_off, t.m2p_cell, t.c_ctr[0],
-                                            t.c_ctr[1], t.c_ctr[2], t.FF, t.pc[0], t.pc[1], t.pc[2], t.accM);
+    static bool attr_set = false;   // per instantiation; the attribute belongs to the function, not the context
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(k_m2p<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m2p_cfg<P>::SMEM);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    k_m2p<P><<<(unsigned)t.n_itemM, M2P_THREADS, m2p_cfg<P>::SMEM, ctx->stream>>>(
+        t.N, ctx->prm.kappa, t.ek, t.itemM, t.m2p_cell, t.m2p_ctr, t.FF, t.pc[0], t.pc[1], t.pc[2], t.accM);
+    return cudaSuccess;
 }
 
 int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed)
@@ -634,20 +705,20 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed)
         }
     }
     if (timed) PB_CUDA(cudaEventRecord(ctx->ev[2], st));
-    if (far) {
+    if (far && t.n_itemM > 0) {
         PB_TRY(pb_prof_begin(ctx, 1));
         switch (t.P) {
-        case 0: launch_m2p<0>(ctx); break;
-        case 1: launch_m2p<1>(ctx); break;
-        case 2: launch_m2p<2>(ctx); break;
-        case 3: launch_m2p<3>(ctx); break;
-        case 4: launch_m2p<4>(ctx); break;
-        case 5: launch_m2p<5>(ctx); break;
-        case 6: launch_m2p<6>(ctx); break;
-        case 7: launch_m2p<7>(ctx); break;
-        case 8: launch_m2p<8>(ctx); break;
-        case 9: launch_m2p<9>(ctx); break;
-        case 10: launch_m2p<10>(ctx); break;
+        case 0: PB_CUDA(launch_m2p<0>(ctx)); break;
+        case 1: PB_CUDA(launch_m2p<1>(ctx)); break;
+        case 2: PB_CUDA(launch_m2p<2>(ctx)); break;
+        case 3: PB_CUDA(launch_m2p<3>(ctx)); break;
+        case 4: PB_CUDA(launch_m2p<4>(ctx)); break;
+        case 5: PB_CUDA(launch_m2p<5>(ctx)); break;
+        case 6: PB_CUDA(launch_m2p<6>(ctx)); break;
+        case 7: PB_CUDA(launch_m2p<7>(ctx)); break;
+        case 8: PB_CUDA(launch_m2p<8>(ctx)); break;
+        case 9: PB_CUDA(launch_m2p<9>(ctx)); break;
+        case 10: PB_CUDA(launch_m2p<10>(ctx)); break;
         default: return pb_fail(ctx, PB_ERR_INVALID_ARG, "unsupported order_P %d", t.P);
         }
         PB_LAUNCH_CHECK();
@@ -655,16 +726,15 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed)
     }
     if (timed) PB_CUDA(cudaEventRecord(ctx->ev[3], st));
     {
-        dim3 grid((unsigned)t.n_groups, (unsigned)t.nslice_p2p);
         PB_TRY(pb_prof_begin(ctx, 0));
-        k_p2p<<<grid, P2P_THREADS, 0, st>>>(t.N, t.K, t.nslice_p2p, ctx->prm.kappa, t.ek, t.p2p_off, t.p2p_lo, t.p2p_hi,
-                                            t.srec, t.pc[0], t.pc[1], t.pc[2], t.accP);
+        k_p2p<<<(unsigned)t.n_itemP, P2P_THREADS, 0, st>>>(t.N, t.K, ctx->prm.kappa, t.ek, t.itemP, t.p2p_lo, t.p2p_hi, t.srec,
+                                                         t.pc[0], t.pc[1], t.pc[2], t.accP);
         PB_LAUNCH_CHECK();
         PB_TRY(pb_prof_end(ctx, 0));
         pb_prof_next(ctx);
     }
     if (timed) PB_CUDA(cudaEventRecord(ctx->ev[4], st));
-    k_combine<<<pb_blocks(t.N, 128), 128, 0, st>>>(t.N, t.nslice_p2p, far ? t.nslice_m2p : 0,
+    k_combine<<<pb_blocks(t.N, 128), 128, 0, st>>>(t.N, t.itemP_off, far ? t.itemM_off : nullptr,
                                                   ctx->prm.eps_in / ctx->prm.eps_out, t.accP, t.accM, t.nr_off,
                                                   t.nr_col, t.nr_val, t.near_entries, t.xphi, t.xdphi, t.perm, y);
     PB_LAUNCH_CHECK();

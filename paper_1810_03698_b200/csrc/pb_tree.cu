@@ -387,6 +387,98 @@ __global__ void k_lists(list_args a)
     }
 }
 
+__global__ void k_m2p_centres(int64_t n, const int32_t* __restrict__ cell, const double* __restrict__ cx,
+                              const double* __restrict__ cy, const double* __restrict__ cz, double4* __restrict__ out)
+{
+    int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    const int32_t c = cell[e];
+    out[e] = make_double4(cx[c], cy[c], cz[c], 0.0);
+}
+
+// ---- work items: equal shares of each group's lists, one thread block each ---------------------
+// A group's P2P list (source-point ranges) or M2P list (cells) is cut into n_g nearly equal
+// pieces so that the grid holds several waves of blocks of similar duration whatever the mesh
+// size.  Piece j of group g writes its partial sums to accumulator slot j; the combine kernel adds
+// a group's slots in order, so the result does not depend on scheduling.
+// lo == nullptr: the list entries are single units (cells); otherwise entry r holds hi[r]-lo[r] units.
+__global__ void k_items_count(int64_t ng, const int32_t* __restrict__ off, const int32_t* __restrict__ lo,
+                              const int32_t* __restrict__ hi, int item_size, int max_items,
+                              int32_t* __restrict__ cnt, int32_t* __restrict__ maxcnt)
+{
+    int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (g >= ng) return;
+    int64_t tot = 0;
+    if (lo) for (int32_t r = off[g]; r < off[g + 1]; ++r) tot += hi[r] - lo[r];
+    else tot = off[g + 1] - off[g];
+    int64_t n = (tot + item_size / 2) / item_size;
+    if (n < 1) n = tot > 0 ? 1 : 0;
+    if (n > max_items) n = max_items;
+    cnt[g] = (int32_t)n;
+    atomicMax(maxcnt, (int32_t)n);
+}
+
+__global__ void k_items_fill(int64_t ng, const int32_t* __restrict__ off, const int32_t* __restrict__ lo,
+                             const int32_t* __restrict__ hi, const int32_t* __restrict__ item_off,
+                             pb_item* __restrict__ items)
+{
+    int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (g >= ng) return;
+    const int32_t i0 = item_off[g], n = item_off[g + 1] - i0;
+    if (n == 0) return;
+    int64_t tot = 0;
+    if (lo) for (int32_t r = off[g]; r < off[g + 1]; ++r) tot += hi[r] - lo[r];
+    else tot = off[g + 1] - off[g];
+    int32_t r = off[g];
+    int64_t passed = 0;                     // units before entry r
+    for (int32_t j = 0; j < n; ++j) {
+        const int64_t b = tot * j / n, e = tot * (j + 1) / n;
+        pb_item it;
+        it.group = (int32_t)g;
+        it.slot = j;
+        it.count = (int32_t)(e - b);
+        it.pad = 0;
+        if (lo) {
+            while (passed + (hi[r] - lo[r]) <= b) { passed += hi[r] - lo[r]; ++r; }
+            it.r = r;
+            it.a = lo[r] + (int32_t)(b - passed);
+        } else {
+            it.r = off[g] + (int32_t)b;
+            it.a = 0;
+        }
+        items[i0 + j] = it;
+    }
+}
+
+// builds one item table; returns the item count and the largest number of items of one group
+static int pb_build_items(pb_ctx* ctx, int64_t G, const int32_t* off, const int32_t* lo, const int32_t* hi,
+                          int item_size, int max_items, int32_t** item_off_out, pb_item** items_out,
+                          int64_t* n_items, int* max_per_group)
+{
+    cudaStream_t st = ctx->stream;
+    int32_t *cnt, *ioff;
+    PB_TRY(pb_dalloc_t(ctx, &cnt, G + 1, CAT_TMP));
+    PB_TRY(pb_dalloc_t(ctx, &ioff, G + 1, CAT_TREE));
+    PB_CUDA(cudaMemsetAsync(cnt, 0, sizeof(int32_t) * (G + 1), st));
+    int32_t* dmax = (int32_t*)ctx->scratch;
+    PB_CUDA(cudaMemsetAsync(dmax, 0, sizeof(int32_t), st));
+    k_items_count<<<pb_blocks(G, 128), 128, 0, st>>>(G, off, lo, hi, item_size, max_items, cnt, dmax);
+    PB_LAUNCH_CHECK();
+    int32_t hmax = 0;
+    PB_CUDA(cudaMemcpyAsync(&hmax, dmax, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    int64_t total = 0;
+    PB_TRY(pb_exclusive_scan_i32(ctx, cnt, ioff, G + 1, &total));   // synchronises
+    pb_item* items;
+    PB_TRY(pb_dalloc_t(ctx, &items, total > 0 ? total : 1, CAT_TREE));
+    k_items_fill<<<pb_blocks(G, 128), 128, 0, st>>>(G, off, lo, hi, ioff, items);
+    PB_LAUNCH_CHECK();
+    *item_off_out = ioff;
+    *items_out = items;
+    *n_items = total;
+    *max_per_group = hmax;
+    return PB_OK;
+}
+
 // ---- host driver ----------------------------------------------------------------------------
 int pb_tree_build_impl(pb_ctx* ctx)
 {
@@ -567,21 +659,30 @@ int pb_tree_build_impl(pb_ctx* ctx)
     a.n_m2p = t.m2p_off; a.n_p2p = t.p2p_off; a.m2p_cell = t.m2p_cell; a.p2p_lo = t.p2p_lo; a.p2p_hi = t.p2p_hi;
     k_lists<1><<<pb_blocks(G, 64), 64, 0, st>>>(a);
     PB_LAUNCH_CHECK();
+    PB_TRY(pb_dalloc_t(ctx, &t.m2p_ctr, tot_m > 0 ? tot_m : 1, CAT_TREE));
+    if (tot_m > 0) {
+        k_m2p_centres<<<pb_blocks(tot_m, 256), 256, 0, st>>>(tot_m, t.m2p_cell, t.c_ctr[0], t.c_ctr[1], t.c_ctr[2], t.m2p_ctr);
+        PB_LAUNCH_CHECK();
+    }
 
-    // partial-sum slices: enough blocks to fill 148 SMs several times over on small meshes
+    // work items: about 8 blocks per resident-block slot (148 SMs x 3 blocks), never less than one
+    // tile of 128 source points / 4 cells per block
     {
-        int64_t want = 148 * 8;
-        int ns = (int)((want + G - 1) / G);
-        if (ns < 1) ns = 1;
-        if (ns > 64) ns = 64;
-        t.nslice_m2p = ns;
-        // P2P blocks hold 8 warps: 4 blocks per SM fill the schedulers
-        ns = (int)((148 * 4 + G - 1) / G);
-        if (ns < 1) ns = 1;
-        if (ns > 32) ns = 32;
-        t.nslice_p2p = ns;
-        PB_TRY(pb_dalloc_t(ctx, &t.accP, (size_t)t.nslice_p2p * 4 * N, CAT_TREE));
-        PB_TRY(pb_dalloc_t(ctx, &t.accM, (size_t)t.nslice_m2p * 4 * N, CAT_TREE));
+        const int64_t slots = 148 * 3 * 8;
+        int64_t szP = (t.p2p_pairs / PB_TG + slots - 1) / slots;
+        if (szP < 128) szP = 128;
+        if (szP > (1 << 30)) szP = 1 << 30;
+        PB_TRY(pb_build_items(ctx, G, t.p2p_off, t.p2p_lo, t.p2p_hi, (int)szP, 64, &t.itemP_off, &t.itemP, &t.n_itemP,
+                              &t.nslot_p2p));
+        int64_t szM = (t.m2p_pairs / PB_TG + slots - 1) / slots;
+        if (szM < 4) szM = 4;
+        if (szM > (1 << 30)) szM = 1 << 30;
+        PB_TRY(pb_build_items(ctx, G, t.m2p_off, nullptr, nullptr, (int)szM, 64, &t.itemM_off, &t.itemM, &t.n_itemM,
+                              &t.nslot_m2p));
+        if (t.nslot_p2p < 1) t.nslot_p2p = 1;
+        if (t.nslot_m2p < 1) t.nslot_m2p = 1;
+        PB_TRY(pb_dalloc_t(ctx, &t.accP, (size_t)t.nslot_p2p * 4 * N, CAT_TREE));
+        PB_TRY(pb_dalloc_t(ctx, &t.accM, (size_t)t.nslot_m2p * 4 * N, CAT_TREE));
     }
     PB_CUDA(cudaStreamSynchronize(st));
     pb_dfree_cat(ctx, CAT_TMP);
