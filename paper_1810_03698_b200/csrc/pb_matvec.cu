@@ -215,111 +215,128 @@ void pb_make_expk(double kappa, pb_expk* k)
 }
 
 // ---- P2M at the leaves: M^V_k = sum_g q^V_g h^k,  M^K_k = sum_g sum_d q^K_{g,d} k_d h^{k-e_d} ---
+// Four plain moment sets per cell are accumulated, S^V, S^x, S^y, S^z (weights q^V, q^K_x, q^K_y,
+// q^K_z), one monomial serving all four; then M^K_(a,b,c) = a S^x_(a-1,b,c) + b S^y_(a,b-1,c) + c S^z_(a,b,c-1).
 #define P2M_CH 32
+#define P2M_LD (PB_MAX_P + 1)     // 11 doubles per point: odd stride, so a warp's reads of one point do not conflict
 __global__ void __launch_bounds__(128)
 k_p2m_leaf(int P, int Nk, int K, const int32_t* __restrict__ leaf_ids, const int32_t* __restrict__ c_first,
            const int32_t* __restrict__ c_last, const double* __restrict__ cx, const double* __restrict__ cy,
            const double* __restrict__ cz, const double4* __restrict__ srec, double* __restrict__ M)
 {
-    __shared__ double pw[3][PB_MAX_P + 1][P2M_CH];
-    __shared__ double wq[4][P2M_CH];
+    __shared__ double pw[3][P2M_CH][P2M_LD];
+    __shared__ double4 wq[P2M_CH];
+    __shared__ double sk[3][PB_MAX_NK];
+    const int nth = blockDim.x;
     const int32_t c = leaf_ids[blockIdx.x];
     const int64_t s0 = (int64_t)c_first[c] * K, s1 = (int64_t)c_last[c] * K;
     const double yc[3] = {cx[c], cy[c], cz[c]};
-    double mv[3] = {0, 0, 0}, mk[3] = {0, 0, 0};   // up to 3 terms per thread (Nk <= 286 < 3*128)
+    int ea[3], eb[3], ec[3];
+#pragma unroll
+    for (int r = 0; r < 3; ++r) {
+        const int k = threadIdx.x + r * nth;
+        ea[r] = k < Nk ? c_ka[k] : 0; eb[r] = k < Nk ? c_kb[k] : 0; ec[r] = k < Nk ? c_kc[k] : 0;
+    }
+    double acc[3][4];
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+        for (int m = 0; m < 4; ++m) acc[r][m] = 0.0;
     for (int64_t base = s0; base < s1; base += P2M_CH) {
-        int np = (int)((s1 - base) < P2M_CH ? (s1 - base) : P2M_CH);
+        const int np = (int)((s1 - base) < P2M_CH ? (s1 - base) : P2M_CH);
         __syncthreads();
         if (threadIdx.x < np) {
-            int64_t s = base + threadIdx.x;
+            const int64_t s = base + threadIdx.x;
             const double4 ra = srec[2 * s], rb = srec[2 * s + 1];
-            double h[3] = {ra.x - yc[0], ra.y - yc[1], ra.z - yc[2]};
+            const double h[3] = {ra.x - yc[0], ra.y - yc[1], ra.z - yc[2]};
             for (int d = 0; d < 3; ++d) {
                 double p = 1.0;
-                for (int e = 0; e <= P; ++e) { pw[d][e][threadIdx.x] = p; p *= h[d]; }
+                for (int e = 0; e <= P; ++e) { pw[d][threadIdx.x][e] = p; p *= h[d]; }
             }
-            wq[0][threadIdx.x] = ra.w;
-            wq[1][threadIdx.x] = rb.x;
-            wq[2][threadIdx.x] = rb.y;
-            wq[3][threadIdx.x] = rb.z;
+            wq[threadIdx.x] = make_double4(ra.w, rb.x, rb.y, rb.z);
         }
         __syncthreads();
+#pragma unroll
         for (int r = 0; r < 3; ++r) {
-            int k = threadIdx.x + r * 128;
-            if (k >= Nk) break;
-            int a = c_ka[k], b = c_kb[k], cc = c_kc[k];
-            double sv = 0, sk = 0;
-            for (int p = 0; p < np; ++p) {
-                double xa = pw[0][a][p], yb = pw[1][b][p], zc = pw[2][cc][p];
-                sv += wq[0][p] * xa * yb * zc;
-                double t = 0;
-                if (a) t += wq[1][p] * a * pw[0][a - 1][p] * yb * zc;
-                if (b) t += wq[2][p] * b * xa * pw[1][b - 1][p] * zc;
-                if (cc) t += wq[3][p] * cc * xa * yb * pw[2][cc - 1][p];
-                sk += t;
+            if (threadIdx.x + r * nth < Nk) {
+#pragma unroll 4
+                for (int p = 0; p < np; ++p) {
+                    const double mono = pw[0][p][ea[r]] * pw[1][p][eb[r]] * pw[2][p][ec[r]];
+                    const double4 w = wq[p];
+                    acc[r][0] = fma(w.x, mono, acc[r][0]);
+                    acc[r][1] = fma(w.y, mono, acc[r][1]);
+                    acc[r][2] = fma(w.z, mono, acc[r][2]);
+                    acc[r][3] = fma(w.w, mono, acc[r][3]);
+                }
             }
-            mv[r] += sv;
-            mk[r] += sk;
         }
     }
+    __syncthreads();
+#pragma unroll
     for (int r = 0; r < 3; ++r) {
-        int k = threadIdx.x + r * 128;
-        if (k >= Nk) break;
-        M[((int64_t)c * 2 + 0) * Nk + k] = mv[r];
-        M[((int64_t)c * 2 + 1) * Nk + k] = mk[r];
+        const int k = threadIdx.x + r * nth;
+        if (k < Nk) {
+            M[((int64_t)c * 2 + 0) * Nk + k] = acc[r][0];
+            sk[0][k] = acc[r][1]; sk[1][k] = acc[r][2]; sk[2][k] = acc[r][3];
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < 3; ++r) {
+        const int k = threadIdx.x + r * nth;
+        if (k < Nk) {
+            const int a = ea[r], b = eb[r], cc = ec[r];
+            double v = 0.0;
+            if (a) v = fma((double)a, sk[0][mom_index(a - 1, b, cc)], v);
+            if (b) v = fma((double)b, sk[1][mom_index(a, b - 1, cc)], v);
+            if (cc) v = fma((double)cc, sk[2][mom_index(a, b, cc - 1)], v);
+            M[((int64_t)c * 2 + 1) * Nk + k] = v;
+        }
     }
 }
 
 // ---- M2M: moments of a parent from its children, M'_k = sum_{l<=k} C(k,l) t^{k-l} M_l -------------
 // Table driven: for every k the (l, k-l, C(k,l)) triples are listed once on the host (mm_*), so a
 // thread does no index arithmetic.  Only cells some M2P list needs (directly or through an accepted
-// ancestor) are visited: `cells` is the compacted list for one BFS generation.
+// ancestor) are visited: `cells` is the compacted list for one BFS generation.  All children are
+// staged in shared memory at once (one global-memory latency per cell).
 __global__ void __launch_bounds__(128)
 k_m2m(const int32_t* __restrict__ cells, int P, int Nk, const int32_t* __restrict__ c_child,
       const int32_t* __restrict__ c_nchild, const double* __restrict__ cx, const double* __restrict__ cy,
       const double* __restrict__ cz, const int32_t* __restrict__ mm_off, const int32_t* __restrict__ mm_ent,
       const double* __restrict__ mm_coef, double* __restrict__ M)
 {
-    __shared__ double cm[2][PB_MAX_NK];
-    __shared__ double tp[3][PB_MAX_P + 1];
+    extern __shared__ double m2m_sm[];                 // cm[8][2*Nk], tp[8][3][PB_MAX_P+1]
+    double* cm = m2m_sm;
+    double* tp = m2m_sm + 8 * 2 * Nk;
+    const int nth = blockDim.x;
     const int64_t c = cells[blockIdx.x];
     const int32_t ch = c_child[c];
     const int nc = c_nchild[c];
-    double acc[2][3] = {{0, 0, 0}, {0, 0, 0}};
-    for (int q = 0; q < nc; ++q) {
-        const int64_t cc = ch + q;
-        __syncthreads();
-        for (int k = threadIdx.x; k < 2 * Nk; k += 128) cm[k / Nk][k % Nk] = M[cc * 2 * Nk + k];
-        if (threadIdx.x < 3) {
-            const double* ctr = threadIdx.x == 0 ? cx : (threadIdx.x == 1 ? cy : cz);
-            double tt = ctr[cc] - ctr[c], p = 1.0;
-            for (int e = 0; e <= P; ++e) { tp[threadIdx.x][e] = p; p *= tt; }
-        }
-        __syncthreads();
-#pragma unroll
-        for (int r = 0; r < 3; ++r) {
-            const int k = threadIdx.x + r * 128;
-            if (k < Nk) {
-                double s0 = 0, s1 = 0;
-                for (int e = mm_off[k]; e < mm_off[k + 1]; ++e) {
-                    const int32_t ent = mm_ent[e];
-                    const double f = mm_coef[e] * tp[0][(ent >> 12) & 15] * tp[1][(ent >> 16) & 15] * tp[2][(ent >> 20) & 15];
-                    const int l = ent & 0xfff;
-                    s0 = fma(f, cm[0][l], s0);
-                    s1 = fma(f, cm[1][l], s1);
-                }
-                acc[0][r] += s0;
-                acc[1][r] += s1;
+    for (int k = threadIdx.x; k < nc * 2 * Nk; k += nth) cm[k] = M[(int64_t)ch * 2 * Nk + k];   // children are consecutive
+    if (threadIdx.x < 3 * nc) {
+        const int q = threadIdx.x / 3, d = threadIdx.x % 3;
+        const double* ctr = d == 0 ? cx : (d == 1 ? cy : cz);
+        double tt = ctr[ch + q] - ctr[c], p = 1.0;
+        for (int e = 0; e <= P; ++e) { tp[(q * 3 + d) * (PB_MAX_P + 1) + e] = p; p *= tt; }
+    }
+    __syncthreads();
+    for (int k = threadIdx.x; k < Nk; k += nth) {
+        double s0 = 0, s1 = 0;
+        const int e0 = mm_off[k], e1 = mm_off[k + 1];
+        for (int e = e0; e < e1; ++e) {
+            const int32_t ent = mm_ent[e];
+            const double cf = mm_coef[e];
+            const int l = ent & 0xfff, dx = (ent >> 12) & 15, dy = (ent >> 16) & 15, dz = (ent >> 20) & 15;
+            for (int q = 0; q < nc; ++q) {
+                const double* t3 = tp + q * 3 * (PB_MAX_P + 1);
+                const double f = cf * t3[dx] * t3[(PB_MAX_P + 1) + dy] * t3[2 * (PB_MAX_P + 1) + dz];
+                s0 = fma(f, cm[q * 2 * Nk + l], s0);
+                s1 = fma(f, cm[q * 2 * Nk + Nk + l], s1);
             }
         }
-    }
-#pragma unroll
-    for (int r = 0; r < 3; ++r) {
-        const int k = threadIdx.x + r * 128;
-        if (k < Nk) {
-            M[(c * 2 + 0) * Nk + k] = acc[0][r];
-            M[(c * 2 + 1) * Nk + k] = acc[1][r];
-        }
+        M[(c * 2 + 0) * Nk + k] = s0;
+        M[(c * 2 + 1) * Nk + k] = s1;
     }
 }
 
@@ -623,36 +640,39 @@ k_p2p(int64_t N, int K, double kappa, pb_expk ek, const pb_item* __restrict__ it
 }
 
 // ---- near/singular table + Eq. (5) combine + un-permute (H8) ------------------------------------------------
-__global__ void k_combine(int64_t N, const int32_t* __restrict__ itemP_off, const int32_t* __restrict__ itemM_off,
-                          double eps_ratio, const double* __restrict__ accP,
-                          const double* __restrict__ accM, const int32_t* __restrict__ nr_off,
-                          const int32_t* __restrict__ nr_col, const double* __restrict__ nr_val, int64_t ne,
-                          const double* __restrict__ xphi, const double* __restrict__ xdphi,
-                          const int32_t* __restrict__ perm, double* __restrict__ y)
+// Block = 32 targets x 4 outputs: thread (tgt, m) adds output m of its target over the group's slots
+// and over its row of the near table, then thread m == 0 forms the two rows of Eq. (5).
+__global__ void __launch_bounds__(128)
+k_combine(int64_t N, const int32_t* __restrict__ itemP_off, const int32_t* __restrict__ itemM_off, double eps_ratio,
+          const double* __restrict__ accP, const double* __restrict__ accM, const int32_t* __restrict__ nr_off,
+          const int32_t* __restrict__ nr_col, const double* __restrict__ nr_val, int64_t ne,
+          const double* __restrict__ xphi, const double* __restrict__ xdphi, const int32_t* __restrict__ perm,
+          double* __restrict__ y)
 {
-    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    double s[4] = {0, 0, 0, 0};
-    const int64_t g = i / PB_TG;
-    const int nsP = itemP_off[g + 1] - itemP_off[g];
-    const int nsM = itemM_off ? itemM_off[g + 1] - itemM_off[g] : 0;
-    for (int q = 0; q < nsP; ++q)
-        for (int m = 0; m < 4; ++m) s[m] += accP[((int64_t)q * 4 + m) * N + i];
-    for (int q = 0; q < nsM; ++q)
-        for (int m = 0; m < 4; ++m) s[m] += accM[((int64_t)q * 4 + m) * N + i];
-    double VL = PB_INV4PI * s[0], KL = PB_INV4PI * s[1], VY = PB_INV4PI * s[2], KY = PB_INV4PI * s[3];
-    for (int32_t e = nr_off[i]; e < nr_off[i + 1]; ++e) {
-        int32_t j = nr_col[e];
-        double ph = xphi[j], dp = xdphi[j];
-        VL = fma(nr_val[e], dp, VL);
-        KL = fma(nr_val[ne + e], ph, KL);
-        VY = fma(nr_val[2 * ne + e], dp, VY);
-        KY = fma(nr_val[3 * ne + e], ph, KY);
+    __shared__ double sm[4][32];
+    const int tgt = threadIdx.x & 31, m = threadIdx.x >> 5;
+    const int64_t i = blockIdx.x * 32LL + tgt;
+    double s = 0.0;
+    if (i < N) {
+        const int64_t g = i / PB_TG;
+        const int nsP = itemP_off[g + 1] - itemP_off[g];
+        const int nsM = itemM_off ? itemM_off[g + 1] - itemM_off[g] : 0;
+        for (int q = 0; q < nsP; ++q) s += accP[((int64_t)q * 4 + m) * N + i];
+        for (int q = 0; q < nsM; ++q) s += accM[((int64_t)q * 4 + m) * N + i];
+        s *= PB_INV4PI;
+        const double* __restrict__ xv = (m & 1) ? xphi : xdphi;     // V_L, V_Y act on dphi; K_L, K_Y on phi
+        const double* __restrict__ val = nr_val + (int64_t)m * ne;
+        for (int32_t e = nr_off[i]; e < nr_off[i + 1]; ++e) s = fma(val[e], xv[nr_col[e]], s);
     }
-    const double phi = xphi[i];
-    const int64_t o = perm[i];
-    y[o] = 0.5 * phi + KL - VL;                    // Eq. (5), first row
-    y[N + o] = 0.5 * phi - KY + eps_ratio * VY;    // Eq. (5), second row
+    sm[m][tgt] = s;
+    __syncthreads();
+    if (m == 0 && i < N) {
+        const double VL = sm[0][tgt], KL = sm[1][tgt], VY = sm[2][tgt], KY = sm[3][tgt];
+        const double phi = xphi[i];
+        const int64_t o = perm[i];
+        y[o] = 0.5 * phi + KL - VL;                    // Eq. (5), first row
+        y[N + o] = 0.5 * phi - KY + eps_ratio * VY;    // Eq. (5), second row
+    }
 }
 
 // ---- host driver ----------------------------------------------------------------------------------------------
@@ -687,14 +707,14 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed)
     if (timed) PB_CUDA(cudaEventRecord(ctx->ev[1], st));
     if (far) {
         if (t.n_need_leaf > 0) {
-            k_p2m_leaf<<<(unsigned)t.n_need_leaf, 128, 0, st>>>(t.P, t.Nk, t.K, t.need_leaf, t.c_first, t.c_last, t.c_ctr[0],
+            k_p2m_leaf<<<(unsigned)t.n_need_leaf, t.Nk <= 96 ? 96 : 128, 0, st>>>(t.P, t.Nk, t.K, t.need_leaf, t.c_first, t.c_last, t.c_ctr[0],
                                                                t.c_ctr[1], t.c_ctr[2], t.srec, t.M);
             PB_LAUNCH_CHECK();
         }
         for (int g = (int)t.m2m_start.size() - 2; g >= 0; --g) {   // deepest generation first
             const int64_t n = t.m2m_start[g + 1] - t.m2m_start[g];
             if (n == 0) continue;
-            k_m2m<<<(unsigned)n, 128, 0, st>>>(t.m2m_cells + t.m2m_start[g], t.P, t.Nk, t.c_child, t.c_nchild, t.c_ctr[0],
+            k_m2m<<<(unsigned)n, t.Nk <= 96 ? 96 : 128, (size_t)(16 * t.Nk + 24 * (PB_MAX_P + 1)) * sizeof(double), st>>>(t.m2m_cells + t.m2m_start[g], t.P, t.Nk, t.c_child, t.c_nchild, t.c_ctr[0],
                                                t.c_ctr[1], t.c_ctr[2], t.mm_off, t.mm_ent, t.mm_coef, t.M);
             PB_LAUNCH_CHECK();
         }
@@ -734,7 +754,7 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed)
         pb_prof_next(ctx);
     }
     if (timed) PB_CUDA(cudaEventRecord(ctx->ev[4], st));
-    k_combine<<<pb_blocks(t.N, 128), 128, 0, st>>>(t.N, t.itemP_off, far ? t.itemM_off : nullptr,
+    k_combine<<<pb_blocks(t.N, 32), 128, 0, st>>>(t.N, t.itemP_off, far ? t.itemM_off : nullptr,
                                                   ctx->prm.eps_in / ctx->prm.eps_out, t.accP, t.accM, t.nr_off,
                                                   t.nr_col, t.nr_val, t.near_entries, t.xphi, t.xdphi, t.perm, y);
     PB_LAUNCH_CHECK();
