@@ -46,88 +46,137 @@ def draw_sites(seed, n, ball_radius, min_sep=1.0, alpha=1.0):
 
 
 def random_chain_globule(seed, n_atoms, ball_radius=None, step=1.5, min_nonbonded=2.0,
-                         group_size=4, alpha=1.0):
+                         group_size=4, alpha=1.0, n_try=32, max_stall=6):
     """Protein-like solute (BASELINE configs[2]): a seeded random-walk chain with
     `step`-Angstrom bonds, bond angle U[100,120] degrees, uniform torsion, radii
     U[1.2,2.0] A, confined to a ball (14 A at 1000 atoms, scaling with n^(1/3)) by
-    rejecting steps that leave it or come within `min_nonbonded` of a non-bonded atom,
-    backtracking on dead ends.  Sites sit on the atom centres with the configs[1]
-    multipole distributions; polarization group = chain index // group_size."""
+    rejecting steps that leave it or come within `min_nonbonded` of a non-bonded atom.
+    On a dead end the walk backtracks a few atoms; after `max_stall` dead ends without
+    progress the chain is broken and a new segment starts at a free spot of the ball (a
+    multi-chain globule, like the paper's larger proteins), so the cost stays linear in
+    n_atoms.  Sites sit on the atom centres with the configs[1] multipole distributions;
+    polarization group = atom index // group_size.
+
+    All candidate steps of one atom are tested at once against a dense cell grid (cell
+    edge = min_nonbonded, up to 8 atoms per cell)."""
     rng = _rng(seed)
     if ball_radius is None:
         ball_radius = 14.0 * (n_atoms / 1000.0) ** (1.0 / 3.0)
-    cell = min_nonbonded
-    grid: dict[tuple, list] = {}
-    pos = np.zeros((n_atoms, 3))
+    cell = float(min_nonbonded)
+    ng = int(np.ceil(2.0 * ball_radius / cell)) + 4
+    origin = -0.5 * ng * cell
+    slots = 8
+    cell_cnt = np.zeros((ng, ng, ng), dtype=np.int32)
+    cell_atoms = -np.ones((ng, ng, ng, slots), dtype=np.int64)
+    pos = np.zeros((n_atoms + 1, 3))                 # row n_atoms: a far-away dummy for empty slots
+    pos[n_atoms] = 1e9
+    nb = np.array([(dx, dy, dz) for dx in (-1, 0, 1) for dy in (-1, 0, 1) for dz in (-1, 0, 1)])
+    r2min = min_nonbonded ** 2
 
-    def key(p):
-        return (int(np.floor(p[0] / cell)), int(np.floor(p[1] / cell)), int(np.floor(p[2] / cell)))
+    def cell_of(p):
+        return np.floor((p - origin) / cell).astype(np.int64)
 
-    def clash(p, skip):
-        k = key(p)
-        for dx in (-1, 0, 1):
-            for dy in (-1, 0, 1):
-                for dz in (-1, 0, 1):
-                    for idx in grid.get((k[0] + dx, k[1] + dy, k[2] + dz), ()):
-                        if idx in skip:
-                            continue
-                        d = pos[idx] - p
-                        if d[0] * d[0] + d[1] * d[1] + d[2] * d[2] < min_nonbonded ** 2:
-                            return True
-        return False
+    def free_mask(cand, skip0, skip1):
+        """cand [m][3] -> bool[m]: inside the ball and clear of every placed atom but the two skipped."""
+        inside = np.einsum("ij,ij->i", cand, cand) <= ball_radius ** 2
+        c = cell_of(cand)[:, None, :] + nb[None, :, :]                     # [m][27][3]
+        ids = cell_atoms[c[..., 0], c[..., 1], c[..., 2]]                  # [m][27][slots]
+        ids = ids.reshape(cand.shape[0], -1)
+        ids = np.where((ids == skip0) | (ids == skip1) | (ids < 0), n_atoms, ids)
+        d = pos[ids] - cand[:, None, :]
+        clear = (np.einsum("ijk,ijk->ij", d, d) >= r2min).all(axis=1)
+        return inside & clear
 
     def place(i, p):
         pos[i] = p
-        grid.setdefault(key(p), []).append(i)
+        c = cell_of(p)
+        k = cell_cnt[c[0], c[1], c[2]]
+        if k >= slots:
+            raise RuntimeError("globule generator: cell overflow")
+        cell_atoms[c[0], c[1], c[2], k] = i
+        cell_cnt[c[0], c[1], c[2]] = k + 1
 
     def unplace(i):
-        grid[key(pos[i])].remove(i)
+        c = cell_of(pos[i])
+        k = cell_cnt[c[0], c[1], c[2]]
+        row = cell_atoms[c[0], c[1], c[2]]
+        j = int(np.nonzero(row[:k] == i)[0][0])
+        row[j] = row[k - 1]
+        row[k - 1] = -1
+        cell_cnt[c[0], c[1], c[2]] = k - 1
 
-    # start near the centre with a random first bond
+    def unit(v):
+        return v / np.linalg.norm(v)
+
+    def start_segment(i):
+        """Atoms i and i+1 of a new chain segment at a free spot (i+1 may run past the end)."""
+        for _ in range(10000):
+            c = rng.uniform(-ball_radius, ball_radius, (64, 3))
+            ok = np.nonzero(free_mask(c, -2, -2))[0]
+            for k in ok:
+                if i + 1 >= n_atoms:
+                    place(i, c[k])
+                    return
+                d = rng.normal(size=(16, 3))
+                d /= np.linalg.norm(d, axis=1)[:, None]
+                c2 = c[k] + step * d
+                ok2 = np.nonzero(free_mask(c2, -2, -2))[0]
+                if ok2.size:
+                    place(i, c[k])
+                    place(i + 1, c2[ok2[0]])
+                    return
+        raise RuntimeError("globule generator: no free spot left in the ball")
+
+    seg_start = 0
+    seg_starts = [0]
     place(0, rng.normal(0, 0.5, 3))
-    d0 = rng.normal(size=3)
-    d0 /= np.linalg.norm(d0)
-    place(1, pos[0] + step * d0)
+    place(1, pos[0] + step * unit(rng.normal(size=3)))
     i = 2
-    fails = 0
+    high = 2                                          # furthest atom index reached so far
+    stall = 0
+    n_segments = 1
     while i < n_atoms:
-        prev = pos[i - 1] - pos[i - 2]
-        prev /= np.linalg.norm(prev)
-        ok = False
-        for _ in range(40):
-            bond = np.deg2rad(rng.uniform(100.0, 120.0))
-            dev = np.pi - bond                      # deviation of the new bond from the old direction
-            tors = rng.uniform(0.0, 2.0 * np.pi)
-            a = np.cross(prev, [1.0, 0.0, 0.0])
-            if np.linalg.norm(a) < 1e-3:
-                a = np.cross(prev, [0.0, 1.0, 0.0])
-            a /= np.linalg.norm(a)
-            b = np.cross(prev, a)
-            dirn = np.cos(dev) * prev + np.sin(dev) * (np.cos(tors) * a + np.sin(tors) * b)
-            p = pos[i - 1] + step * dirn
-            if np.dot(p, p) > ball_radius ** 2:
-                continue
-            if clash(p, (i - 1, i - 2)):
-                continue
-            place(i, p)
-            ok = True
-            break
-        if ok:
+        prev = unit(pos[i - 1] - pos[i - 2])
+        a = np.cross(prev, [1.0, 0.0, 0.0])
+        if np.linalg.norm(a) < 1e-3:
+            a = np.cross(prev, [0.0, 1.0, 0.0])
+        a = unit(a)
+        b = np.cross(prev, a)
+        dev = np.pi - np.deg2rad(rng.uniform(100.0, 120.0, n_try))   # deviation of the new bond from the old direction
+        tors = rng.uniform(0.0, 2.0 * np.pi, n_try)
+        dirn = (np.cos(dev)[:, None] * prev[None, :]
+                + np.sin(dev)[:, None] * (np.cos(tors)[:, None] * a[None, :] + np.sin(tors)[:, None] * b[None, :]))
+        cand = pos[i - 1] + step * dirn
+        ok = np.nonzero(free_mask(cand, i - 1, i - 2))[0]
+        if ok.size:
+            place(i, cand[ok[0]])
             i += 1
+            if i > high:
+                high = i
+                stall = 0
             continue
-        fails += 1
-        back = min(i - 2, 3 + fails % 7)
+        stall += 1
+        if stall > max_stall:                         # trapped: break the chain here
+            seg_start = i
+            seg_starts.append(i)
+            start_segment(i)
+            n_segments += 1
+            i = min(i + 2, n_atoms)
+            high = max(high, i)
+            stall = 0
+            continue
+        back = min(i - seg_start - 2, 1 + stall)
         for j in range(i - 1, i - 1 - back, -1):
             unplace(j)
         i -= back
-        if fails > 200 * n_atoms:
-            raise RuntimeError("globule generator stuck")
+    pos = pos[:n_atoms]
     radii = rng.uniform(1.2, 2.0, n_atoms)
     q, dip, quad = draw_multipoles(rng, n_atoms)
     return dict(pos=pos.copy(), radii=radii, q=q, dip=dip, quad=quad,
                 alpha=np.full(n_atoms, float(alpha)),
                 group=(np.arange(n_atoms) // group_size).astype(np.int32),
-                ball_radius=float(ball_radius))
+                ball_radius=float(ball_radius), n_segments=n_segments,
+                seg_starts=np.array(seg_starts, dtype=np.int64))
 
 
 # ---------------------------------------------------------------------------

@@ -37,20 +37,44 @@ def test_c0_and_c1_configs():
     assert seed_for(1) == 181003698 + 1000
 
 
-def test_globule_chain_geometry():
-    g = random_chain_globule(seed_for(2), 300)
+def _check_chain(g, n):
     p = g["pos"]
+    seg = np.zeros(n, dtype=np.int64)
+    seg[g["seg_starts"][1:]] = 1
+    seg = np.cumsum(seg)                                   # segment id of every atom
+    same1 = seg[1:] == seg[:-1]
     bonds = np.linalg.norm(p[1:] - p[:-1], axis=1)
-    np.testing.assert_allclose(bonds, 1.5, rtol=1e-12)
+    np.testing.assert_allclose(bonds[same1], 1.5, rtol=1e-12)
+    same2 = seg[2:] == seg[:-2]
     a, b = p[:-2] - p[1:-1], p[2:] - p[1:-1]
-    ang = np.degrees(np.arccos(np.einsum("ij,ij->i", a, b) / 2.25))
+    ang = np.degrees(np.arccos(np.einsum("ij,ij->i", a, b)[same2] / 2.25))
     assert ang.min() > 100 - 1e-6 and ang.max() < 120 + 1e-6
     assert np.linalg.norm(p, axis=1).max() <= g["ball_radius"] + 1e-9
     d = np.linalg.norm(p[:, None] - p[None], axis=2)
-    i, j = np.triu_indices(300, 3)
-    assert d[i, j].min() >= 2.0 - 1e-9
+    i, j = np.triu_indices(n, 1)
+    nonbonded = (j - i >= 3) | (seg[i] != seg[j])
+    assert d[i, j][nonbonded].min() >= 2.0 - 1e-9
     assert g["radii"].min() >= 1.2 and g["radii"].max() <= 2.0
+    assert np.diff(g["seg_starts"]).min(initial=2) >= 2      # no single-atom segments inside the chain
+
+
+def test_globule_chain_geometry():
+    g = random_chain_globule(seed_for(2), 300)
+    _check_chain(g, 300)
     assert g["group"][7] == 1 and g["group"].dtype == np.int32
+    g2 = random_chain_globule(seed_for(2), 300)
+    np.testing.assert_array_equal(g["pos"], g2["pos"])          # seeded
+
+
+def test_globule_chain_breaks_keep_the_cost_linear():
+    """A ball this full traps the walk; the generator must break the chain (several segments)
+    rather than thrash, and every segment must still obey the recipe."""
+    import time
+    t0 = time.perf_counter()
+    g = random_chain_globule(seed_for(2), 2000)
+    assert time.perf_counter() - t0 < 30.0
+    assert g["n_segments"] == len(g["seg_starts"]) > 1
+    _check_chain(g, 2000)
 
 
 def test_vdw_surface_is_closed_and_hits_the_panel_count():
