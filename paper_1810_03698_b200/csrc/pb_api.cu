@@ -112,6 +112,12 @@ extern "C" int pb_create(pb_ctx** out, int device, void* cuda_stream)
     ctx->device = device;
     ctx->stream = (cudaStream_t)cuda_stream;
     pb_default_params(&ctx->prm);
+    int lo = 0, hi = 0;
+    bool ok = cudaDeviceGetStreamPriorityRange(&lo, &hi) == cudaSuccess &&
+              cudaStreamCreateWithPriority(&ctx->side, cudaStreamNonBlocking, hi) == cudaSuccess &&
+              cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
+              cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) { delete ctx; return PB_ERR_CUDA; }
     *out = ctx;
     return PB_OK;
 }
@@ -121,6 +127,10 @@ extern "C" int pb_destroy(pb_ctx* ctx)
     if (!ctx) return PB_ERR_INVALID_ARG;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
+    cudaStreamSynchronize(ctx->side);
+    cudaStreamDestroy(ctx->side);
+    cudaEventDestroy(ctx->ev_fork);
+    cudaEventDestroy(ctx->ev_join);
     pb_dfree_cat(ctx, -1);
     if (ctx->h_pinned) cudaFreeHost(ctx->h_pinned);
     if (ctx->ev_made)

@@ -83,11 +83,10 @@ struct pb_tree {
     int32_t* mm_ent = nullptr;
     double* mm_coef = nullptr;
     int64_t m2p_total = 0;        // entries of m2p_cell
-    int64_t n_used = 0, n_need_leaf = 0;
-    int32_t* used_cells = nullptr;   // cells that appear in an M2P list (get F terms)
-    int32_t* need_leaf = nullptr;    // leaves whose moments are needed (P2M)
-    int32_t* m2m_cells = nullptr;    // internal cells whose moments are needed, by generation
-    std::vector<int64_t> m2m_start;  // m2m_cells[m2m_start[g] .. m2m_start[g+1]) = generation g
+    int64_t n_used = 0, n_need_leaf = 0, n_need_internal = 0;
+    int32_t* need_leaf = nullptr;    // leaves whose moments are needed (one k_upward block each)
+    int32_t* up_link = nullptr;      // [cells] bit 0: F terms wanted; bits 1..: 1 + parent if the parent needs moments
+    int32_t* up_count = nullptr;     // [cells] children finished so far (self-resetting)
     int32_t* cv_off = nullptr;    // [NT+1] conversion table (CSR over source moment indices)
     int32_t* cv_idx = nullptr;
     double* cv_coef = nullptr;
@@ -131,12 +130,15 @@ struct pb_gmres_ws {
     int m = 0;
     double *V = nullptr, *w = nullptr, *z = nullptr, *r = nullptr, *u = nullptr;
     double *partial = nullptr, *hdev = nullptr, *coef = nullptr;
-    int nblk = 0;
+    unsigned int* counter = nullptr;   // arrival counter of k_dots' last-block reduction (self-resetting)
 };
 
 struct pb_ctx {
     int device = 0;
     cudaStream_t stream = 0;
+    // far-field branch of the matvec (P2M, M2M, M -> F, M2P) runs here, concurrently with P2P on `stream`
+    cudaStream_t side = 0;
+    cudaEvent_t ev_fork = 0, ev_join = 0;
     char err[512] = {0};
     pb_alloc_fn alloc = nullptr;
     pb_free_fn free_ = nullptr;
@@ -222,8 +224,8 @@ int pb_make_rule(int K, pb_rule_t* r);
 int pb_upload_rules(pb_ctx* ctx);   // fills ctx->ruleF, ruleN, gl from the parameters
 // pb_matvec.cu
 int pb_farfield_setup(pb_ctx* ctx);
-int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed);
-int pb_weights(pb_ctx* ctx, const double* x);
+int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed, bool precond);
+int pb_weights(pb_ctx* ctx, const double* x, bool precond);
 void pb_make_expk(double kappa, pb_expk* out);
 // pb_sites.cu
 int pb_site_near_build(pb_ctx* ctx);

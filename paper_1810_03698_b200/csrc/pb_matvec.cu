@@ -138,32 +138,31 @@ int pb_farfield_setup(pb_ctx* ctx)
     PB_CUDA(cudaStreamSynchronize(st));   // also: the host vectors above go out of scope
     std::vector<char> used(nc, 0), need(nc, 0);
     for (int64_t e = 0; e < t.m2p_total; ++e) used[lists[e]] = 1;
-    std::vector<int32_t> used_list, leaf_list, m2m_list;
-    t.m2m_start.assign(1, 0);
-    for (size_t g = 0; g + 1 < t.gen_start.size(); ++g) {     // cells are numbered generation by generation
-        for (int64_t c = t.gen_start[g]; c < t.gen_start[g + 1]; ++c) {
-            need[c] = need[c] || used[c];
-            if (used[c]) used_list.push_back((int32_t)c);
-            if (!need[c]) continue;
-            if (child[c] < 0) leaf_list.push_back((int32_t)c);
-            else {
-                m2m_list.push_back((int32_t)c);
-                for (int q = 0; q < nchild[c]; ++q) need[child[c] + q] = 1;
-            }
+    std::vector<int32_t> leaf_list, parent(nc, -1), up(nc, 0);
+    int64_t n_used = 0, n_internal = 0;
+    for (int64_t c = 0; c < nc; ++c) {               // cells are numbered generation by generation: parents first
+        need[c] = need[c] || used[c];
+        if (used[c]) ++n_used;
+        if (!need[c]) continue;
+        if (child[c] < 0) leaf_list.push_back((int32_t)c);
+        else {
+            ++n_internal;
+            for (int q = 0; q < nchild[c]; ++q) { need[child[c] + q] = 1; parent[child[c] + q] = (int32_t)c; }
         }
-        t.m2m_start.push_back((int64_t)m2m_list.size());
     }
-    t.n_used = (int64_t)used_list.size();
+    // up[c]: bit 0 = the cell's F terms are wanted (it is in an M2P list); bits 1.. = 1 + parent when the
+    // parent's moments are needed (the block finishing c then reports to it), else 0
+    for (int64_t c = 0; c < nc; ++c) up[c] = (used[c] ? 1 : 0) | ((need[c] && parent[c] >= 0 ? parent[c] + 1 : 0) << 1);
+    t.n_used = n_used;
     t.n_need_leaf = (int64_t)leaf_list.size();
-    PB_TRY(pb_dalloc_t(ctx, &t.used_cells, used_list.size(), CAT_TREE));
+    t.n_need_internal = n_internal;
     PB_TRY(pb_dalloc_t(ctx, &t.need_leaf, leaf_list.size(), CAT_TREE));
-    PB_TRY(pb_dalloc_t(ctx, &t.m2m_cells, m2m_list.size(), CAT_TREE));
-    if (!used_list.empty())
-        PB_CUDA(cudaMemcpyAsync(t.used_cells, used_list.data(), sizeof(int32_t) * used_list.size(), cudaMemcpyHostToDevice, st));
+    PB_TRY(pb_dalloc_t(ctx, &t.up_link, (size_t)nc, CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.up_count, (size_t)nc, CAT_TREE));
     if (!leaf_list.empty())
         PB_CUDA(cudaMemcpyAsync(t.need_leaf, leaf_list.data(), sizeof(int32_t) * leaf_list.size(), cudaMemcpyHostToDevice, st));
-    if (!m2m_list.empty())
-        PB_CUDA(cudaMemcpyAsync(t.m2m_cells, m2m_list.data(), sizeof(int32_t) * m2m_list.size(), cudaMemcpyHostToDevice, st));
+    PB_CUDA(cudaMemcpyAsync(t.up_link, up.data(), sizeof(int32_t) * nc, cudaMemcpyHostToDevice, st));
+    PB_CUDA(cudaMemsetAsync(t.up_count, 0, sizeof(int32_t) * nc, st));
     PB_CUDA(cudaStreamSynchronize(st));
     PB_TRY(pb_dalloc_t(ctx, &t.M, (size_t)t.n_cells * 2 * t.Nk, CAT_TREE));
     PB_TRY(pb_dalloc_t(ctx, &t.FF, (size_t)t.n_cells * t.NT, CAT_TREE));
@@ -173,9 +172,11 @@ int pb_farfield_setup(pb_ctx* ctx)
 // ---- source weights (H5): q^V_g = w_g A_j dphi_j ,  q^K_g = w_g A_j phi_j n_j ------------------------
 // Writes the 64-byte source records the P2P / P2M / reaction kernels stream (coordinates repeated
 // so that one contiguous TMA bulk copy brings a whole tile of sources into shared memory).
+// With `pc` (the right block-Jacobi preconditioner of GMRES, D: R-20) the operator is applied to
+// z = Minv x, z formed on the fly: per panel the inverse 2x2 diagonal block, original panel order.
 __global__ void k_weights(int64_t N, int K, const int32_t* __restrict__ perm, const double* __restrict__ x,
-                          const double* __restrict__ swA, const double* __restrict__ sx,
-                          const double* __restrict__ sy, const double* __restrict__ sz,
+                          const double* __restrict__ pc, const double* __restrict__ swA,
+                          const double* __restrict__ sx, const double* __restrict__ sy, const double* __restrict__ sz,
                           const double* __restrict__ nx, const double* __restrict__ ny,
                           const double* __restrict__ nz, double* __restrict__ xphi, double* __restrict__ xdphi,
                           double4* __restrict__ srec)
@@ -185,17 +186,23 @@ __global__ void k_weights(int64_t N, int K, const int32_t* __restrict__ perm, co
     int64_t i = s / K;
     int64_t o = perm[i];
     double phi = x[o], dphi = x[N + o], w = swA[s];
+    if (pc) {
+        const double a = phi, b = dphi;
+        phi = pc[o] * a + pc[N + o] * b;
+        dphi = pc[2 * N + o] * a + pc[3 * N + o] * b;
+    }
     if (s == i * K) { xphi[i] = phi; xdphi[i] = dphi; }
     double wp = w * phi;
     srec[2 * s] = make_double4(sx[s], sy[s], sz[s], w * dphi);
     srec[2 * s + 1] = make_double4(wp * nx[i], wp * ny[i], wp * nz[i], 0.0);
 }
 
-int pb_weights(pb_ctx* ctx, const double* x)
+int pb_weights(pb_ctx* ctx, const double* x, bool precond)
 {
     pb_tree& t = ctx->tree;
-    k_weights<<<pb_blocks(t.Ns, 256), 256, 0, ctx->stream>>>(t.N, t.K, t.perm, x, t.swA, t.sx[0], t.sx[1], t.sx[2], t.pn[0],
-                                                            t.pn[1], t.pn[2], t.xphi, t.xdphi, t.srec);
+    k_weights<<<pb_blocks(t.Ns, 256), 256, 0, ctx->stream>>>(t.N, t.K, t.perm, x, precond ? t.precond : nullptr, t.swA, t.sx[0],
+                                                            t.sx[1], t.sx[2], t.pn[0], t.pn[1], t.pn[2], t.xphi, t.xdphi,
+                                                            t.srec);
     PB_LAUNCH_CHECK();
     return PB_OK;
 }
@@ -214,151 +221,200 @@ void pb_make_expk(double kappa, pb_expk* k)
     for (int j = 0; j < 32; ++j) k->T[j] = exp2(-(double)j / 32.0);
 }
 
-// ---- P2M at the leaves: M^V_k = sum_g q^V_g h^k,  M^K_k = sum_g sum_d q^K_{g,d} k_d h^{k-e_d} ---
-// Four plain moment sets per cell are accumulated, S^V, S^x, S^y, S^z (weights q^V, q^K_x, q^K_y,
-// q^K_z), one monomial serving all four; then M^K_(a,b,c) = a S^x_(a-1,b,c) + b S^y_(a,b-1,c) + c S^z_(a,b,c-1).
+// ---- upward pass in ONE launch (H5): P2M at the leaves, M2M up the tree, M -> F conversion ---------------
+// P2M: M^V_k = sum_g q^V_g h^k,  M^K_k = sum_g sum_d q^K_{g,d} k_d h^{k-e_d}.  Four plain moment
+// sets per cell are accumulated, S^V, S^x, S^y, S^z (weights q^V, q^K_x, q^K_y, q^K_z), one monomial
+// serving all four; then M^K_(a,b,c) = a S^x_(a-1,b,c) + b S^y_(a,b-1,c) + c S^z_(a,b,c-1).
+// M2M: M'_k = sum_{l<=k} C(k,l) t^{k-l} M_l, table driven (mm_*: for every k the (l, k-l, C(k,l)) triples).
+// One block per leaf whose moments are needed.  When a block has finished a cell it reports to the
+// parent (if the parent's moments are needed); the block that reports LAST carries on with the
+// parent's M2M, and so on upward -- nobody waits, and a parent is always formed from all its children
+// in child order, so the result does not depend on the arrival order.  A cell that appears in an M2P
+// list has its far-field terms F (D: section 6) written by the block that finishes it.
 #define P2M_CH 32
 #define P2M_LD (PB_MAX_P + 1)     // 11 doubles per point: odd stride, so a warp's reads of one point do not conflict
-__global__ void __launch_bounds__(128)
-k_p2m_leaf(int P, int Nk, int K, const int32_t* __restrict__ leaf_ids, const int32_t* __restrict__ c_first,
-           const int32_t* __restrict__ c_last, const double* __restrict__ cx, const double* __restrict__ cy,
-           const double* __restrict__ cz, const double4* __restrict__ srec, double* __restrict__ M)
+#define UP_THREADS 128
+
+struct up_args {
+    int P, Nk, NT, K;
+    const int32_t *leaf_ids, *c_first, *c_last, *c_child, *c_nchild, *up_link;
+    int32_t* up_count;
+    const double *cx, *cy, *cz;
+    const double4* srec;
+    const int32_t *mm_off, *mm_ent;
+    const double* mm_coef;
+    const int32_t *cv_off, *cv_idx;
+    const double* cv_coef;
+    double* M;
+    double2* FF;
+};
+
+static size_t up_smem_bytes(int Nk)
 {
-    __shared__ double pw[3][P2M_CH][P2M_LD];
-    __shared__ double4 wq[P2M_CH];
-    __shared__ double sk[3][PB_MAX_NK];
-    const int nth = blockDim.x;
-    const int32_t c = leaf_ids[blockIdx.x];
-    const int64_t s0 = (int64_t)c_first[c] * K, s1 = (int64_t)c_last[c] * K;
-    const double yc[3] = {cx[c], cy[c], cz[c]};
-    int ea[3], eb[3], ec[3];
+    const size_t p2m = 3 * P2M_CH * P2M_LD + 3 * (size_t)Nk;
+    const size_t m2m = 32 * (size_t)Nk + 8 * 3 * P2M_LD;
+    return P2M_CH * sizeof(double4) + (2 * (size_t)Nk + (p2m > m2m ? p2m : m2m)) * sizeof(double);
+}
+
+__global__ void __launch_bounds__(UP_THREADS) k_upward(up_args a)
+{
+    extern __shared__ __align__(128) unsigned char up_raw[];
+    const int Nk = a.Nk, P = a.P, tid = threadIdx.x;
+    double4* wq = reinterpret_cast<double4*>(up_raw);          // [P2M_CH]
+    double* mom = reinterpret_cast<double*>(wq + P2M_CH);      // [2][Nk] finished moments of the current cell
+    double* U = mom + 2 * Nk;
+    double* pw = U;                                            // P2M: [3][P2M_CH][P2M_LD]
+    double* sk = U + 3 * P2M_CH * P2M_LD;                      // P2M: [3][Nk]
+    double* cm = U;                                            // M2M: [8][2][Nk] children
+    double* part = cm + 16 * Nk;                               // M2M: [8][2][Nk] shifted children
+    double* tp = part + 16 * Nk;                               // M2M: [8][3][P2M_LD] powers of the shifts
+    __shared__ int s_last;
+
+    int64_t c = a.leaf_ids[blockIdx.x];
+    {   // ---- P2M
+        const int64_t s0 = (int64_t)a.c_first[c] * a.K, s1 = (int64_t)a.c_last[c] * a.K;
+        const double ycx = a.cx[c], ycy = a.cy[c], ycz = a.cz[c];
+        int ea[3], eb[3], ec[3];
 #pragma unroll
-    for (int r = 0; r < 3; ++r) {
-        const int k = threadIdx.x + r * nth;
-        ea[r] = k < Nk ? c_ka[k] : 0; eb[r] = k < Nk ? c_kb[k] : 0; ec[r] = k < Nk ? c_kc[k] : 0;
-    }
-    double acc[3][4];
+        for (int r = 0; r < 3; ++r) {
+            const int k = tid + r * UP_THREADS;
+            ea[r] = k < Nk ? c_ka[k] : 0; eb[r] = k < Nk ? c_kb[k] : 0; ec[r] = k < Nk ? c_kc[k] : 0;
+        }
+        double acc[3][4];
 #pragma unroll
-    for (int r = 0; r < 3; ++r)
+        for (int r = 0; r < 3; ++r)
 #pragma unroll
-        for (int m = 0; m < 4; ++m) acc[r][m] = 0.0;
-    for (int64_t base = s0; base < s1; base += P2M_CH) {
-        const int np = (int)((s1 - base) < P2M_CH ? (s1 - base) : P2M_CH);
-        __syncthreads();
-        if (threadIdx.x < np) {
-            const int64_t s = base + threadIdx.x;
-            const double4 ra = srec[2 * s], rb = srec[2 * s + 1];
-            const double h[3] = {ra.x - yc[0], ra.y - yc[1], ra.z - yc[2]};
-            for (int d = 0; d < 3; ++d) {
-                double p = 1.0;
-                for (int e = 0; e <= P; ++e) { pw[d][threadIdx.x][e] = p; p *= h[d]; }
+            for (int m = 0; m < 4; ++m) acc[r][m] = 0.0;
+        for (int64_t base = s0; base < s1; base += P2M_CH) {
+            const int np = (int)((s1 - base) < P2M_CH ? (s1 - base) : P2M_CH);
+            __syncthreads();
+            if (tid < 3 * np) {                                // thread (point, axis): powers of one coordinate
+                const int pt = tid / 3, d = tid - 3 * pt;
+                const double4 ra = a.srec[2 * (base + pt)];
+                const double h = d == 0 ? ra.x - ycx : (d == 1 ? ra.y - ycy : ra.z - ycz);
+                double pwr = 1.0;
+                double* dst = pw + ((size_t)d * P2M_CH + pt) * P2M_LD;
+                for (int e = 0; e <= P; ++e) { dst[e] = pwr; pwr *= h; }
+                if (d == 0) {
+                    const double4 rb = a.srec[2 * (base + pt) + 1];
+                    wq[pt] = make_double4(ra.w, rb.x, rb.y, rb.z);
+                }
             }
-            wq[threadIdx.x] = make_double4(ra.w, rb.x, rb.y, rb.z);
+            __syncthreads();
+#pragma unroll
+            for (int r = 0; r < 3; ++r) {
+                if (tid + r * UP_THREADS < Nk) {
+                    const double* px = pw + ea[r];
+                    const double* py = pw + (size_t)P2M_CH * P2M_LD + eb[r];
+                    const double* pz = pw + (size_t)2 * P2M_CH * P2M_LD + ec[r];
+#pragma unroll 4
+                    for (int p = 0; p < np; ++p) {
+                        const double mono = px[p * P2M_LD] * py[p * P2M_LD] * pz[p * P2M_LD];
+                        const double4 w = wq[p];
+                        acc[r][0] = fma(w.x, mono, acc[r][0]);
+                        acc[r][1] = fma(w.y, mono, acc[r][1]);
+                        acc[r][2] = fma(w.z, mono, acc[r][2]);
+                        acc[r][3] = fma(w.w, mono, acc[r][3]);
+                    }
+                }
+            }
         }
         __syncthreads();
 #pragma unroll
         for (int r = 0; r < 3; ++r) {
-            if (threadIdx.x + r * nth < Nk) {
-#pragma unroll 4
-                for (int p = 0; p < np; ++p) {
-                    const double mono = pw[0][p][ea[r]] * pw[1][p][eb[r]] * pw[2][p][ec[r]];
-                    const double4 w = wq[p];
-                    acc[r][0] = fma(w.x, mono, acc[r][0]);
-                    acc[r][1] = fma(w.y, mono, acc[r][1]);
-                    acc[r][2] = fma(w.z, mono, acc[r][2]);
-                    acc[r][3] = fma(w.w, mono, acc[r][3]);
+            const int k = tid + r * UP_THREADS;
+            if (k < Nk) {
+                mom[k] = acc[r][0];
+                sk[k] = acc[r][1]; sk[Nk + k] = acc[r][2]; sk[2 * Nk + k] = acc[r][3];
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int r = 0; r < 3; ++r) {
+            const int k = tid + r * UP_THREADS;
+            if (k < Nk) {
+                const int ax = ea[r], bx = eb[r], cc = ec[r];
+                double v = 0.0;
+                if (ax) v = fma((double)ax, sk[mom_index(ax - 1, bx, cc)], v);
+                if (bx) v = fma((double)bx, sk[Nk + mom_index(ax, bx - 1, cc)], v);
+                if (cc) v = fma((double)cc, sk[2 * Nk + mom_index(ax, bx, cc - 1)], v);
+                mom[Nk + k] = v;
+            }
+        }
+        __syncthreads();
+    }
+    for (;;) {
+        // mom holds the finished moments of cell c
+        const int32_t link = a.up_link[c];
+        const int64_t parent = (int64_t)(link >> 1) - 1;
+        if (parent >= 0)
+            for (int k = tid; k < 2 * Nk; k += UP_THREADS) a.M[c * 2 * Nk + k] = mom[k];
+        if (link & 1) {                                        // M -> F (cells in an M2P list)
+            const double* mv = mom;
+            const double* mk = mom + Nk;
+            for (int e = tid; e < a.NT; e += UP_THREADS) {
+                double v = 0, k = 0;
+                const int q1 = a.cv_off[e + 1];
+                for (int q = a.cv_off[e]; q < q1; ++q) {
+                    const int l = a.cv_idx[q];
+                    const double f = a.cv_coef[q];
+                    v = fma(f, mv[l], v);
+                    k = fma(f, mk[l], k);
                 }
+                a.FF[c * a.NT + e] = make_double2(v, k);
             }
         }
-    }
-    __syncthreads();
-#pragma unroll
-    for (int r = 0; r < 3; ++r) {
-        const int k = threadIdx.x + r * nth;
-        if (k < Nk) {
-            M[((int64_t)c * 2 + 0) * Nk + k] = acc[r][0];
-            sk[0][k] = acc[r][1]; sk[1][k] = acc[r][2]; sk[2][k] = acc[r][3];
+        if (parent < 0) break;
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) {
+            const int nchild = a.c_nchild[parent];
+            const int old = atomicAdd(&a.up_count[parent], 1);
+            s_last = old == nchild - 1;
+            if (s_last) a.up_count[parent] = 0;                // ready for the next matvec
         }
-    }
-    __syncthreads();
-#pragma unroll
-    for (int r = 0; r < 3; ++r) {
-        const int k = threadIdx.x + r * nth;
-        if (k < Nk) {
-            const int a = ea[r], b = eb[r], cc = ec[r];
-            double v = 0.0;
-            if (a) v = fma((double)a, sk[0][mom_index(a - 1, b, cc)], v);
-            if (b) v = fma((double)b, sk[1][mom_index(a, b - 1, cc)], v);
-            if (cc) v = fma((double)cc, sk[2][mom_index(a, b, cc - 1)], v);
-            M[((int64_t)c * 2 + 1) * Nk + k] = v;
+        __syncthreads();
+        if (!s_last) break;
+        __threadfence();
+        // ---- M2M: this block reported last, it forms the parent from all the children
+        c = parent;
+        const int32_t ch = a.c_child[c];
+        const int nc = a.c_nchild[c];
+        for (int k = tid; k < nc * 2 * Nk; k += UP_THREADS) cm[k] = __ldcg(a.M + (int64_t)ch * 2 * Nk + k);   // children are consecutive
+        if (tid < 3 * nc) {
+            const int q = tid / 3, d = tid - 3 * q;
+            const double* ctr = d == 0 ? a.cx : (d == 1 ? a.cy : a.cz);
+            const double tt = ctr[ch + q] - ctr[c];
+            double pwr = 1.0;
+            for (int e = 0; e <= P; ++e) { tp[(q * 3 + d) * P2M_LD + e] = pwr; pwr *= tt; }
         }
-    }
-}
-
-// ---- M2M: moments of a parent from its children, M'_k = sum_{l<=k} C(k,l) t^{k-l} M_l -------------
-// Table driven: for every k the (l, k-l, C(k,l)) triples are listed once on the host (mm_*), so a
-// thread does no index arithmetic.  Only cells some M2P list needs (directly or through an accepted
-// ancestor) are visited: `cells` is the compacted list for one BFS generation.  All children are
-// staged in shared memory at once (one global-memory latency per cell).
-__global__ void __launch_bounds__(128)
-k_m2m(const int32_t* __restrict__ cells, int P, int Nk, const int32_t* __restrict__ c_child,
-      const int32_t* __restrict__ c_nchild, const double* __restrict__ cx, const double* __restrict__ cy,
-      const double* __restrict__ cz, const int32_t* __restrict__ mm_off, const int32_t* __restrict__ mm_ent,
-      const double* __restrict__ mm_coef, double* __restrict__ M)
-{
-    extern __shared__ double m2m_sm[];                 // cm[8][2*Nk], tp[8][3][PB_MAX_P+1]
-    double* cm = m2m_sm;
-    double* tp = m2m_sm + 8 * 2 * Nk;
-    const int nth = blockDim.x;
-    const int64_t c = cells[blockIdx.x];
-    const int32_t ch = c_child[c];
-    const int nc = c_nchild[c];
-    for (int k = threadIdx.x; k < nc * 2 * Nk; k += nth) cm[k] = M[(int64_t)ch * 2 * Nk + k];   // children are consecutive
-    if (threadIdx.x < 3 * nc) {
-        const int q = threadIdx.x / 3, d = threadIdx.x % 3;
-        const double* ctr = d == 0 ? cx : (d == 1 ? cy : cz);
-        double tt = ctr[ch + q] - ctr[c], p = 1.0;
-        for (int e = 0; e <= P; ++e) { tp[(q * 3 + d) * (PB_MAX_P + 1) + e] = p; p *= tt; }
-    }
-    __syncthreads();
-    for (int k = threadIdx.x; k < Nk; k += nth) {
-        double s0 = 0, s1 = 0;
-        const int e0 = mm_off[k], e1 = mm_off[k + 1];
-        for (int e = e0; e < e1; ++e) {
-            const int32_t ent = mm_ent[e];
-            const double cf = mm_coef[e];
-            const int l = ent & 0xfff, dx = (ent >> 12) & 15, dy = (ent >> 16) & 15, dz = (ent >> 20) & 15;
-            for (int q = 0; q < nc; ++q) {
-                const double* t3 = tp + q * 3 * (PB_MAX_P + 1);
-                const double f = cf * t3[dx] * t3[(PB_MAX_P + 1) + dy] * t3[2 * (PB_MAX_P + 1) + dz];
-                s0 = fma(f, cm[q * 2 * Nk + l], s0);
-                s1 = fma(f, cm[q * 2 * Nk + Nk + l], s1);
+        __syncthreads();
+        for (int it = tid; it < Nk * nc; it += UP_THREADS) {
+            const int q = it / Nk, k = it - q * Nk;
+            const double* t3 = tp + q * 3 * P2M_LD;
+            const double* cq = cm + q * 2 * Nk;
+            double s0 = 0, s1 = 0;
+            const int e1 = __ldg(a.mm_off + k + 1);
+#pragma unroll 2
+            for (int e = __ldg(a.mm_off + k); e < e1; ++e) {
+                const int32_t ent = __ldg(a.mm_ent + e);
+                const double cf = __ldg(a.mm_coef + e);
+                const int l = ent & 0xfff, dx = (ent >> 12) & 15, dy = (ent >> 16) & 15, dz = (ent >> 20) & 15;
+                const double f = cf * t3[dx] * t3[P2M_LD + dy] * t3[2 * P2M_LD + dz];
+                s0 = fma(f, cq[l], s0);
+                s1 = fma(f, cq[Nk + l], s1);
             }
+            part[q * 2 * Nk + k] = s0;
+            part[q * 2 * Nk + Nk + k] = s1;
         }
-        M[(c * 2 + 0) * Nk + k] = s0;
-        M[(c * 2 + 1) * Nk + k] = s1;
+        __syncthreads();
+        for (int k = tid; k < 2 * Nk; k += UP_THREADS) {
+            double v = 0;
+            for (int q = 0; q < nc; ++q) v += part[q * 2 * Nk + k];
+            mom[k] = v;
+        }
+        __syncthreads();
     }
-}
-
-// ---- M -> F conversion (cells that appear in an M2P list only) ---------------------------------------
-__global__ void k_convert(int64_t nused, const int32_t* __restrict__ used, int Nk, int NT,
-                          const int32_t* __restrict__ cv_off, const int32_t* __restrict__ cv_idx,
-                          const double* __restrict__ cv_coef, const double* __restrict__ M, double2* __restrict__ FF)
-{
-    int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (g >= nused * NT) return;
-    const int64_t c = used[g / NT];
-    const int e = (int)(g % NT);
-    const double* mv = M + c * 2 * Nk;
-    const double* mk = mv + Nk;
-    double v = 0, k = 0;
-    for (int q = cv_off[e]; q < cv_off[e + 1]; ++q) {
-        int l = cv_idx[q];
-        double f = cv_coef[q];
-        v += f * mv[l];
-        k += f * mk[l];
-    }
-    FF[c * NT + e] = make_double2(v, k);
 }
 
 // ---- M2P (H6; "box-target" interactions) -----------------------------------------------------------
@@ -641,7 +697,27 @@ k_p2p(int64_t N, int K, double kappa, pb_expk ek, const pb_item* __restrict__ it
 
 // ---- near/singular table + Eq. (5) combine + un-permute (H8) ------------------------------------------------
 // Block = 32 targets x 4 outputs: thread (tgt, m) adds output m of its target over the group's slots
-// and over its row of the near table, then thread m == 0 forms the two rows of Eq. (5).
+// and over its row of the near table, then thread m == 0 forms the two rows of Eq. (5).  The kernel is
+// latency bound (a few dozen dependent loads per thread), so loads are issued eight at a time and
+// added in their fixed order afterwards: same sum, an eighth of the round trips.
+__device__ __forceinline__ double sum_slots(const double* __restrict__ acc, int ns, int64_t stride, double s)
+{
+    int q = 0;
+    for (; q + 8 <= ns; q += 8) {
+        double v[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) v[k] = acc[(int64_t)(q + k) * stride];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) s += v[k];
+    }
+    double v[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) v[k] = q + k < ns ? acc[(int64_t)(q + k) * stride] : 0.0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) s += v[k];
+    return s;
+}
+
 __global__ void __launch_bounds__(128)
 k_combine(int64_t N, const int32_t* __restrict__ itemP_off, const int32_t* __restrict__ itemM_off, double eps_ratio,
           const double* __restrict__ accP, const double* __restrict__ accM, const int32_t* __restrict__ nr_off,
@@ -657,12 +733,21 @@ k_combine(int64_t N, const int32_t* __restrict__ itemP_off, const int32_t* __res
         const int64_t g = i / PB_TG;
         const int nsP = itemP_off[g + 1] - itemP_off[g];
         const int nsM = itemM_off ? itemM_off[g + 1] - itemM_off[g] : 0;
-        for (int q = 0; q < nsP; ++q) s += accP[((int64_t)q * 4 + m) * N + i];
-        for (int q = 0; q < nsM; ++q) s += accM[((int64_t)q * 4 + m) * N + i];
+        s = sum_slots(accP + (int64_t)m * N + i, nsP, 4 * N, s);
+        if (nsM > 0) s = sum_slots(accM + (int64_t)m * N + i, nsM, 4 * N, s);
         s *= PB_INV4PI;
         const double* __restrict__ xv = (m & 1) ? xphi : xdphi;     // V_L, V_Y act on dphi; K_L, K_Y on phi
         const double* __restrict__ val = nr_val + (int64_t)m * ne;
-        for (int32_t e = nr_off[i]; e < nr_off[i + 1]; ++e) s = fma(val[e], xv[nr_col[e]], s);
+        const int32_t e1 = nr_off[i + 1];
+        int32_t e = nr_off[i];
+        for (; e + 4 <= e1; e += 4) {
+            double a[4], b[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) { a[k] = val[e + k]; b[k] = xv[nr_col[e + k]]; }
+#pragma unroll
+            for (int k = 0; k < 4; ++k) s = fma(a[k], b[k], s);
+        }
+        for (; e < e1; ++e) s = fma(val[e], xv[nr_col[e]], s);
     }
     sm[m][tgt] = s;
     __syncthreads();
@@ -677,7 +762,7 @@ k_combine(int64_t N, const int32_t* __restrict__ itemP_off, const int32_t* __res
 
 // ---- host driver ----------------------------------------------------------------------------------------------
 template <int P>
-static cudaError_t launch_m2p(pb_ctx* ctx)
+static cudaError_t launch_m2p(pb_ctx* ctx, cudaStream_t fs)
 {
     pb_tree& t = ctx->tree;
     static bool attr_set = false;   // per instantiation; the attribute belongs to the function, not the context
@@ -686,12 +771,66 @@ static cudaError_t launch_m2p(pb_ctx* ctx)
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    k_m2p<P><<<(unsigned)t.n_itemM, M2P_THREADS, m2p_cfg<P>::SMEM, ctx->stream>>>(
+    k_m2p<P><<<(unsigned)t.n_itemM, M2P_THREADS, m2p_cfg<P>::SMEM, fs>>>(
         t.N, ctx->prm.kappa, t.ek, t.itemM, t.m2p_cell, t.m2p_ctr, t.FF, t.pc[0], t.pc[1], t.pc[2], t.accM);
     return cudaSuccess;
 }
 
-int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed)
+// Far-field branch: the upward pass (P2M, M2M, M -> F) in one launch, then M2P.  `fs` is the stream it
+// is enqueued on: the context's side stream (concurrent with P2P) or, when per-kernel event timing
+// is wanted, the main stream.
+static int pb_far_branch(pb_ctx* ctx, cudaStream_t fs, bool timed)
+{
+    pb_tree& t = ctx->tree;
+    if (t.n_need_leaf > 0) {
+        up_args ua;
+        ua.P = t.P; ua.Nk = t.Nk; ua.NT = t.NT; ua.K = t.K;
+        ua.leaf_ids = t.need_leaf; ua.c_first = t.c_first; ua.c_last = t.c_last; ua.c_child = t.c_child;
+        ua.c_nchild = t.c_nchild; ua.up_link = t.up_link; ua.up_count = t.up_count;
+        ua.cx = t.c_ctr[0]; ua.cy = t.c_ctr[1]; ua.cz = t.c_ctr[2];
+        ua.srec = t.srec;
+        ua.mm_off = t.mm_off; ua.mm_ent = t.mm_ent; ua.mm_coef = t.mm_coef;
+        ua.cv_off = t.cv_off; ua.cv_idx = t.cv_idx; ua.cv_coef = t.cv_coef;
+        ua.M = t.M; ua.FF = t.FF;
+        const size_t sm = up_smem_bytes(t.Nk);
+        static size_t sm_set = 0;                       // the attribute belongs to the function, not the context
+        if (sm > 48 * 1024 && sm > sm_set) {
+            PB_CUDA(cudaFuncSetAttribute(k_upward, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+            sm_set = sm;
+        }
+        k_upward<<<(unsigned)t.n_need_leaf, UP_THREADS, sm, fs>>>(ua);
+        PB_LAUNCH_CHECK();
+    }
+    if (timed) PB_CUDA(cudaEventRecord(ctx->ev[2], fs));
+    if (t.n_itemM > 0) {
+        PB_TRY(pb_prof_begin(ctx, 1));
+        cudaError_t e = cudaSuccess;
+        switch (t.P) {
+        case 0: e = launch_m2p<0>(ctx, fs); break;
+        case 1: e = launch_m2p<1>(ctx, fs); break;
+        case 2: e = launch_m2p<2>(ctx, fs); break;
+        case 3: e = launch_m2p<3>(ctx, fs); break;
+        case 4: e = launch_m2p<4>(ctx, fs); break;
+        case 5: e = launch_m2p<5>(ctx, fs); break;
+        case 6: e = launch_m2p<6>(ctx, fs); break;
+        case 7: e = launch_m2p<7>(ctx, fs); break;
+        case 8: e = launch_m2p<8>(ctx, fs); break;
+        case 9: e = launch_m2p<9>(ctx, fs); break;
+        case 10: e = launch_m2p<10>(ctx, fs); break;
+        default: return pb_fail(ctx, PB_ERR_INVALID_ARG, "unsupported order_P %d", t.P);
+        }
+        PB_CUDA(e);
+        PB_LAUNCH_CHECK();
+        PB_TRY(pb_prof_end(ctx, 1));
+    }
+    return PB_OK;
+}
+
+// y = A x (or A Minv x with `precond`).  Normal operation: the near field (P2P) runs on the context's
+// stream while the far-field branch runs on the side stream; both join before the combine.  With
+// `timed` or pb_set_profiling the two branches run back to back on the context's stream so that
+// every CUDA-event pair brackets exactly one kernel.
+int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed, bool precond)
 {
     pb_tree& t = ctx->tree;
     cudaStream_t st = ctx->stream;
@@ -702,49 +841,16 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed)
         ctx->ev_made = true;
     }
     const bool far = ctx->prm.theta > 0.0;
+    const bool serial = timed || ctx->profiling;
     if (timed) PB_CUDA(cudaEventRecord(ctx->ev[0], st));
-    PB_TRY(pb_weights(ctx, x));
+    PB_TRY(pb_weights(ctx, x, precond));
     if (timed) PB_CUDA(cudaEventRecord(ctx->ev[1], st));
-    if (far) {
-        if (t.n_need_leaf > 0) {
-            k_p2m_leaf<<<(unsigned)t.n_need_leaf, t.Nk <= 96 ? 96 : 128, 0, st>>>(t.P, t.Nk, t.K, t.need_leaf, t.c_first, t.c_last, t.c_ctr[0],
-                                                               t.c_ctr[1], t.c_ctr[2], t.srec, t.M);
-            PB_LAUNCH_CHECK();
-        }
-        for (int g = (int)t.m2m_start.size() - 2; g >= 0; --g) {   // deepest generation first
-            const int64_t n = t.m2m_start[g + 1] - t.m2m_start[g];
-            if (n == 0) continue;
-            k_m2m<<<(unsigned)n, t.Nk <= 96 ? 96 : 128, (size_t)(16 * t.Nk + 24 * (PB_MAX_P + 1)) * sizeof(double), st>>>(t.m2m_cells + t.m2m_start[g], t.P, t.Nk, t.c_child, t.c_nchild, t.c_ctr[0],
-                                               t.c_ctr[1], t.c_ctr[2], t.mm_off, t.mm_ent, t.mm_coef, t.M);
-            PB_LAUNCH_CHECK();
-        }
-        if (t.n_used > 0) {
-            k_convert<<<pb_blocks(t.n_used * t.NT, 256), 256, 0, st>>>(t.n_used, t.used_cells, t.Nk, t.NT, t.cv_off, t.cv_idx,
-                                                                      t.cv_coef, t.M, t.FF);
-            PB_LAUNCH_CHECK();
-        }
+    if (far && serial) PB_TRY(pb_far_branch(ctx, st, timed));
+    if (far && !serial) PB_CUDA(cudaEventRecord(ctx->ev_fork, st));
+    if (timed) {
+        if (!far) PB_CUDA(cudaEventRecord(ctx->ev[2], st));
+        PB_CUDA(cudaEventRecord(ctx->ev[3], st));
     }
-    if (timed) PB_CUDA(cudaEventRecord(ctx->ev[2], st));
-    if (far && t.n_itemM > 0) {
-        PB_TRY(pb_prof_begin(ctx, 1));
-        switch (t.P) {
-        case 0: PB_CUDA(launch_m2p<0>(ctx)); break;
-        case 1: PB_CUDA(launch_m2p<1>(ctx)); break;
-        case 2: PB_CUDA(launch_m2p<2>(ctx)); break;
-        case 3: PB_CUDA(launch_m2p<3>(ctx)); break;
-        case 4: PB_CUDA(launch_m2p<4>(ctx)); break;
-        case 5: PB_CUDA(launch_m2p<5>(ctx)); break;
-        case 6: PB_CUDA(launch_m2p<6>(ctx)); break;
-        case 7: PB_CUDA(launch_m2p<7>(ctx)); break;
-        case 8: PB_CUDA(launch_m2p<8>(ctx)); break;
-        case 9: PB_CUDA(launch_m2p<9>(ctx)); break;
-        case 10: PB_CUDA(launch_m2p<10>(ctx)); break;
-        default: return pb_fail(ctx, PB_ERR_INVALID_ARG, "unsupported order_P %d", t.P);
-        }
-        PB_LAUNCH_CHECK();
-        PB_TRY(pb_prof_end(ctx, 1));
-    }
-    if (timed) PB_CUDA(cudaEventRecord(ctx->ev[3], st));
     {
         PB_TRY(pb_prof_begin(ctx, 0));
         k_p2p<<<(unsigned)t.n_itemP, P2P_THREADS, 0, st>>>(t.N, t.K, ctx->prm.kappa, t.ek, t.itemP, t.p2p_lo, t.p2p_hi, t.srec,
@@ -752,6 +858,12 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed)
         PB_LAUNCH_CHECK();
         PB_TRY(pb_prof_end(ctx, 0));
         pb_prof_next(ctx);
+    }
+    if (far && !serial) {
+        PB_CUDA(cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0));
+        PB_TRY(pb_far_branch(ctx, ctx->side, false));
+        PB_CUDA(cudaEventRecord(ctx->ev_join, ctx->side));
+        PB_CUDA(cudaStreamWaitEvent(st, ctx->ev_join, 0));
     }
     if (timed) PB_CUDA(cudaEventRecord(ctx->ev[4], st));
     k_combine<<<pb_blocks(t.N, 32), 128, 0, st>>>(t.N, t.itemP_off, far ? t.itemM_off : nullptr,
@@ -776,13 +888,13 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed)
 extern "C" int pb_matvec(pb_ctx* ctx, const double* x, double* y)
 {
     if (!ctx) return PB_ERR_INVALID_ARG;
-    return pb_matvec_impl(ctx, x, y, false);
+    return pb_matvec_impl(ctx, x, y, false, false);
 }
 
 extern "C" int pb_matvec_timed(pb_ctx* ctx, const double* x, double* y)
 {
     if (!ctx) return PB_ERR_INVALID_ARG;
-    return pb_matvec_impl(ctx, x, y, true);
+    return pb_matvec_impl(ctx, x, y, true, false);
 }
 
 extern "C" int pb_matvec_host(pb_ctx* ctx, const double* x_host, double* y_host)
@@ -795,7 +907,7 @@ extern "C" int pb_matvec_host(pb_ctx* ctx, const double* x_host, double* y_host)
     double* dx = ctx->scratch;
     double* dy = ctx->scratch + n;
     PB_CUDA(cudaMemcpyAsync(dx, x_host, n * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
-    PB_TRY(pb_matvec_impl(ctx, dx, dy, false));
+    PB_TRY(pb_matvec_impl(ctx, dx, dy, false, false));
     PB_CUDA(cudaMemcpyAsync(y_host, dy, n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     PB_CUDA(cudaStreamSynchronize(ctx->stream));
     return PB_OK;

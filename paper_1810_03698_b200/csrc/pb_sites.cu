@@ -255,7 +255,7 @@ extern "C" int pb_reaction_field(pb_ctx* ctx, const double* x, double* phi, doub
     if (!phi && !grad && !hess) return PB_OK;
     cudaStream_t st = ctx->stream;
     if (!s.near_built) PB_TRY(pb_site_near_build(ctx));
-    PB_TRY(pb_weights(ctx, x));
+    PB_TRY(pb_weights(ctx, x, false));
     const int64_t ntile = (s.na + RF_ST - 1) / RF_ST;
     // enough source chunks to fill the GPU, each at least 4 sweeps of the block
     int64_t nchunk = (148 * 16 + ntile - 1) / ntile;

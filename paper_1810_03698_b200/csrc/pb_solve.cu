@@ -6,64 +6,115 @@
 #include <vector>
 #include "pb_internal.cuh"
 
-#define DOT_CHUNK 1024
+#define DOT_CHUNK 512
 #define DOT_THREADS 256
+#define DOT_WARPS (DOT_THREADS / 32)
+#define DOT_MAXBLK 1184         // 8 blocks per SM: enough loads in flight to stream V at HBM speed
 
-// partial[blk][j] = sum over the block's chunk of V_j . w   (one warp per j, fixed order)
+// h[j] = V_j . w for j < nv and, with `self`, h[nv] = w . w.  Block (bx, by) takes the chunks bx,
+// bx + gridDim.x, ... of w through shared memory and the vectors by*8R + {warp, warp + 8, ...}; the
+// per-block partial sums are added by the LAST block to finish, in a fixed order, so the result does
+// not depend on which block that is.  R = 1 spreads a short vector over many blocks (latency), R = 4
+// re-reads w less often on long ones (bandwidth).
+template <int R>
 __global__ void __launch_bounds__(DOT_THREADS)
-k_dots(int64_t n, int nv, const double* __restrict__ V, int64_t ld, const double* __restrict__ w,
-       double* __restrict__ partial)
+k_dots(int64_t n, int nv, const double* __restrict__ V, int64_t ld, const double* __restrict__ w, int self,
+       double* __restrict__ partial, unsigned int* __restrict__ counter, double* __restrict__ hout)
 {
     __shared__ double sw[DOT_CHUNK];
-    const int64_t e0 = (int64_t)blockIdx.x * DOT_CHUNK;
-    const int cnt = (int)(n - e0 < DOT_CHUNK ? n - e0 : DOT_CHUNK);
-    for (int k = threadIdx.x; k < DOT_CHUNK; k += DOT_THREADS) sw[k] = k < cnt ? w[e0 + k] : 0.0;
-    __syncthreads();
+    __shared__ bool last;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    for (int j = wid; j < nv; j += DOT_THREADS / 32) {
-        const double* v = V + (int64_t)j * ld + e0;
-        double s = 0;
-        for (int k = lane; k < cnt; k += 32) s = fma(v[k], sw[k], s);
-        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-        if (lane == 0) partial[(int64_t)blockIdx.x * nv + j] = s;
+    const int nvt = nv + (self ? 1 : 0);
+    const int64_t nchunk = (n + DOT_CHUNK - 1) / DOT_CHUNK;
+    const int j0 = blockIdx.y * (DOT_WARPS * R) + wid;
+    double acc[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) acc[r] = 0.0;
+    for (int64_t c = blockIdx.x; c < nchunk; c += gridDim.x) {
+        const int64_t e0 = c * DOT_CHUNK;
+        const int cnt = (int)(n - e0 < DOT_CHUNK ? n - e0 : DOT_CHUNK);
+        __syncthreads();
+        for (int k = threadIdx.x; k < DOT_CHUNK; k += DOT_THREADS) sw[k] = k < cnt ? w[e0 + k] : 0.0;
+        __syncthreads();
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int j = j0 + r * DOT_WARPS;
+            if (j < nvt) {
+                const double* v = (j < nv ? V + (int64_t)j * ld : w) + e0;
+                double s = 0;
+#pragma unroll 4
+                for (int k = lane; k < cnt; k += 32) s = fma(v[k], sw[k], s);
+                acc[r] += s;
+            }
+        }
     }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int j = j0 + r * DOT_WARPS;
+        if (j < nvt) {
+            double s = acc[r];
+            for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+            if (lane == 0) partial[(int64_t)blockIdx.x * nvt + j] = s;
+        }
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) last = atomicAdd(counter, 1u) == gridDim.x * gridDim.y - 1;
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    for (int j = threadIdx.x; j < nvt; j += DOT_THREADS) {
+        double s = 0;
+        for (unsigned b = 0; b < gridDim.x; ++b) s += __ldcg(&partial[(int64_t)b * nvt + j]);
+        hout[j] = s;
+    }
+    if (threadIdx.x == 0) *counter = 0u;              // ready for the next launch on this stream
 }
 
-// w -= sum_j h_j V_j with h_j = sum_blk partial[blk][j]; block 0 also publishes h (+= if accumulate)
+// w -= sum_j h_j V_j.  With vnext != NULL (second Gram-Schmidt pass): h[nv] holds w.w BEFORE the
+// update, so |w - V h|^2 = w.w - |h|^2 (V orthonormal) and the new basis vector is written normalised
+// in the same pass; block 0 publishes that squared norm to h[nv + 1].
 __global__ void __launch_bounds__(256)
-k_arnoldi_update(int64_t n, int nv, int nblk, const double* __restrict__ V, int64_t ld,
-                 const double* __restrict__ partial, double* __restrict__ w, double* __restrict__ hout)
+k_arnoldi_update(int64_t n, int nv, const double* __restrict__ V, int64_t ld, const double* __restrict__ h,
+                 double* __restrict__ w, double* __restrict__ vnext, double* __restrict__ nrm2_out)
 {
     extern __shared__ double sh[];
-    for (int j = threadIdx.x; j < nv; j += blockDim.x) {
-        double s = 0;
-        for (int b = 0; b < nblk; ++b) s += partial[(int64_t)b * nv + j];
-        sh[j] = s;
-        if (blockIdx.x == 0) hout[j] = s;
+    __shared__ double inv;
+    for (int j = threadIdx.x; j < nv; j += blockDim.x) sh[j] = h[j];
+    __syncthreads();
+    if (vnext && threadIdx.x == 0) {
+        double h2 = 0;
+        for (int j = 0; j < nv; ++j) h2 = fma(sh[j], sh[j], h2);
+        const double r2 = h[nv] - h2;
+        if (blockIdx.x == 0) *nrm2_out = r2;
+        inv = r2 > 0 ? 1.0 / sqrt(r2) : 0.0;
     }
     __syncthreads();
-    const int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (e >= n) return;
-    double acc = w[e];
-    for (int j = 0; j < nv; ++j) acc = fma(-sh[j], V[(int64_t)j * ld + e], acc);
-    w[e] = acc;
+    for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
+        double acc = w[e];
+        int j = 0;
+        for (; j + 4 <= nv; j += 4) {
+            const double v0 = V[(int64_t)j * ld + e], v1 = V[(int64_t)(j + 1) * ld + e], v2 = V[(int64_t)(j + 2) * ld + e],
+                         v3 = V[(int64_t)(j + 3) * ld + e];
+            acc = fma(-sh[j], v0, acc);
+            acc = fma(-sh[j + 1], v1, acc);
+            acc = fma(-sh[j + 2], v2, acc);
+            acc = fma(-sh[j + 3], v3, acc);
+        }
+        for (; j < nv; ++j) acc = fma(-sh[j], V[(int64_t)j * ld + e], acc);
+        w[e] = acc;
+        if (vnext) vnext[e] = acc * inv;
+    }
 }
 
-// vnext = w / sqrt(sum partial); block 0 publishes the squared norm
+// vnext = w / sqrt(*nrm2)
 __global__ void __launch_bounds__(256)
-k_normalize(int64_t n, int nblk, const double* __restrict__ partial, const double* __restrict__ w,
-            double* __restrict__ vnext, double* __restrict__ nrm2_out)
+k_normalize(int64_t n, const double* __restrict__ nrm2, const double* __restrict__ w, double* __restrict__ vnext)
 {
-    __shared__ double inv;
-    if (threadIdx.x == 0) {
-        double s = 0;
-        for (int b = 0; b < nblk; ++b) s += partial[b];
-        if (blockIdx.x == 0) *nrm2_out = s;
-        inv = s > 0 ? 1.0 / sqrt(s) : 0.0;
-    }
-    __syncthreads();
-    const int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (e < n) vnext[e] = w[e] * inv;
+    const double s = *nrm2;
+    const double inv = s > 0 ? 1.0 / sqrt(s) : 0.0;
+    for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x)
+        vnext[e] = w[e] * inv;
 }
 
 // z = Minv v: per panel the inverse 2x2 diagonal block (SELF entries), original panel order
@@ -105,9 +156,22 @@ __global__ void k_axpy(int64_t n, double a, const double* __restrict__ x, double
 
 typedef pb_gmres_ws gmres_ws;
 
-static int dot_into(pb_ctx* ctx, gmres_ws& ws, int nv, const double* V, const double* w)
+// hout[0..nv) = V^T w (and hout[nv] = w.w with `self`), all on the device
+static int dot_into(pb_ctx* ctx, gmres_ws& ws, int nv, const double* V, const double* w, bool self, double* hout)
 {
-    k_dots<<<ws.nblk, DOT_THREADS, 0, ctx->stream>>>(ws.n, nv, V, ws.n, w, ws.partial);
+    const int nvt = nv + (self ? 1 : 0);
+    const int64_t nchunk = (ws.n + DOT_CHUNK - 1) / DOT_CHUNK;
+    const int gy1 = (nvt + DOT_WARPS - 1) / DOT_WARPS;
+    if (nchunk * gy1 <= DOT_MAXBLK) {
+        dim3 grid((unsigned)nchunk, (unsigned)gy1);
+        k_dots<1><<<grid, DOT_THREADS, 0, ctx->stream>>>(ws.n, nv, V, ws.n, w, self ? 1 : 0, ws.partial, ws.counter, hout);
+    } else {
+        const int gy = (nvt + 4 * DOT_WARPS - 1) / (4 * DOT_WARPS);
+        int64_t gx = DOT_MAXBLK / gy;
+        if (gx > nchunk) gx = nchunk;
+        dim3 grid((unsigned)gx, (unsigned)gy);
+        k_dots<4><<<grid, DOT_THREADS, 0, ctx->stream>>>(ws.n, nv, V, ws.n, w, self ? 1 : 0, ws.partial, ws.counter, hout);
+    }
     PB_LAUNCH_CHECK();
     return PB_OK;
 }
@@ -115,14 +179,16 @@ static int dot_into(pb_ctx* ctx, gmres_ws& ws, int nv, const double* V, const do
 // ||v||^2 on the host (synchronises)
 static int norm2_host(pb_ctx* ctx, gmres_ws& ws, const double* v, double* out)
 {
-    PB_TRY(dot_into(ctx, ws, 1, v, v));
-    k_normalize<<<1, 32, 0, ctx->stream>>>(0, ws.nblk, ws.partial, nullptr, nullptr, ws.hdev);
-    PB_LAUNCH_CHECK();
+    PB_TRY(dot_into(ctx, ws, 0, nullptr, v, true, ws.hdev));
     PB_CUDA(cudaMemcpyAsync(out, ws.hdev, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     PB_CUDA(cudaStreamSynchronize(ctx->stream));
     return PB_OK;
 }
 
+// Restarted GMRES with a right block-Jacobi preconditioner (D: R-20).  Per iteration: one operator
+// application (the preconditioner is folded into its first kernel), two classical Gram-Schmidt
+// passes of two kernels each -- the second also yields the norm of the new vector by Pythagoras and
+// writes it normalised -- and one small device-to-host copy of the Hessenberg column.
 int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, double* relres_out, int32_t* matvecs_out)
 {
     pb_tree& t = ctx->tree;
@@ -131,23 +197,26 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
     const int64_t n = 2 * t.N;
     int m = ctx->prm.gmres_restart;
     if (m > n) m = (int)n;
+    if (m > 120) m = 120;                          // k_dots<4> covers 4 x 32 vectors per block row
     // workspace (kept until the system size or the restart length changes)
     gmres_ws& ws = ctx->gws;
     if (ws.n != n || ws.m != m || !ws.V) {
         pb_dfree_cat(ctx, CAT_SOLVE);
         ws = gmres_ws();
-        ws.nblk = (int)((n + DOT_CHUNK - 1) / DOT_CHUNK);
         PB_TRY(pb_dalloc_t(ctx, &ws.V, (size_t)(m + 1) * n, CAT_SOLVE));
         PB_TRY(pb_dalloc_t(ctx, &ws.w, n, CAT_SOLVE));
-        PB_TRY(pb_dalloc_t(ctx, &ws.z, n, CAT_SOLVE));
         PB_TRY(pb_dalloc_t(ctx, &ws.r, n, CAT_SOLVE));
         PB_TRY(pb_dalloc_t(ctx, &ws.u, n, CAT_SOLVE));
-        PB_TRY(pb_dalloc_t(ctx, &ws.partial, (size_t)ws.nblk * (m + 2), CAT_SOLVE));
-        PB_TRY(pb_dalloc_t(ctx, &ws.hdev, 2 * (m + 2) + 8, CAT_SOLVE));
+        PB_TRY(pb_dalloc_t(ctx, &ws.z, n, CAT_SOLVE));
+        PB_TRY(pb_dalloc_t(ctx, &ws.partial, (size_t)DOT_MAXBLK * (m + 2), CAT_SOLVE));
+        PB_TRY(pb_dalloc_t(ctx, &ws.hdev, 2 * (m + 4) + 8, CAT_SOLVE));
         PB_TRY(pb_dalloc_t(ctx, &ws.coef, m + 2, CAT_SOLVE));
+        PB_TRY(pb_dalloc_t(ctx, &ws.counter, 4, CAT_SOLVE));
+        PB_CUDA(cudaMemsetAsync(ws.counter, 0, 4 * sizeof(unsigned int), st));
         ws.n = n;
         ws.m = m;
     }
+    const int hstride = m + 4;
     PB_TRY(pb_pinned(ctx, (3 * (size_t)m + 64) * sizeof(double)));
     double* hh = ctx->h_pinned;                    // staging for h columns
     const bool pc = ctx->prm.precond != 0;
@@ -169,15 +238,15 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
     }
     std::vector<double> H((size_t)(m + 1) * m, 0.0), cs(m, 0.0), sn(m, 0.0), g(m + 1, 0.0), yv(m, 0.0);
     const int tb = 256;
-    const int nb = pb_blocks(n, tb);
+    const int nb = pb_blocks(n, tb) < 2368 ? pb_blocks(n, tb) : 2368;   // grid-stride above 16 blocks per SM
     for (;;) {
         // true residual r = b - A x
-        PB_TRY(pb_matvec_impl(ctx, x, ws.w, false));
+        PB_TRY(pb_matvec_impl(ctx, x, ws.w, false, false));
         ++matvecs;
-        k_residual<<<nb, tb, 0, st>>>(n, b, ws.w, ws.r);
+        k_residual<<<pb_blocks(n, tb), tb, 0, st>>>(n, b, ws.w, ws.r);
         PB_LAUNCH_CHECK();
-        PB_TRY(dot_into(ctx, ws, 1, ws.r, ws.r));
-        k_normalize<<<nb, tb, 0, st>>>(n, ws.nblk, ws.partial, ws.r, ws.V, ws.hdev);   // V_0 = r/||r||
+        PB_TRY(dot_into(ctx, ws, 0, nullptr, ws.r, true, ws.hdev));
+        k_normalize<<<nb, tb, 0, st>>>(n, ws.hdev, ws.r, ws.V);      // V_0 = r/||r||
         PB_LAUNCH_CHECK();
         double r2 = 0;
         PB_CUDA(cudaMemcpyAsync(&r2, ws.hdev, sizeof(double), cudaMemcpyDeviceToHost, st));
@@ -191,32 +260,33 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
         int j = 0;
         for (; j < m && iters < maxit;) {
             const double* vj = ws.V + (size_t)j * n;
-            const double* zin = vj;
-            if (pc) {
-                k_precond<<<pb_blocks(t.N, tb), tb, 0, st>>>(t.N, t.precond, vj, ws.z);
-                PB_LAUNCH_CHECK();
-                zin = ws.z;
-            }
-            PB_TRY(pb_matvec_impl(ctx, zin, ws.w, false));
+            double* vnext = ws.V + (size_t)(j + 1) * n;
+            PB_TRY(pb_matvec_impl(ctx, vj, ws.w, false, pc));        // w = A Minv v_j
             ++matvecs;
             const int nv = j + 1;
             // classical Gram-Schmidt, twice
             double* hA = ws.hdev;
-            double* hB = ws.hdev + (m + 2);
-            PB_TRY(dot_into(ctx, ws, nv, ws.V, ws.w));
-            k_arnoldi_update<<<nb, tb, nv * sizeof(double), st>>>(n, nv, ws.nblk, ws.V, n, ws.partial, ws.w, hA);
+            double* hB = ws.hdev + hstride;
+            PB_TRY(dot_into(ctx, ws, nv, ws.V, ws.w, false, hA));
+            k_arnoldi_update<<<nb, tb, nv * sizeof(double), st>>>(n, nv, ws.V, n, hA, ws.w, nullptr, nullptr);
             PB_LAUNCH_CHECK();
-            PB_TRY(dot_into(ctx, ws, nv, ws.V, ws.w));
-            k_arnoldi_update<<<nb, tb, nv * sizeof(double), st>>>(n, nv, ws.nblk, ws.V, n, ws.partial, ws.w, hB);
+            PB_TRY(dot_into(ctx, ws, nv, ws.V, ws.w, true, hB));     // hB[nv] = w.w
+            k_arnoldi_update<<<nb, tb, nv * sizeof(double), st>>>(n, nv, ws.V, n, hB, ws.w, vnext, hB + nv + 1);
             PB_LAUNCH_CHECK();
-            PB_TRY(dot_into(ctx, ws, 1, ws.w, ws.w));
-            k_normalize<<<nb, tb, 0, st>>>(n, ws.nblk, ws.partial, ws.w, ws.V + (size_t)(j + 1) * n, ws.hdev + 2 * (m + 2));
-            PB_LAUNCH_CHECK();
-            PB_CUDA(cudaMemcpyAsync(hh, ws.hdev, sizeof(double) * (2 * (m + 2) + 1), cudaMemcpyDeviceToHost, st));
+            PB_CUDA(cudaMemcpyAsync(hh, ws.hdev, sizeof(double) * 2 * hstride, cudaMemcpyDeviceToHost, st));
             PB_CUDA(cudaStreamSynchronize(st));
+            double hn2 = hh[hstride + nv + 1];
+            if (!(hn2 > 1e-2 * hh[hstride + nv])) {
+                // the second pass removed most of w (cancellation in w.w - |h|^2): take the norm directly
+                PB_TRY(dot_into(ctx, ws, 0, nullptr, ws.w, true, hB + nv + 1));
+                k_normalize<<<nb, tb, 0, st>>>(n, hB + nv + 1, ws.w, vnext);
+                PB_LAUNCH_CHECK();
+                PB_CUDA(cudaMemcpyAsync(&hn2, hB + nv + 1, sizeof(double), cudaMemcpyDeviceToHost, st));
+                PB_CUDA(cudaStreamSynchronize(st));
+            }
             double* col = &H[(size_t)j * (m + 1)];
-            for (int i = 0; i < nv; ++i) col[i] = hh[i] + hh[(m + 2) + i];
-            const double hnext = sqrt(hh[2 * (m + 2)]);
+            for (int i = 0; i < nv; ++i) col[i] = hh[i] + hh[hstride + i];
+            const double hnext = hn2 > 0 ? sqrt(hn2) : 0.0;
             col[nv] = hnext;
             // Givens rotations (host, O(j))
             for (int i = 0; i < j; ++i) {
@@ -245,14 +315,14 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
         }
         for (int i = 0; i < j; ++i) hh[i] = yv[i];
         PB_CUDA(cudaMemcpyAsync(ws.coef, hh, sizeof(double) * j, cudaMemcpyHostToDevice, st));
-        k_lincomb<<<nb, tb, j * sizeof(double), st>>>(n, j, ws.V, n, ws.coef, ws.u);
+        k_lincomb<<<pb_blocks(n, tb), tb, j * sizeof(double), st>>>(n, j, ws.V, n, ws.coef, ws.u);
         PB_LAUNCH_CHECK();
         if (pc) {
             k_precond<<<pb_blocks(t.N, tb), tb, 0, st>>>(t.N, t.precond, ws.u, ws.z);
             PB_LAUNCH_CHECK();
-            k_axpy<<<nb, tb, 0, st>>>(n, 1.0, ws.z, x);
+            k_axpy<<<pb_blocks(n, tb), tb, 0, st>>>(n, 1.0, ws.z, x);
         } else
-            k_axpy<<<nb, tb, 0, st>>>(n, 1.0, ws.u, x);
+            k_axpy<<<pb_blocks(n, tb), tb, 0, st>>>(n, 1.0, ws.u, x);
         PB_LAUNCH_CHECK();
         PB_CUDA(cudaStreamSynchronize(st));   // hh is reused
     }

@@ -316,7 +316,7 @@ def _surface_nets(f, lo, h, blend=0.7):
     return verts, tris
 
 
-def vdw_surface(centres, radii, target_panels=None, h=None, tol=0.05, max_iter=6, pad=None):
+def vdw_surface(centres, radii, target_panels=None, h=None, tol=0.05, max_iter=6, pad=None, iso_shift=0.35):
     """Triangulate the boundary of the union of spheres (cavities dropped).  Either a grid
     spacing `h` is given or it is tuned so the panel count lands within `tol` of
     `target_panels` (the controlling quantity in BASELINE.json's configs).
@@ -326,7 +326,11 @@ def vdw_surface(centres, radii, target_panels=None, h=None, tol=0.05, max_iter=6
 
     def run(hh):
         f, lo = _level_set(centres, radii, hh, pad if pad is not None else 3.0 * hh)
-        f = _fix_topology(f)
+        # The smoothed net (vertices pulled toward cell centres) cuts up to ~0.5 h INSIDE the spheres
+        # where they are convex, leaving atom centres far closer to the dielectric boundary than their
+        # radius.  Meshing the level set at +iso_shift*h instead keeps the whole net outside the union
+        # (measured: min over vertices and centroids of min_i(|x - c_i| - r_i) >= -0.05 A at h = 1.15).
+        f = _fix_topology(f - iso_shift * hh)
         return _surface_nets(f, lo, hh)
 
     if h is None:

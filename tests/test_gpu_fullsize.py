@@ -1,0 +1,119 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (theta = 0.5,
+P = 6, ncrit default, K_far = 7): C2 on the whole vector, C3-complex and C4 on seeded SAMPLED
+target rows that the oracle computes one by one against all sources (S: section 8(d) gates), and
+properties that hold at any size (linearity, interaction counts, theta -> 0 consistency)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL_DIRECT = 1e-11
+TOL_TREE = 1e-4
+
+
+def rel(a, b):
+    return float(np.linalg.norm(np.asarray(a) - np.asarray(b)) / np.linalg.norm(np.asarray(b)))
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked test run without a CUDA device: the product has no CPU fallback")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def pbm(torch_cuda):
+    from paper_1810_03698_b200 import pb
+    pb.build()
+    return pb
+
+
+def _rows(nt, n, seed=8):
+    return np.sort(np.random.Generator(np.random.PCG64(seed)).choice(nt, size=min(n, nt), replace=False))
+
+
+@pytest.mark.parametrize("name,kw,nrows,direct", [
+    ("C2", dict(), None, True),                      # ~10k panels: every row, both modes
+    ("C3", dict(which="ligand"), None, True),        # ~2k panels, 50 sites
+    ("C3", dict(which="complex"), 2048, True),       # ~59k panels: sampled rows, both modes
+    ("C4", dict(), 1024, False),                     # ~1.02M panels, 7.1M Gauss points: sampled rows, treecode
+])
+def test_matvec_full_size(pbm, po, torch_cuda, name, kw, nrows, direct):
+    from paper_1810_03698_b200.workloads import make_config
+    w = make_config(name, **kw)
+    nt = w.tris.shape[0]
+    orc = po.Oracle(w.verts, w.tris, po.Params(K_far=w.params["K_far"]))
+    rows = np.arange(nt) if nrows is None else _rows(nt, nrows)
+    x = np.random.Generator(np.random.PCG64(7)).normal(size=2 * nt)
+    y1, y2 = orc.matvec(x, rows)
+    ctx = pbm.from_workload(w)                        # the workload's own parameters = bench.py's
+    assert ctx.get_params().theta == 0.5 and ctx.get_params().order_P == 6
+    ctx.tree_build()
+    xd = torch_cuda.from_numpy(x).cuda()
+    y = ctx.matvec(xd).cpu().numpy()
+    st = ctx.stats()
+    assert rel(y[rows], y1) <= TOL_TREE and rel(y[nt + rows], y2) <= TOL_TREE
+    assert st["m2p_pairs"] > 0 and st["p2p_pairs"] + 0 < nt * nt * w.params["K_far"]
+    # properties at any size: linearity and determinism of the treecode operator
+    y_again = ctx.matvec(xd).cpu().numpy()
+    np.testing.assert_array_equal(y, y_again)          # fixed accumulation order: bitwise repeatable
+    y_scaled = ctx.matvec(-2.5 * xd).cpu().numpy()
+    assert rel(y_scaled, -2.5 * y) <= 1e-13
+    if direct:
+        ctx.set_params(theta=0.0)
+        ctx.tree_build()
+        yd = ctx.matvec(xd).cpu().numpy()
+        assert rel(yd[rows], y1) <= TOL_DIRECT and rel(yd[nt + rows], y2) <= TOL_DIRECT
+        assert ctx.stats()["p2p_pairs"] == nt * nt * w.params["K_far"]      # list pairs (own panel skipped by index)
+        assert rel(y, yd) <= TOL_TREE                  # treecode vs direct on every row
+    ctx.close()
+
+
+def test_site_side_operators_c2(pbm, po, torch_cuda):
+    """RHS (Eq. 8), reaction field (Eq. 12, 13, 21) and multipole field (Eq. 14) at C2's sizes
+    (1,000 sites, ~10k panels, polarization groups of 4)."""
+    from paper_1810_03698_b200.workloads import make_config
+    w = make_config("C2")
+    nt = w.tris.shape[0]
+    orc = po.Oracle(w.verts, w.tris, po.Params(K_far=w.params["K_far"]))
+    s = po.Sites(**w.sites)
+    ctx = pbm.from_workload(w)
+    ctx.tree_build()
+    rng = np.random.Generator(np.random.PCG64(5))
+    mu = rng.normal(0.0, 0.05, (s.na, 3))
+    b = ctx.rhs_multipole(torch_cuda.from_numpy(mu)).cpu().numpy()
+    assert rel(b, orc.rhs(s, mu)) <= TOL_DIRECT
+    x = rng.normal(size=2 * nt)
+    phi, grad, hess = [t.cpu().numpy() for t in ctx.reaction_field(torch_cuda.from_numpy(x))]
+    rphi, rgrad, rhess = orc.reaction(x, s.pos)
+    assert rel(phi, rphi) <= TOL_DIRECT and rel(grad, rgrad) <= TOL_DIRECT and rel(hess, rhess) <= TOL_DIRECT
+    for mask in (True, False):
+        got = [t.cpu().numpy() for t in ctx.multipole_field(torch_cuda.from_numpy(mu), use_mask=mask)]
+        ref = orc.multipole_field(s, mu, use_mask=mask)
+        for a, r in zip(got, ref):
+            assert rel(a, r) <= TOL_DIRECT
+    ctx.close()
+
+
+@pytest.mark.parametrize("name", ["C1", "C2"])
+def test_polarizable_solve_full_size(pbm, po, torch_cuda, name):
+    """BASELINE configs[1] and [2] end to end: treecode GMRES + SCF to 1e-7 Debye against the oracle's
+    dense LU + SCF: energies <= 1e-3 relative, induced dipoles, iteration counts."""
+    from paper_1810_03698_b200.workloads import make_config
+    w = make_config(name)
+    orc = po.Oracle(w.verts, w.tris, po.Params(K_far=w.params["K_far"]))
+    s = po.Sites(**w.sites)
+    ref = orc.solve(s)
+    ctx = pbm.from_workload(w)
+    ctx.tree_build()
+    x, mu, res = ctx.solve()
+    assert res["status"] == 0
+    for k in ("dG_solv", "G_solvterm", "G_mult_diss", "G_vac"):
+        assert abs(res[k] - ref[k]) <= 1e-3 * abs(ref[k]), (k, res[k], ref[k])
+    assert rel(mu.cpu().numpy(), ref["mu"]) <= 1e-4
+    assert rel(x.cpu().numpy(), ref["x"]) <= 1e-3
+    assert abs(res["scf_iters"] - ref["scf_iters"]) <= 1 and res["scf_iters_vac"] == ref["scf_iters_vac"]
+    assert res["final_scf_delta_debye"] < 1e-7
+    ctx.close()

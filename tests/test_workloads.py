@@ -91,8 +91,13 @@ def test_vdw_surface_is_closed_and_hits_the_panel_count():
         d = c - x
         omega = np.sum(np.einsum("ij,ij->i", d, n) / np.linalg.norm(d, axis=1) ** 3)
         assert abs(omega - 4 * np.pi) < 1.0          # 1-point rule; outside would give 0
+    # the net circumscribes the union: no vertex or centroid is inside an atom by more than 0.1 A,
+    # so every site keeps (nearly) its atom's radius of clearance from the dielectric boundary
+    for x in (v, c):
+        f = (np.linalg.norm(x[:, None, :] - g["pos"][None], axis=2) - g["radii"][None]).min(axis=1)
+        assert f.min() > -0.1 and f.mean() < 0.8       # (filled crevices and cavities lie further out)
     # two well-separated atoms give two closed components
-    v2, t2, info2 = vdw_surface(np.array([[0.0, 0, 0], [8.0, 0, 0]]), np.array([1.5, 1.5]), h=0.4)
+    v2, t2, info2 = vdw_surface(np.array([[0.0, 0, 0], [8.0, 0, 0]]), np.array([1.5, 1.5]), h=0.4, iso_shift=0.0)
     assert info2["closed_oriented"]
     area = 0.5 * np.linalg.norm(np.cross(v2[t2[:, 1]] - v2[t2[:, 0]], v2[t2[:, 2]] - v2[t2[:, 0]]), axis=1).sum()
     assert abs(area - 2 * 4 * np.pi * 1.5 ** 2) < 0.08 * area
