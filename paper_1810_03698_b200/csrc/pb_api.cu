@@ -85,7 +85,7 @@ extern "C" void pb_default_params(pb_params* p)
     p->kappa = 0.125;
     p->theta = 0.5;
     p->order_P = 6;
-    p->ncrit = 64;
+    p->ncrit = 0;
     p->K_far = 7;
     p->K_near = 19;
     p->near_tau = 2.0;
@@ -173,8 +173,8 @@ extern "C" int pb_set_params(pb_ctx* ctx, const pb_params* p)
         return pb_fail(ctx, PB_ERR_INVALID_ARG, "K_far must be 1, 3, 4 or 7");
     if (!(p->K_near == 1 || p->K_near == 3 || p->K_near == 4 || p->K_near == 7 || p->K_near == 19))
         return pb_fail(ctx, PB_ERR_INVALID_ARG, "K_near must be 1, 3, 4, 7 or 19");
-    if (p->ncrit < 1 || p->nq_edge < 1 || p->nq_edge > 64 || !(p->near_tau >= 0))
-        return pb_fail(ctx, PB_ERR_INVALID_ARG, "ncrit >= 1, 1 <= nq_edge <= 64, near_tau >= 0 required");
+    if (p->ncrit < 0 || p->nq_edge < 1 || p->nq_edge > 64 || !(p->near_tau >= 0))
+        return pb_fail(ctx, PB_ERR_INVALID_ARG, "ncrit >= 0, 1 <= nq_edge <= 64, near_tau >= 0 required");
     if (p->gmres_restart < 1 || p->gmres_maxit < 1 || p->scf_maxit < 1 || !(p->gmres_tol > 0) ||
         !(p->scf_tol_debye > 0) || !(p->scf_omega > 0))
         return pb_fail(ctx, PB_ERR_INVALID_ARG, "solver limits/tolerances must be positive");
@@ -328,6 +328,7 @@ extern "C" int pb_get_stats(pb_ctx* ctx, pb_stats* out)
     out->prof_p2p_ms = ctx->prof_ms[0];
     out->prof_m2p_ms = ctx->prof_ms[1];
     for (int i = 0; i < 8; ++i) out->last_matvec_ms[i] = ctx->last_ms[i];
+    out->ncrit_used = t.ncrit_used;
     return PB_OK;
 }
 

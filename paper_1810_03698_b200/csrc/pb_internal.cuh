@@ -54,6 +54,7 @@ struct pb_tree {
     double* xdphi = nullptr;      // [N]
     // cells
     int64_t n_cells = 0, n_leaves = 0, n_levels = 0;
+    int ncrit_used = 0;           // leaf capacity in source points this tree was built with
     int32_t* c_first = nullptr;   // [cells] first panel
     int32_t* c_last = nullptr;    // one past last panel
     int32_t* c_child = nullptr;   // first child cell (-1 for leaves)
@@ -63,10 +64,8 @@ struct pb_tree {
     double* c_box = nullptr;      // [cells][6] lo, hi
     std::vector<int64_t> gen_start; // BFS generations: cells [gen_start[g], gen_start[g+1])
     int32_t* leaf_ids = nullptr;  // [n_leaves]
-    // target groups
+    // target groups: PB_TG consecutive Morton-ordered collocation points
     int64_t n_groups = 0;
-    double* g_ctr[3] = {0, 0, 0};
-    double* g_rad = nullptr;
     // lists (CSR per group)
     int32_t* m2p_off = nullptr;   // [groups+1]
     int32_t* m2p_cell = nullptr;
@@ -229,6 +228,7 @@ int pb_weights(pb_ctx* ctx, const double* x, bool precond);
 void pb_make_expk(double kappa, pb_expk* out);
 // pb_sites.cu
 int pb_site_near_build(pb_ctx* ctx);
+int pb_multipole_field_impl(pb_ctx* ctx, const double* mu, int parts, int use_mask, double* phi, double* grad, double* hess);
 // pb_api.cu: profiling ring
 int pb_prof_begin(pb_ctx* ctx, int kernel);
 int pb_prof_end(pb_ctx* ctx, int kernel);

@@ -106,7 +106,7 @@ int pb_farfield_setup(pb_ctx* ctx)
     PB_CUDA(cudaMemcpyAsync(t.cv_off, off.data(), sizeof(int32_t) * off.size(), cudaMemcpyHostToDevice, st));
     PB_CUDA(cudaMemcpyAsync(t.cv_idx, idx.data(), sizeof(int32_t) * idx.size(), cudaMemcpyHostToDevice, st));
     PB_CUDA(cudaMemcpyAsync(t.cv_coef, coef.data(), sizeof(double) * coef.size(), cudaMemcpyHostToDevice, st));
-    // M2M table: for every k the triples (l, k - l, C(k,l)), l <= k componentwise
+    // M2M table: for every k the triples (l, k - l, C(k,l)), l <= k componentwise; l and k - l as moment indices
     std::vector<int32_t> mo(1, 0), me;
     std::vector<double> mc;
     for (int k = 0; k < t.Nk; ++k) {
@@ -114,7 +114,7 @@ int pb_farfield_setup(pb_ctx* ctx)
         for (int la = 0; la <= a; ++la)
             for (int lb = 0; lb <= b; ++lb)
                 for (int lc = 0; lc <= c; ++lc) {
-                    me.push_back(mom_index(la, lb, lc) | ((a - la) << 12) | ((b - lb) << 16) | ((c - lc) << 20));
+                    me.push_back(mom_index(la, lb, lc) | (mom_index(a - la, b - lb, c - lc) << 12));
                     mc.push_back(factorial(a) / (factorial(la) * factorial(a - la)) * factorial(b) /
                                  (factorial(lb) * factorial(b - lb)) * factorial(c) / (factorial(lc) * factorial(c - lc)));
                 }
@@ -252,7 +252,7 @@ struct up_args {
 static size_t up_smem_bytes(int Nk)
 {
     const size_t p2m = 3 * P2M_CH * P2M_LD + 3 * (size_t)Nk;
-    const size_t m2m = 32 * (size_t)Nk + 8 * 3 * P2M_LD;
+    const size_t m2m = 40 * (size_t)Nk + 8 * 3 * P2M_LD;
     return P2M_CH * sizeof(double4) + (2 * (size_t)Nk + (p2m > m2m ? p2m : m2m)) * sizeof(double);
 }
 
@@ -263,15 +263,16 @@ __global__ void __launch_bounds__(UP_THREADS) k_upward(up_args a)
     double4* wq = reinterpret_cast<double4*>(up_raw);          // [P2M_CH]
     double* mom = reinterpret_cast<double*>(wq + P2M_CH);      // [2][Nk] finished moments of the current cell
     double* U = mom + 2 * Nk;
-    double* pw = U;                                            // P2M: [3][P2M_CH][P2M_LD]
-    double* sk = U + 3 * P2M_CH * P2M_LD;                      // P2M: [3][Nk]
+    double* pw = U;                                            // P2M: [3][P2M_CH][P2M_LD] powers of h
+    double* sk = pw + 3 * P2M_CH * P2M_LD;                     // P2M: [3][Nk] the S^x, S^y, S^z sets
     double* cm = U;                                            // M2M: [8][2][Nk] children
     double* part = cm + 16 * Nk;                               // M2M: [8][2][Nk] shifted children
-    double* tp = part + 16 * Nk;                               // M2M: [8][3][P2M_LD] powers of the shifts
+    double* tm = part + 16 * Nk;                               // M2M: [8][Nk] monomials of the shifts
+    double* tp = tm + 8 * Nk;                                  // M2M: [8][3][P2M_LD] powers of the shifts
     __shared__ int s_last;
 
     int64_t c = a.leaf_ids[blockIdx.x];
-    {   // ---- P2M
+    {   // ---- P2M: thread k (and k + 128, k + 256 at high order) sweeps the leaf's points
         const int64_t s0 = (int64_t)a.c_first[c] * a.K, s1 = (int64_t)a.c_last[c] * a.K;
         const double ycx = a.cx[c], ycy = a.cy[c], ycz = a.cz[c];
         int ea[3], eb[3], ec[3];
@@ -291,10 +292,10 @@ __global__ void __launch_bounds__(UP_THREADS) k_upward(up_args a)
             if (tid < 3 * np) {                                // thread (point, axis): powers of one coordinate
                 const int pt = tid / 3, d = tid - 3 * pt;
                 const double4 ra = a.srec[2 * (base + pt)];
-                const double h = d == 0 ? ra.x - ycx : (d == 1 ? ra.y - ycy : ra.z - ycz);
+                const double hh = d == 0 ? ra.x - ycx : (d == 1 ? ra.y - ycy : ra.z - ycz);
                 double pwr = 1.0;
                 double* dst = pw + ((size_t)d * P2M_CH + pt) * P2M_LD;
-                for (int e = 0; e <= P; ++e) { dst[e] = pwr; pwr *= h; }
+                for (int e = 0; e <= P; ++e) { dst[e] = pwr; pwr *= hh; }
                 if (d == 0) {
                     const double4 rb = a.srec[2 * (base + pt) + 1];
                     wq[pt] = make_double4(ra.w, rb.x, rb.y, rb.z);
@@ -323,23 +324,16 @@ __global__ void __launch_bounds__(UP_THREADS) k_upward(up_args a)
 #pragma unroll
         for (int r = 0; r < 3; ++r) {
             const int k = tid + r * UP_THREADS;
-            if (k < Nk) {
-                mom[k] = acc[r][0];
-                sk[k] = acc[r][1]; sk[Nk + k] = acc[r][2]; sk[2 * Nk + k] = acc[r][3];
-            }
+            if (k < Nk) { mom[k] = acc[r][0]; sk[k] = acc[r][1]; sk[Nk + k] = acc[r][2]; sk[2 * Nk + k] = acc[r][3]; }
         }
         __syncthreads();
-#pragma unroll
-        for (int r = 0; r < 3; ++r) {
-            const int k = tid + r * UP_THREADS;
-            if (k < Nk) {
-                const int ax = ea[r], bx = eb[r], cc = ec[r];
-                double v = 0.0;
-                if (ax) v = fma((double)ax, sk[mom_index(ax - 1, bx, cc)], v);
-                if (bx) v = fma((double)bx, sk[Nk + mom_index(ax, bx - 1, cc)], v);
-                if (cc) v = fma((double)cc, sk[2 * Nk + mom_index(ax, bx, cc - 1)], v);
-                mom[Nk + k] = v;
-            }
+        for (int k = tid; k < Nk; k += UP_THREADS) {
+            const int ax = c_ka[k], bx = c_kb[k], cc = c_kc[k];
+            double v = 0.0;
+            if (ax) v = fma((double)ax, sk[mom_index(ax - 1, bx, cc)], v);
+            if (bx) v = fma((double)bx, sk[Nk + mom_index(ax, bx - 1, cc)], v);
+            if (cc) v = fma((double)cc, sk[2 * Nk + mom_index(ax, bx, cc - 1)], v);
+            mom[Nk + k] = v;
         }
         __syncthreads();
     }
@@ -354,10 +348,10 @@ __global__ void __launch_bounds__(UP_THREADS) k_upward(up_args a)
             const double* mk = mom + Nk;
             for (int e = tid; e < a.NT; e += UP_THREADS) {
                 double v = 0, k = 0;
-                const int q1 = a.cv_off[e + 1];
-                for (int q = a.cv_off[e]; q < q1; ++q) {
-                    const int l = a.cv_idx[q];
-                    const double f = a.cv_coef[q];
+                const int q1 = __ldg(a.cv_off + e + 1);
+                for (int q = __ldg(a.cv_off + e); q < q1; ++q) {
+                    const int l = __ldg(a.cv_idx + q);
+                    const double f = __ldg(a.cv_coef + q);
                     v = fma(f, mv[l], v);
                     k = fma(f, mk[l], k);
                 }
@@ -389,18 +383,23 @@ __global__ void __launch_bounds__(UP_THREADS) k_upward(up_args a)
             for (int e = 0; e <= P; ++e) { tp[(q * 3 + d) * P2M_LD + e] = pwr; pwr *= tt; }
         }
         __syncthreads();
-        for (int it = tid; it < Nk * nc; it += UP_THREADS) {
+        for (int it = tid; it < Nk * nc; it += UP_THREADS) {   // monomials t^k of every child's shift
             const int q = it / Nk, k = it - q * Nk;
             const double* t3 = tp + q * 3 * P2M_LD;
+            tm[it] = t3[c_ka[k]] * t3[P2M_LD + c_kb[k]] * t3[2 * P2M_LD + c_kc[k]];
+        }
+        __syncthreads();
+        for (int it = tid; it < Nk * nc; it += UP_THREADS) {
+            const int q = it / Nk, k = it - q * Nk;
+            const double* tq = tm + q * Nk;
             const double* cq = cm + q * 2 * Nk;
             double s0 = 0, s1 = 0;
             const int e1 = __ldg(a.mm_off + k + 1);
-#pragma unroll 2
+#pragma unroll 4
             for (int e = __ldg(a.mm_off + k); e < e1; ++e) {
                 const int32_t ent = __ldg(a.mm_ent + e);
-                const double cf = __ldg(a.mm_coef + e);
-                const int l = ent & 0xfff, dx = (ent >> 12) & 15, dy = (ent >> 16) & 15, dz = (ent >> 20) & 15;
-                const double f = cf * t3[dx] * t3[P2M_LD + dy] * t3[2 * P2M_LD + dz];
+                const double f = __ldg(a.mm_coef + e) * tq[ent >> 12];
+                const int l = ent & 0xfff;
                 s0 = fma(f, cq[l], s0);
                 s1 = fma(f, cq[Nk + l], s1);
             }

@@ -291,101 +291,196 @@ extern "C" int pb_reaction_field(pb_ctx* ctx, const double* x, double* phi, doub
 }
 
 // ---- H12: Coulomb potential / field / field gradient of the multipoles at the other sites ------------------
-#define MF_TILE 32
-__global__ void __launch_bounds__(64)
-k_multipole_field(int64_t na, const double* __restrict__ pos, const double* __restrict__ q,
-                  const double* __restrict__ dip, const double* __restrict__ quad, const double* __restrict__ mu,
-                  const double* __restrict__ alpha, const int32_t* __restrict__ group, double thole_a, double inv_eps,
-                  int use_mask, double* __restrict__ phi, double* __restrict__ grad, double* __restrict__ hess)
+// Block = MF_ST target sites (register tile) x one chunk of source sites swept by the block's threads;
+// per-chunk partial sums are added in a fixed order by k_mfield_finish.  PERM: permanent charge, dipole,
+// quadrupole of the sources (Eq. 7, 31, 32 with the corrections of App. A.2), dropped for same-group pairs
+// when use_mask.  IND: induced dipoles, never masked, Thole-damped (App. A.5).
+// FULL: potential, gradient and Hessian (energies, Eq. 24); otherwise the gradient alone (the SCF loop).
+#define MF_ST 2
+#define MF_THREADS 128
+
+template <bool FULL, bool PERM, bool IND>
+__device__ __forceinline__ void mf_pair(double dx, double dy, double dz, bool masked, double qm, const double* p,
+                                        const double* Q, const double* u, double ia_l, double ia_m, double thole_a,
+                                        double* o)
 {
-    __shared__ double s[17][MF_TILE];
-    __shared__ int32_t sg[MF_TILE];
-    const int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    const bool live = l < na;
-    const int64_t lc = live ? l : na - 1;
-    const double x = pos[3 * lc], y = pos[3 * lc + 1], z = pos[3 * lc + 2], al = alpha[lc];
-    const int32_t gl = group[lc];
-    double P = 0, G[3] = {0, 0, 0}, H[6] = {0, 0, 0, 0, 0, 0};
-    for (int64_t m0 = 0; m0 < na; m0 += MF_TILE) {
-        const int cnt = (int)(na - m0 < MF_TILE ? na - m0 : MF_TILE);
-        __syncthreads();
-        for (int k = threadIdx.x; k < cnt; k += blockDim.x) {
-            const int64_t m = m0 + k;
-            for (int d = 0; d < 3; ++d) {
-                s[d][k] = pos[3 * m + d];
-                s[4 + d][k] = dip[3 * m + d];
-                s[13 + d][k] = mu ? mu[3 * m + d] : 0.0;
-            }
-            s[3][k] = q[m];
-            for (int d = 0; d < 6; ++d) s[7 + d][k] = quad[6 * m + d];
-            s[16][k] = alpha[m];
-            sg[k] = group[m];
-        }
-        __syncthreads();
-        if (!live) continue;
-        for (int k = 0; k < cnt; ++k) {
-            if (m0 + k == l) continue;
-            const double d[3] = {x - s[0][k], y - s[1][k], z - s[2][k]};
-            const double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
-            const double R = sqrt(r2), i1 = 1.0 / R, i2 = i1 * i1, i3 = i1 * i2, i5 = i3 * i2, i7 = i5 * i2, i9 = i7 * i2;
-            if (!(use_mask && sg[k] == gl)) {
-                // permanent charge, dipole, quadrupole of m (Eq. 7, 31, 32 with the corrections of App. A.2)
-                const double qm = s[3][k];
-                const double p[3] = {s[4][k], s[5][k], s[6][k]};
-                const double Q[6] = {s[7][k], s[8][k], s[9][k], s[10][k], s[11][k], s[12][k]};
-                const double pd = p[0] * d[0] + p[1] * d[1] + p[2] * d[2];
-                const double Qd[3] = {Q[0] * d[0] + Q[1] * d[1] + Q[2] * d[2], Q[1] * d[0] + Q[3] * d[1] + Q[4] * d[2],
-                                      Q[2] * d[0] + Q[4] * d[1] + Q[5] * d[2]};
-                const double dQd = Qd[0] * d[0] + Qd[1] * d[1] + Qd[2] * d[2];
-                P += qm * i1 + pd * i3 + 0.5 * dQd * i5;
-                const double gd = -qm * i3 - 3.0 * pd * i5 - 2.5 * dQd * i7;   // coefficient of d in the gradient
-                for (int c = 0; c < 3; ++c) G[c] += gd * d[c] + p[c] * i3 + Qd[c] * i5;
-                const double hdd = 3.0 * qm * i5 + 15.0 * pd * i7 + 17.5 * dQd * i9;   // coefficient of d d^T
-                const double hI = -qm * i3 - 3.0 * pd * i5 - 2.5 * dQd * i7;           // coefficient of I
-                int idx = 0;
-                for (int a = 0; a < 3; ++a)
-                    for (int b = a; b < 3; ++b, ++idx)
-                        H[idx] += hdd * d[a] * d[b] + (a == b ? hI : 0.0) - 3.0 * (p[a] * d[b] + p[b] * d[a]) * i5 +
+    constexpr int G0 = FULL ? 1 : 0;
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    const double i1 = pb_rsqrt(r2), i2 = i1 * i1, i3 = i1 * i2, i5 = i3 * i2, i7 = i5 * i2;
+    const double d[3] = {dx, dy, dz};
+    if (PERM && !masked) {
+        const double pd = p[0] * dx + p[1] * dy + p[2] * dz;
+        const double Qd[3] = {Q[0] * dx + Q[1] * dy + Q[2] * dz, Q[1] * dx + Q[3] * dy + Q[4] * dz,
+                              Q[2] * dx + Q[4] * dy + Q[5] * dz};
+        const double dQd = Qd[0] * dx + Qd[1] * dy + Qd[2] * dz;
+        const double gd = -qm * i3 - 3.0 * pd * i5 - 2.5 * dQd * i7;        // coefficient of d in the gradient
+#pragma unroll
+        for (int c = 0; c < 3; ++c) o[G0 + c] += gd * d[c] + p[c] * i3 + Qd[c] * i5;
+        if (FULL) {
+            const double i9 = i7 * i2;
+            o[0] += qm * i1 + pd * i3 + 0.5 * dQd * i5;
+            const double hdd = 3.0 * qm * i5 + 15.0 * pd * i7 + 17.5 * dQd * i9;   // coefficient of d d^T
+            int idx = 0;
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+#pragma unroll
+                for (int b = a; b < 3; ++b, ++idx)
+                    o[4 + idx] += hdd * d[a] * d[b] + (a == b ? gd : 0.0) - 3.0 * (p[a] * d[b] + p[b] * d[a]) * i5 +
                                   Q[idx] * i5 - 5.0 * (Qd[a] * d[b] + Qd[b] * d[a]) * i7;
-            }
-            if (mu) {
-                // induced dipole of m: never masked, Thole-damped (App. A.5)
-                const double u[3] = {s[13][k], s[14][k], s[15][k]};
-                double l3 = 1.0, l5 = 1.0, l7 = 1.0;
-                const double aa = al * s[16][k];
-                if (aa > 0.0) {
-                    const double au3 = thole_a * r2 * R / sqrt(aa);
-                    const double E = exp(-au3);
-                    l3 = 1.0 - E;
-                    l5 = 1.0 - (1.0 + au3) * E;
-                    l7 = 1.0 - (1.0 + au3 + 0.6 * au3 * au3) * E;
-                }
-                const double ud = u[0] * d[0] + u[1] * d[1] + u[2] * d[2];
-                P += l3 * ud * i3;
-                for (int c = 0; c < 3; ++c) G[c] += l3 * u[c] * i3 - 3.0 * l5 * ud * d[c] * i5;
-                int idx = 0;
-                for (int a = 0; a < 3; ++a)
-                    for (int b = a; b < 3; ++b, ++idx)
-                        H[idx] += -3.0 * l5 * (u[a] * d[b] + u[b] * d[a] + (a == b ? ud : 0.0)) * i5 +
-                                  15.0 * l7 * ud * d[a] * d[b] * i7;
-            }
         }
     }
-    if (!live) return;
-    const double sc = PB_INV4PI * inv_eps;
-    if (phi) phi[l] = sc * P;
-    if (grad) for (int c = 0; c < 3; ++c) grad[3 * l + c] = sc * G[c];
-    if (hess) for (int c = 0; c < 6; ++c) hess[6 * l + c] = sc * H[c];
+    if (IND) {
+        double l3 = 1.0, l5 = 1.0, l7 = 1.0;
+        const double ia = ia_l * ia_m;                      // 1/sqrt(alpha_l alpha_m), 0 when either is 0
+        if (ia > 0.0) {
+            const double au3 = thole_a * r2 * (r2 * i1) * ia;
+            const double E = exp(-au3);
+            l3 = 1.0 - E;
+            l5 = 1.0 - (1.0 + au3) * E;
+            l7 = 1.0 - (1.0 + au3 + 0.6 * au3 * au3) * E;
+        }
+        const double ud = u[0] * dx + u[1] * dy + u[2] * dz;
+        const double g5 = 3.0 * l5 * ud * i5;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) o[G0 + c] += l3 * u[c] * i3 - g5 * d[c];
+        if (FULL) {
+            o[0] += l3 * ud * i3;
+            const double h5 = 3.0 * l5 * i5, h7 = 15.0 * l7 * ud * i7;
+            int idx = 0;
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+#pragma unroll
+                for (int b = a; b < 3; ++b, ++idx)
+                    o[4 + idx] += -h5 * (u[a] * d[b] + u[b] * d[a] + (a == b ? ud : 0.0)) + h7 * d[a] * d[b];
+        }
+    }
+}
+
+template <bool FULL, bool PERM, bool IND>
+__global__ void __launch_bounds__(MF_THREADS)
+k_multipole_field(int64_t na, int64_t chunk, const double* __restrict__ pos, const double* __restrict__ q,
+                  const double* __restrict__ dip, const double* __restrict__ quad, const double* __restrict__ mu,
+                  const double* __restrict__ alpha, const int32_t* __restrict__ group, double thole_a, int use_mask,
+                  double* __restrict__ partial /*[gridDim.x][na][10]*/)
+{
+    constexpr int NO = FULL ? 10 : 3;
+    __shared__ double red[MF_THREADS / 32][MF_ST][NO];
+    const int64_t l0 = (int64_t)blockIdx.y * MF_ST;
+    double r[MF_ST][3], ial[MF_ST], acc[MF_ST][NO];
+    int32_t gl[MF_ST];
+#pragma unroll
+    for (int t = 0; t < MF_ST; ++t) {
+        const int64_t l = l0 + t < na ? l0 + t : na - 1;     // clamp: duplicates are not written
+        r[t][0] = pos[3 * l]; r[t][1] = pos[3 * l + 1]; r[t][2] = pos[3 * l + 2];
+        const double al = alpha[l];
+        ial[t] = al > 0.0 ? rsqrt(al) : 0.0;
+        gl[t] = group[l];
+#pragma unroll
+        for (int c = 0; c < NO; ++c) acc[t][c] = 0.0;
+    }
+    const int64_t m0 = blockIdx.x * chunk, m1 = m0 + chunk < na ? m0 + chunk : na;
+    for (int64_t m = m0 + threadIdx.x; m < m1; m += MF_THREADS) {
+        const double sx = pos[3 * m], sy = pos[3 * m + 1], sz = pos[3 * m + 2];
+        double qm = 0.0, p[3] = {0, 0, 0}, Q[6] = {0, 0, 0, 0, 0, 0}, u[3] = {0, 0, 0}, iam = 0.0;
+        if (PERM) {
+            qm = q[m];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) p[c] = dip[3 * m + c];
+#pragma unroll
+            for (int c = 0; c < 6; ++c) Q[c] = quad[6 * m + c];
+        }
+        if (IND) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) u[c] = mu[3 * m + c];
+            const double am = alpha[m];
+            iam = am > 0.0 ? rsqrt(am) : 0.0;
+        }
+        const int32_t gm = group[m];
+#pragma unroll
+        for (int t = 0; t < MF_ST; ++t) {
+            if (m == l0 + t) continue;
+            mf_pair<FULL, PERM, IND>(r[t][0] - sx, r[t][1] - sy, r[t][2] - sz, use_mask && gm == gl[t], qm, p, Q, u,
+                                     ial[t], iam, thole_a, acc[t]);
+        }
+    }
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+    for (int t = 0; t < MF_ST; ++t)
+#pragma unroll
+        for (int c = 0; c < NO; ++c) {
+            double v = acc[t][c];
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            if (lane == 0) red[w][t][c] = v;
+        }
+    __syncthreads();
+    if (threadIdx.x < MF_ST * NO) {
+        const int t = threadIdx.x / NO, c = threadIdx.x % NO;
+        if (l0 + t < na) {
+            double v = 0;
+            for (int k = 0; k < MF_THREADS / 32; ++k) v += red[k][t][c];
+            partial[((int64_t)blockIdx.x * na + (l0 + t)) * 10 + c] = v;
+        }
+    }
+}
+
+// sum the per-chunk partials (fixed order), scale, write phi/grad/hess
+__global__ void k_mfield_finish(int64_t na, int nchunk, int full, double scale, const double* __restrict__ partial,
+                                double* __restrict__ phi, double* __restrict__ grad, double* __restrict__ hess)
+{
+    const int NO = full ? 10 : 3;
+    int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (g >= na * NO) return;
+    int64_t m = g / NO;
+    int c = (int)(g % NO);
+    double v = 0;
+    for (int k = 0; k < nchunk; ++k) v += partial[((int64_t)k * na + m) * 10 + c];
+    v *= scale;
+    if (!full) grad[3 * m + c] = v;
+    else if (c == 0) { if (phi) phi[m] = v; }
+    else if (c < 4) { if (grad) grad[3 * m + c - 1] = v; }
+    else if (hess) hess[6 * m + c - 4] = v;
+}
+
+// parts: bit 0 = permanent multipoles, bit 1 = induced dipoles `mu`
+int pb_multipole_field_impl(pb_ctx* ctx, const double* mu, int parts, int use_mask, double* phi, double* grad, double* hess)
+{
+    const pb_sites& s = ctx->sites;
+    cudaStream_t st = ctx->stream;
+    if (!mu) parts &= ~2;
+    const bool full = phi || hess;
+    if (!full && !grad) return PB_OK;
+    const int64_t ntile = (s.na + MF_ST - 1) / MF_ST;
+    int64_t nchunk = (148 * 8 + ntile - 1) / ntile;                 // enough blocks to fill the GPU ...
+    const int64_t maxchunk = (s.na + MF_THREADS - 1) / MF_THREADS;  // ... but at least one source per thread
+    if (nchunk > maxchunk) nchunk = maxchunk;
+    if (nchunk < 1) nchunk = 1;
+    int64_t chunk = (s.na + nchunk - 1) / nchunk;
+    nchunk = (s.na + chunk - 1) / chunk;
+    PB_TRY(pb_scratch(ctx, (size_t)nchunk * s.na * 10 * sizeof(double) + 4096));
+    double* partial = ctx->scratch;
+    dim3 grid((unsigned)nchunk, (unsigned)ntile);
+#define MF_LAUNCH(F, PM, IN)                                                                                         \
+    k_multipole_field<F, PM, IN><<<grid, MF_THREADS, 0, st>>>(s.na, chunk, s.pos, s.q, s.dip, s.quad, mu, s.alpha,    \
+                                                              s.group, ctx->prm.thole_a, use_mask, partial)
+    if (parts == 0) {
+        PB_CUDA(cudaMemsetAsync(partial, 0, (size_t)nchunk * s.na * 10 * sizeof(double), st));
+    } else if (full) {
+        if (parts == 3) MF_LAUNCH(true, true, true); else if (parts == 1) MF_LAUNCH(true, true, false); else MF_LAUNCH(true, false, true);
+        PB_LAUNCH_CHECK();
+    } else {
+        if (parts == 3) MF_LAUNCH(false, true, true); else if (parts == 1) MF_LAUNCH(false, true, false); else MF_LAUNCH(false, false, true);
+        PB_LAUNCH_CHECK();
+    }
+#undef MF_LAUNCH
+    k_mfield_finish<<<pb_blocks(s.na * (full ? 10 : 3), 128), 128, 0, st>>>(s.na, (int)nchunk, full ? 1 : 0,
+                                                                            PB_INV4PI / ctx->prm.eps_in, partial, phi, grad, hess);
+    PB_LAUNCH_CHECK();
+    return PB_OK;
 }
 
 extern "C" int pb_multipole_field(pb_ctx* ctx, const double* mu, int use_mask, double* phi, double* grad, double* hess)
 {
     if (!ctx) return PB_ERR_INVALID_ARG;
-    const pb_sites& s = ctx->sites;
-    if (!s.loaded) return pb_fail(ctx, PB_ERR_NOT_READY, "pb_multipole_field: call pb_sites_load first");
-    k_multipole_field<<<pb_blocks(s.na, 64), 64, 0, ctx->stream>>>(s.na, s.pos, s.q, s.dip, s.quad, mu, s.alpha, s.group,
-                                                                   ctx->prm.thole_a, 1.0 / ctx->prm.eps_in, use_mask, phi,
-                                                                   grad, hess);
-    PB_LAUNCH_CHECK();
-    return PB_OK;
+    if (!ctx->sites.loaded) return pb_fail(ctx, PB_ERR_NOT_READY, "pb_multipole_field: call pb_sites_load first");
+    return pb_multipole_field_impl(ctx, mu, 3, use_mask, phi, grad, hess);
 }

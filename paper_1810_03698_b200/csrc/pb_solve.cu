@@ -342,15 +342,17 @@ extern "C" int pb_gmres(pb_ctx* ctx, const double* b, double* x, int32_t* iters,
 
 // ---- SCF and energy kernels ------------------------------------------------------------------------
 // mu_new = (1-w) mu + w alpha 4 pi E,  E = -(grad_solv + grad_mult)   (Eq. 9, 15; SOR P:160; D: R-2)
+// grad_mult = gperm (masked permanent multipoles: constant over the loop, computed once) + gmult (induced dipoles)
 // out[0] = sum_m |mu_new - mu|^2
 __global__ void __launch_bounds__(256)
 k_scf_update(int64_t na, const double* __restrict__ alpha, const double* __restrict__ gsolv,
-             const double* __restrict__ gmult, double omega, double* __restrict__ mu, double* __restrict__ out)
+             const double* __restrict__ gperm, const double* __restrict__ gmult, double omega, double* __restrict__ mu,
+             double* __restrict__ out)
 {
     __shared__ double red[8];
     double s = 0;
     for (int64_t e = threadIdx.x; e < 3 * na; e += blockDim.x) {
-        double E = -(gsolv ? gsolv[e] : 0.0) - gmult[e];
+        double E = -(gsolv ? gsolv[e] : 0.0) - gperm[e] - gmult[e];
         double old = mu[e];
         double nw = (1.0 - omega) * old + omega * alpha[e / 3] * (4.0 * 3.14159265358979323846) * E;
         mu[e] = nw;
@@ -408,13 +410,14 @@ static int pb_solve_core(pb_ctx* ctx, double* x_out, double* mu_out, pb_result* 
     const int64_t n = 2 * t.N, na = s.na;
     // solve-scoped buffers from the scratch category (GMRES re-allocates CAT_SOLVE, so use CAT_TMP here)
     pb_dfree_cat(ctx, CAT_TMP);
-    double *b, *x, *mu, *muv, *gs, *gm, *phi, *hess, *dscal;
+    double *b, *x, *mu, *muv, *gs, *gm, *gp, *phi, *hess, *dscal;
     PB_TRY(pb_dalloc_t(ctx, &b, n, CAT_TMP));
     PB_TRY(pb_dalloc_t(ctx, &x, n, CAT_TMP));
     PB_TRY(pb_dalloc_t(ctx, &mu, 3 * na, CAT_TMP));
     PB_TRY(pb_dalloc_t(ctx, &muv, 3 * na, CAT_TMP));
     PB_TRY(pb_dalloc_t(ctx, &gs, 3 * na, CAT_TMP));
     PB_TRY(pb_dalloc_t(ctx, &gm, 3 * na, CAT_TMP));
+    PB_TRY(pb_dalloc_t(ctx, &gp, 3 * na, CAT_TMP));
     PB_TRY(pb_dalloc_t(ctx, &phi, na, CAT_TMP));
     PB_TRY(pb_dalloc_t(ctx, &hess, 6 * na, CAT_TMP));
     PB_TRY(pb_dalloc_t(ctx, &dscal, 8, CAT_TMP));
@@ -435,10 +438,11 @@ static int pb_solve_core(pb_ctx* ctx, double* x_out, double* mu_out, pb_result* 
     // --- vacuum SCF: mu^v from the multipole field alone
     int it_v = 0;
     if (polarizable) {
+        PB_TRY(pb_multipole_field_impl(ctx, nullptr, 1, 1, nullptr, gp, nullptr));   // masked permanent field, once
         bool conv = false;
         for (it_v = 1; it_v <= ctx->prm.scf_maxit; ++it_v) {
-            PB_TRY(pb_multipole_field(ctx, muv, 1, nullptr, gm, nullptr));
-            k_scf_update<<<1, 256, 0, st>>>(na, s.alpha, nullptr, gm, omega, muv, dscal);
+            PB_TRY(pb_multipole_field_impl(ctx, muv, 2, 1, nullptr, gm, nullptr));
+            k_scf_update<<<1, 256, 0, st>>>(na, s.alpha, nullptr, gp, gm, omega, muv, dscal);
             PB_LAUNCH_CHECK();
             PB_CUDA(cudaMemcpyAsync(h, dscal, sizeof(double), cudaMemcpyDeviceToHost, st));
             PB_CUDA(cudaStreamSynchronize(st));
@@ -461,8 +465,8 @@ static int pb_solve_core(pb_ctx* ctx, double* x_out, double* mu_out, pb_result* 
         mv_total += mv;
         if (!polarizable) { conv = true; break; }
         PB_TRY(pb_reaction_field(ctx, x, nullptr, gs, nullptr));      // step 3: Eq. (13)
-        PB_TRY(pb_multipole_field(ctx, mu, 1, nullptr, gm, nullptr)); // step 3: Eq. (14)
-        k_scf_update<<<1, 256, 0, st>>>(na, s.alpha, gs, gm, omega, mu, dscal);   // steps 4-5 + SOR
+        PB_TRY(pb_multipole_field_impl(ctx, mu, 2, 1, nullptr, gm, nullptr));   // step 3: Eq. (14), induced part
+        k_scf_update<<<1, 256, 0, st>>>(na, s.alpha, gs, gp, gm, omega, mu, dscal);   // steps 4-5 + SOR
         PB_LAUNCH_CHECK();
         PB_CUDA(cudaMemcpyAsync(h, dscal, sizeof(double), cudaMemcpyDeviceToHost, st));
         PB_CUDA(cudaStreamSynchronize(st));

@@ -286,41 +286,15 @@ __global__ void k_inner_geom(int64_t c0, int64_t c1, const int32_t* __restrict__
     for (int d = 0; d < 3; ++d) { cbox[6 * c + d] = lo[d]; cbox[6 * c + 3 + d] = hi[d]; }
 }
 
-// ---- target groups: PB_TG consecutive Morton-ordered collocation points ----------------------
-__global__ void k_group_geom(int64_t ng, int64_t N, const double* __restrict__ px, const double* __restrict__ py,
-                             const double* __restrict__ pz, double* __restrict__ gx, double* __restrict__ gy,
-                             double* __restrict__ gz, double* __restrict__ grad)
-{
-    int64_t w = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
-    int lane = threadIdx.x & 31;
-    if (w >= ng) return;
-    int64_t i0 = w * PB_TG, i1 = i0 + PB_TG < N ? i0 + PB_TG : N;
-    double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
-    for (int64_t i = i0 + lane; i < i1; i += 32) {
-        double p[3] = {px[i], py[i], pz[i]};
-        for (int d = 0; d < 3; ++d) { lo[d] = fmin(lo[d], p[d]); hi[d] = fmax(hi[d], p[d]); }
-    }
-    for (int o = 16; o > 0; o >>= 1)
-        for (int d = 0; d < 3; ++d) {
-            lo[d] = fmin(lo[d], __shfl_xor_sync(0xffffffffu, lo[d], o));
-            hi[d] = fmax(hi[d], __shfl_xor_sync(0xffffffffu, hi[d], o));
-        }
-    double ctr[3] = {0.5 * (lo[0] + hi[0]), 0.5 * (lo[1] + hi[1]), 0.5 * (lo[2] + hi[2])};
-    double r2 = 0;
-    for (int64_t i = i0 + lane; i < i1; i += 32) {
-        double dx = px[i] - ctr[0], dy = py[i] - ctr[1], dz = pz[i] - ctr[2];
-        r2 = fmax(r2, dx * dx + dy * dy + dz * dz);
-    }
-    for (int o = 16; o > 0; o >>= 1) r2 = fmax(r2, __shfl_xor_sync(0xffffffffu, r2, o));
-    if (lane == 0) { gx[w] = ctr[0]; gy[w] = ctr[1]; gz[w] = ctr[2]; grad[w] = sqrt(r2) * (1.0 + 1e-14); }
-}
-
 // ---- interaction lists: top-down traversal per target group (Eq. 28) ------------
-// A cell is accepted (M2P) for the whole group when R_b / R_tb < theta with R_b the cell's
-// bounding radius and R_tb = |centre_cell - centre_group| - r_group, the smallest possible
-// box-target distance over the group; otherwise its children are visited, and leaves go to
-// the P2P list as source-point ranges (adjacent ranges merged).  Cells with fewer than
-// `m2p_min` source points are never accepted: summing them directly is cheaper and exact.
+// One warp per group.  A cell is accepted (M2P) for the whole group when the MAC of Eq. (28),
+// R_b / R_tb < theta, holds for EVERY target of the group: R_b the cell's bounding radius, R_tb the
+// distance from the cell's expansion centre to the target (each lane holds two of the group's
+// targets; the smallest distance is a warp reduction).  R_tb > R_b is required as well, so a cell
+// whose bounding sphere contains a target -- in particular the target's own panel -- is never
+// accepted whatever theta is.  Otherwise the children are visited, and leaves go to the P2P list
+// as source-point ranges (adjacent ranges merged).  Cells with fewer than `m2p_min` source points
+// are never accepted: summing them directly is cheaper and exact.
 struct list_args {
     int64_t ng, N, Ns;
     int K;
@@ -328,58 +302,77 @@ struct list_args {
     int m2p_min;
     const int32_t *c_first, *c_last, *c_child, *c_nchild;
     const double *cx, *cy, *cz, *crad;
-    const double *gx, *gy, *gz, *grad;
+    const double *px, *py, *pz;       // collocation points, Morton order
     int32_t *n_m2p, *n_p2p;           // pass 0: counts ; pass 1: offsets (read)
     int32_t *m2p_cell, *p2p_lo, *p2p_hi;
     unsigned long long* pair_counts;  // [2] p2p, m2p pairs (pass 0)
 };
 
+#define LIST_WARPS 4
+#define LIST_STACK 256
+static_assert(PB_TG == 64, "k_lists keeps two targets per lane");
+
 template <int PASS>
-__global__ void k_lists(list_args a)
+__global__ void __launch_bounds__(LIST_WARPS * 32) k_lists(list_args a)
 {
-    int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    __shared__ int32_t stk[LIST_WARPS][LIST_STACK];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int64_t g = blockIdx.x * (int64_t)LIST_WARPS + wid;
     if (g >= a.ng) return;
-    int64_t ntg = (g + 1) * PB_TG <= a.N ? PB_TG : a.N - g * PB_TG;
+    const int64_t i0 = g * PB_TG;
+    const int64_t ntg = i0 + PB_TG <= a.N ? PB_TG : a.N - i0;
     int nm = 0, nr = 0;
-    int64_t om = PASS ? a.n_m2p[g] : 0, op = PASS ? a.n_p2p[g] : 0;
+    const int64_t om = PASS ? a.n_m2p[g] : 0, op = PASS ? a.n_p2p[g] : 0;
     unsigned long long pp = 0;
     if (a.theta <= 0.0) {   // direct mode: one range, every source point
-        if (PASS) { a.p2p_lo[op] = 0; a.p2p_hi[op] = (int32_t)a.Ns; }
+        if (PASS && lane == 0) { a.p2p_lo[op] = 0; a.p2p_hi[op] = (int32_t)a.Ns; }
         nr = 1;
         pp = (unsigned long long)a.Ns;
     } else {
-        int32_t stack[192];
+        // padding lanes repeat a real target
+        const int64_t ia = i0 + (lane < ntg ? lane : 0), ib = i0 + (lane + 32 < ntg ? lane + 32 : 0);
+        const double ax = a.px[ia], ay = a.py[ia], az = a.pz[ia];
+        const double bx = a.px[ib], by = a.py[ib], bz = a.pz[ib];
+        int32_t* stack = stk[wid];
         int sp = 0;
-        stack[sp++] = 0;
-        double tx = a.gx[g], ty = a.gy[g], tz = a.gz[g], tr = a.grad[g];
+        if (lane == 0) stack[0] = 0;
+        sp = 1;
+        __syncwarp();
         int32_t last_hi = -1;
+        const double th2 = a.theta * a.theta;
         while (sp > 0) {
-            int32_t c = stack[--sp];
-            double dx = a.cx[c] - tx, dy = a.cy[c] - ty, dz = a.cz[c] - tz;
-            double sep = sqrt(dx * dx + dy * dy + dz * dz) - tr;
-            int32_t f = a.c_first[c], l = a.c_last[c];
-            int32_t ch = a.c_child[c];
-            int64_t nsrc = (int64_t)(l - f) * a.K;
-            if (sep > 0.0 && a.crad[c] < a.theta * sep && nsrc >= a.m2p_min) {
-                if (PASS) a.m2p_cell[om + nm] = c;
+            const int32_t c = stack[--sp];
+            __syncwarp();
+            const double cx = a.cx[c], cy = a.cy[c], cz = a.cz[c], cr = a.crad[c];
+            double da = (cx - ax) * (cx - ax) + (cy - ay) * (cy - ay) + (cz - az) * (cz - az);
+            const double db = (cx - bx) * (cx - bx) + (cy - by) * (cy - by) + (cz - bz) * (cz - bz);
+            da = fmin(da, db);
+            for (int o = 16; o > 0; o >>= 1) da = fmin(da, __shfl_xor_sync(0xffffffffu, da, o));
+            const int32_t f = a.c_first[c], l = a.c_last[c];
+            const int32_t ch = a.c_child[c];
+            const int64_t nsrc = (int64_t)(l - f) * a.K;
+            if (cr * cr < th2 * da && cr * cr < da && nsrc >= a.m2p_min) {
+                if (PASS && lane == 0) a.m2p_cell[om + nm] = c;
                 ++nm;
             } else if (ch < 0) {
-                int32_t lo = f * a.K, hi = l * a.K;
+                const int32_t lo = f * a.K, hi = l * a.K;
                 if (lo == last_hi) {
-                    if (PASS) a.p2p_hi[op + nr - 1] = hi;
+                    if (PASS && lane == 0) a.p2p_hi[op + nr - 1] = hi;
                 } else {
-                    if (PASS) { a.p2p_lo[op + nr] = lo; a.p2p_hi[op + nr] = hi; }
+                    if (PASS && lane == 0) { a.p2p_lo[op + nr] = lo; a.p2p_hi[op + nr] = hi; }
                     ++nr;
                 }
                 last_hi = hi;
                 pp += (unsigned long long)(hi - lo);
             } else {
-                int nc = a.c_nchild[c];
-                for (int k = nc - 1; k >= 0; --k) stack[sp++] = ch + k;   // popped in Morton order
+                const int nc = a.c_nchild[c];
+                if (lane < nc) stack[sp + lane] = ch + (nc - 1 - lane);   // popped in Morton order
+                sp += nc;
+                __syncwarp();
             }
         }
     }
-    if (!PASS) {
+    if (!PASS && lane == 0) {
         a.n_m2p[g] = nm;
         a.n_p2p[g] = nr;
         atomicAdd(&a.pair_counts[0], pp * (unsigned long long)ntg);
@@ -567,6 +560,8 @@ int pb_tree_build_impl(pb_ctx* ctx)
         PB_CUDA(cudaMemcpyAsync(t.c_last, &root[1], sizeof(int32_t), cudaMemcpyHostToDevice, st));
         PB_CUDA(cudaStreamSynchronize(st));
     }
+    // leaf capacity: larger leaves shorten the upward pass (the latency-bound part of a small problem)
+    t.ncrit_used = ctx->prm.ncrit > 0 ? ctx->prm.ncrit : (Ns < 65536 ? 256 : 192);
     t.gen_start.clear();
     t.gen_start.push_back(0);
     t.gen_start.push_back(1);
@@ -574,7 +569,7 @@ int pb_tree_build_impl(pb_ctx* ctx)
     for (;;) {
         int64_t c0 = t.gen_start[t.gen_start.size() - 2], c1 = t.gen_start.back();
         int64_t ng = c1 - c0;
-        k_cell_split<<<pb_blocks(ng, 128), 128, 0, st>>>(c0, c1, keys, t.c_first, t.c_last, K, ctx->prm.ncrit, nchild, bounds);
+        k_cell_split<<<pb_blocks(ng, 128), 128, 0, st>>>(c0, c1, keys, t.c_first, t.c_last, K, t.ncrit_used, nchild, bounds);
         PB_LAUNCH_CHECK();
         int64_t total = 0;
         PB_TRY(pb_exclusive_scan_i32(ctx, nchild, choff, ng, &total));
@@ -618,11 +613,6 @@ int pb_tree_build_impl(pb_ctx* ctx)
     // --- target groups
     t.n_groups = (N + PB_TG - 1) / PB_TG;
     const int64_t G = t.n_groups;
-    for (int d = 0; d < 3; ++d) PB_TRY(pb_dalloc_t(ctx, &t.g_ctr[d], G, CAT_TREE));
-    PB_TRY(pb_dalloc_t(ctx, &t.g_rad, G, CAT_TREE));
-    k_group_geom<<<pb_blocks(G * 32, 128), 128, 0, st>>>(G, N, t.pc[0], t.pc[1], t.pc[2], t.g_ctr[0], t.g_ctr[1],
-                                                        t.g_ctr[2], t.g_rad);
-    PB_LAUNCH_CHECK();
 
     // --- interaction lists: count, scan, fill
     PB_TRY(pb_dalloc_t(ctx, &t.m2p_off, G + 1, CAT_TREE));
@@ -633,7 +623,7 @@ int pb_tree_build_impl(pb_ctx* ctx)
     a.m2p_min = 8;   // an M2P pair costs about as much as 8 P2P pairs (D: section 7)
     a.c_first = t.c_first; a.c_last = t.c_last; a.c_child = t.c_child; a.c_nchild = t.c_nchild;
     a.cx = t.c_ctr[0]; a.cy = t.c_ctr[1]; a.cz = t.c_ctr[2]; a.crad = t.c_rad;
-    a.gx = t.g_ctr[0]; a.gy = t.g_ctr[1]; a.gz = t.g_ctr[2]; a.grad = t.g_rad;
+    a.px = t.pc[0]; a.py = t.pc[1]; a.pz = t.pc[2];
     int32_t *cnt_m, *cnt_p;
     PB_TRY(pb_dalloc_t(ctx, &cnt_m, G + 1, CAT_TMP));
     PB_TRY(pb_dalloc_t(ctx, &cnt_p, G + 1, CAT_TMP));
@@ -643,7 +633,7 @@ int pb_tree_build_impl(pb_ctx* ctx)
     PB_CUDA(cudaMemsetAsync(pc, 0, 2 * sizeof(unsigned long long), st));
     a.n_m2p = cnt_m; a.n_p2p = cnt_p; a.m2p_cell = nullptr; a.p2p_lo = nullptr; a.p2p_hi = nullptr;
     a.pair_counts = pc;
-    k_lists<0><<<pb_blocks(G, 64), 64, 0, st>>>(a);
+    k_lists<0><<<pb_blocks(G, LIST_WARPS), LIST_WARPS * 32, 0, st>>>(a);
     PB_LAUNCH_CHECK();
     unsigned long long hpc[2];
     PB_CUDA(cudaMemcpyAsync(hpc, pc, sizeof(hpc), cudaMemcpyDeviceToHost, st));
@@ -657,7 +647,7 @@ int pb_tree_build_impl(pb_ctx* ctx)
     PB_TRY(pb_dalloc_t(ctx, &t.p2p_lo, tot_p, CAT_TREE));
     PB_TRY(pb_dalloc_t(ctx, &t.p2p_hi, tot_p, CAT_TREE));
     a.n_m2p = t.m2p_off; a.n_p2p = t.p2p_off; a.m2p_cell = t.m2p_cell; a.p2p_lo = t.p2p_lo; a.p2p_hi = t.p2p_hi;
-    k_lists<1><<<pb_blocks(G, 64), 64, 0, st>>>(a);
+    k_lists<1><<<pb_blocks(G, LIST_WARPS), LIST_WARPS * 32, 0, st>>>(a);
     PB_LAUNCH_CHECK();
     PB_TRY(pb_dalloc_t(ctx, &t.m2p_ctr, tot_m > 0 ? tot_m : 1, CAT_TREE));
     if (tot_m > 0) {
