@@ -449,9 +449,12 @@ __device__ __forceinline__ void m2p_terms(const double2* __restrict__ ff, double
 
 // One block = one work item: a target group (PB_TG targets) x a run of its accepted cells.  The
 // cells' F terms (N_T x {V,K}, contiguous per cell) and centres arrive in shared memory by TMA bulk
-// copies, CT cells per stage, two stages; the block's M2P_S sub-slices (2 warps each) take different
-// cells of a stage for the same targets, so all shared-memory reads are warp-wide broadcasts.
+// copies, CT cells per stage, M2P_NS stages: a "full" mbarrier per stage (TMA completion) and an
+// "empty" one (one arrival per warp) so that no warp ever waits for another warp, only for data.  The
+// block's M2P_S sub-slices (2 warps each) take different cells of a stage for the same targets, so
+// all shared-memory reads are warp-wide broadcasts.
 #define M2P_S 4
+#define M2P_NS 3
 #define M2P_THREADS (PB_TG * M2P_S)
 static_assert(M2P_S == 4, "the final reduction maps one of the 4 outputs to each sub-slice");
 
@@ -459,23 +462,24 @@ template <int P> struct m2p_cfg {
     static constexpr int NT = pb_nt(P);
     static constexpr int CT = P <= 6 ? 8 : 4;                    // cells per stage
     static constexpr size_t RED_BYTES = (size_t)M2P_S * 4 * PB_TG * sizeof(double);   // final reduction reuses the stages
-    static constexpr size_t FF_BYTES0 = (size_t)2 * CT * NT * sizeof(double2);
+    static constexpr size_t FF_BYTES0 = (size_t)M2P_NS * CT * NT * sizeof(double2);
     static constexpr size_t FF_BYTES = FF_BYTES0 > RED_BYTES ? FF_BYTES0 : RED_BYTES;
-    static constexpr size_t SMEM = FF_BYTES + 2 * CT * sizeof(double4) + 2 * sizeof(uint64_t) + 32 * sizeof(double);
+    static constexpr size_t SMEM = FF_BYTES + M2P_NS * CT * sizeof(double4) + 2 * M2P_NS * sizeof(uint64_t) + 32 * sizeof(double);
 };
 
 template <int P>
-__global__ void __launch_bounds__(M2P_THREADS)
+__global__ void __launch_bounds__(M2P_THREADS, 3)
 k_m2p(int64_t N, double kappa, pb_expk ek, const pb_item* __restrict__ items, const int32_t* __restrict__ m2p_cell,
       const double4* __restrict__ m2p_ctr, const double2* __restrict__ FF, const double* __restrict__ px,
       const double* __restrict__ py, const double* __restrict__ pz, double* __restrict__ acc)
 {
-    constexpr int NT = m2p_cfg<P>::NT, CT = m2p_cfg<P>::CT;
+    constexpr int NT = m2p_cfg<P>::NT, CT = m2p_cfg<P>::CT, NS = M2P_NS;
     extern __shared__ __align__(128) unsigned char smraw[];
-    double2* ff = reinterpret_cast<double2*>(smraw);                                  // [2][CT][NT]
-    double4* ctr = reinterpret_cast<double4*>(smraw + m2p_cfg<P>::FF_BYTES);           // [2][CT]
-    uint64_t* bar = reinterpret_cast<uint64_t*>(ctr + 2 * CT);                         // [2]
-    double* Ts = reinterpret_cast<double*>(bar + 2);                                   // [32]
+    double2* ff = reinterpret_cast<double2*>(smraw);                                  // [NS][CT][NT]
+    double4* ctr = reinterpret_cast<double4*>(smraw + m2p_cfg<P>::FF_BYTES);           // [NS][CT]
+    uint64_t* full = reinterpret_cast<uint64_t*>(ctr + NS * CT);                       // [NS]
+    uint64_t* empty = full + NS;                                                       // [NS]
+    double* Ts = reinterpret_cast<double*>(empty + NS);                                // [32]
     const int tid = threadIdx.x;
     const int tgt = tid & (PB_TG - 1), sub = tid / PB_TG;
     const pb_item item = items[blockIdx.x];
@@ -483,8 +487,11 @@ k_m2p(int64_t N, double kappa, pb_expk ek, const pb_item* __restrict__ items, co
     const int32_t e0 = item.r, count = item.count;
     if (tid < 32) Ts[tid] = ek.T[tid];
     if (tid == 0) {
-        pb_mbar_init(&bar[0], 1);
-        pb_mbar_init(&bar[1], 1);
+#pragma unroll
+        for (int s = 0; s < NS; ++s) {
+            pb_mbar_init(&full[s], 1);
+            pb_mbar_init(&empty[s], M2P_THREADS / 32);
+        }
         pb_mbar_fence_init();
     }
     __syncthreads();
@@ -504,28 +511,35 @@ k_m2p(int64_t N, double kappa, pb_expk ek, const pb_item* __restrict__ items, co
     };
     auto issue = [&](int t, int stage) {
         const int n = count - t * CT < CT ? count - t * CT : CT;
-        pb_mbar_expect_tx(&bar[stage], (uint32_t)(n * (sizeof(double4) + NT * sizeof(double2))));
-        pb_bulk_g2s(ctr + stage * CT, m2p_ctr + e0 + t * CT, (uint32_t)(n * sizeof(double4)), &bar[stage]);
+        pb_mbar_expect_tx(&full[stage], (uint32_t)(n * (sizeof(double4) + NT * sizeof(double2))));
+        pb_bulk_g2s(ctr + stage * CT, m2p_ctr + e0 + t * CT, (uint32_t)(n * sizeof(double4)), &full[stage]);
 #pragma unroll
         for (int j = 0; j < CT; ++j)
             if (j < n)
                 pb_bulk_g2s(ff + ((size_t)stage * CT + j) * NT, FF + (int64_t)idn[j] * NT, (uint32_t)(NT * sizeof(double2)),
-                            &bar[stage]);
+                            &full[stage]);
     };
     if (tid == 0 && ntile > 0) {
         load_ids(0);
-        issue(0, 0);
-        if (ntile > 1) load_ids(1);
+        for (int t = 0; t < NS - 1 && t < ntile; ++t) {
+            issue(t, t);
+            if (t + 1 < ntile) load_ids(t + 1);
+        }
     }
     double VL = 0, KL = 0, VY = 0, KY = 0;
     const double k2 = kappa * kappa;
+    int st = 0, ph = 0;                               // stage and phase of tile t
     for (int t = 0; t < ntile; ++t) {
-        const int st = t & 1;
-        if (tid == 0 && t + 1 < ntile) {              // the other stage was released by the barrier below
-            issue(t + 1, st ^ 1);
-            if (t + 2 < ntile) load_ids(t + 2);
+        if (tid == 0) {
+            const int tn = t + NS - 1;                // refill the stage tile t-1 used, once every warp has left it
+            if (tn < ntile) {
+                const int sn = st == 0 ? NS - 1 : st - 1;
+                if (t > 0) pb_mbar_wait(&empty[sn], (uint32_t)(((t - 1) / NS) & 1));
+                issue(tn, sn);
+                if (tn + 1 < ntile) load_ids(tn + 1);
+            }
         }
-        pb_mbar_wait(&bar[st], (t >> 1) & 1u);
+        pb_mbar_wait(&full[st], (uint32_t)ph);
         const int cnt = count - t * CT < CT ? count - t * CT : CT;
 #pragma unroll 1
         for (int j = sub; j < cnt; j += M2P_S) {
@@ -551,9 +565,12 @@ k_m2p(int64_t N, double kappa, pb_expk ek, const pb_item* __restrict__ items, co
                 uY1 = un;
             }
         }
-        __syncthreads();
+        __syncwarp();
+        if ((tid & 31) == 0) pb_mbar_arrive(&empty[st]);
+        if (++st == NS) { st = 0; ph ^= 1; }
     }
-    // add the sub-slices in a fixed order (the stages are free: every thread passed the last barrier)
+    __syncthreads();
+    // add the sub-slices in a fixed order (the stages are free: every thread passed the barrier above)
     double* red = reinterpret_cast<double*>(smraw);   // [M2P_S][4][PB_TG]
     red[(sub * 4 + 0) * PB_TG + tgt] = VL;
     red[(sub * 4 + 1) * PB_TG + tgt] = KL;
@@ -565,6 +582,189 @@ k_m2p(int64_t N, double kappa, pb_expk ek, const pb_item* __restrict__ items, co
         double v = 0;
 #pragma unroll
         for (int q = 0; q < M2P_S; ++q) v += red[(q * 4 + m) * PB_TG + tgt];
+        if (i < N) acc[((int64_t)item.slot * 4 + m) * N + i] = v;
+    }
+}
+
+// ---- M2P, two targets per thread (orders P <= 6) -------------------------------------------------------------
+// With one target per thread every F term costs one 16-byte shared-memory broadcast per two FMAs, and
+// the shared-memory pipe, not the FP64 pipe, sets the pace (ncu: FP64 pipe 65 % busy).  Here a lane
+// carries targets lane and lane + 32 of the group, so each term read feeds four FMAs; a warp covers the
+// whole group, the block's 8 warps take different cells of a stage.
+#define M2Q_W 8
+#define M2Q_NS 4
+#define M2Q_CT 8
+#define M2Q_THREADS (32 * M2Q_W)
+static_assert(PB_TG == 64, "k_m2p2 keeps two targets per lane");
+
+template <int P> struct m2q_cfg {
+    static constexpr int NT = pb_nt(P);
+    static constexpr size_t RED_BYTES = (size_t)M2Q_W * 4 * PB_TG * sizeof(double);
+    static constexpr size_t FF_BYTES0 = (size_t)M2Q_NS * M2Q_CT * NT * sizeof(double2);
+    static constexpr size_t FF_BYTES = FF_BYTES0 > RED_BYTES ? FF_BYTES0 : RED_BYTES;
+    static constexpr size_t SMEM = FF_BYTES + M2Q_NS * M2Q_CT * sizeof(double4) + 2 * M2Q_NS * sizeof(uint64_t) + 32 * sizeof(double);
+};
+
+template <int P>
+__device__ __forceinline__ void m2p_terms2(const double2* __restrict__ ff, double dx0, double dy0, double dz0, double dx1,
+                                           double dy1, double dz1, double (&WV0)[P + 1], double (&WK0)[P + 1],
+                                           double (&WV1)[P + 1], double (&WK1)[P + 1])
+{
+    int e = 0;
+    double xa0 = 1.0, xa1 = 1.0;
+#pragma unroll
+    for (int a = 0; a <= P; ++a) {
+        double xy0 = xa0, xy1 = xa1;
+#pragma unroll
+        for (int b = 0; b <= P - a; ++b) {
+            double m0 = xy0, m1 = xy1;
+#pragma unroll
+            for (int c = 0; c <= P - a - b; ++c) {
+                const int n = a + b + c;
+#pragma unroll
+                for (int j = 0; j <= (P - n) / 2; ++j) {
+                    const double2 f = ff[e];
+                    ++e;
+                    WV0[n + j] = fma(m0, f.x, WV0[n + j]);
+                    WK0[n + j] = fma(m0, f.y, WK0[n + j]);
+                    WV1[n + j] = fma(m1, f.x, WV1[n + j]);
+                    WK1[n + j] = fma(m1, f.y, WK1[n + j]);
+                }
+                m0 *= dz0; m1 *= dz1;
+            }
+            xy0 *= dy0; xy1 *= dy1;
+        }
+        xa0 *= dx0; xa1 *= dx1;
+    }
+}
+
+// radial part: u_m(R) of both kernels against the (P+1) partial sums per layer (D: section 6)
+template <int P>
+__device__ __forceinline__ void m2p_radial(double dx, double dy, double dz, const double (&WV)[P + 1], const double (&WK)[P + 1],
+                                           double kappa, double k2, const pb_expk& ek, const double* __restrict__ Ts,
+                                           double& VL, double& KL, double& VY, double& KY)
+{
+    const double R2 = dx * dx + dy * dy + dz * dz;
+    const double ri = pb_rsqrt(R2), R = R2 * ri, ri2 = ri * ri;
+    const double ex = pb_exp_mkr(R, ek, Ts);
+    double uL = ri, uY0 = ex * ri, uY1 = ex * fma(kappa, R, 1.0) * ri * ri2;
+    VL = fma(uL, WV[0], VL); KL = fma(uL, WK[0], KL);
+    VY = fma(uY0, WV[0], VY); KY = fma(uY0, WK[0], KY);
+#pragma unroll
+    for (int m = 1; m <= P; ++m) {
+        uL = (2 * m - 1) * uL * ri2;
+        VL = fma(uL, WV[m], VL); KL = fma(uL, WK[m], KL);
+        VY = fma(uY1, WV[m], VY); KY = fma(uY1, WK[m], KY);
+        const double un = ((2 * m + 1) * uY1 + k2 * uY0) * ri2;
+        uY0 = uY1;
+        uY1 = un;
+    }
+}
+
+template <int P>
+__global__ void __launch_bounds__(M2Q_THREADS, 2)
+k_m2p2(int64_t N, double kappa, pb_expk ek, const pb_item* __restrict__ items, const int32_t* __restrict__ m2p_cell,
+       const double4* __restrict__ m2p_ctr, const double2* __restrict__ FF, const double* __restrict__ px,
+       const double* __restrict__ py, const double* __restrict__ pz, double* __restrict__ acc)
+{
+    constexpr int NT = m2q_cfg<P>::NT, CT = M2Q_CT, NS = M2Q_NS;
+    extern __shared__ __align__(128) unsigned char smraw[];
+    double2* ff = reinterpret_cast<double2*>(smraw);                                  // [NS][CT][NT]
+    double4* ctr = reinterpret_cast<double4*>(smraw + m2q_cfg<P>::FF_BYTES);           // [NS][CT]
+    uint64_t* full = reinterpret_cast<uint64_t*>(ctr + NS * CT);                       // [NS]
+    uint64_t* empty = full + NS;                                                       // [NS]
+    double* Ts = reinterpret_cast<double*>(empty + NS);                                // [32]
+    const int tid = threadIdx.x;
+    const int lane = tid & 31, sub = tid >> 5;
+    const pb_item item = items[blockIdx.x];
+    const int64_t g = item.group;
+    const int32_t e0 = item.r, count = item.count;
+    if (tid < 32) Ts[tid] = ek.T[tid];
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) {
+            pb_mbar_init(&full[s], 1);
+            pb_mbar_init(&empty[s], M2Q_W);
+        }
+        pb_mbar_fence_init();
+    }
+    __syncthreads();
+    const int64_t i0 = g * PB_TG + lane, i1 = i0 + 32;
+    const int64_t ic0 = i0 < N ? i0 : N - 1, ic1 = i1 < N ? i1 : N - 1;     // padding lanes repeat the last target; never stored
+    const double tx0 = px[ic0], ty0 = py[ic0], tz0 = pz[ic0];
+    const double tx1 = px[ic1], ty1 = py[ic1], tz1 = pz[ic1];
+    const int ntile = (count + CT - 1) / CT;
+
+    int32_t idn[CT];
+    auto load_ids = [&](int t) {
+#pragma unroll
+        for (int j = 0; j < CT; ++j) {
+            const int32_t e = t * CT + j;
+            idn[j] = e < count ? m2p_cell[e0 + e] : 0;
+        }
+    };
+    auto issue = [&](int t, int stage) {
+        const int n = count - t * CT < CT ? count - t * CT : CT;
+        pb_mbar_expect_tx(&full[stage], (uint32_t)(n * (sizeof(double4) + NT * sizeof(double2))));
+        pb_bulk_g2s(ctr + stage * CT, m2p_ctr + e0 + t * CT, (uint32_t)(n * sizeof(double4)), &full[stage]);
+#pragma unroll
+        for (int j = 0; j < CT; ++j)
+            if (j < n)
+                pb_bulk_g2s(ff + ((size_t)stage * CT + j) * NT, FF + (int64_t)idn[j] * NT, (uint32_t)(NT * sizeof(double2)),
+                            &full[stage]);
+    };
+    if (tid == 0 && ntile > 0) {
+        load_ids(0);
+        for (int t = 0; t < NS - 1 && t < ntile; ++t) {
+            issue(t, t);
+            if (t + 1 < ntile) load_ids(t + 1);
+        }
+    }
+    double VL0 = 0, KL0 = 0, VY0 = 0, KY0 = 0, VL1 = 0, KL1 = 0, VY1 = 0, KY1 = 0;
+    const double k2 = kappa * kappa;
+    int st = 0, ph = 0;                               // stage and phase of tile t
+    for (int t = 0; t < ntile; ++t) {
+        if (tid == 0) {
+            const int tn = t + NS - 1;                // refill the stage tile t-1 used, once every warp has left it
+            if (tn < ntile) {
+                const int sn = st == 0 ? NS - 1 : st - 1;
+                if (t > 0) pb_mbar_wait(&empty[sn], (uint32_t)(((t - 1) / NS) & 1));
+                issue(tn, sn);
+                if (tn + 1 < ntile) load_ids(tn + 1);
+            }
+        }
+        pb_mbar_wait(&full[st], (uint32_t)ph);
+        const int cnt = count - t * CT < CT ? count - t * CT : CT;
+#pragma unroll 1
+        for (int j = sub; j < cnt; j += M2Q_W) {
+            const double4 cc = ctr[st * CT + j];
+            const double dx0 = tx0 - cc.x, dy0 = ty0 - cc.y, dz0 = tz0 - cc.z;
+            const double dx1 = tx1 - cc.x, dy1 = ty1 - cc.y, dz1 = tz1 - cc.z;
+            double WV0[P + 1], WK0[P + 1], WV1[P + 1], WK1[P + 1];
+#pragma unroll
+            for (int m = 0; m <= P; ++m) { WV0[m] = 0.0; WK0[m] = 0.0; WV1[m] = 0.0; WK1[m] = 0.0; }
+            m2p_terms2<P>(ff + ((size_t)st * CT + j) * NT, dx0, dy0, dz0, dx1, dy1, dz1, WV0, WK0, WV1, WK1);
+            m2p_radial<P>(dx0, dy0, dz0, WV0, WK0, kappa, k2, ek, Ts, VL0, KL0, VY0, KY0);
+            m2p_radial<P>(dx1, dy1, dz1, WV1, WK1, kappa, k2, ek, Ts, VL1, KL1, VY1, KY1);
+        }
+        __syncwarp();
+        if (lane == 0) pb_mbar_arrive(&empty[st]);
+        if (++st == NS) { st = 0; ph ^= 1; }
+    }
+    __syncthreads();
+    // add the warps' partial sums in a fixed order (the stages are free: every thread passed the barrier above)
+    double* red = reinterpret_cast<double*>(smraw);   // [M2Q_W][4][PB_TG]
+    red[(sub * 4 + 0) * PB_TG + lane] = VL0; red[(sub * 4 + 0) * PB_TG + lane + 32] = VL1;
+    red[(sub * 4 + 1) * PB_TG + lane] = KL0; red[(sub * 4 + 1) * PB_TG + lane + 32] = KL1;
+    red[(sub * 4 + 2) * PB_TG + lane] = VY0; red[(sub * 4 + 2) * PB_TG + lane + 32] = VY1;
+    red[(sub * 4 + 3) * PB_TG + lane] = KY0; red[(sub * 4 + 3) * PB_TG + lane + 32] = KY1;
+    __syncthreads();
+    {
+        const int m = tid / PB_TG, tgt = tid & (PB_TG - 1);
+        const int64_t i = g * PB_TG + tgt;
+        double v = 0;
+#pragma unroll
+        for (int q = 0; q < M2Q_W; ++q) v += red[(q * 4 + m) * PB_TG + tgt];
         if (i < N) acc[((int64_t)item.slot * 4 + m) * N + i] = v;
     }
 }
@@ -761,6 +961,21 @@ k_combine(int64_t N, const int32_t* __restrict__ itemP_off, const int32_t* __res
 
 // ---- host driver ----------------------------------------------------------------------------------------------
 template <int P>
+static cudaError_t launch_m2p2(pb_ctx* ctx, cudaStream_t fs)
+{
+    pb_tree& t = ctx->tree;
+    static bool attr_set = false;   // per instantiation; the attribute belongs to the function, not the context
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(k_m2p2<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m2q_cfg<P>::SMEM);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    k_m2p2<P><<<(unsigned)t.n_itemM, M2Q_THREADS, m2q_cfg<P>::SMEM, fs>>>(
+        t.N, ctx->prm.kappa, t.ek, t.itemM, t.m2p_cell, t.m2p_ctr, t.FF, t.pc[0], t.pc[1], t.pc[2], t.accM);
+    return cudaSuccess;
+}
+
+template <int P>
 static cudaError_t launch_m2p(pb_ctx* ctx, cudaStream_t fs)
 {
     pb_tree& t = ctx->tree;
@@ -805,13 +1020,13 @@ static int pb_far_branch(pb_ctx* ctx, cudaStream_t fs, bool timed)
         PB_TRY(pb_prof_begin(ctx, 1));
         cudaError_t e = cudaSuccess;
         switch (t.P) {
-        case 0: e = launch_m2p<0>(ctx, fs); break;
-        case 1: e = launch_m2p<1>(ctx, fs); break;
-        case 2: e = launch_m2p<2>(ctx, fs); break;
-        case 3: e = launch_m2p<3>(ctx, fs); break;
-        case 4: e = launch_m2p<4>(ctx, fs); break;
-        case 5: e = launch_m2p<5>(ctx, fs); break;
-        case 6: e = launch_m2p<6>(ctx, fs); break;
+        case 0: e = launch_m2p2<0>(ctx, fs); break;
+        case 1: e = launch_m2p2<1>(ctx, fs); break;
+        case 2: e = launch_m2p2<2>(ctx, fs); break;
+        case 3: e = launch_m2p2<3>(ctx, fs); break;
+        case 4: e = launch_m2p2<4>(ctx, fs); break;
+        case 5: e = launch_m2p2<5>(ctx, fs); break;
+        case 6: e = launch_m2p2<6>(ctx, fs); break;
         case 7: e = launch_m2p<7>(ctx, fs); break;
         case 8: e = launch_m2p<8>(ctx, fs); break;
         case 9: e = launch_m2p<9>(ctx, fs); break;

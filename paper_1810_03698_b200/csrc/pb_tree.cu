@@ -412,7 +412,7 @@ __global__ void k_items_count(int64_t ng, const int32_t* __restrict__ off, const
 }
 
 __global__ void k_items_fill(int64_t ng, const int32_t* __restrict__ off, const int32_t* __restrict__ lo,
-                             const int32_t* __restrict__ hi, const int32_t* __restrict__ item_off,
+                             const int32_t* __restrict__ hi, const int32_t* __restrict__ item_off, int quantum,
                              pb_item* __restrict__ items)
 {
     int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
@@ -425,7 +425,8 @@ __global__ void k_items_fill(int64_t ng, const int32_t* __restrict__ off, const 
     int32_t r = off[g];
     int64_t passed = 0;                     // units before entry r
     for (int32_t j = 0; j < n; ++j) {
-        const int64_t b = tot * j / n, e = tot * (j + 1) / n;
+        // cuts fall on multiples of `quantum` units, so a block's warps all get the same number of cells
+        const int64_t b = tot * j / n / quantum * quantum, e = j + 1 == n ? tot : tot * (j + 1) / n / quantum * quantum;
         pb_item it;
         it.group = (int32_t)g;
         it.slot = j;
@@ -445,7 +446,7 @@ __global__ void k_items_fill(int64_t ng, const int32_t* __restrict__ off, const 
 
 // builds one item table; returns the item count and the largest number of items of one group
 static int pb_build_items(pb_ctx* ctx, int64_t G, const int32_t* off, const int32_t* lo, const int32_t* hi,
-                          int item_size, int max_items, int32_t** item_off_out, pb_item** items_out,
+                          int item_size, int max_items, int quantum, int32_t** item_off_out, pb_item** items_out,
                           int64_t* n_items, int* max_per_group)
 {
     cudaStream_t st = ctx->stream;
@@ -463,7 +464,7 @@ static int pb_build_items(pb_ctx* ctx, int64_t G, const int32_t* off, const int3
     PB_TRY(pb_exclusive_scan_i32(ctx, cnt, ioff, G + 1, &total));   // synchronises
     pb_item* items;
     PB_TRY(pb_dalloc_t(ctx, &items, total > 0 ? total : 1, CAT_TREE));
-    k_items_fill<<<pb_blocks(G, 128), 128, 0, st>>>(G, off, lo, hi, ioff, items);
+    k_items_fill<<<pb_blocks(G, 128), 128, 0, st>>>(G, off, lo, hi, ioff, quantum, items);
     PB_LAUNCH_CHECK();
     *item_off_out = ioff;
     *items_out = items;
@@ -662,12 +663,13 @@ int pb_tree_build_impl(pb_ctx* ctx)
         int64_t szP = (t.p2p_pairs / PB_TG + slots - 1) / slots;
         if (szP < 128) szP = 128;
         if (szP > (1 << 30)) szP = 1 << 30;
-        PB_TRY(pb_build_items(ctx, G, t.p2p_off, t.p2p_lo, t.p2p_hi, (int)szP, 64, &t.itemP_off, &t.itemP, &t.n_itemP,
+        PB_TRY(pb_build_items(ctx, G, t.p2p_off, t.p2p_lo, t.p2p_hi, (int)szP, 64, 4, &t.itemP_off, &t.itemP, &t.n_itemP,
                               &t.nslot_p2p));
         int64_t szM = (t.m2p_pairs / PB_TG + slots - 1) / slots;
-        if (szM < 4) szM = 4;
+        if (szM < 8) szM = 8;
+        szM = (szM + 7) / 8 * 8;                      // whole tiles of 8 cells: one per warp of k_m2p2
         if (szM > (1 << 30)) szM = 1 << 30;
-        PB_TRY(pb_build_items(ctx, G, t.m2p_off, nullptr, nullptr, (int)szM, 64, &t.itemM_off, &t.itemM, &t.n_itemM,
+        PB_TRY(pb_build_items(ctx, G, t.m2p_off, nullptr, nullptr, (int)szM, 64, 8, &t.itemM_off, &t.itemM, &t.n_itemM,
                               &t.nslot_m2p));
         if (t.nslot_p2p < 1) t.nslot_p2p = 1;
         if (t.nslot_m2p < 1) t.nslot_m2p = 1;
