@@ -339,6 +339,100 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_sweep(args):
+    """BASELINE configs[4]: matvec throughput over theta x P on one workload (default C4), each with its
+    error on seeded sampled rows against the oracle's direct sum, then one full polarizable solve at the
+    workload's own theta, P.  One JSON line per case; not the driver's bench line."""
+    import numpy as np
+    import torch
+    from paper_1810_03698_b200 import pb
+    from oracle import pb_oracle as po
+    torch.cuda.set_device(0)
+    w = load_workload(args.workload)
+    nt = int(w.tris.shape[0])
+    x = np.random.Generator(np.random.PCG64(7)).normal(size=2 * nt)
+    rows = np.sort(np.random.Generator(np.random.PCG64(8)).choice(nt, size=min(args.sweep_rows, nt), replace=False))
+    po.build()
+    orc = po.Oracle(w.verts, w.tris, po.Params(K_far=w.params["K_far"]))
+    t0 = time.perf_counter()
+    y1, y2 = orc.matvec(x, rows)
+    t_or = time.perf_counter() - t0
+    yref = np.concatenate([y1, y2])
+    print(json.dumps({"case": "oracle", "workload": w.name, "panels": nt, "rows": int(rows.size), "seconds": t_or,
+                      "cores": po.num_threads(), "pairs_per_s": float(rows.size) * nt * w.params["K_far"] / t_or}), flush=True)
+    ctx = pb.from_workload(w)
+    xd = torch.from_numpy(x).cuda()
+    y = torch.empty_like(xd)
+    idx = torch.from_numpy(np.concatenate([rows, nt + rows])).cuda()
+    cases = set(args.sweep_cases.split(","))
+    for theta in (0.3, 0.5, 0.7):
+        for P in (4, 6, 8):
+            if "matvec" not in cases:
+                break
+            ctx.set_params(theta=theta, order_P=P)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); ctx.tree_build(); e1.record(); e1.synchronize()
+            t_build = e0.elapsed_time(e1)
+            for _ in range(3):
+                ctx.matvec(xd, out=y)
+            ts = []
+            for _ in range(5):
+                e0.record(); ctx.matvec(xd, out=y); e1.record(); e1.synchronize()
+                ts.append(e0.elapsed_time(e1))
+            ms = sorted(ts)[len(ts) // 2]
+            ctx.matvec(xd, out=y, timed=True)
+            st = ctx.stats()
+            lm = st["last_matvec_ms"]
+            got = y[idx].cpu().numpy()
+            err = float(np.linalg.norm(got - yref) / np.linalg.norm(yref))
+            fl_m = m2p_flop_per_pair(P, st["n_terms"])
+            print(json.dumps({
+                "case": "matvec", "workload": w.name, "theta": theta, "order_P": P, "ncrit": int(st["ncrit_used"]),
+                "ms_per_matvec": ms, "tree_build_ms": t_build,
+                "interactions_per_s": float(nt) * st["n_sources"] / (ms * 1e-3),
+                "p2p_pairs": int(st["p2p_pairs"]), "m2p_pairs": int(st["m2p_pairs"]),
+                "serial_ms": {k: lm[k] for k in ("weights", "p2m_m2m", "m2p", "p2p", "near_combine")},
+                "p2p_tflops": P2P_FLOP_PER_PAIR * st["p2p_pairs"] / (lm["p2p"] * 1e-3) / 1e12,
+                "m2p_tflops": fl_m * st["m2p_pairs"] / (lm["m2p"] * 1e-3) / 1e12 if lm["m2p"] > 0 else 0.0,
+                "fp64_peak_tflops": FP64_PEAK_TFLOPS, "rel_l2_vs_oracle_rows": err, "device_gb": st["device_bytes"] / 1e9}), flush=True)
+    ctx.set_params(**{k: v for k, v in w.params.items() if k in ("theta", "order_P")})
+    ctx.tree_build()
+    if "gmres" in cases:
+        # the Krylov vector kernels at this size (HBM-bound: the basis does not fit in L2): a capped GMRES run
+        iters = args.gmres_iters
+        ctx.set_params(gmres_maxit=iters, gmres_tol=1e-30)
+        b = ctx.rhs_multipole()
+        ctx.gmres(b)                                   # warm-up: workspace allocation
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); _, info = ctx.gmres(b); e1.record(); e1.synchronize()
+        ms_g = e0.elapsed_time(e1)
+        e0.record()
+        for _ in range(5):
+            ctx.matvec(xd, out=y)
+        e1.record(); e1.synchronize()
+        ms_mv = e0.elapsed_time(e1) / 5
+        n2 = 2 * nt
+        # per iteration j (nv = j+1 basis vectors): two dot passes read nv+1 vectors, two updates read nv+1 and write 1 (+1 for v_next)
+        byts = sum((2 * (j + 2) + 2 * (j + 2) + 3) * n2 * 8 for j in range(info["iters"]))
+        ms_vec = ms_g - (info["iters"] + 2) * ms_mv
+        print(json.dumps({"case": "gmres_vectors", "workload": w.name, "iters": info["iters"], "ms_total": ms_g, "ms_per_matvec": ms_mv,
+                          "ms_vector_kernels": ms_vec, "algorithmic_gb": byts / 1e9, "gb_per_s": byts / 1e9 / (ms_vec * 1e-3),
+                          "hbm_peak_gb_per_s_measured": 6548.2}), flush=True)
+        ctx.set_params(gmres_maxit=1000, gmres_tol=float(w.params["gmres_tol"]))
+    if "solve" not in cases:
+        ctx.close()
+        return
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    _, _, res = ctx.solve()
+    torch.cuda.synchronize()
+    print(json.dumps({"case": "solve", "workload": w.name, "sites": int(w.sites["pos"].shape[0]), "seconds": time.perf_counter() - t0,
+                      **{k: res[k] for k in ("dG_solv", "scf_iters", "scf_iters_vac", "gmres_iters_total", "matvecs_total",
+                                             "final_scf_delta_debye", "final_gmres_relres", "status")}}), flush=True)
+    ctx.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -352,8 +446,15 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--profiler-range", action="store_true",
                     help="bracket the timed resident steps with cudaProfilerStart/Stop (for ncu --profile-from-start off)")
+    ap.add_argument("--sweep", action="store_true",
+                    help="theta x P matvec sweep with sampled-row accuracy and one full solve (BASELINE configs[4]); use with --workload C4")
+    ap.add_argument("--sweep-rows", type=int, default=1024)
+    ap.add_argument("--sweep-cases", default="matvec,solve", help="comma list of matvec, gmres, solve")
+    ap.add_argument("--gmres-iters", type=int, default=40)
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -21,7 +21,6 @@ __global__ void __launch_bounds__(DOT_THREADS)
 k_dots(int64_t n, int nv, const double* __restrict__ V, int64_t ld, const double* __restrict__ w, int self,
        double* __restrict__ partial, unsigned int* __restrict__ counter, double* __restrict__ hout)
 {
-    __shared__ double sw[DOT_CHUNK];
     __shared__ bool last;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int nvt = nv + (self ? 1 : 0);
@@ -30,21 +29,46 @@ k_dots(int64_t n, int nv, const double* __restrict__ V, int64_t ld, const double
     double acc[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) acc[r] = 0.0;
-    for (int64_t c = blockIdx.x; c < nchunk; c += gridDim.x) {
-        const int64_t e0 = c * DOT_CHUNK;
-        const int cnt = (int)(n - e0 < DOT_CHUNK ? n - e0 : DOT_CHUNK);
-        __syncthreads();
-        for (int k = threadIdx.x; k < DOT_CHUNK; k += DOT_THREADS) sw[k] = k < cnt ? w[e0 + k] : 0.0;
-        __syncthreads();
+    // Warps are independent (no shared memory, no block barrier): a warp keeps its chunk of w in registers
+    // (w is read once per group of R vectors and stays in L2) and streams R basis vectors against it with
+    // eight independent 16-byte loads per lane and vector in flight.
+    if (j0 < nvt) {
+        for (int64_t c = blockIdx.x; c < nchunk; c += gridDim.x) {
+            const int64_t e0 = c * DOT_CHUNK;
+            const int cnt = (int)(n - e0 < DOT_CHUNK ? n - e0 : DOT_CHUNK);
+            if (cnt == DOT_CHUNK) {
+                const double2* w2 = reinterpret_cast<const double2*>(w + e0);
+                double2 b[DOT_CHUNK / 64];
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const int j = j0 + r * DOT_WARPS;
-            if (j < nvt) {
-                const double* v = (j < nv ? V + (int64_t)j * ld : w) + e0;
-                double s = 0;
-#pragma unroll 4
-                for (int k = lane; k < cnt; k += 32) s = fma(v[k], sw[k], s);
-                acc[r] += s;
+                for (int i = 0; i < DOT_CHUNK / 64; ++i) b[i] = w2[lane + 32 * i];
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const int j = j0 + r * DOT_WARPS;
+                    if (j < nvt) {
+                        const double2* v2 = reinterpret_cast<const double2*>((j < nv ? V + (int64_t)j * ld : w) + e0);
+                        double2 a[DOT_CHUNK / 64];
+#pragma unroll
+                        for (int i = 0; i < DOT_CHUNK / 64; ++i) a[i] = v2[lane + 32 * i];
+                        double s = 0;
+#pragma unroll
+                        for (int i = 0; i < DOT_CHUNK / 64; ++i) {
+                            s = fma(a[i].x, b[i].x, s);
+                            s = fma(a[i].y, b[i].y, s);
+                        }
+                        acc[r] += s;
+                    }
+                }
+            } else {
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const int j = j0 + r * DOT_WARPS;
+                    if (j < nvt) {
+                        const double* v = (j < nv ? V + (int64_t)j * ld : w) + e0;
+                        double s = 0;
+                        for (int k = lane; k < cnt; k += 32) s = fma(v[k], w[e0 + k], s);
+                        acc[r] += s;
+                    }
+                }
             }
         }
     }
@@ -63,10 +87,19 @@ k_dots(int64_t n, int nv, const double* __restrict__ V, int64_t ld, const double
     __syncthreads();
     if (!last) return;
     __threadfence();
-    for (int j = threadIdx.x; j < nvt; j += DOT_THREADS) {
-        double s = 0;
-        for (unsigned b = 0; b < gridDim.x; ++b) s += __ldcg(&partial[(int64_t)b * nvt + j]);
-        hout[j] = s;
+    for (int j = wid; j < nvt; j += DOT_WARPS) {        // a warp per vector: lanes stride over the blocks, then a butterfly
+        double s0 = 0, s1 = 0, s2 = 0, s3 = 0;          // four loads in flight; the summation pattern is fixed
+        unsigned b = lane;
+        for (; b + 96 < gridDim.x; b += 128) {
+            s0 += __ldcg(&partial[(int64_t)b * nvt + j]);
+            s1 += __ldcg(&partial[(int64_t)(b + 32) * nvt + j]);
+            s2 += __ldcg(&partial[(int64_t)(b + 64) * nvt + j]);
+            s3 += __ldcg(&partial[(int64_t)(b + 96) * nvt + j]);
+        }
+        for (; b < gridDim.x; b += 32) s0 += __ldcg(&partial[(int64_t)b * nvt + j]);
+        double s = (s0 + s1) + (s2 + s3);
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        if (lane == 0) hout[j] = s;
     }
     if (threadIdx.x == 0) *counter = 0u;              // ready for the next launch on this stream
 }
@@ -162,13 +195,23 @@ static int dot_into(pb_ctx* ctx, gmres_ws& ws, int nv, const double* V, const do
     const int nvt = nv + (self ? 1 : 0);
     const int64_t nchunk = (ws.n + DOT_CHUNK - 1) / DOT_CHUNK;
     const int gy1 = (nvt + DOT_WARPS - 1) / DOT_WARPS;
-    if (nchunk * gy1 <= DOT_MAXBLK) {
+    if (nchunk * gy1 <= DOT_MAXBLK) {                     // short vectors: one chunk per block, spread wide (latency)
         dim3 grid((unsigned)nchunk, (unsigned)gy1);
         k_dots<1><<<grid, DOT_THREADS, 0, ctx->stream>>>(ws.n, nv, V, ws.n, w, self ? 1 : 0, ws.partial, ws.counter, hout);
-    } else {
+    } else {                                              // long vectors: two full waves of resident blocks (bandwidth)
+        static int occ = 0;
+        if (occ == 0) {
+            PB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_dots<4>, DOT_THREADS, 0));
+            if (occ < 1) occ = 1;
+            if (occ > 8) occ = 8;
+        }
+        int nsm = 148;
+        cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, ctx->device);
+        const int resident = 2 * nsm * occ < DOT_MAXBLK ? 2 * nsm * occ : DOT_MAXBLK;
         const int gy = (nvt + 4 * DOT_WARPS - 1) / (4 * DOT_WARPS);
-        int64_t gx = DOT_MAXBLK / gy;
+        int64_t gx = resident / gy;
         if (gx > nchunk) gx = nchunk;
+        if (gx < 1) gx = 1;
         dim3 grid((unsigned)gx, (unsigned)gy);
         k_dots<4><<<grid, DOT_THREADS, 0, ctx->stream>>>(ws.n, nv, V, ws.n, w, self ? 1 : 0, ws.partial, ws.counter, hout);
     }
