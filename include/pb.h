@@ -186,6 +186,21 @@ int pb_solve(pb_ctx* ctx, double* x_out, double* mu_out, pb_result* result);
 /* Same with HOST outputs (x_host [2 nt], mu_host [na][3], either may be NULL). */
 int pb_solve_host(pb_ctx* ctx, double* x_host, double* mu_host, pb_result* result);
 
+/* Binding thermodynamic cycle of Fig. 3 from three finished solves -- the complex AB
+ * and the separate molecules A and B, each its own context / mesh / sites (HOST structs, no GPU work):
+ *   dG_bind_vac  = G_vac,AB - G_vac,A - G_vac,B                        Eq. (26), the polarization energy
+ *                  being implicit in Eq. (24)'s G
+ *   ddG_bind     = dG_solv,AB - dG_solv,A - dG_solv,B                  Eq. (27)
+ *   dG_bind_diss = ddG_bind + dG_bind_vac                              Eq. (25)
+ * all in kcal/mol.  Returns PB_ERR_INVALID_ARG on NULL, PB_ERR_NO_CONVERGENCE if any of the three
+ * solves carries that status (the numbers are still filled in). */
+typedef struct pb_binding {
+    double dG_bind_vac;
+    double ddG_bind;
+    double dG_bind_diss;
+} pb_binding;
+int pb_binding_cycle(const pb_result* ab, const pb_result* a, const pb_result* b, pb_binding* out);
+
 int pb_get_stats(pb_ctx* ctx, pb_stats* out /* HOST */);
 
 /* Profiling: when on, every P2P and M2P launch is bracketed by a CUDA-event pair on the

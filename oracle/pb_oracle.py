@@ -297,3 +297,16 @@ class Oracle:
                     G_solvterm=c * G_solv, G_mult_diss=c * G_mult, G_vac=c * G_vac,
                     dG_solv=c * (G_solv + G_mult - G_vac),
                     phi_solv=phi_s, grad_solv=g_s, hess_solv=h_s)
+
+
+def binding_cycle(sol_ab: dict, sol_a: dict, sol_b: dict) -> dict:
+    """The thermodynamic cycle of Fig. 3 from three `Oracle.solve` results
+    (complex AB, molecule A, molecule B; kcal/mol):
+      Eq. (26)  dG_bind_vac  = G_AB - G_A - G_B + W_pol, with G the vacuum Coulomb energy; using
+                Eq. (24)'s G (permanent dipole d in place of p) carries W_pol implicitly (P:232);
+      Eq. (27)  ddG_bind     = dG_solv,AB - dG_solv,A - dG_solv,B;
+      Eq. (25)  dG_bind_diss = dG_solv,AB + dG_bind_vac - dG_solv,A - dG_solv,B."""
+    dG_bind_vac = sol_ab["G_vac"] - sol_a["G_vac"] - sol_b["G_vac"]
+    ddG_bind = sol_ab["dG_solv"] - sol_a["dG_solv"] - sol_b["dG_solv"]
+    dG_bind_diss = sol_ab["dG_solv"] + dG_bind_vac - sol_a["dG_solv"] - sol_b["dG_solv"]
+    return dict(dG_bind_vac=dG_bind_vac, ddG_bind=ddG_bind, dG_bind_diss=dG_bind_diss)

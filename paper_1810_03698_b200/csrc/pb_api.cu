@@ -303,6 +303,17 @@ extern "C" int pb_tree_build(pb_ctx* ctx)
     return PB_OK;
 }
 
+// Eq. (25)-(27): the binding cycle from three solves (host arithmetic on result structs)
+extern "C" int pb_binding_cycle(const pb_result* ab, const pb_result* a, const pb_result* b, pb_binding* out)
+{
+    if (!ab || !a || !b || !out) return PB_ERR_INVALID_ARG;
+    out->dG_bind_vac = ab->G_vac - a->G_vac - b->G_vac;          // Eq. (26), W_pol implicit in Eq. (24)
+    out->ddG_bind = ab->dG_solv - a->dG_solv - b->dG_solv;       // Eq. (27)
+    out->dG_bind_diss = out->ddG_bind + out->dG_bind_vac;        // Eq. (25)
+    if (ab->status != PB_OK || a->status != PB_OK || b->status != PB_OK) return PB_ERR_NO_CONVERGENCE;
+    return PB_OK;
+}
+
 extern "C" int pb_get_stats(pb_ctx* ctx, pb_stats* out)
 {
     if (!ctx || !out) return PB_ERR_INVALID_ARG;

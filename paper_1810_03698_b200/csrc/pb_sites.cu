@@ -7,17 +7,24 @@
 
 // ---- H10: right-hand side -----------------------------------------------------------------------------
 // b_i = 1/(4 pi eps_in) sum_k [ q_k/R + p_k.d/R^3 + d.Q_k.d/(2 R^5) ],  d = c_i - r_k,  p = dip + mu.
+// Two collocation points per thread: every site value read from shared memory feeds two pairs.
 #define RHS_TILE 64
+#define RHS_TPT 2
 __global__ void __launch_bounds__(128)
 k_rhs(int64_t N, int64_t na, const double* __restrict__ cen, const double* __restrict__ pos,
       const double* __restrict__ q, const double* __restrict__ dip, const double* __restrict__ mu,
       const double* __restrict__ quad, double inv_eps, double* __restrict__ b)
 {
     __shared__ double s[13][RHS_TILE];
-    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    const bool live = i < N;
-    const double x = live ? cen[3 * i] : 1e30, y = live ? cen[3 * i + 1] : 1e30, z = live ? cen[3 * i + 2] : 1e30;
-    double sum = 0;
+    const int64_t i0 = blockIdx.x * (int64_t)(blockDim.x * RHS_TPT) + threadIdx.x;
+    double x[RHS_TPT], y[RHS_TPT], z[RHS_TPT], sum[RHS_TPT];
+#pragma unroll
+    for (int t = 0; t < RHS_TPT; ++t) {
+        const int64_t i = i0 + t * blockDim.x;
+        const int64_t ic = i < N ? i : N - 1;                // padding lanes repeat the last point; never stored
+        x[t] = cen[3 * ic]; y[t] = cen[3 * ic + 1]; z[t] = cen[3 * ic + 2];
+        sum[t] = 0.0;
+    }
     for (int64_t k0 = 0; k0 < na; k0 += RHS_TILE) {
         const int cnt = (int)(na - k0 < RHS_TILE ? na - k0 : RHS_TILE);
         __syncthreads();
@@ -28,22 +35,34 @@ k_rhs(int64_t N, int64_t na, const double* __restrict__ cen, const double* __res
                 s[4 + d][k] = dip[3 * m + d] + (mu ? mu[3 * m + d] : 0.0);
             }
             s[3][k] = q[m];
-            for (int d = 0; d < 6; ++d) s[7 + d][k] = quad[6 * m + d];
+            // d.Q.d/2 = (Qxx dx^2 + Qyy dy^2 + Qzz dz^2)/2 + Qxy dx dy + Qxz dx dz + Qyz dy dz
+            s[7][k] = 0.5 * quad[6 * m]; s[8][k] = quad[6 * m + 1]; s[9][k] = quad[6 * m + 2];
+            s[10][k] = 0.5 * quad[6 * m + 3]; s[11][k] = quad[6 * m + 4]; s[12][k] = 0.5 * quad[6 * m + 5];
         }
         __syncthreads();
+#pragma unroll 2
         for (int k = 0; k < cnt; ++k) {
-            const double dx = x - s[0][k], dy = y - s[1][k], dz = z - s[2][k];
-            const double r2 = dx * dx + dy * dy + dz * dz;
-            const double ri = rsqrt(r2), ri2 = ri * ri, ri3 = ri * ri2, ri5 = ri3 * ri2;
-            const double pd = s[4][k] * dx + s[5][k] * dy + s[6][k] * dz;
-            const double dQd = s[7][k] * dx * dx + s[10][k] * dy * dy + s[12][k] * dz * dz +
-                               2.0 * (s[8][k] * dx * dy + s[9][k] * dx * dz + s[11][k] * dy * dz);
-            sum += s[3][k] * ri + pd * ri3 + 0.5 * dQd * ri5;
+            const double sx = s[0][k], sy = s[1][k], sz = s[2][k], qk = s[3][k];
+            const double p0 = s[4][k], p1 = s[5][k], p2 = s[6][k];
+            const double qxx = s[7][k], qxy = s[8][k], qxz = s[9][k], qyy = s[10][k], qyz = s[11][k], qzz = s[12][k];
+#pragma unroll
+            for (int t = 0; t < RHS_TPT; ++t) {
+                const double dx = x[t] - sx, dy = y[t] - sy, dz = z[t] - sz;
+                const double r2 = dx * dx + dy * dy + dz * dz;
+                const double ri = pb_rsqrt(r2), ri2 = ri * ri, ri3 = ri * ri2, ri5 = ri3 * ri2;
+                const double pd = p0 * dx + p1 * dy + p2 * dz;
+                const double hQ = dx * (qxx * dx + qxy * dy + qxz * dz) + dy * (qyy * dy + qyz * dz) + qzz * dz * dz;
+                sum[t] += qk * ri + pd * ri3 + hQ * ri5;
+            }
         }
     }
-    if (live) {
-        b[i] = PB_INV4PI * inv_eps * sum;
-        b[N + i] = 0.0;   // second block of Eq. (5)'s right side
+#pragma unroll
+    for (int t = 0; t < RHS_TPT; ++t) {
+        const int64_t i = i0 + t * blockDim.x;
+        if (i < N) {
+            b[i] = PB_INV4PI * inv_eps * sum[t];
+            b[N + i] = 0.0;   // second block of Eq. (5)'s right side
+        }
     }
 }
 
@@ -53,8 +72,8 @@ extern "C" int pb_rhs_multipole(pb_ctx* ctx, const double* mu_induced, double* b
     if (!ctx->mesh_loaded || !ctx->sites.loaded) return pb_fail(ctx, PB_ERR_NOT_READY, "pb_rhs_multipole: load mesh and sites first");
     if (!b) return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_rhs_multipole: NULL output");
     const pb_sites& s = ctx->sites;
-    k_rhs<<<pb_blocks(ctx->nt, 128), 128, 0, ctx->stream>>>(ctx->nt, s.na, ctx->cen, s.pos, s.q, s.dip, mu_induced, s.quad,
-                                                          1.0 / ctx->prm.eps_in, b);
+    k_rhs<<<pb_blocks(ctx->nt, 128 * RHS_TPT), 128, 0, ctx->stream>>>(ctx->nt, s.na, ctx->cen, s.pos, s.q, s.dip, mu_induced,
+                                                                    s.quad, 1.0 / ctx->prm.eps_in, b);
     PB_LAUNCH_CHECK();
     return PB_OK;
 }
@@ -70,7 +89,7 @@ __device__ __forceinline__ void react_point(double dx, double dy, double dz, dou
                                             double kz, double* __restrict__ o)
 {
     const double r2 = dx * dx + dy * dy + dz * dz;
-    const double ri = rsqrt(r2), ri2 = ri * ri, ri3 = ri * ri2, ri5 = ri3 * ri2;
+    const double ri = pb_rsqrt(r2), ri2 = ri * ri, ri3 = ri * ri2, ri5 = ri3 * ri2;
     const double kd = kx * dx + ky * dy + kz * dz;
     o[0] += wS * ri - kd * ri3;
     const double g = -wS * ri3 + 3.0 * kd * ri5;   // coefficient of d

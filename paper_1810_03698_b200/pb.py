@@ -27,7 +27,7 @@ EXPORTS = [
     "pb_get_params", "pb_mesh_load", "pb_sites_load", "pb_tree_build", "pb_rhs_multipole", "pb_matvec",
     "pb_matvec_timed", "pb_matvec_host", "pb_reaction_field", "pb_multipole_field", "pb_gmres", "pb_solve",
     "pb_solve_host", "pb_get_stats", "pb_fp64_peak_probe", "pb_set_profiling", "pb_quadrature_rule",
-    "pb_gauss_legendre", "pb_farfield_table",
+    "pb_gauss_legendre", "pb_farfield_table", "pb_binding_cycle",
 ]
 
 
@@ -60,6 +60,10 @@ class Result(ctypes.Structure):
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_ if k != "reserved"}
+
+
+class Binding(ctypes.Structure):
+    _fields_ = [("dG_bind_vac", ctypes.c_double), ("ddG_bind", ctypes.c_double), ("dG_bind_diss", ctypes.c_double)]
 
 
 class Stats(ctypes.Structure):
@@ -135,11 +139,28 @@ def lib():
         L.pb_quadrature_rule.argtypes = [ctypes.c_int, vp, vp]
         L.pb_gauss_legendre.argtypes = [ctypes.c_int, vp, vp]
         L.pb_farfield_table.argtypes = [ctypes.c_int, vp, vp, vp, vp, ctypes.POINTER(i64)]
+        L.pb_binding_cycle.argtypes = [ctypes.POINTER(Result)] * 3 + [ctypes.POINTER(Binding)]
         for name in EXPORTS:
             if name not in ("pb_last_error", "pb_default_params"):
                 getattr(L, name).restype = ctypes.c_int
         _lib = L
     return _lib
+
+
+def binding_cycle(res_ab: dict, res_a: dict, res_b: dict) -> dict:
+    """Eq. (25)-(27) from the result dicts of three `PB.solve()` calls (complex, A, B)."""
+    rs = []
+    for r in (res_ab, res_a, res_b):
+        c = Result()
+        for k, _ in Result._fields_:
+            if k in r:
+                setattr(c, k, r[k])
+        rs.append(c)
+    out = Binding()
+    rc = lib().pb_binding_cycle(ctypes.byref(rs[0]), ctypes.byref(rs[1]), ctypes.byref(rs[2]), ctypes.byref(out))
+    if rc not in (PB_OK, PB_ERR_NO_CONVERGENCE):
+        raise PBError(rc, "pb_binding_cycle")
+    return dict(dG_bind_vac=out.dG_bind_vac, ddG_bind=out.ddG_bind, dG_bind_diss=out.dG_bind_diss, converged=rc == PB_OK)
 
 
 def default_params() -> Params:

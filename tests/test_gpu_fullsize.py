@@ -117,3 +117,53 @@ def test_polarizable_solve_full_size(pbm, po, torch_cuda, name):
     assert abs(res["scf_iters"] - ref["scf_iters"]) <= 1 and res["scf_iters_vac"] == ref["scf_iters_vac"]
     assert res["final_scf_delta_debye"] < 1e-7
     ctx.close()
+
+
+def test_binding_triple_against_oracle(pbm, po, torch_cuda):
+    """BASELINE configs[3]'s shape at a size the oracle can solve densely: receptor globule + ligand 3 A off
+    its surface, three independent polarizable solves (complex, receptor, ligand), the cycle of Eq. (25)-(27)
+    through pb_binding_cycle against the oracle's."""
+    from paper_1810_03698_b200.workloads import make_config
+    sols, ress, scale = [], [], 0.0
+    for which in ("complex", "receptor", "ligand"):
+        w = make_config("C3", which=which, n_receptor=120, n_ligand=12, target_panels=3300)
+        orc = po.Oracle(w.verts, w.tris, po.Params(K_far=w.params["K_far"]))
+        ref = orc.solve(po.Sites(**w.sites))
+        ctx = pbm.from_workload(w)
+        ctx.tree_build()
+        _, _, res = ctx.solve()
+        assert res["status"] == 0
+        assert abs(res["dG_solv"] - ref["dG_solv"]) <= 1e-3 * abs(ref["dG_solv"])
+        assert abs(res["G_vac"] - ref["G_vac"]) <= 1e-6 * abs(ref["G_vac"])
+        scale += abs(ref["dG_solv"])
+        sols.append(ref)
+        ress.append(res)
+        ctx.close()
+    got = pbm.binding_cycle(*ress)
+    want = po.binding_cycle(*sols)
+    assert got["converged"]
+    assert abs(got["dG_bind_vac"] - want["dG_bind_vac"]) <= 1e-6 * (abs(sols[0]["G_vac"]) + abs(sols[1]["G_vac"]))
+    assert abs(got["ddG_bind"] - want["ddG_bind"]) <= 1e-3 * scale         # a difference of three large energies
+    assert abs(got["dG_bind_diss"] - (got["ddG_bind"] + got["dG_bind_vac"])) <= 1e-9 * scale
+
+
+def test_c3_complex_solve_treecode_against_direct_mode(pbm, torch_cuda):
+    """BASELINE configs[3] at full size (~58k panels, 3,050 sites): the oracle cannot afford the dense solve, so
+    the treecode solve is compared with the direct-mode (theta = 0) GPU solve, which the sampled-row test above
+    ties to the oracle at 1e-11 (S: section 8(d) gates)."""
+    from paper_1810_03698_b200.workloads import make_config
+    w = make_config("C3", which="complex")
+    ctx = pbm.from_workload(w)
+    ctx.tree_build()
+    x_t, mu_t, res_t = ctx.solve()
+    ctx.set_params(theta=0.0)
+    ctx.tree_build()
+    x_d, mu_d, res_d = ctx.solve()
+    assert res_t["status"] == 0 and res_d["status"] == 0
+    for k in ("dG_solv", "G_solvterm", "G_mult_diss"):
+        assert abs(res_t[k] - res_d[k]) <= 1e-3 * abs(res_d[k]), (k, res_t[k], res_d[k])
+    assert res_t["G_vac"] == res_d["G_vac"]                                   # no surface involved
+    assert rel(mu_t.cpu().numpy(), mu_d.cpu().numpy()) <= 1e-4
+    assert rel(x_t.cpu().numpy(), x_d.cpu().numpy()) <= 1e-3
+    assert abs(res_t["scf_iters"] - res_d["scf_iters"]) <= 1
+    ctx.close()
