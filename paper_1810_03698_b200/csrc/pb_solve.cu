@@ -4,7 +4,9 @@
 // and the convergence tests; every vector operation is a kernel.
 #include <math.h>
 #include <vector>
+#include <cooperative_groups.h>
 #include "pb_internal.cuh"
+namespace cg = cooperative_groups;
 
 #define DOT_CHUNK 512
 #define DOT_THREADS 256
@@ -150,6 +152,109 @@ k_normalize(int64_t n, const double* __restrict__ nrm2, const double* __restrict
         vnext[e] = w[e] * inv;
 }
 
+// ---- short vectors: both Gram-Schmidt passes, the norm and the new basis vector in ONE cooperative launch -----
+// For 2N up to a few ten thousand the four vector kernels above are pure launch latency.  Here block b owns
+// elements [256 b, 256 b + 256) of w (kept in shared memory across the passes) and the whole grid is resident:
+//   A  partial dots V_j . w over the chunk                   -> grid sync
+//   B  h1 = sum of the partials (fixed order); w -= V h1 ; partial dots V_j . w and w . w -> grid sync
+//   C  h2, s = w.w; r2 = s - |h2|^2; w -= V h2; v_next = w / sqrt(r2)
+// Block 0 writes h1, h2, s, r2 straight into pinned host memory (read by the host after the stream sync).
+// Same arithmetic and summation pattern as k_dots<1> / k_arnoldi_update up to the chunk size.
+#define CGS_CHUNK 256
+__global__ void __launch_bounds__(CGS_CHUNK)
+k_cgs2(int64_t n, int nv, const double* __restrict__ V, int64_t ld, double* __restrict__ w, double* __restrict__ vnext,
+       double* __restrict__ partial /*[2][grid][nv+1]*/, double* __restrict__ hpin, int hstride)
+{
+    cg::grid_group grid = cg::this_grid();
+    extern __shared__ double cgs_sm[];
+    double* sw = cgs_sm;                      // [CGS_CHUNK] this block's chunk of w
+    double* hs = cgs_sm + CGS_CHUNK;          // [nv + 2]
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int nb = gridDim.x, nvt = nv + 1;
+    const int64_t e0 = (int64_t)blockIdx.x * CGS_CHUNK;
+    const int cnt = (int)(n - e0 < CGS_CHUNK ? n - e0 : CGS_CHUNK);
+    sw[tid] = tid < cnt ? w[e0 + tid] : 0.0;
+    __syncthreads();
+    double* part0 = partial;
+    double* part1 = partial + (size_t)nb * nvt;
+    auto dots = [&](double* part, bool self) {
+        for (int j = wid; j < nv + (self ? 1 : 0); j += CGS_CHUNK / 32) {
+            double s = 0;
+            if (j < nv) {
+                const double* v = V + (int64_t)j * ld + e0;
+#pragma unroll
+                for (int i = 0; i < CGS_CHUNK / 32; ++i) {
+                    const int k = lane + 32 * i;
+                    s = fma(k < cnt ? v[k] : 0.0, sw[k], s);
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < CGS_CHUNK / 32; ++i) s = fma(sw[lane + 32 * i], sw[lane + 32 * i], s);
+            }
+            for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+            if (lane == 0) part[(size_t)blockIdx.x * nvt + j] = s;
+        }
+    };
+    auto gather = [&](const double* part, int count) {   // hs[j] = sum over blocks, fixed order
+        __syncthreads();
+        for (int j = tid; j < count; j += CGS_CHUNK) {
+            double s = 0;
+            for (int b = 0; b < nb; ++b) s += __ldcg(&part[(size_t)b * nvt + j]);
+            hs[j] = s;
+        }
+        __syncthreads();
+    };
+    auto update = [&]() -> double {
+        double acc = sw[tid];
+        if (tid < cnt) {
+            const double* v = V + e0 + tid;
+            int j = 0;
+            for (; j + 4 <= nv; j += 4) {
+                const double v0 = v[(int64_t)j * ld], v1 = v[(int64_t)(j + 1) * ld], v2 = v[(int64_t)(j + 2) * ld],
+                             v3 = v[(int64_t)(j + 3) * ld];
+                acc = fma(-hs[j], v0, acc);
+                acc = fma(-hs[j + 1], v1, acc);
+                acc = fma(-hs[j + 2], v2, acc);
+                acc = fma(-hs[j + 3], v3, acc);
+            }
+            for (; j < nv; ++j) acc = fma(-hs[j], v[(int64_t)j * ld], acc);
+        }
+        return acc;
+    };
+    dots(part0, false);
+    __threadfence();
+    grid.sync();
+    gather(part0, nv);
+    if (blockIdx.x == 0)
+        for (int j = tid; j < nv; j += CGS_CHUNK) hpin[j] = hs[j];
+    {
+        const double acc = update();
+        __syncthreads();
+        sw[tid] = acc;
+        __syncthreads();
+    }
+    dots(part1, true);
+    __threadfence();
+    grid.sync();
+    gather(part1, nvt);
+    __shared__ double inv;
+    if (tid == 0) {
+        double h2 = 0;
+        for (int j = 0; j < nv; ++j) h2 = fma(hs[j], hs[j], h2);
+        const double r2 = hs[nv] - h2;
+        inv = r2 > 0 ? 1.0 / sqrt(r2) : 0.0;
+        if (blockIdx.x == 0) hpin[hstride + nv + 1] = r2;
+    }
+    if (blockIdx.x == 0)
+        for (int j = tid; j < nvt; j += CGS_CHUNK) hpin[hstride + j] = hs[j];
+    __syncthreads();
+    const double acc = update();
+    if (tid < cnt) {
+        w[e0 + tid] = acc;
+        vnext[e0 + tid] = acc * inv;
+    }
+}
+
 // z = Minv v: per panel the inverse 2x2 diagonal block (SELF entries), original panel order
 __global__ void k_precond(int64_t N, const double* __restrict__ pc, const double* __restrict__ v, double* __restrict__ z)
 {
@@ -282,6 +387,15 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
     std::vector<double> H((size_t)(m + 1) * m, 0.0), cs(m, 0.0), sn(m, 0.0), g(m + 1, 0.0), yv(m, 0.0);
     const int tb = 256;
     const int nb = pb_blocks(n, tb) < 2368 ? pb_blocks(n, tb) : 2368;   // grid-stride above 16 blocks per SM
+    // short vectors: the whole orthogonalisation in one cooperative launch (one block per 256 elements, all resident)
+    int coop_blocks = 0;
+    {
+        int nsm = 0, coop = 0;
+        cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, ctx->device);
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, ctx->device);
+        const int64_t need = (n + CGS_CHUNK - 1) / CGS_CHUNK;
+        if (coop && need <= nsm && (size_t)2 * need * (m + 1) <= (size_t)DOT_MAXBLK * (m + 2)) coop_blocks = (int)need;
+    }
     for (;;) {
         // true residual r = b - A x
         PB_TRY(pb_matvec_impl(ctx, x, ws.w, false, false));
@@ -310,14 +424,26 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
             // classical Gram-Schmidt, twice
             double* hA = ws.hdev;
             double* hB = ws.hdev + hstride;
-            PB_TRY(dot_into(ctx, ws, nv, ws.V, ws.w, false, hA));
-            k_arnoldi_update<<<nb, tb, nv * sizeof(double), st>>>(n, nv, ws.V, n, hA, ws.w, nullptr, nullptr);
-            PB_LAUNCH_CHECK();
-            PB_TRY(dot_into(ctx, ws, nv, ws.V, ws.w, true, hB));     // hB[nv] = w.w
-            k_arnoldi_update<<<nb, tb, nv * sizeof(double), st>>>(n, nv, ws.V, n, hB, ws.w, vnext, hB + nv + 1);
-            PB_LAUNCH_CHECK();
-            PB_CUDA(cudaMemcpyAsync(hh, ws.hdev, sizeof(double) * 2 * hstride, cudaMemcpyDeviceToHost, st));
-            PB_CUDA(cudaStreamSynchronize(st));
+            if (coop_blocks > 0) {
+                int64_t n_ = n, ld_ = n;
+                int nv_ = nv, hs_ = hstride;
+                const double* V_ = ws.V;
+                double *w_ = ws.w, *vn_ = vnext, *pa_ = ws.partial, *hp_ = hh;
+                void* args[] = {&n_, &nv_, &V_, &ld_, &w_, &vn_, &pa_, &hp_, &hs_};
+                PB_CUDA(cudaLaunchCooperativeKernel((void*)k_cgs2, dim3(coop_blocks), dim3(CGS_CHUNK), args,
+                                                    (size_t)(CGS_CHUNK + m + 4) * sizeof(double), st));
+                PB_LAUNCH_CHECK();
+                PB_CUDA(cudaStreamSynchronize(st));
+            } else {
+                PB_TRY(dot_into(ctx, ws, nv, ws.V, ws.w, false, hA));
+                k_arnoldi_update<<<nb, tb, nv * sizeof(double), st>>>(n, nv, ws.V, n, hA, ws.w, nullptr, nullptr);
+                PB_LAUNCH_CHECK();
+                PB_TRY(dot_into(ctx, ws, nv, ws.V, ws.w, true, hB));     // hB[nv] = w.w
+                k_arnoldi_update<<<nb, tb, nv * sizeof(double), st>>>(n, nv, ws.V, n, hB, ws.w, vnext, hB + nv + 1);
+                PB_LAUNCH_CHECK();
+                PB_CUDA(cudaMemcpyAsync(hh, ws.hdev, sizeof(double) * 2 * hstride, cudaMemcpyDeviceToHost, st));
+                PB_CUDA(cudaStreamSynchronize(st));
+            }
             double hn2 = hh[hstride + nv + 1];
             if (!(hn2 > 1e-2 * hh[hstride + nv])) {
                 // the second pass removed most of w (cancellation in w.w - |h|^2): take the norm directly
