@@ -68,7 +68,9 @@ typedef struct pb_params {
     double scf_tol_debye;   /* RMS change of induced dipoles, Debye (D: R-19)          */
     double scf_omega;       /* SOR factor, 0.7                                        */
     int32_t scf_maxit;
-    int32_t reserved;
+    int32_t site_treecode;  /* reaction field at the sites (Eq. 12, 13, 21): 0 = direct sum over all source
+                               points (the paper's choice), 1 = treecode over the panel tree when
+                               theta > 0 and order_P <= 8, 2 (default) = treecode when N_a * N_s >= 2^31   */
     double thole_a;         /* Thole damping constant, 0.39 (D: R-17)                  */
 } pb_params;
 

@@ -97,6 +97,7 @@ extern "C" void pb_default_params(pb_params* p)
     p->scf_tol_debye = 1e-7;
     p->scf_omega = 0.7;
     p->scf_maxit = 200;
+    p->site_treecode = 2;
     p->thole_a = 0.39;
 }
 
@@ -178,6 +179,7 @@ extern "C" int pb_set_params(pb_ctx* ctx, const pb_params* p)
     if (p->gmres_restart < 1 || p->gmres_maxit < 1 || p->scf_maxit < 1 || !(p->gmres_tol > 0) ||
         !(p->scf_tol_debye > 0) || !(p->scf_omega > 0))
         return pb_fail(ctx, PB_ERR_INVALID_ARG, "solver limits/tolerances must be positive");
+    if (p->site_treecode < 0 || p->site_treecode > 2) return pb_fail(ctx, PB_ERR_INVALID_ARG, "site_treecode must be 0, 1 or 2");
     const pb_params& o = ctx->prm;
     bool shape = o.kappa != p->kappa || o.theta != p->theta || o.order_P != p->order_P ||
                  o.ncrit != p->ncrit || o.K_far != p->K_far || o.K_near != p->K_near ||
@@ -191,6 +193,7 @@ extern "C" int pb_set_params(pb_ctx* ctx, const pb_params* p)
         ctx->gws = pb_gmres_ws();
         ctx->tree = pb_tree();
         ctx->sites.near_built = false;
+        ctx->sites.tree_built = false;
     }
     return PB_OK;
 }
@@ -230,6 +233,7 @@ extern "C" int pb_mesh_load(pb_ctx* ctx, const double* verts, int64_t nv, const 
     pb_dfree_cat(ctx, CAT_MESH);
     ctx->tree = pb_tree();
     ctx->sites.near_built = false;
+        ctx->sites.tree_built = false;
     ctx->mesh_loaded = false;
     ctx->nv = nv;
     ctx->nt = nt;
@@ -294,6 +298,7 @@ extern "C" int pb_tree_build(pb_ctx* ctx)
     ctx->gws = pb_gmres_ws();
     ctx->tree = pb_tree();
     ctx->sites.near_built = false;
+        ctx->sites.tree_built = false;
     PB_TRY(pb_upload_rules(ctx));
     PB_TRY(pb_tree_build_impl(ctx));
     PB_TRY(pb_farfield_setup(ctx));

@@ -13,9 +13,18 @@
 
 #define PB_INV4PI 0.079577471545947667884
 #define PB_MAX_P 10
+#define PB_SITE_THETA_SCALE 0.7   // site lists: theta_site = 0.7 theta (pb_tree.cu, pb_site_lists_build)
 #define PB_TG 64            // targets (panels) per target group = threads per M2P/P2P block
 #define PB_KCAL 332.0636    // e^2/Angstrom -> kcal/mol (D: R-1)
 #define PB_DEBYE 4.80320    // 1 e*Angstrom in Debye (D: R-1)
+
+// Cartesian multi-index (a,b,c) -> position in a moment / coefficient array, graded by n = a+b+c
+__host__ __device__ static inline int mom_index(int a, int b, int c)
+{
+    int n = a + b + c, m = b + c;
+    return n * (n + 1) * (n + 2) / 6 + m * (m + 1) / 2 + c;
+}
+__host__ __device__ static constexpr int pb_nk(int P) { return (P + 1) * (P + 2) * (P + 3) / 6; }
 
 enum pb_mem_cat { CAT_MESH = 0, CAT_SITES = 1, CAT_TREE = 2, CAT_SOLVE = 3, CAT_SITE_NEAR = 4, CAT_TMP = 5, CAT_COUNT = 6 };
 
@@ -121,6 +130,20 @@ struct pb_sites {
     int64_t n_near = 0;
     int32_t* near_site = nullptr;
     int32_t* near_panel = nullptr; // Morton index
+    // treecode for the reaction field (S: section 8(f) item 1): sites in Morton order, groups of 32, their lists,
+    // and the cells whose moments those lists need (a second configuration of the upward pass)
+    bool tree_built = false;
+    int32_t* tperm = nullptr;      // [na] Morton position -> original site index
+    double* tpos[3] = {0, 0, 0};   // [na] sorted positions (SoA)
+    int64_t t_groups = 0, t_m2p_total = 0, t_p2p_pairs = 0, t_m2p_pairs = 0;
+    int32_t *t_m2p_off = nullptr, *t_m2p_cell = nullptr, *t_p2p_off = nullptr, *t_p2p_lo = nullptr, *t_p2p_hi = nullptr;
+    int32_t* t_need_leaf = nullptr;
+    int32_t* t_up_link = nullptr;
+    int64_t t_n_need_leaf = 0;
+    int32_t* nb_idx = nullptr;     // [Nk(P+2)][6] indices of k - e_d, k - 2 e_d (or -1) for the coefficient recurrence
+    int32_t* dv_idx = nullptr;     // [10][Nk(P)] index of kappa + l
+    double* dv_fac = nullptr;      // [10][Nk(P)] (-1)^|kappa| (kappa + l)! / l!
+    int t_P = -1;
 };
 
 // GMRES workspace, kept between solves while the system size and restart length are unchanged
@@ -217,12 +240,19 @@ static inline int pb_blocks(int64_t n, int threads) { return (int)((n + threads 
 int pb_exclusive_scan_i32(pb_ctx* ctx, const int32_t* in, int32_t* out, int64_t n, int64_t* total_host);
 // pb_tree.cu
 int pb_tree_build_impl(pb_ctx* ctx);
+int pb_morton_order(pb_ctx* ctx, const double* pts, int64_t n, int cat, int32_t** perm_out, uint64_t** keys_out);
+int pb_site_lists_build(pb_ctx* ctx);
+// pb_sitetree.cu
+int pb_site_tree_build(pb_ctx* ctx);
+int pb_reaction_field_tree(pb_ctx* ctx, double* phi, double* grad, double* hess);
 // pb_near.cu
 int pb_near_build(pb_ctx* ctx);
 int pb_make_rule(int K, pb_rule_t* r);
 int pb_upload_rules(pb_ctx* ctx);   // fills ctx->ruleF, ruleN, gl from the parameters
 // pb_matvec.cu
 int pb_farfield_setup(pb_ctx* ctx);
+int pb_site_farfield_setup(pb_ctx* ctx);
+int pb_upward(pb_ctx* ctx, cudaStream_t fs, const int32_t* leaf_ids, int64_t n_leaf, const int32_t* up_link);
 int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed, bool precond);
 int pb_weights(pb_ctx* ctx, const double* x, bool precond);
 void pb_make_expk(double kappa, pb_expk* out);

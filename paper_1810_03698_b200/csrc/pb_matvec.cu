@@ -16,13 +16,6 @@
 #include "pb_internal.cuh"
 
 // ---- index tables ------------------------------------------------------------------------------
-__host__ __device__ static inline int mom_index(int a, int b, int c)
-{
-    int n = a + b + c, m = b + c;
-    return n * (n + 1) * (n + 2) / 6 + m * (m + 1) / 2 + c;
-}
-
-__host__ __device__ static constexpr int pb_nk(int P) { return (P + 1) * (P + 2) * (P + 3) / 6; }
 __host__ __device__ static constexpr int pb_nt(int P)
 {
     int t = 0;
@@ -150,9 +143,13 @@ int pb_farfield_setup(pb_ctx* ctx)
             for (int q = 0; q < nchild[c]; ++q) { need[child[c] + q] = 1; parent[child[c] + q] = (int32_t)c; }
         }
     }
-    // up[c]: bit 0 = the cell's F terms are wanted (it is in an M2P list); bits 1.. = 1 + parent when the
-    // parent's moments are needed (the block finishing c then reports to it), else 0
-    for (int64_t c = 0; c < nc; ++c) up[c] = (used[c] ? 1 : 0) | ((need[c] && parent[c] >= 0 ? parent[c] + 1 : 0) << 1);
+    // up[c]: bit 0 = the cell's F terms are wanted (it is in an M2P list); bit 1 = its moments are stored in
+    // M (a parent will read them); bits 2.. = 1 + parent when the parent's moments are needed (the block
+    // finishing c then reports to it), else 0
+    for (int64_t c = 0; c < nc; ++c) {
+        const int32_t par = need[c] && parent[c] >= 0 ? parent[c] + 1 : 0;
+        up[c] = (used[c] ? 1 : 0) | (par ? 2 : 0) | (par << 2);
+    }
     t.n_used = n_used;
     t.n_need_leaf = (int64_t)leaf_list.size();
     t.n_need_internal = n_internal;
@@ -340,8 +337,8 @@ __global__ void __launch_bounds__(UP_THREADS) k_upward(up_args a)
     for (;;) {
         // mom holds the finished moments of cell c
         const int32_t link = a.up_link[c];
-        const int64_t parent = (int64_t)(link >> 1) - 1;
-        if (parent >= 0)
+        const int64_t parent = (int64_t)(link >> 2) - 1;
+        if (link & 2)
             for (int k = tid; k < 2 * Nk; k += UP_THREADS) a.M[c * 2 * Nk + k] = mom[k];
         if (link & 1) {                                        // M -> F (cells in an M2P list)
             const double* mv = mom;
@@ -990,31 +987,74 @@ static cudaError_t launch_m2p(pb_ctx* ctx, cudaStream_t fs)
     return cudaSuccess;
 }
 
+// The upward pass for one set of needed cells: `leaf_ids` (one block each) and the per-cell `up_link` words.
+// The panel matvec and the site-side treecode (pb_sitetree.cu) each have their own set; both write t.M.
+int pb_upward(pb_ctx* ctx, cudaStream_t fs, const int32_t* leaf_ids, int64_t n_leaf, const int32_t* up_link)
+{
+    pb_tree& t = ctx->tree;
+    if (n_leaf <= 0) return PB_OK;
+    up_args ua;
+    ua.P = t.P; ua.Nk = t.Nk; ua.NT = t.NT; ua.K = t.K;
+    ua.leaf_ids = leaf_ids; ua.c_first = t.c_first; ua.c_last = t.c_last; ua.c_child = t.c_child;
+    ua.c_nchild = t.c_nchild; ua.up_link = up_link; ua.up_count = t.up_count;
+    ua.cx = t.c_ctr[0]; ua.cy = t.c_ctr[1]; ua.cz = t.c_ctr[2];
+    ua.srec = t.srec;
+    ua.mm_off = t.mm_off; ua.mm_ent = t.mm_ent; ua.mm_coef = t.mm_coef;
+    ua.cv_off = t.cv_off; ua.cv_idx = t.cv_idx; ua.cv_coef = t.cv_coef;
+    ua.M = t.M; ua.FF = t.FF;
+    const size_t sm = up_smem_bytes(t.Nk);
+    static size_t sm_set = 0;                       // the attribute belongs to the function, not the context
+    if (sm > 48 * 1024 && sm > sm_set) {
+        PB_CUDA(cudaFuncSetAttribute(k_upward, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+        sm_set = sm;
+    }
+    k_upward<<<(unsigned)n_leaf, UP_THREADS, sm, fs>>>(ua);
+    PB_LAUNCH_CHECK();
+    return PB_OK;
+}
+
+// Which cells the SITE lists need (S: section 8(f) item 1): same bookkeeping as in pb_farfield_setup, but every
+// needed cell stores its moments (the site kernel reads M, not the F terms).
+int pb_site_farfield_setup(pb_ctx* ctx)
+{
+    pb_tree& t = ctx->tree;
+    pb_sites& s = ctx->sites;
+    cudaStream_t st = ctx->stream;
+    const int64_t nc = t.n_cells;
+    std::vector<int32_t> child(nc), nchild(nc), lists(s.t_m2p_total > 0 ? s.t_m2p_total : 1);
+    PB_CUDA(cudaMemcpyAsync(child.data(), t.c_child, sizeof(int32_t) * nc, cudaMemcpyDeviceToHost, st));
+    PB_CUDA(cudaMemcpyAsync(nchild.data(), t.c_nchild, sizeof(int32_t) * nc, cudaMemcpyDeviceToHost, st));
+    if (s.t_m2p_total > 0)
+        PB_CUDA(cudaMemcpyAsync(lists.data(), s.t_m2p_cell, sizeof(int32_t) * s.t_m2p_total, cudaMemcpyDeviceToHost, st));
+    PB_CUDA(cudaStreamSynchronize(st));
+    std::vector<char> need(nc, 0);
+    for (int64_t e = 0; e < s.t_m2p_total; ++e) need[lists[e]] = 1;
+    std::vector<int32_t> leaf_list, parent(nc, -1), up(nc, 0);
+    for (int64_t c = 0; c < nc; ++c) {               // parents come before their children
+        if (!need[c]) continue;
+        if (child[c] < 0) leaf_list.push_back((int32_t)c);
+        else
+            for (int q = 0; q < nchild[c]; ++q) { need[child[c] + q] = 1; parent[child[c] + q] = (int32_t)c; }
+    }
+    for (int64_t c = 0; c < nc; ++c)
+        if (need[c]) up[c] = 2 | ((parent[c] >= 0 ? parent[c] + 1 : 0) << 2);
+    s.t_n_need_leaf = (int64_t)leaf_list.size();
+    PB_TRY(pb_dalloc_t(ctx, &s.t_need_leaf, leaf_list.size() > 0 ? leaf_list.size() : 1, CAT_SITE_NEAR));
+    PB_TRY(pb_dalloc_t(ctx, &s.t_up_link, (size_t)nc, CAT_SITE_NEAR));
+    if (!leaf_list.empty())
+        PB_CUDA(cudaMemcpyAsync(s.t_need_leaf, leaf_list.data(), sizeof(int32_t) * leaf_list.size(), cudaMemcpyHostToDevice, st));
+    PB_CUDA(cudaMemcpyAsync(s.t_up_link, up.data(), sizeof(int32_t) * nc, cudaMemcpyHostToDevice, st));
+    PB_CUDA(cudaStreamSynchronize(st));
+    return PB_OK;
+}
+
 // Far-field branch: the upward pass (P2M, M2M, M -> F) in one launch, then M2P.  `fs` is the stream it
 // is enqueued on: the context's side stream (concurrent with P2P) or, when per-kernel event timing
 // is wanted, the main stream.
 static int pb_far_branch(pb_ctx* ctx, cudaStream_t fs, bool timed)
 {
     pb_tree& t = ctx->tree;
-    if (t.n_need_leaf > 0) {
-        up_args ua;
-        ua.P = t.P; ua.Nk = t.Nk; ua.NT = t.NT; ua.K = t.K;
-        ua.leaf_ids = t.need_leaf; ua.c_first = t.c_first; ua.c_last = t.c_last; ua.c_child = t.c_child;
-        ua.c_nchild = t.c_nchild; ua.up_link = t.up_link; ua.up_count = t.up_count;
-        ua.cx = t.c_ctr[0]; ua.cy = t.c_ctr[1]; ua.cz = t.c_ctr[2];
-        ua.srec = t.srec;
-        ua.mm_off = t.mm_off; ua.mm_ent = t.mm_ent; ua.mm_coef = t.mm_coef;
-        ua.cv_off = t.cv_off; ua.cv_idx = t.cv_idx; ua.cv_coef = t.cv_coef;
-        ua.M = t.M; ua.FF = t.FF;
-        const size_t sm = up_smem_bytes(t.Nk);
-        static size_t sm_set = 0;                       // the attribute belongs to the function, not the context
-        if (sm > 48 * 1024 && sm > sm_set) {
-            PB_CUDA(cudaFuncSetAttribute(k_upward, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-            sm_set = sm;
-        }
-        k_upward<<<(unsigned)t.n_need_leaf, UP_THREADS, sm, fs>>>(ua);
-        PB_LAUNCH_CHECK();
-    }
+    PB_TRY(pb_upward(ctx, fs, t.need_leaf, t.n_need_leaf, t.up_link));
     if (timed) PB_CUDA(cudaEventRecord(ctx->ev[2], fs));
     if (t.n_itemM > 0) {
         PB_TRY(pb_prof_begin(ctx, 1));

@@ -202,6 +202,7 @@ int pb_site_near_build(pb_ctx* ctx)
     cudaStream_t st = ctx->stream;
     pb_dfree_cat(ctx, CAT_SITE_NEAR);
     s.near_built = false;
+    s.tree_built = false;
     int32_t *cnt, *off;
     PB_TRY(pb_dalloc_t(ctx, &cnt, t.N + 1, CAT_SITE_NEAR));
     PB_TRY(pb_dalloc_t(ctx, &off, t.N + 1, CAT_SITE_NEAR));
@@ -275,27 +276,36 @@ extern "C" int pb_reaction_field(pb_ctx* ctx, const double* x, double* phi, doub
     cudaStream_t st = ctx->stream;
     if (!s.near_built) PB_TRY(pb_site_near_build(ctx));
     PB_TRY(pb_weights(ctx, x, false));
-    const int64_t ntile = (s.na + RF_ST - 1) / RF_ST;
-    // enough source chunks to fill the GPU, each at least 4 sweeps of the block
-    int64_t nchunk = (148 * 16 + ntile - 1) / ntile;
-    int64_t maxchunk = (t.Ns + 4 * RF_THREADS - 1) / (4 * RF_THREADS);
-    if (nchunk > maxchunk) nchunk = maxchunk;
-    if (nchunk < 1) nchunk = 1;
-    if (nchunk > 1024) nchunk = 1024;
-    int64_t chunk = (t.Ns + nchunk - 1) / nchunk;
-    nchunk = (t.Ns + chunk - 1) / chunk;
-    PB_TRY(pb_scratch(ctx, (size_t)nchunk * s.na * 10 * sizeof(double) + 4096));
-    double* partial = ctx->scratch;
-    dim3 grid((unsigned)nchunk, (unsigned)ntile);
-    const bool H = hess != nullptr;
-    if (H)
-        k_reaction<true><<<grid, RF_THREADS, 0, st>>>(t.Ns, chunk, s.na, s.pos, t.srec, partial);
-    else
-        k_reaction<false><<<grid, RF_THREADS, 0, st>>>(t.Ns, chunk, s.na, s.pos, t.srec, partial);
-    PB_LAUNCH_CHECK();
-    const int NO = H ? 10 : 4;
-    k_reaction_finish<<<pb_blocks(s.na * NO, 128), 128, 0, st>>>(s.na, (int)nchunk, NO, partial, phi, grad, hess);
-    PB_LAUNCH_CHECK();
+    // direct sum over every source point (the paper's choice) or the treecode over the panel tree
+    const int mode = ctx->prm.site_treecode;
+    const bool tree = ctx->prm.theta > 0.0 && ctx->prm.order_P <= 8 &&
+                      (mode == 1 || (mode == 2 && (double)s.na * (double)t.Ns >= 2147483648.0));
+    if (tree) {
+        if (!s.tree_built) PB_TRY(pb_site_tree_build(ctx));
+        PB_TRY(pb_reaction_field_tree(ctx, phi, grad, hess));
+    } else {
+        const int64_t ntile = (s.na + RF_ST - 1) / RF_ST;
+        // enough source chunks to fill the GPU, each at least 4 sweeps of the block
+        int64_t nchunk = (148 * 16 + ntile - 1) / ntile;
+        int64_t maxchunk = (t.Ns + 4 * RF_THREADS - 1) / (4 * RF_THREADS);
+        if (nchunk > maxchunk) nchunk = maxchunk;
+        if (nchunk < 1) nchunk = 1;
+        if (nchunk > 1024) nchunk = 1024;
+        int64_t chunk = (t.Ns + nchunk - 1) / nchunk;
+        nchunk = (t.Ns + chunk - 1) / chunk;
+        PB_TRY(pb_scratch(ctx, (size_t)nchunk * s.na * 10 * sizeof(double) + 4096));
+        double* partial = ctx->scratch;
+        dim3 grid((unsigned)nchunk, (unsigned)ntile);
+        const bool H = hess != nullptr;
+        if (H)
+            k_reaction<true><<<grid, RF_THREADS, 0, st>>>(t.Ns, chunk, s.na, s.pos, t.srec, partial);
+        else
+            k_reaction<false><<<grid, RF_THREADS, 0, st>>>(t.Ns, chunk, s.na, s.pos, t.srec, partial);
+        PB_LAUNCH_CHECK();
+        const int NO = H ? 10 : 4;
+        k_reaction_finish<<<pb_blocks(s.na * NO, 128), 128, 0, st>>>(s.na, (int)nchunk, NO, partial, phi, grad, hess);
+        PB_LAUNCH_CHECK();
+    }
     if (s.n_near > 0) {
         rf_corr_args a;
         a.np = s.n_near; a.K = t.K; a.psite = s.near_site; a.ppanel = s.near_panel; a.pos = s.pos;

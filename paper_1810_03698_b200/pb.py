@@ -15,7 +15,7 @@ from dataclasses import dataclass
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 LIB_PATH = os.path.join(_HERE, "libpb_b200.so")
-SOURCES = ["pb_api.cu", "pb_tree.cu", "pb_near.cu", "pb_matvec.cu", "pb_sites.cu", "pb_solve.cu"]
+SOURCES = ["pb_api.cu", "pb_tree.cu", "pb_near.cu", "pb_matvec.cu", "pb_sites.cu", "pb_sitetree.cu", "pb_solve.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 
@@ -44,7 +44,7 @@ class Params(ctypes.Structure):
         ("K_far", ctypes.c_int32), ("K_near", ctypes.c_int32), ("near_tau", ctypes.c_double),
         ("nq_edge", ctypes.c_int32), ("precond", ctypes.c_int32), ("gmres_tol", ctypes.c_double),
         ("gmres_restart", ctypes.c_int32), ("gmres_maxit", ctypes.c_int32), ("scf_tol_debye", ctypes.c_double),
-        ("scf_omega", ctypes.c_double), ("scf_maxit", ctypes.c_int32), ("reserved", ctypes.c_int32),
+        ("scf_omega", ctypes.c_double), ("scf_maxit", ctypes.c_int32), ("site_treecode", ctypes.c_int32),
         ("thole_a", ctypes.c_double),
     ]
 

@@ -167,3 +167,52 @@ def test_c3_complex_solve_treecode_against_direct_mode(pbm, torch_cuda):
     assert rel(x_t.cpu().numpy(), x_d.cpu().numpy()) <= 1e-3
     assert abs(res_t["scf_iters"] - res_d["scf_iters"]) <= 1
     ctx.close()
+
+
+def test_site_treecode_reaction_field_c2(pbm, po, torch_cuda):
+    """S: section 8(f) item 1 -- the reaction field at the sites by the treecode over the panel tree
+    (site_treecode = 1) against the oracle's direct quadrature: on the converged physical solution the
+    potential, field and field gradient, and end to end the energies and induced dipoles of the solve."""
+    from paper_1810_03698_b200.workloads import make_config
+    w = make_config("C2")
+    orc = po.Oracle(w.verts, w.tris, po.Params(K_far=w.params["K_far"]))
+    s = po.Sites(**w.sites)
+    ref = orc.solve(s)
+    ctx = pbm.from_workload(w, site_treecode=1)
+    ctx.tree_build()
+    phi, grad, hess = [t.cpu().numpy() for t in ctx.reaction_field(torch_cuda.from_numpy(ref["x"]))]
+    assert rel(phi, ref["phi_solv"]) <= 1e-4
+    assert rel(grad, ref["grad_solv"]) <= 1e-3          # each target derivative costs about one order of the expansion
+    assert rel(hess, ref["hess_solv"]) <= 1e-2
+    g_only = ctx.reaction_field(torch_cuda.from_numpy(ref["x"]), want_hess=False)[1].cpu().numpy()
+    assert rel(g_only, grad) <= 1e-13                    # the SCF loop's gradient-only path is the same sum
+    x, mu, res = ctx.solve()
+    assert res["status"] == 0
+    for k in ("dG_solv", "G_solvterm", "G_mult_diss", "G_vac"):
+        assert abs(res[k] - ref[k]) <= 1e-3 * abs(ref[k]), (k, res[k], ref[k])
+    assert rel(mu.cpu().numpy(), ref["mu"]) <= 1e-4
+    assert abs(res["scf_iters"] - ref["scf_iters"]) <= 1
+    ctx.close()
+
+
+def test_site_treecode_matches_direct_sum_at_c4(pbm, torch_cuda):
+    """At BASELINE configs[4]'s size (20,000 sites x 7.26 M Gauss points, where site_treecode = 2 switches the
+    treecode on by itself) against the direct sum on the GPU, which test_site_side_operators_c2 ties to the oracle."""
+    from paper_1810_03698_b200.workloads import make_config
+    import torch
+    w = make_config("C4")
+    nt = w.tris.shape[0]
+    ctx = pbm.from_workload(w)
+    assert ctx.get_params().site_treecode == 2
+    ctx.tree_build()
+    # a smooth surface density (the potential of two interior charges and its normal derivative sign-flipped),
+    # like a physical solution; white noise on a 1 M-panel mesh would be dominated by the nearest panels
+    c = torch.from_numpy(w.verts[w.tris].mean(axis=1)).cuda()
+    x = torch.cat([1.0 / (c - torch.tensor([3.0, 1.0, -2.0], device="cuda", dtype=c.dtype)).norm(dim=1),
+                   -0.1 / (c + torch.tensor([5.0, -4.0, 6.0], device="cuda", dtype=c.dtype)).norm(dim=1) ** 2])
+    tree = [t.clone() for t in ctx.reaction_field(x)]
+    ctx.set_params(site_treecode=0)
+    direct = ctx.reaction_field(x)
+    errs = [float((a - b).norm() / b.norm()) for a, b in zip(tree, direct)]
+    assert errs[0] <= 1e-4 and errs[1] <= 1e-3 and errs[2] <= 2e-2, errs     # (this density's field gradient nearly cancels)
+    ctx.close()
