@@ -295,8 +295,11 @@ def run_ours(args):
     m2p_tf = (m2p_flop_per_pair(P, st1["n_terms"]) * st1["m2p_pairs"] / (m2p_ms * 1e-3) / 1e12) if m2p_ms > 0 else 0.0
     dominant = "k_p2p" if stp["prof_p2p_ms"] >= stp["prof_m2p_ms"] else "k_m2p"
     ach = p2p_tf if dominant == "k_p2p" else m2p_tf
+    # DRAM bytes per launch of the dominant kernel from the committed ncu --set full captures (per workload)
+    traffic = {("C1", "k_p2p"): (2.517e6, "profiles/r01c_ncu_full_C1.md"),
+               ("C4", "k_m2p"): (7.68e8, "profiles/r01b_ncu_full_C4.md")}.get((w.name, dominant), (None, None))
     roofline = {"bound": "alu", "kernel": dominant, "achieved": ach, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "frac": ach / FP64_PEAK_TFLOPS, "traffic": None,
+                "frac": ach / FP64_PEAK_TFLOPS, "traffic": traffic[0], "traffic_source": traffic[1],
                 "peak_source": "148 SM x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md section 7); "
                                "pb_fp64_peak_probe measured %.1f TFLOP/s on this GPU" % ctx.fp64_peak_probe(),
                 "timed_in": "a repeat of the timed steps with per-kernel CUDA events (branches serialised on one "

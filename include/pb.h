@@ -165,8 +165,9 @@ int pb_matvec_host(pb_ctx* ctx, const double* x_host, double* y_host);
 /* Reaction potential of the surface layers at the sites, Eq. (12)
  * phi_solv = -K_L(phi) + V_L(dphi), its gradient (Eq. 13) and Hessian (Eq. 21,
  * P:195; 6-vector xx,xy,xz,yy,yz,zz).  phi [na], grad [na][3], hess [na][6]; NULL outputs
- * are skipped.  Direct sum over all source points; K_near rule for panels with
- * |r_m - c_j| < tau*sqrt(A_j) (D: R-9). */
+ * are skipped.  Far rule over all source points -- summed directly or, per pb_params.site_treecode, by
+ * the treecode over the panel tree (the same order-P Taylor sum and MAC as the matvec, with
+ * theta_site = 0.7 theta) -- and the K_near rule for panels with |r_m - c_j| < tau*sqrt(A_j) (D: R-9). */
 int pb_reaction_field(pb_ctx* ctx, const double* x, double* phi, double* grad, double* hess);
 
 /* Coulomb potential, gradient, Hessian at each site of the multipoles on all OTHER sites,

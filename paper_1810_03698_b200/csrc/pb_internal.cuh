@@ -100,9 +100,11 @@ struct pb_tree {
     double* cv_coef = nullptr;
     // near / singular correction table (CSR per target, Morton order)
     int64_t near_entries = 0;
-    int32_t* nr_off = nullptr;    // [N+1]
-    int32_t* nr_col = nullptr;    // [entries] source panel (Morton)
-    double* nr_val = nullptr;     // [4][entries] VL, KL, VY, KY corrections
+    // ... stored as sliced ELL: slice = 32 consecutive targets, entry k of lane l at el_base[slice] + 32 k + l
+    int64_t el_entries = 0;       // padded entries
+    int32_t* el_base = nullptr;   // [slices + 1]
+    int32_t* el_col = nullptr;    // [el_entries] source panel (Morton); padding: the target itself
+    double* el_val = nullptr;     // [4][el_entries] VL, KL, VY, KY corrections; padding: 0
     double* precond = nullptr;    // [N][4] inverse 2x2 diagonal blocks
     // partial accumulators
     // work items (one thread block each) and their accumulator slots

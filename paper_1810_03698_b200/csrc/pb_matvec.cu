@@ -916,8 +916,8 @@ __device__ __forceinline__ double sum_slots(const double* __restrict__ acc, int 
 
 __global__ void __launch_bounds__(128)
 k_combine(int64_t N, const int32_t* __restrict__ itemP_off, const int32_t* __restrict__ itemM_off, double eps_ratio,
-          const double* __restrict__ accP, const double* __restrict__ accM, const int32_t* __restrict__ nr_off,
-          const int32_t* __restrict__ nr_col, const double* __restrict__ nr_val, int64_t ne,
+          const double* __restrict__ accP, const double* __restrict__ accM, const int32_t* __restrict__ el_base,
+          const int32_t* __restrict__ el_col, const double* __restrict__ el_val, int64_t ne,
           const double* __restrict__ xphi, const double* __restrict__ xdphi, const int32_t* __restrict__ perm,
           double* __restrict__ y)
 {
@@ -925,25 +925,28 @@ k_combine(int64_t N, const int32_t* __restrict__ itemP_off, const int32_t* __res
     const int tgt = threadIdx.x & 31, m = threadIdx.x >> 5;
     const int64_t i = blockIdx.x * 32LL + tgt;
     double s = 0.0;
-    if (i < N) {
-        const int64_t g = i / PB_TG;
+    {
+        const int64_t ic = i < N ? i : N - 1;                      // padding lanes: same loads, nothing stored
+        const int64_t g = ic / PB_TG;
         const int nsP = itemP_off[g + 1] - itemP_off[g];
         const int nsM = itemM_off ? itemM_off[g + 1] - itemM_off[g] : 0;
-        s = sum_slots(accP + (int64_t)m * N + i, nsP, 4 * N, s);
-        if (nsM > 0) s = sum_slots(accM + (int64_t)m * N + i, nsM, 4 * N, s);
+        s = sum_slots(accP + (int64_t)m * N + ic, nsP, 4 * N, s);
+        if (nsM > 0) s = sum_slots(accM + (int64_t)m * N + ic, nsM, 4 * N, s);
         s *= PB_INV4PI;
         const double* __restrict__ xv = (m & 1) ? xphi : xdphi;     // V_L, V_Y act on dphi; K_L, K_Y on phi
-        const double* __restrict__ val = nr_val + (int64_t)m * ne;
-        const int32_t e1 = nr_off[i + 1];
-        int32_t e = nr_off[i];
-        for (; e + 4 <= e1; e += 4) {
+        // the slice's rows of the near table (sliced ELL: the warp reads 32 consecutive entries per step)
+        const int32_t b0 = el_base[blockIdx.x], width = (el_base[blockIdx.x + 1] - b0) / 32;
+        const double* __restrict__ val = el_val + (int64_t)m * ne + b0 + tgt;
+        const int32_t* __restrict__ col = el_col + b0 + tgt;
+        int k = 0;
+        for (; k + 4 <= width; k += 4) {
             double a[4], b[4];
 #pragma unroll
-            for (int k = 0; k < 4; ++k) { a[k] = val[e + k]; b[k] = xv[nr_col[e + k]]; }
+            for (int q = 0; q < 4; ++q) { a[q] = val[32 * (k + q)]; b[q] = xv[col[32 * (k + q)]]; }
 #pragma unroll
-            for (int k = 0; k < 4; ++k) s = fma(a[k], b[k], s);
+            for (int q = 0; q < 4; ++q) s = fma(a[q], b[q], s);
         }
-        for (; e < e1; ++e) s = fma(val[e], xv[nr_col[e]], s);
+        for (; k < width; ++k) s = fma(val[32 * k], xv[col[32 * k]], s);
     }
     sm[m][tgt] = s;
     __syncthreads();
@@ -1121,8 +1124,8 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed, bool pre
     }
     if (timed) PB_CUDA(cudaEventRecord(ctx->ev[4], st));
     k_combine<<<pb_blocks(t.N, 32), 128, 0, st>>>(t.N, t.itemP_off, far ? t.itemM_off : nullptr,
-                                                  ctx->prm.eps_in / ctx->prm.eps_out, t.accP, t.accM, t.nr_off,
-                                                  t.nr_col, t.nr_val, t.near_entries, t.xphi, t.xdphi, t.perm, y);
+                                                  ctx->prm.eps_in / ctx->prm.eps_out, t.accP, t.accM, t.el_base,
+                                                  t.el_col, t.el_val, t.el_entries, t.xphi, t.xdphi, t.perm, y);
     PB_LAUNCH_CHECK();
     ctx->matvec_calls++;
     if (timed) {

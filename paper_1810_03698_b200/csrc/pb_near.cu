@@ -359,6 +359,40 @@ __global__ void k_near_entries(entry_args a, pb_rule_t ruleN, pb_gl_t gl)
 }
 
 // ---- host driver -----------------------------------------------------------------------------------
+// ---- CSR -> sliced ELL: the layout k_combine streams ----------------------------------------------------------
+// Slice = 32 consecutive (Morton-ordered) targets = one warp of k_combine; entry k of lane l of slice s sits at
+// el_base[s] + 32 k + l, so a warp's loads are contiguous.  Rows shorter than the slice's longest are padded
+// with (value 0, column = the target itself).
+__global__ void k_ell_width(int64_t N, const int32_t* __restrict__ off, int32_t* __restrict__ width32)
+{
+    const int64_t w = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (w * 32 >= N) return;
+    const int64_t i = w * 32 + lane;
+    int len = i < N ? off[i + 1] - off[i] : 0;
+    for (int o = 16; o > 0; o >>= 1) len = max(len, __shfl_xor_sync(0xffffffffu, len, o));
+    if (lane == 0) width32[w] = len * 32;
+}
+
+__global__ void k_ell_fill(int64_t N, const int32_t* __restrict__ off, const int32_t* __restrict__ col,
+                           const double* __restrict__ val, int64_t ne, const int32_t* __restrict__ base,
+                           int64_t ne_ell, int32_t* __restrict__ ecol, double* __restrict__ eval)
+{
+    const int64_t w = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (w * 32 >= N) return;
+    const int64_t i = w * 32 + lane;
+    const int32_t b0 = base[w], width = (base[w + 1] - b0) / 32;
+    const int32_t e0 = i < N ? off[i] : 0, len = i < N ? off[i + 1] - e0 : 0;
+    for (int k = 0; k < width; ++k) {
+        const int64_t d = (int64_t)b0 + 32 * k + lane;
+        const bool real = k < len;
+        ecol[d] = real ? col[e0 + k] : (int32_t)(i < N ? i : N - 1);
+#pragma unroll
+        for (int m = 0; m < 4; ++m) eval[(int64_t)m * ne_ell + d] = real ? val[(int64_t)m * ne + e0 + k] : 0.0;
+    }
+}
+
 int pb_near_build(pb_ctx* ctx)
 {
     pb_tree& t = ctx->tree;
@@ -388,34 +422,55 @@ int pb_near_build(pb_ctx* ctx)
     int32_t* cnt;
     PB_TRY(pb_dalloc_t(ctx, &cnt, N + 1, CAT_TMP));
     PB_CUDA(cudaMemsetAsync(cnt, 0, sizeof(int32_t) * (N + 1), st));
-    PB_TRY(pb_dalloc_t(ctx, &t.nr_off, N + 1, CAT_TREE));
+    int32_t* nr_off;
+    PB_TRY(pb_dalloc_t(ctx, &nr_off, N + 1, CAT_TMP));
     a.cnt = cnt; a.off = nullptr; a.col = nullptr; a.row = nullptr; a.cls = nullptr;
     k_near_find<0><<<pb_blocks(N, 64), 64, 0, st>>>(a);
     PB_LAUNCH_CHECK();
     int64_t ne = 0;
-    PB_TRY(pb_exclusive_scan_i32(ctx, cnt, t.nr_off, N + 1, &ne));
+    PB_TRY(pb_exclusive_scan_i32(ctx, cnt, nr_off, N + 1, &ne));
     t.near_entries = ne;
     int32_t* row;
     int8_t* cls;
-    PB_TRY(pb_dalloc_t(ctx, &t.nr_col, ne, CAT_TREE));
-    PB_TRY(pb_dalloc_t(ctx, &t.nr_val, 4 * ne, CAT_TREE));
+    int32_t* nr_col;
+    double* nr_val;
+    PB_TRY(pb_dalloc_t(ctx, &nr_col, ne, CAT_TMP));
+    PB_TRY(pb_dalloc_t(ctx, &nr_val, 4 * ne, CAT_TMP));
     PB_TRY(pb_dalloc_t(ctx, &t.precond, 4 * N, CAT_TREE));
     PB_TRY(pb_dalloc_t(ctx, &row, ne, CAT_TMP));
     PB_TRY(pb_dalloc_t(ctx, &cls, ne, CAT_TMP));
-    a.off = t.nr_off; a.col = t.nr_col; a.row = row; a.cls = cls;
+    a.off = nr_off; a.col = nr_col; a.row = row; a.cls = cls;
     k_near_find<1><<<pb_blocks(N, 64), 64, 0, st>>>(a);
     PB_LAUNCH_CHECK();
 
     entry_args e;
     e.ne = ne; e.K = t.K; e.kappa = ctx->prm.kappa; e.eps_ratio = ctx->prm.eps_in / ctx->prm.eps_out;
-    e.row = row; e.col = t.nr_col; e.perm = t.perm; e.cls = cls;
+    e.row = row; e.col = nr_col; e.perm = t.perm; e.cls = cls;
     e.px = t.pc[0]; e.py = t.pc[1]; e.pz = t.pc[2]; e.nx = t.pn[0]; e.ny = t.pn[1]; e.nz = t.pn[2];
     e.parea = t.parea;
     for (int k = 0; k < 9; ++k) e.pv[k] = t.pv[k];
     e.sx = t.sx[0]; e.sy = t.sx[1]; e.sz = t.sx[2]; e.swA = t.swA;
-    e.val = t.nr_val; e.precond = t.precond; e.N = N;
+    e.val = nr_val; e.precond = t.precond; e.N = N;
     k_near_entries<<<pb_blocks(ne, 128), 128, 0, st>>>(e, ctx->ruleN, ctx->gl);
     PB_LAUNCH_CHECK();
+    // sliced ELL for the combine kernel
+    {
+        const int64_t nsl = (N + 31) / 32;
+        int32_t* width32;
+        PB_TRY(pb_dalloc_t(ctx, &width32, nsl + 1, CAT_TMP));
+        PB_CUDA(cudaMemsetAsync(width32, 0, sizeof(int32_t) * (nsl + 1), st));
+        k_ell_width<<<pb_blocks(nsl * 32, 128), 128, 0, st>>>(N, nr_off, width32);
+        PB_LAUNCH_CHECK();
+        PB_TRY(pb_dalloc_t(ctx, &t.el_base, nsl + 1, CAT_TREE));
+        int64_t ne_ell = 0;
+        PB_TRY(pb_exclusive_scan_i32(ctx, width32, t.el_base, nsl + 1, &ne_ell));
+        if (ne_ell >= 2147483647LL) return pb_fail(ctx, PB_ERR_INVALID_ARG, "near table too large for int32 indexing");
+        t.el_entries = ne_ell;
+        PB_TRY(pb_dalloc_t(ctx, &t.el_col, ne_ell > 0 ? ne_ell : 1, CAT_TREE));
+        PB_TRY(pb_dalloc_t(ctx, &t.el_val, ne_ell > 0 ? 4 * ne_ell : 1, CAT_TREE));
+        k_ell_fill<<<pb_blocks(nsl * 32, 128), 128, 0, st>>>(N, nr_off, nr_col, nr_val, ne, t.el_base, ne_ell, t.el_col, t.el_val);
+        PB_LAUNCH_CHECK();
+    }
     PB_CUDA(cudaStreamSynchronize(st));
     pb_dfree_cat(ctx, CAT_TMP);
     return PB_OK;
