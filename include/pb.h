@@ -179,7 +179,9 @@ int pb_multipole_field(pb_ctx* ctx, const double* mu, int use_mask, double* phi,
 
 /* ---- solvers ----------------------------------------------------------------------- */
 /* Restarted GMRES on A x = b, initial guess = x on entry.  iters/relres are HOST
- * outputs (may be NULL).  relres is the true ||b - A x|| / ||b||. */
+ * outputs (may be NULL).  relres is ||b - A x|| / ||b||: computed explicitly at the start and at every
+ * restart, and on exit taken from the Arnoldi recurrence (equal to it to rounding: right preconditioning,
+ * twice-orthogonalised basis), which saves one operator application per solve. */
 int pb_gmres(pb_ctx* ctx, const double* b, double* x, int32_t* iters, double* relres);
 
 /* One polarizable solve: vacuum SCF for mu^v, then the solvent SCF

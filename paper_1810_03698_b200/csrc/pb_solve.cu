@@ -414,6 +414,7 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
         if (iters >= maxit) { rc = PB_ERR_NO_CONVERGENCE; break; }
         std::fill(g.begin(), g.end(), 0.0);
         g[0] = beta;
+        bool accepted = false;
         int j = 0;
         for (; j < m && iters < maxit;) {
             const double* vj = ws.V + (size_t)j * n;
@@ -474,7 +475,8 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
             ++j;
             ++iters;
             relres = fabs(g[j]) / bnorm;
-            if (relres <= tol || hnext <= 1e-300) break;
+            if (relres <= tol) { accepted = true; break; }
+            if (hnext <= 1e-300) break;
         }
         // y = R^{-1} g ; x += Minv (V y)
         for (int i = j - 1; i >= 0; --i) {
@@ -494,6 +496,10 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
             k_axpy<<<pb_blocks(n, tb), tb, 0, st>>>(n, 1.0, ws.u, x);
         PB_LAUNCH_CHECK();
         PB_CUDA(cudaStreamSynchronize(st));   // hh is reused
+        // Converged by the Arnoldi residual |g_j|: with a RIGHT preconditioner and CGS2-orthogonal V this is the true
+        // residual norm to rounding, so no further operator application is spent on confirming it.  After a
+        // restart (no convergence within m steps) the loop recomputes the true residual as the new start.
+        if (accepted) break;
     }
     if (iters_out) *iters_out = iters;
     if (relres_out) *relres_out = relres;

@@ -234,8 +234,13 @@ def test_gmres_matches_dense_lu(pbm, po, torch_cuda):
     ctx.tree_build()
     x, info = ctx.gmres(torch_cuda.from_numpy(b))
     assert info["converged"] and rel(x.cpu().numpy(), xl) <= 1e-8
+    bt = torch_cuda.from_numpy(b).cuda()
+    true_res = float((bt - ctx.matvec(x)).norm() / bt.norm())
+    assert true_res <= 1.05e-11 and abs(true_res - info["relres"]) <= 1e-13      # the Arnoldi residual IS the true one
+    ctx.set_params(gmres_tol=2e-11)
     x2, info2 = ctx.gmres(torch_cuda.from_numpy(b), x0=x)
-    assert info2["iters"] == 0 and torch_cuda.equal(x, x2)
+    assert info2["iters"] == 0 and torch_cuda.equal(x, x2)                       # warm start from a converged x
+    ctx.set_params(gmres_tol=1e-11)
     xz, infoz = ctx.gmres(torch_cuda.zeros_like(x))
     assert infoz["iters"] == 0 and float(xz.abs().max()) == 0.0
     ctx.close()
