@@ -153,6 +153,8 @@ struct pb_gmres_ws {
     int64_t n = 0;
     int m = 0;
     double *V = nullptr, *w = nullptr, *z = nullptr, *r = nullptr, *u = nullptr;
+    double* ax = nullptr;         // A x of the x last returned (Arnoldi relation), valid while ax_valid
+    bool ax_valid = false;
     double *partial = nullptr, *hdev = nullptr, *coef = nullptr;
     unsigned int* counter = nullptr;   // arrival counter of k_dots' last-block reduction (self-resetting)
 };
@@ -267,4 +269,5 @@ int pb_prof_end(pb_ctx* ctx, int kernel);
 int pb_prof_drain(pb_ctx* ctx);
 void pb_prof_next(pb_ctx* ctx);
 // pb_solve.cu
-int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters, double* relres, int32_t* matvecs);
+int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters, double* relres, int32_t* matvecs,
+                  bool x_is_last_result);

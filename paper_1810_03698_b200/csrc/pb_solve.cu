@@ -337,7 +337,11 @@ static int norm2_host(pb_ctx* ctx, gmres_ws& ws, const double* v, double* out)
 // application (the preconditioner is folded into its first kernel), two classical Gram-Schmidt
 // passes of two kernels each -- the second also yields the norm of the new vector by Pythagoras and
 // writes it normalised -- and one small device-to-host copy of the Hessenberg column.
-int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, double* relres_out, int32_t* matvecs_out)
+// `x_is_last_result`: x still holds exactly what the previous call on this context returned (the SCF loop), so
+// A x is known from the Arnoldi relation A Minv V_j = V_{j+1} Hbar_j and the starting residual costs no operator
+// application: ws.ax is kept up to date with  A x += V_{j+1} (Hbar_j y)  whenever x += Minv V_j y.
+int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, double* relres_out, int32_t* matvecs_out,
+                  bool x_is_last_result)
 {
     pb_tree& t = ctx->tree;
     cudaStream_t st = ctx->stream;
@@ -356,6 +360,7 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
         PB_TRY(pb_dalloc_t(ctx, &ws.r, n, CAT_SOLVE));
         PB_TRY(pb_dalloc_t(ctx, &ws.u, n, CAT_SOLVE));
         PB_TRY(pb_dalloc_t(ctx, &ws.z, n, CAT_SOLVE));
+        PB_TRY(pb_dalloc_t(ctx, &ws.ax, n, CAT_SOLVE));
         PB_TRY(pb_dalloc_t(ctx, &ws.partial, (size_t)DOT_MAXBLK * (m + 2), CAT_SOLVE));
         PB_TRY(pb_dalloc_t(ctx, &ws.hdev, 2 * (m + 4) + 8, CAT_SOLVE));
         PB_TRY(pb_dalloc_t(ctx, &ws.coef, m + 2, CAT_SOLVE));
@@ -364,6 +369,8 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
         ws.n = n;
         ws.m = m;
     }
+    bool have_ax = x_is_last_result && ws.ax_valid;
+    ws.ax_valid = false;
     const int hstride = m + 4;
     PB_TRY(pb_pinned(ctx, (3 * (size_t)m + 64) * sizeof(double)));
     double* hh = ctx->h_pinned;                    // staging for h columns
@@ -384,7 +391,9 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
         if (matvecs_out) *matvecs_out = 0;
         return PB_OK;
     }
-    std::vector<double> H((size_t)(m + 1) * m, 0.0), cs(m, 0.0), sn(m, 0.0), g(m + 1, 0.0), yv(m, 0.0);
+    std::vector<double> H((size_t)(m + 1) * m, 0.0), Hraw((size_t)(m + 1) * m, 0.0), cs(m, 0.0), sn(m, 0.0), g(m + 1, 0.0),
+        yv(m, 0.0);
+
     const int tb = 256;
     const int nb = pb_blocks(n, tb) < 2368 ? pb_blocks(n, tb) : 2368;   // grid-stride above 16 blocks per SM
     // short vectors: the whole orthogonalisation in one cooperative launch (one block per 256 elements, all resident)
@@ -397,10 +406,13 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
         if (coop && need <= nsm && (size_t)2 * need * (m + 1) <= (size_t)DOT_MAXBLK * (m + 2)) coop_blocks = (int)need;
     }
     for (;;) {
-        // true residual r = b - A x
-        PB_TRY(pb_matvec_impl(ctx, x, ws.w, false, false));
-        ++matvecs;
-        k_residual<<<pb_blocks(n, tb), tb, 0, st>>>(n, b, ws.w, ws.r);
+        // residual r = b - A x: A x from the Arnoldi relation when it is known, else by applying the operator
+        if (!have_ax) {
+            PB_TRY(pb_matvec_impl(ctx, x, ws.ax, false, false));
+            ++matvecs;
+        }
+        have_ax = false;                               // after a restart the residual is recomputed from scratch
+        k_residual<<<pb_blocks(n, tb), tb, 0, st>>>(n, b, ws.ax, ws.r);
         PB_LAUNCH_CHECK();
         PB_TRY(dot_into(ctx, ws, 0, nullptr, ws.r, true, ws.hdev));
         k_normalize<<<nb, tb, 0, st>>>(n, ws.hdev, ws.r, ws.V);      // V_0 = r/||r||
@@ -410,7 +422,7 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
         PB_CUDA(cudaStreamSynchronize(st));
         const double beta = sqrt(r2);
         relres = beta / bnorm;
-        if (relres <= tol) break;
+        if (relres <= tol) { ws.ax_valid = true; break; }      // ws.ax = A x for the x we return
         if (iters >= maxit) { rc = PB_ERR_NO_CONVERGENCE; break; }
         std::fill(g.begin(), g.end(), 0.0);
         g[0] = beta;
@@ -456,8 +468,10 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
             }
             double* col = &H[(size_t)j * (m + 1)];
             for (int i = 0; i < nv; ++i) col[i] = hh[i] + hh[hstride + i];
+            for (int i = 0; i < nv; ++i) Hraw[(size_t)j * (m + 1) + i] = col[i];
             const double hnext = hn2 > 0 ? sqrt(hn2) : 0.0;
             col[nv] = hnext;
+            Hraw[(size_t)j * (m + 1) + nv] = hnext;
             // Givens rotations (host, O(j))
             for (int i = 0; i < j; ++i) {
                 double a = cs[i] * col[i] + sn[i] * col[i + 1];
@@ -496,6 +510,19 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
             k_axpy<<<pb_blocks(n, tb), tb, 0, st>>>(n, 1.0, ws.u, x);
         PB_LAUNCH_CHECK();
         PB_CUDA(cudaStreamSynchronize(st));   // hh is reused
+        // A x += V_{j+1} (Hbar_j y)
+        for (int i = 0; i <= j; ++i) {
+            double c = 0;
+            for (int k = (i > 0 ? i - 1 : 0); k < j; ++k) c += Hraw[(size_t)k * (m + 1) + i] * yv[k];
+            hh[i] = c;
+        }
+        PB_CUDA(cudaMemcpyAsync(ws.coef, hh, sizeof(double) * (j + 1), cudaMemcpyHostToDevice, st));
+        k_lincomb<<<pb_blocks(n, tb), tb, (j + 1) * sizeof(double), st>>>(n, j + 1, ws.V, n, ws.coef, ws.u);
+        PB_LAUNCH_CHECK();
+        k_axpy<<<pb_blocks(n, tb), tb, 0, st>>>(n, 1.0, ws.u, ws.ax);
+        PB_LAUNCH_CHECK();
+        PB_CUDA(cudaStreamSynchronize(st));
+        ws.ax_valid = accepted;
         // Converged by the Arnoldi residual |g_j|: with a RIGHT preconditioner and CGS2-orthogonal V this is the true
         // residual norm to rounding, so no further operator application is spent on confirming it.  After a
         // restart (no convergence within m steps) the loop recomputes the true residual as the new start.
@@ -512,7 +539,7 @@ extern "C" int pb_gmres(pb_ctx* ctx, const double* b, double* x, int32_t* iters,
 {
     if (!ctx) return PB_ERR_INVALID_ARG;
     if (!b || !x) return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_gmres: NULL vector");
-    return pb_gmres_impl(ctx, b, x, iters, relres, nullptr);
+    return pb_gmres_impl(ctx, b, x, iters, relres, nullptr, false);
 }
 
 // ---- SCF and energy kernels ------------------------------------------------------------------------
@@ -634,7 +661,7 @@ static int pb_solve_core(pb_ctx* ctx, double* x_out, double* mu_out, pb_result* 
     for (it = 1; it <= ctx->prm.scf_maxit; ++it) {
         int32_t gi = 0, mv = 0;
         PB_TRY(pb_rhs_multipole(ctx, mu, b));                        // step 2: Eq. (5) with p = d + mu
-        int rc = pb_gmres_impl(ctx, b, x, &gi, &relres, &mv);
+        int rc = pb_gmres_impl(ctx, b, x, &gi, &relres, &mv, it > 1);
         if (rc == PB_ERR_NO_CONVERGENCE) status = rc; else if (rc != PB_OK) return rc;
         gm_total += gi;
         mv_total += mv;
@@ -649,7 +676,7 @@ static int pb_solve_core(pb_ctx* ctx, double* x_out, double* mu_out, pb_result* 
         if (delta < tol) {                                            // step 6
             // surface solution consistent with the final mu
             PB_TRY(pb_rhs_multipole(ctx, mu, b));
-            rc = pb_gmres_impl(ctx, b, x, &gi, &relres, &mv);
+            rc = pb_gmres_impl(ctx, b, x, &gi, &relres, &mv, true);
             if (rc == PB_ERR_NO_CONVERGENCE) status = rc; else if (rc != PB_OK) return rc;
             gm_total += gi;
             mv_total += mv;
