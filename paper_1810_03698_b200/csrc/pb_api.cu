@@ -92,7 +92,7 @@ extern "C" void pb_default_params(pb_params* p)
     p->nq_edge = 16;
     p->precond = 1;
     p->gmres_tol = 1e-6;
-    p->gmres_restart = 100;
+    p->gmres_restart = 200;
     p->gmres_maxit = 1000;
     p->scf_tol_debye = 1e-7;
     p->scf_omega = 0.7;

@@ -1103,7 +1103,13 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed, bool pre
     PB_TRY(pb_weights(ctx, x, precond));
     if (timed) PB_CUDA(cudaEventRecord(ctx->ev[1], st));
     if (far && serial) PB_TRY(pb_far_branch(ctx, st, timed));
-    if (far && !serial) PB_CUDA(cudaEventRecord(ctx->ev_fork, st));
+    if (far && !serial) {
+        // the far-field branch is the longer one on small meshes (a latency chain): enqueue it first
+        PB_CUDA(cudaEventRecord(ctx->ev_fork, st));
+        PB_CUDA(cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0));
+        PB_TRY(pb_far_branch(ctx, ctx->side, false));
+        PB_CUDA(cudaEventRecord(ctx->ev_join, ctx->side));
+    }
     if (timed) {
         if (!far) PB_CUDA(cudaEventRecord(ctx->ev[2], st));
         PB_CUDA(cudaEventRecord(ctx->ev[3], st));
@@ -1116,12 +1122,7 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed, bool pre
         PB_TRY(pb_prof_end(ctx, 0));
         pb_prof_next(ctx);
     }
-    if (far && !serial) {
-        PB_CUDA(cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0));
-        PB_TRY(pb_far_branch(ctx, ctx->side, false));
-        PB_CUDA(cudaEventRecord(ctx->ev_join, ctx->side));
-        PB_CUDA(cudaStreamWaitEvent(st, ctx->ev_join, 0));
-    }
+    if (far && !serial) PB_CUDA(cudaStreamWaitEvent(st, ctx->ev_join, 0));
     if (timed) PB_CUDA(cudaEventRecord(ctx->ev[4], st));
     k_combine<<<pb_blocks(t.N, 32), 128, 0, st>>>(t.N, t.itemP_off, far ? t.itemM_off : nullptr,
                                                   ctx->prm.eps_in / ctx->prm.eps_out, t.accP, t.accM, t.el_base,

@@ -349,7 +349,7 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
     const int64_t n = 2 * t.N;
     int m = ctx->prm.gmres_restart;
     if (m > n) m = (int)n;
-    if (m > 120) m = 120;                          // k_dots<4> covers 4 x 32 vectors per block row
+    if (m > 1000) m = 1000;
     // workspace (kept until the system size or the restart length changes)
     gmres_ws& ws = ctx->gws;
     if (ws.n != n || ws.m != m || !ws.V) {
