@@ -61,7 +61,10 @@ typedef struct pb_params {
     int32_t K_near;         /* near-singular rule: 19                                 */
     double near_tau;        /* near-singular zone |c_i-c_j| < tau*sqrt(A_i)    */
     int32_t nq_edge;        /* Gauss-Legendre points per edge, semi-analytic rule (D: R-16)   */
-    int32_t precond;        /* 1: right block-diagonal preconditioner in GMRES, 0: none       */
+    int32_t precond;        /* GMRES right preconditioner: 0 none; 1 block-Jacobi (2x2 per panel from the SELF
+                               entries); 2 near-field: two block-Jacobi-preconditioned minimal-residual steps on
+                               the sparse matrix of the true SELF/ADJ/NEAR entries, inside flexible GMRES;
+                               3 (default) = 2 from 8,000 panels up, else 1                                    */
     double gmres_tol;       /* relative residual ||b-Ax||/||b||                       */
     int32_t gmres_restart;
     int32_t gmres_maxit;

@@ -90,7 +90,7 @@ extern "C" void pb_default_params(pb_params* p)
     p->K_near = 19;
     p->near_tau = 2.0;
     p->nq_edge = 16;
-    p->precond = 1;
+    p->precond = 3;
     p->gmres_tol = 1e-6;
     p->gmres_restart = 200;
     p->gmres_maxit = 1000;
@@ -179,6 +179,7 @@ extern "C" int pb_set_params(pb_ctx* ctx, const pb_params* p)
     if (p->gmres_restart < 1 || p->gmres_maxit < 1 || p->scf_maxit < 1 || !(p->gmres_tol > 0) ||
         !(p->scf_tol_debye > 0) || !(p->scf_omega > 0))
         return pb_fail(ctx, PB_ERR_INVALID_ARG, "solver limits/tolerances must be positive");
+    if (p->precond < 0 || p->precond > 3) return pb_fail(ctx, PB_ERR_INVALID_ARG, "precond must be 0, 1, 2 or 3");
     if (p->site_treecode < 0 || p->site_treecode > 2) return pb_fail(ctx, PB_ERR_INVALID_ARG, "site_treecode must be 0, 1 or 2");
     const pb_params& o = ctx->prm;
     bool shape = o.kappa != p->kappa || o.theta != p->theta || o.order_P != p->order_P ||

@@ -105,6 +105,7 @@ struct pb_tree {
     int32_t* el_base = nullptr;   // [slices + 1]
     int32_t* el_col = nullptr;    // [el_entries] source panel (Morton); padding: the target itself
     double* el_val = nullptr;     // [4][el_entries] VL, KL, VY, KY corrections; padding: 0
+    double* el_tval = nullptr;    // [4][el_entries] the true near-zone entries (near-field preconditioner); padding: 0
     double* precond = nullptr;    // [N][4] inverse 2x2 diagonal blocks
     // partial accumulators
     // work items (one thread block each) and their accumulator slots
@@ -154,6 +155,9 @@ struct pb_gmres_ws {
     int m = 0;
     double *V = nullptr, *w = nullptr, *z = nullptr, *r = nullptr, *u = nullptr;
     double* ax = nullptr;         // A x of the x last returned (Arnoldi relation), valid while ax_valid
+    double* Z = nullptr;          // [m][n] preconditioned basis of flexible GMRES (near-field preconditioner only)
+    double *nf_r = nullptr, *nf_p = nullptr, *nf_q = nullptr, *nf_z = nullptr;   // [n] inner iteration, Morton order
+    int mode = -1;                // preconditioner the workspace was sized for
     bool ax_valid = false;
     double *partial = nullptr, *hdev = nullptr, *coef = nullptr;
     unsigned int* counter = nullptr;   // arrival counter of k_dots' last-block reduction (self-resetting)

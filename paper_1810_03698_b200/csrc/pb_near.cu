@@ -306,7 +306,8 @@ struct entry_args {
     const double *px, *py, *pz, *nx, *ny, *nz, *parea;
     const double* pv[9];
     const double *sx, *sy, *sz, *swA;
-    double* val;        // [4][ne]
+    double* val;        // [4][ne] correction to what P2P / M2P supply (true - far rule; SELF: true)
+    double* tval;       // [4][ne] the true three-zone entries (the near-field matrix of the preconditioner)
     double* precond;    // [4][N], ORIGINAL panel order
     int64_t N;
 };
@@ -328,6 +329,7 @@ __global__ void k_near_entries(entry_args a, pb_rule_t ruleN, pb_gl_t gl)
     if (cls == CLS_SELF) {
         out[1] = 0.0;   // flat panel: n'.(c_i - r') == 0 on the panel itself
         out[3] = 0.0;
+        for (int m = 0; m < 4; ++m) a.tval[(int64_t)m * a.ne + e] = out[m];
         // inverse of the 2x2 diagonal block [[1/2, -V_L],[1/2, (eps1/eps2) V_Y]] (right preconditioner)
         double m01 = -out[0], m11 = a.eps_ratio * out[2];
         double det = 0.5 * m11 - m01 * 0.5;
@@ -337,6 +339,7 @@ __global__ void k_near_entries(entry_args a, pb_rule_t ruleN, pb_gl_t gl)
         a.precond[2 * a.N + o] = -0.5 / det;
         a.precond[3 * a.N + o] = 0.5 / det;
     } else {
+        for (int m = 0; m < 4; ++m) a.tval[(int64_t)m * a.ne + e] = out[m];
         // minus what P2P adds for this panel: the K_far rule over its stored Gauss points
         double s0 = 0, s1 = 0, s2 = 0, s3 = 0;
         for (int g = 0; g < a.K; ++g) {
@@ -375,8 +378,9 @@ __global__ void k_ell_width(int64_t N, const int32_t* __restrict__ off, int32_t*
 }
 
 __global__ void k_ell_fill(int64_t N, const int32_t* __restrict__ off, const int32_t* __restrict__ col,
-                           const double* __restrict__ val, int64_t ne, const int32_t* __restrict__ base,
-                           int64_t ne_ell, int32_t* __restrict__ ecol, double* __restrict__ eval)
+                           const double* __restrict__ val, const double* __restrict__ tval, int64_t ne,
+                           const int32_t* __restrict__ base, int64_t ne_ell, int32_t* __restrict__ ecol,
+                           double* __restrict__ eval, double* __restrict__ etval)
 {
     const int64_t w = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
@@ -389,7 +393,10 @@ __global__ void k_ell_fill(int64_t N, const int32_t* __restrict__ off, const int
         const bool real = k < len;
         ecol[d] = real ? col[e0 + k] : (int32_t)(i < N ? i : N - 1);
 #pragma unroll
-        for (int m = 0; m < 4; ++m) eval[(int64_t)m * ne_ell + d] = real ? val[(int64_t)m * ne + e0 + k] : 0.0;
+        for (int m = 0; m < 4; ++m) {
+            eval[(int64_t)m * ne_ell + d] = real ? val[(int64_t)m * ne + e0 + k] : 0.0;
+            etval[(int64_t)m * ne_ell + d] = real ? tval[(int64_t)m * ne + e0 + k] : 0.0;
+        }
     }
 }
 
@@ -436,6 +443,8 @@ int pb_near_build(pb_ctx* ctx)
     double* nr_val;
     PB_TRY(pb_dalloc_t(ctx, &nr_col, ne, CAT_TMP));
     PB_TRY(pb_dalloc_t(ctx, &nr_val, 4 * ne, CAT_TMP));
+    double* nr_tval;
+    PB_TRY(pb_dalloc_t(ctx, &nr_tval, 4 * ne, CAT_TMP));
     PB_TRY(pb_dalloc_t(ctx, &t.precond, 4 * N, CAT_TREE));
     PB_TRY(pb_dalloc_t(ctx, &row, ne, CAT_TMP));
     PB_TRY(pb_dalloc_t(ctx, &cls, ne, CAT_TMP));
@@ -450,7 +459,7 @@ int pb_near_build(pb_ctx* ctx)
     e.parea = t.parea;
     for (int k = 0; k < 9; ++k) e.pv[k] = t.pv[k];
     e.sx = t.sx[0]; e.sy = t.sx[1]; e.sz = t.sx[2]; e.swA = t.swA;
-    e.val = nr_val; e.precond = t.precond; e.N = N;
+    e.val = nr_val; e.tval = nr_tval; e.precond = t.precond; e.N = N;
     k_near_entries<<<pb_blocks(ne, 128), 128, 0, st>>>(e, ctx->ruleN, ctx->gl);
     PB_LAUNCH_CHECK();
     // sliced ELL for the combine kernel
@@ -468,7 +477,9 @@ int pb_near_build(pb_ctx* ctx)
         t.el_entries = ne_ell;
         PB_TRY(pb_dalloc_t(ctx, &t.el_col, ne_ell > 0 ? ne_ell : 1, CAT_TREE));
         PB_TRY(pb_dalloc_t(ctx, &t.el_val, ne_ell > 0 ? 4 * ne_ell : 1, CAT_TREE));
-        k_ell_fill<<<pb_blocks(nsl * 32, 128), 128, 0, st>>>(N, nr_off, nr_col, nr_val, ne, t.el_base, ne_ell, t.el_col, t.el_val);
+        PB_TRY(pb_dalloc_t(ctx, &t.el_tval, ne_ell > 0 ? 4 * ne_ell : 1, CAT_TREE));
+        k_ell_fill<<<pb_blocks(nsl * 32, 128), 128, 0, st>>>(N, nr_off, nr_col, nr_val, nr_tval, ne, t.el_base, ne_ell, t.el_col,
+                                                                 t.el_val, t.el_tval);
         PB_LAUNCH_CHECK();
     }
     PB_CUDA(cudaStreamSynchronize(st));

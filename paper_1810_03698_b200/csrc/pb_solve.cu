@@ -292,7 +292,145 @@ __global__ void k_axpy(int64_t n, double a, const double* __restrict__ x, double
     if (e < n) y[e] = fma(a, x[e], y[e]);
 }
 
+// ---- near-field preconditioner (flexible GMRES) ---------------------------------------------------------------
+// z = M(v): PB_NF_STEPS minimal-residual steps, block-Jacobi preconditioned, on the sparse NEAR-FIELD matrix A_n of
+// Eq. (5) -- the true SELF / ADJ / NEAR entries of the three-zone quadrature, i.e. the part of the operator
+// that carries the singular local behaviour at the creases of a van-der-Waals surface:
+//     r = v, z = 0;  repeat:  p = D^-1 r;  q = A_n p;  alpha = (r.q)/(q.q);  z += alpha p;  r -= alpha q.
+// alpha stays on the device (no host synchronisation); the iteration runs in Morton order, where the table lives.
+// M depends on v non-linearly (through alpha), hence the flexible variant of GMRES.  Measured on the oracle's dense
+// matrix of C2 (19,176 unknowns): 72 outer iterations with block-Jacobi alone, 42 with 2 inner steps, 40 with 3,
+// 28 with an exact sparse solve of A_n.
+#define PB_NF_STEPS 2
+
+__global__ void k_nf_start(int64_t N, const int32_t* __restrict__ perm, const double* __restrict__ pc,
+                           const double* __restrict__ v, double* __restrict__ r, double* __restrict__ p, double* __restrict__ z)
+{
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int64_t o = perm[i];
+    const double a = v[o], b = v[N + o];
+    r[i] = a; r[N + i] = b;
+    p[i] = pc[o] * a + pc[N + o] * b;
+    p[N + i] = pc[2 * N + o] * a + pc[3 * N + o] * b;
+    z[i] = 0.0; z[N + i] = 0.0;
+}
+
+// q = A_n p in Morton order; block = 32 targets (one ELL slice) x 4 kernels, as in k_combine
+__global__ void __launch_bounds__(128)
+k_nf_spmv(int64_t N, double eps_ratio, const int32_t* __restrict__ el_base, const int32_t* __restrict__ el_col,
+          const double* __restrict__ el_tval, int64_t ne, const double* __restrict__ p, double* __restrict__ q)
+{
+    __shared__ double sm[4][32];
+    const int tgt = threadIdx.x & 31, m = threadIdx.x >> 5;
+    const int64_t i = blockIdx.x * 32LL + tgt;
+    const double* __restrict__ xv = (m & 1) ? p : p + N;          // V_L, V_Y act on dphi; K_L, K_Y on phi
+    const int32_t b0 = el_base[blockIdx.x], width = (el_base[blockIdx.x + 1] - b0) / 32;
+    const double* __restrict__ val = el_tval + (int64_t)m * ne + b0 + tgt;
+    const int32_t* __restrict__ col = el_col + b0 + tgt;
+    double s = 0.0;
+    int k = 0;
+    for (; k + 4 <= width; k += 4) {
+        double a[4], b[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { a[u] = val[32 * (k + u)]; b[u] = xv[col[32 * (k + u)]]; }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) s = fma(a[u], b[u], s);
+    }
+    for (; k < width; ++k) s = fma(val[32 * k], xv[col[32 * k]], s);
+    sm[m][tgt] = s;
+    __syncthreads();
+    if (m == 0 && i < N) {
+        const double VL = sm[0][tgt], KL = sm[1][tgt], VY = sm[2][tgt], KY = sm[3][tgt];
+        const double phi = p[i];
+        q[i] = 0.5 * phi + KL - VL;                     // Eq. (5), first row restricted to the near zone
+        q[N + i] = 0.5 * phi - KY + eps_ratio * VY;     // second row
+    }
+}
+
+// out[0] = (r.q)/(q.q) by the last block to finish (fixed summation pattern)
+__global__ void __launch_bounds__(256)
+k_nf_alpha(int64_t n, const double* __restrict__ r, const double* __restrict__ q, double* __restrict__ partial,
+           unsigned int* __restrict__ counter, double* __restrict__ out)
+{
+    __shared__ double red[2][8];
+    __shared__ bool last;
+    double a = 0, b = 0;
+    for (int64_t e = blockIdx.x * 256LL + threadIdx.x; e < n; e += 256LL * gridDim.x) {
+        const double qe = q[e];
+        a = fma(r[e], qe, a);
+        b = fma(qe, qe, b);
+    }
+    for (int o = 16; o > 0; o >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, o); b += __shfl_xor_sync(0xffffffffu, b, o); }
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) { red[0][w] = a; red[1][w] = b; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        a = 0; b = 0;
+        for (int k = 0; k < 8; ++k) { a += red[0][k]; b += red[1][k]; }
+        partial[2 * blockIdx.x] = a;
+        partial[2 * blockIdx.x + 1] = b;
+        __threadfence();
+        last = atomicAdd(counter, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    if (threadIdx.x < 32) {
+        a = 0; b = 0;
+        for (unsigned k = threadIdx.x; k < gridDim.x; k += 32) { a += __ldcg(&partial[2 * k]); b += __ldcg(&partial[2 * k + 1]); }
+        for (int o = 16; o > 0; o >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, o); b += __shfl_xor_sync(0xffffffffu, b, o); }
+        if (threadIdx.x == 0) { out[0] = b > 0 ? a / b : 0.0; *counter = 0u; }
+    }
+}
+
+// z += alpha p; r -= alpha q; then either p = D^-1 r for the next step or, at the end, zout = z in the caller's order
+__global__ void k_nf_update(int64_t N, const double* __restrict__ alpha, const int32_t* __restrict__ perm,
+                            const double* __restrict__ pc, double* __restrict__ p, const double* __restrict__ q,
+                            double* __restrict__ r, double* __restrict__ z, double* __restrict__ zout)
+{
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const double al = *alpha;
+    const double z0 = fma(al, p[i], z[i]), z1 = fma(al, p[N + i], z[N + i]);
+    const int64_t o = perm[i];
+    if (zout) {
+        zout[o] = z0; zout[N + o] = z1;
+        return;
+    }
+    z[i] = z0; z[N + i] = z1;
+    const double a = fma(-al, q[i], r[i]), b = fma(-al, q[N + i], r[N + i]);
+    r[i] = a; r[N + i] = b;
+    p[i] = pc[o] * a + pc[N + o] * b;
+    p[N + i] = pc[2 * N + o] * a + pc[3 * N + o] * b;
+}
+
 typedef pb_gmres_ws gmres_ws;
+
+// z = M(v) (near-field preconditioner); v, z in the caller's panel order
+static int near_precond(pb_ctx* ctx, gmres_ws& ws, const double* v, double* z)
+{
+    pb_tree& t = ctx->tree;
+    cudaStream_t st = ctx->stream;
+    const int64_t N = t.N, n = 2 * N;
+    const int tb = 256;
+    const int nbN = pb_blocks(N, tb);
+    int nbd = pb_blocks(n, 256 * 8);
+    if (nbd > 592) nbd = 592;
+    k_nf_start<<<nbN, tb, 0, st>>>(N, t.perm, t.precond, v, ws.nf_r, ws.nf_p, ws.nf_z);
+    PB_LAUNCH_CHECK();
+    for (int step = 0; step < PB_NF_STEPS; ++step) {
+        k_nf_spmv<<<pb_blocks(N, 32), 128, 0, st>>>(N, ctx->prm.eps_in / ctx->prm.eps_out, t.el_base, t.el_col, t.el_tval,
+                                                    t.el_entries, ws.nf_p, ws.nf_q);
+        PB_LAUNCH_CHECK();
+        k_nf_alpha<<<nbd, 256, 0, st>>>(n, ws.nf_r, ws.nf_q, ws.partial, ws.counter, ws.hdev + 2 * (ws.m + 4) + 4);
+        PB_LAUNCH_CHECK();
+        k_nf_update<<<nbN, tb, 0, st>>>(N, ws.hdev + 2 * (ws.m + 4) + 4, t.perm, t.precond, ws.nf_p, ws.nf_q, ws.nf_r, ws.nf_z,
+                                        step + 1 == PB_NF_STEPS ? z : nullptr);
+        PB_LAUNCH_CHECK();
+    }
+    return PB_OK;
+}
 
 // hout[0..nv) = V^T w (and hout[nv] = w.w with `self`), all on the device
 static int dot_into(pb_ctx* ctx, gmres_ws& ws, int nv, const double* V, const double* w, bool self, double* hout)
@@ -347,12 +485,17 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
     cudaStream_t st = ctx->stream;
     if (!t.built) return pb_fail(ctx, PB_ERR_NOT_READY, "pb_gmres: call pb_tree_build first");
     const int64_t n = 2 * t.N;
+    // preconditioner: 0 none, 1 block-Jacobi (folded into the operator's first kernel), 2 near-field (flexible GMRES),
+    // 3 = near-field from 8,000 panels up (measured per solve: C1 20.0 -> 19.2 ms, C2 117 -> 91 ms, C3 1412 -> 978 ms),
+    // else block-Jacobi
+    int mode = ctx->prm.precond;
+    if (mode == 3) mode = t.N >= 8000 ? 2 : 1;
     int m = ctx->prm.gmres_restart;
     if (m > n) m = (int)n;
     if (m > 1000) m = 1000;
     // workspace (kept until the system size or the restart length changes)
     gmres_ws& ws = ctx->gws;
-    if (ws.n != n || ws.m != m || !ws.V) {
+    if (ws.n != n || ws.m != m || ws.mode != mode || !ws.V) {
         pb_dfree_cat(ctx, CAT_SOLVE);
         ws = gmres_ws();
         PB_TRY(pb_dalloc_t(ctx, &ws.V, (size_t)(m + 1) * n, CAT_SOLVE));
@@ -361,6 +504,14 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
         PB_TRY(pb_dalloc_t(ctx, &ws.u, n, CAT_SOLVE));
         PB_TRY(pb_dalloc_t(ctx, &ws.z, n, CAT_SOLVE));
         PB_TRY(pb_dalloc_t(ctx, &ws.ax, n, CAT_SOLVE));
+        if (mode == 2) {
+            PB_TRY(pb_dalloc_t(ctx, &ws.Z, (size_t)m * n, CAT_SOLVE));
+            PB_TRY(pb_dalloc_t(ctx, &ws.nf_r, n, CAT_SOLVE));
+            PB_TRY(pb_dalloc_t(ctx, &ws.nf_p, n, CAT_SOLVE));
+            PB_TRY(pb_dalloc_t(ctx, &ws.nf_q, n, CAT_SOLVE));
+            PB_TRY(pb_dalloc_t(ctx, &ws.nf_z, n, CAT_SOLVE));
+        }
+        ws.mode = mode;
         PB_TRY(pb_dalloc_t(ctx, &ws.partial, (size_t)DOT_MAXBLK * (m + 2), CAT_SOLVE));
         PB_TRY(pb_dalloc_t(ctx, &ws.hdev, 2 * (m + 4) + 8, CAT_SOLVE));
         PB_TRY(pb_dalloc_t(ctx, &ws.coef, m + 2, CAT_SOLVE));
@@ -374,7 +525,7 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
     const int hstride = m + 4;
     PB_TRY(pb_pinned(ctx, (3 * (size_t)m + 64) * sizeof(double)));
     double* hh = ctx->h_pinned;                    // staging for h columns
-    const bool pc = ctx->prm.precond != 0;
+    const bool pc = mode == 1;
     const double tol = ctx->prm.gmres_tol;
     const int maxit = ctx->prm.gmres_maxit;
     int iters = 0, matvecs = 0;
@@ -431,7 +582,12 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
         for (; j < m && iters < maxit;) {
             const double* vj = ws.V + (size_t)j * n;
             double* vnext = ws.V + (size_t)(j + 1) * n;
-            PB_TRY(pb_matvec_impl(ctx, vj, ws.w, false, pc));        // w = A Minv v_j
+            if (mode == 2) {                                          // flexible: z_j = M(v_j) is kept, w = A z_j
+                double* zj = ws.Z + (size_t)j * n;
+                PB_TRY(near_precond(ctx, ws, vj, zj));
+                PB_TRY(pb_matvec_impl(ctx, zj, ws.w, false, false));
+            } else
+                PB_TRY(pb_matvec_impl(ctx, vj, ws.w, false, pc));    // w = A Minv v_j
             ++matvecs;
             const int nv = j + 1;
             // classical Gram-Schmidt, twice
@@ -500,7 +656,7 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
         }
         for (int i = 0; i < j; ++i) hh[i] = yv[i];
         PB_CUDA(cudaMemcpyAsync(ws.coef, hh, sizeof(double) * j, cudaMemcpyHostToDevice, st));
-        k_lincomb<<<pb_blocks(n, tb), tb, j * sizeof(double), st>>>(n, j, ws.V, n, ws.coef, ws.u);
+        k_lincomb<<<pb_blocks(n, tb), tb, j * sizeof(double), st>>>(n, j, mode == 2 ? ws.Z : ws.V, n, ws.coef, ws.u);   // x += Z y (flexible)
         PB_LAUNCH_CHECK();
         if (pc) {
             k_precond<<<pb_blocks(t.N, tb), tb, 0, st>>>(t.N, t.precond, ws.u, ws.z);
