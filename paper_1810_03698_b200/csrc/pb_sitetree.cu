@@ -17,6 +17,7 @@
 
 #define ST_MAXP 8                 // coefficient order P + 2 <= 10
 #define ST_GROUP 32               // sites per group = threads per k_site_m2p block
+#define ST_SPLIT 8                // blocks per group: each takes an eighth of the group's cell list
 
 static double st_fact(int n) { double f = 1; for (int i = 2; i <= n; ++i) f *= i; return f; }
 
@@ -73,7 +74,8 @@ int pb_site_tables(pb_ctx* ctx)
 // ---- far field: one block per site group, one lane per site; every lane walks the group's cell list --------
 // a_k of the lane's (site, cell) pair live in shared memory, [k][lane] (conflict free); the cell's moments,
 // the neighbour and derivative tables are the same for all lanes (broadcast loads).
-// out [na][10] (Morton order of the sites): phi, grad, hess WITHOUT the 1/(4 pi); NO = 1, 4 or 10 outputs wanted.
+// out [ST_SPLIT][na][10] (Morton order of the sites; one slab per share of the list, added in order by
+// k_site_finish): phi, grad, hess WITHOUT the 1/(4 pi); NO = 4 or 10 outputs wanted.
 template <int NO>
 __global__ void __launch_bounds__(ST_GROUP)
 k_site_m2p(int64_t na, int P, const double* __restrict__ sx, const double* __restrict__ sy, const double* __restrict__ sz,
@@ -85,6 +87,7 @@ k_site_m2p(int64_t na, int P, const double* __restrict__ sx, const double* __res
     extern __shared__ double st_a[];                   // [NkQ][ST_GROUP]
     const int lane = threadIdx.x;
     const int64_t g = blockIdx.x;
+    const int part = blockIdx.y;                       // this block's share of the group's cell list
     const int64_t i = g * ST_GROUP + lane;
     const int64_t ic = i < na ? i : na - 1;            // padding lanes repeat the last site; never stored
     const double x = sx[ic], y = sy[ic], z = sz[ic];
@@ -94,7 +97,9 @@ k_site_m2p(int64_t na, int P, const double* __restrict__ sx, const double* __res
 #pragma unroll
     for (int q = 0; q < NO; ++q) acc[q] = 0.0;
     double* a = st_a + lane;
-    for (int32_t e = m2p_off[g]; e < m2p_off[g + 1]; ++e) {
+    const int32_t l0 = m2p_off[g], ln = m2p_off[g + 1] - l0;
+    const int32_t e_lo = l0 + (int32_t)((int64_t)ln * part / ST_SPLIT), e_hi = l0 + (int32_t)((int64_t)ln * (part + 1) / ST_SPLIT);
+    for (int32_t e = e_lo; e < e_hi; ++e) {
         const int32_t c = m2p_cell[e];
         const double d[3] = {x - cx[c], y - cy[c], z - cz[c]};
         const double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
@@ -123,7 +128,7 @@ k_site_m2p(int64_t na, int P, const double* __restrict__ sx, const double* __res
     }
     if (i < na) {
 #pragma unroll
-        for (int q = 0; q < NO; ++q) out[i * 10 + q] = acc[q];
+        for (int q = 0; q < NO; ++q) out[((int64_t)part * na + i) * 10 + q] = acc[q];
     }
 }
 
@@ -214,7 +219,9 @@ __global__ void k_site_finish(int64_t na, int NO, const int32_t* __restrict__ pe
     const int64_t i = gidx / NO;
     const int c = (int)(gidx % NO);
     const int64_t m = perm[i];
-    const double v = (nearp[i * 10 + c] + farp[i * 10 + c]) * PB_INV4PI;
+    double f = 0.0;
+    for (int sp = 0; sp < ST_SPLIT; ++sp) f += farp[((int64_t)sp * na + i) * 10 + c];
+    const double v = (nearp[i * 10 + c] + f) * PB_INV4PI;
     if (c == 0) { if (phi) phi[m] = v; }
     else if (c < 4) { if (grad) grad[3 * m + c - 1] = v; }
     else if (hess) hess[6 * m + c - 4] = v;
@@ -239,7 +246,7 @@ int pb_reaction_field_tree(pb_ctx* ctx, double* phi, double* grad, double* hess)
     cudaStream_t st = ctx->stream;
     const bool H = hess != nullptr;
     const int NO = H ? 10 : 4;
-    PB_TRY(pb_scratch(ctx, (size_t)2 * s.na * 10 * sizeof(double) + 4096));
+    PB_TRY(pb_scratch(ctx, (size_t)(1 + ST_SPLIT) * s.na * 10 * sizeof(double) + 4096));
     double* nearp = ctx->scratch;
     double* farp = ctx->scratch + (size_t)s.na * 10;
     PB_TRY(pb_upward(ctx, st, s.t_need_leaf, s.t_n_need_leaf, s.t_up_link));
@@ -252,14 +259,14 @@ int pb_reaction_field_tree(pb_ctx* ctx, double* phi, double* grad, double* hess)
     }
     const unsigned G = (unsigned)s.t_groups;
     if (H) {
-        k_site_m2p<10><<<G, ST_GROUP, sm, st>>>(s.na, t.P, s.tpos[0], s.tpos[1], s.tpos[2], s.t_m2p_off, s.t_m2p_cell, t.c_ctr[0],
+        k_site_m2p<10><<<dim3(G, ST_SPLIT), ST_GROUP, sm, st>>>(s.na, t.P, s.tpos[0], s.tpos[1], s.tpos[2], s.t_m2p_off, s.t_m2p_cell, t.c_ctr[0],
                                                t.c_ctr[1], t.c_ctr[2], t.M, s.nb_idx, s.dv_idx, s.dv_fac, farp);
         PB_LAUNCH_CHECK();
         k_site_p2p<true><<<G * (ST_GROUP / SP_ST), SP_THREADS, 0, st>>>(s.na, s.tpos[0], s.tpos[1], s.tpos[2], s.t_p2p_off,
                                                                         s.t_p2p_lo, s.t_p2p_hi, t.srec, nearp);
         PB_LAUNCH_CHECK();
     } else {
-        k_site_m2p<4><<<G, ST_GROUP, sm, st>>>(s.na, t.P, s.tpos[0], s.tpos[1], s.tpos[2], s.t_m2p_off, s.t_m2p_cell, t.c_ctr[0],
+        k_site_m2p<4><<<dim3(G, ST_SPLIT), ST_GROUP, sm, st>>>(s.na, t.P, s.tpos[0], s.tpos[1], s.tpos[2], s.t_m2p_off, s.t_m2p_cell, t.c_ctr[0],
                                               t.c_ctr[1], t.c_ctr[2], t.M, s.nb_idx, s.dv_idx, s.dv_fac, farp);
         PB_LAUNCH_CHECK();
         k_site_p2p<false><<<G * (ST_GROUP / SP_ST), SP_THREADS, 0, st>>>(s.na, s.tpos[0], s.tpos[1], s.tpos[2], s.t_p2p_off,

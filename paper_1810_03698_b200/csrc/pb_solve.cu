@@ -293,7 +293,7 @@ __global__ void k_axpy(int64_t n, double a, const double* __restrict__ x, double
 }
 
 // ---- near-field preconditioner (flexible GMRES) ---------------------------------------------------------------
-// z = M(v): PB_NF_STEPS minimal-residual steps, block-Jacobi preconditioned, on the sparse NEAR-FIELD matrix A_n of
+// z = M(v): PB_NF_STEPS (2; 4 from 30,000 panels, 6 from 300,000) minimal-residual steps, block-Jacobi preconditioned, on the sparse NEAR-FIELD matrix A_n of
 // Eq. (5) -- the true SELF / ADJ / NEAR entries of the three-zone quadrature, i.e. the part of the operator
 // that carries the singular local behaviour at the creases of a van-der-Waals surface:
 //     r = v, z = 0;  repeat:  p = D^-1 r;  q = A_n p;  alpha = (r.q)/(q.q);  z += alpha p;  r -= alpha q.
@@ -419,14 +419,17 @@ static int near_precond(pb_ctx* ctx, gmres_ws& ws, const double* v, double* z)
     if (nbd > 592) nbd = 592;
     k_nf_start<<<nbN, tb, 0, st>>>(N, t.perm, t.precond, v, ws.nf_r, ws.nf_p, ws.nf_z);
     PB_LAUNCH_CHECK();
-    for (int step = 0; step < PB_NF_STEPS; ++step) {
+    // more inner steps where the operator is expensive: cold-solve iterations at C3 89 / 74 / 68 and at C4 177 / 147 / 137
+    // with 2 / 4 / 6 steps (block-Jacobi alone: 147 and 317)
+    const int nsteps = N < 30000 ? PB_NF_STEPS : (N < 300000 ? 2 * PB_NF_STEPS : 3 * PB_NF_STEPS);
+    for (int step = 0; step < nsteps; ++step) {
         k_nf_spmv<<<pb_blocks(N, 32), 128, 0, st>>>(N, ctx->prm.eps_in / ctx->prm.eps_out, t.el_base, t.el_col, t.el_tval,
                                                     t.el_entries, ws.nf_p, ws.nf_q);
         PB_LAUNCH_CHECK();
         k_nf_alpha<<<nbd, 256, 0, st>>>(n, ws.nf_r, ws.nf_q, ws.partial, ws.counter, ws.hdev + 2 * (ws.m + 4) + 4);
         PB_LAUNCH_CHECK();
         k_nf_update<<<nbN, tb, 0, st>>>(N, ws.hdev + 2 * (ws.m + 4) + 4, t.perm, t.precond, ws.nf_p, ws.nf_q, ws.nf_r, ws.nf_z,
-                                        step + 1 == PB_NF_STEPS ? z : nullptr);
+                                        step + 1 == nsteps ? z : nullptr);
         PB_LAUNCH_CHECK();
     }
     return PB_OK;
