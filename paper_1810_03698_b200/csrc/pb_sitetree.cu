@@ -91,7 +91,7 @@ k_site_m2p(int64_t na, int P, const double* __restrict__ sx, const double* __res
     const int64_t i = g * ST_GROUP + lane;
     const int64_t ic = i < na ? i : na - 1;            // padding lanes repeat the last site; never stored
     const double x = sx[ic], y = sy[ic], z = sz[ic];
-    const int Q = P + 2;
+    const int Q = P + (NO > 4 ? 2 : 1);                // the gradient needs one order more than the sum, the Hessian two
     const int NkQ = pb_nk(Q), NkP = pb_nk(P);
     double acc[NO];
 #pragma unroll
@@ -106,7 +106,8 @@ k_site_m2p(int64_t na, int P, const double* __restrict__ sx, const double* __res
         const double ri = pb_rsqrt(r2), ri2 = ri * ri;
         a[0] = ri;
         for (int k = 1; k < NkQ; ++k) {                // graded order: every neighbour is already there
-            const int32_t* nb = nb_idx + (size_t)k * 8;
+            const int4 na_ = reinterpret_cast<const int4*>(nb_idx)[2 * k], nb_ = reinterpret_cast<const int4*>(nb_idx)[2 * k + 1];
+            const int32_t nb[8] = {na_.x, na_.y, na_.z, na_.w, nb_.x, nb_.y, nb_.z, nb_.w};
             const int n = nb[6];
             double s1 = 0.0, s2 = 0.0;
 #pragma unroll
