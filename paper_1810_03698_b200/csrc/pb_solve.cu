@@ -195,12 +195,13 @@ k_cgs2(int64_t n, int nv, const double* __restrict__ V, int64_t ld, double* __re
             if (lane == 0) part[(size_t)blockIdx.x * nvt + j] = s;
         }
     };
-    auto gather = [&](const double* part, int count) {   // hs[j] = sum over blocks, fixed order
+    auto gather = [&](const double* part, int count) {   // hs[j] = sum over blocks: a warp per j, lanes over blocks, butterfly
         __syncthreads();
-        for (int j = tid; j < count; j += CGS_CHUNK) {
+        for (int j = wid; j < count; j += CGS_CHUNK / 32) {
             double s = 0;
-            for (int b = 0; b < nb; ++b) s += __ldcg(&part[(size_t)b * nvt + j]);
-            hs[j] = s;
+            for (int b = lane; b < nb; b += 32) s += __ldcg(&part[(size_t)b * nvt + j]);
+            for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+            if (lane == 0) hs[j] = s;
         }
         __syncthreads();
     };
