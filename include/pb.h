@@ -14,7 +14,9 @@
  *    panel and site order.  The internal Morton permutation never leaks.
  *  - Work is enqueued on the context's cudaStream_t.  Calls that return host values
  *    (pb_solve, pb_gmres, pb_get_stats, the *_host variants) synchronise that stream;
- *    pb_matvec, pb_rhs_multipole, pb_reaction_field and pb_multipole_field do not.
+ *    pb_matvec, pb_rhs_multipole, pb_reaction_field and pb_multipole_field do not.  pb_matvec runs
+ *    its far-field branch on a library-owned second stream that forks from and joins back into the
+ *    context's stream, so stream order as seen by the caller is unchanged.
  *  - Device memory for internal state is obtained through the allocator callbacks
  *    (pb_set_allocator: the Python binding hands out torch tensors); with no allocator set
  *    the library falls back to cudaMalloc/cudaFree.  Memory is released by pb_destroy or
@@ -145,9 +147,11 @@ int pb_sites_load(pb_ctx* ctx, int64_t na, const double* pos, const double* q, c
 
 /* ---- setup: octree, interaction lists, near/singular table --------------- */
 /* Morton-sorts the panels (63-bit key of the centroid), builds the octree over the K_far
- * Gauss points of whole panels (leaf <= ncrit points), the per-target-group M2P / P2P
- * lists by the MAC of Eq. (28), and the SELF/ADJ/NEAR correction table (semi-analytic and
- * K_near-point entries).  Needs pb_mesh_load. */
+ * Gauss points of whole panels (leaf <= ncrit points), the M2P / P2P lists of every group of 64
+ * consecutive targets (a cell is accepted when the MAC of Eq. (28) holds for each target of the group),
+ * and the SELF/ADJ/NEAR table (semi-analytic and K_near-point entries; both the corrections to the far
+ * rule that the matvec adds and the true entries that the near-field preconditioner uses).  Needs
+ * pb_mesh_load. */
 int pb_tree_build(pb_ctx* ctx);
 
 /* ---- operators --------------------------------------------------------------------- */
