@@ -61,6 +61,31 @@ struct pb_expk {
     double T[32];
 };
 
+// Finer table, shorter polynomial, for the P2P kernel where exp(-kappa r) is evaluated once per pair:
+//   n = rint(r * c1), c1 = 256 kappa / ln 2;  g = r - n * Lk, |kappa g| <= ln2/512;
+//   exp(-kappa r) = 2^-(n>>8) * T256[n&255] * sum_{m<=4} c[m] g^m      (truncation (kappa g)^5/5! < 4e-17)
+struct pb_expk8 {
+    double c1, Lk;
+    double c[5];
+};
+
+__device__ __forceinline__ double pb_exp_mkr8(double r, const pb_expk8& k, const double* __restrict__ T256)
+{
+    const double MAGIC = 6755399441055744.0;   // 1.5 * 2^52: the low word of (v + MAGIC) is rint(v)
+    const double s = fma(r, k.c1, MAGIC);
+    const double nf = s - MAGIC;
+    const double g = fma(nf, -k.Lk, r);
+    unsigned n = (unsigned)__double2loint(s);
+    n = n < 256000u ? n : 256000u;              // exp(-690) already underflows; also tames padding lanes
+    double p = k.c[4];
+    p = fma(p, g, k.c[3]);
+    p = fma(p, g, k.c[2]);
+    p = fma(p, g, k.c[1]);
+    p = fma(p, g, k.c[0]);
+    const double v = p * T256[n & 255u];
+    return __hiloint2double(__double2hiint(v) - (int)((n >> 8) << 20), __double2loint(v));
+}
+
 // 1/sqrt(x) for normal positive x: MUFU.RSQ64H seed (~2^-22) and one third-order step
 //   e = 1 - x y^2,  y <- y + y e (1/2 + 3/8 e)        (error ~ 0.3 e^3 < 2^-60 before rounding)
 __device__ __forceinline__ double pb_rsqrt(double x)

@@ -58,7 +58,8 @@ struct pb_tree {
     // per-matvec source records, 64 B per Gauss point: srec[2s] = (y_x, y_y, y_z, w A dphi),
     // srec[2s+1] = (w A phi n_x, w A phi n_y, w A phi n_z, 0)   (written by k_weights)
     double4* srec = nullptr;
-    pb_expk ek;                   // constants of exp(-kappa r) for this kappa
+    pb_expk ek;                   // constants of exp(-kappa r) for this kappa (M2P)
+    pb_expk8 ek8;                 // ... with the 256-entry table (P2P)
     double* xphi = nullptr;       // [N] phi in Morton order
     double* xdphi = nullptr;      // [N]
     // cells
@@ -264,6 +265,7 @@ int pb_upward(pb_ctx* ctx, cudaStream_t fs, const int32_t* leaf_ids, int64_t n_l
 int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed, bool precond);
 int pb_weights(pb_ctx* ctx, const double* x, bool precond);
 void pb_make_expk(double kappa, pb_expk* out);
+int pb_make_expk8(pb_ctx* ctx, double kappa, pb_expk8* out);
 // pb_sites.cu
 int pb_site_near_build(pb_ctx* ctx);
 int pb_multipole_field_impl(pb_ctx* ctx, const double* mu, int parts, int use_mask, double* phi, double* grad, double* hess);

@@ -204,6 +204,26 @@ int pb_weights(pb_ctx* ctx, const double* x, bool precond)
     return PB_OK;
 }
 
+// constants of pb_exp_mkr8 (pb_device.cuh); the table 2^(-j/256) does not depend on kappa and is uploaded once
+__constant__ double c_T256[256];
+
+int pb_make_expk8(pb_ctx* ctx, double kappa, pb_expk8* k)
+{
+    const double ln2 = 0.693147180559945309417232121458;
+    k->c1 = 256.0 * kappa / ln2;
+    k->Lk = kappa > 0.0 ? ln2 / (256.0 * kappa) : 0.0;
+    double f = 1.0;
+    for (int m = 0; m <= 4; ++m) {
+        k->c[m] = f;
+        f *= -kappa / (double)(m + 1);
+    }
+    double T[256];                                  // constant memory is per device: upload at every tree build
+    for (int j = 0; j < 256; ++j) T[j] = exp2(-(double)j / 256.0);
+    PB_CUDA(cudaMemcpyToSymbolAsync(c_T256, T, sizeof(T), 0, cudaMemcpyHostToDevice, ctx->stream));
+    PB_CUDA(cudaStreamSynchronize(ctx->stream));
+    return PB_OK;
+}
+
 // constants of pb_exp_mkr (pb_device.cuh)
 void pb_make_expk(double kappa, pb_expk* k)
 {
@@ -782,7 +802,7 @@ static_assert(P2P_S == 4, "the final reduction maps one of the 4 outputs to each
 
 template <bool CHECK_SELF>
 __device__ __forceinline__ void p2p_tile(const double4* __restrict__ buf, int cnt, int sub, int32_t s0, int32_t selfLo,
-                                         int K, double kappa, const pb_expk& ek, const double* __restrict__ Ts,
+                                         int K, double kappa, const pb_expk8& ek, const double* __restrict__ Ts,
                                          double tx, double ty, double tz, double& VL, double& KL, double& VY,
                                          double& KY)
 {
@@ -795,7 +815,7 @@ __device__ __forceinline__ void p2p_tile(const double4* __restrict__ buf, int cn
         const double nd = fma(b.z, dz, fma(b.y, dy, b.x * dx));
         const double ri = pb_rsqrt(r2);
         const double r = r2 * ri, ri2 = ri * ri;
-        const double ex = pb_exp_mkr(r, ek, Ts);
+        const double ex = pb_exp_mkr8(r, ek, Ts);
         const double qr = a.w * ri;
         const double kl = nd * (ri2 * ri);
         VL += qr;
@@ -806,20 +826,21 @@ __device__ __forceinline__ void p2p_tile(const double4* __restrict__ buf, int cn
 }
 
 __global__ void __launch_bounds__(P2P_THREADS)
-k_p2p(int64_t N, int K, double kappa, pb_expk ek, const pb_item* __restrict__ items,
+k_p2p(int64_t N, int K, double kappa, pb_expk8 ek, const pb_item* __restrict__ items,
       const int32_t* __restrict__ p2p_lo, const int32_t* __restrict__ p2p_hi, const double4* __restrict__ srec,
       const double* __restrict__ px, const double* __restrict__ py, const double* __restrict__ pz,
       double* __restrict__ acc)
 {
     __shared__ __align__(128) double4 tile[2][2 * P2P_TILE];
     __shared__ __align__(8) uint64_t bar[2];
-    __shared__ double Ts[32];
+    __shared__ double Ts[256];
     const int tid = threadIdx.x;
     const int tgt = tid & (PB_TG - 1), sub = tid / PB_TG;
     const pb_item item = items[blockIdx.x];
     const int64_t g = item.group;
     const int slice = item.slot;
-    if (tid < 32) Ts[tid] = ek.T[tid];
+    static_assert(P2P_THREADS == 256, "one table entry per thread");
+    Ts[tid] = c_T256[tid];
     if (tid == 0) {
         pb_mbar_init(&bar[0], 1);
         pb_mbar_init(&bar[1], 1);
@@ -1116,7 +1137,7 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed, bool pre
     }
     {
         PB_TRY(pb_prof_begin(ctx, 0));
-        k_p2p<<<(unsigned)t.n_itemP, P2P_THREADS, 0, st>>>(t.N, t.K, ctx->prm.kappa, t.ek, t.itemP, t.p2p_lo, t.p2p_hi, t.srec,
+        k_p2p<<<(unsigned)t.n_itemP, P2P_THREADS, 0, st>>>(t.N, t.K, ctx->prm.kappa, t.ek8, t.itemP, t.p2p_lo, t.p2p_hi, t.srec,
                                                          t.pc[0], t.pc[1], t.pc[2], t.accP);
         PB_LAUNCH_CHECK();
         PB_TRY(pb_prof_end(ctx, 0));

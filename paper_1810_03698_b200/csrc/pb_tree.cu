@@ -526,6 +526,7 @@ int pb_tree_build_impl(pb_ctx* ctx)
     t.K = K;
     t.Ns = N * K;
     pb_make_expk(ctx->prm.kappa, &t.ek);
+    PB_TRY(pb_make_expk8(ctx, ctx->prm.kappa, &t.ek8));
     const int64_t Ns = t.Ns;
 
     // --- Morton keys and sort
