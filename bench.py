@@ -43,9 +43,19 @@ P2P_FLOP_PER_PAIR = 80.0
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # SMs x FP64 FMA lanes x 2 x max SM clock
 
 
-def m2p_flop_per_pair(P, n_terms):
+def n_terms_of(P):
+    return sum((P - a - b - c) // 2 + 1 for a in range(P + 1) for b in range(P + 1 - a) for c in range(P + 1 - a - b))
+
+
+def m2p_flop_per_pair(P, n_terms=None):
     nk = (P + 1) * (P + 2) * (P + 3) // 6
-    return 4.0 * n_terms + nk + 6.0 * P + 30.0
+    return 4.0 * (n_terms if n_terms is not None else n_terms_of(P)) + nk + 6.0 * P + 30.0
+
+
+def m2p_flop(P, st):
+    """Algorithmic flop of one M2P launch: pairs at order P plus the pairs the list build flagged for order P - 2."""
+    low = st.get("m2p_pairs_low", 0)
+    return m2p_flop_per_pair(P, st["n_terms"]) * (st["m2p_pairs"] - low) + (m2p_flop_per_pair(P - 2) * low if low else 0.0)
 
 
 class ClockSampler(threading.Thread):
@@ -292,7 +302,7 @@ def run_ours(args):
     p2p_ms = stp["prof_p2p_ms"] / max(stp["prof_p2p_launches"], 1)
     m2p_ms = stp["prof_m2p_ms"] / max(stp["prof_m2p_launches"], 1)
     p2p_tf = P2P_FLOP_PER_PAIR * st1["p2p_pairs"] / (p2p_ms * 1e-3) / 1e12 if p2p_ms > 0 else 0.0
-    m2p_tf = (m2p_flop_per_pair(P, st1["n_terms"]) * st1["m2p_pairs"] / (m2p_ms * 1e-3) / 1e12) if m2p_ms > 0 else 0.0
+    m2p_tf = (m2p_flop(P, st1) / (m2p_ms * 1e-3) / 1e12) if m2p_ms > 0 else 0.0
     dominant = "k_p2p" if stp["prof_p2p_ms"] >= stp["prof_m2p_ms"] else "k_m2p"
     ach = p2p_tf if dominant == "k_p2p" else m2p_tf
     # DRAM bytes per launch of the dominant kernel from the committed ncu --set full captures (per workload)
@@ -326,6 +336,7 @@ def run_ours(args):
                   "scf_iters": res["scf_iters"], "gmres_iters": res["gmres_iters_total"], "matvecs": res["matvecs_total"],
                   "interactions_per_matvec": int(inter_per_mv), "status": res["status"]},
         "evaluated": {"p2p_pairs_per_matvec": int(st1["p2p_pairs"]), "m2p_pairs_per_matvec": int(st1["m2p_pairs"]),
+                      "m2p_pairs_at_order_P_minus_2": int(st1["m2p_pairs_low"]),
                       "pairs_per_s": float(evald_per_mv) * mv_timed / (ms_total * 1e-3) * (world if world > 1 else 1)},
         "e2e": {"value": value_e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                 "ms_per_step": ms_e2e / args.steps},
@@ -396,7 +407,8 @@ def run_sweep(args):
                 "p2p_pairs": int(st["p2p_pairs"]), "m2p_pairs": int(st["m2p_pairs"]),
                 "serial_ms": {k: lm[k] for k in ("weights", "p2m_m2m", "m2p", "p2p", "near_combine")},
                 "p2p_tflops": P2P_FLOP_PER_PAIR * st["p2p_pairs"] / (lm["p2p"] * 1e-3) / 1e12,
-                "m2p_tflops": fl_m * st["m2p_pairs"] / (lm["m2p"] * 1e-3) / 1e12 if lm["m2p"] > 0 else 0.0,
+                "m2p_pairs_low_order": int(st["m2p_pairs_low"]),
+                "m2p_tflops": m2p_flop(P, st) / (lm["m2p"] * 1e-3) / 1e12 if lm["m2p"] > 0 else 0.0,
                 "fp64_peak_tflops": FP64_PEAK_TFLOPS, "rel_l2_vs_oracle_rows": err, "device_gb": st["device_bytes"] / 1e9}), flush=True)
     ctx.set_params(**{k: v for k, v in w.params.items() if k in ("theta", "order_P")})
     ctx.tree_build()

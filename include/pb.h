@@ -115,6 +115,7 @@ typedef struct pb_stats {
                                    0 weights, 1 P2M+M2M+convert, 2 M2P, 3 P2P, 4 near table +
                                    combine, 5 total                                            */
     int64_t ncrit_used;         /* leaf capacity the tree was built with (see pb_params.ncrit)  */
+    int64_t m2p_pairs_low;      /* of m2p_pairs: those evaluated at order P - 2 (cells far inside the MAC) */
 } pb_stats;
 
 typedef void* (*pb_alloc_fn)(void* user, size_t bytes);     /* returns a 256-byte aligned device pointer or NULL */

@@ -346,6 +346,7 @@ extern "C" int pb_get_stats(pb_ctx* ctx, pb_stats* out)
     out->prof_m2p_ms = ctx->prof_ms[1];
     for (int i = 0; i < 8; ++i) out->last_matvec_ms[i] = ctx->last_ms[i];
     out->ncrit_used = t.ncrit_used;
+    out->m2p_pairs_low = t.m2p_pairs_low;
     return PB_OK;
 }
 

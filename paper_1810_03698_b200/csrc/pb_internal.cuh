@@ -83,7 +83,7 @@ struct pb_tree {
     int32_t* p2p_off = nullptr;   // [groups+1]
     int32_t* p2p_lo = nullptr;    // source-point ranges [lo, hi)
     int32_t* p2p_hi = nullptr;
-    int64_t p2p_pairs = 0, m2p_pairs = 0;
+    int64_t p2p_pairs = 0, m2p_pairs = 0, m2p_pairs_low = 0;   // m2p_pairs_low: those evaluated at order P - 2
     // far-field data
     int P = 0, Nk = 0, NT = 0;
     double* M = nullptr;          // [cells][2][Nk] Cartesian moments (V, K)

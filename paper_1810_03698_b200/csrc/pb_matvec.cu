@@ -622,7 +622,9 @@ template <int P> struct m2q_cfg {
     static constexpr size_t SMEM = FF_BYTES + M2Q_NS * M2Q_CT * sizeof(double4) + 2 * M2Q_NS * sizeof(uint64_t) + 32 * sizeof(double);
 };
 
-template <int P>
+// PL <= P: evaluate only the terms of the order-PL sum (|alpha| + 2j <= PL); they are a subset of the order-P terms
+// with the same values F_{alpha,j}, so the same staged array serves both (the skipped entries are never read).
+template <int P, int PL>
 __device__ __forceinline__ void m2p_terms2(const double2* __restrict__ ff, double dx0, double dy0, double dz0, double dx1,
                                            double dy1, double dz1, double (&WV0)[P + 1], double (&WK0)[P + 1],
                                            double (&WV1)[P + 1], double (&WK1)[P + 1])
@@ -640,23 +642,25 @@ __device__ __forceinline__ void m2p_terms2(const double2* __restrict__ ff, doubl
                 const int n = a + b + c;
 #pragma unroll
                 for (int j = 0; j <= (P - n) / 2; ++j) {
-                    const double2 f = ff[e];
+                    if (n + 2 * j <= PL) {
+                        const double2 f = ff[e];
+                        WV0[n + j] = fma(m0, f.x, WV0[n + j]);
+                        WK0[n + j] = fma(m0, f.y, WK0[n + j]);
+                        WV1[n + j] = fma(m1, f.x, WV1[n + j]);
+                        WK1[n + j] = fma(m1, f.y, WK1[n + j]);
+                    }
                     ++e;
-                    WV0[n + j] = fma(m0, f.x, WV0[n + j]);
-                    WK0[n + j] = fma(m0, f.y, WK0[n + j]);
-                    WV1[n + j] = fma(m1, f.x, WV1[n + j]);
-                    WK1[n + j] = fma(m1, f.y, WK1[n + j]);
                 }
-                m0 *= dz0; m1 *= dz1;
+                if (n < PL) { m0 *= dz0; m1 *= dz1; }
             }
-            xy0 *= dy0; xy1 *= dy1;
+            if (a + b < PL) { xy0 *= dy0; xy1 *= dy1; }
         }
-        xa0 *= dx0; xa1 *= dx1;
+        if (a < PL) { xa0 *= dx0; xa1 *= dx1; }
     }
 }
 
 // radial part: u_m(R) of both kernels against the (P+1) partial sums per layer (D: section 6)
-template <int P>
+template <int P, int PL>
 __device__ __forceinline__ void m2p_radial(double dx, double dy, double dz, const double (&WV)[P + 1], const double (&WK)[P + 1],
                                            double kappa, double k2, const pb_expk& ek, const double* __restrict__ Ts,
                                            double& VL, double& KL, double& VY, double& KY)
@@ -668,7 +672,7 @@ __device__ __forceinline__ void m2p_radial(double dx, double dy, double dz, cons
     VL = fma(uL, WV[0], VL); KL = fma(uL, WK[0], KL);
     VY = fma(uY0, WV[0], VY); KY = fma(uY0, WK[0], KY);
 #pragma unroll
-    for (int m = 1; m <= P; ++m) {
+    for (int m = 1; m <= PL; ++m) {                    // p + j <= p + 2j <= PL: partial sums beyond PL are empty
         uL = (2 * m - 1) * uL * ri2;
         VL = fma(uL, WV[m], VL); KL = fma(uL, WK[m], KL);
         VY = fma(uY1, WV[m], VY); KY = fma(uY1, WK[m], KY);
@@ -760,9 +764,16 @@ k_m2p2(int64_t N, double kappa, pb_expk ek, const pb_item* __restrict__ items, c
             double WV0[P + 1], WK0[P + 1], WV1[P + 1], WK1[P + 1];
 #pragma unroll
             for (int m = 0; m <= P; ++m) { WV0[m] = 0.0; WK0[m] = 0.0; WV1[m] = 0.0; WK1[m] = 0.0; }
-            m2p_terms2<P>(ff + ((size_t)st * CT + j) * NT, dx0, dy0, dz0, dx1, dy1, dz1, WV0, WK0, WV1, WK1);
-            m2p_radial<P>(dx0, dy0, dz0, WV0, WK0, kappa, k2, ek, Ts, VL0, KL0, VY0, KY0);
-            m2p_radial<P>(dx1, dy1, dz1, WV1, WK1, kappa, k2, ek, Ts, VL1, KL1, VY1, KY1);
+            constexpr int PL = P >= 4 ? P - 2 : P;
+            if (PL < P && cc.w != 0.0) {              // flagged by the list build: order P - 2 is enough (warp-uniform)
+                m2p_terms2<P, PL>(ff + ((size_t)st * CT + j) * NT, dx0, dy0, dz0, dx1, dy1, dz1, WV0, WK0, WV1, WK1);
+                m2p_radial<P, PL>(dx0, dy0, dz0, WV0, WK0, kappa, k2, ek, Ts, VL0, KL0, VY0, KY0);
+                m2p_radial<P, PL>(dx1, dy1, dz1, WV1, WK1, kappa, k2, ek, Ts, VL1, KL1, VY1, KY1);
+            } else {
+                m2p_terms2<P, P>(ff + ((size_t)st * CT + j) * NT, dx0, dy0, dz0, dx1, dy1, dz1, WV0, WK0, WV1, WK1);
+                m2p_radial<P, P>(dx0, dy0, dz0, WV0, WK0, kappa, k2, ek, Ts, VL0, KL0, VY0, KY0);
+                m2p_radial<P, P>(dx1, dy1, dz1, WV1, WK1, kappa, k2, ek, Ts, VL1, KL1, VY1, KY1);
+            }
         }
         __syncwarp();
         if (lane == 0) pb_mbar_arrive(&empty[st]);

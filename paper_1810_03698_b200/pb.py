@@ -76,7 +76,7 @@ class Stats(ctypes.Structure):
         ("prof_p2p_launches", ctypes.c_int64), ("prof_m2p_launches", ctypes.c_int64),
         ("prof_p2p_ms", ctypes.c_double), ("prof_m2p_ms", ctypes.c_double),
         ("last_matvec_ms", ctypes.c_double * 8),
-        ("ncrit_used", ctypes.c_int64),
+        ("ncrit_used", ctypes.c_int64), ("m2p_pairs_low", ctypes.c_int64),
     ]
 
     def as_dict(self):
