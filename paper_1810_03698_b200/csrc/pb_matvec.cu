@@ -811,6 +811,43 @@ k_m2p2(int64_t N, double kappa, pb_expk ek, const pb_item* __restrict__ items, c
 #define P2P_TILE 256
 static_assert(P2P_S == 4, "the final reduction maps one of the 4 outputs to each sub-slice");
 
+__device__ __forceinline__ void p2p_pair(const double4& a, const double4& b, double tx, double ty, double tz, double kappa,
+                                         const pb_expk8& ek, const double* __restrict__ Ts, double& VL, double& KL,
+                                         double& VY, double& KY)
+{
+    const double dx = tx - a.x, dy = ty - a.y, dz = tz - a.z;
+    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    const double nd = fma(b.z, dz, fma(b.y, dy, b.x * dx));
+    const double ri = pb_rsqrt(r2);
+    const double r = r2 * ri, ri2 = ri * ri;
+    const double ex = pb_exp_mkr8(r, ek, Ts);
+    const double qr = a.w * ri;
+    const double kl = nd * (ri2 * ri);
+    VL += qr;
+    KL += kl;
+    VY = fma(qr, ex, VY);
+    KY = fma(kl * ex, fma(kappa, r, 1.0), KY);
+}
+
+// Two targets per lane (lane and lane + 32 of the group): every source record read from shared memory feeds two pairs,
+// and the loop / address arithmetic is shared; the block's eight warps take interleaved sources of a tile.
+#define P2Q_W 8
+template <bool CHECK_SELF>
+__device__ __forceinline__ void p2p_tile2(const double4* __restrict__ buf, int cnt, int sub, int32_t s0, int32_t self0,
+                                          int32_t self1, int K, double kappa, const pb_expk8& ek,
+                                          const double* __restrict__ Ts, const double (&t0)[3], const double (&t1)[3],
+                                          double (&o0)[4], double (&o1)[4])
+{
+#pragma unroll 2
+    for (int k = sub; k < cnt; k += P2Q_W) {
+        const double4 a = buf[2 * k], b = buf[2 * k + 1];
+        if (!CHECK_SELF || (unsigned)(s0 + k - self0) >= (unsigned)K)          // own panel: by index (D: R-11)
+            p2p_pair(a, b, t0[0], t0[1], t0[2], kappa, ek, Ts, o0[0], o0[1], o0[2], o0[3]);
+        if (!CHECK_SELF || (unsigned)(s0 + k - self1) >= (unsigned)K)
+            p2p_pair(a, b, t1[0], t1[1], t1[2], kappa, ek, Ts, o1[0], o1[1], o1[2], o1[3]);
+    }
+}
+
 template <bool CHECK_SELF>
 __device__ __forceinline__ void p2p_tile(const double4* __restrict__ buf, int cnt, int sub, int32_t s0, int32_t selfLo,
                                          int K, double kappa, const pb_expk8& ek, const double* __restrict__ Ts,
@@ -919,6 +956,94 @@ k_p2p(int64_t N, int K, double kappa, pb_expk8 ek, const pb_item* __restrict__ i
         double v = 0;
 #pragma unroll
         for (int q = 0; q < P2P_S; ++q) v += red[(q * 4 + m) * PB_TG + tgt];
+        if (i < N) acc[((int64_t)slice * 4 + m) * N + i] = v;
+    }
+}
+
+__global__ void __launch_bounds__(P2P_THREADS, 2)
+k_p2p2(int64_t N, int K, double kappa, pb_expk8 ek, const pb_item* __restrict__ items,
+       const int32_t* __restrict__ p2p_lo, const int32_t* __restrict__ p2p_hi, const double4* __restrict__ srec,
+       const double* __restrict__ px, const double* __restrict__ py, const double* __restrict__ pz,
+       double* __restrict__ acc)
+{
+    __shared__ __align__(128) double4 tile[2][2 * P2P_TILE];
+    __shared__ __align__(8) uint64_t bar[2];
+    __shared__ double Ts[256];
+    static_assert(PB_TG == 64 && P2P_THREADS == 32 * P2Q_W, "two targets per lane, eight warps");
+    const int tid = threadIdx.x;
+    const int lane = tid & 31, sub = tid >> 5;
+    const pb_item item = items[blockIdx.x];
+    const int64_t g = item.group;
+    const int slice = item.slot;
+    Ts[tid] = c_T256[tid];
+    if (tid == 0) {
+        pb_mbar_init(&bar[0], 1);
+        pb_mbar_init(&bar[1], 1);
+        pb_mbar_fence_init();
+    }
+    __syncthreads();
+    const int64_t ia = g * PB_TG + lane, ib = ia + 32;
+    const int64_t ica = ia < N ? ia : N - 1, icb = ib < N ? ib : N - 1;   // padding lanes repeat the last target; never stored
+    const double t0[3] = {px[ica], py[ica], pz[ica]}, t1[3] = {px[icb], py[icb], pz[icb]};
+    const int32_t self0 = (int32_t)(ica * K), self1 = (int32_t)(icb * K);
+    const int64_t i1 = (g + 1) * PB_TG < N ? (g + 1) * PB_TG : N;
+    const int32_t grpLo = (int32_t)(g * PB_TG * K), grpHi = (int32_t)(i1 * K);
+
+    int32_t r = item.r, a = item.a;
+    int32_t hi = p2p_hi[r];
+    int64_t remaining = item.count;
+    auto next_tile = [&](int32_t& s0, int& cnt) -> bool {
+        while (remaining > 0) {
+            if (a >= hi) { ++r; a = p2p_lo[r]; hi = p2p_hi[r]; continue; }
+            int64_t c = hi - a;
+            if (c > P2P_TILE) c = P2P_TILE;
+            if (c > remaining) c = remaining;
+            s0 = a; cnt = (int)c;
+            a += (int32_t)c; remaining -= c;
+            return true;
+        }
+        return false;
+    };
+
+    double o0[4] = {0, 0, 0, 0}, o1[4] = {0, 0, 0, 0};
+    int32_t cs0 = 0, ns0 = 0;
+    int ccnt = 0, ncnt = 0;
+    bool have = next_tile(cs0, ccnt);
+    if (have && tid == 0) {
+        pb_mbar_expect_tx(&bar[0], (uint32_t)ccnt * 64u);
+        pb_bulk_g2s(tile[0], srec + 2 * (int64_t)cs0, (uint32_t)ccnt * 64u, &bar[0]);
+    }
+    for (uint32_t it = 0; have; ++it) {
+        const int st = it & 1;
+        const bool more = next_tile(ns0, ncnt);
+        if (more && tid == 0) {                       // the other buffer was released by the barrier below
+            pb_mbar_expect_tx(&bar[st ^ 1], (uint32_t)ncnt * 64u);
+            pb_bulk_g2s(tile[st ^ 1], srec + 2 * (int64_t)ns0, (uint32_t)ncnt * 64u, &bar[st ^ 1]);
+        }
+        pb_mbar_wait(&bar[st], (it >> 1) & 1u);
+        if (cs0 < grpHi && cs0 + ccnt > grpLo)
+            p2p_tile2<true>(tile[st], ccnt, sub, cs0, self0, self1, K, kappa, ek, Ts, t0, t1, o0, o1);
+        else
+            p2p_tile2<false>(tile[st], ccnt, sub, cs0, self0, self1, K, kappa, ek, Ts, t0, t1, o0, o1);
+        __syncthreads();
+        have = more;
+        cs0 = ns0;
+        ccnt = ncnt;
+    }
+    // add the warps' partial sums in a fixed order (tile[0] is free: every thread passed the last barrier)
+    double* red = reinterpret_cast<double*>(tile[0]);   // [P2Q_W][4][PB_TG] = 16 KB = tile[0]
+#pragma unroll
+    for (int m = 0; m < 4; ++m) {
+        red[(sub * 4 + m) * PB_TG + lane] = o0[m];
+        red[(sub * 4 + m) * PB_TG + lane + 32] = o1[m];
+    }
+    __syncthreads();
+    {
+        const int m = tid / PB_TG, tgt = tid & (PB_TG - 1);
+        const int64_t i = g * PB_TG + tgt;
+        double v = 0;
+#pragma unroll
+        for (int q = 0; q < P2Q_W; ++q) v += red[(q * 4 + m) * PB_TG + tgt];
         if (i < N) acc[((int64_t)slice * 4 + m) * N + i] = v;
     }
 }
@@ -1148,8 +1273,14 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed, bool pre
     }
     {
         PB_TRY(pb_prof_begin(ctx, 0));
-        k_p2p<<<(unsigned)t.n_itemP, P2P_THREADS, 0, st>>>(t.N, t.K, ctx->prm.kappa, t.ek8, t.itemP, t.p2p_lo, t.p2p_hi, t.srec,
-                                                         t.pc[0], t.pc[1], t.pc[2], t.accP);
+        // two targets per lane pays once the kernel is throughput-bound (measured: C3 529 -> 516 us, C4 8.43 -> 8.24 ms;
+        // C1 / C2, a few waves of short blocks, are 2-4 % faster with one target per thread and twice the resident warps)
+        if (t.N >= 30000)
+            k_p2p2<<<(unsigned)t.n_itemP, P2P_THREADS, 0, st>>>(t.N, t.K, ctx->prm.kappa, t.ek8, t.itemP, t.p2p_lo, t.p2p_hi,
+                                                              t.srec, t.pc[0], t.pc[1], t.pc[2], t.accP);
+        else
+            k_p2p<<<(unsigned)t.n_itemP, P2P_THREADS, 0, st>>>(t.N, t.K, ctx->prm.kappa, t.ek8, t.itemP, t.p2p_lo, t.p2p_hi,
+                                                             t.srec, t.pc[0], t.pc[1], t.pc[2], t.accP);
         PB_LAUNCH_CHECK();
         PB_TRY(pb_prof_end(ctx, 0));
         pb_prof_next(ctx);
