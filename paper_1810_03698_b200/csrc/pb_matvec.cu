@@ -248,7 +248,7 @@ void pb_make_expk(double kappa, pb_expk* k)
 // parent's M2M, and so on upward -- nobody waits, and a parent is always formed from all its children
 // in child order, so the result does not depend on the arrival order.  A cell that appears in an M2P
 // list has its far-field terms F (D: section 6) written by the block that finishes it.
-#define P2M_CH 32
+#define P2M_CH 96     // <= UP_THREADS; 3 * 96 * 11 doubles of powers still fit under the M2M scratch at P = 6
 #define P2M_LD (PB_MAX_P + 1)     // 11 doubles per point: odd stride, so a warp's reads of one point do not conflict
 #define UP_THREADS 128
 
@@ -303,20 +303,26 @@ __global__ void __launch_bounds__(UP_THREADS) k_upward(up_args a)
         for (int r = 0; r < 3; ++r)
 #pragma unroll
             for (int m = 0; m < 4; ++m) acc[r][m] = 0.0;
+        // thread p stages point p of a chunk (powers of its three coordinates, its four weights); the records of the
+        // next chunk are already in flight while this one is accumulated
+        double4 ra = make_double4(0, 0, 0, 0), rb = ra;
+        if (tid < P2M_CH && s0 + tid < s1) { ra = a.srec[2 * (s0 + tid)]; rb = a.srec[2 * (s0 + tid) + 1]; }
         for (int64_t base = s0; base < s1; base += P2M_CH) {
             const int np = (int)((s1 - base) < P2M_CH ? (s1 - base) : P2M_CH);
             __syncthreads();
-            if (tid < 3 * np) {                                // thread (point, axis): powers of one coordinate
-                const int pt = tid / 3, d = tid - 3 * pt;
-                const double4 ra = a.srec[2 * (base + pt)];
-                const double hh = d == 0 ? ra.x - ycx : (d == 1 ? ra.y - ycy : ra.z - ycz);
-                double pwr = 1.0;
-                double* dst = pw + ((size_t)d * P2M_CH + pt) * P2M_LD;
-                for (int e = 0; e <= P; ++e) { dst[e] = pwr; pwr *= hh; }
-                if (d == 0) {
-                    const double4 rb = a.srec[2 * (base + pt) + 1];
-                    wq[pt] = make_double4(ra.w, rb.x, rb.y, rb.z);
+            if (tid < np) {
+                const double hh[3] = {ra.x - ycx, ra.y - ycy, ra.z - ycz};
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+                    double pwr = 1.0;
+                    double* dst = pw + ((size_t)d * P2M_CH + tid) * P2M_LD;
+                    for (int e = 0; e <= P; ++e) { dst[e] = pwr; pwr *= hh[d]; }
                 }
+                wq[tid] = make_double4(ra.w, rb.x, rb.y, rb.z);
+            }
+            if (tid < P2M_CH && base + P2M_CH + tid < s1) {
+                ra = a.srec[2 * (base + P2M_CH + tid)];
+                rb = a.srec[2 * (base + P2M_CH + tid) + 1];
             }
             __syncthreads();
 #pragma unroll

@@ -466,15 +466,6 @@ static int dot_into(pb_ctx* ctx, gmres_ws& ws, int nv, const double* V, const do
     return PB_OK;
 }
 
-// ||v||^2 on the host (synchronises)
-static int norm2_host(pb_ctx* ctx, gmres_ws& ws, const double* v, double* out)
-{
-    PB_TRY(dot_into(ctx, ws, 0, nullptr, v, true, ws.hdev));
-    PB_CUDA(cudaMemcpyAsync(out, ws.hdev, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
-    PB_CUDA(cudaStreamSynchronize(ctx->stream));
-    return PB_OK;
-}
-
 // Restarted GMRES with a right block-Jacobi preconditioner (D: R-20).  Per iteration: one operator
 // application (the preconditioner is folded into its first kernel), two classical Gram-Schmidt
 // passes of two kernels each -- the second also yields the norm of the new vector by Pythagoras and
@@ -527,25 +518,20 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
     bool have_ax = x_is_last_result && ws.ax_valid;
     ws.ax_valid = false;
     const int hstride = m + 4;
-    PB_TRY(pb_pinned(ctx, (3 * (size_t)m + 64) * sizeof(double)));
-    double* hh = ctx->h_pinned;                    // staging for h columns
+    PB_TRY(pb_pinned(ctx, (5 * (size_t)m + 64) * sizeof(double)));
+    double* hh = ctx->h_pinned;                    // staging for h columns [2][hstride]
+    double* hy = hh + 2 * hstride;                 // staging for y (x += Z y) and for Hbar y (A x += V Hbar y): written at the end
+    double* hc = hy + m;                           // of a cycle only, and every cycle starts with a stream synchronisation
     const bool pc = mode == 1;
     const double tol = ctx->prm.gmres_tol;
     const int maxit = ctx->prm.gmres_maxit;
     int iters = 0, matvecs = 0;
     int rc = PB_OK;
 
-    double bn2 = 0;
-    PB_TRY(norm2_host(ctx, ws, b, &bn2));
-    const double bnorm = sqrt(bn2);
+    // ||b||^2 is read back together with the first residual norm (one synchronisation fewer per solve)
+    PB_TRY(dot_into(ctx, ws, 0, nullptr, b, true, ws.hdev + 2 * hstride));
+    double bnorm = -1.0;
     double relres = 0.0;
-    if (bnorm == 0.0) {
-        PB_CUDA(cudaMemsetAsync(x, 0, sizeof(double) * n, st));
-        if (iters_out) *iters_out = 0;
-        if (relres_out) *relres_out = 0.0;
-        if (matvecs_out) *matvecs_out = 0;
-        return PB_OK;
-    }
     std::vector<double> H((size_t)(m + 1) * m, 0.0), Hraw((size_t)(m + 1) * m, 0.0), cs(m, 0.0), sn(m, 0.0), g(m + 1, 0.0),
         yv(m, 0.0);
 
@@ -572,9 +558,20 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
         PB_TRY(dot_into(ctx, ws, 0, nullptr, ws.r, true, ws.hdev));
         k_normalize<<<nb, tb, 0, st>>>(n, ws.hdev, ws.r, ws.V);      // V_0 = r/||r||
         PB_LAUNCH_CHECK();
-        double r2 = 0;
+        double r2 = 0, bn2 = 0;
         PB_CUDA(cudaMemcpyAsync(&r2, ws.hdev, sizeof(double), cudaMemcpyDeviceToHost, st));
+        if (bnorm < 0) PB_CUDA(cudaMemcpyAsync(&bn2, ws.hdev + 2 * hstride, sizeof(double), cudaMemcpyDeviceToHost, st));
         PB_CUDA(cudaStreamSynchronize(st));
+        if (bnorm < 0) {
+            bnorm = sqrt(bn2);
+            if (bnorm == 0.0) {
+                PB_CUDA(cudaMemsetAsync(x, 0, sizeof(double) * n, st));
+                if (iters_out) *iters_out = 0;
+                if (relres_out) *relres_out = 0.0;
+                if (matvecs_out) *matvecs_out = matvecs;
+                return PB_OK;
+            }
+        }
         const double beta = sqrt(r2);
         relres = beta / bnorm;
         if (relres <= tol) { ws.ax_valid = true; break; }      // ws.ax = A x for the x we return
@@ -658,8 +655,8 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
             for (int k = i + 1; k < j; ++k) s -= H[(size_t)k * (m + 1) + i] * yv[k];
             yv[i] = s / H[(size_t)i * (m + 1) + i];
         }
-        for (int i = 0; i < j; ++i) hh[i] = yv[i];
-        PB_CUDA(cudaMemcpyAsync(ws.coef, hh, sizeof(double) * j, cudaMemcpyHostToDevice, st));
+        for (int i = 0; i < j; ++i) hy[i] = yv[i];
+        PB_CUDA(cudaMemcpyAsync(ws.coef, hy, sizeof(double) * j, cudaMemcpyHostToDevice, st));
         k_lincomb<<<pb_blocks(n, tb), tb, j * sizeof(double), st>>>(n, j, mode == 2 ? ws.Z : ws.V, n, ws.coef, ws.u);   // x += Z y (flexible)
         PB_LAUNCH_CHECK();
         if (pc) {
@@ -669,19 +666,17 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
         } else
             k_axpy<<<pb_blocks(n, tb), tb, 0, st>>>(n, 1.0, ws.u, x);
         PB_LAUNCH_CHECK();
-        PB_CUDA(cudaStreamSynchronize(st));   // hh is reused
         // A x += V_{j+1} (Hbar_j y)
         for (int i = 0; i <= j; ++i) {
             double c = 0;
             for (int k = (i > 0 ? i - 1 : 0); k < j; ++k) c += Hraw[(size_t)k * (m + 1) + i] * yv[k];
-            hh[i] = c;
+            hc[i] = c;
         }
-        PB_CUDA(cudaMemcpyAsync(ws.coef, hh, sizeof(double) * (j + 1), cudaMemcpyHostToDevice, st));
+        PB_CUDA(cudaMemcpyAsync(ws.coef, hc, sizeof(double) * (j + 1), cudaMemcpyHostToDevice, st));
         k_lincomb<<<pb_blocks(n, tb), tb, (j + 1) * sizeof(double), st>>>(n, j + 1, ws.V, n, ws.coef, ws.u);
         PB_LAUNCH_CHECK();
         k_axpy<<<pb_blocks(n, tb), tb, 0, st>>>(n, 1.0, ws.u, ws.ax);
         PB_LAUNCH_CHECK();
-        PB_CUDA(cudaStreamSynchronize(st));
         ws.ax_valid = accepted;
         // Converged by the Arnoldi residual |g_j|: with a RIGHT preconditioner and CGS2-orthogonal V this is the true
         // residual norm to rounding, so no further operator application is spent on confirming it.  After a
@@ -699,7 +694,9 @@ extern "C" int pb_gmres(pb_ctx* ctx, const double* b, double* x, int32_t* iters,
 {
     if (!ctx) return PB_ERR_INVALID_ARG;
     if (!b || !x) return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_gmres: NULL vector");
-    return pb_gmres_impl(ctx, b, x, iters, relres, nullptr, false);
+    PB_TRY(pb_gmres_impl(ctx, b, x, iters, relres, nullptr, false));
+    PB_CUDA(cudaStreamSynchronize(ctx->stream));   // the last updates of x are still in flight when the loop returns
+    return PB_OK;
 }
 
 // ---- SCF and energy kernels ------------------------------------------------------------------------
