@@ -289,6 +289,7 @@ __global__ void __launch_bounds__(UP_THREADS) k_upward(up_args a)
     __shared__ int s_last;
 
     int64_t c = a.leaf_ids[blockIdx.x];
+    int32_t link = a.up_link[c];                               // in flight during the P2M (one L2 round trip off the chain)
     {   // ---- P2M: thread k (and k + 128, k + 256 at high order) sweeps the leaf's points
         const int64_t s0 = (int64_t)a.c_first[c] * a.K, s1 = (int64_t)a.c_last[c] * a.K;
         const double ycx = a.cx[c], ycy = a.cy[c], ycz = a.cz[c];
@@ -362,7 +363,6 @@ __global__ void __launch_bounds__(UP_THREADS) k_upward(up_args a)
     }
     for (;;) {
         // mom holds the finished moments of cell c
-        const int32_t link = a.up_link[c];
         const int64_t parent = (int64_t)(link >> 2) - 1;
         if (link & 2)
             for (int k = tid; k < 2 * Nk; k += UP_THREADS) a.M[c * 2 * Nk + k] = mom[k];
@@ -372,6 +372,7 @@ __global__ void __launch_bounds__(UP_THREADS) k_upward(up_args a)
             for (int e = tid; e < a.NT; e += UP_THREADS) {
                 double v = 0, k = 0;
                 const int q1 = __ldg(a.cv_off + e + 1);
+#pragma unroll 4
                 for (int q = __ldg(a.cv_off + e); q < q1; ++q) {
                     const int l = __ldg(a.cv_idx + q);
                     const double f = __ldg(a.cv_coef + q);
@@ -397,6 +398,7 @@ __global__ void __launch_bounds__(UP_THREADS) k_upward(up_args a)
         c = parent;
         const int32_t ch = a.c_child[c];
         const int nc = a.c_nchild[c];
+        link = a.up_link[c];                                   // the parent's own link word, in flight during its M2M
         for (int k = tid; k < nc * 2 * Nk; k += UP_THREADS) cm[k] = __ldcg(a.M + (int64_t)ch * 2 * Nk + k);   // children are consecutive
         if (tid < 3 * nc) {
             const int q = tid / 3, d = tid - 3 * q;
