@@ -88,7 +88,7 @@ struct pb_tree {
     int P = 0, Nk = 0, NT = 0;
     double* M = nullptr;          // [cells][2][Nk] Cartesian moments (V, K)
     double2* FF = nullptr;        // [cells][NT] converted far-field terms {V, K}
-    int32_t* mm_off = nullptr;    // [Nk+1] M2M table (CSR over k): packed (l | dx<<12 | dy<<16 | dz<<20), binomials
+    int32_t* mm_off = nullptr;    // [Nk+1] M2M table (CSR over k), then [Nk] the terms by falling row length: packed (l | dx<<12 | dy<<16 | dz<<20), binomials
     int32_t* mm_ent = nullptr;
     double* mm_coef = nullptr;
     int64_t m2p_total = 0;        // entries of m2p_cell

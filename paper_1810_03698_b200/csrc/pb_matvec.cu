@@ -12,6 +12,7 @@
 //   u_m = (-2)^m f^(m):  u_0 = G, u_1 = e^{-kR}(1+kR)/R^3, u_{m+1} = ((2m+1) u_m + k^2 u_{m-1})/R^2
 // (k = 0 for the Laplace kernel).  The F (130 numbers per layer at P = 6) are kernel
 // independent, so one pass over them serves V_L, K_L, V_Y and K_Y.
+#include <algorithm>
 #include <math.h>
 #include "pb_internal.cuh"
 
@@ -112,6 +113,13 @@ int pb_farfield_setup(pb_ctx* ctx)
                                  (factorial(lb) * factorial(b - lb)) * factorial(c) / (factorial(lc) * factorial(c - lc)));
                 }
         mo.push_back((int32_t)me.size());
+    }
+    {   // after the Nk + 1 offsets: the terms k ordered by falling row length, so that the rows a warp walks together in
+        // the M2M are about equally long (lexicographic order mixes rows of 1 and of 27 entries)
+        std::vector<int32_t> order(t.Nk);
+        for (int k = 0; k < t.Nk; ++k) order[k] = k;
+        std::stable_sort(order.begin(), order.end(), [&](int32_t x, int32_t y) { return mo[x + 1] - mo[x] > mo[y + 1] - mo[y]; });
+        mo.insert(mo.end(), order.begin(), order.end());
     }
     PB_TRY(pb_dalloc_t(ctx, &t.mm_off, mo.size(), CAT_TREE));
     PB_TRY(pb_dalloc_t(ctx, &t.mm_ent, me.size(), CAT_TREE));
@@ -415,7 +423,7 @@ __global__ void __launch_bounds__(UP_THREADS) k_upward(up_args a)
         }
         __syncthreads();
         for (int it = tid; it < Nk * nc; it += UP_THREADS) {
-            const int q = it / Nk, k = it - q * Nk;
+            const int q = it / Nk, k = __ldg(a.mm_off + Nk + 1 + (it - q * Nk));   // rows by falling length
             const double* tq = tm + q * Nk;
             const double* cq = cm + q * 2 * Nk;
             double s0 = 0, s1 = 0;
