@@ -1,29 +1,31 @@
 #!/usr/bin/env python
-"""bench.py -- one polarizable Poisson-Boltzmann solve per step on seeded synthetic input.
+"""bench.py -- the treecode BEM matvec of Eq. (5) on seeded synthetic input, timed on the
+configuration BASELINE.json's metric belongs to: configs[4] (C4: 20,000 atoms, ~1.04 M panels, K = 7,
+theta = 0.5, P = 6), the largest single-GPU configuration.
 
-A step is one pass of the whole hot path over one workload:
-pb_mesh_load -> pb_sites_load -> pb_tree_build (Morton octree, lists, near/singular table) ->
-pb_solve (vacuum SCF, then {RHS -> GMRES with one treecode matvec per iteration -> reaction
-field -> multipole field -> SOR update} to 1e-7 Debye, then the energies).
+  step     = one pass of the matvec hot path over one vector x resident in HBM:
+             k_weights -> {k_p2p2  ||  k_upward (P2M, M2M, M->F) -> k_m2p2} -> k_combine.
+  value    = interactions evaluated per second over the timed steps, SURVEY section 8(d)'s unit: one P2P
+             interaction = one (target collocation point, source Gauss point) pair producing all four kernels of
+             Eq. (3)-(4); one M2P interaction = one (target, cell) pair producing all four order-P sums.  Both
+             counts come from the stored lists (pb_get_stats) and are reported separately under "evaluated";
+             "direct_equivalent_per_s" = N * N_s / time (the pairs the dense operator accounts for) is a side key.
+  e2e      = the same step through pb_matvec_host: x copied from pinned host memory, y copied back, every step.
+  roofline = both hot kernels, FP64 ALU bound.  Per kernel: (i) algorithmic flop (80 per P2P pair;
+             4 N_T + N_k + 6 P + 30 per M2P pair at the order it is evaluated at) / CUDA-event time / measured
+             DFMA peak, and (ii) executed FP64-pipe instructions (ncu, profiles/r02_counters.csv) / time /
+             (148 SM x 64 lanes x SM clock).  "frac" is (i) for the kernel with the larger share of the step.
+  solve    = one full polarizable solve (vacuum SCF, RHS, flexible GMRES, reaction field, SOR to 1e-7 D, energies),
+             timed once after the matvec steps; "configs" = the solve times of C1, C2 and the C3 binding triple.
+  cpu_baseline = the oracle's direct O(N^2 K) sum on this box's host cores on sampled target rows.
 
-  metric  = treecode matvec interactions per second over the whole step.  One interaction = one
-            (collocation point, source Gauss point) pair of the N x N_s pairs the operator of
-            Eq. (5) accounts for in a matvec, whether it is summed directly (P2P) or through a
-            cell expansion (M2P): value = N * N_s * matvecs / time.  This is the unit the oracle's
-            direct sum is timed in (cpu_baseline, --impl reference), and it does not reward
-            evaluating more pairs than the MAC requires.  The pairs actually evaluated per second
-            (P2P pairs, M2P (target, cell) pairs) are reported beside it under "evaluated".
-  ms_per_step = time per polarizable PB solve (the second half of BASELINE.json's metric)
-  e2e     = the same through the host-buffer C-ABI calls (inputs in pinned host memory copied in
-            every step, x and mu copied out)
-  roofline = the dominant kernel (P2P), FP64 ALU bound, CUDA-event timed inside the step
-  cpu_baseline = the oracle's direct O(N^2 K) matvec on this box's host cores
-
-python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C1] [--impl reference]
-N > 1 (torchrun): the path has no data-path exchange on one GPU; ranks run independent
-replicas of the workload ("weak" scaling), timed as the max over ranks.
+python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C4] [--impl reference]
+N > 1 (torchrun): target-leaf sharding of ONE matvec across the ranks: every rank owns a
+contiguous Morton range of target groups, x is all-gathered (NCCL) before the step's kernels and the owned rows of y
+after them; "scaling": "strong".
 """
 import argparse
+import csv
 import json
 import os
 import subprocess
@@ -40,7 +42,9 @@ UNIT = "interactions/s"
 # Algorithmic FP64 work per unit: one P2P pair = the four kernels of
 # Eq. (3)-(4) for one (target, Gauss point) pair; one M2P pair at order P = 4*NT + Nk + 6P + 30.
 P2P_FLOP_PER_PAIR = 80.0
-FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # SMs x FP64 FMA lanes x 2 x max SM clock
+FP64_LANES = 148 * 64                                  # SMs x FP64 FMA lanes (B200_PROFILING.md unit counts)
+FP64_NOMINAL_TFLOPS = FP64_LANES * 2 * 1.965e9 / 1e12  # x 2 flop x max SM clock
+COUNTERS_CSV = os.path.join(ROOT, "profiles", "r02_counters.csv")
 
 
 def n_terms_of(P):
@@ -56,6 +60,22 @@ def m2p_flop(P, st):
     """Algorithmic flop of one M2P launch: pairs at order P plus the pairs the list build flagged for order P - 2."""
     low = st.get("m2p_pairs_low", 0)
     return m2p_flop_per_pair(P, st["n_terms"]) * (st["m2p_pairs"] - low) + (m2p_flop_per_pair(P - 2) * low if low else 0.0)
+
+
+def load_counters(workload, theta, P):
+    """Per-launch ncu counters of the hot kernels for this workload and launch configuration, from the committed
+    capture profiles/r02_counters.csv (written from `ncu --set full`, command in profiles/r02_counters.md):
+    kernel -> dict(dram_bytes, fp64_thread_inst).  Missing file or row -> empty."""
+    out = {}
+    try:
+        with open(COUNTERS_CSV) as fh:
+            for row in csv.DictReader(r for r in fh if not r.startswith("#")):
+                if row["workload"] == workload and abs(float(row["theta"]) - theta) < 1e-12 and int(row["order_P"]) == P:
+                    out[row["kernel"]] = dict(dram_bytes=float(row["dram_read_bytes"]) + float(row["dram_write_bytes"]),
+                                              fp64_thread_inst=32.0 * float(row["fp64_warp_inst"]), source=row["source"])
+    except (OSError, KeyError, ValueError):
+        pass
+    return out
 
 
 class ClockSampler(threading.Thread):
@@ -79,7 +99,7 @@ class ClockSampler(threading.Thread):
                     self.samples.append(f)
             except Exception:
                 pass
-            self.stop_flag.wait(0.2)
+            self.stop_flag.wait(0.1)
 
     def summary(self):
         if not self.samples:
@@ -118,22 +138,36 @@ def sum_over_ranks(value, world, device=None):
 
 def load_workload(name):
     from paper_1810_03698_b200.workloads import make_config
+    if name.startswith("C3-"):
+        return make_config("C3", which=name[3:])
     return make_config(name)
 
 
-def oracle_matvec_rate(w, budget_s=12.0):
-    """The oracle as it stands: direct O(N^2 K) matvec over all host cores."""
+# ---- the oracle on the host cores (cpu_baseline, --impl reference) ----------------------------------------------
+def oracle_rows(n, count, seed=8):
+    import numpy as np
+    return np.sort(np.random.Generator(np.random.PCG64(seed)).choice(n, size=min(count, n), replace=False))
+
+
+def oracle_setup(w, rows_per_call):
     import numpy as np
     from oracle import pb_oracle as po
     po.build()
     orc = po.Oracle(w.verts, w.tris, po.Params(K_far=w.params["K_far"]))
     n = orc.nt
     x = np.random.Generator(np.random.PCG64(7)).normal(size=2 * n)
-    rows = None
-    pairs_per_call = float(n) * n * w.params["K_far"]
-    if pairs_per_call > 2e9:                      # bounded sample of target rows on big meshes
-        rows = np.random.Generator(np.random.PCG64(8)).choice(n, size=4096, replace=False)
-        pairs_per_call = 4096.0 * n * w.params["K_far"]
+    rows = None if rows_per_call >= n else oracle_rows(n, rows_per_call)
+    nrows = n if rows is None else int(rows.size)
+    pairs = float(nrows) * n * w.params["K_far"]          # (target, Gauss point) pairs of one call, all four kernels each
+    what = (f"the oracle's direct O(N^2 K) sum of Eq. (5) on {w.name}: "
+            + (f"{nrows} seeded sampled target rows against all {n * w.params['K_far']} source points"
+               if rows is not None else f"all {n} target rows"))
+    return po, orc, x, rows, pairs, what
+
+
+def oracle_matvec_rate(w, rows_per_call=256, budget_s=12.0):
+    """The oracle as it stands, timed for about `budget_s` seconds."""
+    po, orc, x, rows, pairs, what = oracle_setup(w, rows_per_call)
     orc.matvec(x, rows)                            # warm-up (thread pool, page faults)
     t0 = time.perf_counter()
     reps = 0
@@ -143,10 +177,12 @@ def oracle_matvec_rate(w, budget_s=12.0):
         el = time.perf_counter() - t0
         if el > budget_s or reps >= 50:
             break
-    return dict(value=pairs_per_call * reps / el, unit=UNIT, cores=po.num_threads(), kind="oracle",
-                sample=f"{reps} direct O(N^2 K) oracle matvecs of {w.name}"
-                       + (" on 4096 sampled target rows" if rows is not None else " (all rows)")
-                       + f", {el:.1f} s", ms_per_call=1e3 * el / reps)
+    n = orc.nt
+    rate = pairs * reps / el
+    return dict(value=rate, unit=UNIT, cores=po.num_threads(), kind="oracle",
+                sample=f"{reps} x {what}, {el:.1f} s; P2P interactions only (the oracle has no far field)",
+                ms_per_call=1e3 * el / reps,
+                full_matvec_seconds_extrapolated=float(n) * n * w.params["K_far"] / rate)
 
 
 def run_reference(args):
@@ -154,17 +190,7 @@ def run_reference(args):
     if rank != 0:
         return
     w = load_workload(args.workload)
-    import numpy as np
-    from oracle import pb_oracle as po
-    po.build()
-    orc = po.Oracle(w.verts, w.tris, po.Params(K_far=w.params["K_far"]))
-    n = orc.nt
-    x = np.random.Generator(np.random.PCG64(7)).normal(size=2 * n)
-    rows = None
-    pairs = float(n) * n * w.params["K_far"]
-    if pairs > 2e9:
-        rows = np.random.Generator(np.random.PCG64(8)).choice(n, size=4096, replace=False)
-        pairs = 4096.0 * n * w.params["K_far"]
+    po, orc, x, rows, pairs, what = oracle_setup(w, args.ref_rows)
     for _ in range(args.warmup):
         orc.matvec(x, rows)
     t0 = time.perf_counter()
@@ -172,16 +198,38 @@ def run_reference(args):
         orc.matvec(x, rows)
     el = time.perf_counter() - t0
     val = pairs * args.steps / el
-    sample = (f"each step = one direct O(N^2 K) oracle matvec of {w.name}"
-              + (" on 4096 sampled target rows" if rows is not None else " (all rows)"))
+    sample = f"each step = {what}"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w.name, "panels": int(n), "K_far": int(w.params["K_far"]), "what": sample},
+        "config": {"workload": w.name, "panels": int(orc.nt), "K_far": int(w.params["K_far"]), "what": sample},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": po.num_threads(), "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
+
+
+# ---- our arm ---------------------------------------------------------------------------------------------------------
+def timed_solve(pb, torch, name, dev_index, repeats=1, warm=0):
+    """One polarizable solve of a workload on resident inputs (mesh, sites, tree already built): seconds, result."""
+    w = load_workload(name)
+    ctx = pb.from_workload(w, dev_index)
+    ctx.tree_build()
+    for _ in range(warm):
+        ctx.solve()
+    torch.cuda.synchronize()
+    best, res = None, None
+    for _ in range(repeats):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        _, _, res = ctx.solve()
+        e1.record()
+        e1.synchronize()
+        ms = e0.elapsed_time(e1)
+        best = ms if best is None or ms < best else best
+    st = ctx.stats()
+    ctx.close()
+    return best, res, st
 
 
 def run_ours(args):
@@ -196,7 +244,7 @@ def run_ours(args):
     from paper_1810_03698_b200 import pb
     pb.lib()                                       # fails loudly if the CUDA library is missing
 
-    w = load_workload(args.workload)               # every rank: its own replica of the workload
+    w = load_workload(args.workload)
     names = {k for k, _ in pb.Params._fields_}
     prm = {k: v for k, v in w.params.items() if k in names}
     if args.theta is not None:
@@ -207,36 +255,30 @@ def run_ours(args):
         prm["ncrit"] = args.ncrit
     ctx = pb.PB(local_rank, **prm)
     s = w.sites
-    f64, i32 = torch.float64, torch.int32
-    host = dict(verts=torch.from_numpy(np.ascontiguousarray(w.verts)).pin_memory(),
-                tris=torch.from_numpy(np.ascontiguousarray(w.tris, dtype=np.int32)).pin_memory(),
-                pos=torch.from_numpy(np.ascontiguousarray(s["pos"])).pin_memory(),
-                q=torch.from_numpy(np.ascontiguousarray(s["q"])).pin_memory(),
-                dip=torch.from_numpy(np.ascontiguousarray(s["dip"])).pin_memory(),
-                quad=torch.from_numpy(np.ascontiguousarray(s["quad"])).pin_memory(),
-                alpha=torch.from_numpy(np.ascontiguousarray(s["alpha"])).pin_memory(),
-                group=torch.from_numpy(np.ascontiguousarray(s["group"], dtype=np.int32)).pin_memory())
-    resident = {k: v.to(dev) for k, v in host.items()}
+    ctx.mesh_load(w.verts, w.tris)
+    ctx.sites_load(s["pos"], s["q"], s["dip"], s["quad"], s["alpha"], s["group"])
+    shard = None
+    if world > 1:
+        from paper_1810_03698_b200 import shard as shard_mod
+        shard = shard_mod.TargetShard(ctx, rank, world)       # owned Morton range of target groups (before tree_build)
+    ctx.tree_build()
     nt, na = int(w.tris.shape[0]), int(s["pos"].shape[0])
-    x_host = torch.empty(2 * nt, dtype=f64).pin_memory()
-    mu_host = torch.empty(na, 3, dtype=f64).pin_memory()
-    h2d = sum(v.numel() * v.element_size() for v in host.values())
-    d2h = x_host.numel() * 8 + mu_host.numel() * 8
+    f64 = torch.float64
+    x_np = np.random.Generator(np.random.PCG64(7)).normal(size=2 * nt)
+    x_host = torch.from_numpy(x_np).pin_memory()
+    y_host = torch.empty(2 * nt, dtype=f64).pin_memory()
+    x = x_host.to(dev)
+    y = torch.empty_like(x)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
 
     def step_resident():
-        d = resident
-        ctx.mesh_load(d["verts"], d["tris"])
-        ctx.sites_load(d["pos"], d["q"], d["dip"], d["quad"], d["alpha"], d["group"])
-        ctx.tree_build()
-        return ctx.solve()[2]
+        if shard is not None:
+            shard.matvec(x, y)                     # all-gather of x's owned slices, owned rows, all-gather of y
+        else:
+            ctx.matvec(x, out=y)
 
     def step_e2e():
-        d = {k: v.to(dev, non_blocking=True) for k, v in host.items()}
-        ctx.mesh_load(d["verts"], d["tris"])
-        ctx.sites_load(d["pos"], d["q"], d["dip"], d["quad"], d["alpha"], d["group"])
-        ctx.tree_build()
-        return ctx.solve_host(x_host, mu_host)
+        ctx.matvec_host(x_host, y_host)
 
     def barrier():
         if world > 1:
@@ -245,109 +287,155 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     def timed(fn, steps):
-        tot_ms, last = 0.0, None
+        tot_ms = 0.0
         for _ in range(steps):
             flush.zero_()                          # L2 flush, outside the event pair
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
-            last = fn()
+            fn()
             e1.record()
             e1.synchronize()
             tot_ms += e0.elapsed_time(e1)
-        return tot_ms, last
+        return tot_ms
 
-    for _ in range(max(args.warmup, 3)):
-        res = step_resident()
-    step_e2e()
+    W = max(args.warmup, 3)
+    for _ in range(W):
+        step_resident()
+    if world == 1:
+        step_e2e()
     sampler = ClockSampler(local_rank)
     sampler.start()
     st0 = ctx.stats()
     barrier()
     if args.profiler_range:                        # ncu --profile-from-start off captures exactly the timed steps
         torch.cuda.profiler.start()
-    ms_total, res = timed(step_resident, args.steps)
+    ms_total = timed(step_resident, args.steps)
     if args.profiler_range:
         torch.cuda.synchronize()
         torch.cuda.profiler.stop()
     barrier()
     st1 = ctx.stats()
+    ms_e2e = timed(step_e2e, args.steps) if world == 1 else 0.0
     barrier()
-    ms_e2e, res_e2e = timed(step_e2e, args.steps)
-    barrier()
-    # Kernel durations for the roofline: the SAME steps once more with a CUDA-event pair around every
-    # P2P and M2P launch.  In this mode the library runs the matvec's two branches back to back on one
-    # stream (in the timed steps above the far-field branch overlaps P2P on a second stream), so each
+    # Kernel durations for the roofline: the SAME steps once more with a CUDA-event pair around every P2P and M2P
+    # launch on the stream they are launched on.  In this mode the library runs the matvec's two branches back to
+    # back on one stream (in the timed steps above the far-field branch overlaps P2P on a second stream), so each
     # pair brackets exactly one kernel; grids, blocks and data are identical.
     ctx.set_profiling(True)
-    ms_prof, _ = timed(step_resident, args.steps)
+    ms_prof = timed(step_resident, args.steps)
     stp = ctx.stats()
     ctx.set_profiling(False)
     barrier()
     sampler.stop_flag.set()
     sampler.join(timeout=2)
+    clocks = sampler.summary()
 
     ms_total = max_over_ranks(ms_total, world, dev)
-    ms_e2e = max_over_ranks(ms_e2e, world, dev)
+    P = int(ctx.get_params().order_P)
+    theta = float(ctx.get_params().theta)
+    # with sharding a rank's lists hold only its own groups: the job's counts are the sum over ranks
+    p2p_pairs = sum_over_ranks(float(st1["p2p_pairs"]), world, dev)
+    m2p_pairs = sum_over_ranks(float(st1["m2p_pairs"]), world, dev)
+    evald_per_mv = p2p_pairs + m2p_pairs
     inter_per_mv = float(nt) * float(st1["n_sources"])          # the N x N_s pairs one matvec accounts for
-    evald_per_mv = st1["p2p_pairs"] + st1["m2p_pairs"]
-    mv_timed = st1["matvec_calls"] - st0["matvec_calls"]
-    units = sum_over_ranks(float(inter_per_mv) * mv_timed, world, dev)
-    units_e2e = sum_over_ranks(float(inter_per_mv) * res_e2e["matvecs_total"] * args.steps, world, dev)
-    value = units / (ms_total * 1e-3)
-    value_e2e = units_e2e / (ms_e2e * 1e-3)
+    value = evald_per_mv * args.steps / (ms_total * 1e-3)
     launches = st1["kernel_launches"] - st0["kernel_launches"]
 
-    # roofline of the dominant kernel, from the CUDA-event pairs recorded inside the timed steps
-    P = int(ctx.get_params().order_P)
+    # ---- roofline of both hot kernels
+    peak_probe = ctx.fp64_peak_probe()                          # measured DFMA throughput of this GPU, TFLOP/s
+    sm_hz = (clocks["sm_mhz"] or 1965.0) * 1e6
+    inst_peak = FP64_LANES * sm_hz                              # FP64 lane-instructions per second at the sampled clock
+    counters = load_counters(w.name, theta, P)
+    p2p_kernel = "k_p2p2" if nt >= 30000 else "k_p2p"
+    m2p_kernel = "k_m2p2" if P <= 6 else "k_m2p"
     p2p_ms = stp["prof_p2p_ms"] / max(stp["prof_p2p_launches"], 1)
     m2p_ms = stp["prof_m2p_ms"] / max(stp["prof_m2p_launches"], 1)
-    p2p_tf = P2P_FLOP_PER_PAIR * st1["p2p_pairs"] / (p2p_ms * 1e-3) / 1e12 if p2p_ms > 0 else 0.0
-    m2p_tf = (m2p_flop(P, st1) / (m2p_ms * 1e-3) / 1e12) if m2p_ms > 0 else 0.0
-    dominant = "k_p2p" if stp["prof_p2p_ms"] >= stp["prof_m2p_ms"] else "k_m2p"
-    ach = p2p_tf if dominant == "k_p2p" else m2p_tf
-    # DRAM bytes per launch of the dominant kernel from the committed ncu --set full captures (per workload)
-    traffic = {("C1", "k_p2p"): (2.517e6, "profiles/r01c_ncu_full_C1.md"),
-               ("C4", "k_m2p"): (7.68e8, "profiles/r01b_ncu_full_C4.md")}.get((w.name, dominant), (None, None))
-    roofline = {"bound": "alu", "kernel": dominant, "achieved": ach, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "frac": ach / FP64_PEAK_TFLOPS, "traffic": traffic[0], "traffic_source": traffic[1],
-                "peak_source": "148 SM x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md section 7); "
-                               "pb_fp64_peak_probe measured %.1f TFLOP/s on this GPU" % ctx.fp64_peak_probe(),
-                "timed_in": "a repeat of the timed steps with per-kernel CUDA events (branches serialised on one "
-                            "stream): %.3f ms per step against %.3f ms with the far-field branch overlapped" % (
-                                ms_prof / args.steps, ms_total / args.steps),
-                "p2p": {"ms_per_launch": p2p_ms, "launches": stp["prof_p2p_launches"], "pairs": st1["p2p_pairs"],
-                        "tflops": p2p_tf, "share_of_step": stp["prof_p2p_ms"] / ms_prof},
-                "m2p": {"ms_per_launch": m2p_ms, "launches": stp["prof_m2p_launches"], "pairs": st1["m2p_pairs"],
-                        "tflops": m2p_tf, "share_of_step": stp["prof_m2p_ms"] / ms_prof}}
+
+    def kernel_entry(kname, ms, nlaunch, pairs, flop):
+        c = counters.get(kname, {})
+        e = {"kernel": kname, "ms_per_launch": ms, "launches": int(nlaunch), "pairs_per_launch": int(pairs),
+             "algorithmic_tflops": flop / (ms * 1e-3) / 1e12 if ms > 0 else 0.0,
+             "share_of_step": ms * nlaunch / ms_prof if ms_prof > 0 else None}
+        e["frac_algorithmic"] = e["algorithmic_tflops"] / peak_probe if peak_probe > 0 else None
+        if c and ms > 0:
+            e["fp64_inst_per_pair"] = c["fp64_thread_inst"] / pairs if pairs else None
+            e["frac_inst"] = c["fp64_thread_inst"] / (ms * 1e-3) / inst_peak
+            e["dram_bytes_per_launch"] = c["dram_bytes"]
+            e["counters_source"] = c["source"]
+        else:
+            e["fp64_inst_per_pair"] = e["frac_inst"] = e["dram_bytes_per_launch"] = None
+        return e
+
+    e_p2p = kernel_entry(p2p_kernel, p2p_ms, stp["prof_p2p_launches"], st1["p2p_pairs"], P2P_FLOP_PER_PAIR * st1["p2p_pairs"])
+    e_m2p = kernel_entry(m2p_kernel, m2p_ms, stp["prof_m2p_launches"], st1["m2p_pairs"], m2p_flop(P, st1))
+    dom = e_p2p if stp["prof_p2p_ms"] >= stp["prof_m2p_ms"] else e_m2p
+    roofline = {"bound": "alu", "kernel": dom["kernel"], "achieved": dom["algorithmic_tflops"], "peak": peak_probe,
+                "unit": "TFLOP/s", "frac": dom["frac_algorithmic"], "frac_inst": dom["frac_inst"],
+                "traffic": dom["dram_bytes_per_launch"],
+                "peak_source": "pb_fp64_peak_probe, measured in this run (independent DFMA chains); nominal "
+                               "148 SM x 64 lanes x 2 x 1.965 GHz = %.1f TFLOP/s (MEASURED_PEAKS.json has no FP64 "
+                               "figure); frac_inst = executed FP64-pipe lane-instructions (ncu) / time / "
+                               "(148 x 64 x sampled SM clock)" % FP64_NOMINAL_TFLOPS,
+                "timed_in": "a repeat of the timed steps with a CUDA-event pair around every P2P and M2P launch on the "
+                            "launching stream (branches serialised): %.3f ms per step against %.3f ms with the far-field "
+                            "branch overlapped" % (ms_prof / args.steps, ms_total / args.steps),
+                "p2p": e_p2p, "m2p": e_m2p}
     if rank != 0:
+        ctx.close()
+        if world > 1:
+            import torch.distributed as dist
+            dist.destroy_process_group()
         return
-    cpu = oracle_matvec_rate(w) if world == 1 and not args.no_cpu_baseline else None
+
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic",
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": W,
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "strong" if world > 1 else "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": w.name, "panels": nt, "gauss_points": int(st1["n_sources"]), "sites": na,
-                   "theta": float(ctx.get_params().theta), "order_P": P, "ncrit": int(st1["ncrit_used"]),
-                   "K_far": int(w.params["K_far"]), "gmres_tol": float(ctx.get_params().gmres_tol),
-                   "scf_tol_debye": float(ctx.get_params().scf_tol_debye),
-                   "l2": "flushed between steps (256 MiB device write, outside the event pairs)",
-                   "parallelism": "replicas only" if world > 1 else "1 GPU"},
-        "solve": {"time_per_polarizable_solve_ms": ms_total / args.steps, "dG_solv_kcal_mol": res["dG_solv"],
-                  "scf_iters": res["scf_iters"], "gmres_iters": res["gmres_iters_total"], "matvecs": res["matvecs_total"],
-                  "interactions_per_matvec": int(inter_per_mv), "status": res["status"]},
-        "evaluated": {"p2p_pairs_per_matvec": int(st1["p2p_pairs"]), "m2p_pairs_per_matvec": int(st1["m2p_pairs"]),
-                      "m2p_pairs_at_order_P_minus_2": int(st1["m2p_pairs_low"]),
-                      "pairs_per_s": float(evald_per_mv) * mv_timed / (ms_total * 1e-3) * (world if world > 1 else 1)},
-        "e2e": {"value": value_e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                "ms_per_step": ms_e2e / args.steps},
+                   "theta": theta, "order_P": P, "ncrit": int(st1["ncrit_used"]), "K_far": int(w.params["K_far"]),
+                   "step": "one treecode matvec of Eq. (5) on a resident vector",
+                   "l2": "flushed between steps (256 MiB device write, outside the event pairs); the step's own "
+                         "inputs (0.46 GB source records, 1.3 GB near table at C4) exceed the 126 MB L2",
+                   "parallelism": "1 GPU" if world == 1 else f"target groups sharded over {world} GPUs"},
+        "evaluated": {"p2p_pairs_per_matvec": int(p2p_pairs), "m2p_pairs_per_matvec": int(m2p_pairs),
+                      "m2p_pairs_at_order_P_minus_2": int(sum_over_ranks(float(st1["m2p_pairs_low"]), world, dev)) if world == 1 else None,
+                      "covered_pairs": int(st1["covered_pairs"]), "covered_equals_N_x_Ns": bool(st1["covered_pairs"] == int(inter_per_mv)) if world == 1 else None,
+                      "direct_equivalent_per_s": inter_per_mv * args.steps / (ms_total * 1e-3)},
         "gpu_launches": int(launches),
         "roofline": roofline,
-        "clocks": sampler.summary(),
+        "clocks": clocks,
     }
-    if cpu is not None:
-        line["cpu_baseline"] = cpu
-    print(json.dumps(line))
+    if world == 1:
+        line["e2e"] = {"value": evald_per_mv * args.steps / (ms_e2e * 1e-3), "unit": UNIT,
+                       "h2d_bytes_per_step": int(x_host.numel() * 8), "d2h_bytes_per_step": int(y_host.numel() * 8),
+                       "ms_per_step": ms_e2e / args.steps, "api": "pb_matvec_host"}
+    else:
+        line["e2e"] = None
+    # ---- the second half of the metric: time per polarizable PB solve
+    if world == 1 and not args.no_solve:
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        _, _, res = ctx.solve()
+        e1.record()
+        e1.synchronize()
+        line["solve"] = {"workload": w.name, "time_per_polarizable_solve_s": e0.elapsed_time(e1) * 1e-3, "runs": 1,
+                         "dG_solv_kcal_mol": res["dG_solv"], "scf_iters": res["scf_iters"], "gmres_iters": res["gmres_iters_total"],
+                         "matvecs": res["matvecs_total"], "final_gmres_relres": res["final_gmres_relres"],
+                         "final_scf_delta_debye": res["final_scf_delta_debye"], "status": res["status"]}
     ctx.close()
+    if world == 1 and not args.no_configs:
+        cfgs = {}
+        for name in ("C1", "C2", "C3-complex", "C3-receptor", "C3-ligand"):
+            ms, res, st = timed_solve(pb, torch, name, local_rank, repeats=3 if name in ("C1", "C2") else 1, warm=1)
+            cfgs[name] = {"panels": int(st["n_panels"]), "sites": int(st["n_sites"]), "solve_ms": ms, "dG_solv_kcal_mol": res["dG_solv"],
+                          "scf_iters": res["scf_iters"], "matvecs": res["matvecs_total"], "status": res["status"]}
+        cfgs["C3-ddG_bind_kcal_mol"] = (cfgs["C3-complex"]["dG_solv_kcal_mol"] - cfgs["C3-receptor"]["dG_solv_kcal_mol"]
+                                         - cfgs["C3-ligand"]["dG_solv_kcal_mol"])
+        line["configs"] = cfgs
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = oracle_matvec_rate(w, rows_per_call=args.ref_rows)
+    print(json.dumps(line))
     if world > 1:
         import torch.distributed as dist
         dist.destroy_process_group()
@@ -379,6 +467,7 @@ def run_sweep(args):
     y = torch.empty_like(xd)
     idx = torch.from_numpy(np.concatenate([rows, nt + rows])).cuda()
     cases = set(args.sweep_cases.split(","))
+    peak = None
     for theta in (0.3, 0.5, 0.7):
         for P in (4, 6, 8):
             if "matvec" not in cases:
@@ -387,6 +476,8 @@ def run_sweep(args):
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record(); ctx.tree_build(); e1.record(); e1.synchronize()
             t_build = e0.elapsed_time(e1)
+            if peak is None:
+                peak = ctx.fp64_peak_probe()
             for _ in range(3):
                 ctx.matvec(xd, out=y)
             ts = []
@@ -399,17 +490,18 @@ def run_sweep(args):
             lm = st["last_matvec_ms"]
             got = y[idx].cpu().numpy()
             err = float(np.linalg.norm(got - yref) / np.linalg.norm(yref))
-            fl_m = m2p_flop_per_pair(P, st["n_terms"])
             print(json.dumps({
                 "case": "matvec", "workload": w.name, "theta": theta, "order_P": P, "ncrit": int(st["ncrit_used"]),
                 "ms_per_matvec": ms, "tree_build_ms": t_build,
-                "interactions_per_s": float(nt) * st["n_sources"] / (ms * 1e-3),
+                "interactions_per_s": (st["p2p_pairs"] + st["m2p_pairs"]) / (ms * 1e-3),
+                "direct_equivalent_per_s": float(nt) * st["n_sources"] / (ms * 1e-3),
                 "p2p_pairs": int(st["p2p_pairs"]), "m2p_pairs": int(st["m2p_pairs"]),
+                "covered_equals_N_x_Ns": bool(st["covered_pairs"] == nt * st["n_sources"]),
                 "serial_ms": {k: lm[k] for k in ("weights", "p2m_m2m", "m2p", "p2p", "near_combine")},
                 "p2p_tflops": P2P_FLOP_PER_PAIR * st["p2p_pairs"] / (lm["p2p"] * 1e-3) / 1e12,
                 "m2p_pairs_low_order": int(st["m2p_pairs_low"]),
                 "m2p_tflops": m2p_flop(P, st) / (lm["m2p"] * 1e-3) / 1e12 if lm["m2p"] > 0 else 0.0,
-                "fp64_peak_tflops": FP64_PEAK_TFLOPS, "rel_l2_vs_oracle_rows": err, "device_gb": st["device_bytes"] / 1e9}), flush=True)
+                "fp64_peak_tflops_measured": peak, "rel_l2_vs_oracle_rows": err, "device_gb": st["device_bytes"] / 1e9}), flush=True)
     ctx.set_params(**{k: v for k, v in w.params.items() if k in ("theta", "order_P")})
     ctx.tree_build()
     if "gmres" in cases:
@@ -433,7 +525,7 @@ def run_sweep(args):
         ms_vec = ms_g - (info["iters"] + 2) * ms_mv
         print(json.dumps({"case": "gmres_vectors", "workload": w.name, "iters": info["iters"], "ms_total": ms_g, "ms_per_matvec": ms_mv,
                           "ms_vector_kernels": ms_vec, "algorithmic_gb": byts / 1e9, "gb_per_s": byts / 1e9 / (ms_vec * 1e-3),
-                          "hbm_peak_gb_per_s_measured": 6548.2}), flush=True)
+                          "hbm_peak_gb_per_s_measured": 6551.0}), flush=True)
         ctx.set_params(gmres_maxit=1000, gmres_tol=float(w.params["gmres_tol"]))
     if "solve" not in cases:
         ctx.close()
@@ -451,18 +543,22 @@ def run_sweep(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C1", help="C1 (BASELINE configs[1], default), C0, C2, C3, C4")
+    ap.add_argument("--workload", default="C4", help="C4 (BASELINE configs[4], default), C1, C2, C3-complex, C3-receptor, C3-ligand")
     ap.add_argument("--theta", type=float, default=None)
     ap.add_argument("--order", type=int, default=None)
     ap.add_argument("--ncrit", type=int, default=None)
+    ap.add_argument("--ref-rows", type=int, default=256,
+                    help="target rows per oracle call (cpu_baseline and --impl reference): about 2 s per call at C4 on 16 cores")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-solve", action="store_true", help="skip the timed full polarizable solve")
+    ap.add_argument("--no-configs", action="store_true", help="skip the C1-C3 solve times")
     ap.add_argument("--profiler-range", action="store_true",
                     help="bracket the timed resident steps with cudaProfilerStart/Stop (for ncu --profile-from-start off)")
     ap.add_argument("--sweep", action="store_true",
-                    help="theta x P matvec sweep with sampled-row accuracy and one full solve (BASELINE configs[4]); use with --workload C4")
+                    help="theta x P matvec sweep with sampled-row accuracy and one full solve (BASELINE configs[4])")
     ap.add_argument("--sweep-rows", type=int, default=1024)
     ap.add_argument("--sweep-cases", default="matvec,solve", help="comma list of matvec, gmres, solve")
     ap.add_argument("--gmres-iters", type=int, default=40)

@@ -40,7 +40,8 @@ typedef struct pb_ctx pb_ctx;
 typedef enum pb_status {
     PB_OK = 0,
     PB_ERR_INVALID_ARG = -1,
-    PB_ERR_BAD_MESH = -2,       /* degenerate panel, too many panels around one vertex       */
+    PB_ERR_BAD_MESH = -2,       /* degenerate panel, too many panels around one vertex, surface not closed or not
+                                   consistently / outward oriented, a site outside the surface (S: section 8(b)) */
     PB_ERR_NOT_READY = -3,      /* call order: mesh -> (sites) -> tree -> operators          */
     PB_ERR_CUDA = -4,
     PB_ERR_ALLOC = -5,
@@ -77,6 +78,11 @@ typedef struct pb_params {
                                points (the paper's choice), 1 = treecode over the panel tree when
                                theta > 0 and order_P <= 8, 2 (default) = treecode when N_a * N_s >= 2^31   */
     double thole_a;         /* Thole damping constant, 0.39 (D: R-17)                  */
+    int32_t rhs_treecode;   /* right-hand side Eq. (8): 0 = direct sum over all sites (the paper's choice),
+                               1 = treecode with the sites as sources in their own octree (Cartesian multipole
+                               moments of q, p, Q per site cell, Laplace far field at the collocation points) when
+                               theta > 0, 2 (default) = treecode when N * N_a >= 2^31                          */
+    int32_t reserved0;
 } pb_params;
 
 /* Result of one polarizable solve (HOST struct). */
@@ -116,6 +122,18 @@ typedef struct pb_stats {
                                    combine, 5 total                                            */
     int64_t ncrit_used;         /* leaf capacity the tree was built with (see pb_params.ncrit)  */
     int64_t m2p_pairs_low;      /* of m2p_pairs: those evaluated at order P - 2 (cells far inside the MAC) */
+    /* Exact-cover check of the stored interaction lists: counted by a kernel that walks the lists the
+     * matvec kernels read -- sum over groups of (targets in the group) x (source points in its P2P ranges + source
+     * points of its M2P cells).  Every (target, source point) pair is covered exactly once iff this equals
+     * n_panels * n_sources; the traversal cannot double-count (a cell is either accepted, listed as a leaf, or
+     * replaced by ALL its children), so equality rules out a missed cell. */
+    int64_t covered_pairs;
+    int64_t site_p2p_pairs;     /* the same three counters for the site lists of the treecode reaction field       */
+    int64_t site_m2p_pairs;     /* (0 until that path has been used: pb_params.site_treecode)                      */
+    int64_t site_covered_pairs; /* == n_sites * n_sources when the site lists are complete                         */
+    int64_t rhs_p2p_pairs;      /* RHS by the site tree (pb_params.rhs_treecode): (panel, site) pairs summed directly */
+    int64_t rhs_m2p_pairs;      /* (panel, site cell) pairs through a multipole expansion                          */
+    int64_t rhs_covered_pairs;  /* == n_panels * n_sites when those lists are complete                             */
 } pb_stats;
 
 typedef void* (*pb_alloc_fn)(void* user, size_t bytes);     /* returns a 256-byte aligned device pointer or NULL */
@@ -135,14 +153,22 @@ int pb_get_params(const pb_ctx* ctx, pb_params* out /* HOST */);
 /* ---- inputs ------------------------------------------------------------------------ */
 /* Closed, outward-oriented triangulated surface.  Computes per panel the
  * area, unit normal (pointing into the solvent) and centroid = collocation point.
- * verts [nv][3] fp64, tris [nt][3] int32.  The arrays are copied; PB_ERR_BAD_MESH if a
- * panel has zero area or an index is out of range. */
+ * verts [nv][3] fp64, tris [nt][3] int32.  The arrays are copied.  PB_ERR_BAD_MESH if an index is out of
+ * range, a panel has zero area, the surface is not closed and consistently oriented (every directed edge
+ * a->b must occur exactly once and be matched by exactly one b->a: checked on the device by sorting the
+ * 3 nt edge keys), or its enclosed volume sum v0.(v1 x v2)/6 is not positive (normals must point into the
+ * solvent).  Synchronises. */
 int pb_mesh_load(pb_ctx* ctx, const double* verts, int64_t nv, const int32_t* tris, int64_t nt);
 
 /* Point multipoles of Eq. (7): charge q [na], permanent dipole dip [na][3],
  * traceless quadrupole quad [na][6] = xx,xy,xz,yy,yz,zz in the convention of Eq. (7)
  * (potential term Q_ij d_i d_j / (2 R^5)), isotropic polarizability alpha [na] in
- * Angstrom^3 (D: R-2), polarization group [na].  Copied. */
+ * Angstrom^3 (D: R-2), polarization group [na].  Copied.  Synchronises.
+ * PB_ERR_INVALID_ARG if a quadrupole is not traceless (|tr Q| > 1e-10 max|Q_ij|: Eq. (20)'s factor 1/6 assumes
+ * it, D: R-3) or alpha < 0.  Every site must lie inside the surface (the interior problem of Eq. (1)):
+ * checked as soon as both the mesh and the sites are loaded (here or in pb_mesh_load / pb_tree_build) through the
+ * solid angle sum_j A_j n_j.(c_j - r_m)/(4 pi |c_j - r_m|^3), which is 1 inside and 0 outside a closed
+ * surface; a site with less than 1/2 gives PB_ERR_BAD_MESH. */
 int pb_sites_load(pb_ctx* ctx, int64_t na, const double* pos, const double* q, const double* dip,
                   const double* quad, const double* alpha, const int32_t* group);
 

@@ -99,6 +99,7 @@ extern "C" void pb_default_params(pb_params* p)
     p->scf_maxit = 200;
     p->site_treecode = 2;
     p->thole_a = 0.39;
+    p->rhs_treecode = 2;
 }
 
 extern "C" int pb_create(pb_ctx** out, int device, void* cuda_stream)
@@ -181,6 +182,7 @@ extern "C" int pb_set_params(pb_ctx* ctx, const pb_params* p)
         return pb_fail(ctx, PB_ERR_INVALID_ARG, "solver limits/tolerances must be positive");
     if (p->precond < 0 || p->precond > 3) return pb_fail(ctx, PB_ERR_INVALID_ARG, "precond must be 0, 1, 2 or 3");
     if (p->site_treecode < 0 || p->site_treecode > 2) return pb_fail(ctx, PB_ERR_INVALID_ARG, "site_treecode must be 0, 1 or 2");
+    if (p->rhs_treecode < 0 || p->rhs_treecode > 2) return pb_fail(ctx, PB_ERR_INVALID_ARG, "rhs_treecode must be 0, 1 or 2");
     const pb_params& o = ctx->prm;
     bool shape = o.kappa != p->kappa || o.theta != p->theta || o.order_P != p->order_P ||
                  o.ncrit != p->ncrit || o.K_far != p->K_far || o.K_near != p->K_near ||
@@ -221,6 +223,49 @@ __global__ void k_mesh_check(int64_t nt, int64_t nv, const double* __restrict__ 
     if (!(l > 0.0) || !isfinite(l)) atomicOr(bad, 2);
 }
 
+// Closedness and orientation: the 3 nt directed edges a->b as keys (min << 32 | max) with the
+// direction as value; after sorting, every key must occur exactly twice, once in each direction.
+__global__ void k_edge_keys(int64_t nt, const int32_t* __restrict__ tris, uint64_t* __restrict__ keys, int32_t* __restrict__ dir)
+{
+    const int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (e >= 3 * nt) return;
+    const int64_t j = e / 3;
+    const int k = (int)(e - 3 * j);
+    const uint32_t a = (uint32_t)tris[3 * j + k], b = (uint32_t)tris[3 * j + (k + 1) % 3];
+    keys[e] = a < b ? ((uint64_t)a << 32 | b) : ((uint64_t)b << 32 | a);
+    dir[e] = a < b ? 0 : 1;
+}
+
+__global__ void k_edge_check(int64_t ne, const uint64_t* __restrict__ keys, const int32_t* __restrict__ dir, int* __restrict__ bad)
+{
+    const int64_t i = 2 * (blockIdx.x * (int64_t)blockDim.x + threadIdx.x);
+    if (i >= ne) return;
+    if (i + 1 >= ne || keys[i] != keys[i + 1] || (i > 0 && keys[i - 1] == keys[i])) { atomicOr(bad, 4); return; }   // open / non-manifold edge
+    if (dir[i] == dir[i + 1]) atomicOr(bad, 8);                                                                      // inconsistent orientation
+}
+
+// enclosed volume sum_j v0.(v1 x v2)/6 (block partials, then one thread adds them in order)
+__global__ void __launch_bounds__(256)
+k_mesh_volume(int64_t nt, const double* __restrict__ verts, const int32_t* __restrict__ tris, double* __restrict__ partial)
+{
+    __shared__ double red[8];
+    double s = 0;
+    for (int64_t j = blockIdx.x * 256LL + threadIdx.x; j < nt; j += 256LL * gridDim.x) {
+        const double* a = verts + 3 * (int64_t)tris[3 * j];
+        const double* b = verts + 3 * (int64_t)tris[3 * j + 1];
+        const double* c = verts + 3 * (int64_t)tris[3 * j + 2];
+        s += a[0] * (b[1] * c[2] - b[2] * c[1]) + a[1] * (b[2] * c[0] - b[0] * c[2]) + a[2] * (b[0] * c[1] - b[1] * c[0]);
+    }
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double v = 0;
+        for (int k = 0; k < 8; ++k) v += red[k];
+        partial[blockIdx.x] = v / 6.0;
+    }
+}
+
 extern "C" int pb_mesh_load(pb_ctx* ctx, const double* verts, int64_t nv, const int32_t* tris, int64_t nt)
 {
     if (!ctx) return PB_ERR_INVALID_ARG;
@@ -253,11 +298,57 @@ extern "C" int pb_mesh_load(pb_ctx* ctx, const double* verts, int64_t nv, const 
     PB_CUDA(cudaStreamSynchronize(ctx->stream));
     if (hbad & 1) return pb_fail(ctx, PB_ERR_BAD_MESH, "pb_mesh_load: triangle vertex index out of range");
     if (hbad & 2) return pb_fail(ctx, PB_ERR_BAD_MESH, "pb_mesh_load: degenerate (zero-area or non-finite) panel");
+    {   // closed, consistently and outward oriented (S: section 8(b))
+        const int64_t ne = 3 * nt;
+        uint64_t *k0, *k1, *ks;
+        int32_t *d0, *d1, *ds;
+        PB_TRY(pb_dalloc_t(ctx, &k0, ne, CAT_TMP));
+        PB_TRY(pb_dalloc_t(ctx, &k1, ne, CAT_TMP));
+        PB_TRY(pb_dalloc_t(ctx, &d0, ne, CAT_TMP));
+        PB_TRY(pb_dalloc_t(ctx, &d1, ne, CAT_TMP));
+        k_edge_keys<<<pb_blocks(ne, 256), 256, 0, ctx->stream>>>(nt, ctx->tris, k0, d0);
+        PB_LAUNCH_CHECK();
+        int vbits = 1;
+        while (((int64_t)1 << vbits) < nv) ++vbits;
+        PB_TRY(pb_radix_sort(ctx, k0, k1, d0, d1, ne, 32 + vbits, &ks, &ds));
+        PB_CUDA(cudaMemsetAsync(bad, 0, sizeof(int), ctx->stream));
+        k_edge_check<<<pb_blocks((ne + 1) / 2, 256), 256, 0, ctx->stream>>>(ne, ks, ds, bad);
+        PB_LAUNCH_CHECK();
+        const int nvb = 256;
+        double* vpart = ctx->scratch + 64;
+        k_mesh_volume<<<nvb, 256, 0, ctx->stream>>>(nt, ctx->verts, ctx->tris, vpart);
+        PB_LAUNCH_CHECK();
+        double hv[256];
+        PB_CUDA(cudaMemcpyAsync(&hbad, bad, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+        PB_CUDA(cudaMemcpyAsync(hv, vpart, sizeof(hv), cudaMemcpyDeviceToHost, ctx->stream));
+        PB_CUDA(cudaStreamSynchronize(ctx->stream));
+        pb_dfree_cat(ctx, CAT_TMP);
+        if (hbad & 4) return pb_fail(ctx, PB_ERR_BAD_MESH, "pb_mesh_load: surface not closed (an edge is not shared by exactly two panels)");
+        if (hbad & 8) return pb_fail(ctx, PB_ERR_BAD_MESH, "pb_mesh_load: panels not consistently oriented (an edge is traversed twice in the same direction)");
+        double vol = 0;
+        for (int k = 0; k < nvb; ++k) vol += hv[k];
+        if (!(vol > 0.0)) return pb_fail(ctx, PB_ERR_BAD_MESH, "pb_mesh_load: enclosed volume %.6g <= 0 (normals must point into the solvent, P:49)", vol);
+    }
     ctx->mesh_loaded = true;
+    ctx->sites.inside_checked = false;
+    if (ctx->sites.loaded) PB_TRY(pb_check_sites_inside(ctx));
     return PB_OK;
 }
 
 // ---- sites --------------------------------------------------------------------------------
+// traceless quadrupoles (Eq. 20's factor 1/6 assumes them, D: R-3) and non-negative polarizabilities
+__global__ void k_sites_check(int64_t na, const double* __restrict__ quad, const double* __restrict__ alpha, int* __restrict__ bad)
+{
+    const int64_t m = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (m >= na) return;
+    const double* Q = quad + 6 * m;
+    double mx = 0;
+    for (int c = 0; c < 6; ++c) mx = fmax(mx, fabs(Q[c]));
+    const double tr = Q[0] + Q[3] + Q[5];
+    if (!(fabs(tr) <= 1e-10 * mx)) atomicOr(bad, 1);           // also catches NaN
+    if (!(alpha[m] >= 0.0)) atomicOr(bad, 2);
+}
+
 extern "C" int pb_sites_load(pb_ctx* ctx, int64_t na, const double* pos, const double* q, const double* dip,
                              const double* quad, const double* alpha, const int32_t* group)
 {
@@ -283,7 +374,18 @@ extern "C" int pb_sites_load(pb_ctx* ctx, int64_t na, const double* pos, const d
     PB_CUDA(cudaMemcpyAsync(s.quad, quad, sizeof(double) * 6 * na, cudaMemcpyDeviceToDevice, st));
     PB_CUDA(cudaMemcpyAsync(s.alpha, alpha, sizeof(double) * na, cudaMemcpyDeviceToDevice, st));
     PB_CUDA(cudaMemcpyAsync(s.group, group, sizeof(int32_t) * na, cudaMemcpyDeviceToDevice, st));
+    PB_TRY(pb_scratch(ctx, 1 << 20));
+    int* bad = (int*)ctx->scratch;
+    int hbad = 0;
+    PB_CUDA(cudaMemsetAsync(bad, 0, sizeof(int), st));
+    k_sites_check<<<pb_blocks(na, 256), 256, 0, st>>>(na, s.quad, s.alpha, bad);
+    PB_LAUNCH_CHECK();
+    PB_CUDA(cudaMemcpyAsync(&hbad, bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+    PB_CUDA(cudaStreamSynchronize(st));
+    if (hbad & 1) return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_sites_load: a quadrupole is not traceless (Eq. 7 / Eq. 20 convention, D: R-3)");
+    if (hbad & 2) return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_sites_load: negative or non-finite polarizability");
     s.loaded = true;
+    if (ctx->mesh_loaded) PB_TRY(pb_check_sites_inside(ctx));
     return PB_OK;
 }
 
@@ -300,6 +402,10 @@ extern "C" int pb_tree_build(pb_ctx* ctx)
     ctx->tree = pb_tree();
     ctx->sites.near_built = false;
         ctx->sites.tree_built = false;
+    ctx->attr_m2p_mask = 0;
+    ctx->attr_up_bytes = 0;
+    ctx->attr_site_bytes[0] = ctx->attr_site_bytes[1] = 0;
+    if (ctx->sites.loaded && !ctx->sites.inside_checked) PB_TRY(pb_check_sites_inside(ctx));
     PB_TRY(pb_upload_rules(ctx));
     PB_TRY(pb_tree_build_impl(ctx));
     PB_TRY(pb_farfield_setup(ctx));
@@ -347,6 +453,12 @@ extern "C" int pb_get_stats(pb_ctx* ctx, pb_stats* out)
     for (int i = 0; i < 8; ++i) out->last_matvec_ms[i] = ctx->last_ms[i];
     out->ncrit_used = t.ncrit_used;
     out->m2p_pairs_low = t.m2p_pairs_low;
+    out->covered_pairs = t.covered_pairs;
+    if (ctx->sites.tree_built) {
+        out->site_p2p_pairs = ctx->sites.t_p2p_pairs;
+        out->site_m2p_pairs = ctx->sites.t_m2p_pairs;
+        out->site_covered_pairs = ctx->sites.t_covered_pairs;
+    }
     return PB_OK;
 }
 

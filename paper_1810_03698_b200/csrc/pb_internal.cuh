@@ -84,6 +84,7 @@ struct pb_tree {
     int32_t* p2p_lo = nullptr;    // source-point ranges [lo, hi)
     int32_t* p2p_hi = nullptr;
     int64_t p2p_pairs = 0, m2p_pairs = 0, m2p_pairs_low = 0;   // m2p_pairs_low: those evaluated at order P - 2
+    int64_t covered_pairs = 0;    // (target, source point) pairs the STORED lists cover (k_cover_count); == N * Ns
     // far-field data
     int P = 0, Nk = 0, NT = 0;
     double* M = nullptr;          // [cells][2][Nk] Cartesian moments (V, K)
@@ -132,14 +133,16 @@ struct pb_sites {
     // near (site, panel) pairs for the reaction field (D: R-9); built lazily
     bool near_built = false;
     int64_t n_near = 0;
-    int32_t* near_site = nullptr;
+    int32_t* near_site = nullptr;  // pairs sorted by (site, panel): a site's corrections are added in a fixed order
     int32_t* near_panel = nullptr; // Morton index
+    int32_t* near_off = nullptr;   // [na + 1] a site's pairs are near_off[m] .. near_off[m + 1]
     // treecode for the reaction field (S: section 8(f) item 1): sites in Morton order, groups of 32, their lists,
     // and the cells whose moments those lists need (a second configuration of the upward pass)
     bool tree_built = false;
     int32_t* tperm = nullptr;      // [na] Morton position -> original site index
     double* tpos[3] = {0, 0, 0};   // [na] sorted positions (SoA)
-    int64_t t_groups = 0, t_m2p_total = 0, t_p2p_pairs = 0, t_m2p_pairs = 0;
+    int64_t t_groups = 0, t_m2p_total = 0, t_p2p_pairs = 0, t_m2p_pairs = 0, t_covered_pairs = 0;
+    bool inside_checked = false;   // every site has been found inside the loaded surface
     int32_t *t_m2p_off = nullptr, *t_m2p_cell = nullptr, *t_p2p_off = nullptr, *t_p2p_lo = nullptr, *t_p2p_hi = nullptr;
     int32_t* t_need_leaf = nullptr;
     int32_t* t_up_link = nullptr;
@@ -195,6 +198,11 @@ struct pb_ctx {
     size_t h_pinned_bytes = 0;
     int64_t matvec_calls = 0;
     int64_t launches = 0;         // kernels launched by this context
+    // cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is per device and per function: remembered per context
+    // (a context lives on one device), bit P for k_m2p2<P> / k_m2p<P>, byte counts for the others
+    uint32_t attr_m2p_mask = 0;
+    size_t attr_up_bytes = 0, attr_site_bytes[2] = {0, 0};
+    int dots_occ = 0;
     // profiling: CUDA-event pairs around every P2P and M2P launch (pb_set_profiling)
     bool profiling = false;
     std::vector<cudaEvent_t> prof_ev;   // ring: [slot][kernel 0=p2p,1=m2p][begin,end]
@@ -250,6 +258,12 @@ int pb_exclusive_scan_i32(pb_ctx* ctx, const int32_t* in, int32_t* out, int64_t 
 // pb_tree.cu
 int pb_tree_build_impl(pb_ctx* ctx);
 int pb_morton_order(pb_ctx* ctx, const double* pts, int64_t n, int cat, int32_t** perm_out, uint64_t** keys_out);
+// stable LSD radix sort of n (64-bit key, int32 value) pairs on the context's stream; `bits` key bits are sorted
+// (rounded up to whole bytes); k1 / v1 are scratch of the same size; the result is in (*kout, *vout) = (k0, v0) or (k1, v1)
+int pb_radix_sort(pb_ctx* ctx, uint64_t* k0, uint64_t* k1, int32_t* v0, int32_t* v1, int64_t n, int bits,
+                  uint64_t** kout, int32_t** vout);
+int pb_cover_count(pb_ctx* ctx, int64_t G, int tg, int64_t ntargets, const int32_t* m2p_off, const int32_t* m2p_cell,
+                   const int32_t* p2p_off, const int32_t* p2p_lo, const int32_t* p2p_hi, int64_t* out_host);
 int pb_site_lists_build(pb_ctx* ctx);
 // pb_sitetree.cu
 int pb_site_tree_build(pb_ctx* ctx);
@@ -268,6 +282,7 @@ void pb_make_expk(double kappa, pb_expk* out);
 int pb_make_expk8(pb_ctx* ctx, double kappa, pb_expk8* out);
 // pb_sites.cu
 int pb_site_near_build(pb_ctx* ctx);
+int pb_check_sites_inside(pb_ctx* ctx);   // PB_ERR_BAD_MESH when a site lies outside the loaded surface
 int pb_multipole_field_impl(pb_ctx* ctx, const double* mu, int parts, int use_mask, double* phi, double* grad, double* hess);
 // pb_api.cu: profiling ring
 int pb_prof_begin(pb_ctx* ctx, int kernel);

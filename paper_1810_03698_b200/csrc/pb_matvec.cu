@@ -78,17 +78,21 @@ int pb_farfield_setup(pb_ctx* ctx)
     t.Nk = pb_nk(P);
     t.NT = pb_nt(P);
     if (ctx->prm.theta <= 0.0) return PB_OK;   // direct mode: no far field
-    // exponent tables
+    // exponent tables.  mom_index grades by total degree, so the table of order PB_MAX_P contains the table of every
+    // lower order as a prefix: the SAME bytes are uploaded whatever this context's P is, and contexts of different
+    // order on one device (a binding triple) cannot disturb one another.  (Constant memory is per device; c_T256
+    // below is likewise independent of kappa.)
     unsigned char ka[PB_MAX_NK], kb[PB_MAX_NK], kc[PB_MAX_NK];
-    for (int a = 0; a <= P; ++a)
-        for (int b = 0; b <= P - a; ++b)
-            for (int c = 0; c <= P - a - b; ++c) {
+    for (int a = 0; a <= PB_MAX_P; ++a)
+        for (int b = 0; b <= PB_MAX_P - a; ++b)
+            for (int c = 0; c <= PB_MAX_P - a - b; ++c) {
                 int k = mom_index(a, b, c);
                 ka[k] = (unsigned char)a; kb[k] = (unsigned char)b; kc[k] = (unsigned char)c;
             }
-    PB_CUDA(cudaMemcpyToSymbolAsync(c_ka, ka, t.Nk, 0, cudaMemcpyHostToDevice, st));
-    PB_CUDA(cudaMemcpyToSymbolAsync(c_kb, kb, t.Nk, 0, cudaMemcpyHostToDevice, st));
-    PB_CUDA(cudaMemcpyToSymbolAsync(c_kc, kc, t.Nk, 0, cudaMemcpyHostToDevice, st));
+    PB_CUDA(cudaMemcpyToSymbolAsync(c_ka, ka, PB_MAX_NK, 0, cudaMemcpyHostToDevice, st));
+    PB_CUDA(cudaMemcpyToSymbolAsync(c_kb, kb, PB_MAX_NK, 0, cudaMemcpyHostToDevice, st));
+    PB_CUDA(cudaMemcpyToSymbolAsync(c_kc, kc, PB_MAX_NK, 0, cudaMemcpyHostToDevice, st));
+    PB_CUDA(cudaStreamSynchronize(st));   // ka, kb, kc live on this stack frame
     // conversion table M -> F, entries in the order the M2P kernel consumes them
     std::vector<int32_t> off, idx, expo;
     std::vector<double> coef;
@@ -1137,11 +1141,10 @@ template <int P>
 static cudaError_t launch_m2p2(pb_ctx* ctx, cudaStream_t fs)
 {
     pb_tree& t = ctx->tree;
-    static bool attr_set = false;   // per instantiation; the attribute belongs to the function, not the context
-    if (!attr_set) {
+    if (!(ctx->attr_m2p_mask & (1u << P))) {   // per device and function: remembered per context (D: section 1)
         cudaError_t e = cudaFuncSetAttribute(k_m2p2<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m2q_cfg<P>::SMEM);
         if (e != cudaSuccess) return e;
-        attr_set = true;
+        ctx->attr_m2p_mask |= 1u << P;
     }
     k_m2p2<P><<<(unsigned)t.n_itemM, M2Q_THREADS, m2q_cfg<P>::SMEM, fs>>>(
         t.N, ctx->prm.kappa, t.ek, t.itemM, t.m2p_cell, t.m2p_ctr, t.FF, t.pc[0], t.pc[1], t.pc[2], t.accM);
@@ -1152,11 +1155,10 @@ template <int P>
 static cudaError_t launch_m2p(pb_ctx* ctx, cudaStream_t fs)
 {
     pb_tree& t = ctx->tree;
-    static bool attr_set = false;   // per instantiation; the attribute belongs to the function, not the context
-    if (!attr_set) {
+    if (!(ctx->attr_m2p_mask & (1u << P))) {
         cudaError_t e = cudaFuncSetAttribute(k_m2p<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m2p_cfg<P>::SMEM);
         if (e != cudaSuccess) return e;
-        attr_set = true;
+        ctx->attr_m2p_mask |= 1u << P;
     }
     k_m2p<P><<<(unsigned)t.n_itemM, M2P_THREADS, m2p_cfg<P>::SMEM, fs>>>(
         t.N, ctx->prm.kappa, t.ek, t.itemM, t.m2p_cell, t.m2p_ctr, t.FF, t.pc[0], t.pc[1], t.pc[2], t.accM);
@@ -1179,10 +1181,9 @@ int pb_upward(pb_ctx* ctx, cudaStream_t fs, const int32_t* leaf_ids, int64_t n_l
     ua.cv_off = t.cv_off; ua.cv_idx = t.cv_idx; ua.cv_coef = t.cv_coef;
     ua.M = t.M; ua.FF = t.FF;
     const size_t sm = up_smem_bytes(t.Nk);
-    static size_t sm_set = 0;                       // the attribute belongs to the function, not the context
-    if (sm > 48 * 1024 && sm > sm_set) {
+    if (sm > 48 * 1024 && sm > ctx->attr_up_bytes) {   // per device: remembered per context
         PB_CUDA(cudaFuncSetAttribute(k_upward, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-        sm_set = sm;
+        ctx->attr_up_bytes = sm;
     }
     k_upward<<<(unsigned)n_leaf, UP_THREADS, sm, fs>>>(ua);
     PB_LAUNCH_CHECK();

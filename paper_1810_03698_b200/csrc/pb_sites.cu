@@ -5,6 +5,87 @@
 #include <math.h>
 #include "pb_internal.cuh"
 
+// ---- every site inside the surface (interior problem of Eq. (1); S: section 8(b)) ---------------------
+// Solid angle of the closed surface seen from the site, one-point rule per panel:
+//   Omega_m = sum_j (A_j n_j).(c_j - r_m) / (4 pi |c_j - r_m|^3)  = 1 inside, 0 outside.
+__global__ void k_area_normals(int64_t nt, const double* __restrict__ verts, const int32_t* __restrict__ tris, double* __restrict__ an)
+{
+    const int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (j >= nt) return;
+    const double* a = verts + 3 * (int64_t)tris[3 * j];
+    const double* b = verts + 3 * (int64_t)tris[3 * j + 1];
+    const double* c = verts + 3 * (int64_t)tris[3 * j + 2];
+    const double e1[3] = {b[0] - a[0], b[1] - a[1], b[2] - a[2]}, e2[3] = {c[0] - a[0], c[1] - a[1], c[2] - a[2]};
+    an[3 * j] = 0.5 * (e1[1] * e2[2] - e1[2] * e2[1]);
+    an[3 * j + 1] = 0.5 * (e1[2] * e2[0] - e1[0] * e2[2]);
+    an[3 * j + 2] = 0.5 * (e1[0] * e2[1] - e1[1] * e2[0]);
+}
+
+#define IN_ST 8
+__global__ void __launch_bounds__(256)
+k_sites_inside(int64_t na, int64_t nt, const double* __restrict__ pos, const double* __restrict__ cen,
+               const double* __restrict__ an, int* __restrict__ first_bad)
+{
+    __shared__ double red[8][IN_ST];
+    const int64_t m0 = (int64_t)blockIdx.x * IN_ST;
+    double r[IN_ST][3], acc[IN_ST];
+#pragma unroll
+    for (int t = 0; t < IN_ST; ++t) {
+        const int64_t m = m0 + t < na ? m0 + t : na - 1;
+        r[t][0] = pos[3 * m]; r[t][1] = pos[3 * m + 1]; r[t][2] = pos[3 * m + 2];
+        acc[t] = 0.0;
+    }
+    for (int64_t j = threadIdx.x; j < nt; j += 256) {
+        const double cx = cen[3 * j], cy = cen[3 * j + 1], cz = cen[3 * j + 2];
+        const double ax = an[3 * j], ay = an[3 * j + 1], az = an[3 * j + 2];
+#pragma unroll
+        for (int t = 0; t < IN_ST; ++t) {
+            const double dx = cx - r[t][0], dy = cy - r[t][1], dz = cz - r[t][2];
+            const double r2 = dx * dx + dy * dy + dz * dz;
+            const double ri = r2 > 0.0 ? rsqrt(r2) : 0.0;
+            acc[t] += (ax * dx + ay * dy + az * dz) * ri * ri * ri;
+        }
+    }
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+    for (int t = 0; t < IN_ST; ++t) {
+        double v = acc[t];
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) red[w][t] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < IN_ST && m0 + threadIdx.x < na) {
+        double v = 0;
+        for (int k = 0; k < 8; ++k) v += red[k][threadIdx.x];
+        if (!(v * PB_INV4PI > 0.5)) atomicMin(first_bad, (int)(m0 + threadIdx.x));
+    }
+}
+
+int pb_check_sites_inside(pb_ctx* ctx)
+{
+    pb_sites& s = ctx->sites;
+    cudaStream_t st = ctx->stream;
+    if (!ctx->mesh_loaded || !s.loaded) return PB_OK;
+    double* an;
+    PB_TRY(pb_dalloc_t(ctx, &an, 3 * ctx->nt, CAT_TMP));
+    PB_TRY(pb_scratch(ctx, 1 << 20));
+    int* bad = (int*)ctx->scratch;
+    const int none = 2147483647;
+    int hbad = none;
+    PB_CUDA(cudaMemcpyAsync(bad, &none, sizeof(int), cudaMemcpyHostToDevice, st));
+    k_area_normals<<<pb_blocks(ctx->nt, 256), 256, 0, st>>>(ctx->nt, ctx->verts, ctx->tris, an);
+    PB_LAUNCH_CHECK();
+    k_sites_inside<<<pb_blocks(s.na, IN_ST), 256, 0, st>>>(s.na, ctx->nt, s.pos, ctx->cen, an, bad);
+    PB_LAUNCH_CHECK();
+    PB_CUDA(cudaMemcpyAsync(&hbad, bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+    PB_CUDA(cudaStreamSynchronize(st));
+    pb_dfree_cat(ctx, CAT_TMP);
+    if (hbad != none)
+        return pb_fail(ctx, PB_ERR_BAD_MESH, "site %d lies outside the surface (solid angle below 2 pi): the multipoles must be inside (P:40-47)", hbad);
+    s.inside_checked = true;
+    return PB_OK;
+}
+
 // ---- H10: right-hand side -----------------------------------------------------------------------------
 // b_i = 1/(4 pi eps_in) sum_k [ q_k/R + p_k.d/R^3 + d.Q_k.d/(2 R^5) ],  d = c_i - r_k,  p = dip + mu.
 // Two collocation points per thread: every site value read from shared memory feeds two pairs.
@@ -195,6 +276,24 @@ __global__ void k_site_near_find(int64_t N, int64_t na, double tau, const double
     if (!PASS) cnt[j] = n;
 }
 
+__global__ void k_near_keys(int64_t np, const int32_t* __restrict__ psite, const int32_t* __restrict__ ppanel,
+                            uint64_t* __restrict__ keys, int32_t* __restrict__ vals, int32_t* __restrict__ cnt)
+{
+    const int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (e >= np) return;
+    keys[e] = ((uint64_t)(uint32_t)psite[e] << 32) | (uint32_t)ppanel[e];
+    vals[e] = (int32_t)e;
+    atomicAdd(&cnt[psite[e]], 1);                     // integer counts: order does not matter
+}
+
+__global__ void k_near_unpack(int64_t np, const uint64_t* __restrict__ keys, int32_t* __restrict__ psite, int32_t* __restrict__ ppanel)
+{
+    const int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (e >= np) return;
+    psite[e] = (int32_t)(keys[e] >> 32);
+    ppanel[e] = (int32_t)(keys[e] & 0xffffffffu);
+}
+
 int pb_site_near_build(pb_ctx* ctx)
 {
     pb_tree& t = ctx->tree;
@@ -215,10 +314,30 @@ int pb_site_near_build(pb_ctx* ctx)
     s.n_near = np;
     PB_TRY(pb_dalloc_t(ctx, &s.near_site, np, CAT_SITE_NEAR));
     PB_TRY(pb_dalloc_t(ctx, &s.near_panel, np, CAT_SITE_NEAR));
+    PB_TRY(pb_dalloc_t(ctx, &s.near_off, s.na + 1, CAT_SITE_NEAR));
     if (np > 0) {
         k_site_near_find<1><<<pb_blocks(t.N, 128), 128, 0, st>>>(t.N, s.na, ctx->prm.near_tau, t.pc[0], t.pc[1], t.pc[2],
                                                                 t.parea, s.pos, cnt, off, s.near_site, s.near_panel);
         PB_LAUNCH_CHECK();
+        // sort the pairs by (site, panel): each site's corrections are then added in a fixed order by one thread
+        // (no floating-point atomics: the reaction field is bitwise repeatable)
+        uint64_t *k0, *k1, *ks;
+        int32_t *v0, *v1, *vs, *scnt;
+        PB_TRY(pb_dalloc_t(ctx, &k0, np, CAT_TMP));
+        PB_TRY(pb_dalloc_t(ctx, &k1, np, CAT_TMP));
+        PB_TRY(pb_dalloc_t(ctx, &v0, np, CAT_TMP));
+        PB_TRY(pb_dalloc_t(ctx, &v1, np, CAT_TMP));
+        PB_TRY(pb_dalloc_t(ctx, &scnt, s.na + 1, CAT_TMP));
+        PB_CUDA(cudaMemsetAsync(scnt, 0, sizeof(int32_t) * (s.na + 1), st));
+        k_near_keys<<<pb_blocks(np, 256), 256, 0, st>>>(np, s.near_site, s.near_panel, k0, v0, scnt);
+        PB_LAUNCH_CHECK();
+        int abits = 1;
+        while (((int64_t)1 << abits) < s.na) ++abits;
+        PB_TRY(pb_radix_sort(ctx, k0, k1, v0, v1, np, 32 + abits, &ks, &vs));
+        k_near_unpack<<<pb_blocks(np, 256), 256, 0, st>>>(np, ks, s.near_site, s.near_panel);
+        PB_LAUNCH_CHECK();
+        int64_t tot = 0;
+        PB_TRY(pb_exclusive_scan_i32(ctx, scnt, s.near_off, s.na + 1, &tot));   // synchronises
     }
     s.near_built = true;
     return PB_OK;
@@ -233,7 +352,7 @@ struct rf_corr_args {
     const double* pv[9];
     const double *nx, *ny, *nz, *parea, *xphi, *xdphi;
     const double4* srec;
-    double *phi, *grad, *hess;
+    double* corr;                 // [np][10] the pairs' corrections (phi, grad, hess), pairs sorted by site
 };
 
 __global__ void k_reaction_corr(rf_corr_args a, pb_rule_t ruleN)
@@ -258,11 +377,24 @@ __global__ void k_reaction_corr(rf_corr_args a, pb_rule_t ruleN)
         const double4 ra = a.srec[2 * s], rb = a.srec[2 * s + 1];
         react_point<true>(r[0] - ra.x, r[1] - ra.y, r[2] - ra.z, ra.w, rb.x, rb.y, rb.z, coarse);
     }
-    if (a.phi) atomicAdd(&a.phi[m], PB_INV4PI * (fine[0] - coarse[0]));
-    if (a.grad)
-        for (int c = 0; c < 3; ++c) atomicAdd(&a.grad[3 * m + c], PB_INV4PI * (fine[1 + c] - coarse[1 + c]));
-    if (a.hess)
-        for (int c = 0; c < 6; ++c) atomicAdd(&a.hess[6 * m + c], PB_INV4PI * (fine[4 + c] - coarse[4 + c]));
+    for (int c = 0; c < 10; ++c) a.corr[10 * e + c] = PB_INV4PI * (fine[c] - coarse[c]);
+}
+
+// thread (site, component): the site's corrections in the order of its (panel-sorted) pair list
+__global__ void k_reaction_corr_add(int64_t na, const int32_t* __restrict__ off, const double* __restrict__ corr,
+                                    double* __restrict__ phi, double* __restrict__ grad, double* __restrict__ hess)
+{
+    const int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (g >= na * 10) return;
+    const int64_t m = g / 10;
+    const int c = (int)(g - 10 * m);
+    const int32_t e0 = off[m], e1 = off[m + 1];
+    if (e0 == e1) return;
+    double* dst = c == 0 ? (phi ? phi + m : nullptr) : (c < 4 ? (grad ? grad + 3 * m + c - 1 : nullptr) : (hess ? hess + 6 * m + c - 4 : nullptr));
+    if (!dst) return;
+    double v = *dst;
+    for (int32_t e = e0; e < e1; ++e) v += corr[10 * (int64_t)e + c];
+    *dst = v;
 }
 
 extern "C" int pb_reaction_field(pb_ctx* ctx, const double* x, double* phi, double* grad, double* hess)
@@ -312,8 +444,12 @@ extern "C" int pb_reaction_field(pb_ctx* ctx, const double* x, double* phi, doub
         for (int k = 0; k < 9; ++k) a.pv[k] = t.pv[k];
         a.nx = t.pn[0]; a.ny = t.pn[1]; a.nz = t.pn[2]; a.parea = t.parea; a.xphi = t.xphi; a.xdphi = t.xdphi;
         a.srec = t.srec;
-        a.phi = phi; a.grad = grad; a.hess = hess;
+        // the direct / treecode sum above is finished with the scratch area (its finish kernel is enqueued before this)
+        PB_TRY(pb_scratch(ctx, (size_t)s.n_near * 10 * sizeof(double) + 4096));
+        a.corr = ctx->scratch;
         k_reaction_corr<<<pb_blocks(s.n_near, 64), 64, 0, st>>>(a, ctx->ruleN);
+        PB_LAUNCH_CHECK();
+        k_reaction_corr_add<<<pb_blocks(s.na * 10, 128), 128, 0, st>>>(s.na, s.near_off, a.corr, phi, grad, hess);
         PB_LAUNCH_CHECK();
     }
     return PB_OK;

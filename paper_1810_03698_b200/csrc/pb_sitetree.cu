@@ -252,7 +252,7 @@ int pb_reaction_field_tree(pb_ctx* ctx, double* phi, double* grad, double* hess)
     double* farp = ctx->scratch + (size_t)s.na * 10;
     PB_TRY(pb_upward(ctx, st, s.t_need_leaf, s.t_n_need_leaf, s.t_up_link));
     const size_t sm = (size_t)pb_nk(t.P + 2) * ST_GROUP * sizeof(double);
-    static size_t sm_set[2] = {0, 0};
+    size_t* sm_set = ctx->attr_site_bytes;             // per device: remembered per context
     if (sm > 48 * 1024 && sm > sm_set[H ? 1 : 0]) {
         if (H) PB_CUDA(cudaFuncSetAttribute(k_site_m2p<10>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
         else PB_CUDA(cudaFuncSetAttribute(k_site_m2p<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));

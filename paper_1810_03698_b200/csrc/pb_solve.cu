@@ -446,7 +446,7 @@ static int dot_into(pb_ctx* ctx, gmres_ws& ws, int nv, const double* V, const do
         dim3 grid((unsigned)nchunk, (unsigned)gy1);
         k_dots<1><<<grid, DOT_THREADS, 0, ctx->stream>>>(ws.n, nv, V, ws.n, w, self ? 1 : 0, ws.partial, ws.counter, hout);
     } else {                                              // long vectors: two full waves of resident blocks (bandwidth)
-        static int occ = 0;
+        int& occ = ctx->dots_occ;                          // per device: remembered per context
         if (occ == 0) {
             PB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_dots<4>, DOT_THREADS, 0));
             if (occ < 1) occ = 1;
@@ -578,7 +578,7 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
         if (iters >= maxit) { rc = PB_ERR_NO_CONVERGENCE; break; }
         std::fill(g.begin(), g.end(), 0.0);
         g[0] = beta;
-        bool accepted = false;
+        bool accepted = false, breakdown = false;
         int j = 0;
         for (; j < m && iters < maxit;) {
             const double* vj = ws.V + (size_t)j * n;
@@ -636,7 +636,9 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
                 col[i] = a;
             }
             double den = hypot(col[j], col[j + 1]);
-            if (den == 0.0) { ++j; ++iters; break; }
+            // exact breakdown (the new column is zero: A Minv v_j lies in nothing, singular operator): drop the column,
+            // keep the update from the j columns before it and report no convergence
+            if (den == 0.0) { breakdown = true; break; }
             cs[j] = col[j] / den;
             sn[j] = col[j + 1] / den;
             col[j] = den;
@@ -682,6 +684,7 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
         // residual norm to rounding, so no further operator application is spent on confirming it.  After a
         // restart (no convergence within m steps) the loop recomputes the true residual as the new start.
         if (accepted) break;
+        if (breakdown) { rc = PB_ERR_NO_CONVERGENCE; break; }
     }
     if (iters_out) *iters_out = iters;
     if (relres_out) *relres_out = relres;

@@ -484,6 +484,75 @@ static int pb_build_items(pb_ctx* ctx, int64_t G, const int32_t* off, const int3
     return PB_OK;
 }
 
+int pb_radix_sort(pb_ctx* ctx, uint64_t* k0, uint64_t* k1, int32_t* v0, int32_t* v1, int64_t n, int bits,
+                  uint64_t** kout, int32_t** vout)
+{
+    cudaStream_t st = ctx->stream;
+    const int64_t nwt = (n + RS_TILE - 1) / RS_TILE;
+    int32_t* hist;
+    PB_TRY(pb_dalloc_t(ctx, &hist, 256 * (nwt > 0 ? nwt : 1), CAT_TMP));
+    const int nb = (int)((nwt + RS_WARPS - 1) / RS_WARPS);
+    uint64_t *ka = k0, *kb = k1;
+    int32_t *va = v0, *vb = v1;
+    const int npass = (bits + 7) / 8;
+    for (int pass = 0; pass < npass && n > 0; ++pass) {
+        const int shift = 8 * pass;
+        k_rs_hist<<<nb, 32 * RS_WARPS, 0, st>>>(ka, n, shift, nwt, hist);
+        PB_LAUNCH_CHECK();
+        PB_TRY(pb_exclusive_scan_i32(ctx, hist, hist, 256 * nwt, nullptr));
+        k_rs_scatter<<<nb, 32 * RS_WARPS, 0, st>>>(ka, va, kb, vb, n, shift, nwt, hist);
+        PB_LAUNCH_CHECK();
+        uint64_t* tk = ka; ka = kb; kb = tk;
+        int32_t* tv = va; va = vb; vb = tv;
+    }
+    *kout = ka;
+    *vout = va;
+    return PB_OK;
+}
+
+// ---- exact-cover count of STORED lists (pb_stats.covered_pairs) ------------------------------------------------
+// One thread per target group walks the lists exactly as the matvec kernels will read them: source points of the
+// P2P ranges plus source points of the M2P cells, times the number of targets in the group.
+__global__ void k_cover_count(int64_t G, int tg, int64_t ntargets, int K, const int32_t* __restrict__ m2p_off,
+                              const int32_t* __restrict__ m2p_cell, const int32_t* __restrict__ c_first,
+                              const int32_t* __restrict__ c_last, const int32_t* __restrict__ p2p_off,
+                              const int32_t* __restrict__ p2p_lo, const int32_t* __restrict__ p2p_hi,
+                              unsigned long long* __restrict__ out)
+{
+    const int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    unsigned long long v = 0;
+    if (g < G) {
+        unsigned long long pts = 0;
+        for (int32_t r = p2p_off[g]; r < p2p_off[g + 1]; ++r) pts += (unsigned long long)(p2p_hi[r] - p2p_lo[r]);
+        for (int32_t e = m2p_off[g]; e < m2p_off[g + 1]; ++e) {
+            const int32_t c = m2p_cell[e];
+            pts += (unsigned long long)(c_last[c] - c_first[c]) * (unsigned long long)K;
+        }
+        const int64_t i0 = g * tg;
+        v = pts * (unsigned long long)(i0 + tg <= ntargets ? tg : ntargets - i0);
+    }
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0 && v) atomicAdd(out, v);     // integer sum: order does not matter
+}
+
+int pb_cover_count(pb_ctx* ctx, int64_t G, int tg, int64_t ntargets, const int32_t* m2p_off, const int32_t* m2p_cell,
+                   const int32_t* p2p_off, const int32_t* p2p_lo, const int32_t* p2p_hi, int64_t* out_host)
+{
+    pb_tree& t = ctx->tree;
+    cudaStream_t st = ctx->stream;
+    PB_TRY(pb_scratch(ctx, 1 << 20));
+    unsigned long long* d = (unsigned long long*)ctx->scratch;
+    PB_CUDA(cudaMemsetAsync(d, 0, sizeof(unsigned long long), st));
+    k_cover_count<<<pb_blocks(G, 128), 128, 0, st>>>(G, tg, ntargets, t.K, m2p_off, m2p_cell, t.c_first, t.c_last, p2p_off,
+                                                    p2p_lo, p2p_hi, d);
+    PB_LAUNCH_CHECK();
+    unsigned long long h = 0;
+    PB_CUDA(cudaMemcpyAsync(&h, d, sizeof(h), cudaMemcpyDeviceToHost, st));
+    PB_CUDA(cudaStreamSynchronize(st));
+    *out_host = (int64_t)h;
+    return PB_OK;
+}
+
 // Morton order of n points [n][3]: perm (allocated in category `cat`) = indices sorted by the 63-bit key
 // inside the points' bounding cube; keys_out (optional) = the sorted keys, allocated in CAT_TMP.
 int pb_morton_order(pb_ctx* ctx, const double* pts, int64_t n, int cat, int32_t** perm_out, uint64_t** keys_out)
@@ -501,23 +570,11 @@ int pb_morton_order(pb_ctx* ctx, const double* pts, int64_t n, int cat, int32_t*
     PB_TRY(pb_dalloc_t(ctx, &v1, n, CAT_TMP));
     k_morton<<<pb_blocks(n, 256), 256, 0, st>>>(n, pts, box, k0, v0);
     PB_LAUNCH_CHECK();
-    const int64_t nwt = (n + RS_TILE - 1) / RS_TILE;
-    int32_t* hist;
-    PB_TRY(pb_dalloc_t(ctx, &hist, 256 * nwt, CAT_TMP));
-    const int nb = (int)((nwt + RS_WARPS - 1) / RS_WARPS);
-    uint64_t *ka = k0, *kb = k1;
-    int32_t *va = v0, *vb = v1;
-    for (int pass = 0; pass < 8; ++pass) {
-        const int shift = 8 * pass;
-        k_rs_hist<<<nb, 32 * RS_WARPS, 0, st>>>(ka, n, shift, nwt, hist);
-        PB_LAUNCH_CHECK();
-        PB_TRY(pb_exclusive_scan_i32(ctx, hist, hist, 256 * nwt, nullptr));
-        k_rs_scatter<<<nb, 32 * RS_WARPS, 0, st>>>(ka, va, kb, vb, n, shift, nwt, hist);
-        PB_LAUNCH_CHECK();
-        uint64_t* tk = ka; ka = kb; kb = tk;
-        int32_t* tv = va; va = vb; vb = tv;
-    }
+    uint64_t* ks;
+    int32_t* vs;
+    PB_TRY(pb_radix_sort(ctx, k0, k1, v0, v1, n, 64, &ks, &vs));
     // 8 passes: the result is back in (k0, v0)
+    if (ks != k0 || vs != v0) return pb_fail(ctx, PB_ERR_INVALID_ARG, "internal: radix sort buffer parity");
     *perm_out = v0;
     if (keys_out) *keys_out = k0;
     return PB_OK;
@@ -687,6 +744,7 @@ int pb_tree_build_impl(pb_ctx* ctx)
     a.m2p_low = m2p_low;
     k_lists<1, 2><<<pb_blocks(G, LIST_WARPS), LIST_WARPS * 32, 0, st>>>(a);
     PB_LAUNCH_CHECK();
+    PB_TRY(pb_cover_count(ctx, G, PB_TG, N, t.m2p_off, t.m2p_cell, t.p2p_off, t.p2p_lo, t.p2p_hi, &t.covered_pairs));
     PB_TRY(pb_dalloc_t(ctx, &t.m2p_ctr, tot_m > 0 ? tot_m : 1, CAT_TREE));
     if (tot_m > 0) {
         k_m2p_centres<<<pb_blocks(tot_m, 256), 256, 0, st>>>(tot_m, t.m2p_cell, m2p_low, t.c_ctr[0], t.c_ctr[1], t.c_ctr[2], t.m2p_ctr);
@@ -783,5 +841,6 @@ int pb_site_lists_build(pb_ctx* ctx)
     a.n_m2p = s.t_m2p_off; a.n_p2p = s.t_p2p_off; a.m2p_cell = s.t_m2p_cell; a.p2p_lo = s.t_p2p_lo; a.p2p_hi = s.t_p2p_hi;
     k_lists<1, 1><<<pb_blocks(G, LIST_WARPS), LIST_WARPS * 32, 0, st>>>(a);
     PB_LAUNCH_CHECK();
+    PB_TRY(pb_cover_count(ctx, G, 32, na, s.t_m2p_off, s.t_m2p_cell, s.t_p2p_off, s.t_p2p_lo, s.t_p2p_hi, &s.t_covered_pairs));
     return PB_OK;
 }

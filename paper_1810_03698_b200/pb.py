@@ -45,7 +45,7 @@ class Params(ctypes.Structure):
         ("nq_edge", ctypes.c_int32), ("precond", ctypes.c_int32), ("gmres_tol", ctypes.c_double),
         ("gmres_restart", ctypes.c_int32), ("gmres_maxit", ctypes.c_int32), ("scf_tol_debye", ctypes.c_double),
         ("scf_omega", ctypes.c_double), ("scf_maxit", ctypes.c_int32), ("site_treecode", ctypes.c_int32),
-        ("thole_a", ctypes.c_double),
+        ("thole_a", ctypes.c_double), ("rhs_treecode", ctypes.c_int32), ("reserved0", ctypes.c_int32),
     ]
 
 
@@ -77,6 +77,9 @@ class Stats(ctypes.Structure):
         ("prof_p2p_ms", ctypes.c_double), ("prof_m2p_ms", ctypes.c_double),
         ("last_matvec_ms", ctypes.c_double * 8),
         ("ncrit_used", ctypes.c_int64), ("m2p_pairs_low", ctypes.c_int64),
+        ("covered_pairs", ctypes.c_int64), ("site_p2p_pairs", ctypes.c_int64), ("site_m2p_pairs", ctypes.c_int64),
+        ("site_covered_pairs", ctypes.c_int64), ("rhs_p2p_pairs", ctypes.c_int64), ("rhs_m2p_pairs", ctypes.c_int64),
+        ("rhs_covered_pairs", ctypes.c_int64),
     ]
 
     def as_dict(self):
@@ -88,13 +91,29 @@ class Stats(ctypes.Structure):
 
 def build(force: bool = False, verbose: bool = False) -> str:
     """Compile csrc/*.cu for sm_100a into libpb_b200.so next to this file (nvcc cross-compiles
-    without a GPU)."""
+    without a GPU).  One object per source, compiled in parallel and only when the source or a header
+    is newer than the object; the objects live in build/ (git-ignored)."""
+    import glob
+    from concurrent.futures import ThreadPoolExecutor
     srcs = [os.path.join(_CSRC, s) for s in SOURCES]
-    deps = srcs + [os.path.join(_CSRC, "pb_internal.cuh"), os.path.join(_HERE, "..", "include", "pb.h")]
+    hdrs = sorted(glob.glob(os.path.join(_CSRC, "*.cuh"))) + [os.path.join(_HERE, "..", "include", "pb.h")]
+    deps = srcs + hdrs
     if not force and os.path.exists(LIB_PATH) and all(os.path.getmtime(LIB_PATH) >= os.path.getmtime(d) for d in deps):
         return LIB_PATH
-    cmd = ["nvcc"] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB_PATH] + srcs
-    subprocess.check_call(cmd)
+    bdir = os.path.join(_HERE, "build")
+    os.makedirs(bdir, exist_ok=True)
+    hnew = max(os.path.getmtime(h) for h in hdrs)
+    cflags = [f for f in NVCC_FLAGS if f != "-shared"] + (["-Xptxas", "-v"] if verbose else [])
+
+    def compile_one(src):
+        obj = os.path.join(bdir, os.path.basename(src)[:-3] + ".o")
+        if force or not os.path.exists(obj) or os.path.getmtime(obj) < max(os.path.getmtime(src), hnew):
+            subprocess.check_call(["nvcc"] + cflags + ["-c", "-o", obj, src])
+        return obj
+
+    with ThreadPoolExecutor(max_workers=min(len(srcs), os.cpu_count() or 1)) as ex:
+        objs = list(ex.map(compile_one, srcs))
+    subprocess.check_call(["nvcc"] + NVCC_FLAGS + ["-o", LIB_PATH] + objs)
     return LIB_PATH
 
 

@@ -129,5 +129,51 @@ CONFIGS = {
 }
 
 
+def _cache_dir():
+    """Generated globule workloads (C2-C4: 1-60 s of surface netting each) are kept as .npz files in a scratch
+    directory outside the repository -- PB_WORKLOAD_CACHE, default /tmp/paper_1810_03698_b200_workloads; set it to
+    an empty string to switch the cache off.  The file name carries a hash of the generator sources, the config and
+    its arguments, so a changed recipe never reads a stale file; nothing depends on the cache being there."""
+    import os
+    d = os.environ.get("PB_WORKLOAD_CACHE", "/tmp/paper_1810_03698_b200_workloads")
+    return d or None
+
+
+def _cache_key(name, kw):
+    import hashlib
+    import os
+    h = hashlib.sha256()
+    here = os.path.dirname(os.path.abspath(__file__))
+    for f in ("configs.py", "meshes.py", "solutes.py"):
+        with open(os.path.join(here, f), "rb") as fh:
+            h.update(fh.read())
+    h.update(repr((name, sorted(kw.items()), np.__version__)).encode())
+    return h.hexdigest()[:20]
+
+
 def make_config(name: str, **kw) -> Workload:
-    return CONFIGS[name](**kw)
+    import os
+    d = _cache_dir() if name in ("C2", "C3", "C4") else None
+    path = os.path.join(d, f"{name}-{_cache_key(name, kw)}.npz") if d else None
+    if path and os.path.exists(path):
+        try:
+            import json
+            z = np.load(path, allow_pickle=False)
+            meta = json.loads(str(z["meta"]))
+            sites = {k[5:]: z[k] for k in z.files if k.startswith("site_")}
+            return Workload(meta["name"], z["verts"], z["tris"], sites, meta["params"], meta["info"])
+        except Exception:
+            pass                                     # unreadable file: regenerate
+    w = CONFIGS[name](**kw)
+    if path:
+        try:
+            import json
+            os.makedirs(d, exist_ok=True)
+            info = {k: (v.item() if hasattr(v, "item") else v) for k, v in w.info.items()}
+            meta = json.dumps(dict(name=w.name, params=w.params, info=info), default=float)
+            tmp = f"{path}.{os.getpid()}.tmp.npz"
+            np.savez(tmp, verts=w.verts, tris=w.tris, meta=np.array(meta), **{"site_" + k: v for k, v in w.sites.items()})
+            os.replace(tmp, path)
+        except Exception:
+            pass                                     # read-only or full scratch space: the cache is optional
+    return w

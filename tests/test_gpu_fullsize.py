@@ -12,7 +12,15 @@ TOL_TREE = 1e-4
 
 
 def rel(a, b):
-    return float(np.linalg.norm(np.asarray(a) - np.asarray(b)) / np.linalg.norm(np.asarray(b)))
+    """Relative error in BOTH norms, the larger of the two: ||a - b||_2 / ||b||_2 (BASELINE.json's stated norm) and
+    max|a - b| / max|b| (so that one bad row among 10^4-10^6 cannot hide under the L2 bound).  Rounding-level
+    comparisons (direct mode, <= 1e-11) take the max norm at face value; for truncation-level ones (treecode, 1e-4:
+    the far-field error is not uniform over the rows) the max norm is allowed twice the L2 bound."""
+    a, b = np.asarray(a, dtype=float), np.asarray(b, dtype=float)
+    d = a - b
+    l2 = float(np.linalg.norm(d) / np.linalg.norm(b))
+    linf = float(np.max(np.abs(d)) / np.max(np.abs(b))) if d.size else 0.0
+    return max(l2, linf if l2 < 1e-9 else 0.5 * linf)
 
 
 @pytest.fixture(scope="module")
@@ -35,10 +43,12 @@ def _rows(nt, n, seed=8):
 
 
 @pytest.mark.parametrize("name,kw,nrows,direct", [
+    ("C1", dict(), None, True),                      # 5,120 panels: every row, both modes
     ("C2", dict(), None, True),                      # ~10k panels: every row, both modes
     ("C3", dict(which="ligand"), None, True),        # ~2k panels, 50 sites
-    ("C3", dict(which="complex"), 2048, True),       # ~59k panels: sampled rows, both modes
-    ("C4", dict(), 1024, False),                     # ~1.02M panels, 7.1M Gauss points: sampled rows, treecode
+    ("C3", dict(which="complex"), 4096, True),       # ~58k panels: 4,096 sampled rows (S: section 8(d) gates), both modes
+    ("C3", dict(which="receptor"), 4096, True),      # ~61k panels
+    ("C4", dict(), 4096, True),                      # ~1.04M panels, 7.26M Gauss points: 4,096 sampled rows, both modes
 ])
 def test_matvec_full_size(pbm, po, torch_cuda, name, kw, nrows, direct):
     from paper_1810_03698_b200.workloads import make_config
@@ -56,6 +66,9 @@ def test_matvec_full_size(pbm, po, torch_cuda, name, kw, nrows, direct):
     st = ctx.stats()
     assert rel(y[rows], y1) <= TOL_TREE and rel(y[nt + rows], y2) <= TOL_TREE
     assert st["m2p_pairs"] > 0 and st["p2p_pairs"] + 0 < nt * nt * w.params["K_far"]
+    # exact cover: the stored lists account for every (target, source point) pair exactly once --
+    # at C4 one missed far panel would be a 1e-6 error, invisible under the 1e-4 bound
+    assert st["covered_pairs"] == nt * nt * w.params["K_far"]
     # properties at any size: linearity and determinism of the treecode operator
     y_again = ctx.matvec(xd).cpu().numpy()
     np.testing.assert_array_equal(y, y_again)          # fixed accumulation order: bitwise repeatable
@@ -67,6 +80,7 @@ def test_matvec_full_size(pbm, po, torch_cuda, name, kw, nrows, direct):
         yd = ctx.matvec(xd).cpu().numpy()
         assert rel(yd[rows], y1) <= TOL_DIRECT and rel(yd[nt + rows], y2) <= TOL_DIRECT
         assert ctx.stats()["p2p_pairs"] == nt * nt * w.params["K_far"]      # list pairs (own panel skipped by index)
+        assert ctx.stats()["covered_pairs"] == nt * nt * w.params["K_far"]
         assert rel(y, yd) <= TOL_TREE                  # treecode vs direct on every row
     ctx.close()
 
@@ -147,25 +161,70 @@ def test_binding_triple_against_oracle(pbm, po, torch_cuda):
     assert abs(got["dG_bind_diss"] - (got["ddG_bind"] + got["dG_bind_vac"])) <= 1e-9 * scale
 
 
-def test_c3_complex_solve_treecode_against_direct_mode(pbm, torch_cuda):
-    """BASELINE configs[3] at full size (~58k panels, 3,050 sites): the oracle cannot afford the dense solve, so
-    the treecode solve is compared with the direct-mode (theta = 0) GPU solve, which the sampled-row test above
-    ties to the oracle at 1e-11 (S: section 8(d) gates)."""
+def test_c3_binding_triple_full_size_treecode_against_direct_mode(pbm, torch_cuda):
+    """BASELINE configs[3] at full size (complex ~58k panels / 3,050 sites, receptor ~61k / 3,000, ligand ~2k / 50):
+    the oracle cannot afford the dense solves, so each treecode solve is compared with the direct-mode (theta = 0)
+    GPU solve, which the sampled-row test above ties to the oracle at 1e-11 (S: section 8(d) gates); then the
+    binding cycle of Eq. (25)-(27) from the three treecode solves against the three direct-mode ones."""
     from paper_1810_03698_b200.workloads import make_config
-    w = make_config("C3", which="complex")
+    tree, direct, scale = [], [], 0.0
+    for which in ("complex", "receptor", "ligand"):
+        w = make_config("C3", which=which)
+        ctx = pbm.from_workload(w)
+        ctx.tree_build()
+        x_t, mu_t, res_t = ctx.solve()
+        x_t, mu_t = x_t.cpu().numpy(), mu_t.cpu().numpy()
+        ctx.set_params(theta=0.0)
+        ctx.tree_build()
+        x_d, mu_d, res_d = ctx.solve()
+        assert res_t["status"] == 0 and res_d["status"] == 0
+        for k in ("dG_solv", "G_solvterm", "G_mult_diss"):
+            assert abs(res_t[k] - res_d[k]) <= 1e-3 * abs(res_d[k]), (which, k, res_t[k], res_d[k])
+        assert res_t["G_vac"] == res_d["G_vac"]                                   # no surface involved
+        assert rel(mu_t, mu_d.cpu().numpy()) <= 1e-4
+        assert rel(x_t, x_d.cpu().numpy()) <= 1e-3
+        assert abs(res_t["scf_iters"] - res_d["scf_iters"]) <= 1
+        assert res_t["final_gmres_relres"] <= 1e-6 and res_t["final_scf_delta_debye"] < 1e-7
+        tree.append(res_t)
+        direct.append(res_d)
+        scale += abs(res_d["dG_solv"])
+        ctx.close()
+    got, want = pbm.binding_cycle(*tree), pbm.binding_cycle(*direct)
+    assert got["converged"] and want["converged"]
+    assert got["dG_bind_vac"] == want["dG_bind_vac"]
+    assert abs(got["ddG_bind"] - want["ddG_bind"]) <= 1e-3 * scale               # a difference of three large energies
+    assert abs(got["dG_bind_diss"] - (got["ddG_bind"] + got["dG_bind_vac"])) <= 1e-9 * scale
+
+
+def test_c4_full_polarizable_solve(pbm, torch_cuda):
+    """BASELINE configs[4]'s full polarizable solve (1.04 M panels, 20,000 sites; theta = 0.5, P = 6): the one place
+    where the 6-step near-field preconditioner inside flexible GMRES, GMRES restarts, the variable-order M2P, the
+    automatic site treecode for the reaction field and the RHS treecode meet.  Neither the oracle nor the direct-mode
+    GPU operator can afford this solve, so it is compared with a solve on a much tighter treecode (theta = 0.3,
+    P = 8: 5.8e-8 per matvec against the oracle's rows, profiles/r01c_sweep_C4.md), itself tied to the oracle by
+    the sampled-row gates above."""
+    from paper_1810_03698_b200.workloads import make_config
+    w = make_config("C4")
     ctx = pbm.from_workload(w)
+    p = ctx.get_params()
+    assert (p.theta, p.order_P, p.site_treecode, p.rhs_treecode, p.precond) == (0.5, 6, 2, 2, 3)
     ctx.tree_build()
-    x_t, mu_t, res_t = ctx.solve()
-    ctx.set_params(theta=0.0)
+    x, mu, res = ctx.solve()
+    st = ctx.stats()
+    assert res["status"] == 0
+    assert res["final_gmres_relres"] <= 1e-6 and res["final_scf_delta_debye"] < 1e-7
+    assert st["covered_pairs"] == st["n_panels"] * st["n_sources"]
+    assert st["site_covered_pairs"] == st["n_sites"] * st["n_sources"]           # the site treecode ran, with complete lists
+    x, mu = x.cpu().numpy(), mu.cpu().numpy()
+    ctx.set_params(theta=0.3, order_P=8)
     ctx.tree_build()
-    x_d, mu_d, res_d = ctx.solve()
-    assert res_t["status"] == 0 and res_d["status"] == 0
-    for k in ("dG_solv", "G_solvterm", "G_mult_diss"):
-        assert abs(res_t[k] - res_d[k]) <= 1e-3 * abs(res_d[k]), (k, res_t[k], res_d[k])
-    assert res_t["G_vac"] == res_d["G_vac"]                                   # no surface involved
-    assert rel(mu_t.cpu().numpy(), mu_d.cpu().numpy()) <= 1e-4
-    assert rel(x_t.cpu().numpy(), x_d.cpu().numpy()) <= 1e-3
-    assert abs(res_t["scf_iters"] - res_d["scf_iters"]) <= 1
+    x_r, mu_r, ref = ctx.solve()
+    assert ref["status"] == 0
+    for k in ("dG_solv", "G_solvterm", "G_mult_diss", "G_vac"):
+        assert abs(res[k] - ref[k]) <= 1e-3 * abs(ref[k]), (k, res[k], ref[k])
+    assert rel(mu, mu_r.cpu().numpy()) <= 1e-4
+    assert rel(x, x_r.cpu().numpy()) <= 1e-3
+    assert abs(res["scf_iters"] - ref["scf_iters"]) <= 1
     ctx.close()
 
 
@@ -181,6 +240,8 @@ def test_site_treecode_reaction_field_c2(pbm, po, torch_cuda):
     ctx = pbm.from_workload(w, site_treecode=1)
     ctx.tree_build()
     phi, grad, hess = [t.cpu().numpy() for t in ctx.reaction_field(torch_cuda.from_numpy(ref["x"]))]
+    st = ctx.stats()
+    assert st["site_m2p_pairs"] > 0 and st["site_covered_pairs"] == st["n_sites"] * st["n_sources"]
     assert rel(phi, ref["phi_solv"]) <= 1e-4
     assert rel(grad, ref["grad_solv"]) <= 1e-3          # each target derivative costs about one order of the expansion
     assert rel(hess, ref["hess_solv"]) <= 1e-2
@@ -211,6 +272,8 @@ def test_site_treecode_matches_direct_sum_at_c4(pbm, torch_cuda):
     x = torch.cat([1.0 / (c - torch.tensor([3.0, 1.0, -2.0], device="cuda", dtype=c.dtype)).norm(dim=1),
                    -0.1 / (c + torch.tensor([5.0, -4.0, 6.0], device="cuda", dtype=c.dtype)).norm(dim=1) ** 2])
     tree = [t.clone() for t in ctx.reaction_field(x)]
+    st = ctx.stats()
+    assert st["site_m2p_pairs"] > 0 and st["site_covered_pairs"] == st["n_sites"] * st["n_sources"]
     ctx.set_params(site_treecode=0)
     direct = ctx.reaction_field(x)
     errs = [float((a - b).norm() / b.norm()) for a, b in zip(tree, direct)]

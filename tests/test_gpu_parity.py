@@ -12,7 +12,15 @@ TOL_ENERGY = 1e-3
 
 
 def rel(a, b):
-    return float(np.linalg.norm(np.asarray(a) - np.asarray(b)) / np.linalg.norm(np.asarray(b)))
+    """Relative error in BOTH norms, the larger of the two: ||a - b||_2 / ||b||_2 (BASELINE.json's stated norm) and
+    max|a - b| / max|b| (so that one bad row among 10^4-10^6 cannot hide under the L2 bound).  Rounding-level
+    comparisons (direct mode, <= 1e-11) take the max norm at face value; for truncation-level ones (treecode, 1e-4:
+    the far-field error is not uniform over the rows) the max norm is allowed twice the L2 bound."""
+    a, b = np.asarray(a, dtype=float), np.asarray(b, dtype=float)
+    d = a - b
+    l2 = float(np.linalg.norm(d) / np.linalg.norm(b))
+    linf = float(np.max(np.abs(d)) / np.max(np.abs(b))) if d.size else 0.0
+    return max(l2, linf if l2 < 1e-9 else 0.5 * linf)
 
 
 @pytest.fixture(scope="module")
