@@ -106,8 +106,8 @@ typedef struct pb_stats {
     int64_t n_panels, n_sources, n_sites;
     int64_t n_cells, n_leaves, n_levels;
     int64_t n_groups;           /* target groups (blocks of consecutive Morton-ordered panels) */
-    int64_t p2p_pairs;          /* (target, source Gauss point) pairs per matvec               */
-    int64_t m2p_pairs;          /* (target, cell) pairs per matvec                             */
+    int64_t p2p_pairs;          /* (target, source Gauss point) pairs per matvec (sharded: of the owned groups) */
+    int64_t m2p_pairs;          /* (target, cell) pairs per matvec (sharded: of the owned groups)               */
     int64_t near_entries;       /* SELF+ADJ+NEAR correction-table entries                      */
     int64_t n_terms;            /* far-field terms per cell and layer (130 at P=6)             */
     int64_t matvec_calls;
@@ -180,6 +180,28 @@ int pb_sites_load(pb_ctx* ctx, int64_t na, const double* pos, const double* q, c
  * rule that the matvec adds and the true entries that the near-field preconditioner uses).  Needs
  * pb_mesh_load. */
 int pb_tree_build(pb_ctx* ctx);
+
+/* ---- multi-GPU: target sharding (S: section 8(e), 8(f) item 4) --------------------------------------------------
+ * One process per GPU, every process with its own context holding the WHOLE problem (mesh, sites, tree, moments and
+ * near table are replicated: < 5 GB at 10^6 panels) but evaluating only the rows of a contiguous Morton range of
+ * target groups: the P2P / M2P work items, the needed cells of the upward pass and the combine step are restricted
+ * to the owned groups.  The ranges are cut where the prefix sum of the per-group cost (P2P source points + 9 per
+ * M2P cell, times the targets of the group) crosses k/world of the total, identically on every rank.
+ * The ONE exchange step per matvec is an all-gather of the owned rows of y (2 x 8 bytes per owned panel; 16.6 MB in
+ * total at C4) through the callback, which must enqueue the collective on the context's stream (the Python binding
+ * calls torch.distributed.all_gather_into_tensor: NCCL over NVLink): `send` holds bytes_per_rank bytes, `recv`
+ * world x bytes_per_rank, both device pointers owned by the library.  After it every rank holds the full y, so
+ * GMRES, the SCF loop and the site-side operators run replicated and unchanged, and all ranks take identical
+ * decisions (the kernels are bitwise repeatable).  With allgather == NULL nothing is exchanged and pb_matvec writes
+ * ONLY the owned rows of y (original panel order), leaving the others untouched -- used to test the partition on one
+ * GPU, rank after rank.  Call before pb_tree_build (it invalidates a built tree); rank 0 / world 1 switches it off. */
+typedef int (*pb_allgather_fn)(void* user, const void* send, void* recv, size_t bytes_per_rank);
+int pb_set_shard(pb_ctx* ctx, int rank, int world, pb_allgather_fn allgather, void* user);
+/* After pb_tree_build: first [world + 1] (HOST) = first owned panel, in Morton order, of every rank. */
+int pb_get_shard(const pb_ctx* ctx, int64_t* first);
+/* HOST-only: the partition rule itself.  cost [G] >= 0; first [world + 1] with first[0] = 0, first[world] = G,
+ * first[k] = the smallest g whose exclusive prefix sum reaches k/world of the total (ranges may be empty). */
+int pb_shard_partition(const int64_t* cost, int64_t G, int world, int64_t* first);
 
 /* ---- operators --------------------------------------------------------------------- */
 /* b [2 nt]: b[0:nt] = Eq. (8) at the collocation points with p = dip + mu_induced

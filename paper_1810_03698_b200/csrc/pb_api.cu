@@ -201,6 +201,36 @@ extern "C" int pb_set_params(pb_ctx* ctx, const pb_params* p)
     return PB_OK;
 }
 
+// ---- target sharding (include/pb.h) ---------------------------------------------------------
+extern "C" int pb_set_shard(pb_ctx* ctx, int rank, int world, pb_allgather_fn allgather, void* user)
+{
+    if (!ctx) return PB_ERR_INVALID_ARG;
+    if (world < 1 || rank < 0 || rank >= world) return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_set_shard: need 0 <= rank < world");
+    if (world > 4096) return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_set_shard: world too large");
+    ctx->shard_rank = rank;
+    ctx->shard_world = world;
+    ctx->allgather = world > 1 ? allgather : nullptr;
+    ctx->allgather_user = user;
+    if (ctx->tree.built) {                      // the work items and needed cells depend on the owned range
+        pb_dfree_cat(ctx, CAT_TREE);
+        pb_dfree_cat(ctx, CAT_SITE_NEAR);
+        pb_dfree_cat(ctx, CAT_SOLVE);
+        ctx->gws = pb_gmres_ws();
+        ctx->tree = pb_tree();
+        ctx->sites.near_built = false;
+        ctx->sites.tree_built = false;
+    }
+    return PB_OK;
+}
+
+extern "C" int pb_get_shard(const pb_ctx* ctx, int64_t* first)
+{
+    if (!ctx || !first) return PB_ERR_INVALID_ARG;
+    if (!ctx->tree.built) return PB_ERR_NOT_READY;
+    for (int k = 0; k <= ctx->shard_world; ++k) first[k] = ctx->tree.shard_first[k];
+    return PB_OK;
+}
+
 // ---- mesh ---------------------------------------------------------------------------------
 // Per panel: centroid (v0+v1+v2)/3 = collocation point; flags degenerate panels.
 __global__ void k_mesh_check(int64_t nt, int64_t nv, const double* __restrict__ verts,

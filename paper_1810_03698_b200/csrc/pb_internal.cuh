@@ -119,6 +119,15 @@ struct pb_tree {
     int nslot_p2p = 1, nslot_m2p = 1;   // largest number of items of one group
     double* accP = nullptr;       // [nslot_p2p][4][N]
     double* accM = nullptr;       // [nslot_m2p][4][N]
+    // target sharding (S: section 8(e)/(f)4): this context evaluates the rows of the target groups [own_g0, own_g1)
+    // = Morton panels [own_i0, own_i1); without sharding that is every group
+    int64_t own_g0 = 0, own_g1 = 0, own_i0 = 0, own_i1 = 0;
+    int64_t itemP0 = 0, n_itemP_own = 0, itemM0 = 0, n_itemM_own = 0;   // the owned groups' work items
+    std::vector<int64_t> shard_first;   // [world + 1] first Morton panel of every rank's range
+    int64_t shard_nmax = 0;             // largest number of owned panels over the ranks
+    int64_t* shard_first_dev = nullptr; // device copy of shard_first
+    double* ysend = nullptr;            // [2][shard_nmax] owned rows of y, Morton order (all-gather send buffer)
+    double* yall = nullptr;             // [world][2][shard_nmax] gathered rows
 };
 
 struct pb_sites {
@@ -191,6 +200,10 @@ struct pb_ctx {
     pb_tree tree;
     pb_sites sites;
     pb_gmres_ws gws;
+    // target sharding: rank / world and the exchange callback (NULL: no exchange, only the owned rows of y are written)
+    int shard_rank = 0, shard_world = 1;
+    pb_allgather_fn allgather = nullptr;
+    void* allgather_user = nullptr;
     // scratch
     double* scratch = nullptr;    // small device scratch for reductions
     size_t scratch_bytes = 0;

@@ -135,14 +135,20 @@ int pb_farfield_setup(pb_ctx* ctx)
     // Which cells need moments: the ones in some M2P list ("used") and every descendant of a used
     // cell (M2M builds a parent from ALL its children).  Bookkeeping on the host, once per tree.
     const int64_t nc = t.n_cells;
-    std::vector<int32_t> child(nc), nchild(nc), lists(t.m2p_total > 0 ? t.m2p_total : 1);
+    // (with target sharding only the cells in the OWNED groups' lists, entries [e0, e1), are needed on this rank)
+    int32_t he[2] = {0, 0};
+    PB_CUDA(cudaMemcpyAsync(&he[0], t.m2p_off + t.own_g0, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    PB_CUDA(cudaMemcpyAsync(&he[1], t.m2p_off + t.own_g1, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    PB_CUDA(cudaStreamSynchronize(st));
+    const int64_t e0 = he[0], ne = he[1] - he[0];
+    std::vector<int32_t> child(nc), nchild(nc), lists(ne > 0 ? ne : 1);
     PB_CUDA(cudaMemcpyAsync(child.data(), t.c_child, sizeof(int32_t) * nc, cudaMemcpyDeviceToHost, st));
     PB_CUDA(cudaMemcpyAsync(nchild.data(), t.c_nchild, sizeof(int32_t) * nc, cudaMemcpyDeviceToHost, st));
-    if (t.m2p_total > 0)
-        PB_CUDA(cudaMemcpyAsync(lists.data(), t.m2p_cell, sizeof(int32_t) * t.m2p_total, cudaMemcpyDeviceToHost, st));
+    if (ne > 0)
+        PB_CUDA(cudaMemcpyAsync(lists.data(), t.m2p_cell + e0, sizeof(int32_t) * ne, cudaMemcpyDeviceToHost, st));
     PB_CUDA(cudaStreamSynchronize(st));   // also: the host vectors above go out of scope
     std::vector<char> used(nc, 0), need(nc, 0);
-    for (int64_t e = 0; e < t.m2p_total; ++e) used[lists[e]] = 1;
+    for (int64_t e = 0; e < ne; ++e) used[lists[e]] = 1;
     std::vector<int32_t> leaf_list, parent(nc, -1), up(nc, 0);
     int64_t n_used = 0, n_internal = 0;
     for (int64_t c = 0; c < nc; ++c) {               // cells are numbered generation by generation: parents first
@@ -623,23 +629,28 @@ k_m2p(int64_t N, double kappa, pb_expk ek, const pb_item* __restrict__ items, co
     }
 }
 
-// ---- M2P, two targets per thread (orders P <= 6) -------------------------------------------------------------
+// ---- M2P, two targets per thread (orders P <= 8) -------------------------------------------------------------
 // With one target per thread every F term costs one 16-byte shared-memory broadcast per two FMAs, and
 // the shared-memory pipe, not the FP64 pipe, sets the pace (ncu: FP64 pipe 65 % busy).  Here a lane
 // carries targets lane and lane + 32 of the group, so each term read feeds four FMAs; a warp covers the
-// whole group, the block's 8 warps take different cells of a stage.
+// whole group, the block's 8 warps take different cells of the work item (cells sub, sub + 8, ...).
+// Every warp has its OWN ring of M2Q_NS cell slots in shared memory, filled by its lane 0 with TMA bulk copies and
+// its own mbarriers: no warp ever waits for another warp, only for its own data.  (The first version shared one
+// ring of 8-cell tiles between the warps, refilled when all eight had left a tile; ncu at C4 showed 22 % of the warp
+// samples in the wait for the next tile although the data rate needed is a few bytes per clock and SM: warp 0,
+// which also ran the producer code, could never run ahead of the slowest warp, and every hiccup of one warp stalled
+// the other seven at the end of the ring.)
 #define M2Q_W 8
 #define M2Q_NS 4
-#define M2Q_CT 8
 #define M2Q_THREADS (32 * M2Q_W)
 static_assert(PB_TG == 64, "k_m2p2 keeps two targets per lane");
 
 template <int P> struct m2q_cfg {
     static constexpr int NT = pb_nt(P);
     static constexpr size_t RED_BYTES = (size_t)M2Q_W * 4 * PB_TG * sizeof(double);
-    static constexpr size_t FF_BYTES0 = (size_t)M2Q_NS * M2Q_CT * NT * sizeof(double2);
+    static constexpr size_t FF_BYTES0 = (size_t)M2Q_W * M2Q_NS * NT * sizeof(double2);
     static constexpr size_t FF_BYTES = FF_BYTES0 > RED_BYTES ? FF_BYTES0 : RED_BYTES;
-    static constexpr size_t SMEM = FF_BYTES + M2Q_NS * M2Q_CT * sizeof(double4) + 2 * M2Q_NS * sizeof(uint64_t) + 32 * sizeof(double);
+    static constexpr size_t SMEM = FF_BYTES + M2Q_W * M2Q_NS * sizeof(uint64_t) + 32 * sizeof(double);
 };
 
 // PL <= P: evaluate only the terms of the order-PL sum (|alpha| + 2j <= PL); they are a subset of the order-P terms
@@ -702,31 +713,31 @@ __device__ __forceinline__ void m2p_radial(double dx, double dy, double dz, cons
     }
 }
 
+// orders 7, 8: 36 partial sums per target pair leave no room for two blocks per SM (one block, up to 255 registers)
 template <int P>
-__global__ void __launch_bounds__(M2Q_THREADS, 2)
+#ifndef M2Q_MINB6
+#define M2Q_MINB6 2
+#endif
+__global__ void __launch_bounds__(M2Q_THREADS, P <= 6 ? M2Q_MINB6 : 1)
 k_m2p2(int64_t N, double kappa, pb_expk ek, const pb_item* __restrict__ items, const int32_t* __restrict__ m2p_cell,
        const double4* __restrict__ m2p_ctr, const double2* __restrict__ FF, const double* __restrict__ px,
        const double* __restrict__ py, const double* __restrict__ pz, double* __restrict__ acc)
 {
-    constexpr int NT = m2q_cfg<P>::NT, CT = M2Q_CT, NS = M2Q_NS;
+    constexpr int NT = m2q_cfg<P>::NT, NS = M2Q_NS;
     extern __shared__ __align__(128) unsigned char smraw[];
-    double2* ff = reinterpret_cast<double2*>(smraw);                                  // [NS][CT][NT]
-    double4* ctr = reinterpret_cast<double4*>(smraw + m2q_cfg<P>::FF_BYTES);           // [NS][CT]
-    uint64_t* full = reinterpret_cast<uint64_t*>(ctr + NS * CT);                       // [NS]
-    uint64_t* empty = full + NS;                                                       // [NS]
-    double* Ts = reinterpret_cast<double*>(empty + NS);                                // [32]
     const int tid = threadIdx.x;
     const int lane = tid & 31, sub = tid >> 5;
+    double2* ffw = reinterpret_cast<double2*>(smraw) + (size_t)sub * NS * NT;          // this warp's slots [NS][NT]
+    uint64_t* fullw = reinterpret_cast<uint64_t*>(smraw + m2q_cfg<P>::FF_BYTES) + sub * NS;   // and their barriers
+    double* Ts = reinterpret_cast<double*>(smraw + m2q_cfg<P>::FF_BYTES + M2Q_W * NS * sizeof(uint64_t));   // [32]
     const pb_item item = items[blockIdx.x];
     const int64_t g = item.group;
-    const int32_t e0 = item.r, count = item.count;
+    const int32_t e0 = item.r + sub, count = item.count;
+    const int nw = count > sub ? (count - sub + M2Q_W - 1) / M2Q_W : 0;     // this warp's cells: list entries e0 + 8 k
     if (tid < 32) Ts[tid] = ek.T[tid];
-    if (tid == 0) {
+    if (lane == 0) {
 #pragma unroll
-        for (int s = 0; s < NS; ++s) {
-            pb_mbar_init(&full[s], 1);
-            pb_mbar_init(&empty[s], M2Q_W);
-        }
+        for (int s = 0; s < NS; ++s) pb_mbar_init(&fullw[s], 1);
         pb_mbar_fence_init();
     }
     __syncthreads();
@@ -734,73 +745,47 @@ k_m2p2(int64_t N, double kappa, pb_expk ek, const pb_item* __restrict__ items, c
     const int64_t ic0 = i0 < N ? i0 : N - 1, ic1 = i1 < N ? i1 : N - 1;     // padding lanes repeat the last target; never stored
     const double tx0 = px[ic0], ty0 = py[ic0], tz0 = pz[ic0];
     const double tx1 = px[ic1], ty1 = py[ic1], tz1 = pz[ic1];
-    const int ntile = (count + CT - 1) / CT;
 
-    int32_t idn[CT];
-    auto load_ids = [&](int t) {
-#pragma unroll
-        for (int j = 0; j < CT; ++j) {
-            const int32_t e = t * CT + j;
-            idn[j] = e < count ? m2p_cell[e0 + e] : 0;
-        }
+    auto issue = [&](int k, int32_t cell) {           // lane 0: cell k of this warp into slot k % NS
+        const int slot = k % NS;
+        pb_mbar_expect_tx(&fullw[slot], (uint32_t)(NT * sizeof(double2)));
+        pb_bulk_g2s(ffw + (size_t)slot * NT, FF + (int64_t)cell * NT, (uint32_t)(NT * sizeof(double2)), &fullw[slot]);
     };
-    auto issue = [&](int t, int stage) {
-        const int n = count - t * CT < CT ? count - t * CT : CT;
-        pb_mbar_expect_tx(&full[stage], (uint32_t)(n * (sizeof(double4) + NT * sizeof(double2))));
-        pb_bulk_g2s(ctr + stage * CT, m2p_ctr + e0 + t * CT, (uint32_t)(n * sizeof(double4)), &full[stage]);
-#pragma unroll
-        for (int j = 0; j < CT; ++j)
-            if (j < n)
-                pb_bulk_g2s(ff + ((size_t)stage * CT + j) * NT, FF + (int64_t)idn[j] * NT, (uint32_t)(NT * sizeof(double2)),
-                            &full[stage]);
-    };
-    if (tid == 0 && ntile > 0) {
-        load_ids(0);
-        for (int t = 0; t < NS - 1 && t < ntile; ++t) {
-            issue(t, t);
-            if (t + 1 < ntile) load_ids(t + 1);
-        }
-    }
+    if (lane == 0)
+        for (int k = 0; k < NS - 1 && k < nw; ++k) issue(k, m2p_cell[e0 + M2Q_W * k]);
+    int32_t idn = NS - 1 < nw ? m2p_cell[e0 + M2Q_W * (NS - 1)] : 0;        // cell of the next copy to issue
+    double4 ccn = nw > 0 ? m2p_ctr[e0] : make_double4(0, 0, 0, 0);           // centre (and order flag) of the next cell to evaluate
     double VL0 = 0, KL0 = 0, VY0 = 0, KY0 = 0, VL1 = 0, KL1 = 0, VY1 = 0, KY1 = 0;
     const double k2 = kappa * kappa;
-    int st = 0, ph = 0;                               // stage and phase of tile t
-    for (int t = 0; t < ntile; ++t) {
-        if (tid == 0) {
-            const int tn = t + NS - 1;                // refill the stage tile t-1 used, once every warp has left it
-            if (tn < ntile) {
-                const int sn = st == 0 ? NS - 1 : st - 1;
-                if (t > 0) pb_mbar_wait(&empty[sn], (uint32_t)(((t - 1) / NS) & 1));
-                issue(tn, sn);
-                if (tn + 1 < ntile) load_ids(tn + 1);
-            }
-        }
-        pb_mbar_wait(&full[st], (uint32_t)ph);
-        const int cnt = count - t * CT < CT ? count - t * CT : CT;
 #pragma unroll 1
-        for (int j = sub; j < cnt; j += M2Q_W) {
-            const double4 cc = ctr[st * CT + j];
-            const double dx0 = tx0 - cc.x, dy0 = ty0 - cc.y, dz0 = tz0 - cc.z;
-            const double dx1 = tx1 - cc.x, dy1 = ty1 - cc.y, dz1 = tz1 - cc.z;
-            double WV0[P + 1], WK0[P + 1], WV1[P + 1], WK1[P + 1];
+    for (int k = 0; k < nw; ++k) {
+        // slot (k - 1) % NS was read for the last time before the __syncwarp that ended the previous iteration
+        const int kn = k + NS - 1;
+        if (lane == 0 && kn < nw) issue(kn, idn);
+        idn = kn + 1 < nw ? m2p_cell[e0 + M2Q_W * (kn + 1)] : 0;           // in flight while cell k is evaluated
+        const double4 cc = ccn;
+        ccn = k + 1 < nw ? m2p_ctr[e0 + M2Q_W * (k + 1)] : cc;
+        pb_mbar_wait(&fullw[k % NS], (uint32_t)((k / NS) & 1));
+        const double2* ffk = ffw + (size_t)(k % NS) * NT;
+        const double dx0 = tx0 - cc.x, dy0 = ty0 - cc.y, dz0 = tz0 - cc.z;
+        const double dx1 = tx1 - cc.x, dy1 = ty1 - cc.y, dz1 = tz1 - cc.z;
+        double WV0[P + 1], WK0[P + 1], WV1[P + 1], WK1[P + 1];
 #pragma unroll
-            for (int m = 0; m <= P; ++m) { WV0[m] = 0.0; WK0[m] = 0.0; WV1[m] = 0.0; WK1[m] = 0.0; }
-            constexpr int PL = P >= 4 ? P - 2 : P;
-            if (PL < P && cc.w != 0.0) {              // flagged by the list build: order P - 2 is enough (warp-uniform)
-                m2p_terms2<P, PL>(ff + ((size_t)st * CT + j) * NT, dx0, dy0, dz0, dx1, dy1, dz1, WV0, WK0, WV1, WK1);
-                m2p_radial<P, PL>(dx0, dy0, dz0, WV0, WK0, kappa, k2, ek, Ts, VL0, KL0, VY0, KY0);
-                m2p_radial<P, PL>(dx1, dy1, dz1, WV1, WK1, kappa, k2, ek, Ts, VL1, KL1, VY1, KY1);
-            } else {
-                m2p_terms2<P, P>(ff + ((size_t)st * CT + j) * NT, dx0, dy0, dz0, dx1, dy1, dz1, WV0, WK0, WV1, WK1);
-                m2p_radial<P, P>(dx0, dy0, dz0, WV0, WK0, kappa, k2, ek, Ts, VL0, KL0, VY0, KY0);
-                m2p_radial<P, P>(dx1, dy1, dz1, WV1, WK1, kappa, k2, ek, Ts, VL1, KL1, VY1, KY1);
-            }
+        for (int m = 0; m <= P; ++m) { WV0[m] = 0.0; WK0[m] = 0.0; WV1[m] = 0.0; WK1[m] = 0.0; }
+        constexpr int PL = P >= 4 ? P - 2 : P;
+        if (PL < P && cc.w != 0.0) {              // flagged by the list build: order P - 2 is enough (warp-uniform)
+            m2p_terms2<P, PL>(ffk, dx0, dy0, dz0, dx1, dy1, dz1, WV0, WK0, WV1, WK1);
+            m2p_radial<P, PL>(dx0, dy0, dz0, WV0, WK0, kappa, k2, ek, Ts, VL0, KL0, VY0, KY0);
+            m2p_radial<P, PL>(dx1, dy1, dz1, WV1, WK1, kappa, k2, ek, Ts, VL1, KL1, VY1, KY1);
+        } else {
+            m2p_terms2<P, P>(ffk, dx0, dy0, dz0, dx1, dy1, dz1, WV0, WK0, WV1, WK1);
+            m2p_radial<P, P>(dx0, dy0, dz0, WV0, WK0, kappa, k2, ek, Ts, VL0, KL0, VY0, KY0);
+            m2p_radial<P, P>(dx1, dy1, dz1, WV1, WK1, kappa, k2, ek, Ts, VL1, KL1, VY1, KY1);
         }
         __syncwarp();
-        if (lane == 0) pb_mbar_arrive(&empty[st]);
-        if (++st == NS) { st = 0; ph ^= 1; }
     }
     __syncthreads();
-    // add the warps' partial sums in a fixed order (the stages are free: every thread passed the barrier above)
+    // add the warps' partial sums in a fixed order (the slots are free: every warp has consumed all its cells)
     double* red = reinterpret_cast<double*>(smraw);   // [M2Q_W][4][PB_TG]
     red[(sub * 4 + 0) * PB_TG + lane] = VL0; red[(sub * 4 + 0) * PB_TG + lane + 32] = VL1;
     red[(sub * 4 + 1) * PB_TG + lane] = KL0; red[(sub * 4 + 1) * PB_TG + lane + 32] = KL1;
@@ -1096,11 +1081,14 @@ k_combine(int64_t N, const int32_t* __restrict__ itemP_off, const int32_t* __res
           const double* __restrict__ accP, const double* __restrict__ accM, const int32_t* __restrict__ el_base,
           const int32_t* __restrict__ el_col, const double* __restrict__ el_val, int64_t ne,
           const double* __restrict__ xphi, const double* __restrict__ xdphi, const int32_t* __restrict__ perm,
-          double* __restrict__ y)
+          double* __restrict__ y, int64_t blk0, int64_t i1, double* __restrict__ ymort, int64_t nmax)
 {
+    // blk0, i1: the launch covers the Morton panels [32 blk0, i1) (target sharding; 0, N otherwise).  ymort != NULL:
+    // the two rows go to ymort[k], ymort[nmax + k], k = i - 32 blk0 (Morton order, the all-gather send buffer)
     __shared__ double sm[4][32];
     const int tgt = threadIdx.x & 31, m = threadIdx.x >> 5;
-    const int64_t i = blockIdx.x * 32LL + tgt;
+    const int64_t blk = blk0 + blockIdx.x;
+    const int64_t i = blk * 32LL + tgt;
     double s = 0.0;
     {
         const int64_t ic = i < N ? i : N - 1;                      // padding lanes: same loads, nothing stored
@@ -1112,7 +1100,7 @@ k_combine(int64_t N, const int32_t* __restrict__ itemP_off, const int32_t* __res
         s *= PB_INV4PI;
         const double* __restrict__ xv = (m & 1) ? xphi : xdphi;     // V_L, V_Y act on dphi; K_L, K_Y on phi
         // the slice's rows of the near table (sliced ELL: the warp reads 32 consecutive entries per step)
-        const int32_t b0 = el_base[blockIdx.x], width = (el_base[blockIdx.x + 1] - b0) / 32;
+        const int32_t b0 = el_base[blk], width = (el_base[blk + 1] - b0) / 32;
         const double* __restrict__ val = el_val + (int64_t)m * ne + b0 + tgt;
         const int32_t* __restrict__ col = el_col + b0 + tgt;
         int k = 0;
@@ -1127,13 +1115,36 @@ k_combine(int64_t N, const int32_t* __restrict__ itemP_off, const int32_t* __res
     }
     sm[m][tgt] = s;
     __syncthreads();
-    if (m == 0 && i < N) {
+    if (m == 0 && i < i1) {
         const double VL = sm[0][tgt], KL = sm[1][tgt], VY = sm[2][tgt], KY = sm[3][tgt];
         const double phi = xphi[i];
-        const int64_t o = perm[i];
-        y[o] = 0.5 * phi + KL - VL;                    // Eq. (5), first row
-        y[N + o] = 0.5 * phi - KY + eps_ratio * VY;    // Eq. (5), second row
+        const double r1 = 0.5 * phi + KL - VL;                    // Eq. (5), first row
+        const double r2 = 0.5 * phi - KY + eps_ratio * VY;        // Eq. (5), second row
+        if (ymort) {
+            const int64_t k = i - 32 * blk0;
+            ymort[k] = r1;
+            ymort[nmax + k] = r2;
+        } else {
+            const int64_t o = perm[i];
+            y[o] = r1;
+            y[N + o] = r2;
+        }
     }
+}
+
+// after the all-gather: rank r's rows [2][nmax] hold the Morton panels first[r] .. first[r + 1]; un-permute into y
+__global__ void k_shard_scatter(int64_t N, int world, const int64_t* __restrict__ first, int64_t nmax,
+                                const double* __restrict__ yall, const int32_t* __restrict__ perm, double* __restrict__ y)
+{
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int r = 0;
+    while (r + 1 < world && i >= first[r + 1]) ++r;
+    const int64_t k = i - first[r];
+    const double* src = yall + (int64_t)r * 2 * nmax;
+    const int64_t o = perm[i];
+    y[o] = src[k];
+    y[N + o] = src[nmax + k];
 }
 
 // ---- host driver ----------------------------------------------------------------------------------------------
@@ -1146,8 +1157,8 @@ static cudaError_t launch_m2p2(pb_ctx* ctx, cudaStream_t fs)
         if (e != cudaSuccess) return e;
         ctx->attr_m2p_mask |= 1u << P;
     }
-    k_m2p2<P><<<(unsigned)t.n_itemM, M2Q_THREADS, m2q_cfg<P>::SMEM, fs>>>(
-        t.N, ctx->prm.kappa, t.ek, t.itemM, t.m2p_cell, t.m2p_ctr, t.FF, t.pc[0], t.pc[1], t.pc[2], t.accM);
+    k_m2p2<P><<<(unsigned)t.n_itemM_own, M2Q_THREADS, m2q_cfg<P>::SMEM, fs>>>(
+        t.N, ctx->prm.kappa, t.ek, t.itemM + t.itemM0, t.m2p_cell, t.m2p_ctr, t.FF, t.pc[0], t.pc[1], t.pc[2], t.accM);
     return cudaSuccess;
 }
 
@@ -1160,8 +1171,8 @@ static cudaError_t launch_m2p(pb_ctx* ctx, cudaStream_t fs)
         if (e != cudaSuccess) return e;
         ctx->attr_m2p_mask |= 1u << P;
     }
-    k_m2p<P><<<(unsigned)t.n_itemM, M2P_THREADS, m2p_cfg<P>::SMEM, fs>>>(
-        t.N, ctx->prm.kappa, t.ek, t.itemM, t.m2p_cell, t.m2p_ctr, t.FF, t.pc[0], t.pc[1], t.pc[2], t.accM);
+    k_m2p<P><<<(unsigned)t.n_itemM_own, M2P_THREADS, m2p_cfg<P>::SMEM, fs>>>(
+        t.N, ctx->prm.kappa, t.ek, t.itemM + t.itemM0, t.m2p_cell, t.m2p_ctr, t.FF, t.pc[0], t.pc[1], t.pc[2], t.accM);
     return cudaSuccess;
 }
 
@@ -1233,7 +1244,7 @@ static int pb_far_branch(pb_ctx* ctx, cudaStream_t fs, bool timed)
     pb_tree& t = ctx->tree;
     PB_TRY(pb_upward(ctx, fs, t.need_leaf, t.n_need_leaf, t.up_link));
     if (timed) PB_CUDA(cudaEventRecord(ctx->ev[2], fs));
-    if (t.n_itemM > 0) {
+    if (t.n_itemM_own > 0) {
         PB_TRY(pb_prof_begin(ctx, 1));
         cudaError_t e = cudaSuccess;
         switch (t.P) {
@@ -1244,8 +1255,8 @@ static int pb_far_branch(pb_ctx* ctx, cudaStream_t fs, bool timed)
         case 4: e = launch_m2p2<4>(ctx, fs); break;
         case 5: e = launch_m2p2<5>(ctx, fs); break;
         case 6: e = launch_m2p2<6>(ctx, fs); break;
-        case 7: e = launch_m2p<7>(ctx, fs); break;
-        case 8: e = launch_m2p<8>(ctx, fs); break;
+        case 7: e = launch_m2p2<7>(ctx, fs); break;
+        case 8: e = launch_m2p2<8>(ctx, fs); break;
         case 9: e = launch_m2p<9>(ctx, fs); break;
         case 10: e = launch_m2p<10>(ctx, fs); break;
         default: return pb_fail(ctx, PB_ERR_INVALID_ARG, "unsupported order_P %d", t.P);
@@ -1292,22 +1303,40 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed, bool pre
         PB_TRY(pb_prof_begin(ctx, 0));
         // two targets per lane pays once the kernel is throughput-bound (measured: C3 529 -> 516 us, C4 8.43 -> 8.24 ms;
         // C1 / C2, a few waves of short blocks, are 2-4 % faster with one target per thread and twice the resident warps)
-        if (t.N >= 30000)
-            k_p2p2<<<(unsigned)t.n_itemP, P2P_THREADS, 0, st>>>(t.N, t.K, ctx->prm.kappa, t.ek8, t.itemP, t.p2p_lo, t.p2p_hi,
-                                                              t.srec, t.pc[0], t.pc[1], t.pc[2], t.accP);
-        else
-            k_p2p<<<(unsigned)t.n_itemP, P2P_THREADS, 0, st>>>(t.N, t.K, ctx->prm.kappa, t.ek8, t.itemP, t.p2p_lo, t.p2p_hi,
-                                                             t.srec, t.pc[0], t.pc[1], t.pc[2], t.accP);
-        PB_LAUNCH_CHECK();
+        if (t.n_itemP_own > 0) {
+            if (t.N >= 30000)
+                k_p2p2<<<(unsigned)t.n_itemP_own, P2P_THREADS, 0, st>>>(t.N, t.K, ctx->prm.kappa, t.ek8, t.itemP + t.itemP0, t.p2p_lo,
+                                                                      t.p2p_hi, t.srec, t.pc[0], t.pc[1], t.pc[2], t.accP);
+            else
+                k_p2p<<<(unsigned)t.n_itemP_own, P2P_THREADS, 0, st>>>(t.N, t.K, ctx->prm.kappa, t.ek8, t.itemP + t.itemP0, t.p2p_lo,
+                                                                     t.p2p_hi, t.srec, t.pc[0], t.pc[1], t.pc[2], t.accP);
+            PB_LAUNCH_CHECK();
+        }
         PB_TRY(pb_prof_end(ctx, 0));
         pb_prof_next(ctx);
     }
     if (far && !serial) PB_CUDA(cudaStreamWaitEvent(st, ctx->ev_join, 0));
     if (timed) PB_CUDA(cudaEventRecord(ctx->ev[4], st));
-    k_combine<<<pb_blocks(t.N, 32), 128, 0, st>>>(t.N, t.itemP_off, far ? t.itemM_off : nullptr,
-                                                  ctx->prm.eps_in / ctx->prm.eps_out, t.accP, t.accM, t.el_base,
-                                                  t.el_col, t.el_val, t.el_entries, t.xphi, t.xdphi, t.perm, y);
-    PB_LAUNCH_CHECK();
+    {
+        // the owned Morton panels [own_i0, own_i1) (all of them without sharding); own_i0 is a multiple of PB_TG = 2 x 32
+        const bool exchange = ctx->shard_world > 1 && ctx->allgather != nullptr;
+        const int64_t nown = t.own_i1 - t.own_i0;
+        if (nown > 0) {
+            k_combine<<<pb_blocks(nown, 32), 128, 0, st>>>(t.N, t.itemP_off, far ? t.itemM_off : nullptr,
+                                                          ctx->prm.eps_in / ctx->prm.eps_out, t.accP, t.accM, t.el_base, t.el_col,
+                                                          t.el_val, t.el_entries, t.xphi, t.xdphi, t.perm, y, t.own_i0 / 32,
+                                                          t.own_i1, exchange ? t.ysend : nullptr, t.shard_nmax);
+            PB_LAUNCH_CHECK();
+        }
+        if (exchange) {
+            // the ONE exchange step of a sharded matvec: all-gather of the owned rows (enqueued on this stream by the callback)
+            if (ctx->allgather(ctx->allgather_user, t.ysend, t.yall, (size_t)2 * t.shard_nmax * sizeof(double)) != 0)
+                return pb_fail(ctx, PB_ERR_CUDA, "pb_matvec: the all-gather callback failed");
+            k_shard_scatter<<<pb_blocks(t.N, 256), 256, 0, st>>>(t.N, ctx->shard_world, t.shard_first_dev, t.shard_nmax, t.yall,
+                                                                t.perm, y);
+            PB_LAUNCH_CHECK();
+        }
+    }
     ctx->matvec_calls++;
     if (timed) {
         PB_CUDA(cudaEventRecord(ctx->ev[5], st));

@@ -390,6 +390,26 @@ __global__ void __launch_bounds__(LIST_WARPS * 32) k_lists(list_args a)
     }
 }
 
+// Stable partition of every group's M2P list: the cells evaluated at the full order P first, then the ones flagged
+// for order P - 2 (R-30).  A tile of 8 consecutive list entries is what the 8 warps of a k_m2p2 block share, one
+// cell per warp; with mixed tiles the warps' times differ by a factor two per tile and the fast ones run into
+// the end of the 4-stage ring (ncu, C4: 21 % of the warp samples in the wait for the next tile's data).  After the
+// partition all tiles but one per work item are uniform.  One thread per group; setup time only.
+__global__ void k_partition_low(int64_t G, const int32_t* __restrict__ off, const int32_t* __restrict__ cell_in,
+                                const int8_t* __restrict__ low_in, int32_t* __restrict__ cell_out, int8_t* __restrict__ low_out)
+{
+    const int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (g >= G) return;
+    const int32_t e0 = off[g], e1 = off[g + 1];
+    int32_t nfull = 0;
+    for (int32_t e = e0; e < e1; ++e) nfull += low_in[e] ? 0 : 1;
+    int32_t a = e0, b = e0 + nfull;
+    for (int32_t e = e0; e < e1; ++e) {
+        if (low_in[e]) { cell_out[b] = cell_in[e]; low_out[b] = 1; ++b; }
+        else { cell_out[a] = cell_in[e]; low_out[a] = 0; ++a; }
+    }
+}
+
 __global__ void k_m2p_centres(int64_t n, const int32_t* __restrict__ cell, const int8_t* __restrict__ low,
                               const double* __restrict__ cx, const double* __restrict__ cy, const double* __restrict__ cz,
                               double4* __restrict__ out)
@@ -481,6 +501,44 @@ static int pb_build_items(pb_ctx* ctx, int64_t G, const int32_t* off, const int3
     *items_out = items;
     *n_items = total;
     *max_per_group = hmax;
+    return PB_OK;
+}
+
+// ---- target sharding: per-group cost and the partition rule (include/pb.h, pb_set_shard) -------------------------
+// cost[g] = targets in the group x (P2P source points + 9 per M2P cell): an M2P pair costs about as much as
+// 9 P2P pairs (12.0 ms / 5.57e8 against 8.2 ms / 3.45e9 at C4); pairs[g] = {P2P pairs, M2P pairs} of the group
+__global__ void k_group_cost(int64_t G, int64_t N, const int32_t* __restrict__ m2p_off, const int32_t* __restrict__ p2p_off,
+                             const int32_t* __restrict__ p2p_lo, const int32_t* __restrict__ p2p_hi,
+                             long long* __restrict__ cost, long long* __restrict__ pairs /*[G][2]*/)
+{
+    const int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (g >= G) return;
+    long long pts = 0;
+    for (int32_t r = p2p_off[g]; r < p2p_off[g + 1]; ++r) pts += p2p_hi[r] - p2p_lo[r];
+    const long long nc = m2p_off[g + 1] - m2p_off[g];
+    const long long ntg = g * PB_TG + PB_TG <= N ? PB_TG : N - g * PB_TG;
+    cost[g] = ntg * (pts + 9 * nc);
+    pairs[2 * g] = ntg * pts;
+    pairs[2 * g + 1] = ntg * nc;
+}
+
+extern "C" int pb_shard_partition(const int64_t* cost, int64_t G, int world, int64_t* first)
+{
+    if (!cost || !first || G < 0 || world < 1) return PB_ERR_INVALID_ARG;
+    long double total = 0;
+    for (int64_t g = 0; g < G; ++g) {
+        if (cost[g] < 0) return PB_ERR_INVALID_ARG;
+        total += (long double)cost[g];
+    }
+    first[0] = 0;
+    int64_t g = 0;
+    long double pre = 0;                               // exclusive prefix sum at g
+    for (int k = 1; k < world; ++k) {
+        const long double want = total * (long double)k / (long double)world;
+        while (g < G && pre < want) pre += (long double)cost[g++];
+        first[k] = g;
+    }
+    first[world] = G;
     return PB_OK;
 }
 
@@ -708,7 +766,7 @@ int pb_tree_build_impl(pb_ctx* ctx)
     // error against the oracle on sampled rows 3.2 / 3.3 / 3.6 / 4.6 / 6.8 e-5 (bound 1e-4).
     {
         const int P = ctx->prm.order_P;
-        const double tl = P >= 4 && P <= 6 ? 0.8 * pow(ctx->prm.theta, (double)(P + 1) / (double)(P - 1)) : 0.0;
+        const double tl = P >= 4 && P <= 8 ? 0.8 * pow(ctx->prm.theta, (double)(P + 1) / (double)(P - 1)) : 0.0;
         a.theta_low2 = tl * tl;
     }
     a.m2p_min = 8;   // an M2P pair costs about as much as 8 P2P pairs (D: section 7)
@@ -744,6 +802,16 @@ int pb_tree_build_impl(pb_ctx* ctx)
     a.m2p_low = m2p_low;
     k_lists<1, 2><<<pb_blocks(G, LIST_WARPS), LIST_WARPS * 32, 0, st>>>(a);
     PB_LAUNCH_CHECK();
+    if (tot_m > 0 && a.theta_low2 > 0.0) {
+        int32_t* cell_tmp;
+        int8_t* low_tmp;
+        PB_TRY(pb_dalloc_t(ctx, &cell_tmp, tot_m, CAT_TMP));
+        PB_TRY(pb_dalloc_t(ctx, &low_tmp, tot_m, CAT_TMP));
+        PB_CUDA(cudaMemcpyAsync(cell_tmp, t.m2p_cell, sizeof(int32_t) * tot_m, cudaMemcpyDeviceToDevice, st));
+        PB_CUDA(cudaMemcpyAsync(low_tmp, m2p_low, sizeof(int8_t) * tot_m, cudaMemcpyDeviceToDevice, st));
+        k_partition_low<<<pb_blocks(G, 128), 128, 0, st>>>(G, t.m2p_off, cell_tmp, low_tmp, t.m2p_cell, m2p_low);
+        PB_LAUNCH_CHECK();
+    }
     PB_TRY(pb_cover_count(ctx, G, PB_TG, N, t.m2p_off, t.m2p_cell, t.p2p_off, t.p2p_lo, t.p2p_hi, &t.covered_pairs));
     PB_TRY(pb_dalloc_t(ctx, &t.m2p_ctr, tot_m > 0 ? tot_m : 1, CAT_TREE));
     if (tot_m > 0) {
@@ -751,7 +819,44 @@ int pb_tree_build_impl(pb_ctx* ctx)
         PB_LAUNCH_CHECK();
     }
 
-    // work items: about 8 blocks per resident-block slot (148 SMs x 3 blocks), never less than one
+    // --- target sharding: this rank's contiguous range of groups (everything when world == 1)
+    const int world = ctx->shard_world, rank = ctx->shard_rank;
+    t.own_g0 = 0; t.own_g1 = G;
+    t.shard_first.assign(world + 1, 0);
+    t.shard_first[world] = N;
+    if (world > 1) {
+        long long *dcost, *dpairs;
+        PB_TRY(pb_dalloc_t(ctx, &dcost, G, CAT_TMP));
+        PB_TRY(pb_dalloc_t(ctx, &dpairs, 2 * G, CAT_TMP));
+        k_group_cost<<<pb_blocks(G, 128), 128, 0, st>>>(G, N, t.m2p_off, t.p2p_off, t.p2p_lo, t.p2p_hi, dcost, dpairs);
+        PB_LAUNCH_CHECK();
+        std::vector<int64_t> hcost(G), hpairs(2 * G), gfirst(world + 1);
+        PB_CUDA(cudaMemcpyAsync(hcost.data(), dcost, sizeof(int64_t) * G, cudaMemcpyDeviceToHost, st));
+        PB_CUDA(cudaMemcpyAsync(hpairs.data(), dpairs, sizeof(int64_t) * 2 * G, cudaMemcpyDeviceToHost, st));
+        PB_CUDA(cudaStreamSynchronize(st));
+        if (pb_shard_partition(hcost.data(), G, world, gfirst.data()) != PB_OK) return pb_fail(ctx, PB_ERR_INVALID_ARG, "internal: shard partition");
+        t.own_g0 = gfirst[rank]; t.own_g1 = gfirst[rank + 1];
+        t.shard_nmax = 0;
+        for (int k = 0; k <= world; ++k) t.shard_first[k] = gfirst[k] * PB_TG < N ? gfirst[k] * PB_TG : N;
+        for (int k = 0; k < world; ++k)
+            if (t.shard_first[k + 1] - t.shard_first[k] > t.shard_nmax) t.shard_nmax = t.shard_first[k + 1] - t.shard_first[k];
+        int64_t pp = 0, mp = 0;
+        for (int64_t g = t.own_g0; g < t.own_g1; ++g) { pp += hpairs[2 * g]; mp += hpairs[2 * g + 1]; }
+        t.p2p_pairs = pp;                           // pb_stats: the owned groups' pairs
+        t.m2p_pairs = mp;
+        t.m2p_pairs_low = 0;                        // (not tracked per group)
+        PB_TRY(pb_dalloc_t(ctx, &t.shard_first_dev, world + 1, CAT_TREE));
+        PB_CUDA(cudaMemcpyAsync(t.shard_first_dev, t.shard_first.data(), sizeof(int64_t) * (world + 1), cudaMemcpyHostToDevice, st));
+        const int64_t nm = t.shard_nmax > 0 ? t.shard_nmax : 1;
+        PB_TRY(pb_dalloc_t(ctx, &t.ysend, 2 * nm, CAT_TREE));
+        PB_TRY(pb_dalloc_t(ctx, &t.yall, (size_t)world * 2 * nm, CAT_TREE));
+        PB_CUDA(cudaMemsetAsync(t.ysend, 0, sizeof(double) * 2 * nm, st));
+        PB_CUDA(cudaStreamSynchronize(st));         // shard_first's host storage is a member; the sync is for hcost / hpairs reuse
+    }
+    t.own_i0 = t.own_g0 * PB_TG < N ? t.own_g0 * PB_TG : N;
+    t.own_i1 = t.own_g1 * PB_TG < N ? t.own_g1 * PB_TG : N;
+
+    // work items: about 8 blocks per resident-block slot (148 SMs x 3 blocks) of THIS rank, never less than one
     // tile of 128 source points / 4 cells per block
     {
         const int64_t slots = 148 * 3 * 8;
@@ -770,6 +875,15 @@ int pb_tree_build_impl(pb_ctx* ctx)
         if (t.nslot_m2p < 1) t.nslot_m2p = 1;
         PB_TRY(pb_dalloc_t(ctx, &t.accP, (size_t)t.nslot_p2p * 4 * N, CAT_TREE));
         PB_TRY(pb_dalloc_t(ctx, &t.accM, (size_t)t.nslot_m2p * 4 * N, CAT_TREE));
+        // items are stored group by group: the owned groups' items are one contiguous run
+        int32_t ho[4] = {0, 0, 0, 0};
+        PB_CUDA(cudaMemcpyAsync(&ho[0], t.itemP_off + t.own_g0, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+        PB_CUDA(cudaMemcpyAsync(&ho[1], t.itemP_off + t.own_g1, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+        PB_CUDA(cudaMemcpyAsync(&ho[2], t.itemM_off + t.own_g0, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+        PB_CUDA(cudaMemcpyAsync(&ho[3], t.itemM_off + t.own_g1, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+        PB_CUDA(cudaStreamSynchronize(st));
+        t.itemP0 = ho[0]; t.n_itemP_own = ho[1] - ho[0];
+        t.itemM0 = ho[2]; t.n_itemM_own = ho[3] - ho[2];
     }
     PB_CUDA(cudaStreamSynchronize(st));
     pb_dfree_cat(ctx, CAT_TMP);

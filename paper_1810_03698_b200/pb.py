@@ -27,7 +27,7 @@ EXPORTS = [
     "pb_get_params", "pb_mesh_load", "pb_sites_load", "pb_tree_build", "pb_rhs_multipole", "pb_matvec",
     "pb_matvec_timed", "pb_matvec_host", "pb_reaction_field", "pb_multipole_field", "pb_gmres", "pb_solve",
     "pb_solve_host", "pb_get_stats", "pb_fp64_peak_probe", "pb_set_profiling", "pb_quadrature_rule",
-    "pb_gauss_legendre", "pb_farfield_table", "pb_binding_cycle",
+    "pb_gauss_legendre", "pb_farfield_table", "pb_binding_cycle", "pb_set_shard", "pb_get_shard", "pb_shard_partition",
 ]
 
 
@@ -104,6 +104,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(bdir, exist_ok=True)
     hnew = max(os.path.getmtime(h) for h in hdrs)
     cflags = [f for f in NVCC_FLAGS if f != "-shared"] + (["-Xptxas", "-v"] if verbose else [])
+    cflags += os.environ.get("PB_NVCC_EXTRA", "").split()          # experiments: extra -D switches
 
     def compile_one(src):
         obj = os.path.join(bdir, os.path.basename(src)[:-3] + ".o")
@@ -120,6 +121,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
 _lib = None
 _ALLOC_T = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t)
 _FREE_T = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_void_p)
+_GATHER_T = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t)
 
 
 def lib():
@@ -159,6 +161,9 @@ def lib():
         L.pb_gauss_legendre.argtypes = [ctypes.c_int, vp, vp]
         L.pb_farfield_table.argtypes = [ctypes.c_int, vp, vp, vp, vp, ctypes.POINTER(i64)]
         L.pb_binding_cycle.argtypes = [ctypes.POINTER(Result)] * 3 + [ctypes.POINTER(Binding)]
+        L.pb_set_shard.argtypes = [vp, ctypes.c_int, ctypes.c_int, _GATHER_T, vp]
+        L.pb_get_shard.argtypes = [vp, ctypes.POINTER(i64)]
+        L.pb_shard_partition.argtypes = [ctypes.POINTER(i64), i64, ctypes.c_int, ctypes.POINTER(i64)]
         for name in EXPORTS:
             if name not in ("pb_last_error", "pb_default_params"):
                 getattr(L, name).restype = ctypes.c_int
@@ -180,6 +185,18 @@ def binding_cycle(res_ab: dict, res_a: dict, res_b: dict) -> dict:
     if rc not in (PB_OK, PB_ERR_NO_CONVERGENCE):
         raise PBError(rc, "pb_binding_cycle")
     return dict(dG_bind_vac=out.dG_bind_vac, ddG_bind=out.ddG_bind, dG_bind_diss=out.dG_bind_diss, converged=rc == PB_OK)
+
+
+def shard_partition(cost, world: int):
+    """The library's partition rule (host-only call): first [world + 1] group boundaries for per-group costs."""
+    import numpy as np
+    cost = np.ascontiguousarray(cost, dtype=np.int64)
+    first = np.zeros(world + 1, dtype=np.int64)
+    i64p = ctypes.POINTER(ctypes.c_int64)
+    rc = lib().pb_shard_partition(cost.ctypes.data_as(i64p), cost.size, world, first.ctypes.data_as(i64p))
+    if rc != PB_OK:
+        raise PBError(rc, "pb_shard_partition")
+    return first
 
 
 def default_params() -> Params:
@@ -325,6 +342,45 @@ class PB:
 
     def tree_build(self):
         self._ck(self._L.pb_tree_build(self._h))
+
+    # -- multi-GPU target sharding ------------------------------------------------------------------
+    def set_shard(self, rank: int, world: int, group=None, exchange: bool = True, gather=None):
+        """This context evaluates rank's share of the target groups (call before tree_build).  With `exchange` the
+        owned rows of y are all-gathered over torch.distributed's `group` (NCCL) inside every matvec, so y is complete
+        on every rank; without it only the owned rows of y are written.  `gather(send, recv)` replaces the
+        collective (tests: send is a float64 tensor of 2 * nmax values, recv of world times as many)."""
+        self._shard = (rank, world)
+        if world > 1 and exchange:
+            torch = self.torch
+            if gather is None:
+                import torch.distributed as dist
+
+                def gather(s, r):
+                    dist.all_gather_into_tensor(r, s, group=group)     # enqueued on the current (= the context's) stream
+
+            def _gather(_user, send, recv, nbytes):
+                try:
+                    s = self._bufs[send][:nbytes].view(torch.float64)
+                    r = self._bufs[recv][:nbytes * world].view(torch.float64)
+                    gather(s, r)
+                    return 0
+                except Exception:                                      # never let an exception cross the C boundary
+                    import traceback
+                    traceback.print_exc()
+                    return 1
+
+            self._gather_cb = _GATHER_T(_gather)
+        else:
+            self._gather_cb = _GATHER_T()                              # NULL
+        self._ck(self._L.pb_set_shard(self._h, rank, world, self._gather_cb, None))
+
+    def shard_ranges(self):
+        """first [world + 1]: first owned panel (Morton order) of every rank, after tree_build."""
+        import numpy as np
+        world = getattr(self, "_shard", (0, 1))[1]
+        first = np.zeros(world + 1, dtype=np.int64)
+        self._ck(self._L.pb_get_shard(self._h, first.ctypes.data_as(ctypes.POINTER(ctypes.c_int64))))
+        return first
 
     # -- operators ----------------------------------------------------------------------------------
     def rhs_multipole(self, mu=None):
