@@ -192,11 +192,13 @@ extern "C" int pb_set_params(pb_ctx* ctx, const pb_params* p)
     if (shape && ctx->tree.built) {
         pb_dfree_cat(ctx, CAT_TREE);
         pb_dfree_cat(ctx, CAT_SITE_NEAR);
+    pb_dfree_cat(ctx, CAT_RHS);
         pb_dfree_cat(ctx, CAT_SOLVE);
         ctx->gws = pb_gmres_ws();
         ctx->tree = pb_tree();
         ctx->sites.near_built = false;
         ctx->sites.tree_built = false;
+        ctx->sites.rhs_built = false;
     }
     return PB_OK;
 }
@@ -214,11 +216,13 @@ extern "C" int pb_set_shard(pb_ctx* ctx, int rank, int world, pb_allgather_fn al
     if (ctx->tree.built) {                      // the work items and needed cells depend on the owned range
         pb_dfree_cat(ctx, CAT_TREE);
         pb_dfree_cat(ctx, CAT_SITE_NEAR);
+    pb_dfree_cat(ctx, CAT_RHS);
         pb_dfree_cat(ctx, CAT_SOLVE);
         ctx->gws = pb_gmres_ws();
         ctx->tree = pb_tree();
         ctx->sites.near_built = false;
         ctx->sites.tree_built = false;
+        ctx->sites.rhs_built = false;
     }
     return PB_OK;
 }
@@ -304,12 +308,14 @@ extern "C" int pb_mesh_load(pb_ctx* ctx, const double* verts, int64_t nv, const 
     PB_CUDA(cudaSetDevice(ctx->device));
     pb_dfree_cat(ctx, CAT_TREE);
     pb_dfree_cat(ctx, CAT_SITE_NEAR);
+    pb_dfree_cat(ctx, CAT_RHS);
     pb_dfree_cat(ctx, CAT_SOLVE);
     ctx->gws = pb_gmres_ws();
     pb_dfree_cat(ctx, CAT_MESH);
     ctx->tree = pb_tree();
     ctx->sites.near_built = false;
         ctx->sites.tree_built = false;
+        ctx->sites.rhs_built = false;
     ctx->mesh_loaded = false;
     ctx->nv = nv;
     ctx->nt = nt;
@@ -387,6 +393,7 @@ extern "C" int pb_sites_load(pb_ctx* ctx, int64_t na, const double* pos, const d
         return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_sites_load: na >= 1 and non-NULL arrays required");
     PB_CUDA(cudaSetDevice(ctx->device));
     pb_dfree_cat(ctx, CAT_SITE_NEAR);
+    pb_dfree_cat(ctx, CAT_RHS);
     pb_dfree_cat(ctx, CAT_SITES);
     pb_sites& s = ctx->sites;
     s = pb_sites();
@@ -427,11 +434,13 @@ extern "C" int pb_tree_build(pb_ctx* ctx)
     PB_CUDA(cudaSetDevice(ctx->device));
     pb_dfree_cat(ctx, CAT_TREE);
     pb_dfree_cat(ctx, CAT_SITE_NEAR);
+    pb_dfree_cat(ctx, CAT_RHS);
     pb_dfree_cat(ctx, CAT_SOLVE);
     ctx->gws = pb_gmres_ws();
     ctx->tree = pb_tree();
     ctx->sites.near_built = false;
         ctx->sites.tree_built = false;
+        ctx->sites.rhs_built = false;
     ctx->attr_m2p_mask = 0;
     ctx->attr_up_bytes = 0;
     ctx->attr_site_bytes[0] = ctx->attr_site_bytes[1] = 0;
@@ -484,6 +493,11 @@ extern "C" int pb_get_stats(pb_ctx* ctx, pb_stats* out)
     out->ncrit_used = t.ncrit_used;
     out->m2p_pairs_low = t.m2p_pairs_low;
     out->covered_pairs = t.covered_pairs;
+    if (ctx->sites.rhs_built) {
+        out->rhs_p2p_pairs = ctx->sites.r_ls.p2p_pairs;
+        out->rhs_m2p_pairs = ctx->sites.r_ls.m2p_pairs;
+        out->rhs_covered_pairs = ctx->sites.r_ls.covered_pairs;
+    }
     if (ctx->sites.tree_built) {
         out->site_p2p_pairs = ctx->sites.t_p2p_pairs;
         out->site_m2p_pairs = ctx->sites.t_m2p_pairs;

@@ -13,6 +13,7 @@
 
 #define PB_INV4PI 0.079577471545947667884
 #define PB_MAX_P 10
+#define PB_MAX_NK_ 286   // pb_nk(PB_MAX_P)
 #define PB_SITE_THETA_SCALE 0.7   // site lists: theta_site = 0.7 theta (pb_tree.cu, pb_site_lists_build)
 #define PB_TG 64            // targets (panels) per target group = threads per M2P/P2P block
 #define PB_KCAL 332.0636    // e^2/Angstrom -> kcal/mol (D: R-1)
@@ -26,7 +27,7 @@ __host__ __device__ static inline int mom_index(int a, int b, int c)
 }
 __host__ __device__ static constexpr int pb_nk(int P) { return (P + 1) * (P + 2) * (P + 3) / 6; }
 
-enum pb_mem_cat { CAT_MESH = 0, CAT_SITES = 1, CAT_TREE = 2, CAT_SOLVE = 3, CAT_SITE_NEAR = 4, CAT_TMP = 5, CAT_COUNT = 6 };
+enum pb_mem_cat { CAT_MESH = 0, CAT_SITES = 1, CAT_TREE = 2, CAT_SOLVE = 3, CAT_SITE_NEAR = 4, CAT_TMP = 5, CAT_RHS = 6, CAT_COUNT = 7 };
 
 // Symmetric Gauss rule on the triangle (barycentric nodes, weights summing to 1) and a
 // Gauss-Legendre rule on [-1,1]; passed to kernels by value.
@@ -97,6 +98,7 @@ struct pb_tree {
     int32_t* need_leaf = nullptr;    // leaves whose moments are needed (one k_upward block each)
     int32_t* up_link = nullptr;      // [cells] bit 0: F terms wanted; bits 1..: 1 + parent if the parent needs moments
     int32_t* up_count = nullptr;     // [cells] children finished so far (self-resetting)
+    unsigned char* kexp = nullptr; // [3][PB_MAX_NK_] exponents (a, b, c) of moment index k (device copy for kernels outside pb_matvec.cu)
     int32_t* cv_off = nullptr;    // [NT+1] conversion table (CSR over source moment indices)
     int32_t* cv_idx = nullptr;
     double* cv_coef = nullptr;
@@ -130,6 +132,18 @@ struct pb_tree {
     double* yall = nullptr;             // [world][2][shard_nmax] gathered rows
 };
 
+// an octree over Morton-sorted items (pb_octree_build) and interaction lists against one (pb_lists_build)
+struct pb_octree {
+    int32_t *c_first = nullptr, *c_last = nullptr, *c_child = nullptr, *c_nchild = nullptr, *leaf_ids = nullptr;
+    double *c_ctr[3] = {0, 0, 0}, *c_rad = nullptr, *c_box = nullptr;
+    int64_t n_cells = 0, n_leaves = 0, n_levels = 0;
+    std::vector<int64_t> gen_start;
+};
+struct pb_lists {
+    int64_t n_groups = 0, m2p_total = 0, p2p_ranges = 0, p2p_pairs = 0, m2p_pairs = 0, covered_pairs = 0;
+    int32_t *m2p_off = nullptr, *m2p_cell = nullptr, *p2p_off = nullptr, *p2p_lo = nullptr, *p2p_hi = nullptr;
+};
+
 struct pb_sites {
     bool loaded = false;
     int64_t na = 0;
@@ -160,6 +174,18 @@ struct pb_sites {
     int32_t* dv_idx = nullptr;     // [10][Nk(P)] index of kappa + l
     double* dv_fac = nullptr;      // [10][Nk(P)] (-1)^|kappa| (kappa + l)! / l!
     int t_P = -1;
+    // treecode for the right-hand side Eq. (8) with the SITES as sources in their own octree (S: section 8(f) item 1,
+    // second half): sites in Morton order, cells, the panel groups' lists against that tree, moments and far-field terms
+    bool rhs_built = false;
+    int32_t* r_perm = nullptr;     // [na] Morton position -> original site index
+    double* r_pos[3] = {0, 0, 0};  // [na] sorted positions (SoA)
+    pb_octree r_oc;
+    pb_lists r_ls;
+    int32_t* r_need = nullptr;     // cells that appear in some list (one block of the moment kernel each)
+    int64_t r_n_need = 0;
+    double* r_FF = nullptr;        // [cells][NTp] far-field terms of the site multipoles (one layer)
+    int r_NTp = 0;                 // row stride: NT rounded up to even (16-byte rows for the TMA copies)
+    int r_P = -1;
 };
 
 // GMRES workspace, kept between solves while the system size and restart length are unchanged
@@ -276,8 +302,16 @@ int pb_morton_order(pb_ctx* ctx, const double* pts, int64_t n, int cat, int32_t*
 int pb_radix_sort(pb_ctx* ctx, uint64_t* k0, uint64_t* k1, int32_t* v0, int32_t* v1, int64_t n, int bits,
                   uint64_t** kout, int32_t** vout);
 int pb_cover_count(pb_ctx* ctx, int64_t G, int tg, int64_t ntargets, const int32_t* m2p_off, const int32_t* m2p_cell,
-                   const int32_t* p2p_off, const int32_t* p2p_lo, const int32_t* p2p_hi, int64_t* out_host);
+                   const int32_t* p2p_off, const int32_t* p2p_lo, const int32_t* p2p_hi, int64_t* out_host,
+                   const int32_t* c_first = nullptr, const int32_t* c_last = nullptr, int K = 0);
+int pb_lists_build(pb_ctx* ctx, int tpl, int64_t ntargets, const double* tx, const double* ty, const double* tz,
+                   const pb_octree& oc, int K, int64_t Ns, double theta, int m2p_min, int cat, pb_lists* out);
+int pb_octree_build(pb_ctx* ctx, const uint64_t* keys, int64_t n, int K, int ncrit, const double* px, const double* py,
+                    const double* pz, int cat, pb_octree* oc);
 int pb_site_lists_build(pb_ctx* ctx);
+// pb_rhstree.cu
+int pb_rhs_tree_build(pb_ctx* ctx);
+int pb_rhs_tree(pb_ctx* ctx, const double* mu, double* b);
 // pb_sitetree.cu
 int pb_site_tree_build(pb_ctx* ctx);
 int pb_reaction_field_tree(pb_ctx* ctx, double* phi, double* grad, double* hess);

@@ -92,6 +92,10 @@ int pb_farfield_setup(pb_ctx* ctx)
     PB_CUDA(cudaMemcpyToSymbolAsync(c_ka, ka, PB_MAX_NK, 0, cudaMemcpyHostToDevice, st));
     PB_CUDA(cudaMemcpyToSymbolAsync(c_kb, kb, PB_MAX_NK, 0, cudaMemcpyHostToDevice, st));
     PB_CUDA(cudaMemcpyToSymbolAsync(c_kc, kc, PB_MAX_NK, 0, cudaMemcpyHostToDevice, st));
+    PB_TRY(pb_dalloc_t(ctx, &t.kexp, 3 * PB_MAX_NK_, CAT_TREE));
+    PB_CUDA(cudaMemcpyAsync(t.kexp, ka, PB_MAX_NK, cudaMemcpyHostToDevice, st));
+    PB_CUDA(cudaMemcpyAsync(t.kexp + PB_MAX_NK_, kb, PB_MAX_NK, cudaMemcpyHostToDevice, st));
+    PB_CUDA(cudaMemcpyAsync(t.kexp + 2 * PB_MAX_NK_, kc, PB_MAX_NK, cudaMemcpyHostToDevice, st));
     PB_CUDA(cudaStreamSynchronize(st));   // ka, kb, kc live on this stack frame
     // conversion table M -> F, entries in the order the M2P kernel consumes them
     std::vector<int32_t> off, idx, expo;

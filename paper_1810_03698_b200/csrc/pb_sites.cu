@@ -153,6 +153,13 @@ extern "C" int pb_rhs_multipole(pb_ctx* ctx, const double* mu_induced, double* b
     if (!ctx->mesh_loaded || !ctx->sites.loaded) return pb_fail(ctx, PB_ERR_NOT_READY, "pb_rhs_multipole: load mesh and sites first");
     if (!b) return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_rhs_multipole: NULL output");
     const pb_sites& s = ctx->sites;
+    {   // direct sum over all sites (the paper's choice) or the treecode with the sites as tree sources
+        const pb_tree& t = ctx->tree;
+        const int mode = ctx->prm.rhs_treecode, P = ctx->prm.order_P;
+        const bool tree = t.built && ctx->prm.theta > 0.0 && P >= 1 && P <= 8 &&
+                          (mode == 1 || (mode == 2 && (double)ctx->nt * (double)s.na >= 2147483648.0));
+        if (tree) return pb_rhs_tree(ctx, mu_induced, b);
+    }
     k_rhs<<<pb_blocks(ctx->nt, 128 * RHS_TPT), 128, 0, ctx->stream>>>(ctx->nt, s.na, ctx->cen, s.pos, s.q, s.dip, mu_induced,
                                                                     s.quad, 1.0 / ctx->prm.eps_in, b);
     PB_LAUNCH_CHECK();

@@ -594,14 +594,16 @@ __global__ void k_cover_count(int64_t G, int tg, int64_t ntargets, int K, const 
 }
 
 int pb_cover_count(pb_ctx* ctx, int64_t G, int tg, int64_t ntargets, const int32_t* m2p_off, const int32_t* m2p_cell,
-                   const int32_t* p2p_off, const int32_t* p2p_lo, const int32_t* p2p_hi, int64_t* out_host)
+                   const int32_t* p2p_off, const int32_t* p2p_lo, const int32_t* p2p_hi, int64_t* out_host,
+                   const int32_t* c_first, const int32_t* c_last, int K)
 {
-    pb_tree& t = ctx->tree;
+    const pb_tree& t = ctx->tree;
+    if (!c_first) { c_first = t.c_first; c_last = t.c_last; K = t.K; }   // default: the panel tree
     cudaStream_t st = ctx->stream;
     PB_TRY(pb_scratch(ctx, 1 << 20));
     unsigned long long* d = (unsigned long long*)ctx->scratch;
     PB_CUDA(cudaMemsetAsync(d, 0, sizeof(unsigned long long), st));
-    k_cover_count<<<pb_blocks(G, 128), 128, 0, st>>>(G, tg, ntargets, t.K, m2p_off, m2p_cell, t.c_first, t.c_last, p2p_off,
+    k_cover_count<<<pb_blocks(G, 128), 128, 0, st>>>(G, tg, ntargets, K, m2p_off, m2p_cell, c_first, c_last, p2p_off,
                                                     p2p_lo, p2p_hi, d);
     PB_LAUNCH_CHECK();
     unsigned long long h = 0;
@@ -635,6 +637,76 @@ int pb_morton_order(pb_ctx* ctx, const double* pts, int64_t n, int cat, int32_t*
     if (ks != k0 || vs != v0) return pb_fail(ctx, PB_ERR_INVALID_ARG, "internal: radix sort buffer parity");
     *perm_out = v0;
     if (keys_out) *keys_out = k0;
+    return PB_OK;
+}
+
+// ---- octree over n Morton-sorted items of K points each (panels with their Gauss points; sites with K = 1) ------
+// keys [n] sorted; px, py, pz [n K] the points in the same order.  Cells are numbered generation by generation
+// (parents before children); a cell with more than `ncrit` points is split at the highest differing 3-bit digit.
+int pb_octree_build(pb_ctx* ctx, const uint64_t* keys, int64_t n, int K, int ncrit, const double* px, const double* py,
+                    const double* pz, int cat, pb_octree* oc)
+{
+    cudaStream_t st = ctx->stream;
+    const int64_t cap = 2 * n + 8;
+    PB_TRY(pb_dalloc_t(ctx, &oc->c_first, cap, cat));
+    PB_TRY(pb_dalloc_t(ctx, &oc->c_last, cap, cat));
+    PB_TRY(pb_dalloc_t(ctx, &oc->c_child, cap, cat));
+    PB_TRY(pb_dalloc_t(ctx, &oc->c_nchild, cap, cat));
+    int32_t *nchild, *choff, *bounds;
+    PB_TRY(pb_dalloc_t(ctx, &nchild, cap, CAT_TMP));
+    PB_TRY(pb_dalloc_t(ctx, &choff, cap, CAT_TMP));
+    PB_TRY(pb_dalloc_t(ctx, &bounds, 9 * cap, CAT_TMP));
+    {
+        int32_t root[2] = {0, (int32_t)n};
+        PB_CUDA(cudaMemcpyAsync(oc->c_first, &root[0], sizeof(int32_t), cudaMemcpyHostToDevice, st));
+        PB_CUDA(cudaMemcpyAsync(oc->c_last, &root[1], sizeof(int32_t), cudaMemcpyHostToDevice, st));
+        PB_CUDA(cudaStreamSynchronize(st));
+    }
+    oc->gen_start.clear();
+    oc->gen_start.push_back(0);
+    oc->gen_start.push_back(1);
+    int64_t ncell = 1;
+    for (;;) {
+        int64_t c0 = oc->gen_start[oc->gen_start.size() - 2], c1 = oc->gen_start.back();
+        int64_t ng = c1 - c0;
+        k_cell_split<<<pb_blocks(ng, 128), 128, 0, st>>>(c0, c1, keys, oc->c_first, oc->c_last, K, ncrit, nchild, bounds);
+        PB_LAUNCH_CHECK();
+        int64_t total = 0;
+        PB_TRY(pb_exclusive_scan_i32(ctx, nchild, choff, ng, &total));
+        if (ncell + total > cap) return pb_fail(ctx, PB_ERR_ALLOC, "octree cell capacity exceeded");
+        k_cell_emit<<<pb_blocks(ng, 128), 128, 0, st>>>(c0, c1, nchild, choff, bounds, ncell, oc->c_first, oc->c_last,
+                                                       oc->c_child, oc->c_nchild);
+        PB_LAUNCH_CHECK();
+        if (total == 0) break;
+        ncell += total;
+        oc->gen_start.push_back(ncell);
+    }
+    oc->n_cells = ncell;
+    oc->n_levels = (int64_t)oc->gen_start.size() - 1;
+    {
+        int32_t* flag = nchild;   // reuse
+        k_mark_leaves<<<pb_blocks(ncell, 256), 256, 0, st>>>(ncell, oc->c_child, flag);
+        PB_LAUNCH_CHECK();
+        int64_t nl = 0;
+        PB_TRY(pb_exclusive_scan_i32(ctx, flag, choff, ncell, &nl));
+        oc->n_leaves = nl;
+        PB_TRY(pb_dalloc_t(ctx, &oc->leaf_ids, nl, cat));
+        k_compact_leaves<<<pb_blocks(ncell, 256), 256, 0, st>>>(ncell, oc->c_child, choff, oc->leaf_ids);
+        PB_LAUNCH_CHECK();
+    }
+    // cell geometry, bottom-up
+    for (int d = 0; d < 3; ++d) PB_TRY(pb_dalloc_t(ctx, &oc->c_ctr[d], ncell, cat));
+    PB_TRY(pb_dalloc_t(ctx, &oc->c_rad, ncell, cat));
+    PB_TRY(pb_dalloc_t(ctx, &oc->c_box, 6 * ncell, cat));
+    k_leaf_geom<<<pb_blocks(oc->n_leaves * 32, 128), 128, 0, st>>>(oc->n_leaves, oc->leaf_ids, oc->c_first, oc->c_last, K, px, py, pz,
+                                                                  oc->c_ctr[0], oc->c_ctr[1], oc->c_ctr[2], oc->c_rad, oc->c_box);
+    PB_LAUNCH_CHECK();
+    for (int g = (int)oc->gen_start.size() - 2; g >= 0; --g) {
+        int64_t c0 = oc->gen_start[g], c1 = oc->gen_start[g + 1];
+        k_inner_geom<<<pb_blocks(c1 - c0, 128), 128, 0, st>>>(c0, c1, oc->c_child, oc->c_nchild, oc->c_ctr[0], oc->c_ctr[1],
+                                                             oc->c_ctr[2], oc->c_rad, oc->c_box);
+        PB_LAUNCH_CHECK();
+    }
     return PB_OK;
 }
 
@@ -683,71 +755,20 @@ int pb_tree_build_impl(pb_ctx* ctx)
         PB_LAUNCH_CHECK();
     }
 
-    // --- octree topology
-    const int64_t cap = 2 * N + 8;
-    PB_TRY(pb_dalloc_t(ctx, &t.c_first, cap, CAT_TREE));
-    PB_TRY(pb_dalloc_t(ctx, &t.c_last, cap, CAT_TREE));
-    PB_TRY(pb_dalloc_t(ctx, &t.c_child, cap, CAT_TREE));
-    PB_TRY(pb_dalloc_t(ctx, &t.c_nchild, cap, CAT_TREE));
-    int32_t *nchild, *choff, *bounds;
-    PB_TRY(pb_dalloc_t(ctx, &nchild, cap, CAT_TMP));
-    PB_TRY(pb_dalloc_t(ctx, &choff, cap, CAT_TMP));
-    PB_TRY(pb_dalloc_t(ctx, &bounds, 9 * cap, CAT_TMP));
-    {
-        int32_t root[2] = {0, (int32_t)N};
-        PB_CUDA(cudaMemcpyAsync(t.c_first, &root[0], sizeof(int32_t), cudaMemcpyHostToDevice, st));
-        PB_CUDA(cudaMemcpyAsync(t.c_last, &root[1], sizeof(int32_t), cudaMemcpyHostToDevice, st));
-        PB_CUDA(cudaStreamSynchronize(st));
-    }
+    // --- octree topology and cell geometry
     // leaf capacity: larger leaves shorten the upward pass (the latency-bound part of a small problem)
     t.ncrit_used = ctx->prm.ncrit > 0 ? ctx->prm.ncrit : (Ns < 65536 ? 256 : 192);
-    t.gen_start.clear();
-    t.gen_start.push_back(0);
-    t.gen_start.push_back(1);
-    int64_t ncell = 1;
-    for (;;) {
-        int64_t c0 = t.gen_start[t.gen_start.size() - 2], c1 = t.gen_start.back();
-        int64_t ng = c1 - c0;
-        k_cell_split<<<pb_blocks(ng, 128), 128, 0, st>>>(c0, c1, keys, t.c_first, t.c_last, K, t.ncrit_used, nchild, bounds);
-        PB_LAUNCH_CHECK();
-        int64_t total = 0;
-        PB_TRY(pb_exclusive_scan_i32(ctx, nchild, choff, ng, &total));
-        if (ncell + total > cap) return pb_fail(ctx, PB_ERR_ALLOC, "octree cell capacity exceeded");
-        k_cell_emit<<<pb_blocks(ng, 128), 128, 0, st>>>(c0, c1, nchild, choff, bounds, ncell, t.c_first, t.c_last,
-                                                       t.c_child, t.c_nchild);
-        PB_LAUNCH_CHECK();
-        if (total == 0) break;
-        ncell += total;
-        t.gen_start.push_back(ncell);
-    }
-    t.n_cells = ncell;
-    t.n_levels = (int64_t)t.gen_start.size() - 1;
-    // leaves
     {
-        int32_t* flag = nchild;   // reuse
-        k_mark_leaves<<<pb_blocks(ncell, 256), 256, 0, st>>>(ncell, t.c_child, flag);
-        PB_LAUNCH_CHECK();
-        int64_t nl = 0;
-        PB_TRY(pb_exclusive_scan_i32(ctx, flag, choff, ncell, &nl));
-        t.n_leaves = nl;
-        PB_TRY(pb_dalloc_t(ctx, &t.leaf_ids, nl, CAT_TREE));
-        k_compact_leaves<<<pb_blocks(ncell, 256), 256, 0, st>>>(ncell, t.c_child, choff, t.leaf_ids);
-        PB_LAUNCH_CHECK();
+        pb_octree oc;
+        PB_TRY(pb_octree_build(ctx, keys, N, K, t.ncrit_used, t.sx[0], t.sx[1], t.sx[2], CAT_TREE, &oc));
+        t.c_first = oc.c_first; t.c_last = oc.c_last; t.c_child = oc.c_child; t.c_nchild = oc.c_nchild;
+        for (int d = 0; d < 3; ++d) t.c_ctr[d] = oc.c_ctr[d];
+        t.c_rad = oc.c_rad; t.c_box = oc.c_box; t.leaf_ids = oc.leaf_ids;
+        t.n_cells = oc.n_cells; t.n_leaves = oc.n_leaves; t.n_levels = oc.n_levels;
+        t.gen_start = oc.gen_start;
     }
-    // --- cell geometry, bottom-up
-    for (int d = 0; d < 3; ++d) PB_TRY(pb_dalloc_t(ctx, &t.c_ctr[d], ncell, CAT_TREE));
-    PB_TRY(pb_dalloc_t(ctx, &t.c_rad, ncell, CAT_TREE));
-    PB_TRY(pb_dalloc_t(ctx, &t.c_box, 6 * ncell, CAT_TREE));
-    k_leaf_geom<<<pb_blocks(t.n_leaves * 32, 128), 128, 0, st>>>(t.n_leaves, t.leaf_ids, t.c_first, t.c_last, K, t.sx[0],
-                                                                t.sx[1], t.sx[2], t.c_ctr[0], t.c_ctr[1], t.c_ctr[2],
-                                                                t.c_rad, t.c_box);
-    PB_LAUNCH_CHECK();
-    for (int g = (int)t.gen_start.size() - 2; g >= 0; --g) {
-        int64_t c0 = t.gen_start[g], c1 = t.gen_start[g + 1];
-        k_inner_geom<<<pb_blocks(c1 - c0, 128), 128, 0, st>>>(c0, c1, t.c_child, t.c_nchild, t.c_ctr[0], t.c_ctr[1],
-                                                             t.c_ctr[2], t.c_rad, t.c_box);
-        PB_LAUNCH_CHECK();
-    }
+    const int64_t ncell = t.n_cells;
+    (void)ncell;
 
     // --- target groups
     t.n_groups = (N + PB_TG - 1) / PB_TG;
@@ -887,6 +908,59 @@ int pb_tree_build_impl(pb_ctx* ctx)
     }
     PB_CUDA(cudaStreamSynchronize(st));
     pb_dfree_cat(ctx, CAT_TMP);
+    return PB_OK;
+}
+
+// ---- generic list build: targets (Morton order, groups of 32 * tpl) against any octree --------------------------------
+int pb_lists_build(pb_ctx* ctx, int tpl, int64_t ntargets, const double* tx, const double* ty, const double* tz,
+                   const pb_octree& oc, int K, int64_t Ns, double theta, int m2p_min, int cat, pb_lists* out)
+{
+    cudaStream_t st = ctx->stream;
+    const int tg = 32 * tpl;
+    const int64_t G = (ntargets + tg - 1) / tg;
+    out->n_groups = G;
+    PB_TRY(pb_dalloc_t(ctx, &out->m2p_off, G + 1, cat));
+    PB_TRY(pb_dalloc_t(ctx, &out->p2p_off, G + 1, cat));
+    list_args a;
+    a.ng = G; a.N = ntargets; a.Ns = Ns; a.K = K;
+    a.theta = theta;
+    a.theta_low2 = 0.0;
+    a.m2p_low = nullptr;
+    a.m2p_min = m2p_min;
+    a.c_first = oc.c_first; a.c_last = oc.c_last; a.c_child = oc.c_child; a.c_nchild = oc.c_nchild;
+    a.cx = oc.c_ctr[0]; a.cy = oc.c_ctr[1]; a.cz = oc.c_ctr[2]; a.crad = oc.c_rad;
+    a.px = tx; a.py = ty; a.pz = tz;
+    int32_t *cnt_m, *cnt_p;
+    PB_TRY(pb_dalloc_t(ctx, &cnt_m, G + 1, CAT_TMP));
+    PB_TRY(pb_dalloc_t(ctx, &cnt_p, G + 1, CAT_TMP));
+    PB_CUDA(cudaMemsetAsync(cnt_m, 0, sizeof(int32_t) * (G + 1), st));
+    PB_CUDA(cudaMemsetAsync(cnt_p, 0, sizeof(int32_t) * (G + 1), st));
+    PB_TRY(pb_scratch(ctx, 1 << 20));
+    unsigned long long* pc = (unsigned long long*)ctx->scratch;
+    PB_CUDA(cudaMemsetAsync(pc, 0, 3 * sizeof(unsigned long long), st));
+    a.n_m2p = cnt_m; a.n_p2p = cnt_p; a.m2p_cell = nullptr; a.p2p_lo = nullptr; a.p2p_hi = nullptr;
+    a.pair_counts = pc;
+    if (tpl == 2) k_lists<0, 2><<<pb_blocks(G, LIST_WARPS), LIST_WARPS * 32, 0, st>>>(a);
+    else k_lists<0, 1><<<pb_blocks(G, LIST_WARPS), LIST_WARPS * 32, 0, st>>>(a);
+    PB_LAUNCH_CHECK();
+    unsigned long long hpc[2];
+    PB_CUDA(cudaMemcpyAsync(hpc, pc, sizeof(hpc), cudaMemcpyDeviceToHost, st));
+    int64_t tot_m = 0, tot_p = 0;
+    PB_TRY(pb_exclusive_scan_i32(ctx, cnt_m, out->m2p_off, G + 1, &tot_m));   // synchronises
+    PB_TRY(pb_exclusive_scan_i32(ctx, cnt_p, out->p2p_off, G + 1, &tot_p));
+    out->p2p_pairs = (int64_t)hpc[0];
+    out->m2p_pairs = (int64_t)hpc[1];
+    out->m2p_total = tot_m;
+    out->p2p_ranges = tot_p;
+    PB_TRY(pb_dalloc_t(ctx, &out->m2p_cell, tot_m > 0 ? tot_m : 1, cat));
+    PB_TRY(pb_dalloc_t(ctx, &out->p2p_lo, tot_p > 0 ? tot_p : 1, cat));
+    PB_TRY(pb_dalloc_t(ctx, &out->p2p_hi, tot_p > 0 ? tot_p : 1, cat));
+    a.n_m2p = out->m2p_off; a.n_p2p = out->p2p_off; a.m2p_cell = out->m2p_cell; a.p2p_lo = out->p2p_lo; a.p2p_hi = out->p2p_hi;
+    if (tpl == 2) k_lists<1, 2><<<pb_blocks(G, LIST_WARPS), LIST_WARPS * 32, 0, st>>>(a);
+    else k_lists<1, 1><<<pb_blocks(G, LIST_WARPS), LIST_WARPS * 32, 0, st>>>(a);
+    PB_LAUNCH_CHECK();
+    PB_TRY(pb_cover_count(ctx, G, tg, ntargets, out->m2p_off, out->m2p_cell, out->p2p_off, out->p2p_lo, out->p2p_hi,
+                          &out->covered_pairs, oc.c_first, oc.c_last, K));
     return PB_OK;
 }
 

