@@ -7,7 +7,8 @@ outer algorithms of the paper written out step by step in numpy/scipy:
   (the plain definition of x = A^{-1} b; the GPU path uses GMRES, P:243);
 * the self-consistent induced-dipole loop, steps 1-6 with SOR omega = 0.7
   (P:151-160), in solvent and in vacuum (P:185, 205);
-* the solvation energy, Eq. (19) with each G from Eq. (24).
+* the solvation energy, Eq. (19) with each G from Eq. (24) (P:182, 213);
+* the two-surface (Stern layer) block system of the paper's sphere test, class SternOracle.
 
 Nothing here imports or calls the CUDA path; only tests/, __graft_entry__.smoke
 and bench.py's cpu_baseline / --impl reference legs may import this module.
@@ -297,6 +298,83 @@ class Oracle:
                     G_solvterm=c * G_solv, G_mult_diss=c * G_mult, G_vac=c * G_vac,
                     dG_solv=c * (G_solv + G_mult - G_vac),
                     phi_solv=phi_s, grad_solv=g_s, hess_solv=h_s)
+
+
+class SternOracle(Oracle):
+    """Two nested closed surfaces ("a spherical molecule ... with a 1 Angstrom Stern layer"): Gamma_1, the
+    dielectric boundary enclosing the multipoles (region 1, eps_in, Laplace), and Gamma_2 around it (the ion-exclusion
+    surface); between them the Stern layer (region 2, eps_stern, Laplace: no ions), outside Gamma_2 the solvent
+    (region 3, eps_out, linearised Poisson-Boltzmann with kappa).  The paper uses this only in its sphere test and
+    does not print the block system; it follows from Green's second identity in each region exactly as Eq. (2)/(5)
+    (P:49-79), with both normals pointing away from the molecule and the interface conditions phi continuous,
+    eps d(phi)/dn continuous on each surface (R-32).  Unknowns per panel: phi and q = d(phi)/dn taken on
+    the INNER side of its surface (region 1 on Gamma_1, region 2 on Gamma_2).  With A = sources on Gamma_1,
+    B = sources on Gamma_2, r12 = eps_in / eps_stern, r23 = eps_stern / eps_out:
+      target i on Gamma_1:  y1 = phi_i/2 + K_L^A phi - V_L^A q                                   (region 1)
+                            y2 = phi_i/2 - K_L^A phi + r12 V_L^A q + K_L^B phi - V_L^B q         (region 2, from outside Gamma_1)
+      target i on Gamma_2:  y1 = phi_i/2 + K_L^B phi - V_L^B q - K_L^A phi + r12 V_L^A q         (region 2, from inside Gamma_2)
+                            y2 = phi_i/2 - K_Y^B phi + r23 V_Y^B q                               (region 3)
+    and the right-hand side is Eq. (8) in the region-1 rows only.  Both meshes are held as ONE union mesh (panels
+    [0, n1) = Gamma_1), so every entry -- including the Gamma_1 <-> Gamma_2 ones, FAR or NEAR by the same distance
+    rule R-8 -- comes from the same orc_rows as the single-surface operator.  The reaction potential at the sites is
+    Eq. (12) over Gamma_1's layers alone; SCF loop and energies are inherited unchanged."""
+
+    def __init__(self, verts1, tris1, verts2, tris2, params: Params | None = None, eps_stern: float | None = None):
+        v1 = _f64(verts1).reshape(-1, 3)
+        t1 = np.ascontiguousarray(tris1, dtype=np.int32).reshape(-1, 3)
+        v2 = _f64(verts2).reshape(-1, 3)
+        t2 = np.ascontiguousarray(tris2, dtype=np.int32).reshape(-1, 3)
+        super().__init__(np.concatenate([v1, v2]), np.concatenate([t1, t2 + v1.shape[0]]), params)
+        self.n1 = t1.shape[0]
+        self.eps_stern = self.p.eps_out if eps_stern is None else float(eps_stern)
+
+    def matrix(self):
+        if self._A is None:
+            VL, KL, VY, KY = self.rows()
+            n, n1 = self.nt, self.n1
+            r12, r23 = self.p.eps_in / self.eps_stern, self.eps_stern / self.p.eps_out
+            A_, B_ = slice(0, n1), slice(n1, n)
+            M = np.zeros((2 * n, 2 * n))
+            phi, q = (lambda s: s), (lambda s: slice(n + s.start, n + s.stop))      # column blocks of phi and q
+            row1, row2 = phi, q                                                      # row blocks y1 and y2
+            # targets on Gamma_1
+            M[row1(A_), phi(A_)] = KL[A_, A_]
+            M[row1(A_), q(A_)] = -VL[A_, A_]
+            M[row2(A_), phi(A_)] = -KL[A_, A_]
+            M[row2(A_), q(A_)] = r12 * VL[A_, A_]
+            M[row2(A_), phi(B_)] = KL[A_, B_]
+            M[row2(A_), q(B_)] = -VL[A_, B_]
+            # targets on Gamma_2
+            M[row1(B_), phi(B_)] = KL[B_, B_]
+            M[row1(B_), q(B_)] = -VL[B_, B_]
+            M[row1(B_), phi(A_)] = -KL[B_, A_]
+            M[row1(B_), q(A_)] = r12 * VL[B_, A_]
+            M[row2(B_), phi(B_)] = -KY[B_, B_]
+            M[row2(B_), q(B_)] = r23 * VY[B_, B_]
+            idx = np.arange(n)
+            M[idx, idx] += 0.5
+            M[n + idx, idx] += 0.5
+            self._A = M
+        return self._A
+
+    def matvec(self, x, rows=None):
+        """(y1[rows], y2[rows]) of the block system above, by the dense rows."""
+        x = _f64(x).reshape(2 * self.nt)
+        y = self.matrix() @ x
+        rows = np.arange(self.nt, dtype=np.int64) if rows is None else np.ascontiguousarray(rows, dtype=np.int64)
+        return y[rows], y[self.nt + rows]
+
+    def rhs(self, s: Sites, mu=None):
+        b = super().rhs(s, mu)
+        b[self.n1:self.nt] = 0.0                     # Eq. (8) stands in the region-1 rows only
+        return b
+
+    def reaction(self, x, pos):
+        """Eq. (12), (13), (21) over Gamma_1's layers (the boundary of the region that holds the sites)."""
+        xa = _f64(x).reshape(2 * self.nt).copy()
+        xa[self.n1:self.nt] = 0.0
+        xa[self.nt + self.n1:] = 0.0
+        return super().reaction(xa, pos)
 
 
 def binding_cycle(sol_ab: dict, sol_a: dict, sol_b: dict) -> dict:
