@@ -172,6 +172,24 @@ int pb_mesh_load(pb_ctx* ctx, const double* verts, int64_t nv, const int32_t* tr
 int pb_sites_load(pb_ctx* ctx, int64_t na, const double* pos, const double* q, const double* dip,
                   const double* quad, const double* alpha, const int32_t* group);
 
+/* Two nested surfaces / Stern layer (S: section 8(f) item 3; D: R-32).  The mesh loaded by pb_mesh_load is
+ * the UNION of two closed, outward-oriented surfaces: panels [0, n_inner) form Gamma_1, the dielectric boundary that
+ * encloses every site (region 1: eps_in, Laplace), the others Gamma_2 around it (the ion-exclusion surface); between
+ * them lies the Stern layer (eps_stern, Laplace), outside Gamma_2 the solvent (eps_out, kappa).  x and y keep their
+ * layout [phi (nt); q (nt)] over the union's panels, q being dphi/dn on the INNER side of the panel's surface, and the
+ * rows become (A = sources on Gamma_1, B = on Gamma_2, r12 = eps_in/eps_stern, r23 = eps_stern/eps_out)
+ *   i on Gamma_1:  y[i]      = phi_i/2 + K_L^A phi - V_L^A q
+ *                  y[nt + i] = phi_i/2 - K_L^A phi + r12 V_L^A q + K_L^B phi - V_L^B q
+ *   i on Gamma_2:  y[i]      = phi_i/2 + K_L^B phi - V_L^B q - K_L^A phi + r12 V_L^A q
+ *                  y[nt + i] = phi_i/2 - K_Y^B phi + r23 V_Y^B q
+ * (Green's second identity per region, as Eq. (2)/(5)).  pb_rhs_multipole puts Eq. (8) in the Gamma_1 rows of
+ * the first block only; pb_reaction_field sums Gamma_1's layers only; pb_gmres / pb_solve work unchanged on the
+ * 2 nt system (right block-Jacobi preconditioner from the SELF entries of the region pair of each surface).
+ * pb_matvec evaluates the union's near and far field twice, once per source surface, through the same kernels.
+ * Call after pb_mesh_load and before pb_tree_build; n_inner = 0 switches back to one surface.  Not combined with
+ * pb_set_shard (PB_ERR_INVALID_ARG at pb_tree_build). */
+int pb_set_stern(pb_ctx* ctx, int64_t n_inner, double eps_stern);
+
 /* ---- setup: octree, interaction lists, near/singular table --------------- */
 /* Morton-sorts the panels (63-bit key of the centroid), builds the octree over the K_far
  * Gauss points of whole panels (leaf <= ncrit points), the M2P / P2P lists of every group of 64

@@ -227,6 +227,29 @@ extern "C" int pb_set_shard(pb_ctx* ctx, int rank, int world, pb_allgather_fn al
     return PB_OK;
 }
 
+extern "C" int pb_set_stern(pb_ctx* ctx, int64_t n_inner, double eps_stern)
+{
+    if (!ctx) return PB_ERR_INVALID_ARG;
+    if (!ctx->mesh_loaded) return pb_fail(ctx, PB_ERR_NOT_READY, "pb_set_stern: call pb_mesh_load first");
+    if (n_inner < 0 || n_inner >= ctx->nt) return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_set_stern: need 0 <= n_inner < panels");
+    if (n_inner > 0 && !(eps_stern > 0)) return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_set_stern: eps_stern must be > 0");
+    ctx->stern_n1 = n_inner;
+    ctx->eps_stern = eps_stern;
+    ctx->sites.inside_checked = false;   // with two surfaces the sites must lie inside both
+    if (ctx->tree.built) {
+        pb_dfree_cat(ctx, CAT_TREE);
+        pb_dfree_cat(ctx, CAT_SITE_NEAR);
+        pb_dfree_cat(ctx, CAT_RHS);
+        pb_dfree_cat(ctx, CAT_SOLVE);
+        ctx->gws = pb_gmres_ws();
+        ctx->tree = pb_tree();
+        ctx->sites.near_built = false;
+        ctx->sites.tree_built = false;
+        ctx->sites.rhs_built = false;
+    }
+    return PB_OK;
+}
+
 extern "C" int pb_get_shard(const pb_ctx* ctx, int64_t* first)
 {
     if (!ctx || !first) return PB_ERR_INVALID_ARG;
@@ -317,6 +340,7 @@ extern "C" int pb_mesh_load(pb_ctx* ctx, const double* verts, int64_t nv, const 
         ctx->sites.tree_built = false;
         ctx->sites.rhs_built = false;
     ctx->mesh_loaded = false;
+    ctx->stern_n1 = 0;             // a new mesh is one surface until pb_set_stern says otherwise
     ctx->nv = nv;
     ctx->nt = nt;
     PB_TRY(pb_dalloc_t(ctx, &ctx->verts, 3 * nv, CAT_MESH));
@@ -444,6 +468,8 @@ extern "C" int pb_tree_build(pb_ctx* ctx)
     ctx->attr_m2p_mask = 0;
     ctx->attr_up_bytes = 0;
     ctx->attr_site_bytes[0] = ctx->attr_site_bytes[1] = 0;
+    if (ctx->stern_n1 > 0 && ctx->shard_world > 1)
+        return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_tree_build: the two-surface (Stern) system is not combined with target sharding");
     if (ctx->sites.loaded && !ctx->sites.inside_checked) PB_TRY(pb_check_sites_inside(ctx));
     PB_TRY(pb_upload_rules(ctx));
     PB_TRY(pb_tree_build_impl(ctx));

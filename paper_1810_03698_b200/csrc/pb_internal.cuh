@@ -61,6 +61,9 @@ struct pb_tree {
     double4* srec = nullptr;
     pb_expk ek;                   // constants of exp(-kappa r) for this kappa (M2P)
     pb_expk8 ek8;                 // ... with the 256-entry table (P2P)
+    unsigned char* psurf = nullptr; // [N] Stern mode: 0 = the panel lies on Gamma_1, 1 = on Gamma_2 (Morton order)
+    double* xphi_full = nullptr;  // [N] Stern mode: phi of every panel (xphi holds one surface's at a time)
+    double* sraw = nullptr;       // [2][4][N] Stern mode: V_L, K_L, V_Y, K_Y sums over the sources of Gamma_1 / Gamma_2
     double* xphi = nullptr;       // [N] phi in Morton order
     double* xdphi = nullptr;      // [N]
     // cells
@@ -227,6 +230,8 @@ struct pb_ctx {
     pb_sites sites;
     pb_gmres_ws gws;
     // target sharding: rank / world and the exchange callback (NULL: no exchange, only the owned rows of y are written)
+    int64_t stern_n1 = 0;         // > 0: panels [0, stern_n1) of the loaded mesh are Gamma_1, the rest Gamma_2 (pb_set_stern)
+    double eps_stern = 0.0;
     int shard_rank = 0, shard_world = 1;
     pb_allgather_fn allgather = nullptr;
     void* allgather_user = nullptr;
@@ -324,7 +329,7 @@ int pb_farfield_setup(pb_ctx* ctx);
 int pb_site_farfield_setup(pb_ctx* ctx);
 int pb_upward(pb_ctx* ctx, cudaStream_t fs, const int32_t* leaf_ids, int64_t n_leaf, const int32_t* up_link);
 int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed, bool precond);
-int pb_weights(pb_ctx* ctx, const double* x, bool precond);
+int pb_weights(pb_ctx* ctx, const double* x, bool precond, int surface = -1);   // surface 0 / 1: only that surface's sources
 void pb_make_expk(double kappa, pb_expk* out);
 int pb_make_expk8(pb_ctx* ctx, double kappa, pb_expk8* out);
 // pb_sites.cu

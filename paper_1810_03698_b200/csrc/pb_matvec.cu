@@ -198,8 +198,11 @@ __global__ void k_weights(int64_t N, int K, const int32_t* __restrict__ perm, co
                           const double* __restrict__ sx, const double* __restrict__ sy, const double* __restrict__ sz,
                           const double* __restrict__ nx, const double* __restrict__ ny,
                           const double* __restrict__ nz, double* __restrict__ xphi, double* __restrict__ xdphi,
-                          double4* __restrict__ srec)
+                          double4* __restrict__ srec, const unsigned char* __restrict__ psurf, int keep,
+                          double* __restrict__ xphi_full)
 {
+    // psurf != NULL (two surfaces, pb_set_stern): only the sources of surface `keep` carry weight in this pass;
+    // xphi_full (first pass) receives phi of every panel for the phi_i/2 terms
     int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (s >= N * K) return;
     int64_t i = s / K;
@@ -210,18 +213,24 @@ __global__ void k_weights(int64_t N, int K, const int32_t* __restrict__ perm, co
         phi = pc[o] * a + pc[N + o] * b;
         dphi = pc[2 * N + o] * a + pc[3 * N + o] * b;
     }
+    if (psurf) {
+        if (xphi_full && s == i * K) xphi_full[i] = phi;
+        if (psurf[i] != keep) { phi = 0.0; dphi = 0.0; }
+    }
     if (s == i * K) { xphi[i] = phi; xdphi[i] = dphi; }
     double wp = w * phi;
     srec[2 * s] = make_double4(sx[s], sy[s], sz[s], w * dphi);
     srec[2 * s + 1] = make_double4(wp * nx[i], wp * ny[i], wp * nz[i], 0.0);
 }
 
-int pb_weights(pb_ctx* ctx, const double* x, bool precond)
+int pb_weights(pb_ctx* ctx, const double* x, bool precond, int surface)
 {
     pb_tree& t = ctx->tree;
+    const bool mask = surface >= 0 && t.psurf != nullptr;
     k_weights<<<pb_blocks(t.Ns, 256), 256, 0, ctx->stream>>>(t.N, t.K, t.perm, x, precond ? t.precond : nullptr, t.swA, t.sx[0],
                                                             t.sx[1], t.sx[2], t.pn[0], t.pn[1], t.pn[2], t.xphi, t.xdphi,
-                                                            t.srec);
+                                                            t.srec, mask ? t.psurf : nullptr, surface,
+                                                            mask && surface == 0 ? t.xphi_full : nullptr);
     PB_LAUNCH_CHECK();
     return PB_OK;
 }
@@ -1085,8 +1094,11 @@ k_combine(int64_t N, const int32_t* __restrict__ itemP_off, const int32_t* __res
           const double* __restrict__ accP, const double* __restrict__ accM, const int32_t* __restrict__ el_base,
           const int32_t* __restrict__ el_col, const double* __restrict__ el_val, int64_t ne,
           const double* __restrict__ xphi, const double* __restrict__ xdphi, const int32_t* __restrict__ perm,
-          double* __restrict__ y, int64_t blk0, int64_t i1, double* __restrict__ ymort, int64_t nmax)
+          double* __restrict__ y, int64_t blk0, int64_t i1, double* __restrict__ ymort, int64_t nmax,
+          double* __restrict__ raw)
 {
+    // raw != NULL (two surfaces): the four sums V_L, K_L, V_Y, K_Y of this pass go to raw[m N + i] (Morton order)
+    // instead of being combined into the rows of Eq. (5)
     // blk0, i1: the launch covers the Morton panels [32 blk0, i1) (target sharding; 0, N otherwise).  ymort != NULL:
     // the two rows go to ymort[k], ymort[nmax + k], k = i - 32 blk0 (Morton order, the all-gather send buffer)
     __shared__ double sm[4][32];
@@ -1116,6 +1128,10 @@ k_combine(int64_t N, const int32_t* __restrict__ itemP_off, const int32_t* __res
             for (int q = 0; q < 4; ++q) s = fma(a[q], b[q], s);
         }
         for (; k < width; ++k) s = fma(val[32 * k], xv[col[32 * k]], s);
+    }
+    if (raw) {
+        if (i < i1) raw[(int64_t)m * N + i] = s;
+        return;
     }
     sm[m][tgt] = s;
     __syncthreads();
@@ -1149,6 +1165,29 @@ __global__ void k_shard_scatter(int64_t N, int world, const int64_t* __restrict_
     const int64_t o = perm[i];
     y[o] = src[k];
     y[N + o] = src[nmax + k];
+}
+
+// Two surfaces (pb_set_stern; D: R-32): the rows of the block system from the per-surface sums.
+// sA = sums over Gamma_1's sources, sB = over Gamma_2's; [4][N] each: V_L, K_L, V_Y, K_Y (1/(4 pi) and near table included)
+__global__ void k_stern_combine(int64_t N, const unsigned char* __restrict__ psurf, const double* __restrict__ sA,
+                                const double* __restrict__ sB, const double* __restrict__ xphi_full, double r12, double r23,
+                                const int32_t* __restrict__ perm, double* __restrict__ y)
+{
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const double h = 0.5 * xphi_full[i];
+    const double VLA = sA[i], KLA = sA[N + i], VLB = sB[i], KLB = sB[N + i];
+    double r1, r2;
+    if (psurf[i] == 0) {
+        r1 = h + KLA - VLA;                               // region 1 (inside Gamma_1)
+        r2 = h - KLA + r12 * VLA + KLB - VLB;             // Stern layer, from outside Gamma_1
+    } else {
+        r1 = h + KLB - VLB - KLA + r12 * VLA;             // Stern layer, from inside Gamma_2
+        r2 = h - sB[3 * N + i] + r23 * sB[2 * N + i];     // solvent (Yukawa), outside Gamma_2
+    }
+    const int64_t o = perm[i];
+    y[o] = r1;
+    y[N + o] = r2;
 }
 
 // ---- host driver ----------------------------------------------------------------------------------------------
@@ -1286,60 +1325,72 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed, bool pre
         for (int k = 0; k < 8; ++k) PB_CUDA(cudaEventCreate(&ctx->ev[k]));
         ctx->ev_made = true;
     }
-    const bool far = ctx->prm.theta > 0.0;
-    const bool serial = timed || ctx->profiling;
-    if (timed) PB_CUDA(cudaEventRecord(ctx->ev[0], st));
-    PB_TRY(pb_weights(ctx, x, precond));
-    if (timed) PB_CUDA(cudaEventRecord(ctx->ev[1], st));
-    if (far && serial) PB_TRY(pb_far_branch(ctx, st, timed));
-    if (far && !serial) {
-        // the far-field branch is the longer one on small meshes (a latency chain): enqueue it first
-        PB_CUDA(cudaEventRecord(ctx->ev_fork, st));
-        PB_CUDA(cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0));
-        PB_TRY(pb_far_branch(ctx, ctx->side, false));
-        PB_CUDA(cudaEventRecord(ctx->ev_join, ctx->side));
-    }
-    if (timed) {
-        if (!far) PB_CUDA(cudaEventRecord(ctx->ev[2], st));
-        PB_CUDA(cudaEventRecord(ctx->ev[3], st));
-    }
-    {
-        PB_TRY(pb_prof_begin(ctx, 0));
-        // two targets per lane pays once the kernel is throughput-bound (measured: C3 529 -> 516 us, C4 8.43 -> 8.24 ms;
-        // C1 / C2, a few waves of short blocks, are 2-4 % faster with one target per thread and twice the resident warps)
-        if (t.n_itemP_own > 0) {
-            if (t.N >= 30000)
-                k_p2p2<<<(unsigned)t.n_itemP_own, P2P_THREADS, 0, st>>>(t.N, t.K, ctx->prm.kappa, t.ek8, t.itemP + t.itemP0, t.p2p_lo,
-                                                                      t.p2p_hi, t.srec, t.pc[0], t.pc[1], t.pc[2], t.accP);
-            else
-                k_p2p<<<(unsigned)t.n_itemP_own, P2P_THREADS, 0, st>>>(t.N, t.K, ctx->prm.kappa, t.ek8, t.itemP + t.itemP0, t.p2p_lo,
-                                                                     t.p2p_hi, t.srec, t.pc[0], t.pc[1], t.pc[2], t.accP);
-            PB_LAUNCH_CHECK();
+    const bool stern = t.psurf != nullptr;
+    // two surfaces: the same kernels twice, once with the sources of Gamma_1 and once with those of Gamma_2 (the
+    // sums are linear in the source weights), then the rows of the block system from the two sets of sums
+    for (int surface = stern ? 0 : -1; surface < (stern ? 2 : 0); ++surface) {
+        const bool far = ctx->prm.theta > 0.0;
+        const bool serial = timed || ctx->profiling;
+        if (timed) PB_CUDA(cudaEventRecord(ctx->ev[0], st));
+        PB_TRY(pb_weights(ctx, x, precond, surface));
+        if (timed) PB_CUDA(cudaEventRecord(ctx->ev[1], st));
+        if (far && serial) PB_TRY(pb_far_branch(ctx, st, timed));
+        if (far && !serial) {
+            // the far-field branch is the longer one on small meshes (a latency chain): enqueue it first
+            PB_CUDA(cudaEventRecord(ctx->ev_fork, st));
+            PB_CUDA(cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0));
+            PB_TRY(pb_far_branch(ctx, ctx->side, false));
+            PB_CUDA(cudaEventRecord(ctx->ev_join, ctx->side));
         }
-        PB_TRY(pb_prof_end(ctx, 0));
-        pb_prof_next(ctx);
+        if (timed) {
+            if (!far) PB_CUDA(cudaEventRecord(ctx->ev[2], st));
+            PB_CUDA(cudaEventRecord(ctx->ev[3], st));
+        }
+        {
+            PB_TRY(pb_prof_begin(ctx, 0));
+            // two targets per lane pays once the kernel is throughput-bound (measured: C3 529 -> 516 us, C4 8.43 -> 8.24 ms;
+            // C1 / C2, a few waves of short blocks, are 2-4 % faster with one target per thread and twice the resident warps)
+            if (t.n_itemP_own > 0) {
+                if (t.N >= 30000)
+                    k_p2p2<<<(unsigned)t.n_itemP_own, P2P_THREADS, 0, st>>>(t.N, t.K, ctx->prm.kappa, t.ek8, t.itemP + t.itemP0, t.p2p_lo,
+                                                                          t.p2p_hi, t.srec, t.pc[0], t.pc[1], t.pc[2], t.accP);
+                else
+                    k_p2p<<<(unsigned)t.n_itemP_own, P2P_THREADS, 0, st>>>(t.N, t.K, ctx->prm.kappa, t.ek8, t.itemP + t.itemP0, t.p2p_lo,
+                                                                         t.p2p_hi, t.srec, t.pc[0], t.pc[1], t.pc[2], t.accP);
+                PB_LAUNCH_CHECK();
+            }
+            PB_TRY(pb_prof_end(ctx, 0));
+            pb_prof_next(ctx);
+        }
+        if (far && !serial) PB_CUDA(cudaStreamWaitEvent(st, ctx->ev_join, 0));
+        if (timed) PB_CUDA(cudaEventRecord(ctx->ev[4], st));
+        {
+            // the owned Morton panels [own_i0, own_i1) (all of them without sharding); own_i0 is a multiple of PB_TG = 2 x 32
+            const bool exchange = ctx->shard_world > 1 && ctx->allgather != nullptr;
+            const int64_t nown = t.own_i1 - t.own_i0;
+            if (nown > 0) {
+                k_combine<<<pb_blocks(nown, 32), 128, 0, st>>>(t.N, t.itemP_off, far ? t.itemM_off : nullptr,
+                                                              ctx->prm.eps_in / ctx->prm.eps_out, t.accP, t.accM, t.el_base, t.el_col,
+                                                              t.el_val, t.el_entries, t.xphi, t.xdphi, t.perm, y, t.own_i0 / 32,
+                                                              t.own_i1, exchange ? t.ysend : nullptr, t.shard_nmax,
+                                                              surface >= 0 ? t.sraw + (size_t)surface * 4 * t.N : nullptr);
+                PB_LAUNCH_CHECK();
+            }
+            if (exchange && surface < 0) {
+                // the ONE exchange step of a sharded matvec: all-gather of the owned rows (enqueued on this stream by the callback)
+                if (ctx->allgather(ctx->allgather_user, t.ysend, t.yall, (size_t)2 * t.shard_nmax * sizeof(double)) != 0)
+                    return pb_fail(ctx, PB_ERR_CUDA, "pb_matvec: the all-gather callback failed");
+                k_shard_scatter<<<pb_blocks(t.N, 256), 256, 0, st>>>(t.N, ctx->shard_world, t.shard_first_dev, t.shard_nmax, t.yall,
+                                                                    t.perm, y);
+                PB_LAUNCH_CHECK();
+            }
+        }
     }
-    if (far && !serial) PB_CUDA(cudaStreamWaitEvent(st, ctx->ev_join, 0));
-    if (timed) PB_CUDA(cudaEventRecord(ctx->ev[4], st));
-    {
-        // the owned Morton panels [own_i0, own_i1) (all of them without sharding); own_i0 is a multiple of PB_TG = 2 x 32
-        const bool exchange = ctx->shard_world > 1 && ctx->allgather != nullptr;
-        const int64_t nown = t.own_i1 - t.own_i0;
-        if (nown > 0) {
-            k_combine<<<pb_blocks(nown, 32), 128, 0, st>>>(t.N, t.itemP_off, far ? t.itemM_off : nullptr,
-                                                          ctx->prm.eps_in / ctx->prm.eps_out, t.accP, t.accM, t.el_base, t.el_col,
-                                                          t.el_val, t.el_entries, t.xphi, t.xdphi, t.perm, y, t.own_i0 / 32,
-                                                          t.own_i1, exchange ? t.ysend : nullptr, t.shard_nmax);
-            PB_LAUNCH_CHECK();
-        }
-        if (exchange) {
-            // the ONE exchange step of a sharded matvec: all-gather of the owned rows (enqueued on this stream by the callback)
-            if (ctx->allgather(ctx->allgather_user, t.ysend, t.yall, (size_t)2 * t.shard_nmax * sizeof(double)) != 0)
-                return pb_fail(ctx, PB_ERR_CUDA, "pb_matvec: the all-gather callback failed");
-            k_shard_scatter<<<pb_blocks(t.N, 256), 256, 0, st>>>(t.N, ctx->shard_world, t.shard_first_dev, t.shard_nmax, t.yall,
-                                                                t.perm, y);
-            PB_LAUNCH_CHECK();
-        }
+    if (stern) {
+        k_stern_combine<<<pb_blocks(t.N, 256), 256, 0, st>>>(t.N, t.psurf, t.sraw, t.sraw + (size_t)4 * t.N, t.xphi_full,
+                                                            ctx->prm.eps_in / ctx->eps_stern, ctx->eps_stern / ctx->prm.eps_out,
+                                                            t.perm, y);
+        PB_LAUNCH_CHECK();
     }
     ctx->matvec_calls++;
     if (timed) {

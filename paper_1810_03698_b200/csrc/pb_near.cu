@@ -310,6 +310,8 @@ struct entry_args {
     double* tval;       // [4][ne] the true three-zone entries (the near-field matrix of the preconditioner)
     double* precond;    // [4][N], ORIGINAL panel order
     int64_t N;
+    const unsigned char* psurf;   // two surfaces (pb_set_stern): the panel's surface, else NULL
+    double r12, r23;              // eps_in / eps_stern, eps_stern / eps_out
 };
 
 // One thread per table entry.
@@ -330,8 +332,10 @@ __global__ void k_near_entries(entry_args a, pb_rule_t ruleN, pb_gl_t gl)
         out[1] = 0.0;   // flat panel: n'.(c_i - r') == 0 on the panel itself
         out[3] = 0.0;
         for (int m = 0; m < 4; ++m) a.tval[(int64_t)m * a.ne + e] = out[m];
-        // inverse of the 2x2 diagonal block [[1/2, -V_L],[1/2, (eps1/eps2) V_Y]] (right preconditioner)
+        // inverse of the 2x2 diagonal block [[1/2, -V_L],[1/2, (eps1/eps2) V_Y]] (right preconditioner); with two
+        // surfaces the second row of a Gamma_1 panel is the Stern layer's Laplace row, of a Gamma_2 panel the solvent's
         double m01 = -out[0], m11 = a.eps_ratio * out[2];
+        if (a.psurf) m11 = a.psurf[i] == 0 ? a.r12 * out[0] : a.r23 * out[2];
         double det = 0.5 * m11 - m01 * 0.5;
         int64_t o = a.perm[i];
         a.precond[o] = m11 / det;
@@ -460,6 +464,9 @@ int pb_near_build(pb_ctx* ctx)
     for (int k = 0; k < 9; ++k) e.pv[k] = t.pv[k];
     e.sx = t.sx[0]; e.sy = t.sx[1]; e.sz = t.sx[2]; e.swA = t.swA;
     e.val = nr_val; e.tval = nr_tval; e.precond = t.precond; e.N = N;
+    e.psurf = t.psurf;
+    e.r12 = t.psurf ? ctx->prm.eps_in / ctx->eps_stern : 0.0;
+    e.r23 = t.psurf ? ctx->eps_stern / ctx->prm.eps_out : 0.0;
     k_near_entries<<<pb_blocks(ne, 128), 128, 0, st>>>(e, ctx->ruleN, ctx->gl);
     PB_LAUNCH_CHECK();
     // sliced ELL for the combine kernel

@@ -24,7 +24,7 @@ __global__ void k_area_normals(int64_t nt, const double* __restrict__ verts, con
 #define IN_ST 8
 __global__ void __launch_bounds__(256)
 k_sites_inside(int64_t na, int64_t nt, const double* __restrict__ pos, const double* __restrict__ cen,
-               const double* __restrict__ an, int* __restrict__ first_bad)
+               const double* __restrict__ an, double thresh, int* __restrict__ first_bad)
 {
     __shared__ double red[8][IN_ST];
     const int64_t m0 = (int64_t)blockIdx.x * IN_ST;
@@ -57,7 +57,7 @@ k_sites_inside(int64_t na, int64_t nt, const double* __restrict__ pos, const dou
     if (threadIdx.x < IN_ST && m0 + threadIdx.x < na) {
         double v = 0;
         for (int k = 0; k < 8; ++k) v += red[k][threadIdx.x];
-        if (!(v * PB_INV4PI > 0.5)) atomicMin(first_bad, (int)(m0 + threadIdx.x));
+        if (!(v * PB_INV4PI > thresh)) atomicMin(first_bad, (int)(m0 + threadIdx.x));
     }
 }
 
@@ -75,7 +75,7 @@ int pb_check_sites_inside(pb_ctx* ctx)
     PB_CUDA(cudaMemcpyAsync(bad, &none, sizeof(int), cudaMemcpyHostToDevice, st));
     k_area_normals<<<pb_blocks(ctx->nt, 256), 256, 0, st>>>(ctx->nt, ctx->verts, ctx->tris, an);
     PB_LAUNCH_CHECK();
-    k_sites_inside<<<pb_blocks(s.na, IN_ST), 256, 0, st>>>(s.na, ctx->nt, s.pos, ctx->cen, an, bad);
+    k_sites_inside<<<pb_blocks(s.na, IN_ST), 256, 0, st>>>(s.na, ctx->nt, s.pos, ctx->cen, an, ctx->stern_n1 > 0 ? 1.5 : 0.5, bad);   // inside BOTH surfaces: 2
     PB_LAUNCH_CHECK();
     PB_CUDA(cudaMemcpyAsync(&hbad, bad, sizeof(int), cudaMemcpyDeviceToHost, st));
     PB_CUDA(cudaStreamSynchronize(st));
@@ -158,11 +158,19 @@ extern "C" int pb_rhs_multipole(pb_ctx* ctx, const double* mu_induced, double* b
         const int mode = ctx->prm.rhs_treecode, P = ctx->prm.order_P;
         const bool tree = t.built && ctx->prm.theta > 0.0 && P >= 1 && P <= 8 &&
                           (mode == 1 || (mode == 2 && (double)ctx->nt * (double)s.na >= 2147483648.0));
-        if (tree) return pb_rhs_tree(ctx, mu_induced, b);
+        if (tree) {
+            PB_TRY(pb_rhs_tree(ctx, mu_induced, b));
+            if (ctx->stern_n1 > 0)
+                PB_CUDA(cudaMemsetAsync(b + ctx->stern_n1, 0, sizeof(double) * (ctx->nt - ctx->stern_n1), ctx->stream));
+            return PB_OK;
+        }
     }
     k_rhs<<<pb_blocks(ctx->nt, 128 * RHS_TPT), 128, 0, ctx->stream>>>(ctx->nt, s.na, ctx->cen, s.pos, s.q, s.dip, mu_induced,
                                                                     s.quad, 1.0 / ctx->prm.eps_in, b);
     PB_LAUNCH_CHECK();
+    // two surfaces: Eq. (8) stands in the region-1 rows (the panels of Gamma_1) only
+    if (ctx->stern_n1 > 0)
+        PB_CUDA(cudaMemsetAsync(b + ctx->stern_n1, 0, sizeof(double) * (ctx->nt - ctx->stern_n1), ctx->stream));
     return PB_OK;
 }
 
@@ -414,7 +422,7 @@ extern "C" int pb_reaction_field(pb_ctx* ctx, const double* x, double* phi, doub
     if (!phi && !grad && !hess) return PB_OK;
     cudaStream_t st = ctx->stream;
     if (!s.near_built) PB_TRY(pb_site_near_build(ctx));
-    PB_TRY(pb_weights(ctx, x, false));
+    PB_TRY(pb_weights(ctx, x, false, t.psurf ? 0 : -1));   // two surfaces: the layers of Gamma_1 only (it bounds the sites' region)
     // direct sum over every source point (the paper's choice) or the treecode over the panel tree
     const int mode = ctx->prm.site_treecode;
     const bool tree = ctx->prm.theta > 0.0 && ctx->prm.order_P <= 8 &&

@@ -485,6 +485,7 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
     // else block-Jacobi
     int mode = ctx->prm.precond;
     if (mode == 3) mode = t.N >= 8000 ? 2 : 1;
+    if (t.psurf && mode == 2) mode = 1;   // two surfaces: the near-field matrix of mode 2 has Eq. (5)'s single-surface rows
     int m = ctx->prm.gmres_restart;
     if (m > n) m = (int)n;
     if (m > 1000) m = 1000;

@@ -153,6 +153,12 @@ __global__ void k_gather(int64_t N, const int32_t* __restrict__ perm, const doub
     }
 }
 
+__global__ void k_panel_surface(int64_t N, const int32_t* __restrict__ perm, int32_t n1, unsigned char* __restrict__ psurf)
+{
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i < N) psurf[i] = perm[i] >= n1 ? 1 : 0;
+}
+
 // ---- octree topology, one BFS generation at a time -----------------------------------------
 // A cell is a range of Morton-sorted panels.  It is split at the highest 3-bit digit in
 // which its first and last keys differ, so every internal cell has >= 2 children.
@@ -752,6 +758,15 @@ int pb_tree_build_impl(pb_ctx* ctx)
         g.parea = t.parea;
         g.swA = t.swA;
         k_gather<<<pb_blocks(N, 128), 128, 0, st>>>(N, t.perm, ctx->verts, ctx->tris, ctx->ruleF, g);
+        PB_LAUNCH_CHECK();
+    }
+
+    // --- two surfaces (pb_set_stern): which surface a panel lies on, Morton order
+    if (ctx->stern_n1 > 0) {
+        PB_TRY(pb_dalloc_t(ctx, &t.psurf, N, CAT_TREE));
+        PB_TRY(pb_dalloc_t(ctx, &t.xphi_full, N, CAT_TREE));
+        PB_TRY(pb_dalloc_t(ctx, &t.sraw, (size_t)8 * N, CAT_TREE));
+        k_panel_surface<<<pb_blocks(N, 256), 256, 0, st>>>(N, t.perm, (int32_t)ctx->stern_n1, t.psurf);
         PB_LAUNCH_CHECK();
     }
 

@@ -27,7 +27,7 @@ EXPORTS = [
     "pb_get_params", "pb_mesh_load", "pb_sites_load", "pb_tree_build", "pb_rhs_multipole", "pb_matvec",
     "pb_matvec_timed", "pb_matvec_host", "pb_reaction_field", "pb_multipole_field", "pb_gmres", "pb_solve",
     "pb_solve_host", "pb_get_stats", "pb_fp64_peak_probe", "pb_set_profiling", "pb_quadrature_rule",
-    "pb_gauss_legendre", "pb_farfield_table", "pb_binding_cycle", "pb_set_shard", "pb_get_shard", "pb_shard_partition",
+    "pb_gauss_legendre", "pb_farfield_table", "pb_binding_cycle", "pb_set_shard", "pb_get_shard", "pb_shard_partition", "pb_set_stern",
 ]
 
 
@@ -161,6 +161,7 @@ def lib():
         L.pb_gauss_legendre.argtypes = [ctypes.c_int, vp, vp]
         L.pb_farfield_table.argtypes = [ctypes.c_int, vp, vp, vp, vp, ctypes.POINTER(i64)]
         L.pb_binding_cycle.argtypes = [ctypes.POINTER(Result)] * 3 + [ctypes.POINTER(Binding)]
+        L.pb_set_stern.argtypes = [vp, i64, dbl]
         L.pb_set_shard.argtypes = [vp, ctypes.c_int, ctypes.c_int, _GATHER_T, vp]
         L.pb_get_shard.argtypes = [vp, ctypes.POINTER(i64)]
         L.pb_shard_partition.argtypes = [ctypes.POINTER(i64), i64, ctypes.c_int, ctypes.POINTER(i64)]
@@ -339,6 +340,10 @@ class PB:
         self._ck(self._L.pb_sites_load(self._h, na, _ptr(pos), _ptr(q), _ptr(dip), _ptr(quad), _ptr(alpha), _ptr(group)))
         torch.cuda.current_stream(self.device).synchronize()   # inputs may be freed by the caller
         self.na = int(na)
+
+    def set_stern(self, n_inner: int, eps_stern: float):
+        """Panels [0, n_inner) of the loaded (union) mesh are Gamma_1, the rest Gamma_2; see include/pb.h."""
+        self._ck(self._L.pb_set_stern(self._h, int(n_inner), float(eps_stern)))
 
     def tree_build(self):
         self._ck(self._L.pb_tree_build(self._h))
