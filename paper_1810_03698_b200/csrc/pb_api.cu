@@ -624,6 +624,83 @@ extern "C" int pb_fp64_peak_probe(pb_ctx* ctx, double* tflops_out)
     return PB_OK;
 }
 
+// ---- FP64 pipe probe: what the pipe sustains with few resident warps, little instruction-level parallelism, and with
+// integer instructions mixed into the stream (D: section 7; profiles/r02_fp64_pipe_probes.md) ----------------------------
+template <int ILP, int NI, int KIND>
+__global__ void __launch_bounds__(128) k_pipe_probe(int iters, double a, double b, int c, double* __restrict__ out)
+{
+    double x[8];
+    int y[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { x[i] = threadIdx.x * 1e-3 + i; y[i] = threadIdx.x + i; }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 8 / ILP; ++r)
+#pragma unroll
+            for (int i = 0; i < ILP; ++i) {
+                x[i] = fma(x[i], a, b);                                     // ILP independent chains, 8 DFMA per iteration
+                if (r * ILP + i < NI) {
+                    if (KIND == 0) y[i] = y[i] * c + it;                    // IMAD (FMA-heavy / integer-multiply pipe)
+                    else y[i] = (y[i] ^ c) & 0x7fffffff;                    // LOP3 (ALU pipe)
+                }
+            }
+    }
+    double s = 0;
+    int t = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { s += x[i]; t += y[i]; }
+    if (s == 123.456 || t == 77) out[0] = s + t;   // never true; keeps the chains alive
+}
+
+template <int ILP, int NI, int KIND>
+static cudaError_t pipe_probe_launch(int blocks, size_t smem, int iters, double* out, cudaStream_t st)
+{
+    cudaError_t e = cudaFuncSetAttribute(k_pipe_probe<ILP, NI, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_pipe_probe<ILP, NI, KIND><<<blocks, 128, smem, st>>>(iters, 0.999999, 1e-6, 3, out);
+    return cudaGetLastError();
+}
+
+extern "C" int pb_fp64_pipe_probe(pb_ctx* ctx, int warps_per_sm, int ilp, int other_per_8, int other_kind, double* pct_out)
+{
+    if (!ctx || !pct_out) return PB_ERR_INVALID_ARG;
+    if (warps_per_sm < 4 || warps_per_sm > 64 || warps_per_sm % 4) return pb_fail(ctx, PB_ERR_INVALID_ARG, "warps_per_sm: 4 .. 64, a multiple of 4");
+    PB_CUDA(cudaSetDevice(ctx->device));
+    PB_TRY(pb_scratch(ctx, 1 << 20));
+    int nsm = 148, mhz = 1965000;
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, ctx->device);
+    cudaDeviceGetAttribute(&mhz, cudaDevAttrClockRate, ctx->device);      // kHz
+    const int bps = warps_per_sm / 4;                                      // blocks of 4 warps; residency limited by dynamic shared memory
+    const size_t smem = (size_t)200 * 1024 / bps - 1024;
+    const int iters = 20000, blocks = nsm * bps;
+    cudaEvent_t e0, e1;
+    PB_CUDA(cudaEventCreate(&e0));
+    PB_CUDA(cudaEventCreate(&e1));
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+        PB_CUDA(cudaEventRecord(e0, ctx->stream));
+        cudaError_t e = cudaErrorInvalidValue;
+#define PROBE_CASE(I, N, K) if (ilp == I && other_per_8 == N && other_kind == K) e = pipe_probe_launch<I, N, K>(blocks, smem, iters, ctx->scratch, ctx->stream);
+        PROBE_CASE(1, 0, 0) PROBE_CASE(2, 0, 0) PROBE_CASE(4, 0, 0) PROBE_CASE(8, 0, 0)
+        PROBE_CASE(8, 2, 0) PROBE_CASE(8, 4, 0) PROBE_CASE(8, 8, 0) PROBE_CASE(8, 2, 1) PROBE_CASE(8, 4, 1) PROBE_CASE(8, 8, 1)
+#undef PROBE_CASE
+        if (e != cudaSuccess) {
+            cudaEventDestroy(e0); cudaEventDestroy(e1);
+            return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_fp64_pipe_probe: ilp in {1,2,4,8} with other_per_8 = 0, or ilp = 8 with other_per_8 in {2,4,8}, kind 0|1");
+        }
+        PB_CUDA(cudaEventRecord(e1, ctx->stream));
+        PB_CUDA(cudaEventSynchronize(e1));
+        float ms = 0;
+        PB_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    const double inst = 8.0 * iters * (double)blocks * 128.0;
+    *pct_out = 100.0 * inst / (best * 1e-3) / ((double)nsm * 64.0 * (double)mhz * 1e3);
+    return PB_OK;
+}
+
 // ---- profiling ring: event pairs around the P2P / M2P launches ------------------------------------------
 #define PROF_SLOTS 512
 extern "C" int pb_set_profiling(pb_ctx* ctx, int on)

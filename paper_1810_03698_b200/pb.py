@@ -27,7 +27,7 @@ EXPORTS = [
     "pb_get_params", "pb_mesh_load", "pb_sites_load", "pb_tree_build", "pb_rhs_multipole", "pb_matvec",
     "pb_matvec_timed", "pb_matvec_host", "pb_reaction_field", "pb_multipole_field", "pb_gmres", "pb_solve",
     "pb_solve_host", "pb_get_stats", "pb_fp64_peak_probe", "pb_set_profiling", "pb_quadrature_rule",
-    "pb_gauss_legendre", "pb_farfield_table", "pb_binding_cycle", "pb_set_shard", "pb_get_shard", "pb_shard_partition", "pb_set_stern",
+    "pb_gauss_legendre", "pb_farfield_table", "pb_binding_cycle", "pb_set_shard", "pb_get_shard", "pb_shard_partition", "pb_set_stern", "pb_fp64_pipe_probe",
 ]
 
 
@@ -157,6 +157,7 @@ def lib():
         L.pb_get_stats.argtypes = [vp, ctypes.POINTER(Stats)]
         L.pb_fp64_peak_probe.argtypes = [vp, ctypes.POINTER(dbl)]
         L.pb_set_profiling.argtypes = [vp, ctypes.c_int]
+        L.pb_fp64_pipe_probe.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(dbl)]
         L.pb_quadrature_rule.argtypes = [ctypes.c_int, vp, vp]
         L.pb_gauss_legendre.argtypes = [ctypes.c_int, vp, vp]
         L.pb_farfield_table.argtypes = [ctypes.c_int, vp, vp, vp, vp, ctypes.POINTER(i64)]
@@ -466,6 +467,27 @@ class PB:
         v = ctypes.c_double(0.0)
         self._ck(self._L.pb_fp64_peak_probe(self._h, ctypes.byref(v)))
         return v.value
+
+
+def fp64_pipe_table(device: int = 0):
+    """The FP64 pipe probe over resident warps, ILP and mixed-in integer instructions (profiles/r02_fp64_pipe_probes.md):
+    rows of (warps_per_sm, ilp, other_per_8, kind, percent of the DFMA issue peak)."""
+    ctx = PB(device)
+    rows = []
+    try:
+        for wps in (4, 8, 16, 32, 64):
+            for ilp in (1, 2, 4, 8):
+                v = ctypes.c_double(0.0)
+                ctx._ck(ctx._L.pb_fp64_pipe_probe(ctx._h, wps, ilp, 0, 0, ctypes.byref(v)))
+                rows.append((wps, ilp, 0, "-", v.value))
+        for kind, name in ((0, "IMAD"), (1, "LOP3")):
+            for ni in (2, 4, 8):
+                v = ctypes.c_double(0.0)
+                ctx._ck(ctx._L.pb_fp64_pipe_probe(ctx._h, 16, 8, ni, kind, ctypes.byref(v)))
+                rows.append((16, 8, ni, name, v.value))
+    finally:
+        ctx.close()
+    return rows
 
 
 def from_workload(w, device: int = 0, **overrides) -> PB:
