@@ -82,7 +82,10 @@ typedef struct pb_params {
                                1 = treecode with the sites as sources in their own octree (Cartesian multipole
                                moments of q, p, Q per site cell, Laplace far field at the collocation points) when
                                theta > 0, 2 (default) = treecode when N * N_a >= 2^31                          */
-    int32_t reserved0;
+    int32_t scf_recycle;    /* pb_solve: 1 (default) = every GMRES solve of the SCF loop starts from the minimal-residual
+                               combination of the corrections found by the loop's earlier solves (a recycled subspace:
+                               u_k with A u_k known from the Arnoldi relation, no extra operator application), then GMRES
+                               as usual to gmres_tol; 0 = plain warm start from the previous x (D: R-20)              */
 } pb_params;
 
 /* Result of one polarizable solve (HOST struct). */

@@ -100,6 +100,7 @@ extern "C" void pb_default_params(pb_params* p)
     p->site_treecode = 2;
     p->thole_a = 0.39;
     p->rhs_treecode = 2;
+    p->scf_recycle = 1;
 }
 
 extern "C" int pb_create(pb_ctx** out, int device, void* cuda_stream)
@@ -183,6 +184,7 @@ extern "C" int pb_set_params(pb_ctx* ctx, const pb_params* p)
     if (p->precond < 0 || p->precond > 3) return pb_fail(ctx, PB_ERR_INVALID_ARG, "precond must be 0, 1, 2 or 3");
     if (p->site_treecode < 0 || p->site_treecode > 2) return pb_fail(ctx, PB_ERR_INVALID_ARG, "site_treecode must be 0, 1 or 2");
     if (p->rhs_treecode < 0 || p->rhs_treecode > 2) return pb_fail(ctx, PB_ERR_INVALID_ARG, "rhs_treecode must be 0, 1 or 2");
+    if (p->scf_recycle < 0 || p->scf_recycle > 1) return pb_fail(ctx, PB_ERR_INVALID_ARG, "scf_recycle must be 0 or 1");
     const pb_params& o = ctx->prm;
     bool shape = o.kappa != p->kappa || o.theta != p->theta || o.order_P != p->order_P ||
                  o.ncrit != p->ncrit || o.K_far != p->K_far || o.K_near != p->K_near ||

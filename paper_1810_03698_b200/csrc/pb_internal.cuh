@@ -203,6 +203,10 @@ struct pb_gmres_ws {
     bool ax_valid = false;
     double *partial = nullptr, *hdev = nullptr, *coef = nullptr;
     unsigned int* counter = nullptr;   // arrival counter of k_dots' last-block reduction (self-resetting)
+    // recycled subspace of the SCF loop (pb_params.scf_recycle): RU[k] = a past solve's correction, RC[k] = A RU[k],
+    // the RC orthonormal; xb / axb = x and A x before the current solve
+    double *RU = nullptr, *RC = nullptr, *xb = nullptr, *axb = nullptr;
+    int nrec = 0, rec_cap = 0;
 };
 
 struct pb_ctx {

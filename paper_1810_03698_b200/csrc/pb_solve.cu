@@ -762,6 +762,80 @@ __global__ void k_any_nonzero(int64_t n, const double* __restrict__ a, int* __re
     if (e < n && a[e] != 0.0) *flag = 1;
 }
 
+// ---- recycled subspace across the solves of one SCF loop (pb_params.scf_recycle; D: R-20) ---------------------------------
+// The right-hand sides of the loop differ by the field of the changing induced dipoles, b_k = b_perm + B mu_k, and the
+// corrections x_k - x_{k-1} of successive solves are nearly parallel (mu converges geometrically).  Every finished solve
+// contributes its correction u and c = A u -- known from the Arnoldi relation that already carries A x, no operator
+// application -- to a pair of bases RU, RC with RC orthonormal and A RU = RC.  The next solve first takes the
+// minimal-residual step in that space, x += RU (RC^T r), A x += RC (RC^T r), and GMRES then starts from the smaller
+// residual and runs to the same tolerance as without it.
+static int recycle_alloc(pb_ctx* ctx, gmres_ws& ws)
+{
+    if (ws.RU || !ws.V) return PB_OK;
+    int cap = ctx->prm.scf_maxit < 48 ? ctx->prm.scf_maxit : 48;
+    if ((size_t)cap * ws.n * sizeof(double) * 2 > ((size_t)4 << 30)) cap = (int)(((size_t)2 << 30) / (ws.n * sizeof(double)));   // <= 4 GB
+    if (cap > ws.m) cap = ws.m;                         // the dot / coefficient buffers are sized for the restart length
+    if (cap < 1) return PB_OK;
+    PB_TRY(pb_dalloc_t(ctx, &ws.RU, (size_t)cap * ws.n, CAT_SOLVE));
+    PB_TRY(pb_dalloc_t(ctx, &ws.RC, (size_t)cap * ws.n, CAT_SOLVE));
+    PB_TRY(pb_dalloc_t(ctx, &ws.xb, ws.n, CAT_SOLVE));
+    PB_TRY(pb_dalloc_t(ctx, &ws.axb, ws.n, CAT_SOLVE));
+    ws.rec_cap = cap;
+    ws.nrec = 0;
+    return PB_OK;
+}
+
+// x += RU a, A x += RC a with a = RC^T (b - A x); needs ws.ax = A x
+static int recycle_project(pb_ctx* ctx, gmres_ws& ws, const double* b, double* x)
+{
+    cudaStream_t st = ctx->stream;
+    const int64_t n = ws.n;
+    const int k = ws.nrec, tb = 256;
+    if (k == 0 || !ws.ax_valid) return PB_OK;
+    k_residual<<<pb_blocks(n, tb), tb, 0, st>>>(n, b, ws.ax, ws.r);
+    PB_LAUNCH_CHECK();
+    PB_TRY(dot_into(ctx, ws, k, ws.RC, ws.r, false, ws.hdev));
+    k_lincomb<<<pb_blocks(n, tb), tb, k * sizeof(double), st>>>(n, k, ws.RU, n, ws.hdev, ws.u);
+    PB_LAUNCH_CHECK();
+    k_axpy<<<pb_blocks(n, tb), tb, 0, st>>>(n, 1.0, ws.u, x);
+    PB_LAUNCH_CHECK();
+    k_lincomb<<<pb_blocks(n, tb), tb, k * sizeof(double), st>>>(n, k, ws.RC, n, ws.hdev, ws.u);
+    PB_LAUNCH_CHECK();
+    k_axpy<<<pb_blocks(n, tb), tb, 0, st>>>(n, 1.0, ws.u, ws.ax);
+    PB_LAUNCH_CHECK();
+    return PB_OK;
+}
+
+// after a solve that moved x from ws.xb (with A x = ws.axb) to x (with A x = ws.ax): append the correction
+static int recycle_append(pb_ctx* ctx, gmres_ws& ws, const double* x)
+{
+    cudaStream_t st = ctx->stream;
+    const int64_t n = ws.n;
+    const int k = ws.nrec, tb = 256;
+    if (k >= ws.rec_cap || !ws.ax_valid) return PB_OK;
+    const int nb = pb_blocks(n, tb) < 2368 ? pb_blocks(n, tb) : 2368;
+    double* u = ws.RU + (size_t)k * n;
+    double* c = ws.RC + (size_t)k * n;
+    k_residual<<<pb_blocks(n, tb), tb, 0, st>>>(n, x, ws.xb, u);          // u = x - xb
+    PB_LAUNCH_CHECK();
+    k_residual<<<pb_blocks(n, tb), tb, 0, st>>>(n, ws.ax, ws.axb, c);     // c = A u
+    PB_LAUNCH_CHECK();
+    for (int pass = 0; pass < 2 && k > 0; ++pass) {                        // Gram-Schmidt twice against the older RC
+        PB_TRY(dot_into(ctx, ws, k, ws.RC, c, false, ws.hdev));
+        k_arnoldi_update<<<nb, tb, k * sizeof(double), st>>>(n, k, ws.RC, n, ws.hdev, c, nullptr, nullptr);
+        PB_LAUNCH_CHECK();
+        k_arnoldi_update<<<nb, tb, k * sizeof(double), st>>>(n, k, ws.RU, n, ws.hdev, u, nullptr, nullptr);
+        PB_LAUNCH_CHECK();
+    }
+    PB_TRY(dot_into(ctx, ws, 0, nullptr, c, true, ws.hdev));               // c.c
+    k_normalize<<<nb, tb, 0, st>>>(n, ws.hdev, c, c);
+    PB_LAUNCH_CHECK();
+    k_normalize<<<nb, tb, 0, st>>>(n, ws.hdev, u, u);
+    PB_LAUNCH_CHECK();
+    ws.nrec = k + 1;
+    return PB_OK;
+}
+
 static int pb_solve_core(pb_ctx* ctx, double* x_out, double* mu_out, pb_result* res, bool host_out)
 {
     pb_tree& t = ctx->tree;
@@ -794,6 +868,7 @@ static int pb_solve_core(pb_ctx* ctx, double* x_out, double* mu_out, pb_result* 
     PB_CUDA(cudaMemcpyAsync(&hflag, dscal, sizeof(int), cudaMemcpyDeviceToHost, st));
     PB_CUDA(cudaStreamSynchronize(st));
     const bool polarizable = hflag != 0;
+    ctx->gws.nrec = 0;                                   // the recycled subspace belongs to one SCF loop
     const double tol = ctx->prm.scf_tol_debye, omega = ctx->prm.scf_omega;
     int status = PB_OK;
     double h[2];
@@ -822,10 +897,32 @@ static int pb_solve_core(pb_ctx* ctx, double* x_out, double* mu_out, pb_result* 
     for (it = 1; it <= ctx->prm.scf_maxit; ++it) {
         int32_t gi = 0, mv = 0;
         PB_TRY(pb_rhs_multipole(ctx, mu, b));                        // step 2: Eq. (5) with p = d + mu
+        const bool recycle = polarizable && ctx->prm.scf_recycle != 0;
+        gmres_ws& ws = ctx->gws;
+        if (recycle && it > 1) {
+            PB_TRY(recycle_alloc(ctx, ws));
+            PB_TRY(recycle_project(ctx, ws, b, x));                  // minimal-residual step in the recycled subspace
+            if (ws.xb && ws.ax_valid) {
+                PB_CUDA(cudaMemcpyAsync(ws.xb, x, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+                PB_CUDA(cudaMemcpyAsync(ws.axb, ws.ax, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+            }
+        }
+        const bool had_ax = it > 1 && ws.ax_valid;
         int rc = pb_gmres_impl(ctx, b, x, &gi, &relres, &mv, it > 1);
         if (rc == PB_ERR_NO_CONVERGENCE) status = rc; else if (rc != PB_OK) return rc;
         gm_total += gi;
         mv_total += mv;
+        if (recycle && gi > 0) {
+            if (it == 1) {                                           // the cold solve: x_b = 0, A x_b = 0
+                PB_TRY(recycle_alloc(ctx, ws));
+                if (ws.xb) {
+                    PB_CUDA(cudaMemsetAsync(ws.xb, 0, sizeof(double) * n, st));
+                    PB_CUDA(cudaMemsetAsync(ws.axb, 0, sizeof(double) * n, st));
+                    PB_TRY(recycle_append(ctx, ws, x));
+                }
+            } else if (ws.xb && had_ax)
+                PB_TRY(recycle_append(ctx, ws, x));
+        }
         if (!polarizable) { conv = true; break; }
         PB_TRY(pb_reaction_field(ctx, x, nullptr, gs, nullptr));      // step 3: Eq. (13)
         PB_TRY(pb_multipole_field_impl(ctx, mu, 2, 1, nullptr, gm, nullptr));   // step 3: Eq. (14), induced part
@@ -837,6 +934,7 @@ static int pb_solve_core(pb_ctx* ctx, double* x_out, double* mu_out, pb_result* 
         if (delta < tol) {                                            // step 6
             // surface solution consistent with the final mu
             PB_TRY(pb_rhs_multipole(ctx, mu, b));
+            if (recycle) PB_TRY(recycle_project(ctx, ws, b, x));
             rc = pb_gmres_impl(ctx, b, x, &gi, &relres, &mv, true);
             if (rc == PB_ERR_NO_CONVERGENCE) status = rc; else if (rc != PB_OK) return rc;
             gm_total += gi;

@@ -45,7 +45,7 @@ class Params(ctypes.Structure):
         ("nq_edge", ctypes.c_int32), ("precond", ctypes.c_int32), ("gmres_tol", ctypes.c_double),
         ("gmres_restart", ctypes.c_int32), ("gmres_maxit", ctypes.c_int32), ("scf_tol_debye", ctypes.c_double),
         ("scf_omega", ctypes.c_double), ("scf_maxit", ctypes.c_int32), ("site_treecode", ctypes.c_int32),
-        ("thole_a", ctypes.c_double), ("rhs_treecode", ctypes.c_int32), ("reserved0", ctypes.c_int32),
+        ("thole_a", ctypes.c_double), ("rhs_treecode", ctypes.c_int32), ("scf_recycle", ctypes.c_int32),
     ]
 
 
