@@ -307,7 +307,8 @@ int pb_farfield_table(int P, int32_t* expo, int32_t* off, int32_t* idx, double* 
 int pb_fp64_peak_probe(pb_ctx* ctx, double* tflops_out /* HOST */);
 /* The same pipe under conditions a real kernel meets: `warps_per_sm` resident warps (4 .. 64), `ilp` independent DFMA
  * chains per thread (1, 2, 4, 8) and, with ilp = 8, `other_per_8` (0, 2, 4, 8) integer instructions per 8 DFMA of
- * `other_kind` 0 = IMAD (FMA-heavy pipe) or 1 = LOP3 (ALU pipe).  *pct_out = DFMA lane-instructions per second as a
+ * `other_kind` 0 = IMAD (FMA-heavy pipe) or 1 = LOP3 (ALU pipe); (ilp 8, other_per_8 0, other_kind 2) = every DFMA with
+ * three DISTINCT vector-register sources instead of two shared ones (operand bandwidth).  *pct_out = DFMA lane-instructions per second as a
  * percentage of SMs x 64 lanes x SM clock (D: section 7).  Synchronises. */
 int pb_fp64_pipe_probe(pb_ctx* ctx, int warps_per_sm, int ilp, int other_per_8, int other_kind, double* pct_out /* HOST */);
 

@@ -631,16 +631,17 @@ extern "C" int pb_fp64_peak_probe(pb_ctx* ctx, double* tflops_out)
 template <int ILP, int NI, int KIND>
 __global__ void __launch_bounds__(128) k_pipe_probe(int iters, double a, double b, int c, double* __restrict__ out)
 {
-    double x[8];
+    double x[8], u[8], v[8];
     int y[8];
 #pragma unroll
-    for (int i = 0; i < 8; ++i) { x[i] = threadIdx.x * 1e-3 + i; y[i] = threadIdx.x + i; }
+    for (int i = 0; i < 8; ++i) { x[i] = threadIdx.x * 1e-3 + i; y[i] = threadIdx.x + i; u[i] = a + 1e-9 * (threadIdx.x + i); v[i] = b * (1 + i); }
     for (int it = 0; it < iters; ++it) {
 #pragma unroll
         for (int r = 0; r < 8 / ILP; ++r)
 #pragma unroll
             for (int i = 0; i < ILP; ++i) {
-                x[i] = fma(x[i], a, b);                                     // ILP independent chains, 8 DFMA per iteration
+                if (KIND == 2) x[i] = fma(x[i], u[i], v[i]);                // three DISTINCT vector registers per DFMA
+                else x[i] = fma(x[i], a, b);                                // ILP independent chains, 8 DFMA per iteration; a, b shared
                 if (r * ILP + i < NI) {
                     if (KIND == 0) y[i] = y[i] * c + it;                    // IMAD (FMA-heavy / integer-multiply pipe)
                     else y[i] = (y[i] ^ c) & 0x7fffffff;                    // LOP3 (ALU pipe)
@@ -650,7 +651,7 @@ __global__ void __launch_bounds__(128) k_pipe_probe(int iters, double a, double 
     double s = 0;
     int t = 0;
 #pragma unroll
-    for (int i = 0; i < 8; ++i) { s += x[i]; t += y[i]; }
+    for (int i = 0; i < 8; ++i) { s += x[i] + u[i] + v[i]; t += y[i]; }
     if (s == 123.456 || t == 77) out[0] = s + t;   // never true; keeps the chains alive
 }
 
@@ -685,10 +686,11 @@ extern "C" int pb_fp64_pipe_probe(pb_ctx* ctx, int warps_per_sm, int ilp, int ot
 #define PROBE_CASE(I, N, K) if (ilp == I && other_per_8 == N && other_kind == K) e = pipe_probe_launch<I, N, K>(blocks, smem, iters, ctx->scratch, ctx->stream);
         PROBE_CASE(1, 0, 0) PROBE_CASE(2, 0, 0) PROBE_CASE(4, 0, 0) PROBE_CASE(8, 0, 0)
         PROBE_CASE(8, 2, 0) PROBE_CASE(8, 4, 0) PROBE_CASE(8, 8, 0) PROBE_CASE(8, 2, 1) PROBE_CASE(8, 4, 1) PROBE_CASE(8, 8, 1)
+        PROBE_CASE(8, 0, 2)
 #undef PROBE_CASE
         if (e != cudaSuccess) {
             cudaEventDestroy(e0); cudaEventDestroy(e1);
-            return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_fp64_pipe_probe: ilp in {1,2,4,8} with other_per_8 = 0, or ilp = 8 with other_per_8 in {2,4,8}, kind 0|1");
+            return pb_fail(ctx, PB_ERR_INVALID_ARG, "pb_fp64_pipe_probe: ilp in {1,2,4,8} with other_per_8 = 0 and kind 0, ilp = 8 with other_per_8 in {2,4,8} and kind 0|1, or (8, 0, 2)");
         }
         PB_CUDA(cudaEventRecord(e1, ctx->stream));
         PB_CUDA(cudaEventSynchronize(e1));

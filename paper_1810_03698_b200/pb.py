@@ -485,6 +485,9 @@ def fp64_pipe_table(device: int = 0):
                 v = ctypes.c_double(0.0)
                 ctx._ck(ctx._L.pb_fp64_pipe_probe(ctx._h, 16, 8, ni, kind, ctypes.byref(v)))
                 rows.append((16, 8, ni, name, v.value))
+        v = ctypes.c_double(0.0)
+        ctx._ck(ctx._L.pb_fp64_pipe_probe(ctx._h, 16, 8, 0, 2, ctypes.byref(v)))
+        rows.append((16, 8, 0, "3 distinct register operands", v.value))
     finally:
         ctx.close()
     return rows
