@@ -634,7 +634,7 @@ __global__ void __launch_bounds__(128) k_pipe_probe(int iters, double a, double 
     double x[8], u[8], v[8];
     int y[8];
 #pragma unroll
-    for (int i = 0; i < 8; ++i) { x[i] = threadIdx.x * 1e-3 + i; y[i] = threadIdx.x + i; u[i] = a + 1e-9 * (threadIdx.x + i); v[i] = b * (1 + i); }
+    for (int i = 0; i < 8; ++i) { x[i] = threadIdx.x * 1e-3 + i; y[i] = threadIdx.x + i; u[i] = a + 1e-9 * (threadIdx.x + i); v[i] = b * (1 + i) + 1e-15 * threadIdx.x; }   // per-thread values: vector registers, not uniform ones
     for (int it = 0; it < iters; ++it) {
 #pragma unroll
         for (int r = 0; r < 8 / ILP; ++r)
