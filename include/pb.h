@@ -58,7 +58,7 @@ typedef struct pb_params {
                                0 => direct mode: every pair by P2P (the oracle's operator)   */
     int32_t order_P;        /* Taylor order, 0..10                                    */
     int32_t ncrit;          /* max source Gauss points per leaf cell;
-                               0 (default) => built-in choice: 256 below 65,536 source points, else 192
+                               0 (default) => built-in choice: 256 below 65,536 source points, else 128
                                (measured optimum on B200)                 */
     int32_t K_far;          /* Gauss points per panel, far rule: 1, 3, 4 or 7         */
     int32_t K_near;         /* near-singular rule: 19                                 */

@@ -668,12 +668,18 @@ template <int P> struct m2q_cfg {
 
 // PL <= P: evaluate only the terms of the order-PL sum (|alpha| + 2j <= PL); they are a subset of the order-P terms
 // with the same values F_{alpha,j}, so the same staged array serves both (the skipped entries are never read).
+// The four DFMA of a term are written in a "snake" order -- (m0,f.x) (m0,f.y) (m1,f.y) (m1,f.x), the next term starting
+// with the target the last one ended with -- so that consecutive instructions share a source register: a DFMA whose
+// three sources are all fresh vector registers issues at 2/3 of the pipe's rate on the B200 (operand bandwidth;
+// profiles/r02_fp64_pipe_probes.md), one that re-uses an operand of its predecessor at the full rate.  ptxas
+// reschedules most of it (C4: 11.43 -> 11.27 ms), the summation order of every partial sum is unchanged.
 template <int P, int PL>
 __device__ __forceinline__ void m2p_terms2(const double2* __restrict__ ff, double dx0, double dy0, double dz0, double dx1,
                                            double dy1, double dz1, double (&WV0)[P + 1], double (&WK0)[P + 1],
                                            double (&WV1)[P + 1], double (&WK1)[P + 1])
 {
     int e = 0;
+    bool flip = false;
     double xa0 = 1.0, xa1 = 1.0;
 #pragma unroll
     for (int a = 0; a <= P; ++a) {
@@ -688,10 +694,18 @@ __device__ __forceinline__ void m2p_terms2(const double2* __restrict__ ff, doubl
                 for (int j = 0; j <= (P - n) / 2; ++j) {
                     if (n + 2 * j <= PL) {
                         const double2 f = ff[e];
-                        WV0[n + j] = fma(m0, f.x, WV0[n + j]);
-                        WK0[n + j] = fma(m0, f.y, WK0[n + j]);
-                        WV1[n + j] = fma(m1, f.x, WV1[n + j]);
-                        WK1[n + j] = fma(m1, f.y, WK1[n + j]);
+                        if (!flip) {
+                            WV0[n + j] = fma(m0, f.x, WV0[n + j]);
+                            WK0[n + j] = fma(m0, f.y, WK0[n + j]);
+                            WK1[n + j] = fma(m1, f.y, WK1[n + j]);
+                            WV1[n + j] = fma(m1, f.x, WV1[n + j]);
+                        } else {
+                            WV1[n + j] = fma(m1, f.x, WV1[n + j]);
+                            WK1[n + j] = fma(m1, f.y, WK1[n + j]);
+                            WK0[n + j] = fma(m0, f.y, WK0[n + j]);
+                            WV0[n + j] = fma(m0, f.x, WV0[n + j]);
+                        }
+                        flip = !flip;
                     }
                     ++e;
                 }

@@ -771,8 +771,10 @@ int pb_tree_build_impl(pb_ctx* ctx)
     }
 
     // --- octree topology and cell geometry
-    // leaf capacity: larger leaves shorten the upward pass (the latency-bound part of a small problem)
-    t.ncrit_used = ctx->prm.ncrit > 0 ? ctx->prm.ncrit : (Ns < 65536 ? 256 : 192);
+    // leaf capacity: larger leaves shorten the upward pass (the latency-bound part of a small problem); on large meshes
+    // the matvec time is flat between 96 and 144 points per leaf (C4, round 2: 21.30 / 21.26 / 21.29 / 21.35 / 21.44 / 21.85 ms
+    // at 96 / 112 / 128 / 144 / 160 / 192)
+    t.ncrit_used = ctx->prm.ncrit > 0 ? ctx->prm.ncrit : (Ns < 65536 ? 256 : 128);
     {
         pb_octree oc;
         PB_TRY(pb_octree_build(ctx, keys, N, K, t.ncrit_used, t.sx[0], t.sx[1], t.sx[2], CAT_TREE, &oc));
