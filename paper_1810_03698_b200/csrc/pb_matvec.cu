@@ -1281,8 +1281,11 @@ int pb_site_farfield_setup(pb_ctx* ctx)
         else
             for (int q = 0; q < nchild[c]; ++q) { need[child[c] + q] = 1; parent[child[c] + q] = (int32_t)c; }
     }
+    std::vector<char> listed(nc, 0);
+    for (int64_t e = 0; e < s.t_m2p_total; ++e) listed[lists[e]] = 1;
+    // bit 0: the cell's far-field terms F are wanted (k_site_grad reads them), bit 1: its moments are stored (k_site_m2p)
     for (int64_t c = 0; c < nc; ++c)
-        if (need[c]) up[c] = 2 | ((parent[c] >= 0 ? parent[c] + 1 : 0) << 2);
+        if (need[c]) up[c] = (listed[c] ? 1 : 0) | 2 | ((parent[c] >= 0 ? parent[c] + 1 : 0) << 2);
     s.t_n_need_leaf = (int64_t)leaf_list.size();
     PB_TRY(pb_dalloc_t(ctx, &s.t_need_leaf, leaf_list.size() > 0 ? leaf_list.size() : 1, CAT_SITE_NEAR));
     PB_TRY(pb_dalloc_t(ctx, &s.t_up_link, (size_t)nc, CAT_SITE_NEAR));

@@ -133,6 +133,170 @@ k_site_m2p(int64_t na, int P, const double* __restrict__ sx, const double* __res
     }
 }
 
+// ---- far field of the potential and its gradient in radial form (the SCF loop's call: no Hessian) ---------------------
+// The order-P Taylor sum of a cell is, exactly (D: section 6),  phi(x) = sum_{|alpha| + 2j <= P} u_{|alpha|+j}(R) d^alpha F_{alpha,j},
+// d = x - y_c, with the single layer F = F^V - F^K of the matvec's far-field terms (phi_solv = V_L(dphi) - K_L(phi),
+// Eq. 12) and u_m = (2m-1)!! / R^(2m+1).  Because u_m'(R)/R = -u_{m+1}, its gradient in the target is
+//     grad phi = sum_m [ u_m G_m - u_{m+1} d W_m ],   W_m = sum_{|alpha|+j=m} d^alpha F,   G_m = sum_{|alpha|+j=m} grad(d^alpha) F,
+// the derivative of the SAME truncated sum that k_site_m2p differentiates through the coefficients a_{kappa+l}; here it
+// costs four FMA per term and four products per monomial instead of an order-(P+1) coefficient recurrence in shared
+// memory (C4: 64 -> see profiles).  One block per group of 32 sites (a lane per site); its 8 warps take the cells
+// w, w + 8, ... of the group's list, each with its own ring of TMA-filled slots as in k_m2p2.
+#define SG_W 8
+#define SG_NS 4
+#define SG_THREADS (32 * SG_W)
+
+__host__ __device__ static constexpr int sg_nt(int P)
+{
+    int t = 0;
+    for (int a = 0; a <= P; ++a)
+        for (int b = 0; b <= P - a; ++b)
+            for (int c = 0; c <= P - a - b; ++c) t += (P - a - b - c) / 2 + 1;
+    return t;
+}
+
+template <int P> struct sg_cfg {
+    static constexpr int NT = sg_nt(P);
+    static constexpr size_t FF_BYTES0 = (size_t)SG_W * SG_NS * NT * sizeof(double2);
+    static constexpr size_t RED_BYTES = (size_t)SG_W * 4 * ST_GROUP * sizeof(double);
+    static constexpr size_t FF_BYTES = FF_BYTES0 > RED_BYTES ? FF_BYTES0 : RED_BYTES;
+    static constexpr size_t SMEM = FF_BYTES + SG_W * SG_NS * sizeof(uint64_t);
+};
+
+template <int P>
+__global__ void __launch_bounds__(SG_THREADS)
+k_site_grad(int64_t na, const double* __restrict__ sx, const double* __restrict__ sy, const double* __restrict__ sz,
+            const int32_t* __restrict__ m2p_off, const int32_t* __restrict__ m2p_cell, const double* __restrict__ cx,
+            const double* __restrict__ cy, const double* __restrict__ cz, const double2* __restrict__ FF,
+            double* __restrict__ out /*[na][10]: phi, grad (Morton order of the sites), without the 1/(4 pi)*/)
+{
+    constexpr int NT = sg_cfg<P>::NT, NS = SG_NS;
+    extern __shared__ __align__(128) unsigned char sgraw[];
+    const int tid = threadIdx.x, lane = tid & 31, sub = tid >> 5;
+    double2* ffw = reinterpret_cast<double2*>(sgraw) + (size_t)sub * NS * NT;
+    uint64_t* fullw = reinterpret_cast<uint64_t*>(sgraw + sg_cfg<P>::FF_BYTES) + sub * NS;
+    const int64_t g = blockIdx.x;
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) pb_mbar_init(&fullw[s], 1);
+        pb_mbar_fence_init();
+    }
+    __syncthreads();
+    const int64_t i = g * ST_GROUP + lane;
+    const int64_t ic = i < na ? i : na - 1;            // padding lanes repeat the last site; never stored
+    const double x = sx[ic], y = sy[ic], z = sz[ic];
+    const int32_t e0 = m2p_off[g] + sub, count = m2p_off[g + 1] - m2p_off[g];
+    const int nw = count > sub ? (count - sub + SG_W - 1) / SG_W : 0;
+    auto issue = [&](int k, int32_t cell) {
+        const int slot = k % NS;
+        pb_mbar_expect_tx(&fullw[slot], (uint32_t)(NT * sizeof(double2)));
+        pb_bulk_g2s(ffw + (size_t)slot * NT, FF + (int64_t)cell * NT, (uint32_t)(NT * sizeof(double2)), &fullw[slot]);
+    };
+    if (lane == 0)
+        for (int k = 0; k < NS - 1 && k < nw; ++k) issue(k, m2p_cell[e0 + SG_W * k]);
+    int32_t idn = NS - 1 < nw ? m2p_cell[e0 + SG_W * (NS - 1)] : 0;
+    int32_t cn = nw > 0 ? m2p_cell[e0] : 0;
+    double cxn = cx[cn], cyn = cy[cn], czn = cz[cn];
+    double o0 = 0.0, o1 = 0.0, o2 = 0.0, o3 = 0.0;
+#pragma unroll 1
+    for (int k = 0; k < nw; ++k) {
+        const int kn = k + NS - 1;
+        if (lane == 0 && kn < nw) issue(kn, idn);
+        idn = kn + 1 < nw ? m2p_cell[e0 + SG_W * (kn + 1)] : 0;
+        const double dx = x - cxn, dy = y - cyn, dz = z - czn;
+        if (k + 1 < nw) {
+            cn = m2p_cell[e0 + SG_W * (k + 1)];
+            cxn = cx[cn]; cyn = cy[cn]; czn = cz[cn];
+        }
+        pb_mbar_wait(&fullw[k % NS], (uint32_t)((k / NS) & 1));
+        const double2* ff = ffw + (size_t)(k % NS) * NT;
+        double W[P + 1], GX[P + 1], GY[P + 1], GZ[P + 1];
+#pragma unroll
+        for (int m = 0; m <= P; ++m) { W[m] = 0.0; GX[m] = 0.0; GY[m] = 0.0; GZ[m] = 0.0; }
+        {
+            int e = 0;
+            double X = 1.0, X1 = 0.0;                  // x^a and a x^(a-1)
+#pragma unroll
+            for (int a = 0; a <= P; ++a) {
+                double Y = 1.0, Y1 = 0.0;
+#pragma unroll
+                for (int b = 0; b <= P - a; ++b) {
+                    const double XY = X * Y, X1Y = X1 * Y, XY1 = X * Y1;
+                    double Z = 1.0, Z1 = 0.0;
+#pragma unroll
+                    for (int c = 0; c <= P - a - b; ++c) {
+                        const int n = a + b + c;
+                        const double mono = XY * Z, mx = X1Y * Z, my = XY1 * Z, mz = XY * Z1;
+#pragma unroll
+                        for (int j = 0; j <= (P - n) / 2; ++j) {
+                            const double2 f2 = ff[e];
+                            ++e;
+                            const double f = f2.x - f2.y;      // V_L(dphi) - K_L(phi)
+                            W[n + j] = fma(mono, f, W[n + j]);
+                            if (a > 0) GX[n + j] = fma(mx, f, GX[n + j]);
+                            if (b > 0) GY[n + j] = fma(my, f, GY[n + j]);
+                            if (c > 0) GZ[n + j] = fma(mz, f, GZ[n + j]);
+                        }
+                        Z1 = (double)(c + 1) * Z;
+                        Z *= dz;
+                    }
+                    Y1 = (double)(b + 1) * Y;
+                    Y *= dy;
+                }
+                X1 = (double)(a + 1) * X;
+                X *= dx;
+            }
+        }
+        const double R2 = dx * dx + dy * dy + dz * dz;
+        const double ri = pb_rsqrt(R2), ri2 = ri * ri;
+        double u = ri, sp = 0.0, sgx = 0.0, sgy = 0.0, sgz = 0.0, sw1 = 0.0;
+#pragma unroll
+        for (int m = 0; m <= P; ++m) {
+            const double un = (2 * m + 1) * u * ri2;           // u_{m+1}
+            sp = fma(u, W[m], sp);
+            sgx = fma(u, GX[m], sgx);
+            sgy = fma(u, GY[m], sgy);
+            sgz = fma(u, GZ[m], sgz);
+            sw1 = fma(un, W[m], sw1);
+            u = un;
+        }
+        o0 += sp;
+        o1 += sgx - dx * sw1;
+        o2 += sgy - dy * sw1;
+        o3 += sgz - dz * sw1;
+        __syncwarp();
+    }
+    __syncthreads();
+    double* red = reinterpret_cast<double*>(sgraw);    // [SG_W][4][ST_GROUP]: the warps' sums, added in warp order
+    red[(sub * 4 + 0) * ST_GROUP + lane] = o0;
+    red[(sub * 4 + 1) * ST_GROUP + lane] = o1;
+    red[(sub * 4 + 2) * ST_GROUP + lane] = o2;
+    red[(sub * 4 + 3) * ST_GROUP + lane] = o3;
+    __syncthreads();
+    if (tid < 4 * ST_GROUP) {
+        const int m = tid / ST_GROUP, l = tid % ST_GROUP;
+        const int64_t ii = g * ST_GROUP + l;
+        if (ii < na) {
+            double v = 0;
+#pragma unroll
+            for (int q = 0; q < SG_W; ++q) v += red[(q * 4 + m) * ST_GROUP + l];
+            out[ii * 10 + m] = v;
+        }
+    }
+}
+
+template <int P>
+static cudaError_t launch_site_grad(pb_ctx* ctx, double* farp)
+{
+    pb_tree& t = ctx->tree;
+    pb_sites& s = ctx->sites;
+    cudaError_t e = cudaFuncSetAttribute(k_site_grad<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sg_cfg<P>::SMEM);
+    if (e != cudaSuccess) return e;
+    k_site_grad<P><<<(unsigned)s.t_groups, SG_THREADS, sg_cfg<P>::SMEM, ctx->stream>>>(
+        s.na, s.tpos[0], s.tpos[1], s.tpos[2], s.t_m2p_off, s.t_m2p_cell, t.c_ctr[0], t.c_ctr[1], t.c_ctr[2], t.FF, farp);
+    return cudaSuccess;
+}
+
 // ---- near field: block = 4 sites of a group x the group's whole P2P list (source-point ranges) ---------------
 // Same per-pair arithmetic as the direct kernel (k_reaction, pb_sites.cu), restated here for the list form.
 template <bool HESS>
@@ -267,8 +431,22 @@ int pb_reaction_field_tree(pb_ctx* ctx, double* phi, double* grad, double* hess)
                                                                         s.t_p2p_lo, s.t_p2p_hi, t.srec, nearp);
         PB_LAUNCH_CHECK();
     } else {
-        k_site_m2p<4><<<dim3(G, ST_SPLIT), ST_GROUP, sm, st>>>(s.na, t.P, s.tpos[0], s.tpos[1], s.tpos[2], s.t_m2p_off, s.t_m2p_cell, t.c_ctr[0],
-                                              t.c_ctr[1], t.c_ctr[2], t.M, s.nb_idx, s.dv_idx, s.dv_fac, farp);
+        // potential and gradient (the SCF loop): radial form, one slab of far-field sums; the other slabs are zero
+        PB_CUDA(cudaMemsetAsync(farp + (size_t)s.na * 10, 0, (size_t)(ST_SPLIT - 1) * s.na * 10 * sizeof(double), st));
+        cudaError_t e = cudaSuccess;
+        switch (t.P) {
+        case 0: e = launch_site_grad<0>(ctx, farp); break;
+        case 1: e = launch_site_grad<1>(ctx, farp); break;
+        case 2: e = launch_site_grad<2>(ctx, farp); break;
+        case 3: e = launch_site_grad<3>(ctx, farp); break;
+        case 4: e = launch_site_grad<4>(ctx, farp); break;
+        case 5: e = launch_site_grad<5>(ctx, farp); break;
+        case 6: e = launch_site_grad<6>(ctx, farp); break;
+        case 7: e = launch_site_grad<7>(ctx, farp); break;
+        case 8: e = launch_site_grad<8>(ctx, farp); break;
+        default: return pb_fail(ctx, PB_ERR_INVALID_ARG, "internal: site treecode needs order_P <= 8");
+        }
+        PB_CUDA(e);
         PB_LAUNCH_CHECK();
         k_site_p2p<false><<<G * (ST_GROUP / SP_ST), SP_THREADS, 0, st>>>(s.na, s.tpos[0], s.tpos[1], s.tpos[2], s.t_p2p_off,
                                                                          s.t_p2p_lo, s.t_p2p_hi, t.srec, nearp);

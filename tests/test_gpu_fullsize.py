@@ -250,7 +250,7 @@ def test_site_treecode_reaction_field_c2(pbm, po, torch_cuda):
     assert rel(grad, ref["grad_solv"]) <= 1e-3          # each target derivative costs about one order of the expansion
     assert rel(hess, ref["hess_solv"]) <= 1e-2
     g_only = ctx.reaction_field(torch_cuda.from_numpy(ref["x"]), want_hess=False)[1].cpu().numpy()
-    assert rel(g_only, grad) <= 1e-13                    # the SCF loop's gradient-only path is the same sum
+    assert rel(g_only, grad) <= 1e-10                    # the SCF loop's gradient-only path (radial form) is the same truncated sum
     x, mu, res = ctx.solve()
     assert res["status"] == 0
     for k in ("dG_solv", "G_solvterm", "G_mult_diss", "G_vac"):
