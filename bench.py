@@ -62,17 +62,20 @@ def m2p_flop(P, st):
     return m2p_flop_per_pair(P, st["n_terms"]) * (st["m2p_pairs"] - low) + (m2p_flop_per_pair(P - 2) * low if low else 0.0)
 
 
-def load_counters(workload, theta, P):
+def load_counters(workload, theta, P, ncrit):
     """Per-launch ncu counters of the hot kernels for this workload and launch configuration, from the committed
     capture profiles/r02_counters.csv (written from `ncu --set full`, command in profiles/r02_counters.md):
-    kernel -> dict(dram_bytes, fp64_thread_inst).  Missing file or row -> empty."""
+    kernel -> dict(dram_bytes, fp64_thread_inst, pairs).  Missing file or row -> empty; a row whose pair count
+    differs from this run's lists is ignored by the caller (the counters belong to another list build)."""
     out = {}
     try:
         with open(COUNTERS_CSV) as fh:
             for row in csv.DictReader(r for r in fh if not r.startswith("#")):
-                if row["workload"] == workload and abs(float(row["theta"]) - theta) < 1e-12 and int(row["order_P"]) == P:
+                if (row["workload"] == workload and abs(float(row["theta"]) - theta) < 1e-12 and int(row["order_P"]) == P
+                        and int(row["ncrit"]) == ncrit):
                     out[row["kernel"]] = dict(dram_bytes=float(row["dram_read_bytes"]) + float(row["dram_write_bytes"]),
-                                              fp64_thread_inst=32.0 * float(row["fp64_warp_inst"]), source=row["source"])
+                                              fp64_thread_inst=32.0 * float(row["fp64_warp_inst"]), pairs=int(row["pairs"]),
+                                              source=row["source"])
     except (OSError, KeyError, ValueError):
         pass
     return out
@@ -344,7 +347,7 @@ def run_ours(args):
     peak_probe = ctx.fp64_peak_probe()                          # measured DFMA throughput of this GPU, TFLOP/s
     sm_hz = (clocks["sm_mhz"] or 1965.0) * 1e6
     inst_peak = FP64_LANES * sm_hz                              # FP64 lane-instructions per second at the sampled clock
-    counters = load_counters(w.name, theta, P)
+    counters = load_counters(w.name, theta, P, int(st1["ncrit_used"]))
     p2p_kernel = "k_p2p2" if nt >= 30000 else "k_p2p"
     m2p_kernel = "k_m2p2" if P <= 8 else "k_m2p"
     p2p_ms = stp["prof_p2p_ms"] / max(stp["prof_p2p_launches"], 1)
@@ -352,6 +355,8 @@ def run_ours(args):
 
     def kernel_entry(kname, ms, nlaunch, pairs, flop):
         c = counters.get(kname, {})
+        if c and c["pairs"] != int(pairs):
+            c = {}                                 # counters of another list build: not this run's kernel
         e = {"kernel": kname, "ms_per_launch": ms, "launches": int(nlaunch), "pairs_per_launch": int(pairs),
              "algorithmic_tflops": flop / (ms * 1e-3) / 1e12 if ms > 0 else 0.0,
              "share_of_step": ms * nlaunch / ms_prof if ms_prof > 0 else None}
