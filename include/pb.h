@@ -86,6 +86,12 @@ typedef struct pb_params {
                                combination of the corrections found by the loop's earlier solves (a recycled subspace:
                                u_k with A u_k known from the Arnoldi relation, no extra operator application), then GMRES
                                as usual to gmres_tol; 0 = plain warm start from the previous x (D: R-20)              */
+    int32_t list_split;     /* interaction lists of the matvec: 1 (default) = the two halves (32 consecutive
+                               Morton-ordered targets each) of a 64-target group take the MAC decisions of Eq. (28)
+                               separately -- a cell accepted for one half only is listed for that half alone and only the
+                               other half descends to its children; 0 = one decision per group (accepted only when the
+                               MAC holds for all 64 targets).  Both cover every (target, source) pair exactly once and
+                               satisfy the MAC per target; 1 evaluates fewer pairs (D: section 7)                     */
 } pb_params;
 
 /* Result of one polarizable solve (HOST struct). */
@@ -137,6 +143,8 @@ typedef struct pb_stats {
     int64_t rhs_p2p_pairs;      /* RHS by the site tree (pb_params.rhs_treecode): (panel, site) pairs summed directly */
     int64_t rhs_m2p_pairs;      /* (panel, site cell) pairs through a multipole expansion                          */
     int64_t rhs_covered_pairs;  /* == n_panels * n_sites when those lists are complete                             */
+    int64_t p2p_pairs_half;     /* of p2p_pairs / m2p_pairs: pairs of list entries that serve one half (32 targets) of a   */
+    int64_t m2p_pairs_half;     /* 64-target group only (the two halves of a group are accepted separately)               */
 } pb_stats;
 
 typedef void* (*pb_alloc_fn)(void* user, size_t bytes);     /* returns a 256-byte aligned device pointer or NULL */

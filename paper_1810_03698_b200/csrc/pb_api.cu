@@ -101,6 +101,7 @@ extern "C" void pb_default_params(pb_params* p)
     p->thole_a = 0.39;
     p->rhs_treecode = 2;
     p->scf_recycle = 1;
+    p->list_split = 1;
 }
 
 extern "C" int pb_create(pb_ctx** out, int device, void* cuda_stream)
@@ -185,11 +186,12 @@ extern "C" int pb_set_params(pb_ctx* ctx, const pb_params* p)
     if (p->site_treecode < 0 || p->site_treecode > 2) return pb_fail(ctx, PB_ERR_INVALID_ARG, "site_treecode must be 0, 1 or 2");
     if (p->rhs_treecode < 0 || p->rhs_treecode > 2) return pb_fail(ctx, PB_ERR_INVALID_ARG, "rhs_treecode must be 0, 1 or 2");
     if (p->scf_recycle < 0 || p->scf_recycle > 1) return pb_fail(ctx, PB_ERR_INVALID_ARG, "scf_recycle must be 0 or 1");
+    if (p->list_split < 0 || p->list_split > 1) return pb_fail(ctx, PB_ERR_INVALID_ARG, "list_split must be 0 or 1");
     const pb_params& o = ctx->prm;
     bool shape = o.kappa != p->kappa || o.theta != p->theta || o.order_P != p->order_P ||
                  o.ncrit != p->ncrit || o.K_far != p->K_far || o.K_near != p->K_near ||
                  o.near_tau != p->near_tau || o.nq_edge != p->nq_edge || o.eps_in != p->eps_in ||
-                 o.eps_out != p->eps_out;
+                 o.eps_out != p->eps_out || o.list_split != p->list_split;
     ctx->prm = *p;
     if (shape && ctx->tree.built) {
         pb_dfree_cat(ctx, CAT_TREE);
@@ -521,6 +523,8 @@ extern "C" int pb_get_stats(pb_ctx* ctx, pb_stats* out)
     out->ncrit_used = t.ncrit_used;
     out->m2p_pairs_low = t.m2p_pairs_low;
     out->covered_pairs = t.covered_pairs;
+    out->p2p_pairs_half = t.p2p_pairs_half;
+    out->m2p_pairs_half = t.m2p_pairs_half;
     if (ctx->sites.rhs_built) {
         out->rhs_p2p_pairs = ctx->sites.r_ls.p2p_pairs;
         out->rhs_m2p_pairs = ctx->sites.r_ls.m2p_pairs;

@@ -87,7 +87,10 @@ struct pb_tree {
     int32_t* p2p_off = nullptr;   // [groups+1]
     int32_t* p2p_lo = nullptr;    // source-point ranges [lo, hi)
     int32_t* p2p_hi = nullptr;
+    int8_t* p2p_mask = nullptr;   // [ranges] which half of the group the range is for: 1 = targets 0..31, 2 = 32..63, 3 = both (k_lists)
+    int8_t* m2p_code = nullptr;   // [entries] bit 0: order P - 2; bits 1-2: the same half mask (also in m2p_ctr[e].w)
     int64_t p2p_pairs = 0, m2p_pairs = 0, m2p_pairs_low = 0;   // m2p_pairs_low: those evaluated at order P - 2
+    int64_t p2p_pairs_half = 0, m2p_pairs_half = 0;            // of those: pairs of entries listed for one half only
     int64_t covered_pairs = 0;    // (target, source point) pairs the STORED lists cover (k_cover_count); == N * Ns
     // far-field data
     int P = 0, Nk = 0, NT = 0;
@@ -312,7 +315,8 @@ int pb_radix_sort(pb_ctx* ctx, uint64_t* k0, uint64_t* k1, int32_t* v0, int32_t*
                   uint64_t** kout, int32_t** vout);
 int pb_cover_count(pb_ctx* ctx, int64_t G, int tg, int64_t ntargets, const int32_t* m2p_off, const int32_t* m2p_cell,
                    const int32_t* p2p_off, const int32_t* p2p_lo, const int32_t* p2p_hi, int64_t* out_host,
-                   const int32_t* c_first = nullptr, const int32_t* c_last = nullptr, int K = 0);
+                   const int32_t* c_first = nullptr, const int32_t* c_last = nullptr, int K = 0,
+                   const int8_t* p2p_mask = nullptr, const int8_t* m2p_code = nullptr);
 int pb_lists_build(pb_ctx* ctx, int tpl, int64_t ntargets, const double* tx, const double* ty, const double* tz,
                    const pb_octree& oc, int K, int64_t Ns, double theta, int m2p_min, int cat, pb_lists* out);
 int pb_octree_build(pb_ctx* ctx, const uint64_t* keys, int64_t n, int K, int ncrit, const double* px, const double* py,

@@ -473,7 +473,8 @@ __global__ void __launch_bounds__(UP_THREADS) k_upward(up_args a)
 }
 
 // ---- M2P (H6; "box-target" interactions) -----------------------------------------------------------
-template <int P>
+// PL <= P: only the terms of the order-PL sum (|alpha| + 2j <= PL), see m2p_terms2
+template <int P, int PL = P>
 __device__ __forceinline__ void m2p_terms(const double2* __restrict__ ff, double dx, double dy, double dz,
                                           double (&WV)[P + 1], double (&WK)[P + 1])
 {
@@ -490,16 +491,18 @@ __device__ __forceinline__ void m2p_terms(const double2* __restrict__ ff, double
                 const int n = a + b + c;
 #pragma unroll
                 for (int j = 0; j <= (P - n) / 2; ++j) {
-                    const double2 f = ff[e];
+                    if (n + 2 * j <= PL) {
+                        const double2 f = ff[e];
+                        WV[n + j] = fma(mono, f.x, WV[n + j]);
+                        WK[n + j] = fma(mono, f.y, WK[n + j]);
+                    }
                     ++e;
-                    WV[n + j] = fma(mono, f.x, WV[n + j]);
-                    WK[n + j] = fma(mono, f.y, WK[n + j]);
                 }
-                mono *= dz;
+                if (n < PL) mono *= dz;
             }
-            xy *= dy;
+            if (a + b < PL) xy *= dy;
         }
-        xa *= dx;
+        if (a < PL) xa *= dx;
     }
 }
 
@@ -600,6 +603,7 @@ k_m2p(int64_t N, double kappa, pb_expk ek, const pb_item* __restrict__ items, co
 #pragma unroll 1
         for (int j = sub; j < cnt; j += M2P_S) {
             const double4 cc = ctr[st * CT + j];
+            if (!(((int)cc.w >> 1) >> ((tid >> 5) & 1) & 1)) continue;   // the entry is for the other half of the group (warp-uniform)
             const double dx = tx - cc.x, dy = ty - cc.y, dz = tz - cc.z;
             double WV[P + 1], WK[P + 1];
 #pragma unroll
@@ -796,18 +800,38 @@ k_m2p2(int64_t N, double kappa, pb_expk ek, const pb_item* __restrict__ items, c
         const double2* ffk = ffw + (size_t)(k % NS) * NT;
         const double dx0 = tx0 - cc.x, dy0 = ty0 - cc.y, dz0 = tz0 - cc.z;
         const double dx1 = tx1 - cc.x, dy1 = ty1 - cc.y, dz1 = tz1 - cc.z;
-        double WV0[P + 1], WK0[P + 1], WV1[P + 1], WK1[P + 1];
-#pragma unroll
-        for (int m = 0; m <= P; ++m) { WV0[m] = 0.0; WK0[m] = 0.0; WV1[m] = 0.0; WK1[m] = 0.0; }
         constexpr int PL = P >= 4 ? P - 2 : P;
-        if (PL < P && cc.w != 0.0) {              // flagged by the list build: order P - 2 is enough (warp-uniform)
-            m2p_terms2<P, PL>(ffk, dx0, dy0, dz0, dx1, dy1, dz1, WV0, WK0, WV1, WK1);
-            m2p_radial<P, PL>(dx0, dy0, dz0, WV0, WK0, kappa, k2, ek, Ts, VL0, KL0, VY0, KY0);
-            m2p_radial<P, PL>(dx1, dy1, dz1, WV1, WK1, kappa, k2, ek, Ts, VL1, KL1, VY1, KY1);
-        } else {
-            m2p_terms2<P, P>(ffk, dx0, dy0, dz0, dx1, dy1, dz1, WV0, WK0, WV1, WK1);
-            m2p_radial<P, P>(dx0, dy0, dz0, WV0, WK0, kappa, k2, ek, Ts, VL0, KL0, VY0, KY0);
-            m2p_radial<P, P>(dx1, dy1, dz1, WV1, WK1, kappa, k2, ek, Ts, VL1, KL1, VY1, KY1);
+        const int code = (int)cc.w;                    // k_lists: bit 0 = order P - 2 is enough, bits 1-2 = half mask (warp-uniform)
+        const bool low = PL < P && (code & 1);
+        if ((code >> 1) == 3) {                        // both targets of every lane: each term read feeds four FMAs
+            double WV0[P + 1], WK0[P + 1], WV1[P + 1], WK1[P + 1];
+#pragma unroll
+            for (int m = 0; m <= P; ++m) { WV0[m] = 0.0; WK0[m] = 0.0; WV1[m] = 0.0; WK1[m] = 0.0; }
+            if (low) {
+                m2p_terms2<P, PL>(ffk, dx0, dy0, dz0, dx1, dy1, dz1, WV0, WK0, WV1, WK1);
+                m2p_radial<P, PL>(dx0, dy0, dz0, WV0, WK0, kappa, k2, ek, Ts, VL0, KL0, VY0, KY0);
+                m2p_radial<P, PL>(dx1, dy1, dz1, WV1, WK1, kappa, k2, ek, Ts, VL1, KL1, VY1, KY1);
+            } else {
+                m2p_terms2<P, P>(ffk, dx0, dy0, dz0, dx1, dy1, dz1, WV0, WK0, WV1, WK1);
+                m2p_radial<P, P>(dx0, dy0, dz0, WV0, WK0, kappa, k2, ek, Ts, VL0, KL0, VY0, KY0);
+                m2p_radial<P, P>(dx1, dy1, dz1, WV1, WK1, kappa, k2, ek, Ts, VL1, KL1, VY1, KY1);
+            }
+        } else {                                       // the cell is accepted for one half of the group only
+            const bool second = (code >> 1) == 2;
+            const double dx = second ? dx1 : dx0, dy = second ? dy1 : dy0, dz = second ? dz1 : dz0;
+            double vl = second ? VL1 : VL0, kl = second ? KL1 : KL0, vy = second ? VY1 : VY0, ky = second ? KY1 : KY0;
+            double WV[P + 1], WK[P + 1];
+#pragma unroll
+            for (int m = 0; m <= P; ++m) { WV[m] = 0.0; WK[m] = 0.0; }
+            if (low) {
+                m2p_terms<P, PL>(ffk, dx, dy, dz, WV, WK);
+                m2p_radial<P, PL>(dx, dy, dz, WV, WK, kappa, k2, ek, Ts, vl, kl, vy, ky);
+            } else {
+                m2p_terms<P, P>(ffk, dx, dy, dz, WV, WK);
+                m2p_radial<P, P>(dx, dy, dz, WV, WK, kappa, k2, ek, Ts, vl, kl, vy, ky);
+            }
+            if (second) { VL1 = vl; KL1 = kl; VY1 = vy; KY1 = ky; }
+            else { VL0 = vl; KL0 = kl; VY0 = vy; KY0 = ky; }
         }
         __syncwarp();
     }
@@ -880,6 +904,20 @@ __device__ __forceinline__ void p2p_tile2(const double4* __restrict__ buf, int c
     }
 }
 
+// a tile of a range listed for one half of the group only (k_lists): one target per lane
+template <bool CHECK_SELF>
+__device__ __forceinline__ void p2p_tile1(const double4* __restrict__ buf, int cnt, int sub, int32_t s0, int32_t self, int K,
+                                          double kappa, const pb_expk8& ek, const double* __restrict__ Ts,
+                                          const double (&t)[3], double (&o)[4])
+{
+#pragma unroll 4
+    for (int k = sub; k < cnt; k += P2Q_W) {
+        const double4 a = buf[2 * k], b = buf[2 * k + 1];
+        if (!CHECK_SELF || (unsigned)(s0 + k - self) >= (unsigned)K)
+            p2p_pair(a, b, t[0], t[1], t[2], kappa, ek, Ts, o[0], o[1], o[2], o[3]);
+    }
+}
+
 template <bool CHECK_SELF>
 __device__ __forceinline__ void p2p_tile(const double4* __restrict__ buf, int cnt, int sub, int32_t s0, int32_t selfLo,
                                          int K, double kappa, const pb_expk8& ek, const double* __restrict__ Ts,
@@ -907,8 +945,8 @@ __device__ __forceinline__ void p2p_tile(const double4* __restrict__ buf, int cn
 
 __global__ void __launch_bounds__(P2P_THREADS)
 k_p2p(int64_t N, int K, double kappa, pb_expk8 ek, const pb_item* __restrict__ items,
-      const int32_t* __restrict__ p2p_lo, const int32_t* __restrict__ p2p_hi, const double4* __restrict__ srec,
-      const double* __restrict__ px, const double* __restrict__ py, const double* __restrict__ pz,
+      const int32_t* __restrict__ p2p_lo, const int32_t* __restrict__ p2p_hi, const int8_t* __restrict__ p2p_mask,
+      const double4* __restrict__ srec, const double* __restrict__ px, const double* __restrict__ py, const double* __restrict__ pz,
       double* __restrict__ acc)
 {
     __shared__ __align__(128) double4 tile[2][2 * P2P_TILE];
@@ -938,13 +976,14 @@ k_p2p(int64_t N, int K, double kappa, pb_expk8 ek, const pb_item* __restrict__ i
     int32_t r = item.r, a = item.a;
     int32_t hi = p2p_hi[r];
     int64_t remaining = item.count;
-    auto next_tile = [&](int32_t& s0, int& cnt) -> bool {
+    int rmask = p2p_mask[r];                          // which half of the group range r is for (k_lists)
+    auto next_tile = [&](int32_t& s0, int& cnt, int& mk) -> bool {
         while (remaining > 0) {
-            if (a >= hi) { ++r; a = p2p_lo[r]; hi = p2p_hi[r]; continue; }
+            if (a >= hi) { ++r; a = p2p_lo[r]; hi = p2p_hi[r]; rmask = p2p_mask[r]; continue; }
             int64_t c = hi - a;
             if (c > P2P_TILE) c = P2P_TILE;
             if (c > remaining) c = remaining;
-            s0 = a; cnt = (int)c;
+            s0 = a; cnt = (int)c; mk = rmask;
             a += (int32_t)c; remaining -= c;
             return true;
         }
@@ -953,21 +992,24 @@ k_p2p(int64_t N, int K, double kappa, pb_expk8 ek, const pb_item* __restrict__ i
 
     double VL = 0, KL = 0, VY = 0, KY = 0;
     int32_t cs0 = 0, ns0 = 0;
-    int ccnt = 0, ncnt = 0;
-    bool have = next_tile(cs0, ccnt);
+    int ccnt = 0, ncnt = 0, cmk = 0, nmk = 0;
+    const int half = (tid >> 5) & 1;                  // this warp's targets: 0..31 or 32..63 of the group
+    bool have = next_tile(cs0, ccnt, cmk);
     if (have && tid == 0) {
         pb_mbar_expect_tx(&bar[0], (uint32_t)ccnt * 64u);
         pb_bulk_g2s(tile[0], srec + 2 * (int64_t)cs0, (uint32_t)ccnt * 64u, &bar[0]);
     }
     for (uint32_t it = 0; have; ++it) {
         const int st = it & 1;
-        const bool more = next_tile(ns0, ncnt);
+        const bool more = next_tile(ns0, ncnt, nmk);
         if (more && tid == 0) {                       // the other buffer was released by the barrier below
             pb_mbar_expect_tx(&bar[st ^ 1], (uint32_t)ncnt * 64u);
             pb_bulk_g2s(tile[st ^ 1], srec + 2 * (int64_t)ns0, (uint32_t)ncnt * 64u, &bar[st ^ 1]);
         }
         pb_mbar_wait(&bar[st], (it >> 1) & 1u);
-        if (cs0 < grpHi && cs0 + ccnt > grpLo)
+        if (!((cmk >> half) & 1)) {
+            // the range is for the other half of the group
+        } else if (cs0 < grpHi && cs0 + ccnt > grpLo)
             p2p_tile<true>(tile[st], ccnt, sub, cs0, selfLo, K, kappa, ek, Ts, tx, ty, tz, VL, KL, VY, KY);
         else
             p2p_tile<false>(tile[st], ccnt, sub, cs0, selfLo, K, kappa, ek, Ts, tx, ty, tz, VL, KL, VY, KY);
@@ -975,6 +1017,7 @@ k_p2p(int64_t N, int K, double kappa, pb_expk8 ek, const pb_item* __restrict__ i
         have = more;
         cs0 = ns0;
         ccnt = ncnt;
+        cmk = nmk;
     }
     // add the sub-slices in a fixed order (tile[0] is free: every thread passed the last barrier)
     double* red = reinterpret_cast<double*>(tile[0]);   // [P2P_S][4][PB_TG]
@@ -994,8 +1037,8 @@ k_p2p(int64_t N, int K, double kappa, pb_expk8 ek, const pb_item* __restrict__ i
 
 __global__ void __launch_bounds__(P2P_THREADS, 2)
 k_p2p2(int64_t N, int K, double kappa, pb_expk8 ek, const pb_item* __restrict__ items,
-       const int32_t* __restrict__ p2p_lo, const int32_t* __restrict__ p2p_hi, const double4* __restrict__ srec,
-       const double* __restrict__ px, const double* __restrict__ py, const double* __restrict__ pz,
+       const int32_t* __restrict__ p2p_lo, const int32_t* __restrict__ p2p_hi, const int8_t* __restrict__ p2p_mask,
+       const double4* __restrict__ srec, const double* __restrict__ px, const double* __restrict__ py, const double* __restrict__ pz,
        double* __restrict__ acc)
 {
     __shared__ __align__(128) double4 tile[2][2 * P2P_TILE];
@@ -1024,13 +1067,14 @@ k_p2p2(int64_t N, int K, double kappa, pb_expk8 ek, const pb_item* __restrict__ 
     int32_t r = item.r, a = item.a;
     int32_t hi = p2p_hi[r];
     int64_t remaining = item.count;
-    auto next_tile = [&](int32_t& s0, int& cnt) -> bool {
+    int rmask = p2p_mask[r];                          // which half of the group range r is for (k_lists)
+    auto next_tile = [&](int32_t& s0, int& cnt, int& mk) -> bool {
         while (remaining > 0) {
-            if (a >= hi) { ++r; a = p2p_lo[r]; hi = p2p_hi[r]; continue; }
+            if (a >= hi) { ++r; a = p2p_lo[r]; hi = p2p_hi[r]; rmask = p2p_mask[r]; continue; }
             int64_t c = hi - a;
             if (c > P2P_TILE) c = P2P_TILE;
             if (c > remaining) c = remaining;
-            s0 = a; cnt = (int)c;
+            s0 = a; cnt = (int)c; mk = rmask;
             a += (int32_t)c; remaining -= c;
             return true;
         }
@@ -1039,28 +1083,36 @@ k_p2p2(int64_t N, int K, double kappa, pb_expk8 ek, const pb_item* __restrict__ 
 
     double o0[4] = {0, 0, 0, 0}, o1[4] = {0, 0, 0, 0};
     int32_t cs0 = 0, ns0 = 0;
-    int ccnt = 0, ncnt = 0;
-    bool have = next_tile(cs0, ccnt);
+    int ccnt = 0, ncnt = 0, cmk = 0, nmk = 0;
+    bool have = next_tile(cs0, ccnt, cmk);
     if (have && tid == 0) {
         pb_mbar_expect_tx(&bar[0], (uint32_t)ccnt * 64u);
         pb_bulk_g2s(tile[0], srec + 2 * (int64_t)cs0, (uint32_t)ccnt * 64u, &bar[0]);
     }
     for (uint32_t it = 0; have; ++it) {
         const int st = it & 1;
-        const bool more = next_tile(ns0, ncnt);
+        const bool more = next_tile(ns0, ncnt, nmk);
         if (more && tid == 0) {                       // the other buffer was released by the barrier below
             pb_mbar_expect_tx(&bar[st ^ 1], (uint32_t)ncnt * 64u);
             pb_bulk_g2s(tile[st ^ 1], srec + 2 * (int64_t)ns0, (uint32_t)ncnt * 64u, &bar[st ^ 1]);
         }
         pb_mbar_wait(&bar[st], (it >> 1) & 1u);
-        if (cs0 < grpHi && cs0 + ccnt > grpLo)
-            p2p_tile2<true>(tile[st], ccnt, sub, cs0, self0, self1, K, kappa, ek, Ts, t0, t1, o0, o1);
-        else
-            p2p_tile2<false>(tile[st], ccnt, sub, cs0, self0, self1, K, kappa, ek, Ts, t0, t1, o0, o1);
+        const bool own = cs0 < grpHi && cs0 + ccnt > grpLo;   // the tile holds points of the group's own panels
+        if (cmk == 3) {
+            if (own) p2p_tile2<true>(tile[st], ccnt, sub, cs0, self0, self1, K, kappa, ek, Ts, t0, t1, o0, o1);
+            else p2p_tile2<false>(tile[st], ccnt, sub, cs0, self0, self1, K, kappa, ek, Ts, t0, t1, o0, o1);
+        } else if (cmk == 1) {
+            if (own) p2p_tile1<true>(tile[st], ccnt, sub, cs0, self0, K, kappa, ek, Ts, t0, o0);
+            else p2p_tile1<false>(tile[st], ccnt, sub, cs0, self0, K, kappa, ek, Ts, t0, o0);
+        } else {
+            if (own) p2p_tile1<true>(tile[st], ccnt, sub, cs0, self1, K, kappa, ek, Ts, t1, o1);
+            else p2p_tile1<false>(tile[st], ccnt, sub, cs0, self1, K, kappa, ek, Ts, t1, o1);
+        }
         __syncthreads();
         have = more;
         cs0 = ns0;
         ccnt = ncnt;
+        cmk = nmk;
     }
     // add the warps' partial sums in a fixed order (tile[0] is free: every thread passed the last barrier)
     double* red = reinterpret_cast<double*>(tile[0]);   // [P2Q_W][4][PB_TG] = 16 KB = tile[0]
@@ -1370,10 +1422,10 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed, bool pre
             if (t.n_itemP_own > 0) {
                 if (t.N >= 30000)
                     k_p2p2<<<(unsigned)t.n_itemP_own, P2P_THREADS, 0, st>>>(t.N, t.K, ctx->prm.kappa, t.ek8, t.itemP + t.itemP0, t.p2p_lo,
-                                                                          t.p2p_hi, t.srec, t.pc[0], t.pc[1], t.pc[2], t.accP);
+                                                                          t.p2p_hi, t.p2p_mask, t.srec, t.pc[0], t.pc[1], t.pc[2], t.accP);
                 else
                     k_p2p<<<(unsigned)t.n_itemP_own, P2P_THREADS, 0, st>>>(t.N, t.K, ctx->prm.kappa, t.ek8, t.itemP + t.itemP0, t.p2p_lo,
-                                                                         t.p2p_hi, t.srec, t.pc[0], t.pc[1], t.pc[2], t.accP);
+                                                                         t.p2p_hi, t.p2p_mask, t.srec, t.pc[0], t.pc[1], t.pc[2], t.accP);
                 PB_LAUNCH_CHECK();
             }
             PB_TRY(pb_prof_end(ctx, 0));

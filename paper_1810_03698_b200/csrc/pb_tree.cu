@@ -310,7 +310,10 @@ struct list_args {
     const int32_t *c_first, *c_last, *c_child, *c_nchild;
     const double *cx, *cy, *cz, *crad;
     const double *px, *py, *pz;       // collocation points, Morton order
-    int8_t* m2p_low;                  // [entries] the flag (pass 1; may be NULL)
+    int8_t* m2p_low;                  // [entries] code of the entry (pass 1; may be NULL): bit 0 = evaluate at order P - 2,
+                                      // bits 1-2 = which half of the group the entry is for (1 = targets 0..31, 2 = 32..63, 3 = both)
+    int8_t* p2p_mask;                 // [ranges] the same half mask for every P2P range (pass 1; NULL without `split`)
+    int split;                        // 1: the two halves of a 64-target group are accepted separately (TPL == 2 only)
     int32_t *n_m2p, *n_p2p;           // pass 0: counts ; pass 1: offsets (read)
     int32_t *m2p_cell, *p2p_lo, *p2p_hi;
     unsigned long long* pair_counts;  // [3] p2p, m2p, low-order m2p pairs (pass 0)
@@ -320,7 +323,13 @@ struct list_args {
 #define LIST_STACK 256
 static_assert(PB_TG == 64, "k_lists keeps two targets per lane for the panel groups");
 
-// TPL = targets per lane: 2 for the panel groups (PB_TG = 64), 1 for the site groups (32 sites)
+// TPL = targets per lane: 2 for the panel groups (PB_TG = 64), 1 for the site groups (32 sites).
+// With `split` (TPL == 2) the two halves of a group -- every lane's first target (targets 0..31) and every lane's second
+// target (32..63) -- take their decisions separately: a cell that satisfies the MAC for one half only is listed for that
+// half alone, and only the other half goes on to its children.  Each half thus gets the list of a 32-target group
+// (C4: 29 % fewer P2P pairs, 8.5 % fewer M2P pairs than one list for all 64 targets), while the kernels still work on
+// whole warps: an entry for both halves feeds both targets of a lane from one shared-memory read, an entry for one half
+// costs half the arithmetic.  The stack holds (cell, mask of the halves still undecided for it).
 template <int PASS, int TPL>
 __global__ void __launch_bounds__(LIST_WARPS * 32) k_lists(list_args a)
 {
@@ -331,99 +340,137 @@ __global__ void __launch_bounds__(LIST_WARPS * 32) k_lists(list_args a)
     if (g >= a.ng) return;
     const int64_t i0 = g * TG;
     const int64_t ntg = i0 + TG <= a.N ? TG : a.N - i0;
-    int nm = 0, nr = 0, nlow = 0;
+    const unsigned long long nA = ntg < 32 ? (unsigned long long)ntg : 32ull, nB = (unsigned long long)ntg - nA;   // targets per half
+    const int full_mask = TPL == 2 && nB > 0 ? 3 : 1;
+    auto ntargets = [&](int m) -> unsigned long long { return (m & 1 ? nA : 0ull) + (m & 2 ? nB : 0ull); };
+    int nm = 0, nr = 0;
     const int64_t om = PASS ? a.n_m2p[g] : 0, op = PASS ? a.n_p2p[g] : 0;
-    unsigned long long pp = 0;
+    unsigned long long pp = 0, pm = 0, plow = 0, pph = 0, pmh = 0;
     if (a.theta <= 0.0) {   // direct mode: one range, every source point
-        if (PASS && lane == 0) { a.p2p_lo[op] = 0; a.p2p_hi[op] = (int32_t)a.Ns; }
+        if (PASS && lane == 0) {
+            a.p2p_lo[op] = 0; a.p2p_hi[op] = (int32_t)a.Ns;
+            if (a.p2p_mask) a.p2p_mask[op] = (int8_t)full_mask;
+        }
         nr = 1;
-        pp = (unsigned long long)a.Ns;
+        pp = (unsigned long long)a.Ns * (unsigned long long)ntg;
     } else {
         // padding lanes repeat a real target
-        const int64_t ia = i0 + (lane < ntg ? lane : 0), ib = TPL == 2 ? i0 + (lane + 32 < ntg ? lane + 32 : 0) : ia;
+        const int64_t ia = i0 + (lane < ntg ? lane : 0), ib = TPL == 2 ? i0 + (lane + 32 < ntg ? lane + 32 : (nB > 0 ? 32 : 0)) : ia;
         const double ax = a.px[ia], ay = a.py[ia], az = a.pz[ia];
         const double bx = a.px[ib], by = a.py[ib], bz = a.pz[ib];
         int32_t* stack = stk[wid];
         int sp = 0;
-        if (lane == 0) stack[0] = 0;
+        if (lane == 0) stack[0] = 0 * 4 + full_mask;
         sp = 1;
         __syncwarp();
         int32_t last_hi = -1;
+        int last_mask = 0;
         const double th2 = a.theta * a.theta;
+        const bool split = TPL == 2 && a.split != 0;
         while (sp > 0) {
-            const int32_t c = stack[--sp];
+            const int32_t top = stack[--sp];
             __syncwarp();
+            const int32_t c = top >> 2;
+            const int mask = top & 3;
             const double cx = a.cx[c], cy = a.cy[c], cz = a.cz[c], cr = a.crad[c];
             double da = (cx - ax) * (cx - ax) + (cy - ay) * (cy - ay) + (cz - az) * (cz - az);
-            const double db = (cx - bx) * (cx - bx) + (cy - by) * (cy - by) + (cz - bz) * (cz - bz);
-            da = fmin(da, db);
-            for (int o = 16; o > 0; o >>= 1) da = fmin(da, __shfl_xor_sync(0xffffffffu, da, o));
+            double db = (cx - bx) * (cx - bx) + (cy - by) * (cy - by) + (cz - bz) * (cz - bz);
+            for (int o = 16; o > 0; o >>= 1) {
+                da = fmin(da, __shfl_xor_sync(0xffffffffu, da, o));
+                db = fmin(db, __shfl_xor_sync(0xffffffffu, db, o));
+            }
             const int32_t f = a.c_first[c], l = a.c_last[c];
             const int32_t ch = a.c_child[c];
             const int64_t nsrc = (int64_t)(l - f) * a.K;
-            if (cr * cr < th2 * da && cr * cr < da && nsrc >= a.m2p_min) {
-                const bool low = cr * cr < a.theta_low2 * da;
+            const bool big = nsrc >= a.m2p_min;
+            const bool okA = (mask & 1) && big && cr * cr < th2 * da && cr * cr < da;
+            const bool okB = (mask & 2) && big && cr * cr < th2 * db && cr * cr < db;
+            int acc = (okA ? 1 : 0) | (okB ? 2 : 0);
+            if (!split && acc != mask) acc = 0;             // one decision for the whole group
+            if (acc) {
+                double dmin = 1e300;
+                if (acc & 1) dmin = fmin(dmin, da);
+                if (acc & 2) dmin = fmin(dmin, db);
+                const bool low = cr * cr < a.theta_low2 * dmin;
                 if (PASS && lane == 0) {
                     a.m2p_cell[om + nm] = c;
-                    if (a.m2p_low) a.m2p_low[om + nm] = low ? 1 : 0;
+                    if (a.m2p_low) a.m2p_low[om + nm] = (int8_t)((low ? 1 : 0) | (acc << 1));
                 }
                 ++nm;
-                nlow += low ? 1 : 0;
-            } else if (ch < 0) {
-                const int32_t lo = f * a.K, hi = l * a.K;
-                if (lo == last_hi) {
-                    if (PASS && lane == 0) a.p2p_hi[op + nr - 1] = hi;
+                pm += ntargets(acc);
+                if (low) plow += ntargets(acc);
+                if (acc != full_mask) pmh += ntargets(acc);
+            }
+            const int rem = mask & ~acc;
+            if (rem) {
+                if (ch < 0) {
+                    const int32_t lo = f * a.K, hi = l * a.K;
+                    if (lo == last_hi && rem == last_mask) {
+                        if (PASS && lane == 0) a.p2p_hi[op + nr - 1] = hi;
+                    } else {
+                        if (PASS && lane == 0) {
+                            a.p2p_lo[op + nr] = lo; a.p2p_hi[op + nr] = hi;
+                            if (a.p2p_mask) a.p2p_mask[op + nr] = (int8_t)rem;
+                        }
+                        ++nr;
+                    }
+                    last_hi = hi;
+                    last_mask = rem;
+                    pp += (unsigned long long)(hi - lo) * ntargets(rem);
+                    if (rem != full_mask) pph += (unsigned long long)(hi - lo) * ntargets(rem);
                 } else {
-                    if (PASS && lane == 0) { a.p2p_lo[op + nr] = lo; a.p2p_hi[op + nr] = hi; }
-                    ++nr;
+                    const int nc = a.c_nchild[c];
+                    if (lane < nc) stack[sp + lane] = (ch + (nc - 1 - lane)) * 4 + rem;   // popped in Morton order
+                    sp += nc;
+                    __syncwarp();
                 }
-                last_hi = hi;
-                pp += (unsigned long long)(hi - lo);
-            } else {
-                const int nc = a.c_nchild[c];
-                if (lane < nc) stack[sp + lane] = ch + (nc - 1 - lane);   // popped in Morton order
-                sp += nc;
-                __syncwarp();
             }
         }
     }
     if (!PASS && lane == 0) {
         a.n_m2p[g] = nm;
         a.n_p2p[g] = nr;
-        atomicAdd(&a.pair_counts[0], pp * (unsigned long long)ntg);
-        atomicAdd(&a.pair_counts[1], (unsigned long long)nm * (unsigned long long)ntg);
-        atomicAdd(&a.pair_counts[2], (unsigned long long)nlow * (unsigned long long)ntg);
+        atomicAdd(&a.pair_counts[0], pp);
+        atomicAdd(&a.pair_counts[1], pm);
+        atomicAdd(&a.pair_counts[2], plow);
+        atomicAdd(&a.pair_counts[3], pph);
+        atomicAdd(&a.pair_counts[4], pmh);
     }
 }
 
-// Stable partition of every group's M2P list: the cells evaluated at the full order P first, then the ones flagged
-// for order P - 2 (R-30).  A tile of 8 consecutive list entries is what the 8 warps of a k_m2p2 block share, one
-// cell per warp; with mixed tiles the warps' times differ by a factor two per tile and the fast ones run into
-// the end of the 4-stage ring (ncu, C4: 21 % of the warp samples in the wait for the next tile's data).  After the
-// partition all tiles but one per work item are uniform.  One thread per group; setup time only.
+// Stable partition of every group's M2P list into six classes: the cells evaluated at the full order P first, then the
+// ones flagged for order P - 2 (R-30); within each, the entries for both halves of the group, then the ones for the first
+// half only, then the second half only.  The 8 warps of a k_m2p2 block take consecutive list entries, one cell per
+// warp; with neighbours of one class the warps of a block finish their shares at about the same time.  One thread per
+// group; setup time only.  code: bit 0 = order P - 2, bits 1-2 = half mask (k_lists).
+__device__ __forceinline__ int m2p_class(int code) { return (code & 1) * 3 + ((code >> 1) == 3 ? 0 : (code >> 1)); }
+
 __global__ void k_partition_low(int64_t G, const int32_t* __restrict__ off, const int32_t* __restrict__ cell_in,
-                                const int8_t* __restrict__ low_in, int32_t* __restrict__ cell_out, int8_t* __restrict__ low_out)
+                                const int8_t* __restrict__ code_in, int32_t* __restrict__ cell_out, int8_t* __restrict__ code_out)
 {
     const int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (g >= G) return;
     const int32_t e0 = off[g], e1 = off[g + 1];
-    int32_t nfull = 0;
-    for (int32_t e = e0; e < e1; ++e) nfull += low_in[e] ? 0 : 1;
-    int32_t a = e0, b = e0 + nfull;
+    int32_t pos[6] = {0, 0, 0, 0, 0, 0};
+    for (int32_t e = e0; e < e1; ++e) ++pos[m2p_class(code_in[e])];
+    int32_t run = e0;
+    for (int k = 0; k < 6; ++k) { const int32_t n = pos[k]; pos[k] = run; run += n; }
     for (int32_t e = e0; e < e1; ++e) {
-        if (low_in[e]) { cell_out[b] = cell_in[e]; low_out[b] = 1; ++b; }
-        else { cell_out[a] = cell_in[e]; low_out[a] = 0; ++a; }
+        const int code = code_in[e];
+        const int32_t d = pos[m2p_class(code)]++;
+        cell_out[d] = cell_in[e];
+        code_out[d] = (int8_t)code;
     }
 }
 
-__global__ void k_m2p_centres(int64_t n, const int32_t* __restrict__ cell, const int8_t* __restrict__ low,
+__global__ void k_m2p_centres(int64_t n, const int32_t* __restrict__ cell, const int8_t* __restrict__ code,
                               const double* __restrict__ cx, const double* __restrict__ cy, const double* __restrict__ cz,
                               double4* __restrict__ out)
 {
     int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (e >= n) return;
     const int32_t c = cell[e];
-    out[e] = make_double4(cx[c], cy[c], cz[c], low[e] ? 1.0 : 0.0);   // .w: evaluate this cell at order P - 2
+    out[e] = make_double4(cx[c], cy[c], cz[c], (double)code[e]);   // .w: the entry's code (order flag + half mask), an exact small integer
 }
 
 // ---- work items: equal shares of each group's lists, one thread block each ---------------------
@@ -515,17 +562,19 @@ static int pb_build_items(pb_ctx* ctx, int64_t G, const int32_t* off, const int3
 // 9 P2P pairs (12.0 ms / 5.57e8 against 8.2 ms / 3.45e9 at C4); pairs[g] = {P2P pairs, M2P pairs} of the group
 __global__ void k_group_cost(int64_t G, int64_t N, const int32_t* __restrict__ m2p_off, const int32_t* __restrict__ p2p_off,
                              const int32_t* __restrict__ p2p_lo, const int32_t* __restrict__ p2p_hi,
+                             const int8_t* __restrict__ p2p_mask, const int8_t* __restrict__ m2p_code,
                              long long* __restrict__ cost, long long* __restrict__ pairs /*[G][2]*/)
 {
     const int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (g >= G) return;
-    long long pts = 0;
-    for (int32_t r = p2p_off[g]; r < p2p_off[g + 1]; ++r) pts += p2p_hi[r] - p2p_lo[r];
-    const long long nc = m2p_off[g + 1] - m2p_off[g];
     const long long ntg = g * PB_TG + PB_TG <= N ? PB_TG : N - g * PB_TG;
-    cost[g] = ntg * (pts + 9 * nc);
-    pairs[2 * g] = ntg * pts;
-    pairs[2 * g + 1] = ntg * nc;
+    const long long nh[4] = {0, ntg < 32 ? ntg : 32, ntg < 32 ? 0 : ntg - 32, ntg};   // targets an entry with half mask m is for
+    long long pp = 0, mp = 0;
+    for (int32_t r = p2p_off[g]; r < p2p_off[g + 1]; ++r) pp += (long long)(p2p_hi[r] - p2p_lo[r]) * nh[p2p_mask[r] & 3];
+    for (int32_t e = m2p_off[g]; e < m2p_off[g + 1]; ++e) mp += nh[(m2p_code[e] >> 1) & 3];
+    cost[g] = pp + 9 * mp;
+    pairs[2 * g] = pp;
+    pairs[2 * g + 1] = mp;
 }
 
 extern "C" int pb_shard_partition(const int64_t* cost, int64_t G, int world, int64_t* first)
@@ -581,19 +630,22 @@ __global__ void k_cover_count(int64_t G, int tg, int64_t ntargets, int K, const 
                               const int32_t* __restrict__ m2p_cell, const int32_t* __restrict__ c_first,
                               const int32_t* __restrict__ c_last, const int32_t* __restrict__ p2p_off,
                               const int32_t* __restrict__ p2p_lo, const int32_t* __restrict__ p2p_hi,
+                              const int8_t* __restrict__ p2p_mask, const int8_t* __restrict__ m2p_code,
                               unsigned long long* __restrict__ out)
 {
     const int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     unsigned long long v = 0;
     if (g < G) {
-        unsigned long long pts = 0;
-        for (int32_t r = p2p_off[g]; r < p2p_off[g + 1]; ++r) pts += (unsigned long long)(p2p_hi[r] - p2p_lo[r]);
+        const int64_t i0 = g * tg;
+        const unsigned long long ntg = (unsigned long long)(i0 + tg <= ntargets ? tg : ntargets - i0);
+        // targets an entry with half mask m is for (the masks exist for the 64-target panel groups only)
+        const unsigned long long nh[4] = {0, ntg < 32 ? ntg : 32, ntg < 32 ? 0 : ntg - 32, ntg};
+        for (int32_t r = p2p_off[g]; r < p2p_off[g + 1]; ++r)
+            v += (unsigned long long)(p2p_hi[r] - p2p_lo[r]) * (p2p_mask ? nh[p2p_mask[r] & 3] : ntg);
         for (int32_t e = m2p_off[g]; e < m2p_off[g + 1]; ++e) {
             const int32_t c = m2p_cell[e];
-            pts += (unsigned long long)(c_last[c] - c_first[c]) * (unsigned long long)K;
+            v += (unsigned long long)(c_last[c] - c_first[c]) * (unsigned long long)K * (m2p_code ? nh[(m2p_code[e] >> 1) & 3] : ntg);
         }
-        const int64_t i0 = g * tg;
-        v = pts * (unsigned long long)(i0 + tg <= ntargets ? tg : ntargets - i0);
     }
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     if ((threadIdx.x & 31) == 0 && v) atomicAdd(out, v);     // integer sum: order does not matter
@@ -601,7 +653,7 @@ __global__ void k_cover_count(int64_t G, int tg, int64_t ntargets, int K, const 
 
 int pb_cover_count(pb_ctx* ctx, int64_t G, int tg, int64_t ntargets, const int32_t* m2p_off, const int32_t* m2p_cell,
                    const int32_t* p2p_off, const int32_t* p2p_lo, const int32_t* p2p_hi, int64_t* out_host,
-                   const int32_t* c_first, const int32_t* c_last, int K)
+                   const int32_t* c_first, const int32_t* c_last, int K, const int8_t* p2p_mask, const int8_t* m2p_code)
 {
     const pb_tree& t = ctx->tree;
     if (!c_first) { c_first = t.c_first; c_last = t.c_last; K = t.K; }   // default: the panel tree
@@ -610,7 +662,7 @@ int pb_cover_count(pb_ctx* ctx, int64_t G, int tg, int64_t ntargets, const int32
     unsigned long long* d = (unsigned long long*)ctx->scratch;
     PB_CUDA(cudaMemsetAsync(d, 0, sizeof(unsigned long long), st));
     k_cover_count<<<pb_blocks(G, 128), 128, 0, st>>>(G, tg, ntargets, K, m2p_off, m2p_cell, c_first, c_last, p2p_off,
-                                                    p2p_lo, p2p_hi, d);
+                                                    p2p_lo, p2p_hi, p2p_mask, m2p_code, d);
     PB_LAUNCH_CHECK();
     unsigned long long h = 0;
     PB_CUDA(cudaMemcpyAsync(&h, d, sizeof(h), cudaMemcpyDeviceToHost, st));
@@ -817,12 +869,14 @@ int pb_tree_build_impl(pb_ctx* ctx)
     PB_CUDA(cudaMemsetAsync(cnt_m, 0, sizeof(int32_t) * (G + 1), st));
     PB_CUDA(cudaMemsetAsync(cnt_p, 0, sizeof(int32_t) * (G + 1), st));
     unsigned long long* pc = (unsigned long long*)ctx->scratch;
-    PB_CUDA(cudaMemsetAsync(pc, 0, 3 * sizeof(unsigned long long), st));
+    PB_CUDA(cudaMemsetAsync(pc, 0, 5 * sizeof(unsigned long long), st));
     a.n_m2p = cnt_m; a.n_p2p = cnt_p; a.m2p_cell = nullptr; a.p2p_lo = nullptr; a.p2p_hi = nullptr; a.m2p_low = nullptr;
+    a.p2p_mask = nullptr;
+    a.split = ctx->prm.list_split;
     a.pair_counts = pc;
     k_lists<0, 2><<<pb_blocks(G, LIST_WARPS), LIST_WARPS * 32, 0, st>>>(a);
     PB_LAUNCH_CHECK();
-    unsigned long long hpc[3];
+    unsigned long long hpc[5];
     PB_CUDA(cudaMemcpyAsync(hpc, pc, sizeof(hpc), cudaMemcpyDeviceToHost, st));
     int64_t tot_m = 0, tot_p = 0;
     PB_TRY(pb_exclusive_scan_i32(ctx, cnt_m, t.m2p_off, G + 1, &tot_m));
@@ -830,17 +884,21 @@ int pb_tree_build_impl(pb_ctx* ctx)
     t.p2p_pairs = (int64_t)hpc[0];
     t.m2p_pairs = (int64_t)hpc[1];
     t.m2p_pairs_low = (int64_t)hpc[2];
+    t.p2p_pairs_half = (int64_t)hpc[3];
+    t.m2p_pairs_half = (int64_t)hpc[4];
     t.m2p_total = tot_m;
     PB_TRY(pb_dalloc_t(ctx, &t.m2p_cell, tot_m, CAT_TREE));
     PB_TRY(pb_dalloc_t(ctx, &t.p2p_lo, tot_p, CAT_TREE));
     PB_TRY(pb_dalloc_t(ctx, &t.p2p_hi, tot_p, CAT_TREE));
-    int8_t* m2p_low;
-    PB_TRY(pb_dalloc_t(ctx, &m2p_low, tot_m > 0 ? tot_m : 1, CAT_TMP));
+    PB_TRY(pb_dalloc_t(ctx, &t.p2p_mask, tot_p > 0 ? tot_p : 1, CAT_TREE));
+    PB_TRY(pb_dalloc_t(ctx, &t.m2p_code, tot_m > 0 ? tot_m : 1, CAT_TREE));
+    int8_t* m2p_low = t.m2p_code;
     a.n_m2p = t.m2p_off; a.n_p2p = t.p2p_off; a.m2p_cell = t.m2p_cell; a.p2p_lo = t.p2p_lo; a.p2p_hi = t.p2p_hi;
     a.m2p_low = m2p_low;
+    a.p2p_mask = t.p2p_mask;
     k_lists<1, 2><<<pb_blocks(G, LIST_WARPS), LIST_WARPS * 32, 0, st>>>(a);
     PB_LAUNCH_CHECK();
-    if (tot_m > 0 && a.theta_low2 > 0.0) {
+    if (tot_m > 0 && (a.theta_low2 > 0.0 || a.split)) {
         int32_t* cell_tmp;
         int8_t* low_tmp;
         PB_TRY(pb_dalloc_t(ctx, &cell_tmp, tot_m, CAT_TMP));
@@ -850,7 +908,8 @@ int pb_tree_build_impl(pb_ctx* ctx)
         k_partition_low<<<pb_blocks(G, 128), 128, 0, st>>>(G, t.m2p_off, cell_tmp, low_tmp, t.m2p_cell, m2p_low);
         PB_LAUNCH_CHECK();
     }
-    PB_TRY(pb_cover_count(ctx, G, PB_TG, N, t.m2p_off, t.m2p_cell, t.p2p_off, t.p2p_lo, t.p2p_hi, &t.covered_pairs));
+    PB_TRY(pb_cover_count(ctx, G, PB_TG, N, t.m2p_off, t.m2p_cell, t.p2p_off, t.p2p_lo, t.p2p_hi, &t.covered_pairs, nullptr, nullptr,
+                          0, t.p2p_mask, t.m2p_code));
     PB_TRY(pb_dalloc_t(ctx, &t.m2p_ctr, tot_m > 0 ? tot_m : 1, CAT_TREE));
     if (tot_m > 0) {
         k_m2p_centres<<<pb_blocks(tot_m, 256), 256, 0, st>>>(tot_m, t.m2p_cell, m2p_low, t.c_ctr[0], t.c_ctr[1], t.c_ctr[2], t.m2p_ctr);
@@ -866,7 +925,8 @@ int pb_tree_build_impl(pb_ctx* ctx)
         long long *dcost, *dpairs;
         PB_TRY(pb_dalloc_t(ctx, &dcost, G, CAT_TMP));
         PB_TRY(pb_dalloc_t(ctx, &dpairs, 2 * G, CAT_TMP));
-        k_group_cost<<<pb_blocks(G, 128), 128, 0, st>>>(G, N, t.m2p_off, t.p2p_off, t.p2p_lo, t.p2p_hi, dcost, dpairs);
+        k_group_cost<<<pb_blocks(G, 128), 128, 0, st>>>(G, N, t.m2p_off, t.p2p_off, t.p2p_lo, t.p2p_hi, t.p2p_mask, t.m2p_code, dcost,
+                                                        dpairs);
         PB_LAUNCH_CHECK();
         std::vector<int64_t> hcost(G), hpairs(2 * G), gfirst(world + 1);
         PB_CUDA(cudaMemcpyAsync(hcost.data(), dcost, sizeof(int64_t) * G, cudaMemcpyDeviceToHost, st));
@@ -943,6 +1003,8 @@ int pb_lists_build(pb_ctx* ctx, int tpl, int64_t ntargets, const double* tx, con
     a.theta = theta;
     a.theta_low2 = 0.0;
     a.m2p_low = nullptr;
+    a.p2p_mask = nullptr;
+    a.split = 0;
     a.m2p_min = m2p_min;
     a.c_first = oc.c_first; a.c_last = oc.c_last; a.c_child = oc.c_child; a.c_nchild = oc.c_nchild;
     a.cx = oc.c_ctr[0]; a.cy = oc.c_ctr[1]; a.cz = oc.c_ctr[2]; a.crad = oc.c_rad;
@@ -954,7 +1016,7 @@ int pb_lists_build(pb_ctx* ctx, int tpl, int64_t ntargets, const double* tx, con
     PB_CUDA(cudaMemsetAsync(cnt_p, 0, sizeof(int32_t) * (G + 1), st));
     PB_TRY(pb_scratch(ctx, 1 << 20));
     unsigned long long* pc = (unsigned long long*)ctx->scratch;
-    PB_CUDA(cudaMemsetAsync(pc, 0, 3 * sizeof(unsigned long long), st));
+    PB_CUDA(cudaMemsetAsync(pc, 0, 5 * sizeof(unsigned long long), st));
     a.n_m2p = cnt_m; a.n_p2p = cnt_p; a.m2p_cell = nullptr; a.p2p_lo = nullptr; a.p2p_hi = nullptr;
     a.pair_counts = pc;
     if (tpl == 2) k_lists<0, 2><<<pb_blocks(G, LIST_WARPS), LIST_WARPS * 32, 0, st>>>(a);
@@ -1016,6 +1078,8 @@ int pb_site_lists_build(pb_ctx* ctx)
     a.theta = ctx->prm.theta * PB_SITE_THETA_SCALE;
     a.theta_low2 = 0.0;
     a.m2p_low = nullptr;
+    a.p2p_mask = nullptr;
+    a.split = 0;
     a.m2p_min = 8;
     a.c_first = t.c_first; a.c_last = t.c_last; a.c_child = t.c_child; a.c_nchild = t.c_nchild;
     a.cx = t.c_ctr[0]; a.cy = t.c_ctr[1]; a.cz = t.c_ctr[2]; a.crad = t.c_rad;
@@ -1027,7 +1091,7 @@ int pb_site_lists_build(pb_ctx* ctx)
     PB_CUDA(cudaMemsetAsync(cnt_p, 0, sizeof(int32_t) * (G + 1), st));
     PB_TRY(pb_scratch(ctx, 1 << 20));
     unsigned long long* pc = (unsigned long long*)ctx->scratch;
-    PB_CUDA(cudaMemsetAsync(pc, 0, 3 * sizeof(unsigned long long), st));
+    PB_CUDA(cudaMemsetAsync(pc, 0, 5 * sizeof(unsigned long long), st));
     a.n_m2p = cnt_m; a.n_p2p = cnt_p; a.m2p_cell = nullptr; a.p2p_lo = nullptr; a.p2p_hi = nullptr;
     a.pair_counts = pc;
     k_lists<0, 1><<<pb_blocks(G, LIST_WARPS), LIST_WARPS * 32, 0, st>>>(a);

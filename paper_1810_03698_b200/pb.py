@@ -46,6 +46,7 @@ class Params(ctypes.Structure):
         ("gmres_restart", ctypes.c_int32), ("gmres_maxit", ctypes.c_int32), ("scf_tol_debye", ctypes.c_double),
         ("scf_omega", ctypes.c_double), ("scf_maxit", ctypes.c_int32), ("site_treecode", ctypes.c_int32),
         ("thole_a", ctypes.c_double), ("rhs_treecode", ctypes.c_int32), ("scf_recycle", ctypes.c_int32),
+        ("list_split", ctypes.c_int32),
     ]
 
 
@@ -79,7 +80,7 @@ class Stats(ctypes.Structure):
         ("ncrit_used", ctypes.c_int64), ("m2p_pairs_low", ctypes.c_int64),
         ("covered_pairs", ctypes.c_int64), ("site_p2p_pairs", ctypes.c_int64), ("site_m2p_pairs", ctypes.c_int64),
         ("site_covered_pairs", ctypes.c_int64), ("rhs_p2p_pairs", ctypes.c_int64), ("rhs_m2p_pairs", ctypes.c_int64),
-        ("rhs_covered_pairs", ctypes.c_int64),
+        ("rhs_covered_pairs", ctypes.c_int64), ("p2p_pairs_half", ctypes.c_int64), ("m2p_pairs_half", ctypes.c_int64),
     ]
 
     def as_dict(self):

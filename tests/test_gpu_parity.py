@@ -151,6 +151,41 @@ def test_treecode_error_falls_with_P_and_theta_and_ncrit_ragged(pbm, po, torch_c
     ctx.close()
 
 
+@pytest.mark.parametrize("target_panels,tail", [(2500, 40), (3500, 16)])
+def test_split_and_whole_group_lists(pbm, po, torch_cuda, target_panels, tail):
+    """pb_params.list_split: the two 32-target halves of a group take the MAC decisions of Eq. (28) separately (1) or
+    together (0).  Either way the stored lists cover every (target, source point) pair exactly once (counted from the
+    lists with their half masks), the matvec stays within the treecode bound of the oracle's dense product, and the
+    split lists evaluate fewer pairs.  The meshes end in a ragged group whose second half is partly filled (N % 64 = 40)
+    or empty (16)."""
+    from paper_1810_03698_b200.workloads import Workload, random_chain_globule, seed_for, vdw_surface
+    g = random_chain_globule(seed_for(2), 120)
+    v, t, _ = vdw_surface(g["pos"], g["radii"], target_panels=target_panels)
+    assert t.shape[0] % 64 == tail
+    sites = {k: g[k] for k in ("pos", "q", "dip", "quad", "alpha", "group")}
+    w = Workload("mini-globule", v, t, sites, dict(eps_in=1.0, eps_out=80.0, kappa=0.125, K_far=7))
+    orc, _, ctx = _setup(pbm, po, w, theta=0.5, order_P=6, ncrit=40)
+    x = _xvec(orc.nt, 9)
+    yref = np.concatenate(orc.matvec(x))
+    st, ys = {}, {}
+    for split in (0, 1):
+        ctx.set_params(list_split=split)
+        ctx.tree_build()
+        ys[split] = ctx.matvec(torch_cuda.from_numpy(x)).cpu().numpy()
+        st[split] = ctx.stats()
+        assert st[split]["covered_pairs"] == orc.nt * orc.nt * 7
+        assert rel(ys[split], yref) <= TOL_TREE
+    assert st[0]["p2p_pairs_half"] == 0 and st[0]["m2p_pairs_half"] == 0
+    assert st[1]["p2p_pairs_half"] > 0 and st[1]["m2p_pairs_half"] > 0
+    assert st[1]["p2p_pairs"] < st[0]["p2p_pairs"]
+    assert st[1]["p2p_pairs"] + 8 * st[1]["m2p_pairs"] < st[0]["p2p_pairs"] + 8 * st[0]["m2p_pairs"]
+    # the same decisions rule in direct mode (one range for everything, no masks to honour)
+    ctx.set_params(theta=0.0, list_split=1)
+    ctx.tree_build()
+    assert rel(ctx.matvec(torch_cuda.from_numpy(x)).cpu().numpy(), yref) <= TOL_DIRECT
+    ctx.close()
+
+
 def test_matvec_is_linear_and_independent_of_sites(pbm, po, torch_cuda):
     """The charge description enters only the RHS and the energy."""
     from paper_1810_03698_b200.workloads import make_config
