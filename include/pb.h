@@ -82,16 +82,25 @@ typedef struct pb_params {
                                1 = treecode with the sites as sources in their own octree (Cartesian multipole
                                moments of q, p, Q per site cell, Laplace far field at the collocation points) when
                                theta > 0, 2 (default) = treecode when N * N_a >= 2^31                          */
-    int32_t scf_recycle;    /* pb_solve: 1 (default) = every GMRES solve of the SCF loop starts from the minimal-residual
-                               combination of the corrections found by the loop's earlier solves (a recycled subspace:
-                               u_k with A u_k known from the Arnoldi relation, no extra operator application), then GMRES
-                               as usual to gmres_tol; 0 = plain warm start from the previous x (D: R-20)              */
+    int32_t scf_recycle;    /* pb_solve, how the systems A x_k = b(mu_k) of the SCF loop share work (they have one operator;
+                               D: R-20).  2 (default) = one GCR process over the whole loop: every search direction u
+                               with A u is kept (orthonormal A u), each system first takes the minimal-residual step in
+                               the stored space and then adds directions, one operator application each, until its
+                               residual has fallen by scf_eta (never below gmres_tol); up to 16 GB of directions, then
+                               restarted GMRES.  1 = flexible GMRES per system, started from the minimal-residual
+                               combination of the earlier systems' net corrections.  0 = GMRES per system, warm start
+                               from the previous x.  Non-polarizable solves (one system) always use GMRES.          */
     int32_t list_split;     /* interaction lists of the matvec: 1 (default) = the two halves (32 consecutive
                                Morton-ordered targets each) of a 64-target group take the MAC decisions of Eq. (28)
                                separately -- a cell accepted for one half only is listed for that half alone and only the
                                other half descends to its children; 0 = one decision per group (accepted only when the
                                MAC holds for all 64 targets).  Both cover every (target, source) pair exactly once and
                                satisfy the MAC per target; 1 evaluates fewer pairs (D: section 7)                     */
+    double scf_eta;         /* scf_recycle = 2: every system of the SCF loop is solved until its relative residual is
+                               max(gmres_tol, scf_eta * the residual it starts with, b(mu_k) - A x_{k-1}) -- the induced
+                               dipoles still change by a factor ~0.6 per step, so early systems need not be solved to
+                               gmres_tol.  The loop only ends on a step whose system was solved to gmres_tol, and the
+                               closing system is, too.  0 = every system to gmres_tol.  Default 0.03.               */
 } pb_params;
 
 /* Result of one polarizable solve (HOST struct). */

@@ -100,7 +100,8 @@ extern "C" void pb_default_params(pb_params* p)
     p->site_treecode = 2;
     p->thole_a = 0.39;
     p->rhs_treecode = 2;
-    p->scf_recycle = 1;
+    p->scf_recycle = 2;
+    p->scf_eta = 0.03;
     p->list_split = 1;
 }
 
@@ -185,7 +186,8 @@ extern "C" int pb_set_params(pb_ctx* ctx, const pb_params* p)
     if (p->precond < 0 || p->precond > 3) return pb_fail(ctx, PB_ERR_INVALID_ARG, "precond must be 0, 1, 2 or 3");
     if (p->site_treecode < 0 || p->site_treecode > 2) return pb_fail(ctx, PB_ERR_INVALID_ARG, "site_treecode must be 0, 1 or 2");
     if (p->rhs_treecode < 0 || p->rhs_treecode > 2) return pb_fail(ctx, PB_ERR_INVALID_ARG, "rhs_treecode must be 0, 1 or 2");
-    if (p->scf_recycle < 0 || p->scf_recycle > 1) return pb_fail(ctx, PB_ERR_INVALID_ARG, "scf_recycle must be 0 or 1");
+    if (p->scf_recycle < 0 || p->scf_recycle > 2) return pb_fail(ctx, PB_ERR_INVALID_ARG, "scf_recycle must be 0, 1 or 2");
+    if (!(p->scf_eta >= 0.0 && p->scf_eta < 1.0)) return pb_fail(ctx, PB_ERR_INVALID_ARG, "0 <= scf_eta < 1 required");
     if (p->list_split < 0 || p->list_split > 1) return pb_fail(ctx, PB_ERR_INVALID_ARG, "list_split must be 0 or 1");
     const pb_params& o = ctx->prm;
     bool shape = o.kappa != p->kappa || o.theta != p->theta || o.order_P != p->order_P ||

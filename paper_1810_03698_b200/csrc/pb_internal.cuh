@@ -210,6 +210,10 @@ struct pb_gmres_ws {
     // the RC orthonormal; xb / axb = x and A x before the current solve
     double *RU = nullptr, *RC = nullptr, *xb = nullptr, *axb = nullptr;
     int nrec = 0, rec_cap = 0;
+    // scf_recycle = 2: GCR with every search direction of the SCF loop kept: GU[k], GC[k] = A GU[k], the GC orthonormal;
+    // gh = device scalars of the orthogonalisation (coefficients [gcap], then a few dot products)
+    double *GU = nullptr, *GC = nullptr, *gh = nullptr;
+    int ngc = 0, gcap = 0;
 };
 
 struct pb_ctx {
@@ -350,5 +354,6 @@ int pb_prof_end(pb_ctx* ctx, int kernel);
 int pb_prof_drain(pb_ctx* ctx);
 void pb_prof_next(pb_ctx* ctx);
 // pb_solve.cu
+// tol_abs > 0 replaces pb_params.gmres_tol (the inexact solves of the SCF loop)
 int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters, double* relres, int32_t* matvecs,
-                  bool x_is_last_result);
+                  bool x_is_last_result, double tol_abs = 0.0);

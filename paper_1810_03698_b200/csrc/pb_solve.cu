@@ -466,42 +466,23 @@ static int dot_into(pb_ctx* ctx, gmres_ws& ws, int nv, const double* V, const do
     return PB_OK;
 }
 
-// Restarted GMRES with a right block-Jacobi preconditioner (D: R-20).  Per iteration: one operator
-// application (the preconditioner is folded into its first kernel), two classical Gram-Schmidt
-// passes of two kernels each -- the second also yields the norm of the new vector by Pythagoras and
-// writes it normalised -- and one small device-to-host copy of the Hessenberg column.
-// `x_is_last_result`: x still holds exactly what the previous call on this context returned (the SCF loop), so
-// A x is known from the Arnoldi relation A Minv V_j = V_{j+1} Hbar_j and the starting residual costs no operator
-// application: ws.ax is kept up to date with  A x += V_{j+1} (Hbar_j y)  whenever x += Minv V_j y.
-int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, double* relres_out, int32_t* matvecs_out,
-                  bool x_is_last_result)
+// workspace (kept until the system size, the restart length or the preconditioner changes); the Krylov bases of
+// GMRES only when asked for (the GCR path of the SCF loop keeps its own)
+static int ws_ensure(pb_ctx* ctx, int mode, int m, bool basis)
 {
     pb_tree& t = ctx->tree;
     cudaStream_t st = ctx->stream;
-    if (!t.built) return pb_fail(ctx, PB_ERR_NOT_READY, "pb_gmres: call pb_tree_build first");
     const int64_t n = 2 * t.N;
-    // preconditioner: 0 none, 1 block-Jacobi (folded into the operator's first kernel), 2 near-field (flexible GMRES),
-    // 3 = near-field from 8,000 panels up (measured per solve: C1 20.0 -> 19.2 ms, C2 117 -> 91 ms, C3 1412 -> 978 ms),
-    // else block-Jacobi
-    int mode = ctx->prm.precond;
-    if (mode == 3) mode = t.N >= 8000 ? 2 : 1;
-    if (t.psurf && mode == 2) mode = 1;   // two surfaces: the near-field matrix of mode 2 has Eq. (5)'s single-surface rows
-    int m = ctx->prm.gmres_restart;
-    if (m > n) m = (int)n;
-    if (m > 1000) m = 1000;
-    // workspace (kept until the system size or the restart length changes)
     gmres_ws& ws = ctx->gws;
-    if (ws.n != n || ws.m != m || ws.mode != mode || !ws.V) {
+    if (ws.n != n || ws.m != m || ws.mode != mode || !ws.r) {
         pb_dfree_cat(ctx, CAT_SOLVE);
         ws = gmres_ws();
-        PB_TRY(pb_dalloc_t(ctx, &ws.V, (size_t)(m + 1) * n, CAT_SOLVE));
         PB_TRY(pb_dalloc_t(ctx, &ws.w, n, CAT_SOLVE));
         PB_TRY(pb_dalloc_t(ctx, &ws.r, n, CAT_SOLVE));
         PB_TRY(pb_dalloc_t(ctx, &ws.u, n, CAT_SOLVE));
         PB_TRY(pb_dalloc_t(ctx, &ws.z, n, CAT_SOLVE));
         PB_TRY(pb_dalloc_t(ctx, &ws.ax, n, CAT_SOLVE));
         if (mode == 2) {
-            PB_TRY(pb_dalloc_t(ctx, &ws.Z, (size_t)m * n, CAT_SOLVE));
             PB_TRY(pb_dalloc_t(ctx, &ws.nf_r, n, CAT_SOLVE));
             PB_TRY(pb_dalloc_t(ctx, &ws.nf_p, n, CAT_SOLVE));
             PB_TRY(pb_dalloc_t(ctx, &ws.nf_q, n, CAT_SOLVE));
@@ -516,6 +497,53 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
         ws.n = n;
         ws.m = m;
     }
+    if (basis && !ws.V) {
+        PB_TRY(pb_dalloc_t(ctx, &ws.V, (size_t)(m + 1) * n, CAT_SOLVE));
+        if (mode == 2) PB_TRY(pb_dalloc_t(ctx, &ws.Z, (size_t)m * n, CAT_SOLVE));
+    }
+    return PB_OK;
+}
+
+// preconditioner of pb_params.precond as it applies to this system: 0 none, 1 block-Jacobi, 2 near-field
+static int precond_mode(pb_ctx* ctx)
+{
+    const pb_tree& t = ctx->tree;
+    int mode = ctx->prm.precond;
+    // 3 = near-field from 8,000 panels up (measured per solve: C1 20.0 -> 19.2 ms, C2 117 -> 91 ms, C3 1412 -> 978 ms),
+    // else block-Jacobi
+    if (mode == 3) mode = t.N >= 8000 ? 2 : 1;
+    if (t.psurf && mode == 2) mode = 1;   // two surfaces: the near-field matrix of mode 2 has Eq. (5)'s single-surface rows
+    return mode;
+}
+
+static int restart_length(pb_ctx* ctx)
+{
+    const int64_t n = 2 * ctx->tree.N;
+    int m = ctx->prm.gmres_restart;
+    if (m > n) m = (int)n;
+    if (m > 1000) m = 1000;
+    return m;
+}
+
+// Restarted GMRES with a right block-Jacobi preconditioner (D: R-20).  Per iteration: one operator
+// application (the preconditioner is folded into its first kernel), two classical Gram-Schmidt
+// passes of two kernels each -- the second also yields the norm of the new vector by Pythagoras and
+// writes it normalised -- and one small device-to-host copy of the Hessenberg column.
+// `x_is_last_result`: x still holds exactly what the previous call on this context returned (the SCF loop), so
+// A x is known from the Arnoldi relation A Minv V_j = V_{j+1} Hbar_j and the starting residual costs no operator
+// application: ws.ax is kept up to date with  A x += V_{j+1} (Hbar_j y)  whenever x += Minv V_j y.
+int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, double* relres_out, int32_t* matvecs_out,
+                  bool x_is_last_result, double tol_abs)
+{
+    pb_tree& t = ctx->tree;
+    cudaStream_t st = ctx->stream;
+    if (!t.built) return pb_fail(ctx, PB_ERR_NOT_READY, "pb_gmres: call pb_tree_build first");
+    const int64_t n = 2 * t.N;
+    // preconditioner: 0 none, 1 block-Jacobi (folded into the operator's first kernel), 2 near-field (flexible GMRES)
+    const int mode = precond_mode(ctx);
+    const int m = restart_length(ctx);
+    PB_TRY(ws_ensure(ctx, mode, m, true));
+    gmres_ws& ws = ctx->gws;
     bool have_ax = x_is_last_result && ws.ax_valid;
     ws.ax_valid = false;
     const int hstride = m + 4;
@@ -524,7 +552,7 @@ int pb_gmres_impl(pb_ctx* ctx, const double* b, double* x, int32_t* iters_out, d
     double* hy = hh + 2 * hstride;                 // staging for y (x += Z y) and for Hbar y (A x += V Hbar y): written at the end
     double* hc = hy + m;                           // of a cycle only, and every cycle starts with a stream synchronisation
     const bool pc = mode == 1;
-    const double tol = ctx->prm.gmres_tol;
+    const double tol = tol_abs > 0.0 ? tol_abs : ctx->prm.gmres_tol;
     const int maxit = ctx->prm.gmres_maxit;
     int iters = 0, matvecs = 0;
     int rc = PB_OK;
@@ -771,7 +799,7 @@ __global__ void k_any_nonzero(int64_t n, const double* __restrict__ a, int* __re
 // residual and runs to the same tolerance as without it.
 static int recycle_alloc(pb_ctx* ctx, gmres_ws& ws)
 {
-    if (ws.RU || !ws.V) return PB_OK;
+    if (ws.RU || !ws.r) return PB_OK;
     int cap = ctx->prm.scf_maxit < 48 ? ctx->prm.scf_maxit : 48;
     if ((size_t)cap * ws.n * sizeof(double) * 2 > ((size_t)4 << 30)) cap = (int)(((size_t)2 << 30) / (ws.n * sizeof(double)));   // <= 4 GB
     if (cap > ws.m) cap = ws.m;                         // the dot / coefficient buffers are sized for the restart length
@@ -836,6 +864,211 @@ static int recycle_append(pb_ctx* ctx, gmres_ws& ws, const double* x)
     return PB_OK;
 }
 
+// ---- GCR over the whole SCF loop (pb_params.scf_recycle = 2; D: R-20) --------------------------------------------------
+// The systems of the loop, A x_k = b_perm + B mu_k, share the operator.  GMRES started afresh for every one of them
+// rebuilds the same slowly converging part of the Krylov space every time (measured at C4: 22 iterations per SCF step
+// on average although the right-hand side changes by a factor 0.6 per step).  Here every search direction ever used is
+// kept: GU[k] and GC[k] = A GU[k], the GC orthonormal (generalised conjugate residuals, Eisenstat / Elman / Schultz
+// 1983, with the preconditioned residual as the new direction; flexible: the preconditioner may change from step to
+// step).  A solve first takes the minimal-residual step in the stored space (one batch of dot products, no operator
+// application), then adds directions until the residual is small enough:
+//     z = M(r);  c = A z;  (c, z) orthogonalised against all (GC, GU) by classical Gram-Schmidt, twice, normalised;
+//     alpha = c . r;  x += alpha u;  A x += alpha c;  r -= alpha c.
+// A x is carried along (linearity of the operator with its fixed lists), so a solve costs exactly one operator
+// application per new direction.  When the store is full the remaining work goes to restarted GMRES.
+__global__ void __launch_bounds__(256)
+k_gcr_orth(int64_t n, int nv, const double* __restrict__ C, const double* __restrict__ U, int64_t ld,
+           const double* __restrict__ h, double* __restrict__ c, double* __restrict__ u)
+{
+    extern __shared__ double sh[];
+    for (int j = threadIdx.x; j < nv; j += blockDim.x) sh[j] = h[j];
+    __syncthreads();
+    for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
+        double ac = c[e], au = u[e];
+        int j = 0;
+        for (; j + 4 <= nv; j += 4) {
+            const double c0 = C[(int64_t)j * ld + e], c1 = C[(int64_t)(j + 1) * ld + e], c2 = C[(int64_t)(j + 2) * ld + e],
+                         c3 = C[(int64_t)(j + 3) * ld + e];
+            const double u0 = U[(int64_t)j * ld + e], u1 = U[(int64_t)(j + 1) * ld + e], u2 = U[(int64_t)(j + 2) * ld + e],
+                         u3 = U[(int64_t)(j + 3) * ld + e];
+            ac = fma(-sh[j], c0, ac); au = fma(-sh[j], u0, au);
+            ac = fma(-sh[j + 1], c1, ac); au = fma(-sh[j + 1], u1, au);
+            ac = fma(-sh[j + 2], c2, ac); au = fma(-sh[j + 2], u2, au);
+            ac = fma(-sh[j + 3], c3, ac); au = fma(-sh[j + 3], u3, au);
+        }
+        for (; j < nv; ++j) { ac = fma(-sh[j], C[(int64_t)j * ld + e], ac); au = fma(-sh[j], U[(int64_t)j * ld + e], au); }
+        c[e] = ac;
+        u[e] = au;
+    }
+}
+
+// the minimal-residual step in the stored space: x += GU a, A x += GC a, r -= GC a with a = GC^T r
+__global__ void __launch_bounds__(256)
+k_gcr_project(int64_t n, int nv, const double* __restrict__ C, const double* __restrict__ U, int64_t ld,
+              const double* __restrict__ a, double* __restrict__ x, double* __restrict__ ax, double* __restrict__ r)
+{
+    extern __shared__ double sh[];
+    for (int j = threadIdx.x; j < nv; j += blockDim.x) sh[j] = a[j];
+    __syncthreads();
+    for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
+        double sc = 0, su = 0;
+        for (int j = 0; j < nv; ++j) {
+            sc = fma(sh[j], C[(int64_t)j * ld + e], sc);
+            su = fma(sh[j], U[(int64_t)j * ld + e], su);
+        }
+        x[e] += su;
+        ax[e] += sc;
+        r[e] -= sc;
+    }
+}
+
+// d = {r . c, c . c} of the orthogonalised, not yet normalised pair: normalise (c, u), then the step along them
+__global__ void __launch_bounds__(256)
+k_gcr_step(int64_t n, const double* __restrict__ d, double* __restrict__ c, double* __restrict__ u, double* __restrict__ x,
+           double* __restrict__ ax, double* __restrict__ r)
+{
+    const double cc = d[1];
+    const double inv = cc > 0 ? 1.0 / sqrt(cc) : 0.0;
+    const double alpha = d[0] * inv;                    // (c / |c|) . r
+    for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
+        const double ce = c[e] * inv, ue = u[e] * inv;
+        c[e] = ce;
+        u[e] = ue;
+        x[e] = fma(alpha, ue, x[e]);
+        ax[e] = fma(alpha, ce, ax[e]);
+        r[e] = fma(-alpha, ce, r[e]);
+    }
+}
+
+static int gcr_alloc(pb_ctx* ctx, gmres_ws& ws)
+{
+    if (ws.GU || !ws.r) return PB_OK;
+    // room for a few hundred directions; at most 16 GB for the two bases (C4: 493 directions of 16.6 MB each)
+    size_t cap = ((size_t)16 << 30) / (2 * (size_t)ws.n * sizeof(double));
+    if (cap > 1024) cap = 1024;
+    if (cap > (size_t)ws.n) cap = (size_t)ws.n;
+    if (cap < 1) return PB_OK;
+    PB_TRY(pb_dalloc_t(ctx, &ws.GU, cap * ws.n, CAT_SOLVE));
+    PB_TRY(pb_dalloc_t(ctx, &ws.GC, cap * ws.n, CAT_SOLVE));
+    PB_TRY(pb_dalloc_t(ctx, &ws.gh, cap + 16, CAT_SOLVE));
+    ws.gcap = (int)cap;
+    ws.ngc = 0;
+    return PB_OK;
+}
+
+// gh[0..k) = GC^T w, in batches of at most ws.m vectors (the size the reduction buffers were made for)
+static int gcr_dots(pb_ctx* ctx, gmres_ws& ws, int k, const double* w)
+{
+    for (int c0 = 0; c0 < k; c0 += ws.m) {
+        const int nv = k - c0 < ws.m ? k - c0 : ws.m;
+        PB_TRY(dot_into(ctx, ws, nv, ws.GC + (size_t)c0 * ws.n, w, false, ws.gh + c0));
+    }
+    return PB_OK;
+}
+
+// One system of the SCF loop.  Needs ws.ax = A x on entry (x = 0, A x = 0 before the first one) and keeps it.
+// tol_factor > 0: stop at max(gmres_tol, tol_factor * the relative residual the system starts with).
+static int gcr_solve(pb_ctx* ctx, const double* b, double* x, double tol_factor, int32_t* iters_out, double* relres_out,
+                     int32_t* matvecs_out, double* tol_out)
+{
+    pb_tree& t = ctx->tree;
+    cudaStream_t st = ctx->stream;
+    const int64_t n = 2 * t.N;
+    const int mode = precond_mode(ctx);
+    PB_TRY(ws_ensure(ctx, mode, restart_length(ctx), false));
+    gmres_ws& ws = ctx->gws;
+    PB_TRY(gcr_alloc(ctx, ws));
+    const int tb = 256;
+    const int nb = pb_blocks(n, tb) < 2368 ? pb_blocks(n, tb) : 2368;
+    double* dsc = ws.gh + ws.gcap;                       // device scalars: [0] b.b, [1] r.r, [2] r.c, [3] c.c
+    int iters = 0, matvecs = 0;
+    k_residual<<<pb_blocks(n, tb), tb, 0, st>>>(n, b, ws.ax, ws.r);
+    PB_LAUNCH_CHECK();
+    PB_TRY(dot_into(ctx, ws, 0, nullptr, b, true, dsc));
+    PB_TRY(dot_into(ctx, ws, 0, nullptr, ws.r, true, dsc + 1));
+    double h[4];
+    PB_CUDA(cudaMemcpyAsync(h, dsc, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    PB_CUDA(cudaStreamSynchronize(st));
+    const double bnorm = sqrt(h[0]);
+    *iters_out = 0; *matvecs_out = 0; *tol_out = ctx->prm.gmres_tol;
+    if (bnorm == 0.0) {
+        PB_CUDA(cudaMemsetAsync(x, 0, sizeof(double) * n, st));
+        PB_CUDA(cudaMemsetAsync(ws.ax, 0, sizeof(double) * n, st));
+        ws.ax_valid = true;
+        *relres_out = 0.0;
+        return PB_OK;
+    }
+    double relres = sqrt(h[1]) / bnorm;
+    // The x of the previous system already solves this one to gmres_tol: keep it.  (Late in the loop the right-hand side
+    // changes by less than gmres_tol * |b|; a step in the stored space would then follow a change it cannot resolve --
+    // measured at C2 with every system solved to 1e-6: the dipole change stops falling at 5e-6 D and oscillates.)
+    if (relres <= ctx->prm.gmres_tol) {
+        ws.ax_valid = true;
+        *relres_out = relres;
+        return PB_OK;
+    }
+    // ... and a system that does need work is solved to a quarter of gmres_tol, so that the small changes of the next
+    // right-hand sides leave its x valid for them (with the target at gmres_tol itself every late step took another
+    // step in the stored space: C3 needed 95 SCF steps instead of 31)
+    double tol = 0.25 * ctx->prm.gmres_tol;
+    if (tol_factor > 0.0 && tol_factor * relres > tol) tol = tol_factor * relres;
+    if (ws.ngc > 0) {
+        PB_TRY(gcr_dots(ctx, ws, ws.ngc, ws.r));
+        k_gcr_project<<<nb, tb, ws.ngc * sizeof(double), st>>>(n, ws.ngc, ws.GC, ws.GU, n, ws.gh, x, ws.ax, ws.r);
+        PB_LAUNCH_CHECK();
+        PB_TRY(dot_into(ctx, ws, 0, nullptr, ws.r, true, dsc + 1));
+        PB_CUDA(cudaMemcpyAsync(h + 1, dsc + 1, sizeof(double), cudaMemcpyDeviceToHost, st));
+        PB_CUDA(cudaStreamSynchronize(st));
+        relres = sqrt(h[1]) / bnorm;
+    }
+    int rc = PB_OK;
+    while (relres > tol) {
+        if (ws.ngc >= ws.gcap || iters >= ctx->prm.gmres_maxit) {
+            // the store is full: restarted GMRES finishes this system from the x and A x reached so far
+            int32_t gi = 0, mv = 0;
+            ws.ax_valid = true;
+            rc = pb_gmres_impl(ctx, b, x, &gi, &relres, &mv, true, tol);
+            iters += gi;
+            matvecs += mv;
+            break;
+        }
+        double* u = ws.GU + (size_t)ws.ngc * n;
+        double* c = ws.GC + (size_t)ws.ngc * n;
+        if (mode == 2) PB_TRY(near_precond(ctx, ws, ws.r, u));
+        else if (mode == 1) {
+            k_precond<<<pb_blocks(t.N, tb), tb, 0, st>>>(t.N, t.precond, ws.r, u);
+            PB_LAUNCH_CHECK();
+        } else
+            PB_CUDA(cudaMemcpyAsync(u, ws.r, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+        PB_TRY(pb_matvec_impl(ctx, u, c, false, false));
+        ++matvecs;
+        for (int pass = 0; pass < 2 && ws.ngc > 0; ++pass) {
+            PB_TRY(gcr_dots(ctx, ws, ws.ngc, c));
+            k_gcr_orth<<<nb, tb, ws.ngc * sizeof(double), st>>>(n, ws.ngc, ws.GC, ws.GU, n, ws.gh, c, u);
+            PB_LAUNCH_CHECK();
+        }
+        PB_TRY(dot_into(ctx, ws, 1, ws.r, c, true, dsc + 2));              // r . c and c . c
+        k_gcr_step<<<nb, tb, 0, st>>>(n, dsc + 2, c, u, x, ws.ax, ws.r);
+        PB_LAUNCH_CHECK();
+        PB_TRY(dot_into(ctx, ws, 0, nullptr, ws.r, true, dsc + 1));
+        PB_CUDA(cudaMemcpyAsync(h, dsc, 4 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        PB_CUDA(cudaStreamSynchronize(st));
+        ++iters;
+        if (!(h[3] > 0.0)) {                            // A M(r) lies in the stored space: nothing new to add (singular operator)
+            rc = pb_fail(ctx, PB_ERR_NO_CONVERGENCE, "GCR: breakdown at relative residual %.3e", relres);
+            break;
+        }
+        ++ws.ngc;
+        relres = sqrt(h[1]) / bnorm;
+    }
+    if (rc == PB_OK) ws.ax_valid = true;
+    *iters_out = iters;
+    *relres_out = relres;
+    *matvecs_out = matvecs;
+    *tol_out = tol;
+    return rc;
+}
+
 static int pb_solve_core(pb_ctx* ctx, double* x_out, double* mu_out, pb_result* res, bool host_out)
 {
     pb_tree& t = ctx->tree;
@@ -894,35 +1127,52 @@ static int pb_solve_core(pb_ctx* ctx, double* x_out, double* mu_out, pb_result* 
     int it = 0, gm_total = 0, mv_total = 0;
     double delta = 0, relres = 0;
     bool conv = false;
+    // scf_recycle = 2: one GCR process over all the systems of the loop, each solved only as far as the loop needs it
+    // (a fixed reduction scf_eta of its starting residual, never below gmres_tol); the loop ends on a step that was
+    // solved to gmres_tol.  1: GMRES per system, started from the stored corrections of the earlier ones.  0: plain.
+    const int recycle_mode = polarizable ? ctx->prm.scf_recycle : 0;
+    bool full_tol = !(ctx->prm.scf_eta > 0.0);
+    if (recycle_mode == 2) {
+        PB_TRY(ws_ensure(ctx, precond_mode(ctx), restart_length(ctx), false));
+        ctx->gws.ngc = 0;                                            // the stored directions belong to one SCF loop
+        PB_CUDA(cudaMemsetAsync(ctx->gws.ax, 0, sizeof(double) * n, st));   // x = 0, A x = 0
+        ctx->gws.ax_valid = true;
+    }
     for (it = 1; it <= ctx->prm.scf_maxit; ++it) {
         int32_t gi = 0, mv = 0;
+        double tol_used = ctx->prm.gmres_tol;
         PB_TRY(pb_rhs_multipole(ctx, mu, b));                        // step 2: Eq. (5) with p = d + mu
-        const bool recycle = polarizable && ctx->prm.scf_recycle != 0;
-        gmres_ws& ws = ctx->gws;
-        if (recycle && it > 1) {
-            PB_TRY(recycle_alloc(ctx, ws));
-            PB_TRY(recycle_project(ctx, ws, b, x));                  // minimal-residual step in the recycled subspace
-            if (ws.xb && ws.ax_valid) {
-                PB_CUDA(cudaMemcpyAsync(ws.xb, x, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
-                PB_CUDA(cudaMemcpyAsync(ws.axb, ws.ax, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+        int rc = PB_OK;
+        if (recycle_mode == 2) {
+            rc = gcr_solve(ctx, b, x, full_tol ? 0.0 : ctx->prm.scf_eta, &gi, &relres, &mv, &tol_used);
+        } else {
+            const bool recycle = recycle_mode == 1;
+            gmres_ws& ws = ctx->gws;
+            if (recycle && it > 1) {
+                PB_TRY(recycle_alloc(ctx, ws));
+                PB_TRY(recycle_project(ctx, ws, b, x));              // minimal-residual step in the recycled subspace
+                if (ws.xb && ws.ax_valid) {
+                    PB_CUDA(cudaMemcpyAsync(ws.xb, x, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+                    PB_CUDA(cudaMemcpyAsync(ws.axb, ws.ax, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+                }
+            }
+            const bool had_ax = it > 1 && ws.ax_valid;
+            rc = pb_gmres_impl(ctx, b, x, &gi, &relres, &mv, it > 1);
+            if (rc == PB_OK && recycle && gi > 0) {
+                if (it == 1) {                                       // the cold solve: x_b = 0, A x_b = 0
+                    PB_TRY(recycle_alloc(ctx, ws));
+                    if (ws.xb) {
+                        PB_CUDA(cudaMemsetAsync(ws.xb, 0, sizeof(double) * n, st));
+                        PB_CUDA(cudaMemsetAsync(ws.axb, 0, sizeof(double) * n, st));
+                        PB_TRY(recycle_append(ctx, ws, x));
+                    }
+                } else if (ws.xb && had_ax)
+                    PB_TRY(recycle_append(ctx, ws, x));
             }
         }
-        const bool had_ax = it > 1 && ws.ax_valid;
-        int rc = pb_gmres_impl(ctx, b, x, &gi, &relres, &mv, it > 1);
         if (rc == PB_ERR_NO_CONVERGENCE) status = rc; else if (rc != PB_OK) return rc;
         gm_total += gi;
         mv_total += mv;
-        if (recycle && gi > 0) {
-            if (it == 1) {                                           // the cold solve: x_b = 0, A x_b = 0
-                PB_TRY(recycle_alloc(ctx, ws));
-                if (ws.xb) {
-                    PB_CUDA(cudaMemsetAsync(ws.xb, 0, sizeof(double) * n, st));
-                    PB_CUDA(cudaMemsetAsync(ws.axb, 0, sizeof(double) * n, st));
-                    PB_TRY(recycle_append(ctx, ws, x));
-                }
-            } else if (ws.xb && had_ax)
-                PB_TRY(recycle_append(ctx, ws, x));
-        }
         if (!polarizable) { conv = true; break; }
         PB_TRY(pb_reaction_field(ctx, x, nullptr, gs, nullptr));      // step 3: Eq. (13)
         PB_TRY(pb_multipole_field_impl(ctx, mu, 2, 1, nullptr, gm, nullptr));   // step 3: Eq. (14), induced part
@@ -931,11 +1181,19 @@ static int pb_solve_core(pb_ctx* ctx, double* x_out, double* mu_out, pb_result* 
         PB_CUDA(cudaMemcpyAsync(h, dscal, sizeof(double), cudaMemcpyDeviceToHost, st));
         PB_CUDA(cudaStreamSynchronize(st));
         delta = sqrt(h[0] / (double)na) * PB_DEBYE;
+        if (delta < tol && tol_used > ctx->prm.gmres_tol) {           // small change after an inexact solve: confirm it
+            full_tol = true;                                          // with systems solved to gmres_tol from here on
+            continue;
+        }
         if (delta < tol) {                                            // step 6
             // surface solution consistent with the final mu
             PB_TRY(pb_rhs_multipole(ctx, mu, b));
-            if (recycle) PB_TRY(recycle_project(ctx, ws, b, x));
-            rc = pb_gmres_impl(ctx, b, x, &gi, &relres, &mv, true);
+            if (recycle_mode == 2)
+                rc = gcr_solve(ctx, b, x, 0.0, &gi, &relres, &mv, &tol_used);
+            else {
+                if (recycle_mode == 1) PB_TRY(recycle_project(ctx, ctx->gws, b, x));
+                rc = pb_gmres_impl(ctx, b, x, &gi, &relres, &mv, true);
+            }
             if (rc == PB_ERR_NO_CONVERGENCE) status = rc; else if (rc != PB_OK) return rc;
             gm_total += gi;
             mv_total += mv;

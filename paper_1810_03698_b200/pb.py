@@ -46,7 +46,7 @@ class Params(ctypes.Structure):
         ("gmres_restart", ctypes.c_int32), ("gmres_maxit", ctypes.c_int32), ("scf_tol_debye", ctypes.c_double),
         ("scf_omega", ctypes.c_double), ("scf_maxit", ctypes.c_int32), ("site_treecode", ctypes.c_int32),
         ("thole_a", ctypes.c_double), ("rhs_treecode", ctypes.c_int32), ("scf_recycle", ctypes.c_int32),
-        ("list_split", ctypes.c_int32),
+        ("list_split", ctypes.c_int32), ("scf_eta", ctypes.c_double),
     ]
 
 
