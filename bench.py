@@ -10,6 +10,10 @@ theta = 0.5, P = 6), the largest single-GPU configuration.
              Eq. (3)-(4); one M2P interaction = one (target, cell) pair producing all four order-P sums.  Both
              counts come from the stored lists (pb_get_stats) and are reported separately under "evaluated";
              "direct_equivalent_per_s" = N * N_s / time (the pairs the dense operator accounts for) is a side key.
+             The count depends on the lists: with pb_params.list_split = 1 (default; the two 32-target halves of a group
+             decided separately) one C4 matvec evaluates 25 % fewer interactions than with one decision per group and
+             takes 8 % less time, so `value` falls while ms_per_step and direct_equivalent_per_s improve; --list-split 0
+             gives the other lists.
   e2e      = the same step through pb_matvec_host: x copied from pinned host memory, y copied back, every step.
   roofline = both hot kernels, FP64 ALU bound.  Per kernel: (i) algorithmic flop (80 per P2P pair;
              4 N_T + N_k + 6 P + 30 per M2P pair at the order it is evaluated at) / CUDA-event time / measured
@@ -259,6 +263,12 @@ def run_ours(args):
         prm["order_P"] = args.order
     if args.ncrit is not None:
         prm["ncrit"] = args.ncrit
+    if args.list_split is not None:
+        prm["list_split"] = args.list_split
+    if args.scf_recycle is not None:
+        prm["scf_recycle"] = args.scf_recycle
+    if args.scf_eta is not None:
+        prm["scf_eta"] = args.scf_eta
     ctx = pb.PB(local_rank, **prm)
     s = w.sites
     ctx.mesh_load(w.verts, w.tris)
@@ -397,6 +407,7 @@ def run_ours(args):
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": w.name, "panels": nt, "gauss_points": int(st1["n_sources"]), "sites": na,
                    "theta": theta, "order_P": P, "ncrit": int(st1["ncrit_used"]), "K_far": int(w.params["K_far"]),
+                   "list_split": int(ctx.get_params().list_split),
                    "step": "one treecode matvec of Eq. (5) on a resident vector",
                    "l2": "flushed between steps (256 MiB device write, outside the event pairs); the step's own "
                          "inputs (0.46 GB source records, 1.3 GB near table at C4) exceed the 126 MB L2",
@@ -404,6 +415,8 @@ def run_ours(args):
                                                                  f"of y's owned rows per step" if sharded else f"{world} replicas")},
         "evaluated": {"p2p_pairs_per_matvec": int(p2p_pairs), "m2p_pairs_per_matvec": int(m2p_pairs),
                       "m2p_pairs_at_order_P_minus_2": int(sum_over_ranks(float(st1["m2p_pairs_low"]), world, dev)) if world == 1 else None,
+                      "p2p_pairs_for_one_half_of_a_group": int(st1["p2p_pairs_half"]) if world == 1 else None,
+                      "m2p_pairs_for_one_half_of_a_group": int(st1["m2p_pairs_half"]) if world == 1 else None,
                       "covered_pairs": int(st1["covered_pairs"]), "covered_equals_N_x_Ns": bool(st1["covered_pairs"] == int(inter_per_mv)) if world == 1 else None,
                       "direct_equivalent_per_s": inter_per_mv * (1 if sharded or world == 1 else world) * args.steps / (ms_total * 1e-3)},
         "gpu_launches": int(launches),
@@ -427,7 +440,8 @@ def run_ours(args):
         line["solve"] = {"workload": w.name, "time_per_polarizable_solve_s": e0.elapsed_time(e1) * 1e-3, "runs": 1,
                          "dG_solv_kcal_mol": res["dG_solv"], "scf_iters": res["scf_iters"], "gmres_iters": res["gmres_iters_total"],
                          "matvecs": res["matvecs_total"], "final_gmres_relres": res["final_gmres_relres"],
-                         "final_scf_delta_debye": res["final_scf_delta_debye"], "status": res["status"]}
+                         "final_scf_delta_debye": res["final_scf_delta_debye"], "status": res["status"],
+                         "scf_recycle": int(ctx.get_params().scf_recycle), "scf_eta": float(ctx.get_params().scf_eta)}
     ctx.close()
     if world == 1 and not args.no_configs:
         cfgs = {}
@@ -555,6 +569,11 @@ def main():
     ap.add_argument("--theta", type=float, default=None)
     ap.add_argument("--order", type=int, default=None)
     ap.add_argument("--ncrit", type=int, default=None)
+    ap.add_argument("--list-split", type=int, default=None, choices=(0, 1),
+                    help="pb_params.list_split: 1 (library default) = the two 32-target halves of a group take the MAC decisions "
+                         "separately, 0 = one decision per 64-target group")
+    ap.add_argument("--scf-recycle", type=int, default=None, choices=(0, 1, 2), help="pb_params.scf_recycle (library default 2)")
+    ap.add_argument("--scf-eta", type=float, default=None, help="pb_params.scf_eta (library default 0.03)")
     ap.add_argument("--ref-rows", type=int, default=256,
                     help="target rows per oracle call (cpu_baseline and --impl reference): about 2 s per call at C4 on 16 cores")
     ap.add_argument("--no-cpu-baseline", action="store_true")
