@@ -472,6 +472,7 @@ extern "C" int pb_tree_build(pb_ctx* ctx)
         ctx->sites.tree_built = false;
         ctx->sites.rhs_built = false;
     ctx->attr_m2p_mask = 0;
+    ctx->attr_p2p_set = false;
     ctx->attr_up_bytes = 0;
     ctx->attr_site_bytes[0] = ctx->attr_site_bytes[1] = 0;
     if (ctx->stern_n1 > 0 && ctx->shard_world > 1)

@@ -87,6 +87,7 @@ struct pb_tree {
     int32_t* p2p_off = nullptr;   // [groups+1]
     int32_t* p2p_lo = nullptr;    // source-point ranges [lo, hi)
     int32_t* p2p_hi = nullptr;
+    int4* p2p_rng = nullptr;      // [ranges + 2] {lo, hi, mask, 0}: one 16-byte load per range for k_p2p2
     int8_t* p2p_mask = nullptr;   // [ranges] which half of the group the range is for: 1 = targets 0..31, 2 = 32..63, 3 = both (k_lists)
     int8_t* m2p_code = nullptr;   // [entries] bit 0: order P - 2; bits 1-2: the same half mask (also in m2p_ctr[e].w)
     int64_t p2p_pairs = 0, m2p_pairs = 0, m2p_pairs_low = 0;   // m2p_pairs_low: those evaluated at order P - 2
@@ -256,6 +257,7 @@ struct pb_ctx {
     // cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is per device and per function: remembered per context
     // (a context lives on one device), bit P for k_m2p2<P> / k_m2p<P>, byte counts for the others
     uint32_t attr_m2p_mask = 0;
+    bool attr_p2p_set = false;
     size_t attr_up_bytes = 0, attr_site_bytes[2] = {0, 0};
     int dots_occ = 0;
     // profiling: CUDA-event pairs around every P2P and M2P launch (pb_set_profiling)

@@ -1035,25 +1035,34 @@ k_p2p(int64_t N, int K, double kappa, pb_expk8 ek, const pb_item* __restrict__ i
     }
 }
 
+// A ring of P2Q_NS tiles: a leaf holds about 40 Gauss points at C4 and a range is a run of adjacent leaves for the same
+// half of the group, often a single one, so a tile is short (the eight warps get five sources each) and one tile of
+// look-ahead did not cover the latency of the next copy plus that of the range descriptor it starts from (ncu source
+// page, C4: 14 % of the kernel's samples before the first pair and in the descriptor loads).  Descriptors are one
+// 16-byte load each and are fetched one range ahead.
+#define P2Q_NS 3
+#define P2Q_SMEM (P2Q_NS * 2 * P2P_TILE * sizeof(double4) + 256 * sizeof(double) + P2Q_NS * sizeof(uint64_t))
 __global__ void __launch_bounds__(P2P_THREADS, 2)
-k_p2p2(int64_t N, int K, double kappa, pb_expk8 ek, const pb_item* __restrict__ items,
-       const int32_t* __restrict__ p2p_lo, const int32_t* __restrict__ p2p_hi, const int8_t* __restrict__ p2p_mask,
+k_p2p2(int64_t N, int K, double kappa, pb_expk8 ek, const pb_item* __restrict__ items, const int4* __restrict__ p2p_rng,
        const double4* __restrict__ srec, const double* __restrict__ px, const double* __restrict__ py, const double* __restrict__ pz,
        double* __restrict__ acc)
 {
-    __shared__ __align__(128) double4 tile[2][2 * P2P_TILE];
-    __shared__ __align__(8) uint64_t bar[2];
-    __shared__ double Ts[256];
+    extern __shared__ __align__(128) unsigned char p2q_raw[];
+    double4* tiles = reinterpret_cast<double4*>(p2q_raw);                                  // [P2Q_NS][2 * P2P_TILE]
+    double* Ts = reinterpret_cast<double*>(p2q_raw + P2Q_NS * 2 * P2P_TILE * sizeof(double4));   // [256]
+    uint64_t* bar = reinterpret_cast<uint64_t*>(Ts + 256);                                 // [P2Q_NS]
     static_assert(PB_TG == 64 && P2P_THREADS == 32 * P2Q_W, "two targets per lane, eight warps");
     const int tid = threadIdx.x;
     const int lane = tid & 31, sub = tid >> 5;
     const pb_item item = items[blockIdx.x];
     const int64_t g = item.group;
     const int slice = item.slot;
+    int32_t r = item.r;
+    int4 rc = p2p_rng[r], rn = p2p_rng[r + 1];           // this range and the next one {lo, hi, mask}
     Ts[tid] = c_T256[tid];
     if (tid == 0) {
-        pb_mbar_init(&bar[0], 1);
-        pb_mbar_init(&bar[1], 1);
+#pragma unroll
+        for (int s = 0; s < P2Q_NS; ++s) pb_mbar_init(&bar[s], 1);
         pb_mbar_fence_init();
     }
     __syncthreads();
@@ -1064,58 +1073,55 @@ k_p2p2(int64_t N, int K, double kappa, pb_expk8 ek, const pb_item* __restrict__ 
     const int64_t i1 = (g + 1) * PB_TG < N ? (g + 1) * PB_TG : N;
     const int32_t grpLo = (int32_t)(g * PB_TG * K), grpHi = (int32_t)(i1 * K);
 
-    int32_t r = item.r, a = item.a;
-    int32_t hi = p2p_hi[r];
+    // this item's share of the group's source list: `count` points from point `a` of range `r` on
+    int32_t a = item.a;
     int64_t remaining = item.count;
-    int rmask = p2p_mask[r];                          // which half of the group range r is for (k_lists)
-    auto next_tile = [&](int32_t& s0, int& cnt, int& mk) -> bool {
+    struct tile_t { int32_t s0; int cnt, mk; };
+    auto next_tile = [&](tile_t& tl, int buf) -> bool {   // the next tile, its copy started into buffer `buf` (thread 0)
         while (remaining > 0) {
-            if (a >= hi) { ++r; a = p2p_lo[r]; hi = p2p_hi[r]; rmask = p2p_mask[r]; continue; }
-            int64_t c = hi - a;
+            if (a >= rc.y) { ++r; rc = rn; rn = p2p_rng[r + 1]; a = rc.x; continue; }
+            int64_t c = rc.y - a;
             if (c > P2P_TILE) c = P2P_TILE;
             if (c > remaining) c = remaining;
-            s0 = a; cnt = (int)c; mk = rmask;
+            tl.s0 = a; tl.cnt = (int)c; tl.mk = rc.z;
+            if (tid == 0) {
+                pb_mbar_expect_tx(&bar[buf], (uint32_t)c * 64u);
+                pb_bulk_g2s(tiles + (size_t)buf * 2 * P2P_TILE, srec + 2 * (int64_t)a, (uint32_t)c * 64u, &bar[buf]);
+            }
             a += (int32_t)c; remaining -= c;
             return true;
         }
+        tl.cnt = 0;
         return false;
     };
 
     double o0[4] = {0, 0, 0, 0}, o1[4] = {0, 0, 0, 0};
-    int32_t cs0 = 0, ns0 = 0;
-    int ccnt = 0, ncnt = 0, cmk = 0, nmk = 0;
-    bool have = next_tile(cs0, ccnt, cmk);
-    if (have && tid == 0) {
-        pb_mbar_expect_tx(&bar[0], (uint32_t)ccnt * 64u);
-        pb_bulk_g2s(tile[0], srec + 2 * (int64_t)cs0, (uint32_t)ccnt * 64u, &bar[0]);
-    }
-    for (uint32_t it = 0; have; ++it) {
-        const int st = it & 1;
-        const bool more = next_tile(ns0, ncnt, nmk);
-        if (more && tid == 0) {                       // the other buffer was released by the barrier below
-            pb_mbar_expect_tx(&bar[st ^ 1], (uint32_t)ncnt * 64u);
-            pb_bulk_g2s(tile[st ^ 1], srec + 2 * (int64_t)ns0, (uint32_t)ncnt * 64u, &bar[st ^ 1]);
-        }
-        pb_mbar_wait(&bar[st], (it >> 1) & 1u);
-        const bool own = cs0 < grpHi && cs0 + ccnt > grpLo;   // the tile holds points of the group's own panels
-        if (cmk == 3) {
-            if (own) p2p_tile2<true>(tile[st], ccnt, sub, cs0, self0, self1, K, kappa, ek, Ts, t0, t1, o0, o1);
-            else p2p_tile2<false>(tile[st], ccnt, sub, cs0, self0, self1, K, kappa, ek, Ts, t0, t1, o0, o1);
-        } else if (cmk == 1) {
-            if (own) p2p_tile1<true>(tile[st], ccnt, sub, cs0, self0, K, kappa, ek, Ts, t0, o0);
-            else p2p_tile1<false>(tile[st], ccnt, sub, cs0, self0, K, kappa, ek, Ts, t0, o0);
+    static_assert(P2Q_NS == 3, "the tiles in flight are kept in three registers sets");
+    tile_t tc, tn, tnn;                                   // tile it, it + 1, it + 2
+    next_tile(tc, 0);
+    next_tile(tn, 1);
+    for (uint32_t it = 0; tc.cnt > 0; ++it) {
+        const int st = it % P2Q_NS;
+        next_tile(tnn, (it + 2) % P2Q_NS);                // its buffer held tile it - 1: released by the barrier below
+        pb_mbar_wait(&bar[st], (it / P2Q_NS) & 1u);
+        const double4* tile = tiles + (size_t)st * 2 * P2P_TILE;
+        const bool own = tc.s0 < grpHi && tc.s0 + tc.cnt > grpLo;   // the tile holds points of the group's own panels
+        if (tc.mk == 3) {
+            if (own) p2p_tile2<true>(tile, tc.cnt, sub, tc.s0, self0, self1, K, kappa, ek, Ts, t0, t1, o0, o1);
+            else p2p_tile2<false>(tile, tc.cnt, sub, tc.s0, self0, self1, K, kappa, ek, Ts, t0, t1, o0, o1);
+        } else if (tc.mk == 1) {
+            if (own) p2p_tile1<true>(tile, tc.cnt, sub, tc.s0, self0, K, kappa, ek, Ts, t0, o0);
+            else p2p_tile1<false>(tile, tc.cnt, sub, tc.s0, self0, K, kappa, ek, Ts, t0, o0);
         } else {
-            if (own) p2p_tile1<true>(tile[st], ccnt, sub, cs0, self1, K, kappa, ek, Ts, t1, o1);
-            else p2p_tile1<false>(tile[st], ccnt, sub, cs0, self1, K, kappa, ek, Ts, t1, o1);
+            if (own) p2p_tile1<true>(tile, tc.cnt, sub, tc.s0, self1, K, kappa, ek, Ts, t1, o1);
+            else p2p_tile1<false>(tile, tc.cnt, sub, tc.s0, self1, K, kappa, ek, Ts, t1, o1);
         }
         __syncthreads();
-        have = more;
-        cs0 = ns0;
-        ccnt = ncnt;
-        cmk = nmk;
+        tc = tn;
+        tn = tnn;
     }
     // add the warps' partial sums in a fixed order (tile[0] is free: every thread passed the last barrier)
-    double* red = reinterpret_cast<double*>(tile[0]);   // [P2Q_W][4][PB_TG] = 16 KB = tile[0]
+    double* red = reinterpret_cast<double*>(tiles);   // [P2Q_W][4][PB_TG] = 16 KB = tile[0]
 #pragma unroll
     for (int m = 0; m < 4; ++m) {
         red[(sub * 4 + m) * PB_TG + lane] = o0[m];
@@ -1420,9 +1426,14 @@ int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed, bool pre
             // two targets per lane pays once the kernel is throughput-bound (measured: C3 529 -> 516 us, C4 8.43 -> 8.24 ms;
             // C1 / C2, a few waves of short blocks, are 2-4 % faster with one target per thread and twice the resident warps)
             if (t.n_itemP_own > 0) {
-                if (t.N >= 30000)
-                    k_p2p2<<<(unsigned)t.n_itemP_own, P2P_THREADS, 0, st>>>(t.N, t.K, ctx->prm.kappa, t.ek8, t.itemP + t.itemP0, t.p2p_lo,
-                                                                          t.p2p_hi, t.p2p_mask, t.srec, t.pc[0], t.pc[1], t.pc[2], t.accP);
+                if (t.N >= 30000) {
+                    if (!ctx->attr_p2p_set) {     // per device and function: remembered per context
+                        PB_CUDA(cudaFuncSetAttribute(k_p2p2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P2Q_SMEM));
+                        ctx->attr_p2p_set = true;
+                    }
+                    k_p2p2<<<(unsigned)t.n_itemP_own, P2P_THREADS, P2Q_SMEM, st>>>(t.N, t.K, ctx->prm.kappa, t.ek8, t.itemP + t.itemP0, t.p2p_rng,
+                                                                                 t.srec, t.pc[0], t.pc[1], t.pc[2], t.accP);
+                }
                 else
                     k_p2p<<<(unsigned)t.n_itemP_own, P2P_THREADS, 0, st>>>(t.N, t.K, ctx->prm.kappa, t.ek8, t.itemP + t.itemP0, t.p2p_lo,
                                                                          t.p2p_hi, t.p2p_mask, t.srec, t.pc[0], t.pc[1], t.pc[2], t.accP);

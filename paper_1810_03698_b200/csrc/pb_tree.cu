@@ -463,6 +463,14 @@ __global__ void k_partition_low(int64_t G, const int32_t* __restrict__ off, cons
     }
 }
 
+__global__ void k_pack_ranges(int64_t n, const int32_t* __restrict__ lo, const int32_t* __restrict__ hi,
+                              const int8_t* __restrict__ mask, int4* __restrict__ out)
+{
+    int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (r >= n + 2) return;
+    out[r] = r < n ? make_int4(lo[r], hi[r], mask[r], 0) : make_int4(0, 0, 0, 0);   // two entries of padding: read ahead, never used
+}
+
 __global__ void k_m2p_centres(int64_t n, const int32_t* __restrict__ cell, const int8_t* __restrict__ code,
                               const double* __restrict__ cx, const double* __restrict__ cy, const double* __restrict__ cz,
                               double4* __restrict__ out)
@@ -910,6 +918,9 @@ int pb_tree_build_impl(pb_ctx* ctx)
     }
     PB_TRY(pb_cover_count(ctx, G, PB_TG, N, t.m2p_off, t.m2p_cell, t.p2p_off, t.p2p_lo, t.p2p_hi, &t.covered_pairs, nullptr, nullptr,
                           0, t.p2p_mask, t.m2p_code));
+    PB_TRY(pb_dalloc_t(ctx, &t.p2p_rng, tot_p + 2, CAT_TREE));
+    k_pack_ranges<<<pb_blocks(tot_p + 2, 256), 256, 0, st>>>(tot_p, t.p2p_lo, t.p2p_hi, t.p2p_mask, t.p2p_rng);
+    PB_LAUNCH_CHECK();
     PB_TRY(pb_dalloc_t(ctx, &t.m2p_ctr, tot_m > 0 ? tot_m : 1, CAT_TREE));
     if (tot_m > 0) {
         k_m2p_centres<<<pb_blocks(tot_m, 256), 256, 0, st>>>(tot_m, t.m2p_cell, m2p_low, t.c_ctr[0], t.c_ctr[1], t.c_ctr[2], t.m2p_ctr);
