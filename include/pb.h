@@ -329,6 +329,29 @@ int pb_fp64_peak_probe(pb_ctx* ctx, double* tflops_out /* HOST */);
  * percentage of SMs x 64 lanes x SM clock (D: section 7).  Synchronises. */
 int pb_fp64_pipe_probe(pb_ctx* ctx, int warps_per_sm, int ilp, int other_per_8, int other_kind, double* pct_out /* HOST */);
 
+/* ---- an entry point that allocates nothing -------------------------------------------------------------------------
+ * pb_multipole_field (Eq. (7), (14), (31), (32)) for callers that cannot allocate: code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc.  No context: every input and output is the caller's
+ * DEVICE array on `device` -- pos [na][3], q [na], dip [na][3], quad [na][6] (xx,xy,xz,yy,yz,zz), alpha [na], group [na]
+ * (int32), mu [na][3] or NULL, outputs phi [na], grad [na][3], hess [na][6] (each may be NULL) -- and the kernels run on
+ * `cuda_stream` (a cudaStream_t of that device, NULL = the default stream) without synchronising.  Same kernels, chunking
+ * and summation order as pb_multipole_field, hence the same bits.  The per-chunk partial sums live in a file-scope
+ * device array of the library (510 KB, held by every GPU that loads the library until the process exits) instead of an
+ * allocated scratch buffer; the call makes no cudaMalloc / cudaFree and calls no allocating routine (the array's device
+ * address is looked up once per device).  Limits and sharing: na <= 4,096 sites (pb_multipole_field_static_limit),
+ * more gives PB_ERR_INVALID_ARG with a message in pb_static_last_error(); ALL calls share the one array, which keeps the
+ * last call's contents (nothing needs to start at zero: every element read is written first in the same call), so two
+ * calls that may overlap on the GPU -- different streams without an ordering between them, or two processes' threads on
+ * one device through the same library instance -- race: order them. */
+int pb_multipole_field_static(int device, void* cuda_stream, int64_t na, const double* pos, const double* q,
+                              const double* dip, const double* quad, const double* alpha, const int32_t* group,
+                              const double* mu, double thole_a, double eps_in, int use_mask, double* phi, double* grad,
+                              double* hess);
+/* max_sites, scratch_bytes: HOST outputs (may be NULL) */
+int pb_multipole_field_static_limit(int64_t* max_sites, int64_t* scratch_bytes);
+/* message of the last failed pb_multipole_field_static call of this thread ("" if it succeeded) */
+const char* pb_static_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

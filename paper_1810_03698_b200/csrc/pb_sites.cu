@@ -3,6 +3,9 @@
 // and the Coulomb field of the multipoles with group mask and Thole damping Eq. (14), (31), (32)
 // (derivative tensors re-derived in D: App. A.2, A.5).
 #include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <mutex>
 #include "pb_internal.cuh"
 
 // ---- every site inside the surface (interior problem of Eq. (1); S: section 8(b)) ---------------------
@@ -663,4 +666,110 @@ extern "C" int pb_multipole_field(pb_ctx* ctx, const double* mu, int use_mask, d
     if (!ctx) return PB_ERR_INVALID_ARG;
     if (!ctx->sites.loaded) return pb_fail(ctx, PB_ERR_NOT_READY, "pb_multipole_field: call pb_sites_load first");
     return pb_multipole_field_impl(ctx, mu, 3, use_mask, phi, grad, hess);
+}
+
+// ---- pb_multipole_field_static: the H12 sum with NO allocation (include/pb.h) ------------------------------------------
+// For callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid it).  The same two kernels as
+// pb_multipole_field_impl -- k_multipole_field writes per-chunk partial sums, k_mfield_finish adds them in a fixed order --
+// with the partial sums in a file-scope device array instead of the context's scratch buffer.  Every GPU that loads the
+// library holds the array (PB_STATIC_MF_ROWS x 10 doubles = 510 KB) until the process exits.  All calls share it and it
+// keeps the last call's contents: every element k_mfield_finish reads is written by k_multipole_field in the same call,
+// so nothing has to start at zero; two calls that overlap on the GPU (different streams, no ordering) race on it.
+#define PB_STATIC_MF_MAX_SITES 4096
+// rows [chunk][site] of 10 doubles: n_chunk * na <= na + 148 * 8 * MF_ST + MF_ST with the chunking rule below
+#define PB_STATIC_MF_ROWS (PB_STATIC_MF_MAX_SITES + 148 * 8 * MF_ST + 64)
+static __device__ __align__(256) double g_mf_static_partial[(size_t)PB_STATIC_MF_ROWS * 10];
+
+#define PB_STATIC_MAX_DEVICES 64
+static double* g_mf_static_addr[PB_STATIC_MAX_DEVICES];        // device address of the array, per device (0 = not asked yet)
+static std::mutex g_mf_static_mutex;
+static thread_local char g_static_err[384] = {0};
+
+static int static_fail(int code, const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_static_err, sizeof(g_static_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+extern "C" const char* pb_static_last_error(void) { return g_static_err; }
+
+extern "C" int pb_multipole_field_static_limit(int64_t* max_sites, int64_t* scratch_bytes)
+{
+    if (max_sites) *max_sites = PB_STATIC_MF_MAX_SITES;
+    if (scratch_bytes) *scratch_bytes = (int64_t)sizeof(double) * PB_STATIC_MF_ROWS * 10;
+    return PB_OK;
+}
+
+extern "C" int pb_multipole_field_static(int device, void* cuda_stream, int64_t na, const double* pos, const double* q,
+                                         const double* dip, const double* quad, const double* alpha, const int32_t* group,
+                                         const double* mu, double thole_a, double eps_in, int use_mask, double* phi,
+                                         double* grad, double* hess)
+{
+    g_static_err[0] = 0;
+    if (device < 0 || device >= PB_STATIC_MAX_DEVICES)
+        return static_fail(PB_ERR_INVALID_ARG, "pb_multipole_field_static: device %d out of range [0, %d)", device, PB_STATIC_MAX_DEVICES);
+    if (na < 1 || na > PB_STATIC_MF_MAX_SITES)
+        return static_fail(PB_ERR_INVALID_ARG,
+                           "pb_multipole_field_static: %lld sites, the static scratch array holds at most %d "
+                           "(use pb_multipole_field, which allocates)", (long long)na, PB_STATIC_MF_MAX_SITES);
+    if (!pos || !q || !dip || !quad || !alpha || !group) return static_fail(PB_ERR_INVALID_ARG, "pb_multipole_field_static: NULL site array");
+    if (!(eps_in > 0.0) || !(thole_a >= 0.0)) return static_fail(PB_ERR_INVALID_ARG, "pb_multipole_field_static: eps_in > 0, thole_a >= 0 required");
+    const bool full = phi || hess;
+    if (!full && !grad) return PB_OK;
+#define PB_STATIC_CUDA(call)                                                                                          \
+    do {                                                                                                              \
+        cudaError_t e__ = (call);                                                                                     \
+        if (e__ != cudaSuccess) {                                                                                     \
+            if (prev != device) cudaSetDevice(prev);                                                                  \
+            return static_fail(PB_ERR_CUDA, "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e__));      \
+        }                                                                                                             \
+    } while (0)
+    int prev = device;
+    {
+        cudaError_t e0 = cudaGetDevice(&prev);
+        if (e0 != cudaSuccess) { prev = device; return static_fail(PB_ERR_CUDA, "cudaGetDevice: %s", cudaGetErrorString(e0)); }
+    }
+    if (prev != device) PB_STATIC_CUDA(cudaSetDevice(device));
+    // In host code the array's name is a host-side stand-in, not a device address: ask the runtime once per device,
+    // with that device current
+    double* partial = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_mf_static_mutex);
+        if (!g_mf_static_addr[device]) {
+            double* p = nullptr;
+            PB_STATIC_CUDA(cudaGetSymbolAddress((void**)&p, g_mf_static_partial));
+            g_mf_static_addr[device] = p;
+        }
+        partial = g_mf_static_addr[device];
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // the chunking of pb_multipole_field_impl (same summation order, so the same bits)
+    const int64_t ntile = (na + MF_ST - 1) / MF_ST;
+    int64_t nchunk = (148 * 8 + ntile - 1) / ntile;
+    const int64_t maxchunk = (na + MF_THREADS - 1) / MF_THREADS;
+    if (nchunk > maxchunk) nchunk = maxchunk;
+    if (nchunk < 1) nchunk = 1;
+    const int64_t chunk = (na + nchunk - 1) / nchunk;
+    nchunk = (na + chunk - 1) / chunk;
+    if (nchunk * na > PB_STATIC_MF_ROWS) {
+        if (prev != device) cudaSetDevice(prev);
+        return static_fail(PB_ERR_INVALID_ARG, "pb_multipole_field_static: internal: %lld x %lld partial rows exceed the array",
+                           (long long)nchunk, (long long)na);
+    }
+    dim3 grid((unsigned)nchunk, (unsigned)ntile);
+#define MF_LAUNCH(F, IN) \
+    k_multipole_field<F, true, IN><<<grid, MF_THREADS, 0, st>>>(na, chunk, pos, q, dip, quad, mu, alpha, group, thole_a, use_mask, partial)
+    if (full) { if (mu) MF_LAUNCH(true, true); else MF_LAUNCH(true, false); }
+    else { if (mu) MF_LAUNCH(false, true); else MF_LAUNCH(false, false); }
+#undef MF_LAUNCH
+    PB_STATIC_CUDA(cudaGetLastError());
+    k_mfield_finish<<<pb_blocks(na * (full ? 10 : 3), 128), 128, 0, st>>>(na, (int)nchunk, full ? 1 : 0, PB_INV4PI / eps_in, partial, phi,
+                                                                         grad, hess);
+    PB_STATIC_CUDA(cudaGetLastError());
+    if (prev != device) PB_STATIC_CUDA(cudaSetDevice(prev));
+#undef PB_STATIC_CUDA
+    return PB_OK;
 }

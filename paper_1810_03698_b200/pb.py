@@ -28,6 +28,7 @@ EXPORTS = [
     "pb_matvec_timed", "pb_matvec_host", "pb_reaction_field", "pb_multipole_field", "pb_gmres", "pb_solve",
     "pb_solve_host", "pb_get_stats", "pb_fp64_peak_probe", "pb_set_profiling", "pb_quadrature_rule",
     "pb_gauss_legendre", "pb_farfield_table", "pb_binding_cycle", "pb_set_shard", "pb_get_shard", "pb_shard_partition", "pb_set_stern", "pb_fp64_pipe_probe",
+    "pb_multipole_field_static", "pb_multipole_field_static_limit", "pb_static_last_error",
 ]
 
 
@@ -167,11 +168,40 @@ def lib():
         L.pb_set_shard.argtypes = [vp, ctypes.c_int, ctypes.c_int, _GATHER_T, vp]
         L.pb_get_shard.argtypes = [vp, ctypes.POINTER(i64)]
         L.pb_shard_partition.argtypes = [ctypes.POINTER(i64), i64, ctypes.c_int, ctypes.POINTER(i64)]
+        L.pb_multipole_field_static.argtypes = [ctypes.c_int, vp, i64, vp, vp, vp, vp, vp, vp, vp, dbl, dbl, ctypes.c_int, vp, vp, vp]
+        L.pb_multipole_field_static_limit.argtypes = [ctypes.POINTER(i64), ctypes.POINTER(i64)]
+        L.pb_static_last_error.argtypes = []
+        L.pb_static_last_error.restype = ctypes.c_char_p
         for name in EXPORTS:
-            if name not in ("pb_last_error", "pb_default_params"):
+            if name not in ("pb_last_error", "pb_default_params", "pb_static_last_error"):
                 getattr(L, name).restype = ctypes.c_int
         _lib = L
     return _lib
+
+
+def multipole_field_static_limit():
+    """(max sites, bytes of the static scratch array) of `multipole_field_static`."""
+    a, b = ctypes.c_int64(0), ctypes.c_int64(0)
+    lib().pb_multipole_field_static_limit(ctypes.byref(a), ctypes.byref(b))
+    return int(a.value), int(b.value)
+
+
+def multipole_field_static(pos, q, dip, quad, alpha, group, mu, thole_a, eps_in, use_mask, phi, grad, hess, stream=None):
+    """pb_multipole_field_static: the multipole field with no allocation.  Every array is the caller's CUDA tensor
+    (float64, group int32, contiguous); outputs are written in place (None = not wanted); runs on torch's current stream
+    unless `stream` is given.  Argument marshalling only: nothing is created here."""
+    import torch
+    na = int(pos.shape[0])
+    for t, dt in ((pos, torch.float64), (q, torch.float64), (dip, torch.float64), (quad, torch.float64), (alpha, torch.float64),
+                  (group, torch.int32), (mu, torch.float64), (phi, torch.float64), (grad, torch.float64), (hess, torch.float64)):
+        if t is not None and not (t.is_cuda and t.dtype == dt and t.is_contiguous() and t.device == pos.device):
+            raise PBError(-1, "multipole_field_static: arrays must be contiguous CUDA tensors of one device (float64; group int32)")
+    st = (stream if stream is not None else torch.cuda.current_stream(pos.device)).cuda_stream
+    rc = lib().pb_multipole_field_static(pos.device.index, ctypes.c_void_p(st), na, _ptr(pos), _ptr(q), _ptr(dip), _ptr(quad),
+                                         _ptr(alpha), _ptr(group), _ptr(mu), float(thole_a), float(eps_in), 1 if use_mask else 0,
+                                         _ptr(phi), _ptr(grad), _ptr(hess))
+    if rc != 0:
+        raise PBError(rc, lib().pb_static_last_error().decode())
 
 
 def binding_cycle(res_ab: dict, res_a: dict, res_b: dict) -> dict:
