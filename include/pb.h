@@ -101,6 +101,9 @@ typedef struct pb_params {
                                dipoles still change by a factor ~0.6 per step, so early systems need not be solved to
                                gmres_tol.  The loop only ends on a step whose system was solved to gmres_tol, and the
                                closing system is, too.  0 = every system to gmres_tol.  Default 0.03.               */
+    int32_t scf_store_mb;   /* scf_recycle = 2: device memory for the stored directions (u and A u, 2 x 16 N bytes per
+                               direction), in MiB; never more than half of the device's free memory.  When the store is
+                               full the rest of the loop's work goes to restarted GMRES.  Default 16384; 0 = no store. */
 } pb_params;
 
 /* Result of one polarizable solve (HOST struct). */

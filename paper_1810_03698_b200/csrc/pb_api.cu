@@ -102,6 +102,7 @@ extern "C" void pb_default_params(pb_params* p)
     p->rhs_treecode = 2;
     p->scf_recycle = 2;
     p->scf_eta = 0.03;
+    p->scf_store_mb = 16384;
     p->list_split = 1;
 }
 
@@ -188,13 +189,19 @@ extern "C" int pb_set_params(pb_ctx* ctx, const pb_params* p)
     if (p->rhs_treecode < 0 || p->rhs_treecode > 2) return pb_fail(ctx, PB_ERR_INVALID_ARG, "rhs_treecode must be 0, 1 or 2");
     if (p->scf_recycle < 0 || p->scf_recycle > 2) return pb_fail(ctx, PB_ERR_INVALID_ARG, "scf_recycle must be 0, 1 or 2");
     if (!(p->scf_eta >= 0.0 && p->scf_eta < 1.0)) return pb_fail(ctx, PB_ERR_INVALID_ARG, "0 <= scf_eta < 1 required");
+    if (p->scf_store_mb < 0) return pb_fail(ctx, PB_ERR_INVALID_ARG, "scf_store_mb >= 0 required");
     if (p->list_split < 0 || p->list_split > 1) return pb_fail(ctx, PB_ERR_INVALID_ARG, "list_split must be 0 or 1");
     const pb_params& o = ctx->prm;
     bool shape = o.kappa != p->kappa || o.theta != p->theta || o.order_P != p->order_P ||
                  o.ncrit != p->ncrit || o.K_far != p->K_far || o.K_near != p->K_near ||
                  o.near_tau != p->near_tau || o.nq_edge != p->nq_edge || o.eps_in != p->eps_in ||
                  o.eps_out != p->eps_out || o.list_split != p->list_split;
+    const bool store = o.scf_store_mb != p->scf_store_mb;       // the solver workspace is sized by it: rebuilt on the next solve
     ctx->prm = *p;
+    if (store && !(shape && ctx->tree.built)) {
+        pb_dfree_cat(ctx, CAT_SOLVE);
+        ctx->gws = pb_gmres_ws();
+    }
     if (shape && ctx->tree.built) {
         pb_dfree_cat(ctx, CAT_TREE);
         pb_dfree_cat(ctx, CAT_SITE_NEAR);

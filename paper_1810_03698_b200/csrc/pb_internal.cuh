@@ -116,7 +116,8 @@ struct pb_tree {
     int32_t* el_base = nullptr;   // [slices + 1]
     int32_t* el_col = nullptr;    // [el_entries] source panel (Morton); padding: the target itself
     double* el_val = nullptr;     // [4][el_entries] VL, KL, VY, KY corrections; padding: 0
-    double* el_tval = nullptr;    // [4][el_entries] the true near-zone entries (near-field preconditioner); padding: 0
+    float* el_tval = nullptr;     // [4][el_entries] the true near-zone entries, rounded to fp32: they only feed the near-field
+                                  // preconditioner, whose SpMV streams this table (half the bytes of fp64); padding: 0
     double* precond = nullptr;    // [N][4] inverse 2x2 diagonal blocks
     // partial accumulators
     // work items (one thread block each) and their accumulator slots

@@ -301,7 +301,8 @@ __global__ void k_axpy(int64_t n, double a, const double* __restrict__ x, double
 // alpha stays on the device (no host synchronisation); the iteration runs in Morton order, where the table lives.
 // M depends on v non-linearly (through alpha), hence the flexible variant of GMRES.  Measured on the oracle's dense
 // matrix of C2 (19,176 unknowns): 72 outer iterations with block-Jacobi alone, 42 with 2 inner steps, 40 with 3,
-// 28 with an exact sparse solve of A_n.
+// 28 with an exact sparse solve of A_n.  The table of A_n is kept in fp32 (half the bytes to stream per step): M only
+// has to be a good approximate inverse, the residuals of the outer iteration come from the fp64 operator.
 #define PB_NF_STEPS 2
 
 __global__ void k_nf_start(int64_t N, const int32_t* __restrict__ perm, const double* __restrict__ pc,
@@ -320,25 +321,25 @@ __global__ void k_nf_start(int64_t N, const int32_t* __restrict__ perm, const do
 // q = A_n p in Morton order; block = 32 targets (one ELL slice) x 4 kernels, as in k_combine
 __global__ void __launch_bounds__(128)
 k_nf_spmv(int64_t N, double eps_ratio, const int32_t* __restrict__ el_base, const int32_t* __restrict__ el_col,
-          const double* __restrict__ el_tval, int64_t ne, const double* __restrict__ p, double* __restrict__ q)
+          const float* __restrict__ el_tval, int64_t ne, const double* __restrict__ p, double* __restrict__ q)
 {
     __shared__ double sm[4][32];
     const int tgt = threadIdx.x & 31, m = threadIdx.x >> 5;
     const int64_t i = blockIdx.x * 32LL + tgt;
     const double* __restrict__ xv = (m & 1) ? p : p + N;          // V_L, V_Y act on dphi; K_L, K_Y on phi
     const int32_t b0 = el_base[blockIdx.x], width = (el_base[blockIdx.x + 1] - b0) / 32;
-    const double* __restrict__ val = el_tval + (int64_t)m * ne + b0 + tgt;
+    const float* __restrict__ val = el_tval + (int64_t)m * ne + b0 + tgt;
     const int32_t* __restrict__ col = el_col + b0 + tgt;
     double s = 0.0;
     int k = 0;
     for (; k + 4 <= width; k += 4) {
         double a[4], b[4];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) { a[u] = val[32 * (k + u)]; b[u] = xv[col[32 * (k + u)]]; }
+        for (int u = 0; u < 4; ++u) { a[u] = (double)val[32 * (k + u)]; b[u] = xv[col[32 * (k + u)]]; }
 #pragma unroll
         for (int u = 0; u < 4; ++u) s = fma(a[u], b[u], s);
     }
-    for (; k < width; ++k) s = fma(val[32 * k], xv[col[32 * k]], s);
+    for (; k < width; ++k) s = fma((double)val[32 * k], xv[col[32 * k]], s);
     sm[m][tgt] = s;
     __syncthreads();
     if (m == 0 && i < N) {
@@ -942,15 +943,22 @@ k_gcr_step(int64_t n, const double* __restrict__ d, double* __restrict__ c, doub
 
 static int gcr_alloc(pb_ctx* ctx, gmres_ws& ws)
 {
-    if (ws.GU || !ws.r) return PB_OK;
-    // room for a few hundred directions; at most 16 GB for the two bases (C4: 493 directions of 16.6 MB each)
-    size_t cap = ((size_t)16 << 30) / (2 * (size_t)ws.n * sizeof(double));
+    if (ws.gh || !ws.r) return PB_OK;
+    // room for a few hundred directions: pb_params.scf_store_mb, 16 GB by default (C4: 493 directions of 2 x 16.6 MB); with no
+    // room at all (cap 0) gcr_solve hands every system to restarted GMRES
+    size_t budget = (size_t)ctx->prm.scf_store_mb << 20;
+    {
+        size_t free_b = 0, total_b = 0;                 // never more than half of what the device has left
+        if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && free_b / 2 < budget) budget = free_b / 2;
+    }
+    size_t cap = budget / (2 * (size_t)ws.n * sizeof(double));
     if (cap > 1024) cap = 1024;
     if (cap > (size_t)ws.n) cap = (size_t)ws.n;
-    if (cap < 1) return PB_OK;
-    PB_TRY(pb_dalloc_t(ctx, &ws.GU, cap * ws.n, CAT_SOLVE));
-    PB_TRY(pb_dalloc_t(ctx, &ws.GC, cap * ws.n, CAT_SOLVE));
     PB_TRY(pb_dalloc_t(ctx, &ws.gh, cap + 16, CAT_SOLVE));
+    if (cap >= 1) {
+        PB_TRY(pb_dalloc_t(ctx, &ws.GU, cap * ws.n, CAT_SOLVE));
+        PB_TRY(pb_dalloc_t(ctx, &ws.GC, cap * ws.n, CAT_SOLVE));
+    }
     ws.gcap = (int)cap;
     ws.ngc = 0;
     return PB_OK;

@@ -48,6 +48,7 @@ class Params(ctypes.Structure):
         ("scf_omega", ctypes.c_double), ("scf_maxit", ctypes.c_int32), ("site_treecode", ctypes.c_int32),
         ("thole_a", ctypes.c_double), ("rhs_treecode", ctypes.c_int32), ("scf_recycle", ctypes.c_int32),
         ("list_split", ctypes.c_int32), ("scf_eta", ctypes.c_double),
+        ("scf_store_mb", ctypes.c_int32),
     ]
 
 

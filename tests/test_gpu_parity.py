@@ -364,7 +364,16 @@ def test_solve_c1_small_polarizable(pbm, po, torch_cuda):
         assert rel(mur.cpu().numpy(), ref["mu"]) <= 2e-6 and rel(xr.cpu().numpy(), ref["x"]) <= 1e-7, (rec, eta)
         dG[(rec, eta)] = rr["matvecs_total"]
     assert dG[(2, 0.03)] < dG[(1, 0.0)] < dG[(0, 0.0)], dG      # operator applications: fewer with every level of sharing
-    ctx.set_params(scf_recycle=2, scf_eta=0.0)
+    # a store too small for the loop (1 MiB = 25 directions of 2 x 20 KB here; the loop needs more): restarted GMRES takes
+    # over where the stored directions end, same fixed point
+    ctx.set_params(scf_recycle=2, scf_eta=0.03, scf_store_mb=1)
+    xr, mur, rr = ctx.solve()
+    assert rr["status"] == 0 and rr["matvecs_total"] > 25 and abs(rr["scf_iters"] - ref["scf_iters"]) <= 2
+    assert abs(rr["dG_solv"] - ref["dG_solv"]) <= 2e-8 * abs(ref["dG_solv"]) and rel(mur.cpu().numpy(), ref["mu"]) <= 2e-6
+    ctx.set_params(scf_store_mb=0)                             # no store at all
+    xr, mur, rr = ctx.solve()
+    assert rr["status"] == 0 and abs(rr["dG_solv"] - ref["dG_solv"]) <= 2e-8 * abs(ref["dG_solv"])
+    ctx.set_params(scf_recycle=2, scf_eta=0.0, scf_store_mb=16384)
     x, mu, res = ctx.solve()
     xh = torch_cuda.empty(2 * orc.nt, dtype=torch_cuda.float64).pin_memory()
     muh = torch_cuda.empty(sites.na, 3, dtype=torch_cuda.float64).pin_memory()
