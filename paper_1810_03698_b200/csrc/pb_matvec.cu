@@ -279,12 +279,19 @@ void pb_make_expk(double kappa, pb_expk* k)
 // parent's M2M, and so on upward -- nobody waits, and a parent is always formed from all its children
 // in child order, so the result does not depend on the arrival order.  A cell that appears in an M2P
 // list has its far-field terms F (D: section 6) written by the block that finishes it.
-#define P2M_CH 96     // <= UP_THREADS; 3 * 96 * 11 doubles of powers still fit under the M2M scratch at P = 6
+// Points staged per P2M chunk (<= UP_THREADS) and children per M2M round: small where the grid is many waves deep and the
+// number of resident blocks counts (a leaf holds 40 points on average at C4), large where the whole grid is resident at once
+// and the length of a block's own chain counts (C1, C2: 0.083 ms against 0.095 ms with the small values)
+#define P2M_CH_SMALL 48
+#define P2M_CH_LARGE 96
+#define M2M_Q_SMALL 4
+#define M2M_Q_LARGE 8
 #define P2M_LD (PB_MAX_P + 1)     // 11 doubles per point: odd stride, so a warp's reads of one point do not conflict
 #define UP_THREADS 128
 
 struct up_args {
     int P, Nk, NT, K;
+    int CH, MQ;      // P2M chunk, M2M round (see above)
     const int32_t *leaf_ids, *c_first, *c_last, *c_child, *c_nchild, *up_link;
     int32_t* up_count;
     const double *cx, *cy, *cz;
@@ -297,26 +304,32 @@ struct up_args {
     double2* FF;
 };
 
-static size_t up_smem_bytes(int Nk)
+static size_t up_smem_bytes(int Nk, int CH, int MQ)
 {
-    const size_t p2m = 3 * P2M_CH * P2M_LD + 3 * (size_t)Nk;
-    const size_t m2m = 40 * (size_t)Nk + 8 * 3 * P2M_LD;
-    return P2M_CH * sizeof(double4) + (2 * (size_t)Nk + (p2m > m2m ? p2m : m2m)) * sizeof(double);
+    const size_t p2m = 3 * (size_t)CH * P2M_LD + 3 * (size_t)Nk;
+    const size_t m2m = 5 * (size_t)MQ * (size_t)Nk + (size_t)MQ * 3 * P2M_LD;
+    return CH * sizeof(double4) + (2 * (size_t)Nk + (p2m > m2m ? p2m : m2m)) * sizeof(double);
 }
 
-__global__ void __launch_bounds__(UP_THREADS) k_upward(up_args a)
+// NR = moments per thread (ceil(N_k / 128): 1 up to P = 6, 2 up to P = 8, 3 for P = 9, 10).  The pass is bound by latency
+// and per-block overhead (one block per leaf), so what counts is the number of resident blocks: with NR = 1 the block
+// needs 64 registers per thread and 17.5 KB of shared memory (8 blocks per SM instead of 6 with the general form): C4
+// 2.94 -> 2.54 ms at P = 6, 8.09 -> 6.09 ms at P = 8.  (10 blocks at 48 registers: 2.48 ms at C4, slower at C3 -- the shared-memory
+// pipe is the next limit, ncu: l1tex 70 % busy.)
+template <int NR>
+__global__ void __launch_bounds__(UP_THREADS, NR == 1 ? 8 : (NR == 2 ? 6 : 4)) k_upward(up_args a)
 {
     extern __shared__ __align__(128) unsigned char up_raw[];
-    const int Nk = a.Nk, P = a.P, tid = threadIdx.x;
-    double4* wq = reinterpret_cast<double4*>(up_raw);          // [P2M_CH]
-    double* mom = reinterpret_cast<double*>(wq + P2M_CH);      // [2][Nk] finished moments of the current cell
+    const int Nk = a.Nk, P = a.P, tid = threadIdx.x, CH = a.CH, MQ = a.MQ;
+    double4* wq = reinterpret_cast<double4*>(up_raw);          // [CH]
+    double* mom = reinterpret_cast<double*>(wq + CH);      // [2][Nk] finished moments of the current cell
     double* U = mom + 2 * Nk;
-    double* pw = U;                                            // P2M: [3][P2M_CH][P2M_LD] powers of h
-    double* sk = pw + 3 * P2M_CH * P2M_LD;                     // P2M: [3][Nk] the S^x, S^y, S^z sets
-    double* cm = U;                                            // M2M: [8][2][Nk] children
-    double* part = cm + 16 * Nk;                               // M2M: [8][2][Nk] shifted children
-    double* tm = part + 16 * Nk;                               // M2M: [8][Nk] monomials of the shifts
-    double* tp = tm + 8 * Nk;                                  // M2M: [8][3][P2M_LD] powers of the shifts
+    double* pw = U;                                            // P2M: [3][CH][P2M_LD] powers of h
+    double* sk = pw + 3 * CH * P2M_LD;                     // P2M: [3][Nk] the S^x, S^y, S^z sets
+    double* cm = U;                                            // M2M: [MQ][2][Nk] children of one round
+    double* part = cm + 2 * MQ * Nk;                        // M2M: [MQ][2][Nk] shifted children
+    double* tm = part + 2 * MQ * Nk;                        // M2M: [MQ][Nk] monomials of the shifts
+    double* tp = tm + MQ * Nk;                              // M2M: [MQ][3][P2M_LD] powers of the shifts
     __shared__ int s_last;
 
     int64_t c = a.leaf_ids[blockIdx.x];
@@ -324,45 +337,45 @@ __global__ void __launch_bounds__(UP_THREADS) k_upward(up_args a)
     {   // ---- P2M: thread k (and k + 128, k + 256 at high order) sweeps the leaf's points
         const int64_t s0 = (int64_t)a.c_first[c] * a.K, s1 = (int64_t)a.c_last[c] * a.K;
         const double ycx = a.cx[c], ycy = a.cy[c], ycz = a.cz[c];
-        int ea[3], eb[3], ec[3];
+        int ea[NR], eb[NR], ec[NR];
 #pragma unroll
-        for (int r = 0; r < 3; ++r) {
+        for (int r = 0; r < NR; ++r) {
             const int k = tid + r * UP_THREADS;
             ea[r] = k < Nk ? c_ka[k] : 0; eb[r] = k < Nk ? c_kb[k] : 0; ec[r] = k < Nk ? c_kc[k] : 0;
         }
-        double acc[3][4];
+        double acc[NR][4];
 #pragma unroll
-        for (int r = 0; r < 3; ++r)
+        for (int r = 0; r < NR; ++r)
 #pragma unroll
             for (int m = 0; m < 4; ++m) acc[r][m] = 0.0;
         // thread p stages point p of a chunk (powers of its three coordinates, its four weights); the records of the
         // next chunk are already in flight while this one is accumulated
         double4 ra = make_double4(0, 0, 0, 0), rb = ra;
-        if (tid < P2M_CH && s0 + tid < s1) { ra = a.srec[2 * (s0 + tid)]; rb = a.srec[2 * (s0 + tid) + 1]; }
-        for (int64_t base = s0; base < s1; base += P2M_CH) {
-            const int np = (int)((s1 - base) < P2M_CH ? (s1 - base) : P2M_CH);
+        if (tid < CH && s0 + tid < s1) { ra = a.srec[2 * (s0 + tid)]; rb = a.srec[2 * (s0 + tid) + 1]; }
+        for (int64_t base = s0; base < s1; base += CH) {
+            const int np = (int)((s1 - base) < CH ? (s1 - base) : CH);
             __syncthreads();
             if (tid < np) {
                 const double hh[3] = {ra.x - ycx, ra.y - ycy, ra.z - ycz};
 #pragma unroll
                 for (int d = 0; d < 3; ++d) {
                     double pwr = 1.0;
-                    double* dst = pw + ((size_t)d * P2M_CH + tid) * P2M_LD;
+                    double* dst = pw + ((size_t)d * CH + tid) * P2M_LD;
                     for (int e = 0; e <= P; ++e) { dst[e] = pwr; pwr *= hh[d]; }
                 }
                 wq[tid] = make_double4(ra.w, rb.x, rb.y, rb.z);
             }
-            if (tid < P2M_CH && base + P2M_CH + tid < s1) {
-                ra = a.srec[2 * (base + P2M_CH + tid)];
-                rb = a.srec[2 * (base + P2M_CH + tid) + 1];
+            if (tid < CH && base + CH + tid < s1) {
+                ra = a.srec[2 * (base + CH + tid)];
+                rb = a.srec[2 * (base + CH + tid) + 1];
             }
             __syncthreads();
 #pragma unroll
-            for (int r = 0; r < 3; ++r) {
+            for (int r = 0; r < NR; ++r) {
                 if (tid + r * UP_THREADS < Nk) {
                     const double* px = pw + ea[r];
-                    const double* py = pw + (size_t)P2M_CH * P2M_LD + eb[r];
-                    const double* pz = pw + (size_t)2 * P2M_CH * P2M_LD + ec[r];
+                    const double* py = pw + (size_t)CH * P2M_LD + eb[r];
+                    const double* pz = pw + (size_t)2 * CH * P2M_LD + ec[r];
 #pragma unroll 4
                     for (int p = 0; p < np; ++p) {
                         const double mono = px[p * P2M_LD] * py[p * P2M_LD] * pz[p * P2M_LD];
@@ -377,7 +390,7 @@ __global__ void __launch_bounds__(UP_THREADS) k_upward(up_args a)
         }
         __syncthreads();
 #pragma unroll
-        for (int r = 0; r < 3; ++r) {
+        for (int r = 0; r < NR; ++r) {
             const int k = tid + r * UP_THREADS;
             if (k < Nk) { mom[k] = acc[r][0]; sk[k] = acc[r][1]; sk[Nk + k] = acc[r][2]; sk[2 * Nk + k] = acc[r][3]; }
         }
@@ -430,45 +443,49 @@ __global__ void __launch_bounds__(UP_THREADS) k_upward(up_args a)
         const int32_t ch = a.c_child[c];
         const int nc = a.c_nchild[c];
         link = a.up_link[c];                                   // the parent's own link word, in flight during its M2M
-        for (int k = tid; k < nc * 2 * Nk; k += UP_THREADS) cm[k] = __ldcg(a.M + (int64_t)ch * 2 * Nk + k);   // children are consecutive
-        if (tid < 3 * nc) {
-            const int q = tid / 3, d = tid - 3 * q;
-            const double* ctr = d == 0 ? a.cx : (d == 1 ? a.cy : a.cz);
-            const double tt = ctr[ch + q] - ctr[c];
-            double pwr = 1.0;
-            for (int e = 0; e <= P; ++e) { tp[(q * 3 + d) * P2M_LD + e] = pwr; pwr *= tt; }
-        }
-        __syncthreads();
-        for (int it = tid; it < Nk * nc; it += UP_THREADS) {   // monomials t^k of every child's shift
-            const int q = it / Nk, k = it - q * Nk;
-            const double* t3 = tp + q * 3 * P2M_LD;
-            tm[it] = t3[c_ka[k]] * t3[P2M_LD + c_kb[k]] * t3[2 * P2M_LD + c_kc[k]];
-        }
-        __syncthreads();
-        for (int it = tid; it < Nk * nc; it += UP_THREADS) {
-            const int q = it / Nk, k = __ldg(a.mm_off + Nk + 1 + (it - q * Nk));   // rows by falling length
-            const double* tq = tm + q * Nk;
-            const double* cq = cm + q * 2 * Nk;
-            double s0 = 0, s1 = 0;
-            const int e1 = __ldg(a.mm_off + k + 1);
-#pragma unroll 4
-            for (int e = __ldg(a.mm_off + k); e < e1; ++e) {
-                const int32_t ent = __ldg(a.mm_ent + e);
-                const double f = __ldg(a.mm_coef + e) * tq[ent >> 12];
-                const int l = ent & 0xfff;
-                s0 = fma(f, cq[l], s0);
-                s1 = fma(f, cq[Nk + l], s1);
+        // the children MQ at a time (they are consecutive); the parent is the sum over ALL of them in child order
+        for (int q0 = 0; q0 < nc; q0 += MQ) {
+            const int nq = nc - q0 < MQ ? nc - q0 : MQ;
+            for (int k = tid; k < nq * 2 * Nk; k += UP_THREADS) cm[k] = __ldcg(a.M + (int64_t)(ch + q0) * 2 * Nk + k);
+            if (tid < 3 * nq) {
+                const int q = tid / 3, d = tid - 3 * q;
+                const double* ctr = d == 0 ? a.cx : (d == 1 ? a.cy : a.cz);
+                const double tt = ctr[ch + q0 + q] - ctr[c];
+                double pwr = 1.0;
+                for (int e = 0; e <= P; ++e) { tp[(q * 3 + d) * P2M_LD + e] = pwr; pwr *= tt; }
             }
-            part[q * 2 * Nk + k] = s0;
-            part[q * 2 * Nk + Nk + k] = s1;
+            __syncthreads();
+            for (int it = tid; it < Nk * nq; it += UP_THREADS) {   // monomials t^k of every child's shift
+                const int q = it / Nk, k = it - q * Nk;
+                const double* t3 = tp + q * 3 * P2M_LD;
+                tm[it] = t3[c_ka[k]] * t3[P2M_LD + c_kb[k]] * t3[2 * P2M_LD + c_kc[k]];
+            }
+            __syncthreads();
+            for (int it = tid; it < Nk * nq; it += UP_THREADS) {
+                const int q = it / Nk, k = __ldg(a.mm_off + Nk + 1 + (it - q * Nk));   // rows by falling length
+                const double* tq = tm + q * Nk;
+                const double* cq = cm + q * 2 * Nk;
+                double s0 = 0, s1 = 0;
+                const int e1 = __ldg(a.mm_off + k + 1);
+#pragma unroll 4
+                for (int e = __ldg(a.mm_off + k); e < e1; ++e) {
+                    const int32_t ent = __ldg(a.mm_ent + e);
+                    const double f = __ldg(a.mm_coef + e) * tq[ent >> 12];
+                    const int l = ent & 0xfff;
+                    s0 = fma(f, cq[l], s0);
+                    s1 = fma(f, cq[Nk + l], s1);
+                }
+                part[q * 2 * Nk + k] = s0;
+                part[q * 2 * Nk + Nk + k] = s1;
+            }
+            __syncthreads();
+            for (int k = tid; k < 2 * Nk; k += UP_THREADS) {
+                double v = q0 ? mom[k] : 0.0;
+                for (int q = 0; q < nq; ++q) v += part[q * 2 * Nk + k];
+                mom[k] = v;
+            }
+            __syncthreads();
         }
-        __syncthreads();
-        for (int k = tid; k < 2 * Nk; k += UP_THREADS) {
-            double v = 0;
-            for (int q = 0; q < nc; ++q) v += part[q * 2 * Nk + k];
-            mom[k] = v;
-        }
-        __syncthreads();
     }
 }
 
@@ -1306,12 +1323,20 @@ int pb_upward(pb_ctx* ctx, cudaStream_t fs, const int32_t* leaf_ids, int64_t n_l
     ua.mm_off = t.mm_off; ua.mm_ent = t.mm_ent; ua.mm_coef = t.mm_coef;
     ua.cv_off = t.cv_off; ua.cv_idx = t.cv_idx; ua.cv_coef = t.cv_coef;
     ua.M = t.M; ua.FF = t.FF;
-    const size_t sm = up_smem_bytes(t.Nk);
+    const int nr = (t.Nk + UP_THREADS - 1) / UP_THREADS;
+    const bool deep = n_leaf >= 148 * 8 * 2;          // more than two waves of blocks even at the highest occupancy
+    ua.CH = deep ? P2M_CH_SMALL : P2M_CH_LARGE;
+    ua.MQ = deep ? M2M_Q_SMALL : M2M_Q_LARGE;
+    const size_t sm = up_smem_bytes(t.Nk, ua.CH, ua.MQ);
     if (sm > 48 * 1024 && sm > ctx->attr_up_bytes) {   // per device: remembered per context
-        PB_CUDA(cudaFuncSetAttribute(k_upward, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+        PB_CUDA(cudaFuncSetAttribute(k_upward<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+        PB_CUDA(cudaFuncSetAttribute(k_upward<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+        PB_CUDA(cudaFuncSetAttribute(k_upward<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
         ctx->attr_up_bytes = sm;
     }
-    k_upward<<<(unsigned)n_leaf, UP_THREADS, sm, fs>>>(ua);
+    if (nr == 1) k_upward<1><<<(unsigned)n_leaf, UP_THREADS, sm, fs>>>(ua);
+    else if (nr == 2) k_upward<2><<<(unsigned)n_leaf, UP_THREADS, sm, fs>>>(ua);
+    else k_upward<3><<<(unsigned)n_leaf, UP_THREADS, sm, fs>>>(ua);
     PB_LAUNCH_CHECK();
     return PB_OK;
 }
