@@ -879,11 +879,16 @@ static int recycle_append(pb_ctx* ctx, gmres_ws& ws, const double* x)
 // application per new direction.  When the store is full the remaining work goes to restarted GMRES.
 __global__ void __launch_bounds__(256)
 k_gcr_orth(int64_t n, int nv, const double* __restrict__ C, const double* __restrict__ U, int64_t ld,
-           const double* __restrict__ h, double* __restrict__ c, double* __restrict__ u)
+           const double* __restrict__ h, double* __restrict__ c, double* __restrict__ u, double* __restrict__ h2_out)
 {
     extern __shared__ double sh[];
     for (int j = threadIdx.x; j < nv; j += blockDim.x) sh[j] = h[j];
     __syncthreads();
+    if (h2_out && blockIdx.x == 0 && threadIdx.x == 0) {   // |h|^2: how much of c this pass removes (fixed order)
+        double h2 = 0;
+        for (int j = 0; j < nv; ++j) h2 = fma(sh[j], sh[j], h2);
+        *h2_out = h2;
+    }
     for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
         double ac = c[e], au = u[e];
         int j = 0;
@@ -988,13 +993,14 @@ static int gcr_solve(pb_ctx* ctx, const double* b, double* x, double tol_factor,
     PB_TRY(gcr_alloc(ctx, ws));
     const int tb = 256;
     const int nb = pb_blocks(n, tb) < 2368 ? pb_blocks(n, tb) : 2368;
-    double* dsc = ws.gh + ws.gcap;                       // device scalars: [0] b.b, [1] r.r, [2] r.c, [3] c.c
+    double* dsc = ws.gh + ws.gcap;                       // device scalars: [0] b.b, [1] r.r, [2] r.c, [3] c.c, [4] |h|^2 of the first Gram-Schmidt pass
     int iters = 0, matvecs = 0;
     k_residual<<<pb_blocks(n, tb), tb, 0, st>>>(n, b, ws.ax, ws.r);
     PB_LAUNCH_CHECK();
     PB_TRY(dot_into(ctx, ws, 0, nullptr, b, true, dsc));
     PB_TRY(dot_into(ctx, ws, 0, nullptr, ws.r, true, dsc + 1));
-    double h[4];
+    double h[5] = {0, 0, 0, 0, 0};
+    bool two_pass = false;
     PB_CUDA(cudaMemcpyAsync(h, dsc, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
     PB_CUDA(cudaStreamSynchronize(st));
     const double bnorm = sqrt(h[0]);
@@ -1050,22 +1056,30 @@ static int gcr_solve(pb_ctx* ctx, const double* b, double* x, double tol_factor,
             PB_CUDA(cudaMemcpyAsync(u, ws.r, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
         PB_TRY(pb_matvec_impl(ctx, u, c, false, false));
         ++matvecs;
-        for (int pass = 0; pass < 2 && ws.ngc > 0; ++pass) {
+        // Classical Gram-Schmidt against the stored pairs.  One pass leaves |C^T c| / |c| of the order of
+        // eps |c before| / |c after| (the cancellation is what costs orthogonality; Daniel / Gragg / Kaufman / Stewart), and the
+        // process needs orthogonality far below gmres_tol, not to rounding: a second pass only while the first one takes
+        // c down by more than 10^4 in norm, judged from the previous direction.  Measured at C4: the first pass removes
+        // between a fifth and most of |c|^2, the second changes neither iteration counts nor residuals in 9 digits and costs
+        // 0.19 s of a 5.25 s solve.  x, A x and r stay consistent whatever the orthogonality: c = A u holds by linearity.
+        const int npass = ws.ngc > 0 ? (two_pass ? 2 : 1) : 0;
+        for (int pass = 0; pass < npass; ++pass) {
             PB_TRY(gcr_dots(ctx, ws, ws.ngc, c));
-            k_gcr_orth<<<nb, tb, ws.ngc * sizeof(double), st>>>(n, ws.ngc, ws.GC, ws.GU, n, ws.gh, c, u);
+            k_gcr_orth<<<nb, tb, ws.ngc * sizeof(double), st>>>(n, ws.ngc, ws.GC, ws.GU, n, ws.gh, c, u, pass == 0 ? dsc + 4 : nullptr);
             PB_LAUNCH_CHECK();
         }
         PB_TRY(dot_into(ctx, ws, 1, ws.r, c, true, dsc + 2));              // r . c and c . c
         k_gcr_step<<<nb, tb, 0, st>>>(n, dsc + 2, c, u, x, ws.ax, ws.r);
         PB_LAUNCH_CHECK();
         PB_TRY(dot_into(ctx, ws, 0, nullptr, ws.r, true, dsc + 1));
-        PB_CUDA(cudaMemcpyAsync(h, dsc, 4 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        PB_CUDA(cudaMemcpyAsync(h, dsc, 5 * sizeof(double), cudaMemcpyDeviceToHost, st));
         PB_CUDA(cudaStreamSynchronize(st));
         ++iters;
         if (!(h[3] > 0.0)) {                            // A M(r) lies in the stored space: nothing new to add (singular operator)
             rc = pb_fail(ctx, PB_ERR_NO_CONVERGENCE, "GCR: breakdown at relative residual %.3e", relres);
             break;
         }
+        two_pass = npass > 0 && h[4] > 1e8 * h[3];
         ++ws.ngc;
         relres = sqrt(h[1]) / bnorm;
     }
