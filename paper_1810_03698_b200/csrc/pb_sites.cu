@@ -515,8 +515,8 @@ __device__ __forceinline__ void mf_pair(double dx, double dy, double dz, bool ma
     if (IND) {
         double l3 = 1.0, l5 = 1.0, l7 = 1.0;
         const double ia = ia_l * ia_m;                      // 1/sqrt(alpha_l alpha_m), 0 when either is 0
-        if (ia > 0.0) {
-            const double au3 = thole_a * r2 * (r2 * i1) * ia;
+        const double au3 = thole_a * r2 * (r2 * i1) * ia;
+        if (ia > 0.0 && au3 < 40.0) {                       // beyond: e^{-au3} < 4.3e-18, the damping factors are 1 to rounding
             const double E = exp(-au3);
             l3 = 1.0 - E;
             l5 = 1.0 - (1.0 + au3) * E;
