@@ -382,6 +382,32 @@ def test_solve_c1_small_polarizable(pbm, po, torch_cuda):
     ctx.close()
 
 
+def test_iteration_limits_are_reported_not_hidden(pbm, po, torch_cuda):
+    """PB_ERR_NO_CONVERGENCE (results still set, include/pb.h): a GMRES / GCR limit too small for the first system and an
+    SCF limit too small for the loop, in each of the three ways the loop's systems share work."""
+    from paper_1810_03698_b200.workloads import make_config
+    w = make_config("C1", subdiv=3)
+    ok = pbm.from_workload(w)
+    ok.tree_build()
+    _, _, good = ok.solve()
+    ok.close()
+    assert good["status"] == 0 and good["scf_iters"] > 5
+    for rec in (0, 1, 2):
+        ctx = pbm.from_workload(w, gmres_maxit=2, scf_recycle=rec, scf_maxit=4)
+        ctx.tree_build()
+        x, mu, res = ctx.solve()
+        assert res["status"] == -6 and res["final_gmres_relres"] > 1e-6, (rec, res)
+        assert bool(torch_cuda.isfinite(x).all()) and bool(torch_cuda.isfinite(mu).all()) and np.isfinite(res["dG_solv"])
+        ctx.close()
+        ctx = pbm.from_workload(w, scf_recycle=rec, scf_maxit=3)
+        ctx.tree_build()
+        x, mu, res = ctx.solve()
+        assert res["status"] == -6 and res["scf_iters"] == 3 and res["final_scf_delta_debye"] > 1e-7, (rec, res)
+        assert res["final_gmres_relres"] <= 1e-6 or rec == 2        # (mode 2 solves early systems inexactly on purpose)
+        assert abs(res["dG_solv"] - good["dG_solv"]) <= 0.05 * abs(good["dG_solv"])
+        ctx.close()
+
+
 # ---- boundary behaviour ------------------------------------------------------------------------------
 def test_error_codes_and_call_order(pbm, torch_cuda):
     from paper_1810_03698_b200.workloads import icosphere
