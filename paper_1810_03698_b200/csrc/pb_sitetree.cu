@@ -158,19 +158,23 @@ __host__ __device__ static constexpr int sg_nt(int P)
 template <int P> struct sg_cfg {
     static constexpr int NT = sg_nt(P);
     static constexpr size_t FF_BYTES0 = (size_t)SG_W * SG_NS * NT * sizeof(double2);
-    static constexpr size_t RED_BYTES = (size_t)SG_W * 4 * ST_GROUP * sizeof(double);
+    static constexpr size_t RED_BYTES = (size_t)SG_W * 10 * ST_GROUP * sizeof(double);
     static constexpr size_t FF_BYTES = FF_BYTES0 > RED_BYTES ? FF_BYTES0 : RED_BYTES;
     static constexpr size_t SMEM = FF_BYTES + SG_W * SG_NS * sizeof(uint64_t);
 };
 
-template <int P>
-__global__ void __launch_bounds__(SG_THREADS)
+// HESS: also the Hessian (the solve's closing call, Eq. 21/24), by differentiating once more:
+//     d_i d_j phi = sum_m [ u_m H_m,ij - u_{m+1} (d_i G_m,j + d_j G_m,i + delta_ij W_m) + u_{m+2} d_i d_j W_m ],
+// H_m,ij = sum_{|alpha|+j=m} d_i d_j (d^alpha) F, in a second sweep over the cell's terms (six more FMA per term; orders
+// P <= 6).
+template <int P, bool HESS>
+__global__ void __launch_bounds__(SG_THREADS, 1)
 k_site_grad(int64_t na, const double* __restrict__ sx, const double* __restrict__ sy, const double* __restrict__ sz,
             const int32_t* __restrict__ m2p_off, const int32_t* __restrict__ m2p_cell, const double* __restrict__ cx,
             const double* __restrict__ cy, const double* __restrict__ cz, const double2* __restrict__ FF,
-            double* __restrict__ out /*[na][10]: phi, grad (Morton order of the sites), without the 1/(4 pi)*/)
+            double* __restrict__ out /*[na][10]: phi, grad, hess (Morton order of the sites), without the 1/(4 pi)*/)
 {
-    constexpr int NT = sg_cfg<P>::NT, NS = SG_NS;
+    constexpr int NT = sg_cfg<P>::NT, NS = SG_NS, NO = HESS ? 10 : 4;
     extern __shared__ __align__(128) unsigned char sgraw[];
     const int tid = threadIdx.x, lane = tid & 31, sub = tid >> 5;
     double2* ffw = reinterpret_cast<double2*>(sgraw) + (size_t)sub * NS * NT;
@@ -197,7 +201,9 @@ k_site_grad(int64_t na, const double* __restrict__ sx, const double* __restrict_
     int32_t idn = NS - 1 < nw ? m2p_cell[e0 + SG_W * (NS - 1)] : 0;
     int32_t cn = nw > 0 ? m2p_cell[e0] : 0;
     double cxn = cx[cn], cyn = cy[cn], czn = cz[cn];
-    double o0 = 0.0, o1 = 0.0, o2 = 0.0, o3 = 0.0;
+    double o[NO];
+#pragma unroll
+    for (int q = 0; q < NO; ++q) o[q] = 0.0;
 #pragma unroll 1
     for (int k = 0; k < nw; ++k) {
         const int kn = k + NS - 1;
@@ -210,10 +216,14 @@ k_site_grad(int64_t na, const double* __restrict__ sx, const double* __restrict_
         }
         pb_mbar_wait(&fullw[k % NS], (uint32_t)((k / NS) & 1));
         const double2* ff = ffw + (size_t)(k % NS) * NT;
-        double W[P + 1], GX[P + 1], GY[P + 1], GZ[P + 1];
+        const double R2 = dx * dx + dy * dy + dz * dz;
+        const double ri = pb_rsqrt(R2), ri2 = ri * ri;
+        double sp = 0.0, sgx = 0.0, sgy = 0.0, sgz = 0.0, sw1 = 0.0;
+        double sw2 = 0.0, g1x = 0.0, g1y = 0.0, g1z = 0.0, sh[6] = {0, 0, 0, 0, 0, 0};
+        {   // first sweep over the cell's terms: W_m and G_m, then their radial sums
+            double W[P + 1], GX[P + 1], GY[P + 1], GZ[P + 1];
 #pragma unroll
-        for (int m = 0; m <= P; ++m) { W[m] = 0.0; GX[m] = 0.0; GY[m] = 0.0; GZ[m] = 0.0; }
-        {
+            for (int m = 0; m <= P; ++m) { W[m] = 0.0; GX[m] = 0.0; GY[m] = 0.0; GZ[m] = 0.0; }
             int e = 0;
             double X = 1.0, X1 = 0.0;                  // x^a and a x^(a-1)
 #pragma unroll
@@ -246,53 +256,119 @@ k_site_grad(int64_t na, const double* __restrict__ sx, const double* __restrict_
                 X1 = (double)(a + 1) * X;
                 X *= dx;
             }
-        }
-        const double R2 = dx * dx + dy * dy + dz * dz;
-        const double ri = pb_rsqrt(R2), ri2 = ri * ri;
-        double u = ri, sp = 0.0, sgx = 0.0, sgy = 0.0, sgz = 0.0, sw1 = 0.0;
+            double u = ri;
 #pragma unroll
-        for (int m = 0; m <= P; ++m) {
-            const double un = (2 * m + 1) * u * ri2;           // u_{m+1}
-            sp = fma(u, W[m], sp);
-            sgx = fma(u, GX[m], sgx);
-            sgy = fma(u, GY[m], sgy);
-            sgz = fma(u, GZ[m], sgz);
-            sw1 = fma(un, W[m], sw1);
-            u = un;
+            for (int m = 0; m <= P; ++m) {
+                const double un = (2 * m + 1) * u * ri2;           // u_{m+1}
+                sp = fma(u, W[m], sp);
+                sgx = fma(u, GX[m], sgx);
+                sgy = fma(u, GY[m], sgy);
+                sgz = fma(u, GZ[m], sgz);
+                sw1 = fma(un, W[m], sw1);
+                if (HESS) {
+                    const double unn = (2 * m + 3) * un * ri2;     // u_{m+2}
+                    sw2 = fma(unn, W[m], sw2);
+                    g1x = fma(un, GX[m], g1x);
+                    g1y = fma(un, GY[m], g1y);
+                    g1z = fma(un, GZ[m], g1z);
+                }
+                u = un;
+            }
         }
-        o0 += sp;
-        o1 += sgx - dx * sw1;
-        o2 += sgy - dy * sw1;
-        o3 += sgz - dz * sw1;
+        if (HESS) {   // second sweep: H_m,ij (six sums per layer; terms of total degree < 2 do not contribute)
+            double HXX[P + 1], HXY[P + 1], HXZ[P + 1], HYY[P + 1], HYZ[P + 1], HZZ[P + 1];
+#pragma unroll
+            for (int m = 0; m <= P; ++m) { HXX[m] = 0.0; HXY[m] = 0.0; HXZ[m] = 0.0; HYY[m] = 0.0; HYZ[m] = 0.0; HZZ[m] = 0.0; }
+            int e = 0;
+            double X = 1.0, X1 = 0.0, X2 = 0.0;        // x^a, a x^(a-1), a (a-1) x^(a-2)
+#pragma unroll
+            for (int a = 0; a <= P; ++a) {
+                double Y = 1.0, Y1 = 0.0, Y2 = 0.0;
+#pragma unroll
+                for (int b = 0; b <= P - a; ++b) {
+                    const double XY = X * Y, X1Y = X1 * Y, XY1 = X * Y1, X2Y = X2 * Y, XY2 = X * Y2, X1Y1 = X1 * Y1;
+                    double Z = 1.0, Z1 = 0.0, Z2 = 0.0;
+#pragma unroll
+                    for (int c = 0; c <= P - a - b; ++c) {
+                        const int n = a + b + c;
+                        const double hxx = X2Y * Z, hxy = X1Y1 * Z, hxz = X1Y * Z1, hyy = XY2 * Z, hyz = XY1 * Z1, hzz = XY * Z2;
+#pragma unroll
+                        for (int j = 0; j <= (P - n) / 2; ++j) {
+                            if (n >= 2) {
+                                const double2 f2 = ff[e];
+                                const double f = f2.x - f2.y;
+                                if (a > 1) HXX[n + j] = fma(hxx, f, HXX[n + j]);
+                                if (a > 0 && b > 0) HXY[n + j] = fma(hxy, f, HXY[n + j]);
+                                if (a > 0 && c > 0) HXZ[n + j] = fma(hxz, f, HXZ[n + j]);
+                                if (b > 1) HYY[n + j] = fma(hyy, f, HYY[n + j]);
+                                if (b > 0 && c > 0) HYZ[n + j] = fma(hyz, f, HYZ[n + j]);
+                                if (c > 1) HZZ[n + j] = fma(hzz, f, HZZ[n + j]);
+                            }
+                            ++e;
+                        }
+                        Z2 = (double)(c + 1) * Z1;
+                        Z1 = (double)(c + 1) * Z;
+                        Z *= dz;
+                    }
+                    Y2 = (double)(b + 1) * Y1;
+                    Y1 = (double)(b + 1) * Y;
+                    Y *= dy;
+                }
+                X2 = (double)(a + 1) * X1;
+                X1 = (double)(a + 1) * X;
+                X *= dx;
+            }
+            double u = ri;
+#pragma unroll
+            for (int m = 0; m <= P; ++m) {
+                sh[0] = fma(u, HXX[m], sh[0]);
+                sh[1] = fma(u, HXY[m], sh[1]);
+                sh[2] = fma(u, HXZ[m], sh[2]);
+                sh[3] = fma(u, HYY[m], sh[3]);
+                sh[4] = fma(u, HYZ[m], sh[4]);
+                sh[5] = fma(u, HZZ[m], sh[5]);
+                u = (2 * m + 1) * u * ri2;
+            }
+        }
+        o[0] += sp;
+        o[1] += sgx - dx * sw1;
+        o[2] += sgy - dy * sw1;
+        o[3] += sgz - dz * sw1;
+        if (HESS) {                                            // xx, xy, xz, yy, yz, zz
+            o[4] += sh[0] - 2.0 * dx * g1x - sw1 + dx * dx * sw2;
+            o[5] += sh[1] - (dx * g1y + dy * g1x) + dx * dy * sw2;
+            o[6] += sh[2] - (dx * g1z + dz * g1x) + dx * dz * sw2;
+            o[7] += sh[3] - 2.0 * dy * g1y - sw1 + dy * dy * sw2;
+            o[8] += sh[4] - (dy * g1z + dz * g1y) + dy * dz * sw2;
+            o[9] += sh[5] - 2.0 * dz * g1z - sw1 + dz * dz * sw2;
+        }
         __syncwarp();
     }
     __syncthreads();
-    double* red = reinterpret_cast<double*>(sgraw);    // [SG_W][4][ST_GROUP]: the warps' sums, added in warp order
-    red[(sub * 4 + 0) * ST_GROUP + lane] = o0;
-    red[(sub * 4 + 1) * ST_GROUP + lane] = o1;
-    red[(sub * 4 + 2) * ST_GROUP + lane] = o2;
-    red[(sub * 4 + 3) * ST_GROUP + lane] = o3;
+    double* red = reinterpret_cast<double*>(sgraw);    // [SG_W][NO][ST_GROUP]: the warps' sums, added in warp order
+#pragma unroll
+    for (int q = 0; q < NO; ++q) red[(sub * NO + q) * ST_GROUP + lane] = o[q];
     __syncthreads();
-    if (tid < 4 * ST_GROUP) {
-        const int m = tid / ST_GROUP, l = tid % ST_GROUP;
+    for (int t = tid; t < NO * ST_GROUP; t += SG_THREADS) {
+        const int m = t / ST_GROUP, l = t % ST_GROUP;
         const int64_t ii = g * ST_GROUP + l;
         if (ii < na) {
             double v = 0;
 #pragma unroll
-            for (int q = 0; q < SG_W; ++q) v += red[(q * 4 + m) * ST_GROUP + l];
+            for (int q = 0; q < SG_W; ++q) v += red[(q * NO + m) * ST_GROUP + l];
             out[ii * 10 + m] = v;
         }
     }
 }
 
-template <int P>
+template <int P, bool HESS>
 static cudaError_t launch_site_grad(pb_ctx* ctx, double* farp)
 {
     pb_tree& t = ctx->tree;
     pb_sites& s = ctx->sites;
-    cudaError_t e = cudaFuncSetAttribute(k_site_grad<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sg_cfg<P>::SMEM);
+    cudaError_t e = cudaFuncSetAttribute(k_site_grad<P, HESS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sg_cfg<P>::SMEM);
     if (e != cudaSuccess) return e;
-    k_site_grad<P><<<(unsigned)s.t_groups, SG_THREADS, sg_cfg<P>::SMEM, ctx->stream>>>(
+    k_site_grad<P, HESS><<<(unsigned)s.t_groups, SG_THREADS, sg_cfg<P>::SMEM, ctx->stream>>>(
         s.na, s.tpos[0], s.tpos[1], s.tpos[2], s.t_m2p_off, s.t_m2p_cell, t.c_ctr[0], t.c_ctr[1], t.c_ctr[2], t.FF, farp);
     return cudaSuccess;
 }
@@ -423,35 +499,50 @@ int pb_reaction_field_tree(pb_ctx* ctx, double* phi, double* grad, double* hess)
         sm_set[H ? 1 : 0] = sm;
     }
     const unsigned G = (unsigned)s.t_groups;
-    if (H) {
+    if (H && t.P > 6) {
+        // orders 7, 8: the radial form's 10 (P + 1) partial sums per cell do not fit the register file; the coefficient
+        // recurrence (k_site_m2p) differentiates the same truncated sum
         k_site_m2p<10><<<dim3(G, ST_SPLIT), ST_GROUP, sm, st>>>(s.na, t.P, s.tpos[0], s.tpos[1], s.tpos[2], s.t_m2p_off, s.t_m2p_cell, t.c_ctr[0],
                                                t.c_ctr[1], t.c_ctr[2], t.M, s.nb_idx, s.dv_idx, s.dv_fac, farp);
         PB_LAUNCH_CHECK();
-        k_site_p2p<true><<<G * (ST_GROUP / SP_ST), SP_THREADS, 0, st>>>(s.na, s.tpos[0], s.tpos[1], s.tpos[2], s.t_p2p_off,
-                                                                        s.t_p2p_lo, s.t_p2p_hi, t.srec, nearp);
-        PB_LAUNCH_CHECK();
     } else {
-        // potential and gradient (the SCF loop): radial form, one slab of far-field sums; the other slabs are zero
+        // radial form, one slab of far-field sums; the other slabs are zero
         PB_CUDA(cudaMemsetAsync(farp + (size_t)s.na * 10, 0, (size_t)(ST_SPLIT - 1) * s.na * 10 * sizeof(double), st));
         cudaError_t e = cudaSuccess;
-        switch (t.P) {
-        case 0: e = launch_site_grad<0>(ctx, farp); break;
-        case 1: e = launch_site_grad<1>(ctx, farp); break;
-        case 2: e = launch_site_grad<2>(ctx, farp); break;
-        case 3: e = launch_site_grad<3>(ctx, farp); break;
-        case 4: e = launch_site_grad<4>(ctx, farp); break;
-        case 5: e = launch_site_grad<5>(ctx, farp); break;
-        case 6: e = launch_site_grad<6>(ctx, farp); break;
-        case 7: e = launch_site_grad<7>(ctx, farp); break;
-        case 8: e = launch_site_grad<8>(ctx, farp); break;
-        default: return pb_fail(ctx, PB_ERR_INVALID_ARG, "internal: site treecode needs order_P <= 8");
+        if (H) {
+            switch (t.P) {
+            case 0: e = launch_site_grad<0, true>(ctx, farp); break;
+            case 1: e = launch_site_grad<1, true>(ctx, farp); break;
+            case 2: e = launch_site_grad<2, true>(ctx, farp); break;
+            case 3: e = launch_site_grad<3, true>(ctx, farp); break;
+            case 4: e = launch_site_grad<4, true>(ctx, farp); break;
+            case 5: e = launch_site_grad<5, true>(ctx, farp); break;
+            default: e = launch_site_grad<6, true>(ctx, farp); break;
+            }
+        } else {
+            switch (t.P) {
+            case 0: e = launch_site_grad<0, false>(ctx, farp); break;
+            case 1: e = launch_site_grad<1, false>(ctx, farp); break;
+            case 2: e = launch_site_grad<2, false>(ctx, farp); break;
+            case 3: e = launch_site_grad<3, false>(ctx, farp); break;
+            case 4: e = launch_site_grad<4, false>(ctx, farp); break;
+            case 5: e = launch_site_grad<5, false>(ctx, farp); break;
+            case 6: e = launch_site_grad<6, false>(ctx, farp); break;
+            case 7: e = launch_site_grad<7, false>(ctx, farp); break;
+            case 8: e = launch_site_grad<8, false>(ctx, farp); break;
+            default: return pb_fail(ctx, PB_ERR_INVALID_ARG, "internal: site treecode needs order_P <= 8");
+            }
         }
         PB_CUDA(e);
         PB_LAUNCH_CHECK();
+    }
+    if (H)
+        k_site_p2p<true><<<G * (ST_GROUP / SP_ST), SP_THREADS, 0, st>>>(s.na, s.tpos[0], s.tpos[1], s.tpos[2], s.t_p2p_off,
+                                                                        s.t_p2p_lo, s.t_p2p_hi, t.srec, nearp);
+    else
         k_site_p2p<false><<<G * (ST_GROUP / SP_ST), SP_THREADS, 0, st>>>(s.na, s.tpos[0], s.tpos[1], s.tpos[2], s.t_p2p_off,
                                                                          s.t_p2p_lo, s.t_p2p_hi, t.srec, nearp);
-        PB_LAUNCH_CHECK();
-    }
+    PB_LAUNCH_CHECK();
     k_site_finish<<<pb_blocks(s.na * NO, 128), 128, 0, st>>>(s.na, NO, s.tperm, nearp, farp, phi, grad, hess);
     PB_LAUNCH_CHECK();
     return PB_OK;
