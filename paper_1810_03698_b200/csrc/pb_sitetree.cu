@@ -166,9 +166,10 @@ template <int P> struct sg_cfg {
 // HESS: also the Hessian (the solve's closing call, Eq. 21/24), by differentiating once more:
 //     d_i d_j phi = sum_m [ u_m H_m,ij - u_{m+1} (d_i G_m,j + d_j G_m,i + delta_ij W_m) + u_{m+2} d_i d_j W_m ],
 // H_m,ij = sum_{|alpha|+j=m} d_i d_j (d^alpha) F, in a second sweep over the cell's terms (six more FMA per term; orders
-// P <= 6).
+// P <= 6).  At P = 5, 6 the compiler keeps the 6 (P + 1) sums of the second sweep in local memory (L1-resident; splitting
+// the sweep further made it spill instead); the call is still 4.3 times faster than the coefficient recurrence (C4: 140 -> 33 ms).
 template <int P, bool HESS>
-__global__ void __launch_bounds__(SG_THREADS, 1)
+__global__ void __launch_bounds__(SG_THREADS, HESS || P > 6 ? 1 : 2)
 k_site_grad(int64_t na, const double* __restrict__ sx, const double* __restrict__ sy, const double* __restrict__ sz,
             const int32_t* __restrict__ m2p_off, const int32_t* __restrict__ m2p_cell, const double* __restrict__ cx,
             const double* __restrict__ cy, const double* __restrict__ cz, const double2* __restrict__ FF,
