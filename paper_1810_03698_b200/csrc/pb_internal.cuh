@@ -342,7 +342,8 @@ int pb_upload_rules(pb_ctx* ctx);   // fills ctx->ruleF, ruleN, gl from the para
 // pb_matvec.cu
 int pb_farfield_setup(pb_ctx* ctx);
 int pb_site_farfield_setup(pb_ctx* ctx);
-int pb_upward(pb_ctx* ctx, cudaStream_t fs, const int32_t* leaf_ids, int64_t n_leaf, const int32_t* up_link);
+// comb: the F terms as the matvec's combined layers (pb_matvec.cu, m2p_radial); the site kernels want {F^V, F^K}
+int pb_upward(pb_ctx* ctx, cudaStream_t fs, const int32_t* leaf_ids, int64_t n_leaf, const int32_t* up_link, bool comb = false);
 int pb_matvec_impl(pb_ctx* ctx, const double* x, double* y, bool timed, bool precond);
 int pb_weights(pb_ctx* ctx, const double* x, bool precond, int surface = -1);   // surface 0 / 1: only that surface's sources
 void pb_make_expk(double kappa, pb_expk* out);

@@ -292,6 +292,8 @@ void pb_make_expk(double kappa, pb_expk* k)
 struct up_args {
     int P, Nk, NT, K;
     int CH, MQ;      // P2M chunk, M2M round (see above)
+    int comb;        // F terms as the combined layers {F^K - F^V, F^K - eps F^V} (m2p_radial) instead of {F^V, F^K}
+    double eps_ratio;
     const int32_t *leaf_ids, *c_first, *c_last, *c_child, *c_nchild, *up_link;
     int32_t* up_count;
     const double *cx, *cy, *cz;
@@ -423,7 +425,7 @@ __global__ void __launch_bounds__(UP_THREADS, NR == 1 ? 8 : (NR == 2 ? 6 : 4)) k
                     v = fma(f, mv[l], v);
                     k = fma(f, mk[l], k);
                 }
-                a.FF[c * a.NT + e] = make_double2(v, k);
+                a.FF[c * a.NT + e] = a.comb ? make_double2(k - v, fma(-a.eps_ratio, v, k)) : make_double2(v, k);
             }
         }
         if (parent < 0) break;
@@ -738,8 +740,13 @@ __device__ __forceinline__ void m2p_terms2(const double2* __restrict__ ff, doubl
     }
 }
 
-// radial part: u_m(R) of both kernels against the (P+1) partial sums per layer (D: section 6)
-template <int P, int PL>
+// radial part: u_m(R) of both kernels against the (P+1) partial sums per layer (D: section 6).
+// COMB: the two layers of the cell's F terms are not {V, K} but the combinations the two rows of Eq. (5) need,
+// {F^K - F^V, F^K - (eps_in / eps_out) F^V} (written so by the upward pass): the Laplace radial functions go with the first
+// layer only, the Yukawa ones with the second, and the results are KL' = K_L - V_L and KY' = K_Y - eps V_Y with VL = VY = 0
+// -- two FMA per layer instead of four, the combine kernel unchanged.  (Not with two surfaces, R-32: there the rows take
+// V and K with per-surface factors.)
+template <int P, int PL, bool COMB>
 __device__ __forceinline__ void m2p_radial(double dx, double dy, double dz, const double (&WV)[P + 1], const double (&WK)[P + 1],
                                            double kappa, double k2, const pb_expk& ek, const double* __restrict__ Ts,
                                            double& VL, double& KL, double& VY, double& KY)
@@ -748,13 +755,23 @@ __device__ __forceinline__ void m2p_radial(double dx, double dy, double dz, cons
     const double ri = pb_rsqrt(R2), R = R2 * ri, ri2 = ri * ri;
     const double ex = pb_exp_mkr(R, ek, Ts);
     double uL = ri, uY0 = ex * ri, uY1 = ex * fma(kappa, R, 1.0) * ri * ri2;
-    VL = fma(uL, WV[0], VL); KL = fma(uL, WK[0], KL);
-    VY = fma(uY0, WV[0], VY); KY = fma(uY0, WK[0], KY);
+    if (COMB) {
+        KL = fma(uL, WV[0], KL);
+        KY = fma(uY0, WK[0], KY);
+    } else {
+        VL = fma(uL, WV[0], VL); KL = fma(uL, WK[0], KL);
+        VY = fma(uY0, WV[0], VY); KY = fma(uY0, WK[0], KY);
+    }
 #pragma unroll
     for (int m = 1; m <= PL; ++m) {                    // p + j <= p + 2j <= PL: partial sums beyond PL are empty
         uL = (2 * m - 1) * uL * ri2;
-        VL = fma(uL, WV[m], VL); KL = fma(uL, WK[m], KL);
-        VY = fma(uY1, WV[m], VY); KY = fma(uY1, WK[m], KY);
+        if (COMB) {
+            KL = fma(uL, WV[m], KL);
+            KY = fma(uY1, WK[m], KY);
+        } else {
+            VL = fma(uL, WV[m], VL); KL = fma(uL, WK[m], KL);
+            VY = fma(uY1, WV[m], VY); KY = fma(uY1, WK[m], KY);
+        }
         const double un = ((2 * m + 1) * uY1 + k2 * uY0) * ri2;
         uY0 = uY1;
         uY1 = un;
@@ -762,7 +779,7 @@ __device__ __forceinline__ void m2p_radial(double dx, double dy, double dz, cons
 }
 
 // orders 7, 8: 36 partial sums per target pair leave no room for two blocks per SM (one block, up to 255 registers)
-template <int P>
+template <int P, bool COMB>
 #ifndef M2Q_MINB6
 #define M2Q_MINB6 2
 #endif
@@ -826,12 +843,12 @@ k_m2p2(int64_t N, double kappa, pb_expk ek, const pb_item* __restrict__ items, c
             for (int m = 0; m <= P; ++m) { WV0[m] = 0.0; WK0[m] = 0.0; WV1[m] = 0.0; WK1[m] = 0.0; }
             if (low) {
                 m2p_terms2<P, PL>(ffk, dx0, dy0, dz0, dx1, dy1, dz1, WV0, WK0, WV1, WK1);
-                m2p_radial<P, PL>(dx0, dy0, dz0, WV0, WK0, kappa, k2, ek, Ts, VL0, KL0, VY0, KY0);
-                m2p_radial<P, PL>(dx1, dy1, dz1, WV1, WK1, kappa, k2, ek, Ts, VL1, KL1, VY1, KY1);
+                m2p_radial<P, PL, COMB>(dx0, dy0, dz0, WV0, WK0, kappa, k2, ek, Ts, VL0, KL0, VY0, KY0);
+                m2p_radial<P, PL, COMB>(dx1, dy1, dz1, WV1, WK1, kappa, k2, ek, Ts, VL1, KL1, VY1, KY1);
             } else {
                 m2p_terms2<P, P>(ffk, dx0, dy0, dz0, dx1, dy1, dz1, WV0, WK0, WV1, WK1);
-                m2p_radial<P, P>(dx0, dy0, dz0, WV0, WK0, kappa, k2, ek, Ts, VL0, KL0, VY0, KY0);
-                m2p_radial<P, P>(dx1, dy1, dz1, WV1, WK1, kappa, k2, ek, Ts, VL1, KL1, VY1, KY1);
+                m2p_radial<P, P, COMB>(dx0, dy0, dz0, WV0, WK0, kappa, k2, ek, Ts, VL0, KL0, VY0, KY0);
+                m2p_radial<P, P, COMB>(dx1, dy1, dz1, WV1, WK1, kappa, k2, ek, Ts, VL1, KL1, VY1, KY1);
             }
         } else {                                       // the cell is accepted for one half of the group only
             const bool second = (code >> 1) == 2;
@@ -842,10 +859,10 @@ k_m2p2(int64_t N, double kappa, pb_expk ek, const pb_item* __restrict__ items, c
             for (int m = 0; m <= P; ++m) { WV[m] = 0.0; WK[m] = 0.0; }
             if (low) {
                 m2p_terms<P, PL>(ffk, dx, dy, dz, WV, WK);
-                m2p_radial<P, PL>(dx, dy, dz, WV, WK, kappa, k2, ek, Ts, vl, kl, vy, ky);
+                m2p_radial<P, PL, COMB>(dx, dy, dz, WV, WK, kappa, k2, ek, Ts, vl, kl, vy, ky);
             } else {
                 m2p_terms<P, P>(ffk, dx, dy, dz, WV, WK);
-                m2p_radial<P, P>(dx, dy, dz, WV, WK, kappa, k2, ek, Ts, vl, kl, vy, ky);
+                m2p_radial<P, P, COMB>(dx, dy, dz, WV, WK, kappa, k2, ek, Ts, vl, kl, vy, ky);
             }
             if (second) { VL1 = vl; KL1 = kl; VY1 = vy; KY1 = ky; }
             else { VL0 = vl; KL0 = kl; VY0 = vy; KY0 = ky; }
@@ -1279,19 +1296,30 @@ __global__ void k_stern_combine(int64_t N, const unsigned char* __restrict__ psu
     y[N + o] = r2;
 }
 
+// the matvec's far field with the two layers combined (m2p_radial): the two-target kernel's orders, one surface
+static bool pb_layers_combined(const pb_ctx* ctx) { return ctx->tree.P <= 8 && !ctx->tree.psurf; }
+
 // ---- host driver ----------------------------------------------------------------------------------------------
+template <int P, bool COMB>
+static cudaError_t launch_m2p2c(pb_ctx* ctx, cudaStream_t fs)
+{
+    pb_tree& t = ctx->tree;
+    const unsigned bit = 1u << (P + (COMB ? 16 : 0));
+    if (!(ctx->attr_m2p_mask & bit)) {   // per device and function: remembered per context (D: section 1)
+        cudaError_t e = cudaFuncSetAttribute(k_m2p2<P, COMB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m2q_cfg<P>::SMEM);
+        if (e != cudaSuccess) return e;
+        ctx->attr_m2p_mask |= bit;
+    }
+    k_m2p2<P, COMB><<<(unsigned)t.n_itemM_own, M2Q_THREADS, m2q_cfg<P>::SMEM, fs>>>(
+        t.N, ctx->prm.kappa, t.ek, t.itemM + t.itemM0, t.m2p_cell, t.m2p_ctr, t.FF, t.pc[0], t.pc[1], t.pc[2], t.accM);
+    return cudaSuccess;
+}
+
+// one surface: combined layers (m2p_radial); two surfaces (R-32): V and K apart
 template <int P>
 static cudaError_t launch_m2p2(pb_ctx* ctx, cudaStream_t fs)
 {
-    pb_tree& t = ctx->tree;
-    if (!(ctx->attr_m2p_mask & (1u << P))) {   // per device and function: remembered per context (D: section 1)
-        cudaError_t e = cudaFuncSetAttribute(k_m2p2<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m2q_cfg<P>::SMEM);
-        if (e != cudaSuccess) return e;
-        ctx->attr_m2p_mask |= 1u << P;
-    }
-    k_m2p2<P><<<(unsigned)t.n_itemM_own, M2Q_THREADS, m2q_cfg<P>::SMEM, fs>>>(
-        t.N, ctx->prm.kappa, t.ek, t.itemM + t.itemM0, t.m2p_cell, t.m2p_ctr, t.FF, t.pc[0], t.pc[1], t.pc[2], t.accM);
-    return cudaSuccess;
+    return pb_layers_combined(ctx) ? launch_m2p2c<P, true>(ctx, fs) : launch_m2p2c<P, false>(ctx, fs);
 }
 
 template <int P>
@@ -1310,7 +1338,7 @@ static cudaError_t launch_m2p(pb_ctx* ctx, cudaStream_t fs)
 
 // The upward pass for one set of needed cells: `leaf_ids` (one block each) and the per-cell `up_link` words.
 // The panel matvec and the site-side treecode (pb_sitetree.cu) each have their own set; both write t.M.
-int pb_upward(pb_ctx* ctx, cudaStream_t fs, const int32_t* leaf_ids, int64_t n_leaf, const int32_t* up_link)
+int pb_upward(pb_ctx* ctx, cudaStream_t fs, const int32_t* leaf_ids, int64_t n_leaf, const int32_t* up_link, bool comb)
 {
     pb_tree& t = ctx->tree;
     if (n_leaf <= 0) return PB_OK;
@@ -1323,6 +1351,8 @@ int pb_upward(pb_ctx* ctx, cudaStream_t fs, const int32_t* leaf_ids, int64_t n_l
     ua.mm_off = t.mm_off; ua.mm_ent = t.mm_ent; ua.mm_coef = t.mm_coef;
     ua.cv_off = t.cv_off; ua.cv_idx = t.cv_idx; ua.cv_coef = t.cv_coef;
     ua.M = t.M; ua.FF = t.FF;
+    ua.comb = comb ? 1 : 0;
+    ua.eps_ratio = ctx->prm.eps_in / ctx->prm.eps_out;
     const int nr = (t.Nk + UP_THREADS - 1) / UP_THREADS;
     const bool deep = n_leaf >= 148 * 8 * 2;          // more than two waves of blocks even at the highest occupancy
     ua.CH = deep ? P2M_CH_SMALL : P2M_CH_LARGE;
@@ -1385,7 +1415,7 @@ int pb_site_farfield_setup(pb_ctx* ctx)
 static int pb_far_branch(pb_ctx* ctx, cudaStream_t fs, bool timed)
 {
     pb_tree& t = ctx->tree;
-    PB_TRY(pb_upward(ctx, fs, t.need_leaf, t.n_need_leaf, t.up_link));
+    PB_TRY(pb_upward(ctx, fs, t.need_leaf, t.n_need_leaf, t.up_link, pb_layers_combined(ctx)));
     if (timed) PB_CUDA(cudaEventRecord(ctx->ev[2], fs));
     if (t.n_itemM_own > 0) {
         PB_TRY(pb_prof_begin(ctx, 1));
