@@ -59,6 +59,7 @@ struct pb_expk {
     double c1, Lk;
     double c[7];
     double T[32];
+    double g[12];     // g[m] = kappa^2 / ((2m+1)(2m-1)): the Yukawa radial recurrence with the layers scaled by (2m-1)!! (m2p_radial)
 };
 
 // Finer table, shorter polynomial, for the P2P kernel where exp(-kappa r) is evaluated once per pair:

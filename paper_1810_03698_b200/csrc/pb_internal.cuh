@@ -109,6 +109,7 @@ struct pb_tree {
     int32_t* cv_off = nullptr;    // [NT+1] conversion table (CSR over source moment indices)
     int32_t* cv_idx = nullptr;
     double* cv_coef = nullptr;
+    double* cv_scale = nullptr;   // cv_coef with every term of layer m scaled by (2m-1)!! (combined layers of the matvec)
     // near / singular correction table (CSR per target, Morton order)
     int64_t near_entries = 0;
     // ... stored as sliced ELL: slice = 32 consecutive targets, entry k of lane l at el_base[slice] + 32 k + l

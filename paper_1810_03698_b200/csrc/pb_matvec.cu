@@ -108,6 +108,16 @@ int pb_farfield_setup(pb_ctx* ctx)
     PB_CUDA(cudaMemcpyAsync(t.cv_off, off.data(), sizeof(int32_t) * off.size(), cudaMemcpyHostToDevice, st));
     PB_CUDA(cudaMemcpyAsync(t.cv_idx, idx.data(), sizeof(int32_t) * idx.size(), cudaMemcpyHostToDevice, st));
     PB_CUDA(cudaMemcpyAsync(t.cv_coef, coef.data(), sizeof(double) * coef.size(), cudaMemcpyHostToDevice, st));
+    // the same coefficients with every term of layer m = |alpha| + j scaled by (2m-1)!!: the matvec's combined layers (m2p_radial)
+    std::vector<double> coef_s(coef);
+    for (int e = 0; e < t.NT; ++e) {
+        const int m = expo[4 * e] + expo[4 * e + 1] + expo[4 * e + 2] + expo[4 * e + 3];
+        double f = 1.0;
+        for (int q = 1; q <= m; ++q) f *= 2.0 * q - 1.0;
+        for (int q = off[e]; q < off[e + 1]; ++q) coef_s[q] *= f;
+    }
+    PB_TRY(pb_dalloc_t(ctx, &t.cv_scale, coef_s.size(), CAT_TREE));
+    PB_CUDA(cudaMemcpyAsync(t.cv_scale, coef_s.data(), sizeof(double) * coef_s.size(), cudaMemcpyHostToDevice, st));
     // M2M table: for every k the triples (l, k - l, C(k,l)), l <= k componentwise; l and k - l as moment indices
     std::vector<int32_t> mo(1, 0), me;
     std::vector<double> mc;
@@ -267,6 +277,8 @@ void pb_make_expk(double kappa, pb_expk* k)
         f *= -kappa / (double)(m + 1);
     }
     for (int j = 0; j < 32; ++j) k->T[j] = exp2(-(double)j / 32.0);
+    k->g[0] = 0.0;
+    for (int m = 1; m < 12; ++m) k->g[m] = kappa * kappa / ((2.0 * m + 1.0) * (2.0 * m - 1.0));
 }
 
 // ---- upward pass in ONE launch (H5): P2M at the leaves, M2M up the tree, M -> F conversion ---------------
@@ -756,22 +768,28 @@ __device__ __forceinline__ void m2p_radial(double dx, double dy, double dz, cons
     const double ex = pb_exp_mkr(R, ek, Ts);
     double uL = ri, uY0 = ex * ri, uY1 = ex * fma(kappa, R, 1.0) * ri * ri2;
     if (COMB) {
+        // the upward pass has also multiplied layer m by (2m-1)!!, so the radial functions here are u_m / (2m-1)!!:
+        // R^-(2m+1) for Laplace (one product per layer) and, for Yukawa, u~_{m+1} = (u~_m + g_m u~_{m-1}) / R^2
         KL = fma(uL, WV[0], KL);
         KY = fma(uY0, WK[0], KY);
-    } else {
-        VL = fma(uL, WV[0], VL); KL = fma(uL, WK[0], KL);
-        VY = fma(uY0, WV[0], VY); KY = fma(uY0, WK[0], KY);
+#pragma unroll
+        for (int m = 1; m <= PL; ++m) {
+            uL *= ri2;
+            KL = fma(uL, WV[m], KL);
+            KY = fma(uY1, WK[m], KY);
+            const double un = fma(ek.g[m], uY0, uY1) * ri2;
+            uY0 = uY1;
+            uY1 = un;
+        }
+        return;
     }
+    VL = fma(uL, WV[0], VL); KL = fma(uL, WK[0], KL);
+    VY = fma(uY0, WV[0], VY); KY = fma(uY0, WK[0], KY);
 #pragma unroll
     for (int m = 1; m <= PL; ++m) {                    // p + j <= p + 2j <= PL: partial sums beyond PL are empty
         uL = (2 * m - 1) * uL * ri2;
-        if (COMB) {
-            KL = fma(uL, WV[m], KL);
-            KY = fma(uY1, WK[m], KY);
-        } else {
-            VL = fma(uL, WV[m], VL); KL = fma(uL, WK[m], KL);
-            VY = fma(uY1, WV[m], VY); KY = fma(uY1, WK[m], KY);
-        }
+        VL = fma(uL, WV[m], VL); KL = fma(uL, WK[m], KL);
+        VY = fma(uY1, WV[m], VY); KY = fma(uY1, WK[m], KY);
         const double un = ((2 * m + 1) * uY1 + k2 * uY0) * ri2;
         uY0 = uY1;
         uY1 = un;
@@ -1349,7 +1367,7 @@ int pb_upward(pb_ctx* ctx, cudaStream_t fs, const int32_t* leaf_ids, int64_t n_l
     ua.cx = t.c_ctr[0]; ua.cy = t.c_ctr[1]; ua.cz = t.c_ctr[2];
     ua.srec = t.srec;
     ua.mm_off = t.mm_off; ua.mm_ent = t.mm_ent; ua.mm_coef = t.mm_coef;
-    ua.cv_off = t.cv_off; ua.cv_idx = t.cv_idx; ua.cv_coef = t.cv_coef;
+    ua.cv_off = t.cv_off; ua.cv_idx = t.cv_idx; ua.cv_coef = comb ? t.cv_scale : t.cv_coef;   // comb: layers scaled by (2m-1)!!
     ua.M = t.M; ua.FF = t.FF;
     ua.comb = comb ? 1 : 0;
     ua.eps_ratio = ctx->prm.eps_in / ctx->prm.eps_out;
