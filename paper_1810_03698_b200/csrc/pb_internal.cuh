@@ -2,6 +2,7 @@
 // Product code.  Nothing here includes, links or calls anything under oracle/.
 #pragma once
 #include <cuda_runtime.h>
+#include <cuda_fp16.h>
 #include <stdint.h>
 #include <stdio.h>
 #include <string.h>
@@ -117,8 +118,9 @@ struct pb_tree {
     int32_t* el_base = nullptr;   // [slices + 1]
     int32_t* el_col = nullptr;    // [el_entries] source panel (Morton); padding: the target itself
     double* el_val = nullptr;     // [4][el_entries] VL, KL, VY, KY corrections; padding: 0
-    float* el_tval = nullptr;     // [4][el_entries] the true near-zone entries, rounded to fp32: they only feed the near-field
-                                  // preconditioner, whose SpMV streams this table (half the bytes of fp64); padding: 0
+    __half* el_tval = nullptr;    // [el_entries][4] (V_L, K_L, V_Y, K_Y interleaved) the true near-zone entries, rounded to fp16 (all are O(1) or smaller; 11 bits): they
+                                  // only feed the near-field preconditioner, whose SpMV streams this table (a quarter of the
+                                  // bytes of fp64); padding: 0
     double* precond = nullptr;    // [N][4] inverse 2x2 diagonal blocks
     // partial accumulators
     // work items (one thread block each) and their accumulator slots

@@ -7,6 +7,7 @@
 // three-zone quadrature of P:245: semi-analytic for SELF and vertex-sharing panels, K_near
 // points inside tau*sqrt(A_i), K_far points elsewhere.
 #include <math.h>
+#include <cuda_fp16.h>
 #include "pb_internal.cuh"
 
 // ---- rules (host) -----------------------------------------------------------------------------
@@ -384,7 +385,7 @@ __global__ void k_ell_width(int64_t N, const int32_t* __restrict__ off, int32_t*
 __global__ void k_ell_fill(int64_t N, const int32_t* __restrict__ off, const int32_t* __restrict__ col,
                            const double* __restrict__ val, const double* __restrict__ tval, int64_t ne,
                            const int32_t* __restrict__ base, int64_t ne_ell, int32_t* __restrict__ ecol,
-                           double* __restrict__ eval, float* __restrict__ etval)
+                           double* __restrict__ eval, __half* __restrict__ etval)
 {
     const int64_t w = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
@@ -399,7 +400,7 @@ __global__ void k_ell_fill(int64_t N, const int32_t* __restrict__ off, const int
 #pragma unroll
         for (int m = 0; m < 4; ++m) {
             eval[(int64_t)m * ne_ell + d] = real ? val[(int64_t)m * ne + e0 + k] : 0.0;
-            etval[(int64_t)m * ne_ell + d] = real ? (float)tval[(int64_t)m * ne + e0 + k] : 0.0f;
+            etval[4 * d + m] = __double2half(real ? tval[(int64_t)m * ne + e0 + k] : 0.0);
         }
     }
 }

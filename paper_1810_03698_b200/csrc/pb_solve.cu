@@ -301,7 +301,7 @@ __global__ void k_axpy(int64_t n, double a, const double* __restrict__ x, double
 // alpha stays on the device (no host synchronisation); the iteration runs in Morton order, where the table lives.
 // M depends on v non-linearly (through alpha), hence the flexible variant of GMRES.  Measured on the oracle's dense
 // matrix of C2 (19,176 unknowns): 72 outer iterations with block-Jacobi alone, 42 with 2 inner steps, 40 with 3,
-// 28 with an exact sparse solve of A_n.  The table of A_n is kept in fp32 (half the bytes to stream per step): M only
+// 28 with an exact sparse solve of A_n.  The table of A_n is kept in fp16 (a quarter of the bytes to stream per step; entries are O(1) or smaller): M only
 // has to be a good approximate inverse, the residuals of the outer iteration come from the fp64 operator.
 #define PB_NF_STEPS 2
 
@@ -318,32 +318,49 @@ __global__ void k_nf_start(int64_t N, const int32_t* __restrict__ perm, const do
     z[i] = 0.0; z[N + i] = 0.0;
 }
 
-// q = A_n p in Morton order; block = 32 targets (one ELL slice) x 4 kernels, as in k_combine
-__global__ void __launch_bounds__(128)
+// q = A_n p in Morton order.  One lane per target, one warp per ELL slice of 32 targets: per entry one column index, the
+// four values of the pair as one 8-byte load (fp16, interleaved) and two gathers, p_j = phi_j and p_{N+j} = dphi_j.  (The
+// first version gave each of the four kernels its own warp: four index loads and four gathers per entry, 150 us per
+// product at C4 against 0.73 GB of table; the gathers, not the table, set the pace.)
+#define NF_WARPS 4
+__global__ void __launch_bounds__(32 * NF_WARPS)
 k_nf_spmv(int64_t N, double eps_ratio, const int32_t* __restrict__ el_base, const int32_t* __restrict__ el_col,
-          const float* __restrict__ el_tval, int64_t ne, const double* __restrict__ p, double* __restrict__ q)
+          const uint2* __restrict__ el_tval /*[entries] 4 x fp16: V_L, K_L, V_Y, K_Y*/, const double* __restrict__ p,
+          double* __restrict__ q)
 {
-    __shared__ double sm[4][32];
-    const int tgt = threadIdx.x & 31, m = threadIdx.x >> 5;
-    const int64_t i = blockIdx.x * 32LL + tgt;
-    const double* __restrict__ xv = (m & 1) ? p : p + N;          // V_L, V_Y act on dphi; K_L, K_Y on phi
-    const int32_t b0 = el_base[blockIdx.x], width = (el_base[blockIdx.x + 1] - b0) / 32;
-    const float* __restrict__ val = el_tval + (int64_t)m * ne + b0 + tgt;
-    const int32_t* __restrict__ col = el_col + b0 + tgt;
-    double s = 0.0;
+    const int lane = threadIdx.x & 31;
+    const int64_t sl = blockIdx.x * (int64_t)NF_WARPS + (threadIdx.x >> 5);
+    if (sl * 32 >= N) return;
+    const int64_t i = sl * 32 + lane;
+    const int32_t b0 = el_base[sl], width = (el_base[sl + 1] - b0) / 32;
+    const uint2* __restrict__ val = el_tval + b0 + lane;
+    const int32_t* __restrict__ col = el_col + b0 + lane;
+    double VL = 0.0, KL = 0.0, VY = 0.0, KY = 0.0;
+    auto add = [&](uint2 v, double ph, double dp) {
+        const float2 lo = __half22float2(*reinterpret_cast<const __half2*>(&v.x));   // V_L, K_L
+        const float2 hi = __half22float2(*reinterpret_cast<const __half2*>(&v.y));   // V_Y, K_Y
+        VL = fma((double)lo.x, dp, VL); KL = fma((double)lo.y, ph, KL);
+        VY = fma((double)hi.x, dp, VY); KY = fma((double)hi.y, ph, KY);
+    };
     int k = 0;
     for (; k + 4 <= width; k += 4) {
-        double a[4], b[4];
+        uint2 v[4];
+        double ph[4], dp[4];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) { a[u] = (double)val[32 * (k + u)]; b[u] = xv[col[32 * (k + u)]]; }
+        for (int u = 0; u < 4; ++u) {
+            const int32_t j = col[32 * (k + u)];
+            v[u] = val[32 * (k + u)];
+            ph[u] = p[j];
+            dp[u] = p[N + j];
+        }
 #pragma unroll
-        for (int u = 0; u < 4; ++u) s = fma(a[u], b[u], s);
+        for (int u = 0; u < 4; ++u) add(v[u], ph[u], dp[u]);
     }
-    for (; k < width; ++k) s = fma((double)val[32 * k], xv[col[32 * k]], s);
-    sm[m][tgt] = s;
-    __syncthreads();
-    if (m == 0 && i < N) {
-        const double VL = sm[0][tgt], KL = sm[1][tgt], VY = sm[2][tgt], KY = sm[3][tgt];
+    for (; k < width; ++k) {
+        const int32_t j = col[32 * k];
+        add(val[32 * k], p[j], p[N + j]);
+    }
+    if (i < N) {
         const double phi = p[i];
         q[i] = 0.5 * phi + KL - VL;                     // Eq. (5), first row restricted to the near zone
         q[N + i] = 0.5 * phi - KY + eps_ratio * VY;     // second row
@@ -425,8 +442,8 @@ static int near_precond(pb_ctx* ctx, gmres_ws& ws, const double* v, double* z)
     // with 2 / 4 / 6 steps (block-Jacobi alone: 147 and 317)
     const int nsteps = N < 30000 ? PB_NF_STEPS : (N < 300000 ? 2 * PB_NF_STEPS : 3 * PB_NF_STEPS);
     for (int step = 0; step < nsteps; ++step) {
-        k_nf_spmv<<<pb_blocks(N, 32), 128, 0, st>>>(N, ctx->prm.eps_in / ctx->prm.eps_out, t.el_base, t.el_col, t.el_tval,
-                                                    t.el_entries, ws.nf_p, ws.nf_q);
+        k_nf_spmv<<<pb_blocks((N + 31) / 32, NF_WARPS), 32 * NF_WARPS, 0, st>>>(N, ctx->prm.eps_in / ctx->prm.eps_out, t.el_base, t.el_col,
+                                                                              reinterpret_cast<const uint2*>(t.el_tval), ws.nf_p, ws.nf_q);
         PB_LAUNCH_CHECK();
         k_nf_alpha<<<nbd, 256, 0, st>>>(n, ws.nf_r, ws.nf_q, ws.partial, ws.counter, ws.hdev + 2 * (ws.m + 4) + 4);
         PB_LAUNCH_CHECK();
