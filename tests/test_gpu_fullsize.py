@@ -89,6 +89,34 @@ def test_matvec_full_size(pbm, po, torch_cuda, name, kw, nrows, direct):
     ctx.close()
 
 
+def test_orders_4_to_10_at_c3_against_direct_mode(pbm, torch_cuda):
+    """Every order's kernels where the grid is many waves deep (C3 complex, 10,406 leaves: the upward pass with one, two
+    and three moments per thread and the small P2M chunk / M2M round; k_m2p2 with combined layers up to P = 8, k_m2p for
+    9 and 10) against the direct mode (itself equal to the oracle on sampled rows, test_matvec_full_size) on every row:
+    the error falls with the order and meets the bounds measured at C2 (test_high_order_m2p_at_c2), and the lists stay
+    an exact cover."""
+    from paper_1810_03698_b200.workloads import make_config
+    w = make_config("C3", which="complex")
+    nt = w.tris.shape[0]
+    x = torch_cuda.from_numpy(np.random.Generator(np.random.PCG64(7)).normal(size=2 * nt)).cuda()
+    ctx = pbm.from_workload(w, theta=0.0)
+    ctx.tree_build()
+    yd = ctx.matvec(x).cpu().numpy()
+    errs = {}
+    for P in (4, 6, 7, 8, 9, 10):
+        ctx.set_params(theta=0.5, order_P=P)
+        ctx.tree_build()
+        y = ctx.matvec(x).cpu().numpy()
+        st = ctx.stats()
+        assert st["covered_pairs"] == nt * nt * w.params["K_far"] and st["n_leaves"] > 2368
+        d = y - yd
+        errs[P] = float(np.linalg.norm(d) / np.linalg.norm(yd))
+        np.testing.assert_array_equal(y, ctx.matvec(x).cpu().numpy())      # bitwise repeatable at every order
+    assert errs[4] <= 1e-3 and errs[6] <= TOL_TREE and errs[7] <= 5e-5 and errs[8] <= 2.5e-5 and errs[9] <= 1.2e-5 and errs[10] <= 6e-6, errs
+    assert errs[4] > errs[6] > errs[7] > errs[8] > errs[9] > errs[10], errs
+    ctx.close()
+
+
 def test_site_side_operators_c2(pbm, po, torch_cuda):
     """RHS (Eq. 8), reaction field (Eq. 12, 13, 21) and multipole field (Eq. 14) at C2's sizes
     (1,000 sites, ~10k panels, polarization groups of 4)."""
