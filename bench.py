@@ -61,9 +61,11 @@ def m2p_flop_per_pair(P, n_terms=None):
 
 
 def m2p_flop(P, st):
-    """Algorithmic flop of one M2P launch: pairs at order P plus the pairs the list build flagged for order P - 2."""
-    low = st.get("m2p_pairs_low", 0)
-    return m2p_flop_per_pair(P, st["n_terms"]) * (st["m2p_pairs"] - low) + (m2p_flop_per_pair(P - 2) * low if low else 0.0)
+    """Algorithmic flop of one M2P launch: every pair at the order it is evaluated at -- P, or P - 1 / P - 2 for the pairs
+    the list build flagged (R-30)."""
+    low, mid = st.get("m2p_pairs_low", 0), st.get("m2p_pairs_mid", 0)
+    return (m2p_flop_per_pair(P, st["n_terms"]) * (st["m2p_pairs"] - low - mid) + (m2p_flop_per_pair(P - 2) * low if low else 0.0)
+            + (m2p_flop_per_pair(P - 1) * mid if mid else 0.0))
 
 
 def load_counters(workload, theta, P, ncrit):
@@ -415,6 +417,7 @@ def run_ours(args):
                                                                  f"of y's owned rows per step" if sharded else f"{world} replicas")},
         "evaluated": {"p2p_pairs_per_matvec": int(p2p_pairs), "m2p_pairs_per_matvec": int(m2p_pairs),
                       "m2p_pairs_at_order_P_minus_2": int(sum_over_ranks(float(st1["m2p_pairs_low"]), world, dev)) if world == 1 else None,
+                      "m2p_pairs_at_order_P_minus_1": int(st1["m2p_pairs_mid"]) if world == 1 else None,
                       "p2p_pairs_for_one_half_of_a_group": int(st1["p2p_pairs_half"]) if world == 1 else None,
                       "m2p_pairs_for_one_half_of_a_group": int(st1["m2p_pairs_half"]) if world == 1 else None,
                       "covered_pairs": int(st1["covered_pairs"]), "covered_equals_N_x_Ns": bool(st1["covered_pairs"] == int(inter_per_mv)) if world == 1 else None,
@@ -523,7 +526,7 @@ def run_sweep(args):
                 "covered_equals_N_x_Ns": bool(st["covered_pairs"] == nt * st["n_sources"]),
                 "serial_ms": {k: lm[k] for k in ("weights", "p2m_m2m", "m2p", "p2p", "near_combine")},
                 "p2p_tflops": P2P_FLOP_PER_PAIR * st["p2p_pairs"] / (lm["p2p"] * 1e-3) / 1e12,
-                "m2p_pairs_low_order": int(st["m2p_pairs_low"]),
+                "m2p_pairs_low_order": int(st["m2p_pairs_low"]), "m2p_pairs_mid_order": int(st["m2p_pairs_mid"]),
                 "m2p_tflops": m2p_flop(P, st) / (lm["m2p"] * 1e-3) / 1e12 if lm["m2p"] > 0 else 0.0,
                 "fp64_peak_tflops_measured": peak, "rel_l2_vs_oracle_rows": err, "device_gb": st["device_bytes"] / 1e9}), flush=True)
     ctx.set_params(**{k: v for k, v in w.params.items() if k in ("theta", "order_P")})

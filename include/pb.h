@@ -157,6 +157,7 @@ typedef struct pb_stats {
     int64_t rhs_covered_pairs;  /* == n_panels * n_sites when those lists are complete                             */
     int64_t p2p_pairs_half;     /* of p2p_pairs / m2p_pairs: pairs of list entries that serve one half (32 targets) of a   */
     int64_t m2p_pairs_half;     /* 64-target group only (the two halves of a group are accepted separately)               */
+    int64_t m2p_pairs_mid;      /* of m2p_pairs: those evaluated at order P - 1 (D: R-30)                                  */
 } pb_stats;
 
 typedef void* (*pb_alloc_fn)(void* user, size_t bytes);     /* returns a 256-byte aligned device pointer or NULL */

@@ -535,6 +535,7 @@ extern "C" int pb_get_stats(pb_ctx* ctx, pb_stats* out)
     out->covered_pairs = t.covered_pairs;
     out->p2p_pairs_half = t.p2p_pairs_half;
     out->m2p_pairs_half = t.m2p_pairs_half;
+    out->m2p_pairs_mid = t.m2p_pairs_mid;
     if (ctx->sites.rhs_built) {
         out->rhs_p2p_pairs = ctx->sites.r_ls.p2p_pairs;
         out->rhs_m2p_pairs = ctx->sites.r_ls.m2p_pairs;

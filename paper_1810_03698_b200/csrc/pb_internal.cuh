@@ -90,8 +90,9 @@ struct pb_tree {
     int32_t* p2p_hi = nullptr;
     int4* p2p_rng = nullptr;      // [ranges + 2] {lo, hi, mask, 0}: one 16-byte load per range for k_p2p2
     int8_t* p2p_mask = nullptr;   // [ranges] which half of the group the range is for: 1 = targets 0..31, 2 = 32..63, 3 = both (k_lists)
-    int8_t* m2p_code = nullptr;   // [entries] bit 0: order P - 2; bits 1-2: the same half mask (also in m2p_ctr[e].w)
+    int8_t* m2p_code = nullptr;   // [entries] bit 0: order P - 2; bit 3: order P - 1; bits 1-2: the same half mask (also in m2p_ctr[e].w)
     int64_t p2p_pairs = 0, m2p_pairs = 0, m2p_pairs_low = 0;   // m2p_pairs_low: those evaluated at order P - 2
+    int64_t m2p_pairs_mid = 0;                                  // ... at order P - 1
     int64_t p2p_pairs_half = 0, m2p_pairs_half = 0;            // of those: pairs of entries listed for one half only
     int64_t covered_pairs = 0;    // (target, source point) pairs the STORED lists cover (k_cover_count); == N * Ns
     // far-field data

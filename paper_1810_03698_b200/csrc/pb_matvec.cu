@@ -852,32 +852,41 @@ k_m2p2(int64_t N, double kappa, pb_expk ek, const pb_item* __restrict__ items, c
         const double2* ffk = ffw + (size_t)(k % NS) * NT;
         const double dx0 = tx0 - cc.x, dy0 = ty0 - cc.y, dz0 = tz0 - cc.z;
         const double dx1 = tx1 - cc.x, dy1 = ty1 - cc.y, dz1 = tz1 - cc.z;
-        constexpr int PL = P >= 4 ? P - 2 : P;
-        const int code = (int)cc.w;                    // k_lists: bit 0 = order P - 2 is enough, bits 1-2 = half mask (warp-uniform)
-        const bool low = PL < P && (code & 1);
-        if ((code >> 1) == 3) {                        // both targets of every lane: each term read feeds four FMAs
+        constexpr int PL = P >= 4 ? P - 2 : P, PM = P >= 4 ? P - 1 : P;
+        // k_lists: bit 0 = order P - 2 is enough, bit 3 = order P - 1 is, bits 1-2 = half mask (all warp-uniform)
+        const int code = (int)cc.w;
+        const int tier = PL < P ? ((code & 1) ? 2 : ((code & 8) ? 1 : 0)) : 0;
+        const int half = (code >> 1) & 3;
+        if (half == 3) {                               // both targets of every lane: each term read feeds four FMAs
             double WV0[P + 1], WK0[P + 1], WV1[P + 1], WK1[P + 1];
 #pragma unroll
             for (int m = 0; m <= P; ++m) { WV0[m] = 0.0; WK0[m] = 0.0; WV1[m] = 0.0; WK1[m] = 0.0; }
-            if (low) {
+            if (tier == 2) {
                 m2p_terms2<P, PL>(ffk, dx0, dy0, dz0, dx1, dy1, dz1, WV0, WK0, WV1, WK1);
                 m2p_radial<P, PL, COMB>(dx0, dy0, dz0, WV0, WK0, kappa, k2, ek, Ts, VL0, KL0, VY0, KY0);
                 m2p_radial<P, PL, COMB>(dx1, dy1, dz1, WV1, WK1, kappa, k2, ek, Ts, VL1, KL1, VY1, KY1);
+            } else if (tier == 1) {
+                m2p_terms2<P, PM>(ffk, dx0, dy0, dz0, dx1, dy1, dz1, WV0, WK0, WV1, WK1);
+                m2p_radial<P, PM, COMB>(dx0, dy0, dz0, WV0, WK0, kappa, k2, ek, Ts, VL0, KL0, VY0, KY0);
+                m2p_radial<P, PM, COMB>(dx1, dy1, dz1, WV1, WK1, kappa, k2, ek, Ts, VL1, KL1, VY1, KY1);
             } else {
                 m2p_terms2<P, P>(ffk, dx0, dy0, dz0, dx1, dy1, dz1, WV0, WK0, WV1, WK1);
                 m2p_radial<P, P, COMB>(dx0, dy0, dz0, WV0, WK0, kappa, k2, ek, Ts, VL0, KL0, VY0, KY0);
                 m2p_radial<P, P, COMB>(dx1, dy1, dz1, WV1, WK1, kappa, k2, ek, Ts, VL1, KL1, VY1, KY1);
             }
         } else {                                       // the cell is accepted for one half of the group only
-            const bool second = (code >> 1) == 2;
+            const bool second = half == 2;
             const double dx = second ? dx1 : dx0, dy = second ? dy1 : dy0, dz = second ? dz1 : dz0;
             double vl = second ? VL1 : VL0, kl = second ? KL1 : KL0, vy = second ? VY1 : VY0, ky = second ? KY1 : KY0;
             double WV[P + 1], WK[P + 1];
 #pragma unroll
             for (int m = 0; m <= P; ++m) { WV[m] = 0.0; WK[m] = 0.0; }
-            if (low) {
+            if (tier == 2) {
                 m2p_terms<P, PL>(ffk, dx, dy, dz, WV, WK);
                 m2p_radial<P, PL, COMB>(dx, dy, dz, WV, WK, kappa, k2, ek, Ts, vl, kl, vy, ky);
+            } else if (tier == 1) {
+                m2p_terms<P, PM>(ffk, dx, dy, dz, WV, WK);
+                m2p_radial<P, PM, COMB>(dx, dy, dz, WV, WK, kappa, k2, ek, Ts, vl, kl, vy, ky);
             } else {
                 m2p_terms<P, P>(ffk, dx, dy, dz, WV, WK);
                 m2p_radial<P, P, COMB>(dx, dy, dz, WV, WK, kappa, k2, ek, Ts, vl, kl, vy, ky);

@@ -305,18 +305,19 @@ struct list_args {
     int64_t ng, N, Ns;
     int K;
     double theta;
-    double theta_low2;                // > 0: cells with (R_b/R_tb)^2 below it for every target are flagged low order
+    double theta_low2;                // > 0: cells with (R_b/R_tb)^2 below it for every target are flagged for order P - 2
+    double theta_mid2;                // > 0: ... and, of the others, the ones below this for order P - 1 (R-30)
     int m2p_min;
     const int32_t *c_first, *c_last, *c_child, *c_nchild;
     const double *cx, *cy, *cz, *crad;
     const double *px, *py, *pz;       // collocation points, Morton order
-    int8_t* m2p_low;                  // [entries] code of the entry (pass 1; may be NULL): bit 0 = evaluate at order P - 2,
+    int8_t* m2p_low;                  // [entries] code of the entry (pass 1; may be NULL): bit 0 = evaluate at order P - 2, bit 3 = at order P - 1,
                                       // bits 1-2 = which half of the group the entry is for (1 = targets 0..31, 2 = 32..63, 3 = both)
     int8_t* p2p_mask;                 // [ranges] the same half mask for every P2P range (pass 1; NULL without `split`)
     int split;                        // 1: the two halves of a 64-target group are accepted separately (TPL == 2 only)
     int32_t *n_m2p, *n_p2p;           // pass 0: counts ; pass 1: offsets (read)
     int32_t *m2p_cell, *p2p_lo, *p2p_hi;
-    unsigned long long* pair_counts;  // [3] p2p, m2p, low-order m2p pairs (pass 0)
+    unsigned long long* pair_counts;  // [6] p2p, m2p, order-(P-2) m2p, one-half p2p, one-half m2p, order-(P-1) m2p pairs (pass 0)
 };
 
 #define LIST_WARPS 4
@@ -345,7 +346,7 @@ __global__ void __launch_bounds__(LIST_WARPS * 32) k_lists(list_args a)
     auto ntargets = [&](int m) -> unsigned long long { return (m & 1 ? nA : 0ull) + (m & 2 ? nB : 0ull); };
     int nm = 0, nr = 0;
     const int64_t om = PASS ? a.n_m2p[g] : 0, op = PASS ? a.n_p2p[g] : 0;
-    unsigned long long pp = 0, pm = 0, plow = 0, pph = 0, pmh = 0;
+    unsigned long long pp = 0, pm = 0, plow = 0, pph = 0, pmh = 0, pmid = 0;
     if (a.theta <= 0.0) {   // direct mode: one range, every source point
         if (PASS && lane == 0) {
             a.p2p_lo[op] = 0; a.p2p_hi[op] = (int32_t)a.Ns;
@@ -392,13 +393,15 @@ __global__ void __launch_bounds__(LIST_WARPS * 32) k_lists(list_args a)
                 if (acc & 1) dmin = fmin(dmin, da);
                 if (acc & 2) dmin = fmin(dmin, db);
                 const bool low = cr * cr < a.theta_low2 * dmin;
+                const bool mid = !low && cr * cr < a.theta_mid2 * dmin;
                 if (PASS && lane == 0) {
                     a.m2p_cell[om + nm] = c;
-                    if (a.m2p_low) a.m2p_low[om + nm] = (int8_t)((low ? 1 : 0) | (acc << 1));
+                    if (a.m2p_low) a.m2p_low[om + nm] = (int8_t)((low ? 1 : 0) | (acc << 1) | (mid ? 8 : 0));
                 }
                 ++nm;
                 pm += ntargets(acc);
                 if (low) plow += ntargets(acc);
+                if (mid) pmid += ntargets(acc);
                 if (acc != full_mask) pmh += ntargets(acc);
             }
             const int rem = mask & ~acc;
@@ -435,15 +438,20 @@ __global__ void __launch_bounds__(LIST_WARPS * 32) k_lists(list_args a)
         atomicAdd(&a.pair_counts[2], plow);
         atomicAdd(&a.pair_counts[3], pph);
         atomicAdd(&a.pair_counts[4], pmh);
+        atomicAdd(&a.pair_counts[5], pmid);
     }
 }
 
-// Stable partition of every group's M2P list into six classes: the cells evaluated at the full order P first, then the
-// ones flagged for order P - 2 (R-30); within each, the entries for both halves of the group, then the ones for the first
-// half only, then the second half only.  The 8 warps of a k_m2p2 block take consecutive list entries, one cell per
-// warp; with neighbours of one class the warps of a block finish their shares at about the same time.  One thread per
-// group; setup time only.  code: bit 0 = order P - 2, bits 1-2 = half mask (k_lists).
-__device__ __forceinline__ int m2p_class(int code) { return (code & 1) * 3 + ((code >> 1) == 3 ? 0 : (code >> 1)); }
+// Stable partition of every group's M2P list into nine classes: the cells evaluated at the full order P first, then the
+// ones flagged for order P - 1, then the ones for order P - 2 (R-30); within each, the entries for both halves of the group,
+// then the ones for the first half only, then the second half only.  The 8 warps of a k_m2p2 block take consecutive list
+// entries, one cell per warp; with neighbours of one class the warps of a block finish their shares at about the same
+// time.  One thread per group; setup time only.  code: bit 0 = order P - 2, bit 3 = order P - 1, bits 1-2 = half mask (k_lists).
+__device__ __forceinline__ int m2p_class(int code)
+{
+    const int tier = (code & 1) ? 2 : ((code & 8) ? 1 : 0), half = (code >> 1) & 3;
+    return tier * 3 + (half == 3 ? 0 : half);
+}
 
 __global__ void k_partition_low(int64_t G, const int32_t* __restrict__ off, const int32_t* __restrict__ cell_in,
                                 const int8_t* __restrict__ code_in, int32_t* __restrict__ cell_out, int8_t* __restrict__ code_out)
@@ -451,10 +459,10 @@ __global__ void k_partition_low(int64_t G, const int32_t* __restrict__ off, cons
     const int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (g >= G) return;
     const int32_t e0 = off[g], e1 = off[g + 1];
-    int32_t pos[6] = {0, 0, 0, 0, 0, 0};
+    int32_t pos[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
     for (int32_t e = e0; e < e1; ++e) ++pos[m2p_class(code_in[e])];
     int32_t run = e0;
-    for (int k = 0; k < 6; ++k) { const int32_t n = pos[k]; pos[k] = run; run += n; }
+    for (int k = 0; k < 9; ++k) { const int32_t n = pos[k]; pos[k] = run; run += n; }
     for (int32_t e = e0; e < e1; ++e) {
         const int code = code_in[e];
         const int32_t d = pos[m2p_class(code)]++;
@@ -866,6 +874,10 @@ int pb_tree_build_impl(pb_ctx* ctx)
         const int P = ctx->prm.order_P;
         const double tl = P >= 4 && P <= 8 ? 0.8 * pow(ctx->prm.theta, (double)(P + 1) / (double)(P - 1)) : 0.0;
         a.theta_low2 = tl * tl;
+        // ... and between the two, order P - 1 for ratio <= 0.8 theta^((P+1)/P): truncation error ratio^P <= 0.8^P theta^(P+1),
+        // a smaller share of the error the MAC admits than the order-(P-2) cells take (0.26 against 0.33 at P = 6)
+        const double tm = P >= 4 && P <= 8 ? 0.8 * pow(ctx->prm.theta, (double)(P + 1) / (double)P) : 0.0;
+        a.theta_mid2 = tm * tm;
     }
     a.m2p_min = 8;   // an M2P pair costs about as much as 8 P2P pairs (D: section 7)
     a.c_first = t.c_first; a.c_last = t.c_last; a.c_child = t.c_child; a.c_nchild = t.c_nchild;
@@ -877,14 +889,14 @@ int pb_tree_build_impl(pb_ctx* ctx)
     PB_CUDA(cudaMemsetAsync(cnt_m, 0, sizeof(int32_t) * (G + 1), st));
     PB_CUDA(cudaMemsetAsync(cnt_p, 0, sizeof(int32_t) * (G + 1), st));
     unsigned long long* pc = (unsigned long long*)ctx->scratch;
-    PB_CUDA(cudaMemsetAsync(pc, 0, 5 * sizeof(unsigned long long), st));
+    PB_CUDA(cudaMemsetAsync(pc, 0, 6 * sizeof(unsigned long long), st));
     a.n_m2p = cnt_m; a.n_p2p = cnt_p; a.m2p_cell = nullptr; a.p2p_lo = nullptr; a.p2p_hi = nullptr; a.m2p_low = nullptr;
     a.p2p_mask = nullptr;
     a.split = ctx->prm.list_split;
     a.pair_counts = pc;
     k_lists<0, 2><<<pb_blocks(G, LIST_WARPS), LIST_WARPS * 32, 0, st>>>(a);
     PB_LAUNCH_CHECK();
-    unsigned long long hpc[5];
+    unsigned long long hpc[6];
     PB_CUDA(cudaMemcpyAsync(hpc, pc, sizeof(hpc), cudaMemcpyDeviceToHost, st));
     int64_t tot_m = 0, tot_p = 0;
     PB_TRY(pb_exclusive_scan_i32(ctx, cnt_m, t.m2p_off, G + 1, &tot_m));
@@ -894,6 +906,7 @@ int pb_tree_build_impl(pb_ctx* ctx)
     t.m2p_pairs_low = (int64_t)hpc[2];
     t.p2p_pairs_half = (int64_t)hpc[3];
     t.m2p_pairs_half = (int64_t)hpc[4];
+    t.m2p_pairs_mid = (int64_t)hpc[5];
     t.m2p_total = tot_m;
     PB_TRY(pb_dalloc_t(ctx, &t.m2p_cell, tot_m, CAT_TREE));
     PB_TRY(pb_dalloc_t(ctx, &t.p2p_lo, tot_p, CAT_TREE));
@@ -954,6 +967,7 @@ int pb_tree_build_impl(pb_ctx* ctx)
         t.p2p_pairs = pp;                           // pb_stats: the owned groups' pairs
         t.m2p_pairs = mp;
         t.m2p_pairs_low = 0;                        // (not tracked per group)
+        t.m2p_pairs_mid = 0;
         PB_TRY(pb_dalloc_t(ctx, &t.shard_first_dev, world + 1, CAT_TREE));
         PB_CUDA(cudaMemcpyAsync(t.shard_first_dev, t.shard_first.data(), sizeof(int64_t) * (world + 1), cudaMemcpyHostToDevice, st));
         const int64_t nm = t.shard_nmax > 0 ? t.shard_nmax : 1;
@@ -1013,6 +1027,7 @@ int pb_lists_build(pb_ctx* ctx, int tpl, int64_t ntargets, const double* tx, con
     a.ng = G; a.N = ntargets; a.Ns = Ns; a.K = K;
     a.theta = theta;
     a.theta_low2 = 0.0;
+    a.theta_mid2 = 0.0;
     a.m2p_low = nullptr;
     a.p2p_mask = nullptr;
     a.split = 0;
@@ -1027,7 +1042,7 @@ int pb_lists_build(pb_ctx* ctx, int tpl, int64_t ntargets, const double* tx, con
     PB_CUDA(cudaMemsetAsync(cnt_p, 0, sizeof(int32_t) * (G + 1), st));
     PB_TRY(pb_scratch(ctx, 1 << 20));
     unsigned long long* pc = (unsigned long long*)ctx->scratch;
-    PB_CUDA(cudaMemsetAsync(pc, 0, 5 * sizeof(unsigned long long), st));
+    PB_CUDA(cudaMemsetAsync(pc, 0, 6 * sizeof(unsigned long long), st));
     a.n_m2p = cnt_m; a.n_p2p = cnt_p; a.m2p_cell = nullptr; a.p2p_lo = nullptr; a.p2p_hi = nullptr;
     a.pair_counts = pc;
     if (tpl == 2) k_lists<0, 2><<<pb_blocks(G, LIST_WARPS), LIST_WARPS * 32, 0, st>>>(a);
@@ -1088,6 +1103,7 @@ int pb_site_lists_build(pb_ctx* ctx)
     // 8e-4, 8e-5; field gradient 1.4e-1, 1.6e-2, 1.4e-3; time 91, 165, 299 ms against 766 ms direct).
     a.theta = ctx->prm.theta * PB_SITE_THETA_SCALE;
     a.theta_low2 = 0.0;
+    a.theta_mid2 = 0.0;
     a.m2p_low = nullptr;
     a.p2p_mask = nullptr;
     a.split = 0;
@@ -1102,7 +1118,7 @@ int pb_site_lists_build(pb_ctx* ctx)
     PB_CUDA(cudaMemsetAsync(cnt_p, 0, sizeof(int32_t) * (G + 1), st));
     PB_TRY(pb_scratch(ctx, 1 << 20));
     unsigned long long* pc = (unsigned long long*)ctx->scratch;
-    PB_CUDA(cudaMemsetAsync(pc, 0, 5 * sizeof(unsigned long long), st));
+    PB_CUDA(cudaMemsetAsync(pc, 0, 6 * sizeof(unsigned long long), st));
     a.n_m2p = cnt_m; a.n_p2p = cnt_p; a.m2p_cell = nullptr; a.p2p_lo = nullptr; a.p2p_hi = nullptr;
     a.pair_counts = pc;
     k_lists<0, 1><<<pb_blocks(G, LIST_WARPS), LIST_WARPS * 32, 0, st>>>(a);

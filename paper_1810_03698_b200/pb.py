@@ -83,6 +83,7 @@ class Stats(ctypes.Structure):
         ("covered_pairs", ctypes.c_int64), ("site_p2p_pairs", ctypes.c_int64), ("site_m2p_pairs", ctypes.c_int64),
         ("site_covered_pairs", ctypes.c_int64), ("rhs_p2p_pairs", ctypes.c_int64), ("rhs_m2p_pairs", ctypes.c_int64),
         ("rhs_covered_pairs", ctypes.c_int64), ("p2p_pairs_half", ctypes.c_int64), ("m2p_pairs_half", ctypes.c_int64),
+        ("m2p_pairs_mid", ctypes.c_int64),
     ]
 
     def as_dict(self):

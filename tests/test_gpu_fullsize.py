@@ -70,6 +70,8 @@ def test_matvec_full_size(pbm, po, torch_cuda, name, kw, nrows, direct):
     st = ctx.stats()
     assert rel(y[rows], y1) <= TOL_TREE and rel(y[nt + rows], y2) <= TOL_TREE
     assert st["m2p_pairs"] > 0 and st["p2p_pairs"] + 0 < nt * nt * w.params["K_far"]
+    # variable order (R-30): some pairs at order P - 2, some at P - 1, the rest at P; the bound above holds with them
+    assert st["m2p_pairs_low"] > 0 and st["m2p_pairs_mid"] > 0 and st["m2p_pairs_low"] + st["m2p_pairs_mid"] < st["m2p_pairs"]
     # exact cover: the stored lists account for every (target, source point) pair exactly once --
     # at C4 one missed far panel would be a 1e-6 error, invisible under the 1e-4 bound
     assert st["covered_pairs"] == nt * nt * w.params["K_far"]
